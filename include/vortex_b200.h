@@ -1,0 +1,180 @@
+/*
+ * vortex_b200.h -- C ABI of the B200 (sm_100a) sparse decode hot path of
+ * arxiv/paper_2606_06453 ("Vortex": dynamic sparse attention over a paged KV cache).
+ *
+ * One decode step, per layer (PAPER.md:87-99 section 3.1; :546 App. G shared pipeline):
+ *   (a1) page summaries      channel-wise min / max of the keys of each page          (:546)
+ *   (a2) page scores         u[h,j] = sum_c max(q_h[c]*M_j[c], q_h[c]*m_j[c]),
+ *                            aggregated over the query heads of one KV head            (:552, :92)
+ *   (a3) top-k pages         per (request, KV head); first n_sink and last n_local
+ *                            pages always kept; ties -> lower logical page             (:92 Eq.3, :280)
+ *   (a4) sparse attention    softmax(q K_I^T * sm_scale) V_I over the selected pages,
+ *                            reached through the page table, split along pages         (:92 Eq.4, :200)
+ *   (a5) combine             merge the splits by log-sum-exp                           (:75)
+ *
+ * Conventions
+ *  - All pointers are DEVICE pointers unless the parameter is marked "host".  Buffers are
+ *    caller-owned; the library never allocates or frees device memory and keeps scratch
+ *    only in the workspace given to vx_create.
+ *  - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = default
+ *    stream), never synchronise, never read device memory on the host, and can be captured
+ *    in a CUDA graph -- except vx_sparse_decode_step_host, which is synchronous.
+ *  - Return value is a vx_status; nothing throws or aborts across the ABI.  Only
+ *    host-visible arguments are validated.  vx_last_error gives a text for the last
+ *    failure on that context.
+ *  - A context is bound to one geometry and one device and is not thread-safe.
+ *  - Inputs must be finite; behaviour on NaN/Inf is undefined (padding uses -1 / -inf).
+ *  - There is no CPU fallback: without a CUDA device every compute call returns VX_ERR_CUDA.
+ *
+ * Page table = the paper's layout metadata C = (b, p, I) (PAPER.md:166 Eq.5, :438):
+ * request i owns logical pages 0..P_i-1, P_i = ceil(seq_lens[i] / page_size); logical page j
+ * lives in physical page page_indices[page_indptr[i] + j]; only the last page may be partial.
+ * Named caches (the summaries) are paged with the SAME physical ids as the KV pool (:180).
+ */
+#ifndef VORTEX_B200_H_
+#define VORTEX_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vx_ctx vx_ctx; /* opaque */
+typedef void *vx_stream;      /* cudaStream_t */
+
+typedef enum {
+  VX_OK = 0,
+  VX_ERR_INVALID_ARG = 1, /* null pointer, negative size, inconsistent sizes */
+  VX_ERR_UNSUPPORTED = 2, /* geometry / dtype / option the kernels are not built for */
+  VX_ERR_WORKSPACE = 3,   /* workspace too small for this call's sizes */
+  VX_ERR_CUDA = 4         /* CUDA runtime / launch failure (text in vx_last_error) */
+} vx_status;
+
+typedef enum { VX_DT_BF16 = 0, VX_DT_F32 = 1 } vx_dtype;
+
+/* aggregation of per-head envelope scores over the heads of one KV head.
+ * SUM ranks like the paper's mean ("topK(Sum(s))"); MAX is the
+ * max_h variant of App. G (:556).  MAX returns VX_ERR_UNSUPPORTED in this round. */
+typedef enum { VX_AGG_SUM = 0, VX_AGG_MAX = 1 } vx_agg;
+
+typedef struct {
+  int32_t dtype;        /* vx_dtype of q, K, V, summaries and out */
+  int32_t num_q_heads;  /* Hq */
+  int32_t num_kv_heads; /* Hkv; Hq % Hkv == 0; MLA: 1 */
+  int32_t qk_dim;       /* d: width of q and K rows (MLA: 576 = 512 latent + 64 RoPE) */
+  int32_t v_dim;        /* dv: width of V rows and of out (MLA: 512) */
+  int32_t page_size;    /* b tokens per page */
+  int32_t kv_shared;    /* 1 = MLA absorbed: V_t = K_t[0:v_dim]; pool.v is ignored */
+  float sm_scale;       /* softmax scale of (a4); scores of (a2) are unscaled (:92 Eq.2) */
+  int32_t n_sink;       /* first pages always selected (:280) */
+  int32_t n_local;      /* last pages always selected (:280); precondition n_sink+n_local <= budget[i] */
+  int32_t agg;          /* vx_agg */
+} vx_geom;
+
+typedef struct {
+  int32_t batch;               /* host: number of requests B */
+  const int32_t *page_indptr;  /* dev [B+1], page_indptr[0] = 0 */
+  const int32_t *page_indices; /* dev [total_pages] physical page ids in logical order */
+  const int32_t *seq_lens;     /* dev [B] tokens incl. the one just appended, >= 1 */
+  int32_t total_pages;         /* host copy of page_indptr[B] */
+  int32_t max_pages_per_req;   /* host upper bound of P_i (sizes grids) */
+} vx_page_table;
+
+/* K and V pools, addressed in ELEMENTS:
+ *   elem(page p, token t, head h, channel c) = p*stride_page + t*stride_token + h*stride_head + c
+ * The same strides serve k and v.  Rows (qk_dim channels) are contiguous and 16-byte aligned:
+ * base pointers and all strides must be multiples of 16 bytes. */
+typedef struct {
+  const void *k;
+  const void *v; /* ignored when geom.kv_shared */
+  int64_t stride_page, stride_token, stride_head;
+  int32_t num_pool_pages;
+} vx_kv_pool;
+
+/* ---- context ------------------------------------------------------------------------ */
+
+/* Bytes of device workspace a context needs for calls with batch <= max_batch,
+ * total_pages <= max_total_pages, max_pages_per_req <= max_pages_per_req, max_budget <= max_budget.
+ * Returns 0 if the geometry is invalid. */
+size_t vx_workspace_bytes(const vx_geom *g, int32_t max_batch, int32_t max_total_pages,
+                          int32_t max_pages_per_req, int32_t max_budget);
+
+/* Create a context on CUDA device `device` (host int).  `workspace` is device memory of
+ * `workspace_bytes` (256-byte aligned), owned by the caller and kept alive until vx_destroy.
+ * The max_* values are the ones given to vx_workspace_bytes. */
+vx_status vx_create(vx_ctx **out, const vx_geom *g, int device, void *workspace,
+                    size_t workspace_bytes, int32_t max_batch, int32_t max_total_pages,
+                    int32_t max_pages_per_req, int32_t max_budget);
+void vx_destroy(vx_ctx *ctx);
+
+/* Text of the last error on this context (ctx == NULL: last vx_create failure).  Owned by
+ * the library; valid until the next call on the same context. */
+const char *vx_last_error(const vx_ctx *ctx);
+
+/* Number of kernel launches the last compute call on this context enqueued (host counter). */
+int32_t vx_last_launch_count(const vx_ctx *ctx);
+
+/* ---- (a1) summaries: PAPER.md:546 envelope, :89 query-independent, :529 per block ---- */
+/* For request i, rebuilds from the K pool the summary of every logical page
+ * j >= first_new_pos[i] / page_size (first_new_pos == NULL: only the last page, i.e. the page
+ * the newest token fell into; first_new_pos[i] = 0 rebuilds all pages of the request):
+ *   summary[p, h, 0, c] = min_t K[p, t, h, c],  summary[p, h, 1, c] = max_t K[p, t, h, c]
+ * over the page's VALID tokens (position < seq_lens[i]).  Idempotent.
+ * summary: dev [num_pool_pages, Hkv, 2, qk_dim] in the K dtype (min/max are exact). */
+vx_status vx_page_summary_update(vx_ctx *ctx, const vx_kv_pool *pool, const vx_page_table *pt,
+                                 const int32_t *first_new_pos /* dev [B] or NULL */,
+                                 void *summary, vx_stream stream);
+
+/* ---- (a2) scores: PAPER.md:552, aggregated per KV head (:92) ------------------------- */
+/* scores[kvh * total_pages + page_indptr[i] + j] (fp32, ragged layout of PAPER.md:436)
+ *   = AGG_{h in group(kvh)} sum_c max(q[i,h,c] * max_c, q[i,h,c] * min_c)  of page j of request i.
+ * q: dev [B, Hq, qk_dim].  fp32 accumulation. */
+vx_status vx_page_score(vx_ctx *ctx, const void *q, const void *summary, const vx_page_table *pt,
+                        float *scores /* dev [Hkv, total_pages] */, vx_stream stream);
+
+/* ---- (a3) selection: PAPER.md:92 Eq.3, :194 radix top-k, :280 forced pages ----------- */
+/* Per (request i, KV head kvh), k = budget[i] pages INCLUDING the forced ones:
+ * k >= P_i selects every page; otherwise the first n_sink and last n_local logical pages plus
+ * the k - #forced best-scoring of the rest (ties: lower logical index).  Exact.
+ * sel_phys / sel_logical: dev [B, Hkv, max_budget], entries in ASCENDING logical order,
+ * padded with -1; sel_logical may be NULL.  sel_count: dev [B, Hkv] = min(k, P_i).
+ * max_budget (host) >= every budget[i]. */
+vx_status vx_topk_pages(vx_ctx *ctx, const float *scores, const vx_page_table *pt,
+                        const int32_t *budget /* dev [B] */, int32_t max_budget,
+                        int32_t *sel_phys, int32_t *sel_logical, int32_t *sel_count,
+                        vx_stream stream);
+
+/* ---- (a4)+(a5) attention over the selected pages: PAPER.md:92 Eq.4, :200, :75 -------- */
+/* out[i,h,:] = softmax_t(sm_scale * q[i,h].K_t) V_t over the valid tokens of the pages listed
+ * in sel_logical/sel_phys[i, h/g, 0:sel_count]; lse[i,h] = natural log of the softmax
+ * denominator.  Split-KV partials live in the workspace and are merged by LSE.
+ * out: dev [B, Hq, v_dim] in geom.dtype; lse: dev [B, Hq] fp32 (may be NULL). */
+vx_status vx_sparse_paged_decode(vx_ctx *ctx, const void *q, const vx_kv_pool *pool,
+                                 const vx_page_table *pt, const int32_t *sel_phys,
+                                 const int32_t *sel_logical, const int32_t *sel_count,
+                                 int32_t max_budget, void *out, float *lse, vx_stream stream);
+
+/* ---- (a6) the fused step: (a1 append rows) -> a2 -> a3 -> a4 -> a5 in one call -------- */
+#define VX_STEP_UPDATE_SUMMARY 1u /* flags bit 0: first rebuild the last page's summary of each request */
+/* sel_phys / sel_logical / sel_count are optional outputs (NULL = keep them in the workspace). */
+vx_status vx_sparse_decode_step(vx_ctx *ctx, const void *q, const vx_kv_pool *pool, void *summary,
+                                const vx_page_table *pt, const int32_t *budget, int32_t max_budget,
+                                uint32_t flags, void *out, float *lse, int32_t *sel_phys,
+                                int32_t *sel_logical, int32_t *sel_count, vx_stream stream);
+
+/* The same step fed from HOST buffers (the serving loop's per-step inputs): copies q, the page
+ * table arrays and the budgets host->device into the workspace, runs the fused step, copies
+ * out (and lse if not NULL) device->host and synchronises `stream`.  The KV and summary pools
+ * are resident device state.  h_* are host pointers (pinned memory recommended). */
+vx_status vx_sparse_decode_step_host(vx_ctx *ctx, const void *h_q, const vx_kv_pool *pool,
+                                     void *summary, int32_t batch, const int32_t *h_page_indptr,
+                                     const int32_t *h_page_indices, const int32_t *h_seq_lens,
+                                     const int32_t *h_budget, int32_t max_budget, uint32_t flags,
+                                     void *h_out, float *h_lse, vx_stream stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VORTEX_B200_H_ */

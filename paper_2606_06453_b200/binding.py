@@ -1,0 +1,222 @@
+"""Thin ctypes binding over libvortex_b200.so (include/vortex_b200.h).
+
+Argument marshalling only: every step of the path runs in the CUDA kernels behind the C
+ABI.  torch is used for device memory and streams.  There is no CPU fallback -- if the
+library is missing or the device is not a B200, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_PKG, "libvortex_b200.so")
+
+VX_OK, VX_ERR_INVALID_ARG, VX_ERR_UNSUPPORTED, VX_ERR_WORKSPACE, VX_ERR_CUDA = range(5)
+VX_DT_BF16, VX_DT_F32 = 0, 1
+VX_AGG_SUM, VX_AGG_MAX = 0, 1
+VX_STEP_UPDATE_SUMMARY = 1
+
+EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",
+           "vx_page_summary_update", "vx_page_score", "vx_topk_pages", "vx_sparse_paged_decode",
+           "vx_sparse_decode_step", "vx_sparse_decode_step_host"]
+
+
+class VxGeom(C.Structure):
+    _fields_ = [("dtype", C.c_int32), ("num_q_heads", C.c_int32), ("num_kv_heads", C.c_int32),
+                ("qk_dim", C.c_int32), ("v_dim", C.c_int32), ("page_size", C.c_int32),
+                ("kv_shared", C.c_int32), ("sm_scale", C.c_float), ("n_sink", C.c_int32),
+                ("n_local", C.c_int32), ("agg", C.c_int32)]
+
+
+class VxPageTable(C.Structure):
+    _fields_ = [("batch", C.c_int32), ("page_indptr", C.c_void_p), ("page_indices", C.c_void_p),
+                ("seq_lens", C.c_void_p), ("total_pages", C.c_int32), ("max_pages_per_req", C.c_int32)]
+
+
+class VxKvPool(C.Structure):
+    _fields_ = [("k", C.c_void_p), ("v", C.c_void_p), ("stride_page", C.c_int64),
+                ("stride_token", C.c_int64), ("stride_head", C.c_int64), ("num_pool_pages", C.c_int32)]
+
+
+class VortexError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"vortex_b200 status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree library (build it with `python -m paper_2606_06453_b200.build`)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_06453_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    P, I32, U32, SZ = C.c_void_p, C.c_int32, C.c_uint32, C.c_size_t
+    G, T, K = C.POINTER(VxGeom), C.POINTER(VxPageTable), C.POINTER(VxKvPool)
+    sig = {
+        "vx_workspace_bytes": (SZ, [G, I32, I32, I32, I32]),
+        "vx_create": (I32, [C.POINTER(P), G, C.c_int, P, SZ, I32, I32, I32, I32]),
+        "vx_destroy": (None, [P]),
+        "vx_last_error": (C.c_char_p, [P]),
+        "vx_last_launch_count": (I32, [P]),
+        "vx_page_summary_update": (I32, [P, K, T, P, P, P]),
+        "vx_page_score": (I32, [P, P, P, T, P, P]),
+        "vx_topk_pages": (I32, [P, P, T, P, I32, P, P, P, P]),
+        "vx_sparse_paged_decode": (I32, [P, P, K, T, P, P, P, I32, P, P, P]),
+        "vx_sparse_decode_step": (I32, [P, P, K, P, T, P, I32, U32, P, P, P, P, P, P]),
+        "vx_sparse_decode_step_host": (I32, [P, P, K, P, I32, P, P, P, P, I32, U32, P, P, P]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    return None if t is None else C.c_void_p(t.data_ptr())
+
+
+def _stream(stream):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+class PageTable:
+    """Device page table C = (b, p, I) plus the host scalars that size grids."""
+
+    def __init__(self, page_indptr, page_indices, seq_lens, total_pages: int, max_pages_per_req: int):
+        for t in (page_indptr, page_indices, seq_lens):
+            assert t.dtype == torch.int32 and t.is_contiguous()
+        self.tensors = (page_indptr, page_indices, seq_lens)
+        self.c = VxPageTable(seq_lens.numel(), page_indptr.data_ptr(), page_indices.data_ptr(),
+                             seq_lens.data_ptr(), int(total_pages), int(max_pages_per_req))
+
+    @property
+    def batch(self):
+        return self.c.batch
+
+
+class KvPool:
+    """K/V pools [N_pool, Hkv, page, d] (or any layout expressed by element strides)."""
+
+    def __init__(self, k, v, stride_page: int, stride_token: int, stride_head: int):
+        self.tensors = (k, v)
+        self.c = VxKvPool(k.data_ptr(), 0 if v is None else v.data_ptr(), stride_page, stride_token,
+                          stride_head, k.shape[0])
+
+
+class Context:
+    """One geometry on one device; owns its workspace tensor."""
+
+    def __init__(self, *, dtype, num_q_heads, num_kv_heads, qk_dim, v_dim, page_size, sm_scale,
+                 n_sink, n_local, kv_shared=False, agg=VX_AGG_SUM, max_batch, max_total_pages,
+                 max_pages_per_req, max_budget, device="cuda:0"):
+        self.lib = load_library()
+        self.torch_dtype = dtype
+        dt = {torch.bfloat16: VX_DT_BF16, torch.float32: VX_DT_F32}[dtype]
+        self.geom = VxGeom(dt, num_q_heads, num_kv_heads, qk_dim, v_dim, page_size, int(kv_shared),
+                           float(sm_scale), n_sink, n_local, agg)
+        self.device = torch.device(device)
+        self.max = (int(max_batch), int(max_total_pages), int(max_pages_per_req), int(max_budget))
+        need = self.lib.vx_workspace_bytes(C.byref(self.geom), *self.max)
+        if need == 0:
+            raise VortexError(VX_ERR_UNSUPPORTED, "geometry rejected by vx_workspace_bytes")
+        if self.device.type != "cuda":
+            raise VortexError(VX_ERR_CUDA, "vortex_b200 needs a CUDA device; there is no CPU path")
+        self.workspace = torch.empty(need + 256, dtype=torch.uint8, device=self.device)
+        base = (self.workspace.data_ptr() + 255) // 256 * 256
+        self._h = C.c_void_p()
+        st = self.lib.vx_create(C.byref(self._h), C.byref(self.geom), self.device.index or 0,
+                                C.c_void_p(base), need, *self.max)
+        if st != VX_OK:
+            raise VortexError(st, self.lib.vx_last_error(None).decode())
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self.lib.vx_destroy(self._h)
+            self._h = C.c_void_p()
+
+    __del__ = close
+
+    def _check(self, st):
+        if st != VX_OK:
+            raise VortexError(st, self.lib.vx_last_error(self._h).decode())
+
+    @property
+    def last_launch_count(self) -> int:
+        return int(self.lib.vx_last_launch_count(self._h))
+
+    # ---- the calls of include/vortex_b200.h, same names ---------------------------------
+    def page_summary_update(self, pool: KvPool, pt: PageTable, summary, first_new_pos=None, stream=None):
+        self._check(self.lib.vx_page_summary_update(self._h, C.byref(pool.c), C.byref(pt.c),
+                                                    _ptr(first_new_pos), _ptr(summary), _stream(stream)))
+
+    def page_score(self, q, summary, pt: PageTable, scores, stream=None):
+        self._check(self.lib.vx_page_score(self._h, _ptr(q), _ptr(summary), C.byref(pt.c), _ptr(scores),
+                                           _stream(stream)))
+
+    def topk_pages(self, scores, pt: PageTable, budget, max_budget, sel_phys, sel_logical, sel_count,
+                   stream=None):
+        self._check(self.lib.vx_topk_pages(self._h, _ptr(scores), C.byref(pt.c), _ptr(budget), max_budget,
+                                           _ptr(sel_phys), _ptr(sel_logical), _ptr(sel_count),
+                                           _stream(stream)))
+
+    def sparse_paged_decode(self, q, pool: KvPool, pt: PageTable, sel_phys, sel_logical, sel_count,
+                            max_budget, out, lse=None, stream=None):
+        self._check(self.lib.vx_sparse_paged_decode(self._h, _ptr(q), C.byref(pool.c), C.byref(pt.c),
+                                                    _ptr(sel_phys), _ptr(sel_logical), _ptr(sel_count),
+                                                    max_budget, _ptr(out), _ptr(lse), _stream(stream)))
+
+    def sparse_decode_step(self, q, pool: KvPool, summary, pt: PageTable, budget, max_budget, out,
+                           lse=None, sel_phys=None, sel_logical=None, sel_count=None, flags=0,
+                           stream=None):
+        self._check(self.lib.vx_sparse_decode_step(self._h, _ptr(q), C.byref(pool.c), _ptr(summary),
+                                                   C.byref(pt.c), _ptr(budget), max_budget, flags,
+                                                   _ptr(out), _ptr(lse), _ptr(sel_phys),
+                                                   _ptr(sel_logical), _ptr(sel_count), _stream(stream)))
+
+    def sparse_decode_step_host(self, h_q, pool: KvPool, summary, h_page_indptr, h_page_indices,
+                                h_seq_lens, h_budget, max_budget, h_out, h_lse=None, flags=0,
+                                stream=None):
+        """Host (CPU, ideally pinned) tensors in, host tensors out; synchronous."""
+        for t in (h_q, h_page_indptr, h_page_indices, h_seq_lens, h_budget, h_out):
+            assert t.device.type == "cpu" and t.is_contiguous()
+        self._check(self.lib.vx_sparse_decode_step_host(
+            self._h, _ptr(h_q), C.byref(pool.c), _ptr(summary), h_seq_lens.numel(), _ptr(h_page_indptr),
+            _ptr(h_page_indices), _ptr(h_seq_lens), _ptr(h_budget), max_budget, flags, _ptr(h_out),
+            _ptr(h_lse), _stream(stream)))
+
+
+# ---- conveniences used by tests / bench (allocation + marshalling only) -----------------------
+def context_for(w, device=None, **over) -> Context:
+    """Context sized for a workloads.Workload."""
+    s = w.spec
+    kw = dict(dtype={"bf16": torch.bfloat16, "f32": torch.float32}[s.dtype], num_q_heads=s.num_q_heads,
+              num_kv_heads=s.num_kv_heads, qk_dim=s.qk_dim, v_dim=s.v_dim, page_size=s.page_size,
+              sm_scale=s.sm_scale, n_sink=s.n_sink, n_local=s.n_local, kv_shared=s.kv_shared,
+              max_batch=s.batch, max_total_pages=w.total_pages, max_pages_per_req=w.max_pages_per_req,
+              max_budget=w.max_budget, device=device or w.q.device)
+    kw.update(over)
+    return Context(**kw)
+
+
+def tables_for(w):
+    sp, st, sh = w.strides
+    pool = KvPool(w.k_pool, w.v_pool, sp, st, sh)
+    pt = PageTable(w.page_indptr, w.page_indices, w.seq_lens, w.total_pages, w.max_pages_per_req)
+    return pool, pt
+
+
+def alloc_summary(w):
+    s = w.spec
+    return torch.zeros(w.num_pool_pages, s.num_kv_heads, 2, s.qk_dim, dtype=w.k_pool.dtype,
+                       device=w.k_pool.device)

@@ -1,0 +1,283 @@
+// vx_api.cu -- the C ABI of include/vortex_b200.h: context, workspace, validation, dispatch.
+// Every step of the path runs in the kernels of this directory; there is no CPU fallback.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "vx_internal.h"
+
+namespace vx {
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+static size_t elem_size(int32_t dtype) { return dtype == VX_DT_BF16 ? 2 : 4; }
+
+Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32_t max_total_pages,
+                          int32_t max_budget) {
+  Workspace w{};
+  size_t off = 0;
+  char* b = static_cast<char*>(base);
+  auto take = [&](size_t bytes) -> void* {
+    void* p = b ? b + off : nullptr;
+    off = align_up(off + bytes, 256);
+    return p;
+  };
+  const size_t B = (size_t)max_batch, Hq = (size_t)g.num_q_heads, Hkv = (size_t)g.num_kv_heads;
+  const size_t esz = elem_size(g.dtype);
+  w.scores = static_cast<float*>(take(Hkv * (size_t)max_total_pages * 4));
+  w.sel_phys = static_cast<int32_t*>(take(B * Hkv * (size_t)max_budget * 4));
+  w.sel_logical = static_cast<int32_t*>(take(B * Hkv * (size_t)max_budget * 4));
+  w.sel_count = static_cast<int32_t*>(take(B * Hkv * 4));
+  w.part_o = static_cast<float*>(take(B * Hq * kMaxSplits * (size_t)g.v_dim * 4));
+  w.part_lse = static_cast<float*>(take(B * Hq * kMaxSplits * 4));
+  w.h_q = take(B * Hq * (size_t)g.qk_dim * esz);
+  w.h_indptr = static_cast<int32_t*>(take((B + 1) * 4));
+  w.h_indices = static_cast<int32_t*>(take((size_t)max_total_pages * 4));
+  w.h_seq_lens = static_cast<int32_t*>(take(B * 4));
+  w.h_budget = static_cast<int32_t*>(take(B * 4));
+  w.h_out = take(B * Hq * (size_t)g.v_dim * esz);
+  w.h_lse = static_cast<float*>(take(B * Hq * 4));
+  w.bytes = off;
+  return w;
+}
+
+static char g_create_err[512] = "";
+
+static vx_status fail(vx_ctx* c, vx_status st, const char* fmt, ...) {
+  char* dst = c ? c->err : g_create_err;
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(dst, 512, fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+static const char* check_geom(const vx_geom* g, vx_status* st) {
+  *st = VX_ERR_INVALID_ARG;
+  if (!g) return "geom is NULL";
+  if (g->dtype != VX_DT_BF16 && g->dtype != VX_DT_F32) return "dtype must be VX_DT_BF16 or VX_DT_F32";
+  if (g->num_q_heads <= 0 || g->num_kv_heads <= 0 || g->num_q_heads % g->num_kv_heads != 0)
+    return "num_q_heads must be a positive multiple of num_kv_heads";
+  if (g->qk_dim <= 0 || g->v_dim <= 0 || g->page_size <= 0) return "qk_dim, v_dim, page_size must be positive";
+  if (g->n_sink < 0 || g->n_local < 0) return "n_sink, n_local must be >= 0";
+  if (g->kv_shared && g->v_dim > g->qk_dim) return "kv_shared needs v_dim <= qk_dim";
+  *st = VX_ERR_UNSUPPORTED;
+  if (g->agg != VX_AGG_SUM) return "only VX_AGG_SUM is built in this round";
+  if (!score_geometry_supported(*g)) return "qk_dim / dtype not supported by the score kernel";
+  if (g->kv_shared ? !mla_geometry_supported(*g) : !gqa_geometry_supported(*g))
+    return "(dtype, qk_dim, v_dim, heads) not supported by the decode kernels";
+  *st = VX_OK;
+  return nullptr;
+}
+
+static vx_status check_cuda(vx_ctx* c, cudaError_t e, const char* what) {
+  if (e == cudaSuccess) return VX_OK;
+  return fail(c, VX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+}
+
+static vx_status check_table(vx_ctx* c, const vx_page_table* pt) {
+  if (!pt) return fail(c, VX_ERR_INVALID_ARG, "page table is NULL");
+  if (pt->batch < 0 || pt->total_pages < 0 || pt->max_pages_per_req < 0)
+    return fail(c, VX_ERR_INVALID_ARG, "negative size in page table");
+  if (pt->batch > 0 && (!pt->page_indptr || !pt->page_indices || !pt->seq_lens))
+    return fail(c, VX_ERR_INVALID_ARG, "page table has NULL arrays");
+  if (pt->batch > c->max_batch || pt->total_pages > c->max_total_pages)
+    return fail(c, VX_ERR_WORKSPACE, "batch %d / total_pages %d exceed the context's maxima %d / %d",
+                pt->batch, pt->total_pages, c->max_batch, c->max_total_pages);
+  return VX_OK;
+}
+
+static vx_status check_pool(vx_ctx* c, const vx_kv_pool* pool) {
+  if (!pool || !pool->k) return fail(c, VX_ERR_INVALID_ARG, "kv pool / k is NULL");
+  if (!c->g.kv_shared && !pool->v) return fail(c, VX_ERR_INVALID_ARG, "kv pool v is NULL");
+  const int64_t per16 = 16 / (int64_t)elem_size(c->g.dtype);
+  if (pool->stride_page % per16 || pool->stride_token % per16 || pool->stride_head % per16 ||
+      ((uintptr_t)pool->k & 15) || (!c->g.kv_shared && ((uintptr_t)pool->v & 15)))
+    return fail(c, VX_ERR_INVALID_ARG, "pool pointers and strides must be multiples of 16 bytes");
+  return VX_OK;
+}
+
+}  // namespace vx
+
+using namespace vx;
+
+extern "C" {
+
+size_t vx_workspace_bytes(const vx_geom* g, int32_t max_batch, int32_t max_total_pages,
+                          int32_t max_pages_per_req, int32_t max_budget) {
+  vx_status st;
+  if (check_geom(g, &st) || max_batch < 0 || max_total_pages < 0 || max_pages_per_req < 0 || max_budget < 0)
+    return 0;
+  return carve_workspace(*g, nullptr, max_batch, max_total_pages, max_budget).bytes;
+}
+
+vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace, size_t workspace_bytes,
+                    int32_t max_batch, int32_t max_total_pages, int32_t max_pages_per_req,
+                    int32_t max_budget) {
+  if (!out) return fail(nullptr, VX_ERR_INVALID_ARG, "out is NULL");
+  *out = nullptr;
+  vx_status st;
+  if (const char* why = check_geom(g, &st)) return fail(nullptr, st, "%s", why);
+  if (max_batch < 0 || max_total_pages < 0 || max_pages_per_req < 0 || max_budget < 0)
+    return fail(nullptr, VX_ERR_INVALID_ARG, "negative maximum");
+  const size_t need = carve_workspace(*g, nullptr, max_batch, max_total_pages, max_budget).bytes;
+  if (!workspace || ((uintptr_t)workspace & 255))
+    return fail(nullptr, VX_ERR_INVALID_ARG, "workspace must be a 256-byte aligned device pointer");
+  if (workspace_bytes < need)
+    return fail(nullptr, VX_ERR_WORKSPACE, "workspace has %zu bytes, %zu needed", workspace_bytes, need);
+  cudaError_t e = cudaSetDevice(device);
+  if (e != cudaSuccess) return fail(nullptr, VX_ERR_CUDA, "cudaSetDevice(%d): %s", device, cudaGetErrorString(e));
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, device);
+  if (e != cudaSuccess) return fail(nullptr, VX_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e));
+  if (prop.major != 10)
+    return fail(nullptr, VX_ERR_UNSUPPORTED, "device %d is sm_%d%d; this library is built for sm_100a only",
+                device, prop.major, prop.minor);
+  vx_ctx* c = new (std::nothrow) vx_ctx();
+  if (!c) return fail(nullptr, VX_ERR_INVALID_ARG, "out of host memory");
+  c->g = *g;
+  c->device = device;
+  c->num_sms = prop.multiProcessorCount;
+  c->max_batch = max_batch;
+  c->max_total_pages = max_total_pages;
+  c->max_pages_per_req = max_pages_per_req;
+  c->max_budget = max_budget;
+  c->ws = carve_workspace(*g, workspace, max_batch, max_total_pages, max_budget);
+  c->launches = 0;
+  c->err[0] = 0;
+  *out = c;
+  return VX_OK;
+}
+
+void vx_destroy(vx_ctx* ctx) { delete ctx; }
+
+const char* vx_last_error(const vx_ctx* ctx) { return ctx ? ctx->err : g_create_err; }
+
+int32_t vx_last_launch_count(const vx_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+vx_status vx_page_summary_update(vx_ctx* c, const vx_kv_pool* pool, const vx_page_table* pt,
+                                 const int32_t* first_new_pos, void* summary, vx_stream stream) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  c->launches = 0;
+  if (vx_status st = check_table(c, pt)) return st;
+  if (vx_status st = check_pool(c, pool)) return st;
+  if (!summary) return fail(c, VX_ERR_INVALID_ARG, "summary is NULL");
+  return check_cuda(c, launch_summary_update(c, *pool, *pt, first_new_pos, summary, (cudaStream_t)stream),
+                    "vx_page_summary_update");
+}
+
+vx_status vx_page_score(vx_ctx* c, const void* q, const void* summary, const vx_page_table* pt, float* scores,
+                        vx_stream stream) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  c->launches = 0;
+  if (vx_status st = check_table(c, pt)) return st;
+  if (!q || !summary || !scores) return fail(c, VX_ERR_INVALID_ARG, "q / summary / scores is NULL");
+  return check_cuda(c, launch_page_score(c, q, summary, *pt, scores, (cudaStream_t)stream), "vx_page_score");
+}
+
+vx_status vx_topk_pages(vx_ctx* c, const float* scores, const vx_page_table* pt, const int32_t* budget,
+                        int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
+                        vx_stream stream) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  c->launches = 0;
+  if (vx_status st = check_table(c, pt)) return st;
+  if (!scores || !budget || !sel_phys || !sel_count)
+    return fail(c, VX_ERR_INVALID_ARG, "scores / budget / sel_phys / sel_count is NULL");
+  if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
+  return check_cuda(c, launch_topk_pages(c, scores, *pt, budget, max_budget, sel_phys, sel_logical, sel_count,
+                                         (cudaStream_t)stream), "vx_topk_pages");
+}
+
+static vx_status decode_dispatch(vx_ctx* c, const void* q, const vx_kv_pool* pool, const vx_page_table* pt,
+                                 const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
+                                 int32_t max_budget, void* out, float* lse, cudaStream_t s) {
+  cudaError_t e = c->g.kv_shared
+                      ? launch_decode_mla(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s)
+                      : launch_decode_gqa(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
+  return check_cuda(c, e, "vx_sparse_paged_decode");
+}
+
+vx_status vx_sparse_paged_decode(vx_ctx* c, const void* q, const vx_kv_pool* pool, const vx_page_table* pt,
+                                 const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
+                                 int32_t max_budget, void* out, float* lse, vx_stream stream) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  c->launches = 0;
+  if (vx_status st = check_table(c, pt)) return st;
+  if (vx_status st = check_pool(c, pool)) return st;
+  if (!q || !sel_phys || !sel_logical || !sel_count || !out)
+    return fail(c, VX_ERR_INVALID_ARG, "q / sel_phys / sel_logical / sel_count / out is NULL");
+  if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
+  if (pt->batch == 0) return VX_OK;
+  return decode_dispatch(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse,
+                         (cudaStream_t)stream);
+}
+
+vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool, void* summary,
+                                const vx_page_table* pt, const int32_t* budget, int32_t max_budget,
+                                uint32_t flags, void* out, float* lse, int32_t* sel_phys, int32_t* sel_logical,
+                                int32_t* sel_count, vx_stream stream) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  c->launches = 0;
+  if (vx_status st = check_table(c, pt)) return st;
+  if (vx_status st = check_pool(c, pool)) return st;
+  if (!q || !summary || !budget || !out) return fail(c, VX_ERR_INVALID_ARG, "q / summary / budget / out is NULL");
+  if (max_budget <= 0 || max_budget > c->max_budget)
+    return fail(c, VX_ERR_WORKSPACE, "max_budget %d outside (0, %d]", max_budget, c->max_budget);
+  if (pt->batch == 0) return VX_OK;
+  cudaStream_t s = (cudaStream_t)stream;
+  int32_t* sp = sel_phys ? sel_phys : c->ws.sel_phys;
+  int32_t* sl = sel_logical ? sel_logical : c->ws.sel_logical;
+  int32_t* sc = sel_count ? sel_count : c->ws.sel_count;
+  if (flags & VX_STEP_UPDATE_SUMMARY)
+    if (vx_status st = check_cuda(c, launch_summary_update(c, *pool, *pt, nullptr, summary, s), "summary update"))
+      return st;
+  if (vx_status st = check_cuda(c, launch_page_score(c, q, summary, *pt, c->ws.scores, s), "page score")) return st;
+  if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, s),
+                                "top-k pages"))
+    return st;
+  return decode_dispatch(c, q, pool, pt, sp, sl, sc, max_budget, out, lse, s);
+}
+
+vx_status vx_sparse_decode_step_host(vx_ctx* c, const void* h_q, const vx_kv_pool* pool, void* summary,
+                                     int32_t batch, const int32_t* h_page_indptr, const int32_t* h_page_indices,
+                                     const int32_t* h_seq_lens, const int32_t* h_budget, int32_t max_budget,
+                                     uint32_t flags, void* h_out, float* h_lse, vx_stream stream) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  c->launches = 0;
+  if (batch < 0 || batch > c->max_batch) return fail(c, VX_ERR_WORKSPACE, "batch %d outside [0, %d]", batch, c->max_batch);
+  if (batch == 0) return VX_OK;
+  if (!h_q || !h_page_indptr || !h_page_indices || !h_seq_lens || !h_budget || !h_out)
+    return fail(c, VX_ERR_INVALID_ARG, "a host input / output pointer is NULL");
+  const int32_t total = h_page_indptr[batch];
+  if (total < 0 || total > c->max_total_pages)
+    return fail(c, VX_ERR_WORKSPACE, "total_pages %d outside [0, %d]", total, c->max_total_pages);
+  int32_t max_pages = 0;
+  for (int32_t i = 0; i < batch; ++i) {
+    const int32_t p = h_page_indptr[i + 1] - h_page_indptr[i];
+    if (p < 0) return fail(c, VX_ERR_INVALID_ARG, "page_indptr is not non-decreasing at %d", i);
+    if (p > max_pages) max_pages = p;
+  }
+  const vx_geom& g = c->g;
+  const size_t esz = elem_size(g.dtype);
+  cudaStream_t s = (cudaStream_t)stream;
+  Workspace& w = c->ws;
+  const size_t q_bytes = (size_t)batch * g.num_q_heads * g.qk_dim * esz;
+  const size_t o_bytes = (size_t)batch * g.num_q_heads * g.v_dim * esz;
+  cudaError_t e = cudaMemcpyAsync(w.h_q, h_q, q_bytes, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_indptr, h_page_indptr, (size_t)(batch + 1) * 4, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_indices, h_page_indices, (size_t)total * 4, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_seq_lens, h_seq_lens, (size_t)batch * 4, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_budget, h_budget, (size_t)batch * 4, cudaMemcpyHostToDevice, s);
+  if (vx_status st = check_cuda(c, e, "host->device copies")) return st;
+  vx_page_table pt{batch, w.h_indptr, w.h_indices, w.h_seq_lens, total, max_pages};
+  vx_status st = vx_sparse_decode_step(c, w.h_q, pool, summary, &pt, w.h_budget, max_budget, flags, w.h_out,
+                                       w.h_lse, nullptr, nullptr, nullptr, stream);
+  if (st != VX_OK) return st;
+  e = cudaMemcpyAsync(h_out, w.h_out, o_bytes, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess && h_lse)
+    e = cudaMemcpyAsync(h_lse, w.h_lse, (size_t)batch * g.num_q_heads * 4, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  return check_cuda(c, e, "device->host copies");
+}
+
+}  // extern "C"

@@ -1,0 +1,72 @@
+// vx_internal.h -- context, workspace carving and kernel launcher prototypes (host side).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/vortex_b200.h"
+
+namespace vx {
+
+constexpr int kMaxSplits = 32;   // split-KV fan-out bound (workspace is sized for it)
+
+struct Workspace {               // device pointers carved from the caller's workspace
+  float* scores;                 // [Hkv, max_total_pages]
+  int32_t* sel_phys;             // [max_batch, Hkv, max_budget]
+  int32_t* sel_logical;          // [max_batch, Hkv, max_budget]
+  int32_t* sel_count;            // [max_batch, Hkv]
+  float* part_o;                 // [max_batch, Hq, kMaxSplits, v_dim]
+  float* part_lse;               // [max_batch, Hq, kMaxSplits]
+  // staging for vx_sparse_decode_step_host
+  void* h_q;                     // [max_batch, Hq, qk_dim] elements
+  int32_t* h_indptr;             // [max_batch + 1]
+  int32_t* h_indices;            // [max_total_pages]
+  int32_t* h_seq_lens;           // [max_batch]
+  int32_t* h_budget;             // [max_batch]
+  void* h_out;                   // [max_batch, Hq, v_dim] elements
+  float* h_lse;                  // [max_batch, Hq]
+  size_t bytes;                  // total
+};
+
+// carve (base may be null: only sizes are computed)
+Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32_t max_total_pages,
+                          int32_t max_budget);
+
+}  // namespace vx
+
+struct vx_ctx {
+  vx_geom g;
+  int device;
+  int num_sms;
+  int32_t max_batch, max_total_pages, max_pages_per_req, max_budget;
+  vx::Workspace ws;
+  int32_t launches;              // kernels enqueued by the last compute call
+  char err[512];
+};
+
+namespace vx {
+
+// every launcher returns cudaGetLastError() after its launches and adds to ctx->launches
+cudaError_t launch_summary_update(vx_ctx* c, const vx_kv_pool& pool, const vx_page_table& pt,
+                                  const int32_t* first_new_pos, void* summary, cudaStream_t s);
+cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
+                              float* scores, cudaStream_t s);
+cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
+                              const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
+                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s);
+cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                              const int32_t* sel_phys, const int32_t* sel_logical,
+                              const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
+                              cudaStream_t s);
+cudaError_t launch_decode_mla(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                              const int32_t* sel_phys, const int32_t* sel_logical,
+                              const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
+                              cudaStream_t s);
+cudaError_t launch_combine(vx_ctx* c, int32_t batch, int num_splits, void* out, float* lse,
+                           cudaStream_t s);
+
+// geometry support predicates (used by vx_create validation)
+bool gqa_geometry_supported(const vx_geom& g);
+bool mla_geometry_supported(const vx_geom& g);
+bool score_geometry_supported(const vx_geom& g);
+
+}  // namespace vx
