@@ -1,0 +1,351 @@
+#!/usr/bin/env python
+"""bench.py -- times the fused sparse decode step (all hot-path rows a1..a5) on synthetic, seeded
+decode workloads shaped like BASELINE.json's configs, and prints ONE JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2|C3|C4|C5|C1] [--impl reference]
+
+metric : sparse decode step time in microseconds (lower is better), with the achieved HBM GB/s and
+         the fraction of the bytes roofline (summary bytes + selected-KV bytes + Q/O bytes).
+value  : device-timed (CUDA events on the launching stream, L2 flushed between steps), inputs resident.
+e2e    : the same step through vx_sparse_decode_step_host: pinned HOST q / page table / budgets in,
+         HOST out / lse back, copies inside the timed region.
+N > 1  : one process per GPU (torchrun), every rank runs its own seeded copy of the workload
+         (requests shard with no exchange step: "weak" scaling, no collective on the data path);
+         time = max over ranks.
+--impl reference : the fp64 CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "sparse_decode_step_us"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json "about 8 TB/s"
+FALLBACK_HBM_GBS = 6650.0         # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--config", default="C2", help="workload: C1..C5 (default C2 = BASELINE.json configs[1])")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--also", default="C3,C4", help="extra configs timed briefly and reported under 'also'")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def algorithmic_bytes(w, sel_count=None):
+    """Bytes roofline of one step: every summary row once, every selected
+    page's K and V tokens once, Q in and O out.  Page table / scores / partials are not counted."""
+    import torch
+    s = w.spec
+    esz = 2 if s.dtype == "bf16" else 4
+    b = s.page_size
+    n = w.seq_lens.cpu().long()
+    P = (n + b - 1) // b
+    summary = int(P.sum()) * s.num_kv_heads * 2 * s.qk_dim * esz
+    k = torch.minimum(w.budget.cpu().long(), P)
+    tokens = (k - 1) * b + (n - (P - 1) * b)          # the partial last page is always selected (n_local >= 1)
+    per_tok = (s.qk_dim if s.kv_shared else s.qk_dim + s.v_dim) * esz
+    kv = int(tokens.sum()) * s.num_kv_heads * per_tok
+    qo = s.batch * s.num_q_heads * (s.qk_dim + s.v_dim) * esz
+    return dict(summary=summary, kv=kv, qo=qo, total=summary + kv + qo)
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons during the timed region (NVML; ~20 ms period)."""
+
+    def __init__(self, index):
+        super().__init__(daemon=True)
+        self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+
+    def run(self):
+        try:
+            import pynvml as nv
+            nv.nvmlInit()
+            h = nv.nvmlDeviceGetHandleByIndex(self.index)
+            self.max_mhz = nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM)
+            names = {"hw_slowdown": 0x8, "sw_power_cap": 0x4, "sw_thermal_slowdown": 0x20,
+                     "hw_thermal_slowdown": 0x40, "hw_power_brake": 0x80}
+            while not self.stop_flag:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
+                self.reasons |= {k for k, bit in names.items() if r & bit}
+                time.sleep(0.02)
+        except Exception as e:  # NVML unavailable: report that rather than guessing
+            self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+
+    def result(self):
+        self.stop_flag = True
+        self.join(timeout=2)
+        med = statistics.median(self.samples) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+class Runner:
+    """One workload resident on one GPU: context, pools, summaries, outputs, L2 flush buffer."""
+
+    def __init__(self, cfg, device, seed_offset=0):
+        import torch
+        import paper_2606_06453_b200 as vx
+        from paper_2606_06453_b200.workloads import make_workload
+        self.torch, self.vx = torch, vx
+        self.w = w = make_workload(cfg, device=device, seed_offset=seed_offset)
+        self.ctx = vx.context_for(w)
+        self.pool, self.pt = vx.tables_for(w)
+        self.summary = vx.alloc_summary(w)
+        self.ctx.page_summary_update(self.pool, self.pt, self.summary, first_new_pos=torch.zeros_like(w.seq_lens))
+        s = w.spec
+        self.out = torch.empty(s.batch, s.num_q_heads, s.v_dim, dtype=w.q.dtype, device=device)
+        self.lse = torch.empty(s.batch, s.num_q_heads, dtype=torch.float32, device=device)
+        self.scores = torch.empty(s.num_kv_heads, w.total_pages, dtype=torch.float32, device=device)
+        self.sel_phys = torch.empty(s.batch, s.num_kv_heads, w.max_budget, dtype=torch.int32, device=device)
+        self.sel_logical = torch.empty_like(self.sel_phys)
+        self.sel_count = torch.empty(s.batch, s.num_kv_heads, dtype=torch.int32, device=device)
+        self.flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
+        pin = lambda t: t.cpu().contiguous().pin_memory()
+        self.h = dict(q=pin(w.q), indptr=pin(w.page_indptr), indices=pin(w.page_indices), seq=pin(w.seq_lens),
+                      budget=pin(w.budget), out=torch.empty_like(self.out, device="cpu").pin_memory(),
+                      lse=torch.empty_like(self.lse, device="cpu").pin_memory())
+        torch.cuda.synchronize()
+
+    # the stages, each through the C ABI
+    def step(self):
+        self.ctx.sparse_decode_step(self.w.q, self.pool, self.summary, self.pt, self.w.budget, self.w.max_budget,
+                                    self.out, self.lse, self.sel_phys, self.sel_logical, self.sel_count,
+                                    flags=self.vx.VX_STEP_UPDATE_SUMMARY)
+
+    def step_host(self):
+        h = self.h
+        self.ctx.sparse_decode_step_host(h["q"], self.pool, self.summary, h["indptr"], h["indices"], h["seq"],
+                                         h["budget"], self.w.max_budget, h["out"], h["lse"],
+                                         flags=self.vx.VX_STEP_UPDATE_SUMMARY)
+
+    def stage_summary(self):
+        self.ctx.page_summary_update(self.pool, self.pt, self.summary, first_new_pos=None)
+
+    def stage_score(self):
+        self.ctx.page_score(self.w.q, self.summary, self.pt, self.scores)
+
+    def stage_topk(self):
+        self.ctx.topk_pages(self.scores, self.pt, self.w.budget, self.w.max_budget, self.sel_phys,
+                            self.sel_logical, self.sel_count)
+
+    def stage_decode(self):
+        self.ctx.sparse_paged_decode(self.w.q, self.pool, self.pt, self.sel_phys, self.sel_logical, self.sel_count,
+                                     self.w.max_budget, self.out, self.lse)
+
+    def time_device(self, fn, steps, warmup):
+        """per-step CUDA-event times (ms) on the current stream, L2 flushed before every step."""
+        torch = self.torch
+        for _ in range(warmup):
+            self.flush.zero_()
+            fn()
+        torch.cuda.synchronize()
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            self.flush.zero_()
+            a.record()
+            fn()
+            b.record()
+        torch.cuda.synchronize()
+        return [a.elapsed_time(b) for a, b in evs]
+
+    def time_host(self, fn, steps, warmup):
+        """wall-clock per step (ms) of a synchronous host-buffer call, L2 flushed before every step."""
+        torch = self.torch
+        out = []
+        for it in range(warmup + steps):
+            self.flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            fn()
+            t1 = time.perf_counter()
+            if it >= warmup:
+                out.append((t1 - t0) * 1e3)
+        return out
+
+
+def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None):
+    """Time the oracle (as it stands) on the first n_requests requests of the workload.
+    Returns (seconds for score + top-k + attention on the sample, requests in sample, batch, threads)."""
+    from oracle import vx_oracle as vo
+    from paper_2606_06453_b200.workloads import make_workload, subproblem
+    from tests.oracle_io import to_oracle
+    w = workload if workload is not None else make_workload(cfg, device=device, seed_offset=seed_offset)
+    n_requests = min(n_requests, w.spec.batch)
+    sub = subproblem(w, range(n_requests))
+    q, pool, pt = to_oracle(sub)
+    s = sub.spec
+    summary = vo.page_summary(pool, pt, s.num_kv_heads, s.qk_dim)       # built outside the timed step
+    t0 = time.perf_counter()
+    vo.decode_step(q, pool, pt, vo.as_np(sub.budget), sub.max_budget, s.num_q_heads, s.num_kv_heads, s.qk_dim,
+                   s.v_dim, s.sm_scale, s.n_sink, s.n_local, summary=summary)
+    return time.perf_counter() - t0, n_requests, w.spec.batch, vo.num_threads()
+
+
+SAMPLE_REQUESTS = {"C1": 1, "C2": 4, "C3": 1, "C4": 8, "C5": 8}
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2606_06453_b200.workloads import make_workload
+    nreq = SAMPLE_REQUESTS.get(args.config, 1)
+    w = make_workload(args.config, device=_gen_device())     # inputs only; the oracle runs on the host cores
+    times = []
+    steps = max(1, min(args.steps, 3))
+    for it in range(min(args.warmup, 1) + steps):
+        t, n, batch, threads = oracle_sample_time(args.config, nreq, workload=w)
+        if it >= min(args.warmup, 1):
+            times.append(t)
+    us = statistics.mean(times) / n * batch * 1e6        # scaled from the sample to the whole batch
+    line = {"impl": "reference", "metric": METRIC, "value": us, "unit": "us", "n_gpus": args.gpus, "steps": steps,
+            "warmup": min(args.warmup, 1), "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": args.config, "l2": "n/a (CPU)"},
+            "cpu_baseline": {"value": us, "unit": "us", "cores": threads, "kind": "oracle",
+                             "sample": f"{n} of {batch} requests per step, scaled by {batch}/{n}"},
+            "e2e": {"value": us, "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def _gen_device():
+    import torch
+    return "cuda:0" if torch.cuda.is_available() else "cpu"
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    import torch
+    import torch.distributed as dist
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    device = f"cuda:{local}"
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(device))
+    import __graft_entry__
+    if rank == 0:
+        __graft_entry__.build()
+    if world > 1:
+        dist.barrier()
+
+    peak, peak_src = measured_peak()
+    r = Runner(args.config, device, seed_offset=rank)
+    w, s = r.w, r.w.spec
+    bytes_ = algorithmic_bytes(w)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- the timed region: K fused steps, device-timed, max over ranks --------------------------
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    times = r.time_device(r.step, args.steps, max(args.warmup, 3))
+    launches_per_step = r.ctx.last_launch_count
+    barrier()
+    clocks = sampler.result()
+    ms = statistics.mean(times)
+    if world > 1:
+        t = torch.tensor([ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # ---- end to end through the host-buffer entry point ------------------------------------------
+    e2e_times = r.time_host(r.step_host, min(args.steps, 30), 3)
+    e2e_ms = statistics.mean(e2e_times)
+    if world > 1:
+        t = torch.tensor([e2e_ms], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item())
+    esz = 2 if s.dtype == "bf16" else 4
+    h2d = s.batch * s.num_q_heads * s.qk_dim * esz + 4 * (s.batch + 1 + w.total_pages + 2 * s.batch)
+    d2h = s.batch * s.num_q_heads * s.v_dim * esz + 4 * s.batch * s.num_q_heads
+
+    # ---- per-stage times and the dominant kernel's roofline (rank 0) ------------------------------
+    line = None
+    if rank == 0:
+        r.step()
+        stage = {}
+        for name, fn in (("summary_append", r.stage_summary), ("page_score", r.stage_score),
+                         ("topk_pages", r.stage_topk), ("sparse_paged_decode", r.stage_decode)):
+            stage[name] = statistics.mean(r.time_device(fn, min(args.steps, 30), 3)) * 1e3      # us
+        stage_bytes = {"page_score": bytes_["summary"], "sparse_paged_decode": bytes_["kv"] + bytes_["qo"]}
+        dom = max(stage_bytes, key=lambda k: stage[k])
+        achieved = stage_bytes[dom] / (stage[dom] * 1e-6) / 1e9
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                    "algorithmic_bytes": stage_bytes[dom], "us": stage[dom]}
+        step_gbs = bytes_["total"] / (ms * 1e-3) / 1e9
+        cpu = None
+        if not args.no_cpu_baseline:
+            t, n, batch, threads = oracle_sample_time(args.config, SAMPLE_REQUESTS.get(args.config, 1), workload=w)
+            cpu = {"value": t / n * batch * 1e6, "unit": "us", "cores": threads, "kind": "oracle",
+                   "sample": f"first {n} of {batch} requests, one pass (score + top-k + attention), scaled by {batch}/{n}"}
+        also = {}
+        for name in [c for c in args.also.split(",") if c and c != args.config]:
+            del r
+            torch.cuda.empty_cache()
+            r = Runner(name, device)
+            tt = statistics.mean(r.time_device(r.step, 20, 3))
+            b2 = algorithmic_bytes(r.w)
+            also[name] = {"us": tt * 1e3, "hbm_gbs": b2["total"] / (tt * 1e-3) / 1e9,
+                          "roofline_frac": b2["total"] / (tt * 1e-3) / 1e9 / peak, "bytes": b2["total"]}
+        line = {"metric": METRIC, "value": ms * 1e3, "unit": "us", "n_gpus": world, "steps": args.steps,
+                "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
+                "vs_baseline": None, "dtype": s.dtype, "data": "synthetic",
+                "config": {"workload": args.config, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
+                           "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
+                           "seq_len": list(s.seq_len), "budget_pages": w.max_budget,
+                           "l2": "flushed before every step (512 MiB memset)", "parallelism": f"dp{world}"},
+                "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
+                "step_bytes": bytes_, "stage_us": stage, "roofline": roofline, "cpu_baseline": cpu,
+                "e2e": {"value": e2e_ms * 1e3, "unit": "us", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+                "gpu_launches": launches_per_step * args.steps, "launches_per_step": launches_per_step,
+                "clocks": clocks, "also": also}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()
