@@ -2,6 +2,7 @@
 // Every step of the path runs in the kernels of this directory; there is no CPU fallback.
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -145,6 +146,8 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->ws = carve_workspace(*g, workspace, max_batch, max_total_pages, max_budget);
   c->launches = 0;
   c->err[0] = 0;
+  const char* fg = getenv("VX_FORCE_GENERIC");
+  c->force_generic = fg && fg[0] == '1';
   *out = c;
   return VX_OK;
 }

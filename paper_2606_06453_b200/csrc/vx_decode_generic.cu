@@ -211,6 +211,8 @@ cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
                               const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                               int32_t max_budget, void* out, float* lse, cudaStream_t s) {
   const vx_geom& g = c->g;
+  if (gqa_mma_supported(g) && !c->force_generic)
+    return launch_decode_gqa_mma(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
 #define VX_GO(T, D, HPW, WT) \
   return launch_generic_t<T, D, D, HPW, WT>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s)
   if (g.dtype == VX_DT_F32) {

@@ -40,6 +40,7 @@ struct vx_ctx {
   int32_t max_batch, max_total_pages, max_pages_per_req, max_budget;
   vx::Workspace ws;
   int32_t launches;              // kernels enqueued by the last compute call
+  bool force_generic;            // VX_FORCE_GENERIC=1 in the environment: CUDA-core decode path only (debug)
   char err[512];
 };
 
@@ -57,6 +58,11 @@ cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
                               cudaStream_t s);
+cudaError_t launch_decode_gqa_mma(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                                  const int32_t* sel_phys, const int32_t* sel_logical,
+                                  const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
+                                  cudaStream_t s);
+bool gqa_mma_supported(const vx_geom& g);
 cudaError_t launch_decode_mla(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
