@@ -67,6 +67,11 @@ cudaError_t launch_decode_mla(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
                               cudaStream_t s);
+cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                                 const int32_t* sel_phys, const int32_t* sel_logical,
+                                 const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
+                                 cudaStream_t s);
+bool mla_tc_supported(const vx_geom& g);
 cudaError_t launch_combine(vx_ctx* c, int32_t batch, int num_splits, void* out, float* lse,
                            cudaStream_t s);
 
