@@ -3,153 +3,288 @@
 // query heads of one KV head by SUM (reading G2).
 //
 // With SUM the per-head maxima collapse exactly (max(q*M, q*m) = max(q,0)*M + min(q,0)*m, M >= m):
-//     S[kvh,j] = Qp . M_j + Qm . m_j,   Qp = sum_h max(q_h,0),  Qm = sum_h min(q_h,0)
-// so the kernel is one fp32 dot product per summary row: 1 flop per byte, a pure HBM stream
-// (2*d*esz bytes per (page, KV head), gathered through the page table in >=512 B rows).
+//     S[kvh,j] = [Qm | Qp] . [m_j | M_j],   Qp = sum_h max(q_h,0),  Qm = sum_h min(q_h,0)
+// i.e. one fp32 dot product per summary row: 1 flop per byte, a pure HBM stream of 2*d*esz bytes per
+// (page, KV head), gathered through the page table.
 //
-// Mapping: a CTA takes PB consecutive logical pages of one request for all KV heads; a warp takes
-// one KV head and 32 pages; G lanes share one summary row, each lane reading 16-byte vectors
-// l, l+G, .. of the min half and of the max half (128 B contiguous per G=8 lanes per load).
-// Qp/Qm live in registers (fp32), page ids are fetched 32 at a time and shuffled out.
+// Persistent kernel, one CTA per SM.  The summary pool is [N_pool, Hkv, 2, d], so all KV heads of a
+// page are ONE contiguous chunk (4 KB at Hkv=8, d=128 bf16): a producer warp gathers PG pages per
+// stage with cp.async.bulk (TMA bulk copy, completion on an mbarrier) into a 4-stage shared-memory
+// ring (~128 KB in flight per SM, no registers or LSU slots spent on the gather); 8 consumer warps
+// read rows from shared memory conflict-free (a warp reads one whole row per instruction), multiply
+// with their register-resident slice of [Qm | Qp] and reduce with a transposed shuffle butterfly.
+// Every CTA walks a contiguous range of the flat (ragged) page list, cut into groups
+// that never straddle a request, so producer and consumers derive the same schedule independently.
 #include "vx_common.cuh"
 #include "vx_internal.h"
 
 namespace vx {
 
-constexpr int kScoreThreads = 256;
-constexpr int kScorePagesPerWarp = 32;
+constexpr int kScConsumerWarps = 8;
+constexpr int kScThreads = (kScConsumerWarps + 1) * kWarp;
+constexpr int kScStages = 3;
 
-template <typename T, int D, int G, int PB>
-__global__ void __launch_bounds__(kScoreThreads)
-score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int num_kv_heads,
-             const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
-             const int32_t* __restrict__ seq_lens, int page_size, int total_pages,
+__device__ __forceinline__ void sc_mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void sc_mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tWAIT_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+      "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void sc_mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void sc_mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+
+// the schedule both roles follow: groups of <= PG pages inside one request, over flat pages [begin, end)
+struct GroupIter {
+  int flat, end, req, req_end;
+  const int32_t* indptr;
+  __device__ GroupIter(int begin, int end_, int batch, const int32_t* page_indptr) : flat(begin), end(end_), indptr(page_indptr) {
+    int lo = 0, hi = batch;                      // largest req with indptr[req] <= begin
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (page_indptr[mid] <= begin) lo = mid; else hi = mid;
+    }
+    req = lo;
+    req_end = page_indptr[req + 1];
+  }
+  __device__ bool next(int pg, int& first, int& count, int& request) {
+    if (flat >= end) return false;
+    while (flat >= req_end) { ++req; req_end = indptr[req + 1]; }   // also skips empty requests
+    first = flat;
+    count = min(pg, min(req_end, end) - flat);
+    request = req;
+    flat += count;
+    return true;
+  }
+};
+
+template <typename T, int D, int PG, int HKV>
+__global__ void __launch_bounds__(kScThreads, 2)
+score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int batch,
+             const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices, int total_pages,
              float* __restrict__ scores) {
   constexpr int PER = Elem<T>::kPerVec;
-  constexpr int NVEC = D / PER;                 // 16-byte vectors per half row
-  constexpr int NI = (NVEC + G - 1) / G;        // vectors per lane per half row
-  constexpr int RW = kWarp / G;                 // summary rows per warp pass
-  constexpr int NPASS = kScorePagesPerWarp / RW;
-  constexpr int NWARPS = kScoreThreads / kWarp;
-  static_assert(D % PER == 0 && kWarp % G == 0 && PB % kScorePagesPerWarp == 0, "shape");
+  constexpr int ROW_ELEMS = 2 * D;               // [min | max] of one (page, KV head)
+  constexpr int NCH = ROW_ELEMS / PER;           // 16-byte chunks per row
+  constexpr int NIT = (NCH + kWarp - 1) / kWarp; // chunks per lane
+  constexpr int RPW = PG * HKV / kScConsumerWarps;   // rows per warp per group
+  constexpr int ROW_BYTES = ROW_ELEMS * (int)sizeof(T);
+  constexpr int PAGE_BYTES = HKV * ROW_BYTES;
+  constexpr int STAGE_BYTES = PG * PAGE_BYTES;
+  static_assert(ROW_ELEMS % PER == 0 && kScConsumerWarps % HKV == 0, "shape");
+  static_assert(RPW == 1 || RPW == 2 || RPW == 4 || RPW == 8, "rows per warp must be a power of two <= 8");
 
-  extern __shared__ float s_q[];                // [Hkv][2][D]: Qm (pairs with min), Qp (pairs with max)
-  const int i = blockIdx.y;
-  const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
-  const int page0 = blockIdx.x * PB;
-  if (page0 >= n_pages) return;
-  const int grp = num_q_heads / num_kv_heads;
-
-  for (int e = threadIdx.x; e < num_kv_heads * D; e += kScoreThreads) {
-    const int kvh = e / D, c = e % D;
-    const T* qrow = q + ((int64_t)i * num_q_heads + kvh * grp) * D + c;
-    float qp = 0.f, qm = 0.f;
-    for (int r = 0; r < grp; ++r) {
-      const float x = Elem<T>::to_float(qrow[(int64_t)r * D]);
-      qp += fmaxf(x, 0.f);
-      qm += fminf(x, 0.f);
-    }
-    s_q[(kvh * 2 + 0) * D + c] = qm;
-    s_q[(kvh * 2 + 1) * D + c] = qp;
-  }
-  __syncthreads();
+  extern __shared__ __align__(128) uint8_t smem[];
+  __shared__ __align__(8) uint64_t s_full[kScStages], s_empty[kScStages];
+  float* s_q = reinterpret_cast<float*>(smem + (size_t)kScStages * STAGE_BYTES);   // [HKV][2*D]: Qm | Qp
 
   const int warp = threadIdx.x / kWarp, lane = threadIdx.x % kWarp;
-  const int sub = lane % G, row_in_pass = lane / G;
-  const int row_base = page_indptr[i];
-  constexpr int NSUB = PB / kScorePagesPerWarp;
-  int cur_kvh = -1;
-  float qm[NI][PER], qp[NI][PER];
+  const int begin = (int)((int64_t)total_pages * blockIdx.x / gridDim.x);
+  const int end = (int)((int64_t)total_pages * (blockIdx.x + 1) / gridDim.x);
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kScStages; ++s) {
+      sc_mbar_init(smem_u32(&s_full[s]), 1);
+      sc_mbar_init(smem_u32(&s_empty[s]), kScConsumerWarps);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (begin >= end) return;
+  GroupIter it(begin, end, batch, page_indptr);
+  int first, count, req;
 
-  for (int u = warp; u < num_kv_heads * NSUB; u += NWARPS) {
-    const int kvh = u % num_kv_heads;
-    const int p_first = page0 + (u / num_kv_heads) * kScorePagesPerWarp;
-    if (p_first >= n_pages) continue;
-    if (kvh != cur_kvh) {
-      cur_kvh = kvh;
-#pragma unroll
-      for (int it = 0; it < NI; ++it) {
-        const int v = sub + it * G;
-#pragma unroll
-        for (int e = 0; e < PER; ++e) {
-          qm[it][e] = v < NVEC ? s_q[(kvh * 2 + 0) * D + v * PER + e] : 0.f;
-          qp[it][e] = v < NVEC ? s_q[(kvh * 2 + 1) * D + v * PER + e] : 0.f;
-        }
+  if (warp == kScConsumerWarps) {
+    // ---- producer: one bulk copy per page (all KV heads of the page are contiguous) ----------
+    for (int g = 0; it.next(PG, first, count, req); ++g) {
+      const int s = g % kScStages;
+      if (g >= kScStages) sc_mbar_wait(smem_u32(&s_empty[s]), ((g / kScStages) - 1) & 1);
+      const uint32_t bar = smem_u32(&s_full[s]);
+      if (lane == 0) sc_mbar_expect_tx(bar, (uint32_t)(count * PAGE_BYTES));
+      __syncwarp();
+      for (int l = lane; l < count; l += kWarp) {
+        const int64_t phys = page_indices[first + l];
+        bulk_g2s(smem_u32(smem + (size_t)s * STAGE_BYTES + (size_t)l * PAGE_BYTES),
+                 reinterpret_cast<const uint8_t*>(summary) + phys * PAGE_BYTES, (uint32_t)PAGE_BYTES, bar);
       }
     }
-    const int my_page = p_first + lane;
-    const int my_phys = my_page < n_pages ? page_indices[row_base + my_page] : -1;
-    float mine = 0.f;
-#pragma unroll 2
-    for (int pass = 0; pass < NPASS; ++pass) {
-      const int phys = __shfl_sync(0xffffffffu, my_phys, pass * RW + row_in_pass);
+    return;
+  }
+
+  // ---- consumers: warp w owns KV head w % HKV and rows w + 8k of every group ---------------------
+  const int grp = num_q_heads / HKV;
+  const int kvh = warp % HKV;
+  float qreg[NIT][PER];
+  int cur_req = -1;
+  for (int g = 0; it.next(PG, first, count, req); ++g) {
+    const int s = g % kScStages;
+    if (req != cur_req) {                        // new request: rebuild [Qm | Qp] for all KV heads (rare)
+      asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
+      for (int e = threadIdx.x; e < HKV * D; e += kScConsumerWarps * kWarp) {
+        const int h = e / D, c = e % D;
+        const T* qrow = q + ((int64_t)req * num_q_heads + h * grp) * D + c;
+        float qp = 0.f, qm = 0.f;
+        for (int r = 0; r < grp; ++r) {
+          const float x = Elem<T>::to_float(qrow[(int64_t)r * D]);
+          qp += fmaxf(x, 0.f);
+          qm += fminf(x, 0.f);
+        }
+        s_q[h * ROW_ELEMS + c] = qm;
+        s_q[h * ROW_ELEMS + D + c] = qp;
+      }
+      asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
+      cur_req = req;
+#pragma unroll
+      for (int t = 0; t < NIT; ++t) {
+        const int c = lane + t * kWarp;
+#pragma unroll
+        for (int e = 0; e < PER; ++e) qreg[t][e] = (NCH % kWarp == 0 || c < NCH) ? s_q[kvh * ROW_ELEMS + c * PER + e] : 0.f;
+      }
+    }
+    sc_mbar_wait(smem_u32(&s_full[s]), (g / kScStages) & 1);
+    const int rows = count * HKV;                // row r = page (r / HKV), head (r % HKV)
+    const uint8_t* stage = smem + (size_t)s * STAGE_BYTES + lane * 16;
+    uint4 v[RPW][NIT];
+#pragma unroll
+    for (int k = 0; k < RPW; ++k) {
+      const int r = warp + k * kScConsumerWarps;
+#pragma unroll
+      for (int t = 0; t < NIT; ++t) {
+        const bool ok = r < rows && (NCH % kWarp == 0 || lane + t * kWarp < NCH);
+        v[k][t] = ok ? *reinterpret_cast<const uint4*>(stage + r * ROW_BYTES + t * kWarp * 16) : make_uint4(0, 0, 0, 0);
+      }
+    }
+    __syncwarp();
+    if (lane == 0) sc_mbar_arrive(smem_u32(&s_empty[s]));    // stage consumed: its rows are in registers
+    float part[RPW];
+#pragma unroll
+    for (int k = 0; k < RPW; ++k) {
       float acc = 0.f;
-      if (phys >= 0) {
-        const T* row = summary + ((int64_t)phys * num_kv_heads + kvh) * 2 * D;
-        uint4 lo[NI], hi[NI];
 #pragma unroll
-        for (int it = 0; it < NI; ++it) {
-          const int v = sub + it * G;
-          if (NVEC % G == 0 || v < NVEC) {
-            lo[it] = ldg_stream(row + v * PER);
-            hi[it] = ldg_stream(row + D + v * PER);
-          } else {
-            lo[it] = make_uint4(0, 0, 0, 0);
-            hi[it] = make_uint4(0, 0, 0, 0);
-          }
-        }
+      for (int t = 0; t < NIT; ++t) {
+        float f[PER];
+        Elem<T>::unpack(v[k][t], f);
 #pragma unroll
-        for (int it = 0; it < NI; ++it) {
-          float a[PER], b[PER];
-          Elem<T>::unpack(lo[it], a);
-          Elem<T>::unpack(hi[it], b);
-#pragma unroll
-          for (int e = 0; e < PER; ++e) acc = fmaf(qm[it][e], a[e], fmaf(qp[it][e], b[e], acc));
-        }
+        for (int e = 0; e < PER; ++e) acc = fmaf(qreg[t][e], f[e], acc);
       }
-      acc = warp_sum<G>(acc);                    // every lane of the row's group holds the row score
-      const float s_r = __shfl_sync(0xffffffffu, acc, (lane % RW) * G);
-      if (lane / RW == pass) mine = s_r;         // lane r keeps the score of page p_first + r
+      part[k] = acc;
     }
-    if (my_page < n_pages) scores[(int64_t)kvh * total_pages + row_base + my_page] = mine;
+    // transposed butterfly: RPW partial sums over 32 lanes -> lanes [k*32/RPW, (k+1)*32/RPW) hold the total of row k
+    float tot;
+    if constexpr (RPW == 8) {
+      float a4[4], a2[2];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const bool up = lane & 16;
+        a4[j] = (up ? part[j + 4] : part[j]) + __shfl_xor_sync(0xffffffffu, up ? part[j] : part[j + 4], 16);
+      }
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const bool up = lane & 8;
+        a2[j] = (up ? a4[j + 2] : a4[j]) + __shfl_xor_sync(0xffffffffu, up ? a4[j] : a4[j + 2], 8);
+      }
+      const bool up = lane & 4;
+      tot = (up ? a2[1] : a2[0]) + __shfl_xor_sync(0xffffffffu, up ? a2[0] : a2[1], 4);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 2);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 1);
+    } else if constexpr (RPW == 4) {
+      float a2[2];
+#pragma unroll
+      for (int j = 0; j < 2; ++j) {
+        const bool up = lane & 16;
+        a2[j] = (up ? part[j + 2] : part[j]) + __shfl_xor_sync(0xffffffffu, up ? part[j] : part[j + 2], 16);
+      }
+      const bool up = lane & 8;
+      tot = (up ? a2[1] : a2[0]) + __shfl_xor_sync(0xffffffffu, up ? a2[0] : a2[1], 8);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 4);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 2);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 1);
+    } else if constexpr (RPW == 2) {
+      const bool up = lane & 16;
+      tot = (up ? part[1] : part[0]) + __shfl_xor_sync(0xffffffffu, up ? part[0] : part[1], 16);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 8);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 4);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 2);
+      tot += __shfl_xor_sync(0xffffffffu, tot, 1);
+    } else {
+      tot = warp_sum(part[0]);
+    }
+    constexpr int LPR = kWarp / RPW;             // lanes per row after the butterfly
+    const int r = warp + (lane / LPR) * kScConsumerWarps;
+    if ((lane % LPR) == 0 && r < rows) scores[(int64_t)kvh * total_pages + first + r / HKV] = tot;
   }
 }
 
 bool score_geometry_supported(const vx_geom& g) {
   if (g.agg != VX_AGG_SUM) return false;
+  const int hkv = g.num_kv_heads;
+  if (hkv != 1 && hkv != 2 && hkv != 4 && hkv != 8) return false;   // a consumer warp owns one KV head
   if (g.dtype == VX_DT_BF16) return g.qk_dim == 128 || g.qk_dim == 64 || g.qk_dim == 576 || g.qk_dim == 256;
   return g.qk_dim == 64 || g.qk_dim == 128;
 }
 
-template <typename T, int D, int G>
+template <typename T, int D, int PG, int HKV>
 static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
                                   float* scores, cudaStream_t s) {
-  constexpr int PB = 64;
   const vx_geom& g = c->g;
-  dim3 grid((pt.max_pages_per_req + PB - 1) / PB, pt.batch);
-  const size_t smem = (size_t)g.num_kv_heads * 2 * D * sizeof(float);
-  score_kernel<T, D, G, PB><<<grid, kScoreThreads, smem, s>>>(
-      static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, g.num_kv_heads,
-      pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, pt.total_pages, scores);
+  constexpr size_t page_bytes = (size_t)HKV * 2 * D * sizeof(T);
+  constexpr size_t smem = kScStages * PG * page_bytes + (size_t)HKV * 2 * D * sizeof(float);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(score_kernel<T, D, PG, HKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  int ctas = c->num_sms * 2;                     // two CTAs per SM (3 x ~32 KB stages each)
+  const int min_pages = 2 * PG;                  // do not spread tiny inputs over every SM
+  if ((int64_t)ctas * min_pages > pt.total_pages) ctas = (pt.total_pages + min_pages - 1) / min_pages;
+  if (ctas < 1) ctas = 1;
+  score_kernel<T, D, PG, HKV><<<ctas, kScThreads, smem, s>>>(
+      static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, pt.batch, pt.page_indptr,
+      pt.page_indices, pt.total_pages, scores);
   c->launches += 1;
   return cudaGetLastError();
 }
 
+// PG pages per stage so that a stage is ~32 KB and every consumer warp gets 1..8 rows of it
+template <typename T, int D>
+static cudaError_t launch_score_d(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
+                                  float* scores, cudaStream_t s) {
+  constexpr int row_bytes = 2 * D * (int)sizeof(T);
+  constexpr int pg8 = 32768 / (8 * row_bytes) < 1 ? 1 : 32768 / (8 * row_bytes);   // Hkv = 8
+  switch (c->g.num_kv_heads) {
+    case 8: return launch_score_t<T, D, (pg8 > 8 ? 8 : pg8), 8>(c, q, summary, pt, scores, s);
+    case 4: return launch_score_t<T, D, (2 * pg8 > 16 ? 16 : 2 * pg8), 4>(c, q, summary, pt, scores, s);
+    case 2: return launch_score_t<T, D, (4 * pg8 > 32 ? 32 : (4 * pg8 < 4 ? 4 : 4 * pg8)), 2>(c, q, summary, pt, scores, s);
+    case 1: return launch_score_t<T, D, (8 * pg8 > 32 ? 32 : (8 * pg8 < 8 ? 8 : 8 * pg8)), 1>(c, q, summary, pt, scores, s);
+  }
+  return cudaErrorInvalidValue;
+}
+
 cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
                               float* scores, cudaStream_t s) {
-  if (pt.batch == 0 || pt.max_pages_per_req == 0) return cudaSuccess;
+  if (pt.batch == 0 || pt.total_pages == 0) return cudaSuccess;
   const vx_geom& g = c->g;
   if (g.dtype == VX_DT_BF16) {
     switch (g.qk_dim) {
-      case 64: return launch_score_t<__nv_bfloat16, 64, 8>(c, q, summary, pt, scores, s);
-      case 128: return launch_score_t<__nv_bfloat16, 128, 8>(c, q, summary, pt, scores, s);
-      case 256: return launch_score_t<__nv_bfloat16, 256, 16>(c, q, summary, pt, scores, s);
-      case 576: return launch_score_t<__nv_bfloat16, 576, 32>(c, q, summary, pt, scores, s);
+      case 64: return launch_score_d<__nv_bfloat16, 64>(c, q, summary, pt, scores, s);
+      case 128: return launch_score_d<__nv_bfloat16, 128>(c, q, summary, pt, scores, s);
+      case 256: return launch_score_d<__nv_bfloat16, 256>(c, q, summary, pt, scores, s);
+      case 576: return launch_score_d<__nv_bfloat16, 576>(c, q, summary, pt, scores, s);
     }
   } else {
     switch (g.qk_dim) {
-      case 64: return launch_score_t<float, 64, 8>(c, q, summary, pt, scores, s);
-      case 128: return launch_score_t<float, 128, 16>(c, q, summary, pt, scores, s);
+      case 64: return launch_score_d<float, 64>(c, q, summary, pt, scores, s);
+      case 128: return launch_score_d<float, 128>(c, q, summary, pt, scores, s);
     }
   }
   return cudaErrorInvalidValue;
