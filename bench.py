@@ -79,6 +79,7 @@ class ClockSampler(threading.Thread):
     def __init__(self, index):
         super().__init__(daemon=True)
         self.index, self.stop_flag, self.samples, self.reasons, self.max_mhz = index, False, [], set(), None
+        self.ready = threading.Event()
 
     def run(self):
         try:
@@ -95,9 +96,11 @@ class ClockSampler(threading.Thread):
                 except Exception:
                     r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(h)
                 self.reasons |= {k for k, bit in names.items() if r & bit}
-                time.sleep(0.02)
+                self.ready.set()
+                time.sleep(0.001)
         except Exception as e:  # NVML unavailable: report that rather than guessing
             self.reasons.add(f"nvml_unavailable:{type(e).__name__}")
+        self.ready.set()
 
     def result(self):
         self.stop_flag = True
@@ -128,6 +131,7 @@ class Runner:
         self.sel_logical = torch.empty_like(self.sel_phys)
         self.sel_count = torch.empty(s.batch, s.num_kv_heads, dtype=torch.int32, device=device)
         self.flush = torch.empty(512 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
+        self.flush_rd = torch.zeros(64 << 20, dtype=torch.int32, device=device)  # 256 MiB read sweep
         pin = lambda t: t.cpu().contiguous().pin_memory()
         self.h = dict(q=pin(w.q), indptr=pin(w.page_indptr), indices=pin(w.page_indices), seq=pin(w.seq_lens),
                       budget=pin(w.budget), out=torch.empty_like(self.out, device="cpu").pin_memory(),
@@ -160,16 +164,23 @@ class Runner:
         self.ctx.sparse_paged_decode(self.w.q, self.pool, self.pt, self.sel_phys, self.sel_logical, self.sel_count,
                                      self.w.max_budget, self.out, self.lse)
 
+    def flush_l2(self):
+        """Cold L2 for the next step: a 512 MiB write sweep, then a 256 MiB read sweep so the L2 is left
+        full of CLEAN foreign lines (a write-only flush leaves ~126 MB of dirty lines whose write-back
+        the timed step would pay for).  Outside the timed events.  DESIGN.md section 8.1."""
+        self.flush.zero_()
+        self.flush_rd.max()
+
     def time_device(self, fn, steps, warmup):
         """per-step CUDA-event times (ms) on the current stream, L2 flushed before every step."""
         torch = self.torch
         for _ in range(warmup):
-            self.flush.zero_()
+            self.flush_l2()
             fn()
         torch.cuda.synchronize()
         evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         for a, b in evs:
-            self.flush.zero_()
+            self.flush_l2()
             a.record()
             fn()
             b.record()
@@ -181,7 +192,7 @@ class Runner:
         torch = self.torch
         out = []
         for it in range(warmup + steps):
-            self.flush.zero_()
+            self.flush_l2()
             torch.cuda.synchronize()
             t0 = time.perf_counter()
             fn()
@@ -278,6 +289,7 @@ def main():
     barrier()
     sampler = ClockSampler(local)
     sampler.start()
+    sampler.ready.wait(timeout=10)          # NVML is up and the first sample is in before the timed region
     times = r.time_device(r.step, args.steps, max(args.warmup, 3))
     launches_per_step = r.ctx.last_launch_count
     barrier()
@@ -334,7 +346,7 @@ def main():
                 "config": {"workload": args.config, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
                            "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
                            "seq_len": list(s.seq_len), "budget_pages": w.max_budget,
-                           "l2": "flushed before every step (512 MiB memset)", "parallelism": f"dp{world}"},
+                           "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"},
                 "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
                 "step_bytes": bytes_, "stage_us": stage, "roofline": roofline, "cpu_baseline": cpu,
                 "e2e": {"value": e2e_ms * 1e3, "unit": "us", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
