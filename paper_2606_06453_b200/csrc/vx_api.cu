@@ -31,6 +31,7 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   w.sel_count = static_cast<int32_t*>(take(B * Hkv * 4));
   w.part_o = static_cast<float*>(take(B * Hq * kMaxSplits * (size_t)g.v_dim * 4));
   w.part_lse = static_cast<float*>(take(B * Hq * kMaxSplits * 4));
+  w.unit_counter = static_cast<int32_t*>(take(B * Hkv * 4));
   w.h_q = take(B * Hq * (size_t)g.qk_dim * esz);
   w.h_indptr = static_cast<int32_t*>(take((B + 1) * 4));
   w.h_indices = static_cast<int32_t*>(take((size_t)max_total_pages * 4));
@@ -148,6 +149,15 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->err[0] = 0;
   const char* fg = getenv("VX_FORCE_GENERIC");
   c->force_generic = fg && fg[0] == '1';
+  const char* np = getenv("VX_NO_PDL");
+  c->use_pdl = !(np && np[0] == '1');
+  // split-arrival counters start at zero and every step leaves them at zero
+  e = cudaMemset(c->ws.unit_counter, 0, (size_t)(max_batch > 0 ? max_batch : 1) * g->num_kv_heads * 4);
+  if (e == cudaSuccess) e = cudaDeviceSynchronize();
+  if (e != cudaSuccess) {
+    delete c;
+    return fail(nullptr, VX_ERR_CUDA, "workspace initialisation: %s", cudaGetErrorString(e));
+  }
   *out = c;
   return VX_OK;
 }
@@ -193,10 +203,11 @@ vx_status vx_topk_pages(vx_ctx* c, const float* scores, const vx_page_table* pt,
 
 static vx_status decode_dispatch(vx_ctx* c, const void* q, const vx_kv_pool* pool, const vx_page_table* pt,
                                  const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
-                                 int32_t max_budget, void* out, float* lse, cudaStream_t s) {
+                                 int32_t max_budget, void* out, float* lse, cudaStream_t s,
+                                 const DecodeOpts& opt = DecodeOpts()) {
   cudaError_t e = c->g.kv_shared
-                      ? launch_decode_mla(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s)
-                      : launch_decode_gqa(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
+                      ? launch_decode_mla(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt)
+                      : launch_decode_gqa(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt);
   return check_cuda(c, e, "vx_sparse_paged_decode");
 }
 
@@ -231,14 +242,23 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   int32_t* sp = sel_phys ? sel_phys : c->ws.sel_phys;
   int32_t* sl = sel_logical ? sel_logical : c->ws.sel_logical;
   int32_t* sc = sel_count ? sel_count : c->ws.sel_count;
-  if (flags & VX_STEP_UPDATE_SUMMARY)
-    if (vx_status st = check_cuda(c, launch_summary_update(c, *pool, *pt, nullptr, summary, s), "summary update"))
+  // (a1) With n_local >= 1 the newest page is a forced page: its score never decides the selection and its keys
+  // are staged by the decode kernel anyway, so the decode kernel rebuilds its summary (same result, no extra
+  // launch, no extra HBM bytes).  Otherwise the summary kernel runs first.
+  DecodeOpts opt;
+  opt.pdl = c->use_pdl;
+  if (flags & VX_STEP_UPDATE_SUMMARY) {
+    if (c->g.n_local >= 1 && decode_folds_summary(c)) {
+      opt.summary_upd = summary;
+    } else if (vx_status st = check_cuda(c, launch_summary_update(c, *pool, *pt, nullptr, summary, s), "summary update")) {
       return st;
+    }
+  }
   if (vx_status st = check_cuda(c, launch_page_score(c, q, summary, *pt, c->ws.scores, s), "page score")) return st;
-  if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, s),
-                                "top-k pages"))
+  if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, s,
+                                                     c->use_pdl), "top-k pages"))
     return st;
-  return decode_dispatch(c, q, pool, pt, sp, sl, sc, max_budget, out, lse, s);
+  return decode_dispatch(c, q, pool, pt, sp, sl, sc, max_budget, out, lse, s, opt);
 }
 
 vx_status vx_sparse_decode_step_host(vx_ctx* c, const void* h_q, const vx_kv_pool* pool, void* summary,

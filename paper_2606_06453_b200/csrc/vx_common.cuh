@@ -73,4 +73,56 @@ __device__ __forceinline__ uint32_t float_to_key(float f) {
 
 __device__ __forceinline__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
+// ---- programmatic dependent launch (PDL): the kernels of one decode step are chained so that a
+// kernel's prologue (index loads, barrier / TMEM set-up, Q staging) overlaps its predecessor's tail.
+// pdl_wait(): everything the preceding kernel wrote is visible after it (no-op without the attribute).
+// pdl_trigger(): this CTA no longer needs the next kernel to stay away.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+__device__ __forceinline__ float ldcg_f32(const float* p) {
+  float v;
+  asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));
+  return v;
+}
+
+// ---- (a5) in-kernel LSE merge: the LAST split CTA of a unit to finish merges the unit's
+// partials.  Call with the whole CTA after its own partial (o, lse) is written.  Returns true in the CTA
+// that must merge.  counter is zero on entry to the step and is left zero.
+__device__ __forceinline__ bool last_split_arrives(int* counter, int num_splits, int* s_flag) {
+  __threadfence();                               // this thread's partial stores are visible device-wide
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const int old = atomicAdd(counter, 1);
+    const bool last = old == num_splits - 1;
+    if (last) *counter = 0;                      // self-cleaning: ready for the next step
+    *s_flag = last;
+  }
+  __syncthreads();
+  const bool last = *s_flag != 0;
+  if (last) __threadfence();                     // acquire the other CTAs' partials
+  return last;
+}
+
+// merge rows [row0, row0 + n_rows) of part_o [rows, n_part, v_dim] / part_lse [rows, n_part] into out / lse
+template <typename T>
+__device__ __forceinline__ void merge_partials(const float* part_o, const float* part_lse, int64_t row0, int n_rows,
+                                               int n_part, int v_dim, T* out, float* lse) {
+  for (int e = threadIdx.x; e < n_rows * v_dim; e += blockDim.x) {
+    const int64_t row = row0 + e / v_dim;
+    const int c = e % v_dim;
+    const float* ls = part_lse + row * n_part;
+    float mx = -INFINITY;
+    for (int s = 0; s < n_part; ++s) mx = fmaxf(mx, ldcg_f32(ls + s));
+    float z = 0.f, o = 0.f;
+    for (int s = 0; s < n_part; ++s) {
+      const float w = mx == -INFINITY ? 0.f : __expf(ldcg_f32(ls + s) - mx);
+      z += w;
+      if (w != 0.f) o = fmaf(w, ldcg_f32(part_o + (row * n_part + s) * v_dim + c), o);
+    }
+    out[row * v_dim + c] = Elem<T>::from_float(z > 0.f ? o / z : 0.f);
+    if (c == 0 && lse != nullptr) lse[row] = z > 0.f ? mx + logf(z) : -INFINITY;
+  }
+}
+
 }  // namespace vx

@@ -58,6 +58,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
                       const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ sel_phys,
                       const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count,
                       int max_budget, int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
+                      int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd,
                       __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out) {
   constexpr int ROWB = D * 2;                 // bytes per token row
   constexpr int CH = ROWB / 16;               // 16-byte chunks per row
@@ -66,22 +67,15 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   constexpr int CP_ITERS = kGqaPage * CH / kWarp;
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float s_m[kGqaWarps][8], s_l[kGqaWarps][8];
-  __shared__ int s_valid[kGqaWarps][kGqaStages];   // valid tokens of the page staged in each slot
+  __shared__ int s_valid[kGqaWarps][kGqaStages];   // valid tokens of the page staged in each slot (bit 8: newest page)
+  __shared__ int s_phys[kGqaWarps][kGqaStages];    // its physical id
+  __shared__ int s_last;
 
   const int split = blockIdx.x, kvh = blockIdx.y, i = blockIdx.z;
   const int warp = threadIdx.x / kWarp, lane = threadIdx.x % kWarp;
   const int grp = num_q_heads / num_kv_heads;
   const int n_tok = seq_lens[i];
-  const int cnt = sel_count[i * num_kv_heads + kvh];
-  const int per_split = (cnt + num_splits - 1) / num_splits;
-  const int r_begin = min(split * per_split, cnt), r_end = min(r_begin + per_split, cnt);
-  const int32_t* phys_list = sel_phys + ((int64_t)i * num_kv_heads + kvh) * max_budget;
-  const int32_t* log_list = sel_logical + ((int64_t)i * num_kv_heads + kvh) * max_budget;
-  // this warp's pages: r_begin + warp, + kGqaWarps, ...
-  const int my_pages = r_end - r_begin > warp ? (r_end - r_begin - warp + kGqaWarps - 1) / kGqaWarps : 0;
-
-  uint8_t* ring = smem + (size_t)warp * kGqaStages * 2 * PAGEB;
-  const uint32_t ring_u32 = smem_u32(ring);
+  const int newest_page = (n_tok - 1) / kGqaPage;
 
   // Q^T as the B operand: qb[ks] = Q[head lane/4][16*ks + 2*(lane%4) + {0,1}], [.. + 8 ..]
   uint32_t qb[KS][2];
@@ -95,6 +89,18 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
       qb[ks][1] = h < grp ? *reinterpret_cast<const uint32_t*>(qrow + c + 8) : 0u;
     }
   }
+  pdl_wait();                                   // the selection lists come from the preceding kernel of the step
+
+  const int cnt = sel_count[i * num_kv_heads + kvh];
+  const int per_split = (cnt + num_splits - 1) / num_splits;
+  const int r_begin = min(split * per_split, cnt), r_end = min(r_begin + per_split, cnt);
+  const int32_t* phys_list = sel_phys + ((int64_t)i * num_kv_heads + kvh) * max_budget;
+  const int32_t* log_list = sel_logical + ((int64_t)i * num_kv_heads + kvh) * max_budget;
+  // this warp's pages: r_begin + warp, + kGqaWarps, ...
+  const int my_pages = r_end - r_begin > warp ? (r_end - r_begin - warp + kGqaWarps - 1) / kGqaWarps : 0;
+
+  uint8_t* ring = smem + (size_t)warp * kGqaStages * 2 * PAGEB;
+  const uint32_t ring_u32 = smem_u32(ring);
 
   int id_phys = 0, id_valid = 0;                // lane j: this warp's (base + j)-th page
   auto fetch_ids = [&](int base) {
@@ -102,7 +108,8 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     if (p < my_pages) {
       const int r = r_begin + warp + p * kGqaWarps;
       id_phys = phys_list[r];
-      id_valid = min(kGqaPage, n_tok - log_list[r] * kGqaPage);
+      const int lg = log_list[r];
+      id_valid = min(kGqaPage, n_tok - lg * kGqaPage) | (lg == newest_page ? 256 : 0);
     }
   };
   auto issue = [&](int p) {                     // all lanes: copy page p of this warp into slot p % stages
@@ -110,15 +117,16 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     const int valid = __shfl_sync(0xffffffffu, id_valid, p & 31);
     const int64_t base = (int64_t)phys * stride_page + (int64_t)kvh * stride_head;
     const uint32_t dst = ring_u32 + (uint32_t)(p % kGqaStages) * 2 * PAGEB;
-    if (lane == 0) s_valid[warp][p % kGqaStages] = valid;
+    if (lane == 0) { s_valid[warp][p % kGqaStages] = valid; s_phys[warp][p % kGqaStages] = phys; }
+    const int nv = valid & 255;
 #pragma unroll
     for (int it = 0; it < CP_ITERS; ++it) {
       const int x = it * kWarp + lane;
       const int t = x / CH, c = x % CH;
       const uint32_t off = t * ROWB + ((c ^ (t & 7)) * 16);
       const int64_t src = base + (int64_t)t * stride_token + c * 8;
-      cp_async16_zfill(dst + off, kpool + src, t < valid);
-      cp_async16_zfill(dst + PAGEB + off, vpool + src, t < valid);
+      cp_async16_zfill(dst + off, kpool + src, t < nv);
+      cp_async16_zfill(dst + PAGEB + off, vpool + src, t < nv);
     }
   };
 
@@ -137,7 +145,9 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   for (int p = 0; p < my_pages; ++p) {
     cp_async_wait<kGqaStages - 2>();            // page p has landed (this lane's copies)
     __syncwarp();                               // ... and every lane's; also: all lanes are done with page p-1
-    const int valid = s_valid[warp][p % kGqaStages];
+    const int valid_enc = s_valid[warp][p % kGqaStages];
+    const int valid = valid_enc & 255;
+    const int phys_p = s_phys[warp][p % kGqaStages];
     {
       const int nxt = p + kGqaStages - 1;       // refill the slot page p-1 used
       if ((nxt & 31) == 0 && nxt < my_pages) fetch_ids(nxt);   // ids of pages nxt .. nxt+31 (p's were read above)
@@ -145,6 +155,35 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
       cp_async_commit();
     }
     const uint32_t kst = ring_u32 + (uint32_t)(p % kGqaStages) * 2 * PAGEB, vst = kst + PAGEB;
+
+    if (summary_upd != nullptr && (valid_enc & 256)) {
+      // (a1) this is the request's newest page: rebuild its min / max summary from the staged keys
+      // (exact in bf16).  Lane owns W consecutive 32-bit words (2 channels each) of the row.
+      constexpr int W = ROWB / 128;
+      const int byte0 = lane * W * 4, c = byte0 / 16, o16 = byte0 % 16;
+      __nv_bfloat162 lo[W], hi[W];
+#pragma unroll
+      for (int w = 0; w < W; ++w) {
+        const uint32_t x = *reinterpret_cast<const uint32_t*>(ring + (size_t)(p % kGqaStages) * 2 * PAGEB + o16 + w * 4 + (c * 16));
+        lo[w] = hi[w] = *reinterpret_cast<const __nv_bfloat162*>(&x);       // token 0 (c ^ 0 = c)
+      }
+      for (int t = 1; t < valid; ++t) {
+#pragma unroll
+        for (int w = 0; w < W; ++w) {
+          const uint32_t x = *reinterpret_cast<const uint32_t*>(ring + (size_t)(p % kGqaStages) * 2 * PAGEB + t * ROWB +
+                                                                ((c ^ (t & 7)) * 16) + o16 + w * 4);
+          const __nv_bfloat162 v = *reinterpret_cast<const __nv_bfloat162*>(&x);
+          lo[w] = __hmin2(lo[w], v);
+          hi[w] = __hmax2(hi[w], v);
+        }
+      }
+      __nv_bfloat16* dst = summary_upd + (((int64_t)phys_p * num_kv_heads + kvh) * 2) * D + lane * W * 2;
+#pragma unroll
+      for (int w = 0; w < W; ++w) {
+        *reinterpret_cast<__nv_bfloat162*>(dst + 2 * w) = lo[w];
+        *reinterpret_cast<__nv_bfloat162*>(dst + D + 2 * w) = hi[w];
+      }
+    }
 
     // S^T[16 tokens x 8 heads] = K[16 x D] . Q^T
     float s[4] = {0.f, 0.f, 0.f, 0.f};
@@ -194,6 +233,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     }
   }
   cp_async_wait<0>();
+  pdl_trigger();
 
   // per-warp denominators: sum the lane partials of each head column
 #pragma unroll
@@ -241,6 +281,10 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
       if (d == 0) part_lse[head_row * num_splits + split] = lse;
     }
   }
+  if (num_splits > 1) {                         // (a5) the last split of this (request, KV head) merges by LSE
+    if (last_split_arrives(unit_counter + i * num_kv_heads + kvh, num_splits, &s_last))
+      merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads + kvh * grp, grp, num_splits, D, out, lse_out);
+  }
 }
 
 bool gqa_mma_supported(const vx_geom& g) {
@@ -252,7 +296,7 @@ bool gqa_mma_supported(const vx_geom& g) {
 template <int D>
 static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                     const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
-                                    int32_t max_budget, void* out, float* lse, cudaStream_t s) {
+                                    int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
   const vx_geom& g = c->g;
   constexpr int smem = kGqaWarps * kGqaStages * 2 * kGqaPage * D * 2;
   static bool attr_set = false;
@@ -261,31 +305,34 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  // splits: cover the SMs (2 CTAs each) about twice, but keep >= 2 pages per warp per split
+  // splits: whole waves of equal CTAs.  cost(sp) = waves x (pages per warp + ~3 pages of pipeline fill)
   const int units = pt.batch * g.num_kv_heads;
-  int splits = (c->num_sms * 2 * 2 + units - 1) / units;
-  const int cap = (max_budget + kGqaWarps * 2 - 1) / (kGqaWarps * 2);
-  if (splits > cap) splits = cap;
-  if (splits > kMaxSplits) splits = kMaxSplits;
-  if (splits < 1) splits = 1;
+  const int slots = c->num_sms * 2;              // 96 KB of shared memory per CTA -> 2 CTAs per SM
+  int splits = 1, best_cost = 1 << 30;
+  for (int sp = 1; sp <= kMaxSplits && sp <= max_budget; ++sp) {
+    const int waves = (units * sp + slots - 1) / slots;
+    const int cost = waves * (((max_budget + sp - 1) / sp + kGqaWarps - 1) / kGqaWarps + 3);
+    if (cost < best_cost) { best_cost = cost; splits = sp; }
+  }
   dim3 grid(splits, g.num_kv_heads, pt.batch);
-  decode_gqa_mma_kernel<D><<<grid, kGqaWarps * kWarp, smem, s>>>(
+  cudaError_t e = launch_kernel(decode_gqa_mma_kernel<D>, grid, dim3(kGqaWarps * kWarp), (size_t)smem, s, opt.pdl,
       static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(pool.k),
       static_cast<const __nv_bfloat16*>(pool.v), pool.stride_page, pool.stride_token, pool.stride_head,
       g.num_q_heads, g.num_kv_heads, g.sm_scale * kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget,
-      splits, c->ws.part_o, c->ws.part_lse, static_cast<__nv_bfloat16*>(out), lse);
+      splits, c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd),
+      static_cast<__nv_bfloat16*>(out), lse);
   c->launches += 1;
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess || splits == 1) return e;
-  return launch_combine(c, pt.batch, splits, out, lse, s);
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
+
+bool decode_folds_summary(const vx_ctx* c) { return !c->force_generic && gqa_mma_supported(c->g); }
 
 cudaError_t launch_decode_gqa_mma(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
-                                  int32_t max_budget, void* out, float* lse, cudaStream_t s) {
+                                  int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
   if (c->g.qk_dim == 128)
-    return launch_gqa_mma_t<128>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
-  return launch_gqa_mma_t<64>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
+    return launch_gqa_mma_t<128>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt);
+  return launch_gqa_mma_t<64>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt);
 }
 
 }  // namespace vx

@@ -371,7 +371,7 @@ bool mla_tc_supported(const vx_geom& g) {
 
 cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                  const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
-                                 int32_t max_budget, void* out, float* lse, cudaStream_t s) {
+                                 int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
   const vx_geom& g = c->g;
   static bool attr_set = false;
   if (!attr_set) {

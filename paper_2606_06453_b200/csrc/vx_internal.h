@@ -16,6 +16,7 @@ struct Workspace {               // device pointers carved from the caller's wor
   int32_t* sel_count;            // [max_batch, Hkv]
   float* part_o;                 // [max_batch, Hq, kMaxSplits, v_dim]
   float* part_lse;               // [max_batch, Hq, kMaxSplits]
+  int32_t* unit_counter;         // [max_batch, Hkv] split-arrival counters; zero between steps
   // staging for vx_sparse_decode_step_host
   void* h_q;                     // [max_batch, Hq, qk_dim] elements
   int32_t* h_indptr;             // [max_batch + 1]
@@ -41,10 +42,36 @@ struct vx_ctx {
   vx::Workspace ws;
   int32_t launches;              // kernels enqueued by the last compute call
   bool force_generic;            // VX_FORCE_GENERIC=1 in the environment: CUDA-core decode path only (debug)
+  bool use_pdl;                  // chain the kernels of a step with programmatic dependent launch (VX_NO_PDL=1: off)
   char err[512];
 };
 
 namespace vx {
+
+// One kernel launch; pdl = allow it to start while its predecessor in the stream drains (the kernel
+// itself calls pdl_wait() before touching what the predecessor wrote).
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t s,
+                                 bool pdl, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
+// how a decode launch is embedded in a step
+struct DecodeOpts {
+  void* summary_upd = nullptr;   // non-null: also rebuild the summary of each request's newest page (a1), whose
+                                 // keys the kernel stages anyway (it is a forced local page)
+  bool pdl = false;              // launched as a programmatic dependent of the preceding kernel
+};
 
 // every launcher returns cudaGetLastError() after its launches and adds to ctx->launches
 cudaError_t launch_summary_update(vx_ctx* c, const vx_kv_pool& pool, const vx_page_table& pt,
@@ -53,24 +80,25 @@ cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, con
                               float* scores, cudaStream_t s);
 cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
-                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s);
+                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl = false);
 cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
-                              cudaStream_t s);
+                              cudaStream_t s, const DecodeOpts& opt = DecodeOpts());
 cudaError_t launch_decode_gqa_mma(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* sel_phys, const int32_t* sel_logical,
                                   const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
-                                  cudaStream_t s);
+                                  cudaStream_t s, const DecodeOpts& opt = DecodeOpts());
 bool gqa_mma_supported(const vx_geom& g);
+bool decode_folds_summary(const vx_ctx* c);   // the decode path of this context can take DecodeOpts::summary_upd
 cudaError_t launch_decode_mla(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
-                              cudaStream_t s);
+                              cudaStream_t s, const DecodeOpts& opt = DecodeOpts());
 cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                  const int32_t* sel_phys, const int32_t* sel_logical,
                                  const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
-                                 cudaStream_t s);
+                                 cudaStream_t s, const DecodeOpts& opt = DecodeOpts());
 bool mla_tc_supported(const vx_geom& g);
 cudaError_t launch_combine(vx_ctx* c, int32_t batch, int num_splits, void* out, float* lse,
                            cudaStream_t s);

@@ -99,6 +99,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  pdl_trigger();                                // single-wave persistent grid: the selection kernel may queue up behind us
   if (begin >= end) return;
   GroupIter it(begin, end, batch, page_indptr);
   int first, count, req;

@@ -1,73 +1,70 @@
 // vx_topk.cu -- (a3) exact top-k page selection per (request, KV head).
-// PAPER.md:92 Eq.3 (arg-top-k of the block scores), :194 (radix top-k), :280 (first block and last
-// blocks always attended; readings G4-G6: budget includes the forced pages, ties go to the
-// lower logical page, k >= P selects everything).
+// PAPER.md:92 Eq.3 (arg-top-k of the block scores), :194 (radix top-k, "highly sensitive to the score
+// distribution"), :280 (first block and last blocks always attended; readings G4-G6: the
+// budget includes the forced pages, ties go to the lower logical page, k >= P selects everything).
 //
-// One CTA per (request, KV head).  Scores become order-preserving uint32 keys held in shared memory
-// (forced pages get the reserved key 0xFFFFFFFF so they always win); a 4-pass, 8-bit MSB radix
-// select finds the k-th largest key and how many pages equal to it are still needed; a final
-// ordered pass emits the selection in ascending logical order (so ties resolve to the lowest
-// index and the partial last page comes last) together with the physical page ids.
+// One CTA per (request, KV head).  Scores become order-preserving uint32 keys held in shared memory.
+// The select is a radix select made insensitive to the score distribution: the block first reduces
+// the min / max key of the non-forced pages and histograms (key - min) >> shift into 2048 bins that
+// span exactly that range, so one pass resolves 11 bits of the LIVE range (page scores of one request
+// cluster in a few exponent values; a fixed MSB-first digit would spend its first passes on bits that
+// are identical for every page).  The bin that holds the k-th key usually has a handful of members:
+// they are ranked directly (all-pairs count in shared memory); only if it holds more than kList keys
+// (heavy ties) the select recurses into that bin, 11 more bits per pass, down to single key values.
+// The result is the exact threshold key and how many keys equal to it are taken; the ordered emission
+// then resolves ties to the lowest logical index and writes ids in ascending logical order (so the
+// partial last page comes last) together with the physical page ids.
 // Integer work on a few KB per problem -- latency-bound, not bandwidth-bound.
 #include "vx_common.cuh"
 #include "vx_internal.h"
 
 namespace vx {
 
-constexpr int kTopkThreads = 512;
-constexpr int kTopkWarps = kTopkThreads / kWarp;
 constexpr int kTopkSmemKeys = 48 * 1024;        // keys cached in shared memory (192 KB); more -> re-read scores
+constexpr int kBins = 2048;                     // 11 bits per pass
+constexpr int kBinBits = 11;
+constexpr int kList = 256;                      // threshold-bin members ranked directly
+constexpr uint32_t kForcedKey = 0xFFFFFFFFu;    // not the key of any finite float
 
+__device__ __forceinline__ bool page_forced(int j, int n_pages, int n_sink, int n_local) {
+  return (j < n_sink) || (j >= n_pages - n_local);
+}
 __device__ __forceinline__ uint32_t page_key(const float* __restrict__ sc, int j, int n_pages, int n_sink,
                                              int n_local) {
-  const bool forced = (j < n_sink) || (j >= n_pages - n_local);
-  return forced ? 0xFFFFFFFFu : float_to_key(sc[j]);
+  return page_forced(j, n_pages, n_sink, n_local) ? kForcedKey : float_to_key(sc[j]);
 }
 
-// inclusive block scan of two counters; returns exclusive prefix, totals via smem
-__device__ __forceinline__ int2 block_exclusive_scan2(int2 v, int2* s_warp /*[kTopkWarps]*/, int2* total) {
-  const int lane = threadIdx.x % kWarp, warp = threadIdx.x / kWarp;
-  int2 inc = v;
-#pragma unroll
-  for (int o = 1; o < kWarp; o <<= 1) {
-    const int ax = __shfl_up_sync(0xffffffffu, inc.x, o), ay = __shfl_up_sync(0xffffffffu, inc.y, o);
-    if (lane >= o) { inc.x += ax; inc.y += ay; }
-  }
-  if (lane == kWarp - 1) s_warp[warp] = inc;
-  __syncthreads();
-  int2 base = make_int2(0, 0), tot = make_int2(0, 0);
-  for (int w = 0; w < kTopkWarps; ++w) {
-    const int2 t = s_warp[w];
-    if (w < warp) { base.x += t.x; base.y += t.y; }
-    tot.x += t.x; tot.y += t.y;
-  }
-  *total = tot;
-  return make_int2(base.x + inc.x - v.x, base.y + inc.y - v.y);
-}
-
-__global__ void __launch_bounds__(kTopkThreads)
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS)
 topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
             const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
             const int32_t* __restrict__ seq_lens, int page_size, const int32_t* __restrict__ budget,
             int n_sink, int n_local, int max_budget, int smem_keys, int32_t* __restrict__ sel_phys,
             int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count) {
+  constexpr int WARPS = THREADS / kWarp;
+  constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
+  static_assert(kBins % THREADS == 0 && THREADS >= kList, "shape");
   extern __shared__ uint32_t s_keys[];
-  __shared__ int s_hist[256];
-  __shared__ int s_suffix[257];
-  __shared__ int s_bin, s_need;
-  __shared__ int2 s_warp[kTopkWarps];
+  __shared__ int s_hist[kBins];
+  __shared__ uint32_t s_list[kList];
+  __shared__ uint32_t s_wmin[WARPS], s_wmax[WARPS];
+  __shared__ int s_wsum[WARPS];
+  __shared__ int2 s_wcnt[WARPS];
+  __shared__ int s_bin, s_above, s_cnt, s_nlist, s_need_eq;
+  __shared__ uint32_t s_thr;
 
   const int kvh = blockIdx.x, i = blockIdx.y;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
   const int k = min(budget[i], max_budget);
   const int row0 = page_indptr[i];
+  pdl_wait();                                   // the scores (and, in a step, nothing else) come from the predecessor
   const int64_t out0 = ((int64_t)i * num_kv_heads + kvh) * max_budget;
   const int n_sel = min(k, n_pages);
   if (tid == 0) sel_count[i * num_kv_heads + kvh] = n_sel;
 
   if (k >= n_pages) {                           // G6: budget covers the request -> every page
-    for (int r = tid; r < max_budget; r += kTopkThreads) {
+    for (int r = tid; r < max_budget; r += THREADS) {
       const bool ok = r < n_pages;
       sel_phys[out0 + r] = ok ? page_indices[row0 + r] : -1;
       if (sel_logical) sel_logical[out0 + r] = ok ? r : -1;
@@ -77,109 +74,178 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
 
   const float* sc = scores + (int64_t)kvh * total_pages + row0;
   const bool cached = n_pages <= smem_keys;
-  if (cached) {
-    for (int j = tid; j < n_pages; j += kTopkThreads) s_keys[j] = page_key(sc, j, n_pages, n_sink, n_local);
+  // ---- keys, and the min / max key of the non-forced pages ------------------------------------
+  uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+  for (int j = tid; j < n_pages; j += THREADS) {
+    const uint32_t key = page_key(sc, j, n_pages, n_sink, n_local);
+    if (cached) s_keys[j] = key;
+    if (key != kForcedKey) { kmin = min(kmin, key); kmax = max(kmax, key); }
   }
+  kmin = __reduce_min_sync(0xffffffffu, kmin);
+  kmax = __reduce_max_sync(0xffffffffu, kmax);
+  if (lane == 0) { s_wmin[warp] = kmin; s_wmax[warp] = kmax; }
   __syncthreads();
+#pragma unroll
+  for (int w = 0; w < WARPS; ++w) { kmin = min(kmin, s_wmin[w]); kmax = max(kmax, s_wmax[w]); }
   auto key_at = [&](int j) -> uint32_t {
     return cached ? s_keys[j] : page_key(sc, j, n_pages, n_sink, n_local);
   };
 
-  // ---- radix select: find thr = k-th largest key; `need` = how many keys == thr are taken ----
-  uint32_t prefix = 0, mask = 0;
-  int need = k;
-#pragma unroll 1
-  for (int shift = 24; shift >= 0; shift -= 8) {
-    if (tid < 256) s_hist[tid] = 0;
-    __syncthreads();
-    for (int j0 = 0; j0 < n_pages; j0 += kTopkThreads) {
-      const int j = j0 + tid;
-      const bool act = j < n_pages;
-      const uint32_t key = act ? key_at(j) : 0u;
-      const bool in = act && ((key & mask) == prefix);
-      const unsigned bin = (key >> shift) & 255u;
-      // warp-aggregated histogram: one atomic per distinct bin per warp (scores are often clustered
-      // in a few exponent bins, "highly sensitive to the score distribution")
-      const unsigned active = __ballot_sync(0xffffffffu, in);
-      if (in) {
-        const unsigned peers = __match_any_sync(active, bin);
-        if ((tid % kWarp) == __ffs(peers) - 1) atomicAdd(&s_hist[bin], __popc(peers));
-      }
-    }
-    __syncthreads();
-    // suffix counts: s_suffix[b] = #keys in bins >= b
-    if (tid < 256) s_suffix[tid] = s_hist[tid];
-    if (tid == 0) s_suffix[256] = 0;
-    __syncthreads();
-    for (int o = 1; o < 256; o <<= 1) {
-      int add = 0;
-      if (tid < 256 && tid + o < 256) add = s_suffix[tid + o];
-      __syncthreads();
-      if (tid < 256) s_suffix[tid] += add;
-      __syncthreads();
-    }
-    if (tid < 256 && s_suffix[tid] >= need && s_suffix[tid + 1] < need) {
-      s_bin = tid;
-      s_need = need - s_suffix[tid + 1];
-    }
-    __syncthreads();
-    prefix |= (uint32_t)s_bin << shift;
-    mask |= 255u << shift;
-    need = s_need;
-    __syncthreads();
-  }
-  const uint32_t thr = prefix;                  // k-th largest key; take all > thr and the first `need` == thr
+  const int sink = min(n_sink, n_pages), local = min(n_local, n_pages);
+  const int n_forced = min(n_pages, sink + local);
+  int need = k - n_forced;                      // non-forced pages still to take (precondition: >= 0)
+  uint32_t thr = kForcedKey;                    // take keys > thr, and the first need_eq keys == thr
+  int need_eq = 0;
 
-  // ---- ordered emission ------------------------------------------------------------------
-  const int per = (n_pages + kTopkThreads - 1) / kTopkThreads;
-  const int j_begin = min(tid * per, n_pages), j_end = min(j_begin + per, n_pages);
-  int2 cnt = make_int2(0, 0);                   // x: keys > thr, y: keys == thr in my chunk
-  for (int j = j_begin; j < j_end; ++j) {
-    const uint32_t key = key_at(j);
-    cnt.x += key > thr;
-    cnt.y += key == thr;
+  if (need > 0) {
+    // ---- radix select over the live key range [lo, lo + width) ----------------------------------
+    uint32_t lo = kmin;
+    uint64_t width = (uint64_t)(kmax - kmin) + 1;
+    int shift = max(0, (32 - __clz(kmax - kmin)) - kBinBits);     // ((kmax - kmin) >> shift) < kBins
+#pragma unroll 1
+    while (true) {
+      for (int b = tid; b < kBins; b += THREADS) s_hist[b] = 0;
+      __syncthreads();
+      for (int j = tid; j < n_pages; j += THREADS) {
+        const uint32_t key = key_at(j);
+        if (key != kForcedKey && key >= lo && (uint64_t)(key - lo) < width) atomicAdd(&s_hist[(key - lo) >> shift], 1);
+      }
+      __syncthreads();
+      // threshold bin: the highest b with  #keys in bins > b  <  need  <=  #keys in bins >= b
+      int h[BPT], mine = 0;
+#pragma unroll
+      for (int e = 0; e < BPT; ++e) { h[e] = s_hist[tid * BPT + e]; mine += h[e]; }
+      int inc = mine;                           // inclusive suffix sum over threads (tid' >= tid)
+#pragma unroll
+      for (int o = 1; o < kWarp; o <<= 1) {
+        const int a = __shfl_down_sync(0xffffffffu, inc, o);
+        if (lane + o < kWarp) inc += a;
+      }
+      if (lane == 0) s_wsum[warp] = inc;
+      __syncthreads();
+      int run = inc - mine;                     // keys in bins owned by higher threads
+#pragma unroll
+      for (int w = 0; w < WARPS; ++w) run += (w > warp) ? s_wsum[w] : 0;
+#pragma unroll
+      for (int e = BPT - 1; e >= 0; --e) {
+        if (run < need && run + h[e] >= need) { s_bin = tid * BPT + e; s_above = run; s_cnt = h[e]; }
+        run += h[e];
+      }
+      if (tid == 0) s_nlist = 0;
+      __syncthreads();
+      const int bin = s_bin, cnt = s_cnt;
+      need -= s_above;                          // still to take from the threshold bin
+      const uint32_t bin_lo = lo + ((uint32_t)bin << shift);
+      if (shift == 0) {                         // the bin is one key value: take the first `need` by index
+        thr = bin_lo;
+        need_eq = need;
+        break;
+      }
+      if (cnt <= kList) {                       // rank the few members of the bin directly
+        const uint64_t bin_w = (uint64_t)1 << shift;
+        for (int j = tid; j < n_pages; j += THREADS) {
+          const uint32_t key = key_at(j);
+          if (key != kForcedKey && key >= bin_lo && (uint64_t)(key - bin_lo) < bin_w && (uint64_t)(key - lo) < width)
+            s_list[atomicAdd(&s_nlist, 1)] = key;
+        }
+        __syncthreads();
+        if (tid < cnt) {
+          const uint32_t mykey = s_list[tid];
+          int gt = 0, ge = 0;
+          for (int j = 0; j < cnt; ++j) {
+            const uint32_t o = s_list[j];
+            gt += o > mykey;
+            ge += o >= mykey;
+          }
+          if (gt < need && need <= ge) { s_thr = mykey; s_need_eq = need - gt; }   // same values from every tie
+        }
+        __syncthreads();
+        thr = s_thr;
+        need_eq = s_need_eq;
+        break;
+      }
+      lo = bin_lo;                              // heavy ties: recurse into the bin, 11 more bits
+      width = (uint64_t)1 << shift;
+      shift = max(0, shift - kBinBits);
+    }
   }
-  int2 total;
-  const int2 before = block_exclusive_scan2(cnt, s_warp, &total);
-  int gt = before.x, eq = before.y;
-  for (int j = j_begin; j < j_end; ++j) {
-    const uint32_t key = key_at(j);
-    const bool take = key > thr || (key == thr && eq < need);
-    if (take) {
-      const int pos = gt + min(eq, need);
+
+  pdl_trigger();
+  // ---- ordered emission: warp w owns a contiguous run of pages, 32 at a time ------------------
+  // class of a page: sure (forced or key > thr) / tie (key == thr, the first need_eq by index are taken)
+  const int per_warp = ((n_pages + WARPS - 1) / WARPS + kWarp - 1) / kWarp * kWarp;
+  const int j_begin = min(warp * per_warp, n_pages), j_end = min(j_begin + per_warp, n_pages);
+  int n_sure = 0, n_tie = 0;                    // warp-uniform
+  for (int base = j_begin; base < j_end; base += kWarp) {
+    const int j = base + lane;
+    const uint32_t key = j < j_end ? key_at(j) : 0u;
+    const bool sure = j < j_end && (key == kForcedKey || key > thr);
+    const bool tie = j < j_end && key != kForcedKey && key == thr;
+    n_sure += __popc(__ballot_sync(0xffffffffu, sure));
+    n_tie += __popc(__ballot_sync(0xffffffffu, tie));
+  }
+  if (lane == 0) s_wcnt[warp] = make_int2(n_sure, n_tie);
+  __syncthreads();
+  int gt = 0, eq = 0;                           // sure / tie pages before this warp's run
+#pragma unroll
+  for (int w = 0; w < WARPS; ++w) {
+    const int2 c = s_wcnt[w];
+    gt += (w < warp) ? c.x : 0;
+    eq += (w < warp) ? c.y : 0;
+  }
+  const unsigned lt_mask = (1u << lane) - 1u;
+  for (int base = j_begin; base < j_end; base += kWarp) {
+    const int j = base + lane;
+    const uint32_t key = j < j_end ? key_at(j) : 0u;
+    const bool sure = j < j_end && (key == kForcedKey || key > thr);
+    const bool tie = j < j_end && key != kForcedKey && key == thr;
+    const unsigned b_sure = __ballot_sync(0xffffffffu, sure), b_tie = __ballot_sync(0xffffffffu, tie);
+    const int my_gt = gt + __popc(b_sure & lt_mask), my_eq = eq + __popc(b_tie & lt_mask);
+    const bool take = sure || (tie && my_eq < need_eq);
+    const int pos = my_gt + min(my_eq, need_eq);
+    if (take && pos < n_sel) {
       sel_phys[out0 + pos] = page_indices[row0 + j];
       if (sel_logical) sel_logical[out0 + pos] = j;
     }
-    gt += key > thr;
-    eq += key == thr;
+    gt += __popc(b_sure);
+    eq += __popc(b_tie);
   }
-  for (int r = n_sel + tid; r < max_budget; r += kTopkThreads) {
+  for (int r = n_sel + tid; r < max_budget; r += THREADS) {
     sel_phys[out0 + r] = -1;
     if (sel_logical) sel_logical[out0 + r] = -1;
   }
 }
 
-cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
-                              const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
-                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s) {
-  if (pt.batch == 0) return cudaSuccess;
+template <int THREADS>
+static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
+                                 int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
+                                 cudaStream_t s, bool pdl) {
   const vx_geom& g = c->g;
   const int keys = pt.max_pages_per_req <= kTopkSmemKeys ? pt.max_pages_per_req : 0;
   const size_t smem = (size_t)(keys > 0 ? keys : 1) * sizeof(uint32_t);
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(topk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    cudaError_t e = cudaFuncSetAttribute(topk_kernel<THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          kTopkSmemKeys * (int)sizeof(uint32_t));
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
   dim3 grid(g.num_kv_heads, pt.batch);
-  topk_kernel<<<grid, kTopkThreads, smem, s>>>(scores, g.num_kv_heads, pt.total_pages, pt.page_indptr,
-                                               pt.page_indices, pt.seq_lens, g.page_size, budget,
-                                               g.n_sink, g.n_local, max_budget, keys, sel_phys,
-                                               sel_logical, sel_count);
+  cudaError_t e = launch_kernel(topk_kernel<THREADS>, grid, dim3(THREADS), smem, s, pdl, scores, g.num_kv_heads,
+                                pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
+                                g.n_sink, g.n_local, max_budget, keys, sel_phys, sel_logical, sel_count);
   c->launches += 1;
-  return cudaGetLastError();
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
+                              const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
+                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl) {
+  if (pt.batch == 0) return cudaSuccess;
+  // block size by problem size: ~4-8 candidates per thread
+  if (pt.max_pages_per_req <= 1024) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
+  if (pt.max_pages_per_req <= 4096) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
+  return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
 }
 
 }  // namespace vx
