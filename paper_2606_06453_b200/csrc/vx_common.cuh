@@ -104,24 +104,46 @@ __device__ __forceinline__ bool last_split_arrives(int* counter, int num_splits,
   return last;
 }
 
-// merge rows [row0, row0 + n_rows) of part_o [rows, n_part, v_dim] / part_lse [rows, n_part] into out / lse
+// merge rows [row0, row0 + n_rows) of part_o [rows, n_part, v_dim] / part_lse [rows, n_part] into out / lse.
+// s_w: n_rows * n_part floats of shared-memory scratch.  The split weights are computed once per row; the
+// value loads are independent 16-byte L2 reads (the partials were just written by other SMs: ld.global.cg).
+__device__ __forceinline__ float4 ldcg_f32x4(const float* p) {
+  float4 v;
+  asm volatile("ld.global.cg.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ void store4(float* dst, float4 v) { *reinterpret_cast<float4*>(dst) = v; }
+__device__ __forceinline__ void store4(__nv_bfloat16* dst, float4 v) {
+  __nv_bfloat162 a = __floats2bfloat162_rn(v.x, v.y), b = __floats2bfloat162_rn(v.z, v.w);
+  uint2 u = make_uint2(*reinterpret_cast<uint32_t*>(&a), *reinterpret_cast<uint32_t*>(&b));
+  *reinterpret_cast<uint2*>(dst) = u;
+}
 template <typename T>
 __device__ __forceinline__ void merge_partials(const float* part_o, const float* part_lse, int64_t row0, int n_rows,
-                                               int n_part, int v_dim, T* out, float* lse) {
-  for (int e = threadIdx.x; e < n_rows * v_dim; e += blockDim.x) {
-    const int64_t row = row0 + e / v_dim;
-    const int c = e % v_dim;
-    const float* ls = part_lse + row * n_part;
+                                               int n_part, int v_dim, T* out, float* lse, float* s_w) {
+  for (int r = threadIdx.x; r < n_rows; r += blockDim.x) {
+    const float* ls = part_lse + (row0 + r) * n_part;
     float mx = -INFINITY;
     for (int s = 0; s < n_part; ++s) mx = fmaxf(mx, ldcg_f32(ls + s));
-    float z = 0.f, o = 0.f;
+    float z = 0.f;
+    for (int s = 0; s < n_part; ++s) z += mx == -INFINITY ? 0.f : __expf(ldcg_f32(ls + s) - mx);
+    const float inv = z > 0.f ? 1.f / z : 0.f;
+    for (int s = 0; s < n_part; ++s) s_w[r * n_part + s] = mx == -INFINITY ? 0.f : __expf(ldcg_f32(ls + s) - mx) * inv;
+    if (lse != nullptr) lse[row0 + r] = z > 0.f ? mx + logf(z) : -INFINITY;
+  }
+  __syncthreads();
+  const int vec = v_dim / 4;
+#pragma unroll 4
+  for (int e = threadIdx.x; e < n_rows * vec; e += blockDim.x) {
+    const int r = e / vec, c = (e % vec) * 4;
+    const float* src = part_o + (row0 + r) * n_part * v_dim + c;
+    float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int s = 0; s < n_part; ++s) {
-      const float w = mx == -INFINITY ? 0.f : __expf(ldcg_f32(ls + s) - mx);
-      z += w;
-      if (w != 0.f) o = fmaf(w, ldcg_f32(part_o + (row * n_part + s) * v_dim + c), o);
+      const float w = s_w[r * n_part + s];
+      const float4 v = ldcg_f32x4(src + (int64_t)s * v_dim);
+      o.x = fmaf(w, v.x, o.x); o.y = fmaf(w, v.y, o.y); o.z = fmaf(w, v.z, o.z); o.w = fmaf(w, v.w, o.w);
     }
-    out[row * v_dim + c] = Elem<T>::from_float(z > 0.f ? o / z : 0.f);
-    if (c == 0 && lse != nullptr) lse[row] = z > 0.f ? mx + logf(z) : -INFINITY;
+    store4(out + (row0 + r) * v_dim + c, o);
   }
 }
 

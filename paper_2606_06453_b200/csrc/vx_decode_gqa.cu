@@ -283,7 +283,8 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   }
   if (num_splits > 1) {                         // (a5) the last split of this (request, KV head) merges by LSE
     if (last_split_arrives(unit_counter + i * num_kv_heads + kvh, num_splits, &s_last))
-      merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads + kvh * grp, grp, num_splits, D, out, lse_out);
+      merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads + kvh * grp, grp, num_splits, D, out, lse_out,
+                                     reinterpret_cast<float*>(smem));
   }
 }
 
@@ -325,7 +326,7 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
-bool decode_folds_summary(const vx_ctx* c) { return !c->force_generic && gqa_mma_supported(c->g); }
+bool decode_folds_summary(const vx_ctx* c) { return !c->force_generic && (gqa_mma_supported(c->g) || mla_tc_supported(c->g)); }
 
 cudaError_t launch_decode_gqa_mma(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,

@@ -1,18 +1,30 @@
-// vx_decode_mla.cu -- (a4) sparse paged decode for the MLA absorbed-latent geometry on tcgen05.
+// vx_decode_mla.cu -- (a4)+(a5)(+a1) sparse paged decode for the MLA absorbed-latent geometry on tcgen05.
 // PAPER.md:92 Eq.4 over the selected pages (:200); :202 / :262 cuda_mla role (one latent KV head of
 // width 576 = 512 latent + 64 RoPE shared by all query heads, V = first 512 latent channels, G8).
 //
 // Per 64-token page the work is two dense contractions, ~60 flop per HBM byte:
 //     S^T[64 tokens x 32 heads]  = K[64 x 576] . Q^T          36 x tcgen05.mma  M=64  N=32 K=16
 //     O^T[512 x 32 heads]       += V^T[512 x 64] . P^T   4 x 4 x tcgen05.mma  M=128 N=32 K=16
-// with tokens / channels on the MMA M axis and the 32 heads on N, so no tile is padded.  The page
-// (73,728 B, read once for K and V) is staged by 16-byte cp.async into the 128-byte-swizzled
-// shared-memory layout both MMAs consume: K-major for K in S^T, MN-major (transposed) for V^T.
-// S^T and O^T live in TMEM; the softmax threads (one per token row) read S^T with tcgen05.ld,
-// reduce the per-head maxima across lanes, write P (bf16) back to shared memory as the B operand.
-// O^T is rescaled in TMEM only when a head's running maximum grows by more than 2^8 (lazy
-// rescaling); the denominators are per-thread partial sums reduced once at the end.
-// Two page stages: page p+1 is in flight while page p is computed.
+// with tokens / channels on the MMA M axis and the 32 heads on N, so no tile is padded.
+//
+// Warp-specialised, one CTA per SM:
+//   warp 0      TMA producer.  The latent page (73,728 B, read once for K and V) arrives as nine
+//               [64 tokens x 64 channels] boxes (cp.async.bulk.tensor, 128-byte swizzle) -- exactly the
+//               shared-memory layout both MMAs consume (K-major for K in S^T, MN-major for V^T).  The
+//               ring is managed per BOX PAIR (16 KB = 128 value channels): 10 pair slots + 2 RoPE slots
+//               = 2.5 pages, each slot released by the tcgen05.commit of the last MMA that reads it, so
+//               ~1.5 pages (110 KB) per SM are always in flight.
+//   warp 1      MMA issuer (one lane).  QK(p+1) is issued BEFORE PV(p): the tensor pipe works on the
+//               next page's scores while the softmax warps turn S(p) into P(p).  S^T is double-buffered
+//               in TMEM, O^T (512 x 32 fp32) lives in TMEM for the whole CTA.
+//   warps 2..5  softmax: tcgen05.ld S^T (one token row per thread), head maxima by a transposed shuffle
+//               butterfly + one named barrier, lazy O^T rescale (only when a running max grows by more
+//               than 2^8), P (bf16) to shared memory as the B operand of PV, double-buffered.
+// Splits of a request merge in-kernel (the last split to arrive merges by LSE).  In the
+// fused step the CTA holding the request's newest page also rebuilds that page's min / max summary from
+// the staged tile (a1; the newest page is a forced local page).
+#include <cuda.h>
+
 #include "vx_common.cuh"
 #include "vx_internal.h"
 
@@ -20,16 +32,24 @@ namespace vx {
 
 namespace mla {
 constexpr int D = 576, DV = 512, PAGE = 64, NH = 32;      // geometry this kernel is built for
-constexpr int THREADS = 128;
+constexpr int THREADS = 192;                              // producer warp, MMA warp, 4 softmax warps
+constexpr int SOFTMAX_THREADS = 128;
 constexpr int CHUNKS = D * 2 / 16;                        // 72 16-byte chunks per token row
 constexpr int ATOMS = CHUNKS / 8;                         // 9 swizzle atoms (64 channels each)
 constexpr int K_ATOM_BYTES = PAGE * 128;                  // 8192: 64 rows x 128 B
+constexpr int PAIR_BYTES = 2 * K_ATOM_BYTES;              // 16384: 128 value channels
 constexpr int Q_ATOM_BYTES = NH * 128;                    // 4096
-constexpr int STAGE_BYTES = ATOMS * K_ATOM_BYTES;         // 73728
 constexpr int Q_BYTES = ATOMS * Q_ATOM_BYTES;             // 36864
 constexpr int P_BYTES = NH * 128;                         // 4096: [32 heads][64 tokens] bf16
-constexpr int SMEM_BYTES = 2 * STAGE_BYTES + Q_BYTES + P_BYTES + 1024;   // + alignment slack
-constexpr int TMEM_COLS = 256;                            // S^T: cols [0,32); O^T block mb: cols [32+32mb, ..)
+constexpr int N_PAIR = 10, N_ROPE = 2;                    // ring slots
+constexpr int PAIRS_PER_PAGE = DV / 128;                  // 4
+constexpr int OFF_PAIR = 0;
+constexpr int OFF_ROPE = OFF_PAIR + N_PAIR * PAIR_BYTES;  // 163840
+constexpr int OFF_Q = OFF_ROPE + N_ROPE * K_ATOM_BYTES;   // 180224
+constexpr int OFF_P = OFF_Q + Q_BYTES;                    // 217088
+constexpr int SMEM_BYTES = OFF_P + 2 * P_BYTES + 1024;    // 226304 incl. alignment slack
+constexpr int TMEM_COLS = 256;                            // S^T buffers: cols [0,32), [32,64); O^T block mb: [64+32mb, ..)
+constexpr int TM_O = 64;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.f;                  // log2 units
@@ -156,32 +176,90 @@ __device__ __forceinline__ float lanes_sum_transposed(const float (&v)[32], int 
   const bool up = lane & 1;
   return (up ? d[1] : d[0]) + __shfl_xor_sync(0xffffffffu, up ? d[0] : d[1], 1);
 }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// one [64 channels x 64 tokens] box of page `page` -> 8 KB of 128-byte-swizzled shared memory
+__device__ __forceinline__ void tma_box(uint32_t dst, const CUtensorMap* map, int channel0, int page, uint32_t bar) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+      ::"r"(dst), "l"(map), "r"(channel0), "r"(0), "r"(page), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void softmax_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(SOFTMAX_THREADS) : "memory"); }
+
+// barrier indices
+constexpr int B_PAIR_FULL = 0, B_PAIR_EMPTY = N_PAIR, B_ROPE_FULL = 2 * N_PAIR, B_ROPE_EMPTY = B_ROPE_FULL + N_ROPE,
+              B_S_FULL = B_ROPE_EMPTY + N_ROPE, B_S_EMPTY = B_S_FULL + 2, B_P_FULL = B_S_EMPTY + 2,
+              B_PV_DONE = B_P_FULL + 2, N_BARS = B_PV_DONE + 2;
 }  // namespace mla
 
 __global__ void __launch_bounds__(mla::THREADS, 1)
-decode_mla_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ kpool, int64_t stride_page,
-                  int64_t stride_token, int num_q_heads, float scale_log2, const int32_t* __restrict__ seq_lens,
-                  const int32_t* __restrict__ sel_phys, const int32_t* __restrict__ sel_logical,
-                  const int32_t* __restrict__ sel_count, int max_budget, int num_splits,
-                  float* __restrict__ part_o, float* __restrict__ part_lse, __nv_bfloat16* __restrict__ out,
-                  float* __restrict__ lse_out) {
+decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16* __restrict__ q, int num_q_heads,
+                  float scale_log2, const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ sel_phys,
+                  const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count, int max_budget,
+                  int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
+                  int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd,
+                  __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out) {
   using namespace mla;
   extern __shared__ uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t s_bar[2];           // [0]: S^T ready, [1]: O^T accumulated
+  __shared__ __align__(8) uint64_t s_bar[N_BARS];
   __shared__ uint32_t s_tmem;
-  __shared__ float s_wred[4][NH], s_mref[NH], s_fac[NH];
-  __shared__ int s_flag;
+  __shared__ float s_wred[2][4][NH], s_lred[4][NH];
+  __shared__ int s_last;
 
   const int split = blockIdx.x, i = blockIdx.z;
   const int tid = threadIdx.x, warp = tid / kWarp, lane = tid % kWarp;
+  const uint32_t raw = smem_u32(smem_raw);
+  const uint32_t base = (raw + 1023u) & ~1023u;        // swizzle atoms need 1024-byte alignment
+  uint8_t* sm = smem_raw + (base - raw);
+  const uint32_t bar0 = smem_u32(&s_bar[0]);
+  auto bar = [&](int idx) -> uint32_t { return bar0 + 8u * (uint32_t)idx; };
   const int n_tok = seq_lens[i];
+  const int newest_page = (n_tok - 1) / PAGE;
+
+  // ---- prologue (overlaps the preceding kernel under PDL): barriers, TMEM, Q tile ---------------------
+  if (warp == 1) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(TMEM_COLS));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  if (tid == 0) {
+    for (int s = 0; s < N_PAIR; ++s) { mbar_init(bar(B_PAIR_FULL + s), 1); mbar_init(bar(B_PAIR_EMPTY + s), 1); }
+    for (int s = 0; s < N_ROPE; ++s) { mbar_init(bar(B_ROPE_FULL + s), 1); mbar_init(bar(B_ROPE_EMPTY + s), 1); }
+    for (int b = 0; b < 2; ++b) {
+      mbar_init(bar(B_S_FULL + b), 1);
+      mbar_init(bar(B_S_EMPTY + b), 4);
+      mbar_init(bar(B_P_FULL + b), 4);
+      mbar_init(bar(B_PV_DONE + b), 1);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("prefetch.tensormap [%0];" ::"l"(&kmap) : "memory");
+  }
+  if (warp >= 2) {                                     // Q[32 x 576] -> K-major swizzled B operand (zero rows past Hq)
+    for (int x = tid - 64; x < NH * CHUNKS; x += SOFTMAX_THREADS) {
+      const int h = x / CHUNKS, c = x % CHUNKS;
+      uint4 v = make_uint4(0, 0, 0, 0);
+      if (h < num_q_heads) v = *reinterpret_cast<const uint4*>(q + ((int64_t)i * num_q_heads + h) * D + c * 8);
+      const uint32_t off = (c >> 3) * Q_ATOM_BYTES + (h >> 3) * 1024 + (h & 7) * 128 + (((c & 7) ^ (h & 7)) << 4);
+      *reinterpret_cast<uint4*>(sm + OFF_Q + off) = v;
+    }
+    fence_async_proxy();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = s_tmem;
+  pdl_wait();                                          // the selection lists come from the preceding kernel of the step
+
   const int cnt = sel_count[i];
   const int per_split = (cnt + num_splits - 1) / num_splits;
   const int r_begin = min(split * per_split, cnt), r_end = min(r_begin + per_split, cnt);
   const int n_pages = r_end - r_begin;
   const int32_t* phys_list = sel_phys + (int64_t)i * max_budget + r_begin;
   const int32_t* log_list = sel_logical + (int64_t)i * max_budget + r_begin;
-  const int dim_of_thread = warp * 32 + lane;          // O^T row (within a 128-channel block) this thread reads
+  const uint32_t q_base = base + OFF_Q, p_base = base + OFF_P;
 
   if (n_pages == 0) {                                  // empty split: contributes nothing to the merge
     for (int e = tid; e < num_q_heads * DV; e += THREADS) {
@@ -195,178 +273,253 @@ decode_mla_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __re
       if (num_splits == 1) { if (lse_out) lse_out[row] = -INFINITY; }
       else part_lse[row * num_splits + split] = -INFINITY;
     }
-    return;
-  }
-
-  const uint32_t raw = smem_u32(smem_raw);
-  const uint32_t base = (raw + 1023u) & ~1023u;        // swizzle atoms need 1024-byte alignment
-  uint8_t* sm = smem_raw + (base - raw);
-  const uint32_t q_base = base + 2 * STAGE_BYTES, p_base = q_base + Q_BYTES;
-  const uint32_t bar_s = smem_u32(&s_bar[0]), bar_o = smem_u32(&s_bar[1]);
-
-  auto issue_page = [&](int p) {                       // all threads: page p -> stage p & 1 (zero-fill invalid rows)
-    const int64_t phys = phys_list[p];
-    const int valid = min(PAGE, n_tok - log_list[p] * PAGE);
-    const __nv_bfloat16* src = kpool + phys * stride_page;
-    const uint32_t dst = base + (uint32_t)(p & 1) * STAGE_BYTES;
-#pragma unroll 4
-    for (int x = tid; x < PAGE * CHUNKS; x += THREADS) {
-      const int r = x / CHUNKS, c = x % CHUNKS;
-      const uint32_t off = (c >> 3) * K_ATOM_BYTES + (r >> 3) * 1024 + (r & 7) * 128 + (((c & 7) ^ (r & 7)) << 4);
-      const int n = r < valid ? 16 : 0;
-      asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst + off),
-                   "l"(src + (int64_t)r * stride_token + c * 8), "r"(n));
-    }
-  };
-
-  // ---- prologue: TMEM, barriers, Q tile, first page ------------------------------------------
-  if (warp == 0) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&s_tmem)), "n"(TMEM_COLS));
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
-  }
-  if (tid == 0) {
-    mbar_init(bar_s, 1);
-    mbar_init(bar_o, 1);
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  issue_page(0);
-  cp_async_commit();
-  for (int x = tid; x < NH * CHUNKS; x += THREADS) {   // Q[32 x 576] -> K-major swizzled B operand (zero rows past Hq)
-    const int h = x / CHUNKS, c = x % CHUNKS;
-    uint4 v = make_uint4(0, 0, 0, 0);
-    if (h < num_q_heads) v = *reinterpret_cast<const uint4*>(q + ((int64_t)i * num_q_heads + h) * D + c * 8);
-    const uint32_t off = (c >> 3) * Q_ATOM_BYTES + (h >> 3) * 1024 + (h & 7) * 128 + (((c & 7) ^ (h & 7)) << 4);
-    *reinterpret_cast<uint4*>(sm + 2 * STAGE_BYTES + off) = v;
-  }
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = s_tmem;
-  const uint32_t t_lane = tmem + ((uint32_t)(warp * 32) << 16);
-
-  float l_thr[NH];
+  } else if (warp == 0) {
+    // ===== TMA producer ===================================================================================
+    int my_phys = 0;
+    for (int p = 0; p < n_pages; ++p) {
+      if ((p & 31) == 0) my_phys = p + lane < n_pages ? phys_list[p + lane] : 0;
+      const int phys = __shfl_sync(0xffffffffu, my_phys, p & 31);
+      if (lane == 0) {
+        const int rs = p % N_ROPE, ru = p / N_ROPE;
+        if (ru >= 1) mbar_wait(bar(B_ROPE_EMPTY + rs), (ru - 1) & 1);
+        mbar_expect_tx(bar(B_ROPE_FULL + rs), K_ATOM_BYTES);
+        tma_box(base + OFF_ROPE + rs * K_ATOM_BYTES, &kmap, DV, phys, bar(B_ROPE_FULL + rs));
 #pragma unroll
-  for (int j = 0; j < NH; ++j) l_thr[j] = 0.f;
-
-  for (int p = 0; p < n_pages; ++p) {
-    const uint32_t stage = base + (uint32_t)(p & 1) * STAGE_BYTES;
-    if (p > 0) mbar_wait(bar_o, (p - 1) & 1);          // PV of page p-1 done: P and the other stage are free
-    if (p + 1 < n_pages) issue_page(p + 1);
-    cp_async_commit();
-    cp_async_wait<1>();                                // page p has landed (this thread's copies)
-    fence_async_proxy();                               // make cp.async / st.shared data visible to the MMA proxy
-    __syncthreads();
-    if (tid == 0) {
-      tc_fence_after();
-#pragma unroll 4
-      for (int ks = 0; ks < D / 16; ++ks) {
-        const uint32_t a = stage + (ks >> 2) * K_ATOM_BYTES + (ks & 3) * 32;
-        const uint32_t b = q_base + (ks >> 2) * Q_ATOM_BYTES + (ks & 3) * 32;
-        umma(tmem, smem_desc(a, 16, 1024), smem_desc(b, 16, 1024), IDESC_QK, ks > 0);
+        for (int j = 0; j < PAIRS_PER_PAGE; ++j) {
+          const int g = p * PAIRS_PER_PAGE + j, ps = g % N_PAIR, u = g / N_PAIR;
+          if (u >= 1) mbar_wait(bar(B_PAIR_EMPTY + ps), (u - 1) & 1);
+          mbar_expect_tx(bar(B_PAIR_FULL + ps), PAIR_BYTES);
+          const uint32_t dst = base + OFF_PAIR + ps * PAIR_BYTES;
+          tma_box(dst, &kmap, 128 * j, phys, bar(B_PAIR_FULL + ps));
+          tma_box(dst + K_ATOM_BYTES, &kmap, 128 * j + 64, phys, bar(B_PAIR_FULL + ps));
+        }
       }
-      umma_commit(bar_s);
+      __syncwarp();
     }
-    const int valid = min(PAGE, n_tok - log_list[p] * PAGE);
-    const int row = warp * 16 + lane;                  // M = 64: token row r sits in TMEM lane (r % 16) + 32 * (r / 16)
-    const bool live = lane < 16 && row < valid;
-    mbar_wait(bar_s, p & 1);
-    tc_fence_after();
-    float s[NH];
-    tmem_ld32(t_lane, s);
+  } else if (warp == 1) {
+    // ===== MMA issuer: QK(p) is issued before PV(p-1) ====================================================
+    for (int p = 0; p <= n_pages; ++p) {
+      if (p < n_pages) {
+        const int b = p & 1;
+        if (p >= 2) mbar_wait(bar(B_S_EMPTY + b), ((p >> 1) - 1) & 1);   // softmax has read S(p-2)
+        const int rs = p % N_ROPE;
+        mbar_wait(bar(B_ROPE_FULL + rs), (p / N_ROPE) & 1);
+        tc_fence_after();
+        if (lane == 0) {
+          const uint32_t a = base + OFF_ROPE + rs * K_ATOM_BYTES, bq = q_base + 8 * Q_ATOM_BYTES;
 #pragma unroll
-    for (int j = 0; j < NH; ++j) s[j] = live ? s[j] * scale_log2 : -INFINITY;
-    s_wred[warp][lane] = lanes_max_transposed(s, lane);
-    __syncthreads();
-    if (warp == 0) {                                   // lane = head: tile maximum, lazy running reference
-      const float tmax = fmaxf(fmaxf(s_wred[0][lane], s_wred[1][lane]), fmaxf(s_wred[2][lane], s_wred[3][lane]));
-      bool grow = false;
-      if (p == 0) {
-        s_mref[lane] = tmax;
-      } else {
-        const float old = s_mref[lane];
-        grow = tmax > old + kRescaleThreshold;
-        s_fac[lane] = grow ? exp2f(old - tmax) : 1.f;
-        if (grow) s_mref[lane] = tmax;
-      }
-      const bool any = __any_sync(0xffffffffu, grow);
-      if (lane == 0) s_flag = any;
-    }
-    __syncthreads();
-    if (p > 0 && s_flag) {                             // rare: rescale O^T in TMEM and the partial denominators
+          for (int ks = 0; ks < 4; ++ks)
+            umma(tmem + b * 32, smem_desc(a + ks * 32, 16, 1024), smem_desc(bq + ks * 32, 16, 1024), IDESC_QK, ks > 0);
+          umma_commit(bar(B_ROPE_EMPTY + rs));
+        }
 #pragma unroll 1
-      for (int mb = 0; mb < DV / 128; ++mb) {
-        float o[NH];
-        tmem_ld32(t_lane + 32 + 32 * mb, o);
+        for (int j = 0; j < PAIRS_PER_PAGE; ++j) {
+          const int g = p * PAIRS_PER_PAGE + j, ps = g % N_PAIR;
+          mbar_wait(bar(B_PAIR_FULL + ps), (g / N_PAIR) & 1);
+          tc_fence_after();
+          if (lane == 0) {
 #pragma unroll
-        for (int j = 0; j < NH; ++j) o[j] *= s_fac[j];
-        tmem_st32(t_lane + 32 + 32 * mb, o);
+            for (int ks = 0; ks < 8; ++ks) {
+              const uint32_t a = base + OFF_PAIR + ps * PAIR_BYTES + (ks >> 2) * K_ATOM_BYTES + (ks & 3) * 32;
+              const uint32_t bq = q_base + (2 * j + (ks >> 2)) * Q_ATOM_BYTES + (ks & 3) * 32;
+              umma(tmem + b * 32, smem_desc(a, 16, 1024), smem_desc(bq, 16, 1024), IDESC_QK, true);
+            }
+          }
+        }
+        if (lane == 0) umma_commit(bar(B_S_FULL + b));
+        __syncwarp();
       }
+      if (p >= 1) {
+        const int pq = p - 1, b = pq & 1;
+        mbar_wait(bar(B_P_FULL + b), (pq >> 1) & 1);     // P(pq) written, O^T rescaled if it had to be
+        tc_fence_after();
+        if (lane == 0) {
 #pragma unroll
-      for (int j = 0; j < NH; ++j) l_thr[j] *= s_fac[j];
+          for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
+            const int g = pq * PAIRS_PER_PAGE + mb, ps = g % N_PAIR;
+            const uint32_t a = base + OFF_PAIR + ps * PAIR_BYTES;
+#pragma unroll
+            for (int ks = 0; ks < PAGE / 16; ++ks)
+              umma(tmem + TM_O + 32 * mb, smem_desc(a + ks * 2048, K_ATOM_BYTES, 1024),
+                   smem_desc(p_base + b * P_BYTES + ks * 32, 16, 1024), IDESC_PV, pq > 0 || ks > 0);
+            umma_commit(bar(B_PAIR_EMPTY + ps));         // this pair slot may be refilled
+          }
+          umma_commit(bar(B_PV_DONE + b));
+        }
+        __syncwarp();
+      }
     }
-    if (lane < 16) {                                   // P[head][token] bf16, K-major swizzled B operand
-      uint8_t* pdst = sm + 2 * STAGE_BYTES + Q_BYTES + (row & 7) * 2;
-      const int tc = row >> 3;
+    pdl_trigger();
+  } else {
+    // ===== softmax warps (one S^T token row per thread; 16 live lanes per warp at M = 64) ==================
+    const int sp = warp & 3;                             // TMEM sub-partition this warp may access
+    const int stid = tid - 64;
+    const uint32_t t_lane = tmem + ((uint32_t)(sp * 32) << 16);
+    const int row = sp * 16 + lane;                      // M = 64: token row r sits in TMEM lane (r % 16) + 32 * (r / 16)
+    float m_ref[NH], l_thr[NH];
+#pragma unroll
+    for (int j = 0; j < NH; ++j) { m_ref[j] = 0.f; l_thr[j] = 0.f; }
+    int lg = log_list[0];
+    int valid = PAGE;
+    for (int p = 0; p < n_pages; ++p) {
+      const int b = p & 1;
+      valid = min(PAGE, n_tok - lg * PAGE);
+      if (p + 1 < n_pages) lg = log_list[p + 1];         // prefetch for the next page
+      const bool live = lane < 16 && row < valid;
+      mbar_wait(bar(B_S_FULL + b), (p >> 1) & 1);
+      tc_fence_after();
+      float s[NH];
+      tmem_ld32(t_lane + b * 32, s);
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_S_EMPTY + b));    // S buffer b may be overwritten by QK(p+2)
+#pragma unroll
+      for (int j = 0; j < NH; ++j) s[j] = live ? s[j] * scale_log2 : -INFINITY;
+      s_wred[b][sp][lane] = lanes_max_transposed(s, lane);
+      softmax_barrier();
+      // every thread keeps the per-head running reference (lazy: it moves only on a growth > 2^8)
+      float fac[NH];
+      bool grow_any = false;
 #pragma unroll
       for (int j = 0; j < NH; ++j) {
-        const float pj = exp2f(s[j] - s_mref[j]);
-        l_thr[j] += pj;
-        *reinterpret_cast<__nv_bfloat16*>(pdst + (j >> 3) * 1024 + (j & 7) * 128 + ((tc ^ (j & 7)) << 4)) =
-            __float2bfloat16_rn(pj);
+        const float tmax = fmaxf(fmaxf(s_wred[b][0][j], s_wred[b][1][j]), fmaxf(s_wred[b][2][j], s_wred[b][3][j]));
+        const bool grow = p > 0 && tmax > m_ref[j] + kRescaleThreshold;
+        fac[j] = grow ? exp2f(m_ref[j] - tmax) : 1.f;
+        if (p == 0 || grow) m_ref[j] = tmax;
+        grow_any |= grow;
+      }
+      if (p >= 2) mbar_wait(bar(B_PV_DONE + b), ((p >> 1) - 1) & 1);     // PV(p-2) done: P buffer b is free
+      if (grow_any) {                                    // rare: rescale O^T in TMEM and the partial denominators
+        mbar_wait(bar(B_PV_DONE + ((p - 1) & 1)), ((p - 1) >> 1) & 1);   // PV(p-1) done: O^T is stable
+        tc_fence_after();
+#pragma unroll 1
+        for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
+          float o[NH];
+          tmem_ld32(t_lane + TM_O + 32 * mb, o);
+#pragma unroll
+          for (int j = 0; j < NH; ++j) o[j] *= fac[j];
+          tmem_st32(t_lane + TM_O + 32 * mb, o);
+        }
+#pragma unroll
+        for (int j = 0; j < NH; ++j) l_thr[j] *= fac[j];
+        tc_fence_before();
+      }
+      if (valid < PAGE) {                                // partial page: zero the stale value rows (0 x garbage must be 0)
+        const int n_rows = PAGE - valid;
+        for (int x = stid; x < n_rows * 64; x += SOFTMAX_THREADS) {
+          const int r = valid + x / 64, a = (x % 64) >> 3, c = x & 7;
+          const int g = p * PAIRS_PER_PAGE + (a >> 1), ps = g % N_PAIR;
+          *reinterpret_cast<uint4*>(sm + OFF_PAIR + ps * PAIR_BYTES + (a & 1) * K_ATOM_BYTES + (r >> 3) * 1024 +
+                                    (r & 7) * 128 + c * 16) = make_uint4(0, 0, 0, 0);
+        }
+      }
+      if (lane < 16) {                                   // P[head][token] bf16, K-major swizzled B operand
+        uint8_t* pdst = sm + OFF_P + b * P_BYTES + (row & 7) * 2;
+        const int tc = row >> 3;
+#pragma unroll
+        for (int j = 0; j < NH; ++j) {
+          const float pj = exp2f(s[j] - m_ref[j]);
+          l_thr[j] += pj;
+          *reinterpret_cast<__nv_bfloat16*>(pdst + (j >> 3) * 1024 + (j & 7) * 128 + ((tc ^ (j & 7)) << 4)) =
+              __float2bfloat16_rn(pj);
+        }
+      }
+      fence_async_proxy();                               // P / zeroed rows visible to the MMA proxy
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(B_P_FULL + b));
+    }
+    // ---- epilogue ------------------------------------------------------------------------------------------
+    const int pl = n_pages - 1;
+    if (summary_upd != nullptr && lg == newest_page && stid < CHUNKS) {
+      // (a1) the request's newest page is this CTA's last page: rebuild its min / max summary from the staged
+      // tile (exact in bf16).  Thread owns one 16-byte channel chunk over the valid tokens.
+      const int cc = stid, a = cc >> 3;
+      const uint8_t* atom = a < 8 ? sm + OFF_PAIR + ((pl * PAIRS_PER_PAGE + (a >> 1)) % N_PAIR) * PAIR_BYTES + (a & 1) * K_ATOM_BYTES
+                                  : sm + OFF_ROPE + (pl % N_ROPE) * K_ATOM_BYTES;
+      uint4 lo4 = *reinterpret_cast<const uint4*>(atom + ((cc & 7) << 4)), hi4 = lo4;     // token 0
+      __nv_bfloat162* lo = reinterpret_cast<__nv_bfloat162*>(&lo4);
+      __nv_bfloat162* hi = reinterpret_cast<__nv_bfloat162*>(&hi4);
+      for (int r = 1; r < valid; ++r) {
+        const uint4 v4 = *reinterpret_cast<const uint4*>(atom + (r >> 3) * 1024 + (r & 7) * 128 + (((cc & 7) ^ (r & 7)) << 4));
+        const __nv_bfloat162* v = reinterpret_cast<const __nv_bfloat162*>(&v4);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) { lo[e] = __hmin2(lo[e], v[e]); hi[e] = __hmax2(hi[e], v[e]); }
+      }
+      __nv_bfloat16* dst = summary_upd + (int64_t)phys_list[pl] * 2 * D + cc * 8;
+      *reinterpret_cast<uint4*>(dst) = lo4;
+      *reinterpret_cast<uint4*>(dst + D) = hi4;
+    }
+    s_lred[sp][lane] = lanes_sum_transposed(l_thr, lane);
+    softmax_barrier();
+    mbar_wait(bar(B_PV_DONE + (pl & 1)), (pl >> 1) & 1);   // the last PV has landed in TMEM
+    tc_fence_after();
+#pragma unroll 1
+    for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
+      float o[NH];
+      tmem_ld32(t_lane + TM_O + 32 * mb, o);
+      const int d = mb * 128 + sp * 32 + lane;
+#pragma unroll
+      for (int j = 0; j < NH; ++j) {
+        if (j < num_q_heads) {
+          const float lsum = s_lred[0][j] + s_lred[1][j] + s_lred[2][j] + s_lred[3][j];
+          const float val = o[j] / lsum;
+          const int64_t orow = (int64_t)i * num_q_heads + j;
+          if (num_splits == 1) out[orow * DV + d] = __float2bfloat16_rn(val);
+          else part_o[(orow * num_splits + split) * DV + d] = val;
+        }
       }
     }
-    fence_async_proxy();
-    tc_fence_before();
-    __syncthreads();
-    if (tid == 0) {
-      tc_fence_after();
-#pragma unroll
-      for (int ks = 0; ks < PAGE / 16; ++ks)
-#pragma unroll
-        for (int mb = 0; mb < DV / 128; ++mb)
-          umma(tmem + 32 + 32 * mb, smem_desc(stage + 2 * mb * K_ATOM_BYTES + ks * 2048, K_ATOM_BYTES, 1024),
-               smem_desc(p_base + ks * 32, 16, 1024), IDESC_PV, p > 0 || ks > 0);
-      umma_commit(bar_o);
-    }
-  }
-  cp_async_wait<0>();
-  mbar_wait(bar_o, (n_pages - 1) & 1);
-  tc_fence_after();
-
-  // ---- epilogue: denominators, normalise, write the partial (or final) result -------------------
-  s_wred[warp][lane] = lanes_sum_transposed(l_thr, lane);
-  __syncthreads();
-  if (warp == 0) s_fac[lane] = s_wred[0][lane] + s_wred[1][lane] + s_wred[2][lane] + s_wred[3][lane];
-  __syncthreads();
-#pragma unroll 1
-  for (int mb = 0; mb < DV / 128; ++mb) {
-    float o[NH];
-    tmem_ld32(t_lane + 32 + 32 * mb, o);
-    const int d = mb * 128 + dim_of_thread;
 #pragma unroll
     for (int j = 0; j < NH; ++j) {
-      if (j < num_q_heads) {
-        const float val = o[j] / s_fac[j];
-        const int64_t row = (int64_t)i * num_q_heads + j;
-        if (num_splits == 1) out[row * DV + d] = __float2bfloat16_rn(val);
-        else part_o[(row * num_splits + split) * DV + d] = val;
+      if (stid == j && j < num_q_heads) {
+        const float lsum = s_lred[0][j] + s_lred[1][j] + s_lred[2][j] + s_lred[3][j];
+        const float lse = (m_ref[j] + log2f(lsum)) * kLn2;
+        const int64_t orow = (int64_t)i * num_q_heads + j;
+        if (num_splits == 1) { if (lse_out) lse_out[orow] = lse; }
+        else part_lse[orow * num_splits + split] = lse;
       }
     }
   }
-  if (tid < num_q_heads) {
-    const float lse = (s_mref[tid] + log2f(s_fac[tid])) * kLn2;
-    const int64_t row = (int64_t)i * num_q_heads + tid;
-    if (num_splits == 1) { if (lse_out) lse_out[row] = lse; }
-    else part_lse[row * num_splits + split] = lse;
-  }
+
+  // ---- (a5) the last split of the request to arrive merges the partials; release TMEM -------------------
   tc_fence_before();
+  if (num_splits > 1) {
+    if (last_split_arrives(unit_counter + i, num_splits, &s_last))
+      merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads, num_q_heads, num_splits, DV, out, lse_out,
+                                     reinterpret_cast<float*>(sm + OFF_Q));
+  }
   __syncthreads();
-  if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
+  if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
 }
 
 bool mla_tc_supported(const vx_geom& g) {
   return g.kv_shared && g.dtype == VX_DT_BF16 && g.num_kv_heads == 1 && g.qk_dim == mla::D && g.v_dim == mla::DV &&
          g.page_size == mla::PAGE && g.num_q_heads <= mla::NH;
+}
+
+// tensor map over the latent pool: dims (channel, token in page, page), box = 64 channels x 64 tokens, 128-byte swizzle
+static cudaError_t make_latent_map(CUtensorMap* map, const vx_kv_pool& pool) {
+  typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+  static encode_fn encode = nullptr;
+  if (!encode) {
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return e;
+    if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+    encode = reinterpret_cast<encode_fn>(fn);
+  }
+  if (pool.num_pool_pages <= 0) return cudaErrorInvalidValue;
+  const cuuint64_t dims[3] = {(cuuint64_t)mla::D, (cuuint64_t)mla::PAGE, (cuuint64_t)pool.num_pool_pages};
+  const cuuint64_t strides[2] = {(cuuint64_t)pool.stride_token * 2, (cuuint64_t)pool.stride_page * 2};
+  const cuuint32_t box[3] = {64, (cuuint32_t)mla::PAGE, 1};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(pool.k), dims, strides, box, estr,
+                            CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
 cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
@@ -379,23 +532,24 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  // one CTA per SM (190 KB of shared memory): pick the split count that minimises
-  // waves x pages-per-CTA (+1 page of prologue per wave)
+  CUtensorMap kmap;
+  if (cudaError_t e = make_latent_map(&kmap, pool)) return e;
+  // one CTA per SM (221 KB of shared memory): whole waves of equal CTAs,
+  // cost(sp) = waves x (pages per CTA + ~2 pages of pipeline fill and epilogue)
   int best = 1, best_cost = 1 << 30;
   for (int sp = 1; sp <= kMaxSplits && sp <= max_budget; ++sp) {
     const int waves = (pt.batch * sp + c->num_sms - 1) / c->num_sms;
-    const int cost = waves * ((max_budget + sp - 1) / sp + 1);
+    const int cost = waves * ((max_budget + sp - 1) / sp + 2);
     if (cost < best_cost) { best_cost = cost; best = sp; }
   }
   dim3 grid(best, 1, pt.batch);
-  decode_mla_kernel<<<grid, mla::THREADS, mla::SMEM_BYTES, s>>>(
-      static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(pool.k), pool.stride_page,
-      pool.stride_token, g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count,
-      max_budget, best, c->ws.part_o, c->ws.part_lse, static_cast<__nv_bfloat16*>(out), lse);
+  cudaError_t e = launch_kernel(decode_mla_kernel, grid, dim3(mla::THREADS), (size_t)mla::SMEM_BYTES, s, opt.pdl, kmap,
+                                static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens,
+                                sel_phys, sel_logical, sel_count, max_budget, best, c->ws.part_o, c->ws.part_lse,
+                                c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd),
+                                static_cast<__nv_bfloat16*>(out), lse);
   c->launches += 1;
-  cudaError_t e = cudaGetLastError();
-  if (e != cudaSuccess || best == 1) return e;
-  return launch_combine(c, pt.batch, best, out, lse, s);
+  return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 }  // namespace vx
