@@ -3,23 +3,27 @@
 // width 576 = 512 latent + 64 RoPE shared by all query heads, V = first 512 latent channels, G8).
 //
 // Per 64-token page the work is two dense contractions, ~60 flop per HBM byte:
-//     S^T[64 tokens x 32 heads]  = K[64 x 576] . Q^T          36 x tcgen05.mma  M=64  N=32 K=16
-//     O^T[512 x 32 heads]       += V^T[512 x 64] . P^T   4 x 4 x tcgen05.mma  M=128 N=32 K=16
-// with tokens / channels on the MMA M axis and the 32 heads on N, so no tile is padded.
+//     S[32 heads x 64 tokens]  = Q[32 x 576] . K^T           36 x tcgen05.mma  M=128 N=64 K=16
+//     O^T[512 x 32 heads]     += V^T[512 x 64] . P^T     4 x 4 x tcgen05.mma  M=128 N=32 K=16
+// S keeps the heads on the MMA M axis (rows 32..127 of the A tile are don't-care shared memory: every D row
+// depends on its own A row only).  Measured on B200: an M=64 MMA (tokens on M) issues every ~90 cycles, an
+// M=128 one every ~40, and with heads on TMEM lanes a softmax thread owns one head -- running max, sum and
+// the P row are thread-local, no cross-lane or cross-warp reduction in the loop.
 //
 // Warp-specialised, one CTA per SM:
 //   warp 0      TMA producer.  The latent page (73,728 B, read once for K and V) arrives as nine
 //               [64 tokens x 64 channels] boxes (cp.async.bulk.tensor, 128-byte swizzle) -- exactly the
-//               shared-memory layout both MMAs consume (K-major for K in S^T, MN-major for V^T).  The
-//               ring is managed per BOX PAIR (16 KB = 128 value channels): 10 pair slots + 2 RoPE slots
-//               = 2.5 pages, each slot released by the tcgen05.commit of the last MMA that reads it, so
-//               ~1.5 pages (110 KB) per SM are always in flight.
-//   warp 1      MMA issuer (one lane).  QK(p+1) is issued BEFORE PV(p): the tensor pipe works on the
-//               next page's scores while the softmax warps turn S(p) into P(p).  S^T is double-buffered
-//               in TMEM, O^T (512 x 32 fp32) lives in TMEM for the whole CTA.
-//   warps 2..5  softmax: tcgen05.ld S^T (one token row per thread), head maxima by a transposed shuffle
-//               butterfly + one named barrier, lazy O^T rescale (only when a running max grows by more
-//               than 2^8), P (bf16) to shared memory as the B operand of PV, double-buffered.
+//               shared-memory layout both MMAs consume (K-major B operand of S, MN-major A operand of O^T).
+//               The ring is managed per BOX PAIR (16 KB = 128 value channels): 10 pair slots + 2 RoPE slots
+//               = 2.5 pages, each slot released by the tcgen05.commit of the last MMA that reads it.
+//   warp 1      MMA issuer (one elected lane, polling): PV(p) goes out the moment P(p) is ready, QK of the
+//               following pages box pair by box pair as the tiles land.  S is double-buffered in TMEM, O^T
+//               (512 x 32 fp32) lives in TMEM for the whole CTA.
+//   warp 4      softmax (TMEM lanes 0..31 = heads): tcgen05.ld S, thread-local max / exp2 / sum, P row (bf16,
+//               128 B) to shared memory as the B operand of PV, double-buffered.  O^T is rescaled lazily (only
+//               when a head's running max grows by more than 2^8): the softmax warp publishes the factors,
+//               warps 2, 3, 5 rescale the TMEM lanes it cannot reach.
+//   warps 2..5  epilogue: O^T / l -> partial or final output.
 // Splits of a request merge in-kernel (the last split to arrive merges by LSE).  In the
 // fused step the CTA holding the request's newest page also rebuilds that page's min / max summary from
 // the staged tile (a1; the newest page is a forced local page).
@@ -32,8 +36,9 @@ namespace vx {
 
 namespace mla {
 constexpr int D = 576, DV = 512, PAGE = 64, NH = 32;      // geometry this kernel is built for
-constexpr int THREADS = 192;                              // producer warp, MMA warp, 4 softmax warps
+constexpr int THREADS = 192;                              // producer warp, MMA warp, 4 epilogue warps (one = softmax)
 constexpr int SOFTMAX_THREADS = 128;
+constexpr int SOFTMAX_WARP = 4;                           // warp % 4 == 0: TMEM lanes 0..31
 constexpr int CHUNKS = D * 2 / 16;                        // 72 16-byte chunks per token row
 constexpr int ATOMS = CHUNKS / 8;                         // 9 swizzle atoms (64 channels each)
 constexpr int K_ATOM_BYTES = PAGE * 128;                  // 8192: 64 rows x 128 B
@@ -43,19 +48,20 @@ constexpr int Q_BYTES = ATOMS * Q_ATOM_BYTES;             // 36864
 constexpr int P_BYTES = NH * 128;                         // 4096: [32 heads][64 tokens] bf16
 constexpr int N_PAIR = 10, N_ROPE = 2;                    // ring slots
 constexpr int PAIRS_PER_PAGE = DV / 128;                  // 4
-constexpr int OFF_PAIR = 0;
-constexpr int OFF_ROPE = OFF_PAIR + N_PAIR * PAIR_BYTES;  // 163840
-constexpr int OFF_Q = OFF_ROPE + N_ROPE * K_ATOM_BYTES;   // 180224
-constexpr int OFF_P = OFF_Q + Q_BYTES;                    // 217088
-constexpr int SMEM_BYTES = OFF_P + 2 * P_BYTES + 1024;    // 226304 incl. alignment slack
-constexpr int TMEM_COLS = 256;                            // S^T buffers: cols [0,32), [32,64); O^T block mb: [64+32mb, ..)
-constexpr int TM_O = 64;
+// Q first: the M=128 A tile of S reads 16 KB from each Q atom, i.e. past Q into P / the ring (don't-care rows)
+constexpr int OFF_Q = 0;
+constexpr int OFF_P = OFF_Q + Q_BYTES;                    // 36864
+constexpr int OFF_PAIR = OFF_P + 2 * P_BYTES;             // 45056
+constexpr int OFF_ROPE = OFF_PAIR + N_PAIR * PAIR_BYTES;  // 208896
+constexpr int SMEM_BYTES = OFF_ROPE + N_ROPE * K_ATOM_BYTES + 1024;   // 226304 incl. alignment slack
+constexpr int TMEM_COLS = 256;                            // S buffer b: cols [64b, 64b+64); O^T block mb: [128+32mb, ..)
+constexpr int TM_O = 128;
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.f;                  // log2 units
 
 // instruction descriptors (kind::f16): D fp32, A/B bf16
-constexpr uint32_t IDESC_QK = (1u << 4) | (1u << 7) | (1u << 10) | ((NH >> 3) << 17) | ((64u >> 4) << 24);
+constexpr uint32_t IDESC_QK = (1u << 4) | (1u << 7) | (1u << 10) | ((64u >> 3) << 17) | ((128u >> 4) << 24);   // M128 N64
 constexpr uint32_t IDESC_PV = (1u << 4) | (1u << 7) | (1u << 10) | (1u << 15) | ((NH >> 3) << 17) | ((128u >> 4) << 24);
 
 // shared-memory matrix descriptor, 128-byte swizzle, Blackwell version bit
@@ -118,64 +124,6 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const float (&v)[32]) 
   asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
 }
 
-// max over the 32 lanes of v[j] for every j; lane L returns the result for j == L
-// (transposed butterfly: 16 + 8 + 4 + 2 + 1 shuffles instead of 32 x 5)
-__device__ __forceinline__ float lanes_max_transposed(const float (&v)[32], int lane) {
-  float a[16], b[8], c[4], d[2];
-#pragma unroll
-  for (int j = 0; j < 16; ++j) {
-    const bool up = lane & 16;
-    const float r = __shfl_xor_sync(0xffffffffu, up ? v[j] : v[j + 16], 16);
-    a[j] = fmaxf(up ? v[j + 16] : v[j], r);
-  }
-#pragma unroll
-  for (int j = 0; j < 8; ++j) {
-    const bool up = lane & 8;
-    const float r = __shfl_xor_sync(0xffffffffu, up ? a[j] : a[j + 8], 8);
-    b[j] = fmaxf(up ? a[j + 8] : a[j], r);
-  }
-#pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    const bool up = lane & 4;
-    const float r = __shfl_xor_sync(0xffffffffu, up ? b[j] : b[j + 4], 4);
-    c[j] = fmaxf(up ? b[j + 4] : b[j], r);
-  }
-#pragma unroll
-  for (int j = 0; j < 2; ++j) {
-    const bool up = lane & 2;
-    const float r = __shfl_xor_sync(0xffffffffu, up ? c[j] : c[j + 2], 2);
-    d[j] = fmaxf(up ? c[j + 2] : c[j], r);
-  }
-  const bool up = lane & 1;
-  const float r = __shfl_xor_sync(0xffffffffu, up ? d[0] : d[1], 1);
-  return fmaxf(up ? d[1] : d[0], r);
-}
-// same with a sum
-__device__ __forceinline__ float lanes_sum_transposed(const float (&v)[32], int lane) {
-  float a[16], b[8], c[4], d[2];
-#pragma unroll
-  for (int j = 0; j < 16; ++j) {
-    const bool up = lane & 16;
-    a[j] = (up ? v[j + 16] : v[j]) + __shfl_xor_sync(0xffffffffu, up ? v[j] : v[j + 16], 16);
-  }
-#pragma unroll
-  for (int j = 0; j < 8; ++j) {
-    const bool up = lane & 8;
-    b[j] = (up ? a[j + 8] : a[j]) + __shfl_xor_sync(0xffffffffu, up ? a[j] : a[j + 8], 8);
-  }
-#pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    const bool up = lane & 4;
-    c[j] = (up ? b[j + 4] : b[j]) + __shfl_xor_sync(0xffffffffu, up ? b[j] : b[j + 4], 4);
-  }
-#pragma unroll
-  for (int j = 0; j < 2; ++j) {
-    const bool up = lane & 2;
-    d[j] = (up ? c[j + 2] : c[j]) + __shfl_xor_sync(0xffffffffu, up ? c[j] : c[j + 2], 2);
-  }
-  const bool up = lane & 1;
-  return (up ? d[1] : d[0]) + __shfl_xor_sync(0xffffffffu, up ? d[0] : d[1], 1);
-}
 __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
 }
@@ -188,12 +136,29 @@ __device__ __forceinline__ void tma_box(uint32_t dst, const CUtensorMap* map, in
       "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
       ::"r"(dst), "l"(map), "r"(channel0), "r"(0), "r"(page), "r"(bar) : "memory");
 }
+// one lane of a converged warp; ptxas then feeds tcgen05 / TMA operands straight from that lane (no per-lane loop)
+__device__ __forceinline__ bool elect_one() {
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {   // non-blocking
+  uint32_t ok;
+  asm volatile("{\n\t.reg .pred p;\n\tmbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
 __device__ __forceinline__ void softmax_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(SOFTMAX_THREADS) : "memory"); }
 
 // barrier indices
 constexpr int B_PAIR_FULL = 0, B_PAIR_EMPTY = N_PAIR, B_ROPE_FULL = 2 * N_PAIR, B_ROPE_EMPTY = B_ROPE_FULL + N_ROPE,
               B_S_FULL = B_ROPE_EMPTY + N_ROPE, B_S_EMPTY = B_S_FULL + 2, B_P_FULL = B_S_EMPTY + 2,
-              B_PV_DONE = B_P_FULL + 2, N_BARS = B_PV_DONE + 2;
+              B_PV_DONE = B_P_FULL + 2, B_DECIDE = B_PV_DONE + 2, B_ACK = B_DECIDE + 2, N_BARS = B_ACK + 2;
 }  // namespace mla
 
 __global__ void __launch_bounds__(mla::THREADS, 1)
@@ -207,7 +172,9 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t s_bar[N_BARS];
   __shared__ uint32_t s_tmem;
-  __shared__ float s_wred[2][4][NH], s_lred[4][NH];
+  __shared__ float s_fac[2][NH];                       // lazy-rescale factors of page p (buffer p & 1)
+  __shared__ int s_flag[2];                            // ... and whether any head needs them
+  __shared__ float s_l[NH], s_m[NH];                   // final denominators / references
   __shared__ int s_last;
 
   const int split = blockIdx.x, i = blockIdx.z;
@@ -230,14 +197,16 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
     for (int s = 0; s < N_ROPE; ++s) { mbar_init(bar(B_ROPE_FULL + s), 1); mbar_init(bar(B_ROPE_EMPTY + s), 1); }
     for (int b = 0; b < 2; ++b) {
       mbar_init(bar(B_S_FULL + b), 1);
-      mbar_init(bar(B_S_EMPTY + b), 4);
-      mbar_init(bar(B_P_FULL + b), 4);
+      mbar_init(bar(B_S_EMPTY + b), 1);
+      mbar_init(bar(B_P_FULL + b), 1);
       mbar_init(bar(B_PV_DONE + b), 1);
+      mbar_init(bar(B_DECIDE + b), 1);
+      mbar_init(bar(B_ACK + b), 3);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&kmap) : "memory");
   }
-  if (warp >= 2) {                                     // Q[32 x 576] -> K-major swizzled B operand (zero rows past Hq)
+  if (warp >= 2) {                                     // Q[32 x 576] -> K-major swizzled A operand (zero rows past Hq)
     for (int x = tid - 64; x < NH * CHUNKS; x += SOFTMAX_THREADS) {
       const int h = x / CHUNKS, c = x % CHUNKS;
       uint4 v = make_uint4(0, 0, 0, 0);
@@ -279,7 +248,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
     for (int p = 0; p < n_pages; ++p) {
       if ((p & 31) == 0) my_phys = p + lane < n_pages ? phys_list[p + lane] : 0;
       const int phys = __shfl_sync(0xffffffffu, my_phys, p & 31);
-      if (lane == 0) {
+      if (elect_one()) {
         const int rs = p % N_ROPE, ru = p / N_ROPE;
         if (ru >= 1) mbar_wait(bar(B_ROPE_EMPTY + rs), (ru - 1) & 1);
         mbar_expect_tx(bar(B_ROPE_FULL + rs), K_ATOM_BYTES);
@@ -297,161 +266,208 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       __syncwarp();
     }
   } else if (warp == 1) {
-    // ===== MMA issuer: QK(p) is issued before PV(p-1) ====================================================
-    for (int p = 0; p <= n_pages; ++p) {
-      if (p < n_pages) {
-        const int b = p & 1;
-        if (p >= 2) mbar_wait(bar(B_S_EMPTY + b), ((p >> 1) - 1) & 1);   // softmax has read S(p-2)
-        const int rs = p % N_ROPE;
-        mbar_wait(bar(B_ROPE_FULL + rs), (p / N_ROPE) & 1);
-        tc_fence_after();
-        if (lane == 0) {
-          const uint32_t a = base + OFF_ROPE + rs * K_ATOM_BYTES, bq = q_base + 8 * Q_ATOM_BYTES;
+    // ===== MMA issuer: the whole warp runs the (warp-uniform) polling state machine, one elected lane issues.
+    // PV(p) goes out the moment P(p) is ready -- it frees ring slots -- and QK of the following pages is issued
+    // box pair by box pair as the tiles land, so the tensor pipe works on S(p+1) while the softmax warp turns
+    // S(p) into P(p).
+    int qk_p = 0, qk_g = 0;                              // next QK page / group in it (0 = RoPE box, 1..4 = box pairs)
+    int pv_p = 0;                                        // next PV page
+    while (pv_p < n_pages) {
+      bool pv_ready = pv_p < qk_p && mbar_test(bar(B_P_FULL + (pv_p & 1)), (pv_p >> 1) & 1);
+      pv_ready = __shfl_sync(0xffffffffu, pv_ready, 0);
+      if (pv_ready) {
+        tc_fence_after();                                // P(pv_p) written, O^T rescaled if it had to be
+        const int b = pv_p & 1;
+        if (elect_one()) {
 #pragma unroll
-          for (int ks = 0; ks < 4; ++ks)
-            umma(tmem + b * 32, smem_desc(a + ks * 32, 16, 1024), smem_desc(bq + ks * 32, 16, 1024), IDESC_QK, ks > 0);
-          umma_commit(bar(B_ROPE_EMPTY + rs));
-        }
-#pragma unroll 1
-        for (int j = 0; j < PAIRS_PER_PAGE; ++j) {
-          const int g = p * PAIRS_PER_PAGE + j, ps = g % N_PAIR;
-          mbar_wait(bar(B_PAIR_FULL + ps), (g / N_PAIR) & 1);
-          tc_fence_after();
-          if (lane == 0) {
+          for (int ks = 0; ks < PAGE / 16; ++ks)         // ks-major: consecutive MMAs go to different O^T blocks
 #pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              const uint32_t a = base + OFF_PAIR + ps * PAIR_BYTES + (ks >> 2) * K_ATOM_BYTES + (ks & 3) * 32;
-              const uint32_t bq = q_base + (2 * j + (ks >> 2)) * Q_ATOM_BYTES + (ks & 3) * 32;
-              umma(tmem + b * 32, smem_desc(a, 16, 1024), smem_desc(bq, 16, 1024), IDESC_QK, true);
+            for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
+              const int ps = (pv_p * PAIRS_PER_PAGE + mb) % N_PAIR;
+              umma(tmem + TM_O + 32 * mb, smem_desc(base + OFF_PAIR + ps * PAIR_BYTES + ks * 2048, K_ATOM_BYTES, 1024),
+                   smem_desc(p_base + b * P_BYTES + ks * 32, 16, 1024), IDESC_PV, pv_p > 0 || ks > 0);
             }
-          }
-        }
-        if (lane == 0) umma_commit(bar(B_S_FULL + b));
-        __syncwarp();
-      }
-      if (p >= 1) {
-        const int pq = p - 1, b = pq & 1;
-        mbar_wait(bar(B_P_FULL + b), (pq >> 1) & 1);     // P(pq) written, O^T rescaled if it had to be
-        tc_fence_after();
-        if (lane == 0) {
 #pragma unroll
-          for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
-            const int g = pq * PAIRS_PER_PAGE + mb, ps = g % N_PAIR;
-            const uint32_t a = base + OFF_PAIR + ps * PAIR_BYTES;
-#pragma unroll
-            for (int ks = 0; ks < PAGE / 16; ++ks)
-              umma(tmem + TM_O + 32 * mb, smem_desc(a + ks * 2048, K_ATOM_BYTES, 1024),
-                   smem_desc(p_base + b * P_BYTES + ks * 32, 16, 1024), IDESC_PV, pq > 0 || ks > 0);
-            umma_commit(bar(B_PAIR_EMPTY + ps));         // this pair slot may be refilled
-          }
+          for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb)    // the pair slots may be refilled
+            umma_commit(bar(B_PAIR_EMPTY + (pv_p * PAIRS_PER_PAGE + mb) % N_PAIR));
           umma_commit(bar(B_PV_DONE + b));
         }
         __syncwarp();
+        ++pv_p;
+        continue;
+      }
+      if (qk_p < n_pages) {
+        const int b = qk_p & 1;
+        if (qk_g == 0) {
+          const int rs = qk_p % N_ROPE;
+          bool ok = (qk_p < 2 || mbar_test(bar(B_S_EMPTY + b), ((qk_p >> 1) - 1) & 1)) &&     // softmax has read S(p-2)
+                    mbar_test(bar(B_ROPE_FULL + rs), (qk_p / N_ROPE) & 1);
+          ok = __shfl_sync(0xffffffffu, ok, 0);
+          if (ok) {
+            tc_fence_after();
+            if (elect_one()) {
+              const uint32_t kb = base + OFF_ROPE + rs * K_ATOM_BYTES, qa = q_base + 8 * Q_ATOM_BYTES;
+#pragma unroll
+              for (int ks = 0; ks < 4; ++ks)
+                umma(tmem + b * 64, smem_desc(qa + ks * 32, 16, 1024), smem_desc(kb + ks * 32, 16, 1024), IDESC_QK, ks > 0);
+              umma_commit(bar(B_ROPE_EMPTY + rs));
+            }
+            __syncwarp();
+            qk_g = 1;
+          }
+        } else {
+          const int j = qk_g - 1, g = qk_p * PAIRS_PER_PAGE + j, ps = g % N_PAIR;
+          bool ok = mbar_test(bar(B_PAIR_FULL + ps), (g / N_PAIR) & 1);
+          ok = __shfl_sync(0xffffffffu, ok, 0);
+          if (ok) {
+            tc_fence_after();
+            if (elect_one()) {
+#pragma unroll
+              for (int ks = 0; ks < 8; ++ks) {
+                const uint32_t kb = base + OFF_PAIR + ps * PAIR_BYTES + (ks >> 2) * K_ATOM_BYTES + (ks & 3) * 32;
+                const uint32_t qa = q_base + (2 * j + (ks >> 2)) * Q_ATOM_BYTES + (ks & 3) * 32;
+                umma(tmem + b * 64, smem_desc(qa, 16, 1024), smem_desc(kb, 16, 1024), IDESC_QK, true);
+              }
+              if (qk_g == PAIRS_PER_PAGE) umma_commit(bar(B_S_FULL + b));
+            }
+            __syncwarp();
+            if (++qk_g > PAIRS_PER_PAGE) { qk_g = 0; ++qk_p; }
+          }
+        }
       }
     }
     pdl_trigger();
   } else {
-    // ===== softmax warps (one S^T token row per thread; 16 live lanes per warp at M = 64) ==================
+    // ===== warps 2..5: softmax (warp 4) + rescale helpers, then the epilogue ==============================
     const int sp = warp & 3;                             // TMEM sub-partition this warp may access
-    const int stid = tid - 64;
     const uint32_t t_lane = tmem + ((uint32_t)(sp * 32) << 16);
-    const int row = sp * 16 + lane;                      // M = 64: token row r sits in TMEM lane (r % 16) + 32 * (r / 16)
-    float m_ref[NH], l_thr[NH];
-#pragma unroll
-    for (int j = 0; j < NH; ++j) { m_ref[j] = 0.f; l_thr[j] = 0.f; }
-    int lg = log_list[0];
-    int valid = PAGE;
-    for (int p = 0; p < n_pages; ++p) {
-      const int b = p & 1;
-      valid = min(PAGE, n_tok - lg * PAGE);
-      if (p + 1 < n_pages) lg = log_list[p + 1];         // prefetch for the next page
-      const bool live = lane < 16 && row < valid;
-      mbar_wait(bar(B_S_FULL + b), (p >> 1) & 1);
-      tc_fence_after();
-      float s[NH];
-      tmem_ld32(t_lane + b * 32, s);
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(B_S_EMPTY + b));    // S buffer b may be overwritten by QK(p+2)
-#pragma unroll
-      for (int j = 0; j < NH; ++j) s[j] = live ? s[j] * scale_log2 : -INFINITY;
-      s_wred[b][sp][lane] = lanes_max_transposed(s, lane);
-      softmax_barrier();
-      // every thread keeps the per-head running reference (lazy: it moves only on a growth > 2^8)
-      float fac[NH];
-      bool grow_any = false;
-#pragma unroll
-      for (int j = 0; j < NH; ++j) {
-        const float tmax = fmaxf(fmaxf(s_wred[b][0][j], s_wred[b][1][j]), fmaxf(s_wred[b][2][j], s_wred[b][3][j]));
-        const bool grow = p > 0 && tmax > m_ref[j] + kRescaleThreshold;
-        fac[j] = grow ? exp2f(m_ref[j] - tmax) : 1.f;
-        if (p == 0 || grow) m_ref[j] = tmax;
-        grow_any |= grow;
-      }
-      if (p >= 2) mbar_wait(bar(B_PV_DONE + b), ((p >> 1) - 1) & 1);     // PV(p-2) done: P buffer b is free
-      if (grow_any) {                                    // rare: rescale O^T in TMEM and the partial denominators
-        mbar_wait(bar(B_PV_DONE + ((p - 1) & 1)), ((p - 1) >> 1) & 1);   // PV(p-1) done: O^T is stable
-        tc_fence_after();
-#pragma unroll 1
-        for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
-          float o[NH];
-          tmem_ld32(t_lane + TM_O + 32 * mb, o);
-#pragma unroll
-          for (int j = 0; j < NH; ++j) o[j] *= fac[j];
-          tmem_st32(t_lane + TM_O + 32 * mb, o);
-        }
-#pragma unroll
-        for (int j = 0; j < NH; ++j) l_thr[j] *= fac[j];
-        tc_fence_before();
-      }
-      if (valid < PAGE) {                                // partial page: zero the stale value rows (0 x garbage must be 0)
-        const int n_rows = PAGE - valid;
-        for (int x = stid; x < n_rows * 64; x += SOFTMAX_THREADS) {
-          const int r = valid + x / 64, a = (x % 64) >> 3, c = x & 7;
-          const int g = p * PAIRS_PER_PAGE + (a >> 1), ps = g % N_PAIR;
-          *reinterpret_cast<uint4*>(sm + OFF_PAIR + ps * PAIR_BYTES + (a & 1) * K_ATOM_BYTES + (r >> 3) * 1024 +
-                                    (r & 7) * 128 + c * 16) = make_uint4(0, 0, 0, 0);
-        }
-      }
-      if (lane < 16) {                                   // P[head][token] bf16, K-major swizzled B operand
-        uint8_t* pdst = sm + OFF_P + b * P_BYTES + (row & 7) * 2;
-        const int tc = row >> 3;
-#pragma unroll
-        for (int j = 0; j < NH; ++j) {
-          const float pj = exp2f(s[j] - m_ref[j]);
-          l_thr[j] += pj;
-          *reinterpret_cast<__nv_bfloat16*>(pdst + (j >> 3) * 1024 + (j & 7) * 128 + ((tc ^ (j & 7)) << 4)) =
-              __float2bfloat16_rn(pj);
-        }
-      }
-      fence_async_proxy();                               // P / zeroed rows visible to the MMA proxy
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(B_P_FULL + b));
-    }
-    // ---- epilogue ------------------------------------------------------------------------------------------
     const int pl = n_pages - 1;
-    if (summary_upd != nullptr && lg == newest_page && stid < CHUNKS) {
-      // (a1) the request's newest page is this CTA's last page: rebuild its min / max summary from the staged
-      // tile (exact in bf16).  Thread owns one 16-byte channel chunk over the valid tokens.
-      const int cc = stid, a = cc >> 3;
-      const uint8_t* atom = a < 8 ? sm + OFF_PAIR + ((pl * PAIRS_PER_PAGE + (a >> 1)) % N_PAIR) * PAIR_BYTES + (a & 1) * K_ATOM_BYTES
-                                  : sm + OFF_ROPE + (pl % N_ROPE) * K_ATOM_BYTES;
-      uint4 lo4 = *reinterpret_cast<const uint4*>(atom + ((cc & 7) << 4)), hi4 = lo4;     // token 0
-      __nv_bfloat162* lo = reinterpret_cast<__nv_bfloat162*>(&lo4);
-      __nv_bfloat162* hi = reinterpret_cast<__nv_bfloat162*>(&hi4);
-      for (int r = 1; r < valid; ++r) {
-        const uint4 v4 = *reinterpret_cast<const uint4*>(atom + (r >> 3) * 1024 + (r & 7) * 128 + (((cc & 7) ^ (r & 7)) << 4));
-        const __nv_bfloat162* v = reinterpret_cast<const __nv_bfloat162*>(&v4);
+    if (warp == SOFTMAX_WARP) {
+      // thread = head `lane` (TMEM lane); columns = the 64 tokens of the page
+      float m_ref = 0.f, l_sum = 0.f;
+      int lg = log_list[0];
+      for (int p = 0; p < n_pages; ++p) {
+        const int b = p & 1;
+        const int valid = min(PAGE, n_tok - lg * PAGE);
+        if (p + 1 < n_pages) lg = log_list[p + 1];       // prefetch for the next page
+        mbar_wait(bar(B_S_FULL + b), (p >> 1) & 1);
+        tc_fence_after();
+        float s[PAGE];
+        tmem_ld32(t_lane + b * 64, *reinterpret_cast<float(*)[32]>(&s[0]));
+        tmem_ld32(t_lane + b * 64 + 32, *reinterpret_cast<float(*)[32]>(&s[32]));
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(B_S_EMPTY + b));  // S buffer b may be overwritten by QK(p+2)
+        float tmax = -INFINITY;
 #pragma unroll
-        for (int e = 0; e < 4; ++e) { lo[e] = __hmin2(lo[e], v[e]); hi[e] = __hmax2(hi[e], v[e]); }
+        for (int t = 0; t < PAGE; ++t) {
+          s[t] = t < valid ? s[t] * scale_log2 : -INFINITY;
+          tmax = fmaxf(tmax, s[t]);
+        }
+        // lazy running reference: it moves only on a growth > 2^8 (token 0 of a page is always valid: tmax finite)
+        const bool grow = p > 0 && tmax > m_ref + kRescaleThreshold;
+        const float fac = grow ? exp2f(m_ref - tmax) : 1.f;
+        if (p == 0 || grow) m_ref = tmax;
+        l_sum *= fac;
+        const bool grow_any = __any_sync(0xffffffffu, grow);
+        // publish the decision to the helper warps (they acknowledged page p-2 before its buffer is reused)
+        if (p >= 2) mbar_wait(bar(B_ACK + b), ((p >> 1) - 1) & 1);
+        s_fac[b][lane] = fac;
+        if (lane == 0) s_flag[b] = grow_any;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(B_DECIDE + b));
+        if (p >= 2) mbar_wait(bar(B_PV_DONE + b), ((p >> 1) - 1) & 1);   // PV(p-2) done: P buffer b is free
+        if (grow_any) {                                  // rare: rescale O^T in TMEM (my 32 lanes; helpers do theirs)
+          mbar_wait(bar(B_PV_DONE + ((p - 1) & 1)), ((p - 1) >> 1) & 1); // PV(p-1) done: O^T is stable
+          tc_fence_after();
+#pragma unroll 1
+          for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
+            float o[NH];
+            tmem_ld32(t_lane + TM_O + 32 * mb, o);
+#pragma unroll
+            for (int j = 0; j < NH; ++j) o[j] *= s_fac[b][j];
+            tmem_st32(t_lane + TM_O + 32 * mb, o);
+          }
+          tc_fence_before();
+          mbar_wait(bar(B_ACK + b), (p >> 1) & 1);        // the helpers have rescaled their lanes
+        }
+        if (valid < PAGE) {                              // partial page: zero the stale value rows (0 x garbage must be 0)
+          const int n_rows = PAGE - valid;
+          for (int xx = lane; xx < n_rows * 64; xx += kWarp) {
+            const int r = valid + xx / 64, a = (xx % 64) >> 3, c = xx & 7;
+            const int ps = (p * PAIRS_PER_PAGE + (a >> 1)) % N_PAIR;
+            *reinterpret_cast<uint4*>(sm + OFF_PAIR + ps * PAIR_BYTES + (a & 1) * K_ATOM_BYTES + (r >> 3) * 1024 +
+                                      (r & 7) * 128 + c * 16) = make_uint4(0, 0, 0, 0);
+          }
+        }
+        // P[head = lane][token] bf16: one 128-byte row of the K-major swizzled B operand
+        uint8_t* prow = sm + OFF_P + b * P_BYTES + (lane >> 3) * 1024 + (lane & 7) * 128;
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          uint32_t w[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const float p0 = ex2_approx(s[8 * c + 2 * e] - m_ref), p1 = ex2_approx(s[8 * c + 2 * e + 1] - m_ref);
+            l_sum += p0 + p1;
+            __nv_bfloat162 v = __floats2bfloat162_rn(p0, p1);
+            w[e] = *reinterpret_cast<uint32_t*>(&v);
+          }
+          *reinterpret_cast<uint4*>(prow + ((c ^ (lane & 7)) << 4)) = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+        fence_async_proxy();                             // P / zeroed rows visible to the MMA proxy
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(B_P_FULL + b));
       }
-      __nv_bfloat16* dst = summary_upd + (int64_t)phys_list[pl] * 2 * D + cc * 8;
-      *reinterpret_cast<uint4*>(dst) = lo4;
-      *reinterpret_cast<uint4*>(dst + D) = hi4;
+      s_l[lane] = l_sum;
+      s_m[lane] = m_ref;
+    } else {
+      // helper warps: follow the softmax warp's decisions; rescale their TMEM lanes of O^T when asked (rare)
+      for (int p = 0; p < n_pages; ++p) {
+        const int b = p & 1;
+        mbar_wait(bar(B_DECIDE + b), (p >> 1) & 1);
+        if (s_flag[b]) {
+          mbar_wait(bar(B_PV_DONE + ((p - 1) & 1)), ((p - 1) >> 1) & 1);
+          tc_fence_after();
+#pragma unroll 1
+          for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
+            float o[NH];
+            tmem_ld32(t_lane + TM_O + 32 * mb, o);
+#pragma unroll
+            for (int j = 0; j < NH; ++j) o[j] *= s_fac[b][j];
+            tmem_st32(t_lane + TM_O + 32 * mb, o);
+          }
+          tc_fence_before();
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(B_ACK + b));
+      }
+      // (a1) the request's newest page is this CTA's last page: rebuild its min / max summary from the staged
+      // tile (exact in bf16).  One helper thread per 16-byte channel chunk over the valid tokens.
+      const int hidx = (warp == 5 ? 2 : warp - 2) * kWarp + lane;      // 0..95
+      const int lg_last = log_list[pl];
+      if (summary_upd != nullptr && lg_last == newest_page && hidx < CHUNKS) {
+        mbar_wait(bar(B_S_FULL + (pl & 1)), (pl >> 1) & 1);            // QK(last) done: every box of the page has landed
+        const int valid = min(PAGE, n_tok - lg_last * PAGE);
+        const int cc = hidx, a = cc >> 3;
+        const uint8_t* atom = a < 8 ? sm + OFF_PAIR + ((pl * PAIRS_PER_PAGE + (a >> 1)) % N_PAIR) * PAIR_BYTES + (a & 1) * K_ATOM_BYTES
+                                    : sm + OFF_ROPE + (pl % N_ROPE) * K_ATOM_BYTES;
+        uint4 lo4 = *reinterpret_cast<const uint4*>(atom + ((cc & 7) << 4)), hi4 = lo4;     // token 0
+        __nv_bfloat162* lo = reinterpret_cast<__nv_bfloat162*>(&lo4);
+        __nv_bfloat162* hi = reinterpret_cast<__nv_bfloat162*>(&hi4);
+        for (int r = 1; r < valid; ++r) {
+          const uint4 v4 = *reinterpret_cast<const uint4*>(atom + (r >> 3) * 1024 + (r & 7) * 128 + (((cc & 7) ^ (r & 7)) << 4));
+          const __nv_bfloat162* v = reinterpret_cast<const __nv_bfloat162*>(&v4);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) { lo[e] = __hmin2(lo[e], v[e]); hi[e] = __hmax2(hi[e], v[e]); }
+        }
+        __nv_bfloat16* dst = summary_upd + (int64_t)phys_list[pl] * 2 * D + cc * 8;
+        *reinterpret_cast<uint4*>(dst) = lo4;
+        *reinterpret_cast<uint4*>(dst + D) = hi4;
+      }
     }
-    s_lred[sp][lane] = lanes_sum_transposed(l_thr, lane);
-    softmax_barrier();
-    mbar_wait(bar(B_PV_DONE + (pl & 1)), (pl >> 1) & 1);   // the last PV has landed in TMEM
+    // ---- epilogue (warps 2..5): O^T / l -> partial or final output ----------------------------------------
+    softmax_barrier();                                   // s_l / s_m published
+    mbar_wait(bar(B_PV_DONE + (pl & 1)), (pl >> 1) & 1); // the last PV has landed in TMEM
     tc_fence_after();
 #pragma unroll 1
     for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
@@ -461,23 +477,18 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
 #pragma unroll
       for (int j = 0; j < NH; ++j) {
         if (j < num_q_heads) {
-          const float lsum = s_lred[0][j] + s_lred[1][j] + s_lred[2][j] + s_lred[3][j];
-          const float val = o[j] / lsum;
+          const float val = o[j] / s_l[j];
           const int64_t orow = (int64_t)i * num_q_heads + j;
           if (num_splits == 1) out[orow * DV + d] = __float2bfloat16_rn(val);
           else part_o[(orow * num_splits + split) * DV + d] = val;
         }
       }
     }
-#pragma unroll
-    for (int j = 0; j < NH; ++j) {
-      if (stid == j && j < num_q_heads) {
-        const float lsum = s_lred[0][j] + s_lred[1][j] + s_lred[2][j] + s_lred[3][j];
-        const float lse = (m_ref[j] + log2f(lsum)) * kLn2;
-        const int64_t orow = (int64_t)i * num_q_heads + j;
-        if (num_splits == 1) { if (lse_out) lse_out[orow] = lse; }
-        else part_lse[orow * num_splits + split] = lse;
-      }
+    if (warp == SOFTMAX_WARP && lane < num_q_heads) {
+      const float lse = (s_m[lane] + log2f(s_l[lane])) * kLn2;
+      const int64_t orow = (int64_t)i * num_q_heads + lane;
+      if (num_splits == 1) { if (lse_out) lse_out[orow] = lse; }
+      else part_lse[orow * num_splits + split] = lse;
     }
   }
 
@@ -486,7 +497,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   if (num_splits > 1) {
     if (last_split_arrives(unit_counter + i, num_splits, &s_last))
       merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads, num_q_heads, num_splits, DV, out, lse_out,
-                                     reinterpret_cast<float*>(sm + OFF_Q));
+                                    reinterpret_cast<float*>(sm + OFF_PAIR));
   }
   __syncthreads();
   if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
