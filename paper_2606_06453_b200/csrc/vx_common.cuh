@@ -90,9 +90,9 @@ __device__ __forceinline__ float ldcg_f32(const float* p) {
 // partials.  Call with the whole CTA after its own partial (o, lse) is written.  Returns true in the CTA
 // that must merge.  counter is zero on entry to the step and is left zero.
 __device__ __forceinline__ bool last_split_arrives(int* counter, int num_splits, int* s_flag) {
-  __threadfence();                               // this thread's partial stores are visible device-wide
-  __syncthreads();
+  __syncthreads();                               // every thread's partial stores happen-before thread 0's fence ...
   if (threadIdx.x == 0) {
+    __threadfence();                             // ... which is cumulative: they are visible device-wide before the count
     const int old = atomicAdd(counter, 1);
     const bool last = old == num_splits - 1;
     if (last) *counter = 0;                      // self-cleaning: ready for the next step
@@ -121,19 +121,22 @@ __device__ __forceinline__ void store4(__nv_bfloat16* dst, float4 v) {
 template <typename T>
 __device__ __forceinline__ void merge_partials(const float* part_o, const float* part_lse, int64_t row0, int n_rows,
                                                int n_part, int v_dim, T* out, float* lse, float* s_w) {
+  for (int e = threadIdx.x; e < n_rows * n_part; e += blockDim.x)       // all lse values in one round trip
+    s_w[e] = ldcg_f32(part_lse + row0 * n_part + e);
+  __syncthreads();
   for (int r = threadIdx.x; r < n_rows; r += blockDim.x) {
-    const float* ls = part_lse + (row0 + r) * n_part;
+    float* w = s_w + r * n_part;
     float mx = -INFINITY;
-    for (int s = 0; s < n_part; ++s) mx = fmaxf(mx, ldcg_f32(ls + s));
+    for (int s = 0; s < n_part; ++s) mx = fmaxf(mx, w[s]);
     float z = 0.f;
-    for (int s = 0; s < n_part; ++s) z += mx == -INFINITY ? 0.f : __expf(ldcg_f32(ls + s) - mx);
+    for (int s = 0; s < n_part; ++s) z += mx == -INFINITY ? 0.f : __expf(w[s] - mx);
     const float inv = z > 0.f ? 1.f / z : 0.f;
-    for (int s = 0; s < n_part; ++s) s_w[r * n_part + s] = mx == -INFINITY ? 0.f : __expf(ldcg_f32(ls + s) - mx) * inv;
+    for (int s = 0; s < n_part; ++s) w[s] = mx == -INFINITY ? 0.f : __expf(w[s] - mx) * inv;
     if (lse != nullptr) lse[row0 + r] = z > 0.f ? mx + logf(z) : -INFINITY;
   }
   __syncthreads();
   const int vec = v_dim / 4;
-#pragma unroll 4
+#pragma unroll 8
   for (int e = threadIdx.x; e < n_rows * vec; e += blockDim.x) {
     const int r = e / vec, c = (e % vec) * 4;
     const float* src = part_o + (row0 + r) * n_part * v_dim + c;

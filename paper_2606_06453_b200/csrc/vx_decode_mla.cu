@@ -3,21 +3,23 @@
 // width 576 = 512 latent + 64 RoPE shared by all query heads, V = first 512 latent channels, G8).
 //
 // Per 64-token page the work is two dense contractions, ~60 flop per HBM byte:
-//     S[32 heads x 64 tokens]  = Q[32 x 576] . K^T           36 x tcgen05.mma  M=128 N=64 K=16
+//     S[32 heads x 64 tokens]  = Q[32 x 576] . K^T           36 x tcgen05.mma  M=128 N=64 K=16, A = Q in TMEM
 //     O^T[512 x 32 heads]     += V^T[512 x 64] . P^T     4 x 4 x tcgen05.mma  M=128 N=32 K=16
-// S keeps the heads on the MMA M axis (rows 32..127 of the A tile are don't-care shared memory: every D row
-// depends on its own A row only).  Measured on B200: an M=64 MMA (tokens on M) issues every ~90 cycles, an
-// M=128 one every ~40, and with heads on TMEM lanes a softmax thread owns one head -- running max, sum and
-// the P row are thread-local, no cross-lane or cross-warp reduction in the loop.
+// S keeps the heads on the MMA M axis (TMEM lanes 32..127 of the A operand are don't-care: every D row depends
+// on its own A row only), and Q -- constant for the whole CTA -- is the A operand held in TENSOR MEMORY
+// (288 columns, written once with tcgen05.st).  Measured on B200 (clock64 traces): with a K-major A tile in
+// shared memory an MMA of this shape retires every ~107 cycles (the 128-row A fetch dominates the skinny
+// N = 64 math), which made the tensor pipe, not HBM, the bound.  With heads on TMEM lanes a softmax thread owns
+// one head: running max, sum and the P row are thread-local, no cross-lane or cross-warp reduction in the loop.
 //
 // Warp-specialised, one CTA per SM:
 //   warp 0      TMA producer.  The latent page (73,728 B, read once for K and V) arrives as nine
 //               [64 tokens x 64 channels] boxes (cp.async.bulk.tensor, 128-byte swizzle) -- exactly the
 //               shared-memory layout both MMAs consume (K-major B operand of S, MN-major A operand of O^T).
-//               The ring is managed per BOX PAIR (16 KB = 128 value channels): 10 pair slots + 2 RoPE slots
-//               = 2.5 pages, each slot released by the tcgen05.commit of the last MMA that reads it.
+//               The ring is managed per BOX PAIR (16 KB = 128 value channels): 12 pair slots + 3 RoPE slots
+//               = 3 pages, each slot released by the tcgen05.commit of the last MMA that reads it.
 //   warp 1      MMA issuer (one elected lane, polling): PV(p) goes out the moment P(p) is ready, QK of the
-//               following pages box pair by box pair as the tiles land.  S is double-buffered in TMEM, O^T
+//               following pages box pair by box pair as the tiles land.  S (64 columns) and O^T
 //               (512 x 32 fp32) lives in TMEM for the whole CTA.
 //   warp 4      softmax (TMEM lanes 0..31 = heads): tcgen05.ld S, thread-local max / exp2 / sum, P row (bf16,
 //               128 B) to shared memory as the B operand of PV, double-buffered.  O^T is rescaled lazily (only
@@ -43,19 +45,17 @@ constexpr int CHUNKS = D * 2 / 16;                        // 72 16-byte chunks p
 constexpr int ATOMS = CHUNKS / 8;                         // 9 swizzle atoms (64 channels each)
 constexpr int K_ATOM_BYTES = PAGE * 128;                  // 8192: 64 rows x 128 B
 constexpr int PAIR_BYTES = 2 * K_ATOM_BYTES;              // 16384: 128 value channels
-constexpr int Q_ATOM_BYTES = NH * 128;                    // 4096
-constexpr int Q_BYTES = ATOMS * Q_ATOM_BYTES;             // 36864
 constexpr int P_BYTES = NH * 128;                         // 4096: [32 heads][64 tokens] bf16
-constexpr int N_PAIR = 10, N_ROPE = 2;                    // ring slots
+constexpr int N_PAIR = 12, N_ROPE = 3;                    // ring slots: 3 pages
 constexpr int PAIRS_PER_PAGE = DV / 128;                  // 4
-// Q first: the M=128 A tile of S reads 16 KB from each Q atom, i.e. past Q into P / the ring (don't-care rows)
-constexpr int OFF_Q = 0;
-constexpr int OFF_P = OFF_Q + Q_BYTES;                    // 36864
-constexpr int OFF_PAIR = OFF_P + 2 * P_BYTES;             // 45056
-constexpr int OFF_ROPE = OFF_PAIR + N_PAIR * PAIR_BYTES;  // 208896
-constexpr int SMEM_BYTES = OFF_ROPE + N_ROPE * K_ATOM_BYTES + 1024;   // 226304 incl. alignment slack
-constexpr int TMEM_COLS = 256;                            // S buffer b: cols [64b, 64b+64); O^T block mb: [128+32mb, ..)
-constexpr int TM_O = 128;
+constexpr int OFF_P = 0;
+constexpr int OFF_PAIR = OFF_P + 2 * P_BYTES;             // 8192
+constexpr int OFF_ROPE = OFF_PAIR + N_PAIR * PAIR_BYTES;  // 204800
+constexpr int SMEM_BYTES = OFF_ROPE + N_ROPE * K_ATOM_BYTES + 1024;   // 230400 incl. alignment slack
+constexpr int TMEM_COLS = 512;
+constexpr int TM_Q = 0;                                   // Q[head = lane][576 bf16] as 288 32-bit columns (A operand of S)
+constexpr int TM_S = 320;                                 // S[head][64 tokens]
+constexpr int TM_O = 384;                                 // O^T block mb: [384 + 32mb, +32)
 constexpr float kLog2e = 1.4426950408889634f;
 constexpr float kLn2 = 0.6931471805599453f;
 constexpr float kRescaleThreshold = 8.f;                  // log2 units
@@ -74,6 +74,13 @@ __device__ __forceinline__ void umma(uint32_t d_tmem, uint64_t a_desc, uint64_t 
       "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
       ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"((uint32_t)accumulate));
+}
+// same with the A operand in tensor memory (32-bit columns, two bf16 along K per column)
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, bool accumulate) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"((uint32_t)accumulate));
 }
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
@@ -157,7 +164,7 @@ __device__ __forceinline__ void softmax_barrier() { asm volatile("bar.sync 1, %0
 
 // barrier indices
 constexpr int B_PAIR_FULL = 0, B_PAIR_EMPTY = N_PAIR, B_ROPE_FULL = 2 * N_PAIR, B_ROPE_EMPTY = B_ROPE_FULL + N_ROPE,
-              B_S_FULL = B_ROPE_EMPTY + N_ROPE, B_S_EMPTY = B_S_FULL + 2, B_P_FULL = B_S_EMPTY + 2,
+              B_S_FULL = B_ROPE_EMPTY + N_ROPE, B_S_EMPTY = B_S_FULL + 1, B_P_FULL = B_S_EMPTY + 1,
               B_PV_DONE = B_P_FULL + 2, B_DECIDE = B_PV_DONE + 2, B_ACK = B_DECIDE + 2, N_BARS = B_ACK + 2;
 }  // namespace mla
 
@@ -174,7 +181,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   __shared__ uint32_t s_tmem;
   __shared__ float s_fac[2][NH];                       // lazy-rescale factors of page p (buffer p & 1)
   __shared__ int s_flag[2];                            // ... and whether any head needs them
-  __shared__ float s_l[NH], s_m[NH];                   // final denominators / references
+  __shared__ float s_l[NH], s_m[NH], s_inv[NH];        // final denominators / references
   __shared__ int s_last;
 
   const int split = blockIdx.x, i = blockIdx.z;
@@ -195,9 +202,9 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   if (tid == 0) {
     for (int s = 0; s < N_PAIR; ++s) { mbar_init(bar(B_PAIR_FULL + s), 1); mbar_init(bar(B_PAIR_EMPTY + s), 1); }
     for (int s = 0; s < N_ROPE; ++s) { mbar_init(bar(B_ROPE_FULL + s), 1); mbar_init(bar(B_ROPE_EMPTY + s), 1); }
+    mbar_init(bar(B_S_FULL), 1);
+    mbar_init(bar(B_S_EMPTY), 1);
     for (int b = 0; b < 2; ++b) {
-      mbar_init(bar(B_S_FULL + b), 1);
-      mbar_init(bar(B_S_EMPTY + b), 1);
       mbar_init(bar(B_P_FULL + b), 1);
       mbar_init(bar(B_PV_DONE + b), 1);
       mbar_init(bar(B_DECIDE + b), 1);
@@ -206,20 +213,47 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("prefetch.tensormap [%0];" ::"l"(&kmap) : "memory");
   }
-  if (warp >= 2) {                                     // Q[32 x 576] -> K-major swizzled A operand (zero rows past Hq)
-    for (int x = tid - 64; x < NH * CHUNKS; x += SOFTMAX_THREADS) {
-      const int h = x / CHUNKS, c = x % CHUNKS;
-      uint4 v = make_uint4(0, 0, 0, 0);
-      if (h < num_q_heads) v = *reinterpret_cast<const uint4*>(q + ((int64_t)i * num_q_heads + h) * D + c * 8);
-      const uint32_t off = (c >> 3) * Q_ATOM_BYTES + (h >> 3) * 1024 + (h & 7) * 128 + (((c & 7) ^ (h & 7)) << 4);
-      *reinterpret_cast<uint4*>(sm + OFF_Q + off) = v;
-    }
-    fence_async_proxy();
-  }
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = s_tmem;
+  // Q[32 x 576] -> TMEM lanes 0..31 (heads), 288 columns (zero rows past Hq): coalesced through the (still
+  // idle) ring, row pitch padded to 1168 B so that the per-head reads are bank-conflict free
+  constexpr int Q_PITCH = D * 2 + 16;
+  if (warp >= 2) {
+    constexpr int Q_IT = NH * CHUNKS / SOFTMAX_THREADS;          // 18 independent 16-byte loads per thread
+    static_assert(NH * CHUNKS % SOFTMAX_THREADS == 0, "Q staging");
+    uint4 qv[Q_IT];
+#pragma unroll
+    for (int k = 0; k < Q_IT; ++k) {
+      const int x = tid - 64 + k * SOFTMAX_THREADS, h = x / CHUNKS, c = x % CHUNKS;
+      qv[k] = h < num_q_heads ? *reinterpret_cast<const uint4*>(q + ((int64_t)i * num_q_heads + h) * D + c * 8)
+                              : make_uint4(0, 0, 0, 0);
+    }
+#pragma unroll
+    for (int k = 0; k < Q_IT; ++k) {
+      const int x = tid - 64 + k * SOFTMAX_THREADS, h = x / CHUNKS, c = x % CHUNKS;
+      *reinterpret_cast<uint4*>(sm + OFF_PAIR + h * Q_PITCH + c * 16) = qv[k];
+    }
+    softmax_barrier();
+    if (warp == SOFTMAX_WARP) {
+      const uint4* qrow = reinterpret_cast<const uint4*>(sm + OFF_PAIR + lane * Q_PITCH);
+#pragma unroll 1
+      for (int c = 0; c < D / 64; ++c) {               // 64 channels = 32 columns at a time
+        float w[32];
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+          const uint4 v = qrow[c * 8 + e];
+          w[4 * e + 0] = __uint_as_float(v.x); w[4 * e + 1] = __uint_as_float(v.y);
+          w[4 * e + 2] = __uint_as_float(v.z); w[4 * e + 3] = __uint_as_float(v.w);
+        }
+        tmem_st32(tmem + TM_Q + 32 * c, w);
+      }
+      tc_fence_before();
+    }
+  }
+  __syncthreads();
+  tc_fence_after();
   pdl_wait();                                          // the selection lists come from the preceding kernel of the step
 
   const int cnt = sel_count[i];
@@ -228,7 +262,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   const int n_pages = r_end - r_begin;
   const int32_t* phys_list = sel_phys + (int64_t)i * max_budget + r_begin;
   const int32_t* log_list = sel_logical + (int64_t)i * max_budget + r_begin;
-  const uint32_t q_base = base + OFF_Q, p_base = base + OFF_P;
+  const uint32_t p_base = base + OFF_P;
 
   if (n_pages == 0) {                                  // empty split: contributes nothing to the merge
     for (int e = tid; e < num_q_heads * DV; e += THREADS) {
@@ -270,12 +304,33 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
     // PV(p) goes out the moment P(p) is ready -- it frees ring slots -- and QK of the following pages is issued
     // box pair by box pair as the tiles land, so the tensor pipe works on S(p+1) while the softmax warp turns
     // S(p) into P(p).
+    // Barrier tests cost ~100+ cycles each; the tests for the NEXT state are issued before this state's MMAs so
+    // that their latency hides behind the (queue-limited) MMA issue.  Flags are monotonic: once true they stay
+    // true until consumed.
     int qk_p = 0, qk_g = 0;                              // next QK page / group in it (0 = RoPE box, 1..4 = box pairs)
     int pv_p = 0;                                        // next PV page
+    auto test_pv = [&](int pv, int qk) -> bool {
+      return pv < qk && pv < n_pages && mbar_test(bar(B_P_FULL + (pv & 1)), (pv >> 1) & 1);
+    };
+    auto test_qk = [&](int qp, int qg) -> bool {
+      if (qp >= n_pages) return false;
+      if (qg == 0) {
+        const int rs = qp % N_ROPE;
+        return (qp < 1 || mbar_test(bar(B_S_EMPTY), (qp - 1) & 1)) &&             // softmax has read S(p-1)
+               mbar_test(bar(B_ROPE_FULL + rs), (qp / N_ROPE) & 1);
+      }
+      const int g = qp * PAIRS_PER_PAGE + qg - 1;
+      return mbar_test(bar(B_PAIR_FULL + g % N_PAIR), (g / N_PAIR) & 1);
+    };
+    bool f_pv = false, f_qk = false;
     while (pv_p < n_pages) {
-      bool pv_ready = pv_p < qk_p && mbar_test(bar(B_P_FULL + (pv_p & 1)), (pv_p >> 1) & 1);
-      pv_ready = __shfl_sync(0xffffffffu, pv_ready, 0);
-      if (pv_ready) {
+      if (!f_pv) f_pv = test_pv(pv_p, qk_p);
+      if (!f_qk) f_qk = test_qk(qk_p, qk_g);
+      const uint32_t fl = __shfl_sync(0xffffffffu, (f_pv ? 1u : 0u) | (f_qk ? 2u : 0u), 0);
+      f_pv = fl & 1u;
+      f_qk = fl & 2u;
+      if (f_pv) {
+        const bool n_pv = test_pv(pv_p + 1, qk_p);       // prefetch the next state's test
         tc_fence_after();                                // P(pv_p) written, O^T rescaled if it had to be
         const int b = pv_p & 1;
         if (elect_one()) {
@@ -294,46 +349,37 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
         }
         __syncwarp();
         ++pv_p;
-        continue;
-      }
-      if (qk_p < n_pages) {
-        const int b = qk_p & 1;
+        f_pv = n_pv;
+      } else if (f_qk) {
+        const int nq_g = qk_g == PAIRS_PER_PAGE ? 0 : qk_g + 1, nq_p = qk_g == PAIRS_PER_PAGE ? qk_p + 1 : qk_p;
+        const bool n_qk = test_qk(nq_p, nq_g);           // prefetch the next state's tests
+        const bool n_pv = test_pv(pv_p, nq_p);
+        tc_fence_after();
         if (qk_g == 0) {
           const int rs = qk_p % N_ROPE;
-          bool ok = (qk_p < 2 || mbar_test(bar(B_S_EMPTY + b), ((qk_p >> 1) - 1) & 1)) &&     // softmax has read S(p-2)
-                    mbar_test(bar(B_ROPE_FULL + rs), (qk_p / N_ROPE) & 1);
-          ok = __shfl_sync(0xffffffffu, ok, 0);
-          if (ok) {
-            tc_fence_after();
-            if (elect_one()) {
-              const uint32_t kb = base + OFF_ROPE + rs * K_ATOM_BYTES, qa = q_base + 8 * Q_ATOM_BYTES;
+          if (elect_one()) {
+            const uint32_t kb = base + OFF_ROPE + rs * K_ATOM_BYTES;
 #pragma unroll
-              for (int ks = 0; ks < 4; ++ks)
-                umma(tmem + b * 64, smem_desc(qa + ks * 32, 16, 1024), smem_desc(kb + ks * 32, 16, 1024), IDESC_QK, ks > 0);
-              umma_commit(bar(B_ROPE_EMPTY + rs));
-            }
-            __syncwarp();
-            qk_g = 1;
+            for (int ks = 0; ks < 4; ++ks)               // channels 512 + 16 ks: Q columns 256 + 8 ks
+              umma_ts(tmem + TM_S, tmem + TM_Q + 256 + 8 * ks, smem_desc(kb + ks * 32, 16, 1024), IDESC_QK, ks > 0);
+            umma_commit(bar(B_ROPE_EMPTY + rs));
           }
         } else {
-          const int j = qk_g - 1, g = qk_p * PAIRS_PER_PAGE + j, ps = g % N_PAIR;
-          bool ok = mbar_test(bar(B_PAIR_FULL + ps), (g / N_PAIR) & 1);
-          ok = __shfl_sync(0xffffffffu, ok, 0);
-          if (ok) {
-            tc_fence_after();
-            if (elect_one()) {
+          const int j = qk_g - 1, ps = (qk_p * PAIRS_PER_PAGE + j) % N_PAIR;
+          if (elect_one()) {
 #pragma unroll
-              for (int ks = 0; ks < 8; ++ks) {
-                const uint32_t kb = base + OFF_PAIR + ps * PAIR_BYTES + (ks >> 2) * K_ATOM_BYTES + (ks & 3) * 32;
-                const uint32_t qa = q_base + (2 * j + (ks >> 2)) * Q_ATOM_BYTES + (ks & 3) * 32;
-                umma(tmem + b * 64, smem_desc(qa, 16, 1024), smem_desc(kb, 16, 1024), IDESC_QK, true);
-              }
-              if (qk_g == PAIRS_PER_PAGE) umma_commit(bar(B_S_FULL + b));
+            for (int ks = 0; ks < 8; ++ks) {
+              const uint32_t kb = base + OFF_PAIR + ps * PAIR_BYTES + (ks >> 2) * K_ATOM_BYTES + (ks & 3) * 32;
+              umma_ts(tmem + TM_S, tmem + TM_Q + 64 * j + 8 * ks, smem_desc(kb, 16, 1024), IDESC_QK, true);
             }
-            __syncwarp();
-            if (++qk_g > PAIRS_PER_PAGE) { qk_g = 0; ++qk_p; }
+            if (qk_g == PAIRS_PER_PAGE) umma_commit(bar(B_S_FULL));
           }
         }
+        __syncwarp();
+        qk_g = nq_g;
+        qk_p = nq_p;
+        f_qk = n_qk;
+        f_pv = n_pv;
       }
     }
     pdl_trigger();
@@ -350,14 +396,14 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
         const int b = p & 1;
         const int valid = min(PAGE, n_tok - lg * PAGE);
         if (p + 1 < n_pages) lg = log_list[p + 1];       // prefetch for the next page
-        mbar_wait(bar(B_S_FULL + b), (p >> 1) & 1);
+        mbar_wait(bar(B_S_FULL), p & 1);
         tc_fence_after();
         float s[PAGE];
-        tmem_ld32(t_lane + b * 64, *reinterpret_cast<float(*)[32]>(&s[0]));
-        tmem_ld32(t_lane + b * 64 + 32, *reinterpret_cast<float(*)[32]>(&s[32]));
+        tmem_ld32(t_lane + TM_S, *reinterpret_cast<float(*)[32]>(&s[0]));
+        tmem_ld32(t_lane + TM_S + 32, *reinterpret_cast<float(*)[32]>(&s[32]));
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar(B_S_EMPTY + b));  // S buffer b may be overwritten by QK(p+2)
+        if (lane == 0) mbar_arrive(bar(B_S_EMPTY));      // S may be overwritten by QK(p+1)
         float tmax = -INFINITY;
 #pragma unroll
         for (int t = 0; t < PAGE; ++t) {
@@ -420,6 +466,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       }
       s_l[lane] = l_sum;
       s_m[lane] = m_ref;
+      s_inv[lane] = 1.f / l_sum;
     } else {
       // helper warps: follow the softmax warp's decisions; rescale their TMEM lanes of O^T when asked (rare)
       for (int p = 0; p < n_pages; ++p) {
@@ -446,7 +493,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       const int hidx = (warp == 5 ? 2 : warp - 2) * kWarp + lane;      // 0..95
       const int lg_last = log_list[pl];
       if (summary_upd != nullptr && lg_last == newest_page && hidx < CHUNKS) {
-        mbar_wait(bar(B_S_FULL + (pl & 1)), (pl >> 1) & 1);            // QK(last) done: every box of the page has landed
+        mbar_wait(bar(B_S_FULL), pl & 1);                              // QK(last) done: every box of the page has landed
         const int valid = min(PAGE, n_tok - lg_last * PAGE);
         const int cc = hidx, a = cc >> 3;
         const uint8_t* atom = a < 8 ? sm + OFF_PAIR + ((pl * PAIRS_PER_PAGE + (a >> 1)) % N_PAIR) * PAIR_BYTES + (a & 1) * K_ATOM_BYTES
@@ -477,7 +524,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
 #pragma unroll
       for (int j = 0; j < NH; ++j) {
         if (j < num_q_heads) {
-          const float val = o[j] / s_l[j];
+          const float val = o[j] * s_inv[j];
           const int64_t orow = (int64_t)i * num_q_heads + j;
           if (num_splits == 1) out[orow * DV + d] = __float2bfloat16_rn(val);
           else part_o[(orow * num_splits + split) * DV + d] = val;
