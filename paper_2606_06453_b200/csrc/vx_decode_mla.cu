@@ -168,6 +168,56 @@ constexpr int B_PAIR_FULL = 0, B_PAIR_EMPTY = N_PAIR, B_ROPE_FULL = 2 * N_PAIR, 
               B_PV_DONE = B_P_FULL + 2, B_DECIDE = B_PV_DONE + 2, B_ACK = B_DECIDE + 2, N_BARS = B_ACK + 2;
 }  // namespace mla
 
+// (a5) LSE merge of the splits of request i, run by the last split CTA to arrive.
+// Partials are [request][split][channel][head] fp32; the merged tile is transposed through shared memory so that
+// the bf16 output rows [head][channel] are written with coalesced 16-byte stores.
+__device__ __forceinline__ void merge_splits(const float* part_o, const float* part_lse, int i, int num_q_heads,
+                                             int n_part, __nv_bfloat16* out, float* lse, uint8_t* scratch) {
+  using namespace mla;
+  constexpr int PITCH = DV * 2 + 16;                    // bf16 row pitch of the staged tile (bank spread)
+  float* s_w = reinterpret_cast<float*>(scratch);       // [n_part][NH] split weights
+  uint8_t* tile = scratch + kMaxSplits * NH * 4;
+  const int64_t row0 = (int64_t)i * num_q_heads;
+  for (int e = threadIdx.x; e < num_q_heads * n_part; e += blockDim.x)      // all lse values in one round trip
+    s_w[(e % n_part) * NH + e / n_part] = ldcg_f32(part_lse + row0 * n_part + e);
+  __syncthreads();
+  if (threadIdx.x < NH) {
+    const int j = threadIdx.x;
+    if (j < num_q_heads) {
+      float mx = -INFINITY;
+      for (int s = 0; s < n_part; ++s) mx = fmaxf(mx, s_w[s * NH + j]);
+      float z = 0.f;
+      for (int s = 0; s < n_part; ++s) z += mx == -INFINITY ? 0.f : __expf(s_w[s * NH + j] - mx);
+      const float inv = z > 0.f ? 1.f / z : 0.f;
+      for (int s = 0; s < n_part; ++s) s_w[s * NH + j] = mx == -INFINITY ? 0.f : __expf(s_w[s * NH + j] - mx) * inv;
+      if (lse != nullptr) lse[row0 + j] = z > 0.f ? mx + logf(z) : -INFINITY;
+    } else {
+      for (int s = 0; s < n_part; ++s) s_w[s * NH + j] = 0.f;
+    }
+  }
+  __syncthreads();
+  const float* src0 = part_o + (int64_t)i * n_part * DV * NH;
+#pragma unroll 4
+  for (int e = threadIdx.x; e < DV * (NH / 4); e += blockDim.x) {            // e -> (channel d, heads j4 .. j4+3)
+    const int d = e / (NH / 4), j4 = (e % (NH / 4)) * 4;
+    float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int s = 0; s < n_part; ++s) {
+      const float4 w = *reinterpret_cast<const float4*>(s_w + s * NH + j4);
+      const float4 v = ldcg_f32x4(src0 + ((int64_t)s * DV + d) * NH + j4);
+      o.x = fmaf(w.x, v.x, o.x); o.y = fmaf(w.y, v.y, o.y); o.z = fmaf(w.z, v.z, o.z); o.w = fmaf(w.w, v.w, o.w);
+    }
+    *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 0) * PITCH + d * 2) = __float2bfloat16_rn(o.x);
+    *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 1) * PITCH + d * 2) = __float2bfloat16_rn(o.y);
+    *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 2) * PITCH + d * 2) = __float2bfloat16_rn(o.z);
+    *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 3) * PITCH + d * 2) = __float2bfloat16_rn(o.w);
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < num_q_heads * (DV / 8); e += blockDim.x) {   // 16 bytes per thread, rows contiguous
+    const int j = e / (DV / 8), c = e % (DV / 8);
+    *reinterpret_cast<uint4*>(out + (row0 + j) * DV + c * 8) = *reinterpret_cast<const uint4*>(tile + j * PITCH + c * 16);
+  }
+}
+
 __global__ void __launch_bounds__(mla::THREADS, 1)
 decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16* __restrict__ q, int num_q_heads,
                   float scale_log2, const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ sel_phys,
@@ -265,11 +315,10 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   const uint32_t p_base = base + OFF_P;
 
   if (n_pages == 0) {                                  // empty split: contributes nothing to the merge
-    for (int e = tid; e < num_q_heads * DV; e += THREADS) {
+    for (int e = tid; e < NH * DV; e += THREADS) {       // partial layout: [request][split][channel][head]
       const int h = e / DV, d = e % DV;
-      const int64_t row = (int64_t)i * num_q_heads + h;
-      if (num_splits == 1) out[row * DV + d] = __float2bfloat16_rn(0.f);
-      else part_o[(row * num_splits + split) * DV + d] = 0.f;
+      if (num_splits > 1) part_o[(((int64_t)i * num_splits + split) * DV + d) * NH + h] = 0.f;
+      else if (h < num_q_heads) out[((int64_t)i * num_q_heads + h) * DV + d] = __float2bfloat16_rn(0.f);
     }
     if (tid < num_q_heads) {
       const int64_t row = (int64_t)i * num_q_heads + tid;
@@ -521,14 +570,16 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       float o[NH];
       tmem_ld32(t_lane + TM_O + 32 * mb, o);
       const int d = mb * 128 + sp * 32 + lane;
+      if (num_splits > 1) {                              // partial [request][split][channel][head]: 128 contiguous bytes per thread
+        float4* dst = reinterpret_cast<float4*>(part_o + (((int64_t)i * num_splits + split) * DV + d) * NH);
 #pragma unroll
-      for (int j = 0; j < NH; ++j) {
-        if (j < num_q_heads) {
-          const float val = o[j] * s_inv[j];
-          const int64_t orow = (int64_t)i * num_q_heads + j;
-          if (num_splits == 1) out[orow * DV + d] = __float2bfloat16_rn(val);
-          else part_o[(orow * num_splits + split) * DV + d] = val;
-        }
+        for (int j4 = 0; j4 < NH / 4; ++j4)
+          dst[j4] = make_float4(o[4 * j4] * s_inv[4 * j4], o[4 * j4 + 1] * s_inv[4 * j4 + 1],
+                                o[4 * j4 + 2] * s_inv[4 * j4 + 2], o[4 * j4 + 3] * s_inv[4 * j4 + 3]);
+      } else {
+#pragma unroll
+        for (int j = 0; j < NH; ++j)
+          if (j < num_q_heads) out[((int64_t)i * num_q_heads + j) * DV + d] = __float2bfloat16_rn(o[j] * s_inv[j]);
       }
     }
     if (warp == SOFTMAX_WARP && lane < num_q_heads) {
@@ -543,8 +594,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   tc_fence_before();
   if (num_splits > 1) {
     if (last_split_arrives(unit_counter + i, num_splits, &s_last))
-      merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads, num_q_heads, num_splits, DV, out, lse_out,
-                                    reinterpret_cast<float*>(sm + OFF_PAIR));
+      merge_splits(part_o, part_lse, i, num_q_heads, num_splits, out, lse_out, sm + OFF_PAIR);
   }
   __syncthreads();
   if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
@@ -595,7 +645,7 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
   // one CTA per SM (221 KB of shared memory): whole waves of equal CTAs,
   // cost(sp) = waves x (pages per CTA + ~2 pages of pipeline fill and epilogue)
   int best = 1, best_cost = 1 << 30;
-  for (int sp = 1; sp <= kMaxSplits && sp <= max_budget; ++sp) {
+  for (int sp = 1; sp <= kMaxSplits && sp <= max_budget && sp <= g.num_q_heads; ++sp) {   // partial buffer: splits <= Hq
     const int waves = (pt.batch * sp + c->num_sms - 1) / c->num_sms;
     const int cost = waves * ((max_budget + sp - 1) / sp + 2);
     if (cost < best_cost) { best_cost = cost; best = sp; }
