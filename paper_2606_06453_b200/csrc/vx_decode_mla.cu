@@ -197,19 +197,42 @@ __device__ __forceinline__ void merge_splits(const float* part_o, const float* p
   }
   __syncthreads();
   const float* src0 = part_o + (int64_t)i * n_part * DV * NH;
-#pragma unroll 4
-  for (int e = threadIdx.x; e < DV * (NH / 4); e += blockDim.x) {            // e -> (channel d, heads j4 .. j4+3)
+  constexpr int N_E = DV * (NH / 4), UNR = 8;           // e -> (channel d, heads j4 .. j4+3); UNR x n_part loads in flight
+  auto put = [&](int e, float4 o) {
     const int d = e / (NH / 4), j4 = (e % (NH / 4)) * 4;
-    float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int s = 0; s < n_part; ++s) {
-      const float4 w = *reinterpret_cast<const float4*>(s_w + s * NH + j4);
-      const float4 v = ldcg_f32x4(src0 + ((int64_t)s * DV + d) * NH + j4);
-      o.x = fmaf(w.x, v.x, o.x); o.y = fmaf(w.y, v.y, o.y); o.z = fmaf(w.z, v.z, o.z); o.w = fmaf(w.w, v.w, o.w);
-    }
     *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 0) * PITCH + d * 2) = __float2bfloat16_rn(o.x);
     *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 1) * PITCH + d * 2) = __float2bfloat16_rn(o.y);
     *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 2) * PITCH + d * 2) = __float2bfloat16_rn(o.z);
     *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 3) * PITCH + d * 2) = __float2bfloat16_rn(o.w);
+  };
+  for (int e0 = threadIdx.x; e0 < N_E; e0 += UNR * blockDim.x) {
+    float4 acc[UNR];
+#pragma unroll
+    for (int k = 0; k < UNR; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int s0 = 0; s0 < n_part; s0 += 2) {            // two splits at a time: 2 * UNR independent 16-byte L2 reads
+      const bool two = s0 + 1 < n_part;
+      float4 va[UNR], vb[UNR];
+#pragma unroll
+      for (int k = 0; k < UNR; ++k) {
+        const int e = e0 + k * blockDim.x;
+        const bool ok = e < N_E;
+        va[k] = ok ? ldcg_f32x4(src0 + (int64_t)s0 * DV * NH + e * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+        vb[k] = ok && two ? ldcg_f32x4(src0 + (int64_t)(s0 + 1) * DV * NH + e * 4) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int k = 0; k < UNR; ++k) {
+        const int j4 = ((e0 + k * blockDim.x) % (NH / 4)) * 4;
+        const float4 wa = *reinterpret_cast<const float4*>(s_w + s0 * NH + j4);
+        const float4 wb = two ? *reinterpret_cast<const float4*>(s_w + (s0 + 1) * NH + j4) : make_float4(0.f, 0.f, 0.f, 0.f);
+        acc[k].x += wa.x * va[k].x + wb.x * vb[k].x;
+        acc[k].y += wa.y * va[k].y + wb.y * vb[k].y;
+        acc[k].z += wa.z * va[k].z + wb.z * vb[k].z;
+        acc[k].w += wa.w * va[k].w + wb.w * vb[k].w;
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < UNR; ++k)
+      if (e0 + k * blockDim.x < N_E) put(e0 + k * blockDim.x, acc[k]);
   }
   __syncthreads();
   for (int e = threadIdx.x; e < num_q_heads * (DV / 8); e += blockDim.x) {   // 16 bytes per thread, rows contiguous
