@@ -38,7 +38,9 @@ namespace vx {
 
 namespace mla {
 constexpr int D = 576, DV = 512, PAGE = 64, NH = 32;      // geometry this kernel is built for
-constexpr int THREADS = 192;                              // producer warp, MMA warp, 4 epilogue warps (one = softmax)
+constexpr int THREADS = 224;                              // TMA producer, QK issuer, 4 epilogue warps (one = softmax), PV issuer
+constexpr int PV_WARP = 6;
+constexpr int PAGE_BYTES = PAGE * D * 2;                  // 73728
 constexpr int SOFTMAX_THREADS = 128;
 constexpr int SOFTMAX_WARP = 4;                           // warp % 4 == 0: TMEM lanes 0..31
 constexpr int CHUNKS = D * 2 / 16;                        // 72 16-byte chunks per token row
@@ -163,7 +165,7 @@ __device__ __forceinline__ float ex2_approx(float x) {
 __device__ __forceinline__ void softmax_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(SOFTMAX_THREADS) : "memory"); }
 
 // barrier indices
-constexpr int B_PAIR_FULL = 0, B_PAIR_EMPTY = N_PAIR, B_ROPE_FULL = 2 * N_PAIR, B_ROPE_EMPTY = B_ROPE_FULL + N_ROPE,
+constexpr int B_PAGE_FULL = 0, B_PAIR_EMPTY = N_ROPE, B_ROPE_EMPTY = B_PAIR_EMPTY + N_PAIR,
               B_S_FULL = B_ROPE_EMPTY + N_ROPE, B_S_EMPTY = B_S_FULL + 1, B_P_FULL = B_S_EMPTY + 1,
               B_PV_DONE = B_P_FULL + 2, B_DECIDE = B_PV_DONE + 2, B_ACK = B_DECIDE + 2, N_BARS = B_ACK + 2;
 }  // namespace mla
@@ -273,8 +275,8 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
   if (tid == 0) {
-    for (int s = 0; s < N_PAIR; ++s) { mbar_init(bar(B_PAIR_FULL + s), 1); mbar_init(bar(B_PAIR_EMPTY + s), 1); }
-    for (int s = 0; s < N_ROPE; ++s) { mbar_init(bar(B_ROPE_FULL + s), 1); mbar_init(bar(B_ROPE_EMPTY + s), 1); }
+    for (int s = 0; s < N_PAIR; ++s) mbar_init(bar(B_PAIR_EMPTY + s), 1);
+    for (int s = 0; s < N_ROPE; ++s) { mbar_init(bar(B_PAGE_FULL + s), 1); mbar_init(bar(B_ROPE_EMPTY + s), 1); }
     mbar_init(bar(B_S_FULL), 1);
     mbar_init(bar(B_S_EMPTY), 1);
     for (int b = 0; b < 2; ++b) {
@@ -293,7 +295,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   // Q[32 x 576] -> TMEM lanes 0..31 (heads), 288 columns (zero rows past Hq): coalesced through the (still
   // idle) ring, row pitch padded to 1168 B so that the per-head reads are bank-conflict free
   constexpr int Q_PITCH = D * 2 + 16;
-  if (warp >= 2) {
+  if (warp >= 2 && warp <= 5) {
     constexpr int Q_IT = NH * CHUNKS / SOFTMAX_THREADS;          // 18 independent 16-byte loads per thread
     static_assert(NH * CHUNKS % SOFTMAX_THREADS == 0, "Q staging");
     uint4 qv[Q_IT];
@@ -349,110 +351,74 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       else part_lse[row * num_splits + split] = -INFINITY;
     }
   } else if (warp == 0) {
-    // ===== TMA producer ===================================================================================
+    // ===== TMA producer: page p -> ring page p % 3 (4 pair slots + 1 RoPE slot), one full barrier per page =====
+    static_assert(N_PAIR == N_ROPE * PAIRS_PER_PAGE, "the ring is a whole number of pages");
     int my_phys = 0;
     for (int p = 0; p < n_pages; ++p) {
       if ((p & 31) == 0) my_phys = p + lane < n_pages ? phys_list[p + lane] : 0;
       const int phys = __shfl_sync(0xffffffffu, my_phys, p & 31);
       if (elect_one()) {
-        const int rs = p % N_ROPE, ru = p / N_ROPE;
-        if (ru >= 1) mbar_wait(bar(B_ROPE_EMPTY + rs), (ru - 1) & 1);
-        mbar_expect_tx(bar(B_ROPE_FULL + rs), K_ATOM_BYTES);
-        tma_box(base + OFF_ROPE + rs * K_ATOM_BYTES, &kmap, DV, phys, bar(B_ROPE_FULL + rs));
+        const int rs = p % N_ROPE, u = p / N_ROPE;
+        const uint32_t full = bar(B_PAGE_FULL + rs);
+        if (u >= 1) mbar_wait(bar(B_ROPE_EMPTY + rs), (u - 1) & 1);      // QK(p-3) done (it also observed the last phase)
+        mbar_expect_tx(full, PAGE_BYTES);
+        tma_box(base + OFF_ROPE + rs * K_ATOM_BYTES, &kmap, DV, phys, full);
 #pragma unroll
         for (int j = 0; j < PAIRS_PER_PAGE; ++j) {
-          const int g = p * PAIRS_PER_PAGE + j, ps = g % N_PAIR, u = g / N_PAIR;
-          if (u >= 1) mbar_wait(bar(B_PAIR_EMPTY + ps), (u - 1) & 1);
-          mbar_expect_tx(bar(B_PAIR_FULL + ps), PAIR_BYTES);
+          const int ps = rs * PAIRS_PER_PAGE + j;
+          if (u >= 1) mbar_wait(bar(B_PAIR_EMPTY + ps), (u - 1) & 1);    // PV(p-3) has read this pair
           const uint32_t dst = base + OFF_PAIR + ps * PAIR_BYTES;
-          tma_box(dst, &kmap, 128 * j, phys, bar(B_PAIR_FULL + ps));
-          tma_box(dst + K_ATOM_BYTES, &kmap, 128 * j + 64, phys, bar(B_PAIR_FULL + ps));
+          tma_box(dst, &kmap, 128 * j, phys, full);
+          tma_box(dst + K_ATOM_BYTES, &kmap, 128 * j + 64, phys, full);
         }
       }
       __syncwarp();
     }
   } else if (warp == 1) {
-    // ===== MMA issuer: the whole warp runs the (warp-uniform) polling state machine, one elected lane issues.
-    // PV(p) goes out the moment P(p) is ready -- it frees ring slots -- and QK of the following pages is issued
-    // box pair by box pair as the tiles land, so the tensor pipe works on S(p+1) while the softmax warp turns
-    // S(p) into P(p).
-    // Barrier tests cost ~100+ cycles each; the tests for the NEXT state are issued before this state's MMAs so
-    // that their latency hides behind the (queue-limited) MMA issue.  Flags are monotonic: once true they stay
-    // true until consumed.
-    int qk_p = 0, qk_g = 0;                              // next QK page / group in it (0 = RoPE box, 1..4 = box pairs)
-    int pv_p = 0;                                        // next PV page
-    auto test_pv = [&](int pv, int qk) -> bool {
-      return pv < qk && pv < n_pages && mbar_test(bar(B_P_FULL + (pv & 1)), (pv >> 1) & 1);
-    };
-    auto test_qk = [&](int qp, int qg) -> bool {
-      if (qp >= n_pages) return false;
-      if (qg == 0) {
-        const int rs = qp % N_ROPE;
-        return (qp < 1 || mbar_test(bar(B_S_EMPTY), (qp - 1) & 1)) &&             // softmax has read S(p-1)
-               mbar_test(bar(B_ROPE_FULL + rs), (qp / N_ROPE) & 1);
-      }
-      const int g = qp * PAIRS_PER_PAGE + qg - 1;
-      return mbar_test(bar(B_PAIR_FULL + g % N_PAIR), (g / N_PAIR) & 1);
-    };
-    bool f_pv = false, f_qk = false;
-    while (pv_p < n_pages) {
-      if (!f_pv) f_pv = test_pv(pv_p, qk_p);
-      if (!f_qk) f_qk = test_qk(qk_p, qk_g);
-      const uint32_t fl = __shfl_sync(0xffffffffu, (f_pv ? 1u : 0u) | (f_qk ? 2u : 0u), 0);
-      f_pv = fl & 1u;
-      f_qk = fl & 2u;
-      if (f_pv) {
-        const bool n_pv = test_pv(pv_p + 1, qk_p);       // prefetch the next state's test
-        tc_fence_after();                                // P(pv_p) written, O^T rescaled if it had to be
-        const int b = pv_p & 1;
-        if (elect_one()) {
+    // ===== QK issuer: S(p) = Q . K(p)^T, 36 MMAs back to back once the page has landed and S is free ==========
+    // (barrier waits are blocking and in a fixed order -- polling several mbarriers cost ~150 cycles per test and
+    //  made the issue loop, not the tensor pipe, the bound)
+    for (int p = 0; p < n_pages; ++p) {
+      const int rs = p % N_ROPE;
+      if (p >= 1) mbar_wait(bar(B_S_EMPTY), (p - 1) & 1);                // softmax has read S(p-1)
+      mbar_wait(bar(B_PAGE_FULL + rs), (p / N_ROPE) & 1);
+      tc_fence_after();
+      if (elect_one()) {
 #pragma unroll
-          for (int ks = 0; ks < PAGE / 16; ++ks)         // ks-major: consecutive MMAs go to different O^T blocks
+        for (int j = 0; j < PAIRS_PER_PAGE; ++j)
 #pragma unroll
-            for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) {
-              const int ps = (pv_p * PAIRS_PER_PAGE + mb) % N_PAIR;
-              umma(tmem + TM_O + 32 * mb, smem_desc(base + OFF_PAIR + ps * PAIR_BYTES + ks * 2048, K_ATOM_BYTES, 1024),
-                   smem_desc(p_base + b * P_BYTES + ks * 32, 16, 1024), IDESC_PV, pv_p > 0 || ks > 0);
-            }
-#pragma unroll
-          for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb)    // the pair slots may be refilled
-            umma_commit(bar(B_PAIR_EMPTY + (pv_p * PAIRS_PER_PAGE + mb) % N_PAIR));
-          umma_commit(bar(B_PV_DONE + b));
-        }
-        __syncwarp();
-        ++pv_p;
-        f_pv = n_pv;
-      } else if (f_qk) {
-        const int nq_g = qk_g == PAIRS_PER_PAGE ? 0 : qk_g + 1, nq_p = qk_g == PAIRS_PER_PAGE ? qk_p + 1 : qk_p;
-        const bool n_qk = test_qk(nq_p, nq_g);           // prefetch the next state's tests
-        const bool n_pv = test_pv(pv_p, nq_p);
-        tc_fence_after();
-        if (qk_g == 0) {
-          const int rs = qk_p % N_ROPE;
-          if (elect_one()) {
-            const uint32_t kb = base + OFF_ROPE + rs * K_ATOM_BYTES;
-#pragma unroll
-            for (int ks = 0; ks < 4; ++ks)               // channels 512 + 16 ks: Q columns 256 + 8 ks
-              umma_ts(tmem + TM_S, tmem + TM_Q + 256 + 8 * ks, smem_desc(kb + ks * 32, 16, 1024), IDESC_QK, ks > 0);
-            umma_commit(bar(B_ROPE_EMPTY + rs));
+          for (int ks = 0; ks < 8; ++ks) {
+            const uint32_t kb = base + OFF_PAIR + (rs * PAIRS_PER_PAGE + j) * PAIR_BYTES + (ks >> 2) * K_ATOM_BYTES + (ks & 3) * 32;
+            umma_ts(tmem + TM_S, tmem + TM_Q + 64 * j + 8 * ks, smem_desc(kb, 16, 1024), IDESC_QK, j > 0 || ks > 0);
           }
-        } else {
-          const int j = qk_g - 1, ps = (qk_p * PAIRS_PER_PAGE + j) % N_PAIR;
-          if (elect_one()) {
 #pragma unroll
-            for (int ks = 0; ks < 8; ++ks) {
-              const uint32_t kb = base + OFF_PAIR + ps * PAIR_BYTES + (ks >> 2) * K_ATOM_BYTES + (ks & 3) * 32;
-              umma_ts(tmem + TM_S, tmem + TM_Q + 64 * j + 8 * ks, smem_desc(kb, 16, 1024), IDESC_QK, true);
-            }
-            if (qk_g == PAIRS_PER_PAGE) umma_commit(bar(B_S_FULL));
-          }
-        }
-        __syncwarp();
-        qk_g = nq_g;
-        qk_p = nq_p;
-        f_qk = n_qk;
-        f_pv = n_pv;
+        for (int ks = 0; ks < 4; ++ks)                                   // RoPE channels 512 + 16 ks: Q columns 256 + 8 ks
+          umma_ts(tmem + TM_S, tmem + TM_Q + 256 + 8 * ks, smem_desc(base + OFF_ROPE + rs * K_ATOM_BYTES + ks * 32, 16, 1024),
+                  IDESC_QK, true);
+        umma_commit(bar(B_ROPE_EMPTY + rs));
+        umma_commit(bar(B_S_FULL));
       }
+      __syncwarp();
+    }
+  } else if (warp == PV_WARP) {
+    // ===== PV issuer: O^T += V(p)^T . P(p)^T the moment P(p) is written; frees the page's pair slots ============
+    for (int p = 0; p < n_pages; ++p) {
+      const int b = p & 1, rs = p % N_ROPE;
+      mbar_wait(bar(B_P_FULL + b), (p >> 1) & 1);                        // P(p) written, O^T rescaled if it had to be
+      tc_fence_after();
+      if (elect_one()) {
+#pragma unroll
+        for (int ks = 0; ks < PAGE / 16; ++ks)                           // ks-major: consecutive MMAs go to different O^T blocks
+#pragma unroll
+          for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb)
+            umma(tmem + TM_O + 32 * mb,
+                 smem_desc(base + OFF_PAIR + (rs * PAIRS_PER_PAGE + mb) * PAIR_BYTES + ks * 2048, K_ATOM_BYTES, 1024),
+                 smem_desc(p_base + b * P_BYTES + ks * 32, 16, 1024), IDESC_PV, p > 0 || ks > 0);
+#pragma unroll
+        for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) umma_commit(bar(B_PAIR_EMPTY + rs * PAIRS_PER_PAGE + mb));
+        umma_commit(bar(B_PV_DONE + b));
+      }
+      __syncwarp();
     }
     pdl_trigger();
   } else {
