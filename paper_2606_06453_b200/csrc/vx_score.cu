@@ -22,7 +22,6 @@ namespace vx {
 
 constexpr int kScConsumerWarps = 8;
 constexpr int kScThreads = (kScConsumerWarps + 1) * kWarp;
-constexpr int kScStages = 3;
 
 __device__ __forceinline__ void sc_mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
@@ -68,7 +67,7 @@ struct GroupIter {
   }
 };
 
-template <typename T, int D, int PG, int HKV>
+template <typename T, int D, int PG, int HKV, int kScStages>
 __global__ void __launch_bounds__(kScThreads, 2)
 score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int batch,
              const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices, int total_pages,
@@ -106,17 +105,29 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
 
   if (warp == kScConsumerWarps) {
     // ---- producer: one bulk copy per page (all KV heads of the page are contiguous) ----------
+    // The physical ids of the CTA's flat page range are prefetched 32 at a time (one coalesced load, two chunks
+    // in registers), so that no index load sits between a freed stage and its refill.
+    int chunk0 = begin;                                   // flat index of id_cur's lane 0
+    int id_cur = chunk0 + lane < end ? page_indices[chunk0 + lane] : 0;
+    int id_nxt = chunk0 + kWarp + lane < end ? page_indices[chunk0 + kWarp + lane] : 0;
     for (int g = 0; it.next(PG, first, count, req); ++g) {
       const int s = g % kScStages;
       if (g >= kScStages) sc_mbar_wait(smem_u32(&s_empty[s]), ((g / kScStages) - 1) & 1);
       const uint32_t bar = smem_u32(&s_full[s]);
       if (lane == 0) sc_mbar_expect_tx(bar, (uint32_t)(count * PAGE_BYTES));
       __syncwarp();
-      for (int l = lane; l < count; l += kWarp) {
-        const int64_t phys = page_indices[first + l];
-        bulk_g2s(smem_u32(smem + (size_t)s * STAGE_BYTES + (size_t)l * PAGE_BYTES),
-                 reinterpret_cast<const uint8_t*>(summary) + phys * PAGE_BYTES, (uint32_t)PAGE_BYTES, bar);
+      static_assert(PG <= kWarp, "a group is at most one id chunk long");
+      if (first >= chunk0 + kWarp) {                      // the group starts in the next chunk: rotate, prefetch one more
+        chunk0 += kWarp;
+        id_cur = id_nxt;
+        id_nxt = chunk0 + kWarp + lane < end ? page_indices[chunk0 + kWarp + lane] : 0;
       }
+      const int off = first + lane - chunk0;              // lane l copies page first + l (valid for l < count)
+      const int a = __shfl_sync(0xffffffffu, id_cur, off & 31), b = __shfl_sync(0xffffffffu, id_nxt, off & 31);
+      const int64_t phys = off < kWarp ? a : b;
+      if (lane < count)
+        bulk_g2s(smem_u32(smem + (size_t)s * STAGE_BYTES + (size_t)lane * PAGE_BYTES),
+                 reinterpret_cast<const uint8_t*>(summary) + phys * PAGE_BYTES, (uint32_t)PAGE_BYTES, bar);
     }
     return;
   }
@@ -238,10 +249,13 @@ static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary,
                                   float* scores, cudaStream_t s) {
   const vx_geom& g = c->g;
   constexpr size_t page_bytes = (size_t)HKV * 2 * D * sizeof(T);
-  constexpr size_t smem = kScStages * PG * page_bytes + (size_t)HKV * 2 * D * sizeof(float);
+  // as many ~16-32 KB stages as two CTAs per SM can hold (>= 3): the bytes in flight, not the math, set the rate
+  constexpr size_t q_bytes = (size_t)HKV * 2 * D * sizeof(float);
+  constexpr int kScStages = (int)((110 * 1024 - q_bytes) / (PG * page_bytes)) < 3 ? 3 : ((int)((110 * 1024 - q_bytes) / (PG * page_bytes)) > 8 ? 8 : (int)((110 * 1024 - q_bytes) / (PG * page_bytes)));
+  constexpr size_t smem = kScStages * PG * page_bytes + q_bytes;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(score_kernel<T, D, PG, HKV>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(score_kernel<T, D, PG, HKV, kScStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
@@ -249,7 +263,7 @@ static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary,
   const int min_pages = 2 * PG;                  // do not spread tiny inputs over every SM
   if ((int64_t)ctas * min_pages > pt.total_pages) ctas = (pt.total_pages + min_pages - 1) / min_pages;
   if (ctas < 1) ctas = 1;
-  score_kernel<T, D, PG, HKV><<<ctas, kScThreads, smem, s>>>(
+  score_kernel<T, D, PG, HKV, kScStages><<<ctas, kScThreads, smem, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, pt.batch, pt.page_indptr,
       pt.page_indices, pt.total_pages, scores);
   c->launches += 1;
