@@ -47,13 +47,16 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
 struct GroupIter {
   int flat, end, req, req_end;
   const int32_t* indptr;
+  // Called by a converged warp.  The request holding flat page `begin` = number of indptr[1..batch] entries <= begin
+  // (indptr is sorted): counted with independent strided loads -- one memory latency instead of the log2(batch)
+  // dependent ones of a binary search (cold, that was several microseconds at the head of every CTA).
   __device__ GroupIter(int begin, int end_, int batch, const int32_t* page_indptr) : flat(begin), end(end_), indptr(page_indptr) {
-    int lo = 0, hi = batch;                      // largest req with indptr[req] <= begin
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (page_indptr[mid] <= begin) lo = mid; else hi = mid;
-    }
-    req = lo;
+    const int lane = threadIdx.x % kWarp;
+    int below = 0;
+    for (int r = lane; r < batch; r += kWarp) below += page_indptr[r + 1] <= begin;
+#pragma unroll
+    for (int o = kWarp / 2; o > 0; o >>= 1) below += __shfl_xor_sync(0xffffffffu, below, o);
+    req = min(below, batch - 1);
     req_end = page_indptr[req + 1];
   }
   __device__ bool next(int pg, int& first, int& count, int& request) {
@@ -141,17 +144,33 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     const int s = g % kScStages;
     if (req != cur_req) {                        // new request: rebuild [Qm | Qp] for all KV heads (rare)
       asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
-      for (int e = threadIdx.x; e < HKV * D; e += kScConsumerWarps * kWarp) {
-        const int h = e / D, c = e % D;
-        const T* qrow = q + ((int64_t)req * num_q_heads + h * grp) * D + c;
-        float qp = 0.f, qm = 0.f;
-        for (int r = 0; r < grp; ++r) {
-          const float x = Elem<T>::to_float(qrow[(int64_t)r * D]);
-          qp += fmaxf(x, 0.f);
-          qm += fminf(x, 0.f);
+      // one thread per (KV head, 16-byte channel vector); the group's heads are read 8 at a time with all
+      // loads of a batch in flight together (a head-by-head loop costs one memory latency per head)
+      constexpr int NV = D / PER;
+      for (int e = threadIdx.x; e < HKV * NV; e += kScConsumerWarps * kWarp) {
+        const int h = e / NV, c = e % NV;
+        const T* qbase = q + ((int64_t)req * num_q_heads + h * grp) * D + c * PER;
+        float qp[PER], qm[PER];
+#pragma unroll
+        for (int k = 0; k < PER; ++k) { qp[k] = 0.f; qm[k] = 0.f; }
+        for (int r0 = 0; r0 < grp; r0 += 8) {
+          uint4 v[8];
+#pragma unroll
+          for (int k = 0; k < 8; ++k)
+            v[k] = r0 + k < grp ? *reinterpret_cast<const uint4*>(qbase + (int64_t)(r0 + k) * D) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+          for (int k = 0; k < 8; ++k) {                  // zeros add nothing: heads past the group need no branch
+            float f[PER];
+            Elem<T>::unpack(v[k], f);
+#pragma unroll
+            for (int x = 0; x < PER; ++x) { qp[x] += fmaxf(f[x], 0.f); qm[x] += fminf(f[x], 0.f); }
+          }
         }
-        s_q[h * ROW_ELEMS + c] = qm;
-        s_q[h * ROW_ELEMS + D + c] = qp;
+#pragma unroll
+        for (int x = 0; x < PER; ++x) {
+          s_q[h * ROW_ELEMS + c * PER + x] = qm[x];
+          s_q[h * ROW_ELEMS + D + c * PER + x] = qp[x];
+        }
       }
       asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
       cur_req = req;
