@@ -194,6 +194,7 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
     eq += (w < warp) ? c.y : 0;
   }
   const unsigned lt_mask = (1u << lane) - 1u;
+  const bool staged = n_sel <= kBins;           // the histogram is free now: stage the selected logical ids in it
   for (int base = j_begin; base < j_end; base += kWarp) {
     const int j = base + lane;
     const uint32_t key = j < j_end ? key_at(j) : 0u;
@@ -204,11 +205,22 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
     const bool take = sure || (tie && my_eq < need_eq);
     const int pos = my_gt + min(my_eq, need_eq);
     if (take && pos < n_sel) {
-      sel_phys[out0 + pos] = page_indices[row0 + j];
-      if (sel_logical) sel_logical[out0 + pos] = j;
+      if (staged) s_hist[pos] = j;                // logical ids first; the page-table gather runs as one parallel pass
+      else {
+        sel_phys[out0 + pos] = page_indices[row0 + j];
+        if (sel_logical) sel_logical[out0 + pos] = j;
+      }
     }
     gt += __popc(b_sure);
     eq += __popc(b_tie);
+  }
+  if (staged) {                                   // every selected page: one independent gather + two stores
+    __syncthreads();
+    for (int r = tid; r < n_sel; r += THREADS) {
+      const int j = s_hist[r];
+      sel_phys[out0 + r] = page_indices[row0 + j];
+      if (sel_logical) sel_logical[out0 + r] = j;
+    }
   }
   for (int r = n_sel + tid; r < max_budget; r += THREADS) {
     sel_phys[out0 + r] = -1;
