@@ -55,6 +55,20 @@ def measured_peak():
     return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def ncu_traffic(cfg, stage):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
+    `ncu --set full` capture (profiles/r1b_traffic.csv; commands in profiles/r1b_steps.md), or None."""
+    kernel = {"page_score": ("score_kernel",), "sparse_paged_decode": ("decode_gqa_mma_kernel", "decode_mla_kernel")}[stage]
+    path = os.path.join(ROOT, "profiles", "r1b_traffic.csv")
+    if not os.path.exists(path):
+        return None
+    import csv
+    for row in csv.DictReader(open(path)):
+        if row["config"] == cfg and row["kernel"] in kernel:
+            return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
+    return None
+
+
 def algorithmic_bytes(w, sel_count=None):
     """Bytes roofline of one step: every summary row once, every selected
     page's K and V tokens once, Q in and O out.  Page table / scores / partials are not counted."""
@@ -323,7 +337,7 @@ def main():
         dom = max(stage_bytes, key=lambda k: stage[k])
         achieved = stage_bytes[dom] / (stage[dom] * 1e-6) / 1e9
         roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                    "frac": achieved / peak, "traffic": ncu_traffic(args.config, dom), "peak_source": peak_src,
                     "algorithmic_bytes": stage_bytes[dom], "us": stage[dom]}
         step_gbs = bytes_["total"] / (ms * 1e-3) / 1e9
         cpu = None
