@@ -15,6 +15,8 @@
 // then resolves ties to the lowest logical index and writes ids in ascending logical order (so the
 // partial last page comes last) together with the physical page ids.
 // Integer work on a few KB per problem -- latency-bound, not bandwidth-bound.
+#include <cstdlib>
+
 #include "vx_common.cuh"
 #include "vx_internal.h"
 
@@ -254,9 +256,13 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
                               int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl) {
   if (pt.batch == 0) return cudaSuccess;
-  // block size by problem size: ~4-8 candidates per thread
-  if (pt.max_pages_per_req <= 1024) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
-  if (pt.max_pages_per_req <= 4096) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
+  // block size by problem size (VX_TOPK_THREADS overrides, for tuning)
+  static int force = -1;
+  if (force < 0) { const char* e = getenv("VX_TOPK_THREADS"); force = e ? atoi(e) : 0; }
+  const int n = pt.max_pages_per_req;
+  const int th = force ? force : (n <= 1024 ? 256 : n <= 4096 ? 512 : 1024);
+  if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
+  if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
   return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
 }
 
