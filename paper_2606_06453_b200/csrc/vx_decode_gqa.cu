@@ -59,7 +59,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
                       const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count,
                       int max_budget, int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                       int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd,
-                      __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out) {
+                      __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0) {
   constexpr int ROWB = D * 2;                 // bytes per token row
   constexpr int CH = ROWB / 16;               // 16-byte chunks per row
   constexpr int PAGEB = kGqaPage * ROWB;      // bytes of one K (or V) page chunk
@@ -71,7 +71,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   __shared__ int s_phys[kGqaWarps][kGqaStages];    // its physical id
   __shared__ int s_last;
 
-  const int split = blockIdx.x, kvh = blockIdx.y, i = blockIdx.z;
+  const int split = blockIdx.x, kvh = blockIdx.y, i = blockIdx.z + req0;
   const int warp = threadIdx.x / kWarp, lane = threadIdx.x % kWarp;
   const int grp = num_q_heads / num_kv_heads;
   const int n_tok = seq_lens[i];
@@ -307,7 +307,8 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
     attr_set = true;
   }
   // splits: whole waves of equal CTAs.  cost(sp) = waves x (pages per warp + ~3 pages of pipeline fill)
-  const int units = pt.batch * g.num_kv_heads;
+  const int n_req = opt.rr.count < 0 ? pt.batch : opt.rr.count;
+  const int units = n_req * g.num_kv_heads;
   const int slots = c->num_sms * 2;              // 96 KB of shared memory per CTA -> 2 CTAs per SM
   int splits = 1, best_cost = 1 << 30;
   for (int sp = 1; sp <= kMaxSplits && sp <= max_budget; ++sp) {
@@ -315,13 +316,13 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
     const int cost = waves * (((max_budget + sp - 1) / sp + kGqaWarps - 1) / kGqaWarps + 3);
     if (cost < best_cost) { best_cost = cost; splits = sp; }
   }
-  dim3 grid(splits, g.num_kv_heads, pt.batch);
+  dim3 grid(splits, g.num_kv_heads, n_req);
   cudaError_t e = launch_kernel(decode_gqa_mma_kernel<D>, grid, dim3(kGqaWarps * kWarp), (size_t)smem, s, opt.pdl,
       static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(pool.k),
       static_cast<const __nv_bfloat16*>(pool.v), pool.stride_page, pool.stride_token, pool.stride_head,
       g.num_q_heads, g.num_kv_heads, g.sm_scale * kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget,
       splits, c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd),
-      static_cast<__nv_bfloat16*>(out), lse);
+      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

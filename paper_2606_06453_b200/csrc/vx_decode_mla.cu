@@ -249,7 +249,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
                   const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count, int max_budget,
                   int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                   int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd,
-                  __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out) {
+                  __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0) {
   using namespace mla;
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t s_bar[N_BARS];
@@ -259,7 +259,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   __shared__ float s_l[NH], s_m[NH], s_inv[NH];        // final denominators / references
   __shared__ int s_last;
 
-  const int split = blockIdx.x, i = blockIdx.z;
+  const int split = blockIdx.x, i = blockIdx.z + req0;
   const int tid = threadIdx.x, warp = tid / kWarp, lane = tid % kWarp;
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;        // swizzle atoms need 1024-byte alignment
@@ -633,18 +633,19 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
   if (cudaError_t e = make_latent_map(&kmap, pool)) return e;
   // one CTA per SM (221 KB of shared memory): whole waves of equal CTAs,
   // cost(sp) = waves x (pages per CTA + ~2 pages of pipeline fill and epilogue)
+  const int n_req = opt.rr.count < 0 ? pt.batch : opt.rr.count;
   int best = 1, best_cost = 1 << 30;
   for (int sp = 1; sp <= kMaxSplits && sp <= max_budget && sp <= g.num_q_heads; ++sp) {   // partial buffer: splits <= Hq
-    const int waves = (pt.batch * sp + c->num_sms - 1) / c->num_sms;
+    const int waves = (n_req * sp + c->num_sms - 1) / c->num_sms;
     const int cost = waves * ((max_budget + sp - 1) / sp + 2);
     if (cost < best_cost) { best_cost = cost; best = sp; }
   }
-  dim3 grid(best, 1, pt.batch);
+  dim3 grid(best, 1, n_req);
   cudaError_t e = launch_kernel(decode_mla_kernel, grid, dim3(mla::THREADS), (size_t)mla::SMEM_BYTES, s, opt.pdl, kmap,
                                 static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens,
                                 sel_phys, sel_logical, sel_count, max_budget, best, c->ws.part_o, c->ws.part_lse,
                                 c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd),
-                                static_cast<__nv_bfloat16*>(out), lse);
+                                static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

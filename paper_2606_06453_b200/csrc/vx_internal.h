@@ -43,6 +43,9 @@ struct vx_ctx {
   int32_t launches;              // kernels enqueued by the last compute call
   bool force_generic;            // VX_FORCE_GENERIC=1 in the environment: CUDA-core decode path only (debug)
   bool use_pdl;                  // chain the kernels of a step with programmatic dependent launch (VX_NO_PDL=1: off)
+  int chains;                    // request windows run as concurrent kernel chains inside a fused step (VX_CHAINS, 1 or 2)
+  cudaStream_t aux_stream;       // second chain's stream; fork / join with the caller's stream by events
+  cudaEvent_t ev_fork, ev_join;
   char err[512];
 };
 
@@ -66,8 +69,17 @@ inline cudaError_t launch_kernel(void (*kernel)(KArgs...), dim3 grid, dim3 block
   return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+// a window of requests [begin, begin + count) of the page table; count < 0 = the whole batch.  The fused step runs
+// two such windows as independent kernel chains on two streams so that one chain's start-up and tail latencies
+// (index chains, first-stage latency, selection phases, split merge) overlap the other chain's streaming.
+struct ReqRange {
+  int begin = 0;
+  int count = -1;
+};
+
 // how a decode launch is embedded in a step
 struct DecodeOpts {
+  ReqRange rr;
   void* summary_upd = nullptr;   // non-null: also rebuild the summary of each request's newest page (a1), whose
                                  // keys the kernel stages anyway (it is a forced local page)
   bool pdl = false;              // launched as a programmatic dependent of the preceding kernel
@@ -77,10 +89,11 @@ struct DecodeOpts {
 cudaError_t launch_summary_update(vx_ctx* c, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* first_new_pos, void* summary, cudaStream_t s);
 cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
-                              float* scores, cudaStream_t s);
+                              float* scores, cudaStream_t s, const ReqRange& rr = ReqRange());
 cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
-                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl = false);
+                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl = false,
+                              const ReqRange& rr = ReqRange());
 cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,

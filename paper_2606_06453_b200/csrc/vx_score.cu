@@ -74,7 +74,7 @@ template <typename T, int D, int PG, int HKV, int kScStages>
 __global__ void __launch_bounds__(kScThreads, 2)
 score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int batch,
              const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices, int total_pages,
-             float* __restrict__ scores) {
+             float* __restrict__ scores, int req_begin, int req_end) {
   constexpr int PER = Elem<T>::kPerVec;
   constexpr int ROW_ELEMS = 2 * D;               // [min | max] of one (page, KV head)
   constexpr int NCH = ROW_ELEMS / PER;           // 16-byte chunks per row
@@ -91,8 +91,9 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   float* s_q = reinterpret_cast<float*>(smem + (size_t)kScStages * STAGE_BYTES);   // [HKV][2*D]: Qm | Qp
 
   const int warp = threadIdx.x / kWarp, lane = threadIdx.x % kWarp;
-  const int begin = (int)((int64_t)total_pages * blockIdx.x / gridDim.x);
-  const int end = (int)((int64_t)total_pages * (blockIdx.x + 1) / gridDim.x);
+  const int flat_lo = page_indptr[req_begin], flat_span = page_indptr[req_end] - flat_lo;   // this launch's request window
+  const int begin = flat_lo + (int)((int64_t)flat_span * blockIdx.x / gridDim.x);
+  const int end = flat_lo + (int)((int64_t)flat_span * (blockIdx.x + 1) / gridDim.x);
   if (threadIdx.x == 0) {
     for (int s = 0; s < kScStages; ++s) {
       sc_mbar_init(smem_u32(&s_full[s]), 1);
@@ -265,7 +266,7 @@ bool score_geometry_supported(const vx_geom& g) {
 
 template <typename T, int D, int PG, int HKV>
 static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
-                                  float* scores, cudaStream_t s) {
+                                  float* scores, cudaStream_t s, const ReqRange& rr) {
   const vx_geom& g = c->g;
   constexpr size_t page_bytes = (size_t)HKV * 2 * D * sizeof(T);
   // as many ~16-32 KB stages as two CTAs per SM can hold (>= 3): the bytes in flight, not the math, set the rate
@@ -280,11 +281,12 @@ static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary,
   }
   int ctas = c->num_sms * 2;                     // two CTAs per SM (3 x ~32 KB stages each)
   const int min_pages = 2 * PG;                  // do not spread tiny inputs over every SM
-  if ((int64_t)ctas * min_pages > pt.total_pages) ctas = (pt.total_pages + min_pages - 1) / min_pages;
+  const int64_t est_pages = rr.count < 0 ? pt.total_pages : (int64_t)pt.total_pages * rr.count / (pt.batch > 0 ? pt.batch : 1) + 1;
+  if ((int64_t)ctas * min_pages > est_pages) ctas = (int)((est_pages + min_pages - 1) / min_pages);
   if (ctas < 1) ctas = 1;
   score_kernel<T, D, PG, HKV, kScStages><<<ctas, kScThreads, smem, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, pt.batch, pt.page_indptr,
-      pt.page_indices, pt.total_pages, scores);
+      pt.page_indices, pt.total_pages, scores, rr.begin, rr.begin + (rr.count < 0 ? pt.batch : rr.count));
   c->launches += 1;
   return cudaGetLastError();
 }
@@ -292,33 +294,33 @@ static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary,
 // PG pages per stage so that a stage is ~32 KB and every consumer warp gets 1..8 rows of it
 template <typename T, int D>
 static cudaError_t launch_score_d(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
-                                  float* scores, cudaStream_t s) {
+                                  float* scores, cudaStream_t s, const ReqRange& rr) {
   constexpr int row_bytes = 2 * D * (int)sizeof(T);
   constexpr int pg8 = 32768 / (8 * row_bytes) < 1 ? 1 : 32768 / (8 * row_bytes);   // Hkv = 8
   switch (c->g.num_kv_heads) {
-    case 8: return launch_score_t<T, D, (pg8 > 8 ? 8 : pg8), 8>(c, q, summary, pt, scores, s);
-    case 4: return launch_score_t<T, D, (2 * pg8 > 16 ? 16 : 2 * pg8), 4>(c, q, summary, pt, scores, s);
-    case 2: return launch_score_t<T, D, (4 * pg8 > 32 ? 32 : (4 * pg8 < 4 ? 4 : 4 * pg8)), 2>(c, q, summary, pt, scores, s);
-    case 1: return launch_score_t<T, D, (8 * pg8 > 32 ? 32 : (8 * pg8 < 8 ? 8 : 8 * pg8)), 1>(c, q, summary, pt, scores, s);
+    case 8: return launch_score_t<T, D, (pg8 > 8 ? 8 : pg8), 8>(c, q, summary, pt, scores, s, rr);
+    case 4: return launch_score_t<T, D, (2 * pg8 > 16 ? 16 : 2 * pg8), 4>(c, q, summary, pt, scores, s, rr);
+    case 2: return launch_score_t<T, D, (4 * pg8 > 32 ? 32 : (4 * pg8 < 4 ? 4 : 4 * pg8)), 2>(c, q, summary, pt, scores, s, rr);
+    case 1: return launch_score_t<T, D, (8 * pg8 > 32 ? 32 : (8 * pg8 < 8 ? 8 : 8 * pg8)), 1>(c, q, summary, pt, scores, s, rr);
   }
   return cudaErrorInvalidValue;
 }
 
 cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
-                              float* scores, cudaStream_t s) {
+                              float* scores, cudaStream_t s, const ReqRange& rr) {
   if (pt.batch == 0 || pt.total_pages == 0) return cudaSuccess;
   const vx_geom& g = c->g;
   if (g.dtype == VX_DT_BF16) {
     switch (g.qk_dim) {
-      case 64: return launch_score_d<__nv_bfloat16, 64>(c, q, summary, pt, scores, s);
-      case 128: return launch_score_d<__nv_bfloat16, 128>(c, q, summary, pt, scores, s);
-      case 256: return launch_score_d<__nv_bfloat16, 256>(c, q, summary, pt, scores, s);
-      case 576: return launch_score_d<__nv_bfloat16, 576>(c, q, summary, pt, scores, s);
+      case 64: return launch_score_d<__nv_bfloat16, 64>(c, q, summary, pt, scores, s, rr);
+      case 128: return launch_score_d<__nv_bfloat16, 128>(c, q, summary, pt, scores, s, rr);
+      case 256: return launch_score_d<__nv_bfloat16, 256>(c, q, summary, pt, scores, s, rr);
+      case 576: return launch_score_d<__nv_bfloat16, 576>(c, q, summary, pt, scores, s, rr);
     }
   } else {
     switch (g.qk_dim) {
-      case 64: return launch_score_d<float, 64>(c, q, summary, pt, scores, s);
-      case 128: return launch_score_d<float, 128>(c, q, summary, pt, scores, s);
+      case 64: return launch_score_d<float, 64>(c, q, summary, pt, scores, s, rr);
+      case 128: return launch_score_d<float, 128>(c, q, summary, pt, scores, s, rr);
     }
   }
   return cudaErrorInvalidValue;

@@ -42,7 +42,7 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
             const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
             const int32_t* __restrict__ seq_lens, int page_size, const int32_t* __restrict__ budget,
             int n_sink, int n_local, int max_budget, int smem_keys, int32_t* __restrict__ sel_phys,
-            int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count) {
+            int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count, int req0) {
   constexpr int WARPS = THREADS / kWarp;
   constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
   static_assert(kBins % THREADS == 0 && THREADS >= kList, "shape");
@@ -55,7 +55,7 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
   __shared__ int s_bin, s_above, s_cnt, s_nlist, s_need_eq;
   __shared__ uint32_t s_thr;
 
-  const int kvh = blockIdx.x, i = blockIdx.y;
+  const int kvh = blockIdx.x, i = blockIdx.y + req0;
   const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
   const int k = min(budget[i], max_budget);
@@ -233,7 +233,7 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
 template <int THREADS>
 static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
                                  int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
-                                 cudaStream_t s, bool pdl) {
+                                 cudaStream_t s, bool pdl, const ReqRange& rr) {
   const vx_geom& g = c->g;
   const int keys = pt.max_pages_per_req <= kTopkSmemKeys ? pt.max_pages_per_req : 0;
   const size_t smem = (size_t)(keys > 0 ? keys : 1) * sizeof(uint32_t);
@@ -244,26 +244,26 @@ static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_t
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  dim3 grid(g.num_kv_heads, pt.batch);
+  dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
   cudaError_t e = launch_kernel(topk_kernel<THREADS>, grid, dim3(THREADS), smem, s, pdl, scores, g.num_kv_heads,
                                 pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
-                                g.n_sink, g.n_local, max_budget, keys, sel_phys, sel_logical, sel_count);
+                                g.n_sink, g.n_local, max_budget, keys, sel_phys, sel_logical, sel_count, rr.begin);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
-                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl) {
+                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl, const ReqRange& rr) {
   if (pt.batch == 0) return cudaSuccess;
   // block size by problem size (VX_TOPK_THREADS overrides, for tuning)
   static int force = -1;
   if (force < 0) { const char* e = getenv("VX_TOPK_THREADS"); force = e ? atoi(e) : 0; }
   const int n = pt.max_pages_per_req;
   const int th = force ? force : (n <= 1024 ? 256 : n <= 4096 ? 512 : 1024);
-  if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
-  if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
-  return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl);
+  if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr);
+  if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr);
+  return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr);
 }
 
 }  // namespace vx
