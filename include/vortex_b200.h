@@ -55,8 +55,9 @@ typedef enum {
 typedef enum { VX_DT_BF16 = 0, VX_DT_F32 = 1 } vx_dtype;
 
 /* aggregation of per-head envelope scores over the heads of one KV head.
- * SUM ranks like the paper's mean ("topK(Sum(s))"); MAX is the
- * max_h variant of App. G (:556).  MAX returns VX_ERR_UNSUPPORTED in this round. */
+ * SUM ranks like the paper's mean ("topK(Sum(s))"); MAX is the max_h variant of
+ * App. G (:556), built for GQA groups of <= 8 heads (g flop per byte on CUDA cores); for the 32-head
+ * MLA group vx_create returns VX_ERR_UNSUPPORTED. */
 typedef enum { VX_AGG_SUM = 0, VX_AGG_MAX = 1 } vx_agg;
 
 typedef struct {

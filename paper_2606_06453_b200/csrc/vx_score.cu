@@ -70,7 +70,7 @@ struct GroupIter {
   }
 };
 
-template <typename T, int D, int PG, int HKV, int kScStages>
+template <typename T, int D, int PG, int HKV, int kScStages, int AGG>
 __global__ void __launch_bounds__(kScThreads, 2)
 score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int batch,
              const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices, int total_pages,
@@ -88,7 +88,8 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
 
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ __align__(8) uint64_t s_full[kScStages], s_empty[kScStages];
-  float* s_q = reinterpret_cast<float*>(smem + (size_t)kScStages * STAGE_BYTES);   // [HKV][2*D]: Qm | Qp
+  float* s_q = reinterpret_cast<float*>(smem + (size_t)kScStages * STAGE_BYTES);   // SUM: [HKV][2*D] fp32: Qm | Qp
+  T* s_qh = reinterpret_cast<T*>(smem + (size_t)kScStages * STAGE_BYTES);          // MAX: [Hq][2*D] in T: min(q_h,0) | max(q_h,0)
 
   const int warp = threadIdx.x / kWarp, lane = threadIdx.x % kWarp;
   const int flat_lo = page_indptr[req_begin], flat_span = page_indptr[req_end] - flat_lo;   // this launch's request window
@@ -145,6 +146,21 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     const int s = g % kScStages;
     if (req != cur_req) {                        // new request: rebuild [Qm | Qp] for all KV heads (rare)
       asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
+      if constexpr (AGG == VX_AGG_MAX) {
+        // per-head vectors (PAPER.md:556 max_h variant): u[h] = [min(q_h,0) | max(q_h,0)] . [m | M], exact in T
+        constexpr int NVH = D / PER;
+        for (int e = threadIdx.x; e < num_q_heads * NVH; e += kScConsumerWarps * kWarp) {
+          const int h = e / NVH, c = e % NVH;
+          const uint4 raw = *reinterpret_cast<const uint4*>(q + ((int64_t)req * num_q_heads + h) * D + c * PER);
+          float f[PER];
+          Elem<T>::unpack(raw, f);
+#pragma unroll
+          for (int x = 0; x < PER; ++x) {
+            s_qh[h * ROW_ELEMS + c * PER + x] = Elem<T>::from_float(fminf(f[x], 0.f));
+            s_qh[h * ROW_ELEMS + D + c * PER + x] = Elem<T>::from_float(fmaxf(f[x], 0.f));
+          }
+        }
+      } else {
       // one thread per (KV head, 16-byte channel vector); the group's heads are read 8 at a time with all
       // loads of a batch in flight together (a head-by-head loop costs one memory latency per head)
       constexpr int NV = D / PER;
@@ -173,13 +189,16 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
           s_q[h * ROW_ELEMS + D + c * PER + x] = qp[x];
         }
       }
+      }
       asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
       cur_req = req;
+      if constexpr (AGG == VX_AGG_SUM) {
 #pragma unroll
-      for (int t = 0; t < NIT; ++t) {
-        const int c = lane + t * kWarp;
+        for (int t = 0; t < NIT; ++t) {
+          const int c = lane + t * kWarp;
 #pragma unroll
-        for (int e = 0; e < PER; ++e) qreg[t][e] = (NCH % kWarp == 0 || c < NCH) ? s_q[kvh * ROW_ELEMS + c * PER + e] : 0.f;
+          for (int e = 0; e < PER; ++e) qreg[t][e] = (NCH % kWarp == 0 || c < NCH) ? s_q[kvh * ROW_ELEMS + c * PER + e] : 0.f;
+        }
       }
     }
     sc_mbar_wait(smem_u32(&s_full[s]), (g / kScStages) & 1);
@@ -197,6 +216,31 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     }
     __syncwarp();
     if (lane == 0) sc_mbar_arrive(smem_u32(&s_empty[s]));    // stage consumed: its rows are in registers
+    if constexpr (AGG == VX_AGG_MAX) {
+      // g dot products per row, the head vectors read from shared memory (conflict-free: a warp reads one row)
+#pragma unroll
+      for (int k = 0; k < RPW; ++k) {
+        const int r = warp + k * kScConsumerWarps;
+        float best = -INFINITY;
+        for (int h = 0; h < grp; ++h) {
+          float acc = 0.f;
+#pragma unroll
+          for (int t = 0; t < NIT; ++t) {
+            const int c = lane + t * kWarp;
+            if (NCH % kWarp == 0 || c < NCH) {
+              float f[PER], qf[PER];
+              Elem<T>::unpack(v[k][t], f);
+              Elem<T>::unpack(*reinterpret_cast<const uint4*>(s_qh + (kvh * grp + h) * ROW_ELEMS + c * PER), qf);
+#pragma unroll
+              for (int e = 0; e < PER; ++e) acc = fmaf(qf[e], f[e], acc);
+            }
+          }
+          best = fmaxf(best, warp_sum(acc));
+        }
+        if (lane == 0 && r < rows) scores[(int64_t)kvh * total_pages + first + r / HKV] = best;
+      }
+      continue;
+    }
     float part[RPW];
 #pragma unroll
     for (int k = 0; k < RPW; ++k) {
@@ -257,38 +301,48 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
 }
 
 bool score_geometry_supported(const vx_geom& g) {
-  if (g.agg != VX_AGG_SUM) return false;
+  if (g.agg != VX_AGG_SUM && g.agg != VX_AGG_MAX) return false;
   const int hkv = g.num_kv_heads;
+  // MAX costs g flop per byte: CUDA cores carry it for GQA groups (g <= 8); the MLA group (g = 32) would need
+  // the tensor cores for the scoring too -- not built (NEXT-1)
+  if (g.agg == VX_AGG_MAX && (g.kv_shared || g.num_q_heads / hkv > 8)) return false;
   if (hkv != 1 && hkv != 2 && hkv != 4 && hkv != 8) return false;   // a consumer warp owns one KV head
   if (g.dtype == VX_DT_BF16) return g.qk_dim == 128 || g.qk_dim == 64 || g.qk_dim == 576 || g.qk_dim == 256;
   return g.qk_dim == 64 || g.qk_dim == 128;
 }
 
-template <typename T, int D, int PG, int HKV>
-static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
+template <typename T, int D, int PG, int HKV, int AGG>
+static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
                                   float* scores, cudaStream_t s, const ReqRange& rr) {
   const vx_geom& g = c->g;
   constexpr size_t page_bytes = (size_t)HKV * 2 * D * sizeof(T);
   // as many ~16-32 KB stages as two CTAs per SM can hold (>= 3): the bytes in flight, not the math, set the rate
-  constexpr size_t q_bytes = (size_t)HKV * 2 * D * sizeof(float);
+  constexpr size_t q_bytes = AGG == VX_AGG_MAX ? (size_t)HKV * 8 * 2 * D * sizeof(T) : (size_t)HKV * 2 * D * sizeof(float);
   constexpr int kScStages = (int)((110 * 1024 - q_bytes) / (PG * page_bytes)) < 3 ? 3 : ((int)((110 * 1024 - q_bytes) / (PG * page_bytes)) > 8 ? 8 : (int)((110 * 1024 - q_bytes) / (PG * page_bytes)));
   constexpr size_t smem = kScStages * PG * page_bytes + q_bytes;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(score_kernel<T, D, PG, HKV, kScStages>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(score_kernel<T, D, PG, HKV, kScStages, AGG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  int ctas = c->num_sms * 2;                     // two CTAs per SM (3 x ~32 KB stages each)
+  int ctas = c->num_sms * (2 * smem + 4096 <= 227 * 1024 ? 2 : 1);   // two CTAs per SM when they fit
   const int min_pages = 2 * PG;                  // do not spread tiny inputs over every SM
   const int64_t est_pages = rr.count < 0 ? pt.total_pages : (int64_t)pt.total_pages * rr.count / (pt.batch > 0 ? pt.batch : 1) + 1;
   if ((int64_t)ctas * min_pages > est_pages) ctas = (int)((est_pages + min_pages - 1) / min_pages);
   if (ctas < 1) ctas = 1;
-  score_kernel<T, D, PG, HKV, kScStages><<<ctas, kScThreads, smem, s>>>(
+  score_kernel<T, D, PG, HKV, kScStages, AGG><<<ctas, kScThreads, smem, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, pt.batch, pt.page_indptr,
       pt.page_indices, pt.total_pages, scores, rr.begin, rr.begin + (rr.count < 0 ? pt.batch : rr.count));
   c->launches += 1;
   return cudaGetLastError();
+}
+
+template <typename T, int D, int PG, int HKV>
+static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
+                                  float* scores, cudaStream_t s, const ReqRange& rr) {
+  if (c->g.agg == VX_AGG_MAX) return launch_score_agg<T, D, PG, HKV, VX_AGG_MAX>(c, q, summary, pt, scores, s, rr);
+  return launch_score_agg<T, D, PG, HKV, VX_AGG_SUM>(c, q, summary, pt, scores, s, rr);
 }
 
 // PG pages per stage so that a stage is ~32 KB and every consumer warp gets 1..8 rows of it

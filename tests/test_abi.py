@@ -53,9 +53,12 @@ def test_workspace_bytes_and_geometry_validation(vx):
     assert big >= 8 * 65536 * 4 + 32 * 32 * 32 * 128 * 4
     assert ws(geom(vx, num_q_heads=30), 4, 1000, 500, 64) == 0          # Hq % Hkv != 0
     assert ws(geom(vx, qk_dim=80, v_dim=80), 4, 1000, 500, 64) == 0     # unsupported width
-    assert ws(geom(vx, agg=1), 4, 1000, 500, 64) == 0                   # MAX aggregation not built yet
+    assert ws(geom(vx, agg=1), 4, 1000, 500, 64) > 0                    # max_h aggregation: GQA groups of <= 8 heads
+    assert ws(geom(vx, agg=2), 4, 1000, 500, 64) == 0                   # unknown aggregation
     assert ws(geom(vx, dtype=0, num_q_heads=32, num_kv_heads=1, qk_dim=576, v_dim=512, page_size=64,
                    kv_shared=1), 64, 50000, 1024, 32) > 0              # MLA geometry
+    assert ws(geom(vx, dtype=0, num_q_heads=32, num_kv_heads=1, qk_dim=576, v_dim=512, page_size=64,
+                   kv_shared=1, agg=1), 64, 50000, 1024, 32) == 0      # max_h over the 32-head MLA group: not built
     assert ws(geom(vx, dtype=1, num_q_heads=4, num_kv_heads=1, qk_dim=64, v_dim=64), 1, 64, 64, 8) > 0
 
 

@@ -186,6 +186,54 @@ def test_fused_step_matches_oracle(name, flags):
         assert rec >= 0.99
 
 
+@pytest.mark.parametrize("name", ["C1", "C2-small", "C3-small", "C5-small"])
+def test_max_aggregation_scores_and_step_match_oracle(name):
+    """VX_AGG_MAX (the max_h envelope variant): scores and the fused step against the oracle."""
+    import paper_2606_06453_b200 as vxm
+    vx, w, _, pool, pt = setup(name)
+    ctx = vxm.context_for(w, agg=vxm.binding.VX_AGG_MAX)
+    summary = build_summary(vx, w, ctx, pool, pt)
+    ref = oracle_step(w, agg=vo.AGG_MAX)
+    scores = torch.full((w.spec.num_kv_heads, w.total_pages), float("nan"), device="cuda:0")
+    ctx.page_score(w.q, summary, pt, scores)
+    torch.cuda.synchronize()
+    got = scores.cpu().numpy().astype(np.float64)
+    assert np.abs(got - ref["scores"]).max() <= 2e-5 * np.abs(ref["scores"]).max()
+    # the invariant that defines the variant: S_max[j] >= u[h, j] for every head, with equality for one of them
+    grp = w.spec.num_q_heads // w.spec.num_kv_heads
+    u = ref["u"].reshape(w.spec.num_kv_heads, grp, -1)
+    assert (got[:, None, :] >= u - 2e-5 * np.abs(u).max()).all()
+    o = outputs(w)
+    ctx.sparse_decode_step(w.q, pool, summary, pt, w.budget, w.max_budget, o["out"], o["lse"], o["sel_phys"],
+                           o["sel_logical"], o["sel_count"], flags=1)
+    torch.cuda.synchronize()
+    sl, sc = o["sel_logical"].cpu().numpy(), o["sel_count"].cpu().numpy()
+    check_selection(w, sl, o["sel_phys"].cpu().numpy(), sc, ref)
+    o_ref, l_ref = oracle_attention_on(w, sl, sc)
+    check_attention(w.spec.dtype, o["out"].float().cpu().numpy(), o["lse"].cpu().numpy(), o_ref, l_ref)
+
+
+def test_step_without_local_pages_runs_the_summary_kernel_first():
+    """n_local = 0: the newest page is not forced, so its refreshed summary must be in place BEFORE scoring
+    (the decode kernel cannot fold the update); stale summaries of the newest pages must not change the result."""
+    from paper_2606_06453_b200.workloads import SPECS
+    spec = replace(SPECS["C2-small"], n_local=0, n_sink=1)
+    vx, w, ctx, pool, pt = setup(spec)
+    summary = build_summary(vx, w, ctx, pool, pt)
+    lastp = [int(w.page_indices[int(w.page_indptr[i + 1]) - 1]) for i in range(w.spec.batch)]
+    summary[lastp] = 0
+    o = outputs(w)
+    ctx.sparse_decode_step(w.q, pool, summary, pt, w.budget, w.max_budget, o["out"], o["lse"], o["sel_phys"],
+                           o["sel_logical"], o["sel_count"], flags=1)
+    torch.cuda.synchronize()
+    assert ctx.last_launch_count >= 4
+    ref = oracle_step(w)
+    sl, sc = o["sel_logical"].cpu().numpy(), o["sel_count"].cpu().numpy()
+    check_selection(w, sl, o["sel_phys"].cpu().numpy(), sc, ref)
+    o_ref, l_ref = oracle_attention_on(w, sl, sc)
+    check_attention(w.spec.dtype, o["out"].float().cpu().numpy(), o["lse"].cpu().numpy(), o_ref, l_ref)
+
+
 @pytest.mark.parametrize("name", ["C1", "C4-small", "C5-small"])
 def test_host_step_equals_device_step(name):
     vx, w, ctx, pool, pt = setup(name)
