@@ -151,6 +151,9 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->force_generic = fg && fg[0] == '1';
   const char* np = getenv("VX_NO_PDL");
   c->use_pdl = !(np && np[0] == '1');
+  const char* pm = getenv("VX_PREFETCH_MB");
+  c->prefetch_mb = pm ? atoi(pm) : 0;               // measured: no gain at 16 MB, slower beyond (the prefetch delays the selection kernel)
+  c->use_prefetch = c->prefetch_mb > 0;
   const char* ch = getenv("VX_CHAINS");
   c->chains = ch && atoi(ch) >= 2 ? 2 : 1;      // measured: no gain on C2..C4 (the chains mostly serialise on shared memory), +3 % on C5
   c->aux_stream = nullptr;
@@ -290,8 +293,25 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
     rr.count = two ? (ch == 0 ? n0 : pt->batch - n0) : -1;
     opt.rr = rr;
     if (vx_status st = check_cuda(c, launch_page_score(c, q, summary, *pt, c->ws.scores, cs, rr), "page score")) return st;
+    // L2 prefetch plan for the decode kernel's first pages (fast decode paths with contiguous page chunks only)
+    PrefetchPlan pf;
+    const int64_t esz = (int64_t)elem_size(c->g.dtype);
+    if (c->use_prefetch && decode_folds_summary(c) && pool->stride_token == c->g.qk_dim) {
+      const int n_req = rr.count < 0 ? pt->batch : rr.count;
+      pf.k = pool->k;
+      pf.v = c->g.kv_shared ? nullptr : pool->v;
+      pf.page_bytes = pool->stride_page * esz;
+      pf.head_bytes = pool->stride_head * esz;
+      pf.chunk_bytes = (uint32_t)(c->g.page_size * c->g.qk_dim * esz);
+      pf.splits = c->g.kv_shared ? decode_mla_splits(c, n_req, max_budget) : decode_gqa_splits(c, n_req, max_budget);
+      const int64_t per_page = (int64_t)pf.chunk_bytes * (pf.v ? 2 : 1);
+      const int64_t units = (int64_t)n_req * c->g.num_kv_heads * pf.splits;
+      const int64_t budget_bytes = (int64_t)c->prefetch_mb << 20;
+      pf.pages_per_split = (int)(budget_bytes / (units * per_page > 0 ? units * per_page : 1));
+      if (pf.pages_per_split < 1) pf.k = nullptr;
+    }
     if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, cs,
-                                                       c->use_pdl, rr), "top-k pages"))
+                                                       c->use_pdl, rr, pf), "top-k pages"))
       return st;
     if (vx_status st = decode_dispatch(c, q, pool, pt, sp, sl, sc, max_budget, out, lse, cs, opt)) return st;
     total_launches = c->launches;

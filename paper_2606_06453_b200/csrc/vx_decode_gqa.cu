@@ -308,14 +308,7 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
   }
   // splits: whole waves of equal CTAs.  cost(sp) = waves x (pages per warp + ~3 pages of pipeline fill)
   const int n_req = opt.rr.count < 0 ? pt.batch : opt.rr.count;
-  const int units = n_req * g.num_kv_heads;
-  const int slots = c->num_sms * 2;              // 96 KB of shared memory per CTA -> 2 CTAs per SM
-  int splits = 1, best_cost = 1 << 30;
-  for (int sp = 1; sp <= kMaxSplits && sp <= max_budget; ++sp) {
-    const int waves = (units * sp + slots - 1) / slots;
-    const int cost = waves * (((max_budget + sp - 1) / sp + kGqaWarps - 1) / kGqaWarps + 3);
-    if (cost < best_cost) { best_cost = cost; splits = sp; }
-  }
+  const int splits = decode_gqa_splits(c, n_req, max_budget);
   dim3 grid(splits, g.num_kv_heads, n_req);
   cudaError_t e = launch_kernel(decode_gqa_mma_kernel<D>, grid, dim3(kGqaWarps * kWarp), (size_t)smem, s, opt.pdl,
       static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(pool.k),
@@ -325,6 +318,18 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+int decode_gqa_splits(const vx_ctx* c, int n_req, int max_budget) {
+  const int units = n_req * c->g.num_kv_heads;
+  const int slots = c->num_sms * 2;              // 96 KB of shared memory per CTA -> 2 CTAs per SM
+  int splits = 1, best_cost = 1 << 30;
+  for (int sp = 1; sp <= kMaxSplits && sp <= max_budget; ++sp) {
+    const int waves = (units * sp + slots - 1) / slots;
+    const int cost = waves * (((max_budget + sp - 1) / sp + kGqaWarps - 1) / kGqaWarps + 3);
+    if (cost < best_cost) { best_cost = cost; splits = sp; }
+  }
+  return splits;
 }
 
 bool decode_folds_summary(const vx_ctx* c) { return !c->force_generic && (gqa_mma_supported(c->g) || mla_tc_supported(c->g)); }

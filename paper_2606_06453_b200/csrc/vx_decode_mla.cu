@@ -619,6 +619,16 @@ static cudaError_t make_latent_map(CUtensorMap* map, const vx_kv_pool& pool) {
   return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
 }
 
+int decode_mla_splits(const vx_ctx* c, int n_req, int max_budget) {
+  int best = 1, best_cost = 1 << 30;
+  for (int sp = 1; sp <= kMaxSplits && sp <= max_budget && sp <= c->g.num_q_heads; ++sp) {   // partial buffer: splits <= Hq
+    const int waves = (n_req * sp + c->num_sms - 1) / c->num_sms;
+    const int cost = waves * ((max_budget + sp - 1) / sp + 2);
+    if (cost < best_cost) { best_cost = cost; best = sp; }
+  }
+  return best;
+}
+
 cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                  const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                                  int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
@@ -634,12 +644,7 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
   // one CTA per SM (221 KB of shared memory): whole waves of equal CTAs,
   // cost(sp) = waves x (pages per CTA + ~2 pages of pipeline fill and epilogue)
   const int n_req = opt.rr.count < 0 ? pt.batch : opt.rr.count;
-  int best = 1, best_cost = 1 << 30;
-  for (int sp = 1; sp <= kMaxSplits && sp <= max_budget && sp <= g.num_q_heads; ++sp) {   // partial buffer: splits <= Hq
-    const int waves = (n_req * sp + c->num_sms - 1) / c->num_sms;
-    const int cost = waves * ((max_budget + sp - 1) / sp + 2);
-    if (cost < best_cost) { best_cost = cost; best = sp; }
-  }
+  const int best = decode_mla_splits(c, n_req, max_budget);
   dim3 grid(best, 1, n_req);
   cudaError_t e = launch_kernel(decode_mla_kernel, grid, dim3(mla::THREADS), (size_t)mla::SMEM_BYTES, s, opt.pdl, kmap,
                                 static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens,

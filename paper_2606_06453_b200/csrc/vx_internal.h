@@ -43,6 +43,8 @@ struct vx_ctx {
   int32_t launches;              // kernels enqueued by the last compute call
   bool force_generic;            // VX_FORCE_GENERIC=1 in the environment: CUDA-core decode path only (debug)
   bool use_pdl;                  // chain the kernels of a step with programmatic dependent launch (VX_NO_PDL=1: off)
+  bool use_prefetch;             // the selection kernel prefetches the decode kernel's first pages into L2 (VX_PREFETCH_MB=0: off)
+  int prefetch_mb;               // prefetch budget, MiB (default 48 of the 126 MB L2)
   int chains;                    // request windows run as concurrent kernel chains inside a fused step (VX_CHAINS, 1 or 2)
   cudaStream_t aux_stream;       // second chain's stream; fork / join with the caller's stream by events
   cudaEvent_t ev_fork, ev_join;
@@ -77,6 +79,20 @@ struct ReqRange {
   int count = -1;
 };
 
+// What the selection kernel prefetches into L2 for the decode kernel that follows it in a step: the first
+// `pages_per_split` pages of every split of every (request, KV head), K and V chunks (`chunk_bytes` contiguous
+// bytes each).  Between the end of the selection and the decode kernel's first loads HBM would sit idle; the
+// prefetch moves up to ~48 MB of the decode kernel's stream into that gap.  k == nullptr: no prefetch.
+struct PrefetchPlan {
+  const void* k = nullptr;
+  const void* v = nullptr;                       // nullptr: K only (MLA latent)
+  int64_t page_bytes = 0, head_bytes = 0;        // byte strides of a page / a KV head in the pool
+  uint32_t chunk_bytes = 0;                      // page_size * row bytes, contiguous
+  int splits = 1, pages_per_split = 0;
+};
+int decode_gqa_splits(const vx_ctx* c, int n_req, int max_budget);
+int decode_mla_splits(const vx_ctx* c, int n_req, int max_budget);
+
 // how a decode launch is embedded in a step
 struct DecodeOpts {
   ReqRange rr;
@@ -93,7 +109,7 @@ cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, con
 cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
                               int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl = false,
-                              const ReqRange& rr = ReqRange());
+                              const ReqRange& rr = ReqRange(), const PrefetchPlan& pf = PrefetchPlan());
 cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,

@@ -42,7 +42,7 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
             const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
             const int32_t* __restrict__ seq_lens, int page_size, const int32_t* __restrict__ budget,
             int n_sink, int n_local, int max_budget, int smem_keys, int32_t* __restrict__ sel_phys,
-            int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count, int req0) {
+            int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count, int req0, const PrefetchPlan pf) {
   constexpr int WARPS = THREADS / kWarp;
   constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
   static_assert(kBins % THREADS == 0 && THREADS >= kList, "shape");
@@ -218,10 +218,18 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
   }
   if (staged) {                                   // every selected page: one independent gather + two stores
     __syncthreads();
+    const int per_split = (n_sel + pf.splits - 1) / pf.splits;
     for (int r = tid; r < n_sel; r += THREADS) {
       const int j = s_hist[r];
-      sel_phys[out0 + r] = page_indices[row0 + j];
+      const int phys = page_indices[row0 + j];
+      sel_phys[out0 + r] = phys;
       if (sel_logical) sel_logical[out0 + r] = j;
+      // the decode kernel starts every split at its first pages: pull those into L2 while HBM is idle
+      if (pf.k != nullptr && r % per_split < pf.pages_per_split) {
+        const int64_t off = (int64_t)phys * pf.page_bytes + (int64_t)kvh * pf.head_bytes;
+        l2_prefetch(static_cast<const uint8_t*>(pf.k) + off, pf.chunk_bytes);
+        if (pf.v != nullptr) l2_prefetch(static_cast<const uint8_t*>(pf.v) + off, pf.chunk_bytes);
+      }
     }
   }
   for (int r = n_sel + tid; r < max_budget; r += THREADS) {
@@ -233,7 +241,7 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
 template <int THREADS>
 static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
                                  int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
-                                 cudaStream_t s, bool pdl, const ReqRange& rr) {
+                                 cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf) {
   const vx_geom& g = c->g;
   const int keys = pt.max_pages_per_req <= kTopkSmemKeys ? pt.max_pages_per_req : 0;
   const size_t smem = (size_t)(keys > 0 ? keys : 1) * sizeof(uint32_t);
@@ -247,23 +255,24 @@ static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_t
   dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
   cudaError_t e = launch_kernel(topk_kernel<THREADS>, grid, dim3(THREADS), smem, s, pdl, scores, g.num_kv_heads,
                                 pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
-                                g.n_sink, g.n_local, max_budget, keys, sel_phys, sel_logical, sel_count, rr.begin);
+                                g.n_sink, g.n_local, max_budget, keys, sel_phys, sel_logical, sel_count, rr.begin, pf);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
-                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl, const ReqRange& rr) {
+                              int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl, const ReqRange& rr,
+                              const PrefetchPlan& pf) {
   if (pt.batch == 0) return cudaSuccess;
   // block size by problem size (VX_TOPK_THREADS overrides, for tuning)
   static int force = -1;
   if (force < 0) { const char* e = getenv("VX_TOPK_THREADS"); force = e ? atoi(e) : 0; }
   const int n = pt.max_pages_per_req;
   const int th = force ? force : (n <= 1024 ? 256 : n <= 4096 ? 512 : 1024);
-  if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr);
-  if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr);
-  return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr);
+  if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
+  if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
+  return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
 }
 
 }  // namespace vx
