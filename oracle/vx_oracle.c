@@ -19,6 +19,8 @@
  *   attention o = softmax(q K_I^T * sm_scale) V_I over the tokens of the selected
  *             pages (:92 Eq. 4), lse = natural log of the softmax denominator
  *   combine   split-softmax merge by log-sum-exp (:75 Flash-Decoding)
+ *   block top-k flow: centroid = mean of the block's keys, rounded to the KV dtype
+ *             (:92 Eq. 1); score = group sum of q_h . centroid (:92 Eq. 2); pins in tests/test_oracle_centroid.py
  *
  * Every function is the plain definition: no blocking, no fusion, no reordering.
  * All arithmetic is double.  Inputs are read in their storage dtype (bf16 bits or
@@ -140,6 +142,83 @@ void vxo_page_score(const void *q, int dtype, const double *summary, int num_q_h
           else if (u > agg_val) agg_val = u;
         }
         s_out[(int64_t)kvh * T + col] = agg_val;
+      }
+    }
+  }
+}
+
+/* ------------------------------------------------------------------------- *
+ * Block top-k flow (section 3.1, the equations around "(2)" at :92):
+ *   centroid  kc[j,c] = mean_t K[page j, t, c] over the page's VALID tokens         (Eq. 1)
+ *   score     s[j]    = mean_{h in group} q_h . kc[j]                               (Eq. 2)
+ * The centroid is stored in the KV dtype: for bf16 pools the exact mean (a sum of at most a few
+ * hundred bf16 values is exact in double) is rounded to bf16, round-to-nearest-even, and returned
+ * as that bf16 value widened to double.  Scores are returned as the group SUM (ranks like the mean,
+ * same convention as the envelope score; reading G2).
+ * ------------------------------------------------------------------------- */
+static double round_to_storage(double x, int dtype) {
+  float f = (float)x;                         /* fp32 storage: one rounding */
+  if (dtype == VXO_F32) return (double)f;
+  /* bf16: round the DOUBLE to 8 significand bits directly (no double rounding through float) */
+  if (x == 0.0 || x != x) return x;
+  int e;
+  double m = frexp(x, &e);                    /* x = m * 2^e, 0.5 <= |m| < 1 */
+  double scaled = ldexp(m, 8);                /* 8 significand bits: |scaled| in [128, 256) */
+  double r = nearbyint(scaled);               /* default rounding mode: to nearest, ties to even */
+  return ldexp(r, e - 8);
+}
+
+void vxo_page_centroid(const void *k, int dtype, int64_t stride_page, int64_t stride_token,
+                       int64_t stride_head, int num_kv_heads, int qk_dim, int page_size,
+                       int batch, const int32_t *page_indptr, const int32_t *page_indices,
+                       const int32_t *seq_lens, const int32_t *first_page,
+                       double *centroid /* [num_pool_pages, Hkv, d] */) {
+#pragma omp parallel for schedule(dynamic)
+  for (int i = 0; i < batch; ++i) {
+    int n = seq_lens[i];
+    int P = num_pages_of(n, page_size);
+    for (int j = first_page ? first_page[i] : 0; j < P; ++j) {
+      int64_t phys = page_indices[page_indptr[i] + j];
+      int t_end = n - j * page_size;
+      if (t_end > page_size) t_end = page_size;
+      for (int h = 0; h < num_kv_heads; ++h) {
+        double *kc = centroid + (phys * num_kv_heads + h) * (int64_t)qk_dim;
+        for (int c = 0; c < qk_dim; ++c) {
+          double sum = 0.0;
+          for (int t = 0; t < t_end; ++t)
+            sum += ld_elem(k, dtype, phys * stride_page + t * stride_token + h * stride_head + c);
+          kc[c] = round_to_storage(sum / (double)t_end, dtype);
+        }
+      }
+    }
+  }
+}
+
+void vxo_centroid_score(const void *q, int dtype, const double *centroid, int num_q_heads,
+                        int num_kv_heads, int qk_dim, int batch, const int32_t *page_indptr,
+                        const int32_t *page_indices, const int32_t *seq_lens, int page_size,
+                        double *u_out /* [Hq, T] per-head q_h . kc, may be NULL */,
+                        double *s_out /* [Hkv, T] group sum */) {
+  int g = num_q_heads / num_kv_heads;
+  int64_t T = page_indptr[batch];
+#pragma omp parallel for schedule(dynamic)
+  for (int i = 0; i < batch; ++i) {
+    int P = num_pages_of(seq_lens[i], page_size);
+    for (int j = 0; j < P; ++j) {
+      int64_t col = page_indptr[i] + j;
+      int64_t phys = page_indices[col];
+      for (int kvh = 0; kvh < num_kv_heads; ++kvh) {
+        const double *kc = centroid + (phys * num_kv_heads + kvh) * (int64_t)qk_dim;
+        double total = 0.0;
+        for (int r = 0; r < g; ++r) {
+          int h = kvh * g + r;
+          double u = 0.0;
+          for (int c = 0; c < qk_dim; ++c)
+            u += ld_elem(q, dtype, ((int64_t)i * num_q_heads + h) * qk_dim + c) * kc[c];
+          if (u_out) u_out[(int64_t)h * T + col] = u;
+          total += u;
+        }
+        s_out[(int64_t)kvh * T + col] = total;
       }
     }
   }

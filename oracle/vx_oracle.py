@@ -141,6 +141,34 @@ def page_score(q: np.ndarray, summary: np.ndarray, pt: PageTable, num_q_heads: i
     return u, s
 
 
+def page_centroid(pool: Pool, pt: PageTable, num_kv_heads: int, qk_dim: int, first_page=None,
+                  centroid: np.ndarray | None = None) -> np.ndarray:
+    """Block top-k summaries (Eq.1): float64 [num_pool_pages, Hkv, d], the mean over the valid
+    tokens rounded to the KV dtype (bf16 / fp32).  Untouched pages stay NaN."""
+    if centroid is None:
+        centroid = np.full((pool.num_pool_pages, num_kv_heads, qk_dim), np.nan, dtype=np.float64)
+    fp = _i32(first_page) if first_page is not None else None
+    lib().vxo_page_centroid(_p(pool.k), _dt(pool.k), C.c_int64(pool.stride_page),
+                            C.c_int64(pool.stride_token), C.c_int64(pool.stride_head),
+                            num_kv_heads, qk_dim, pt.page_size, pt.batch, _p(pt.page_indptr),
+                            _p(pt.page_indices), _p(pt.seq_lens), _p(fp), _p(centroid))
+    return centroid
+
+
+def centroid_score(q: np.ndarray, centroid: np.ndarray, pt: PageTable, num_q_heads: int,
+                   num_kv_heads: int):
+    """returns (u [Hq, T] per-head q_h . centroid, S [Hkv, T] group sums; Eq.2), float64."""
+    d = centroid.shape[-1]
+    T = pt.total_pages
+    u = np.zeros((num_q_heads, T), dtype=np.float64)
+    s = np.zeros((num_kv_heads, T), dtype=np.float64)
+    centroid = np.ascontiguousarray(centroid, dtype=np.float64)
+    lib().vxo_centroid_score(_p(q), _dt(q), _p(centroid), num_q_heads, num_kv_heads, d, pt.batch,
+                             _p(pt.page_indptr), _p(pt.page_indices), _p(pt.seq_lens), pt.page_size,
+                             _p(u), _p(s))
+    return u, s
+
+
 def topk_pages(scores: np.ndarray, pt: PageTable, budget, n_sink: int, n_local: int,
                max_budget: int):
     """returns (sel_logical, sel_phys [B,Hkv,max_budget] pad -1, sel_count [B,Hkv], thr [B,Hkv])."""
@@ -210,11 +238,18 @@ def combine(o_part: np.ndarray, lse_part: np.ndarray):
 
 def decode_step(q, pool: Pool, pt: PageTable, budget, max_budget: int, num_q_heads: int,
                 num_kv_heads: int, qk_dim: int, v_dim: int, sm_scale: float, n_sink: int,
-                n_local: int, agg: int = AGG_SUM, summary: np.ndarray | None = None):
-    """the whole step in the paper's order: summary -> score -> top-k -> attention."""
-    if summary is None:
-        summary = page_summary(pool, pt, num_kv_heads, qk_dim)
-    u, s = page_score(q, summary, pt, num_q_heads, num_kv_heads, agg)
+                n_local: int, agg: int = AGG_SUM, summary: np.ndarray | None = None,
+                kind: str = "envelope"):
+    """the whole step in the paper's order: summary -> score -> top-k -> attention.
+    kind = "envelope" (Quest) or "centroid" (block top-k, Eq.1-2)."""
+    if kind == "centroid":
+        if summary is None:
+            summary = page_centroid(pool, pt, num_kv_heads, qk_dim)
+        u, s = centroid_score(q, summary, pt, num_q_heads, num_kv_heads)
+    else:
+        if summary is None:
+            summary = page_summary(pool, pt, num_kv_heads, qk_dim)
+        u, s = page_score(q, summary, pt, num_q_heads, num_kv_heads, agg)
     sl, sp, sc, thr = topk_pages(s, pt, budget, n_sink, n_local, max_budget)
     out, lse = sparse_attention(q, pool, pt, sl, sc, num_q_heads, num_kv_heads, qk_dim, v_dim, sm_scale)
     return dict(summary=summary, u=u, scores=s, sel_logical=sl, sel_phys=sp, sel_count=sc,
