@@ -42,6 +42,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--also", default="C3,C4", help="extra configs timed briefly and reported under 'also'")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--summary", default="envelope", choices=["envelope", "centroid"],
+                    help="page summary / score flow: Quest envelope (default, the north star) or block top-k centroid")
     return ap.parse_args()
 
 
@@ -69,7 +71,7 @@ def ncu_traffic(cfg, stage):
     return None
 
 
-def algorithmic_bytes(w, sel_count=None):
+def algorithmic_bytes(w, sel_count=None, summary="envelope"):
     """Bytes roofline of one step: every summary row once, every selected
     page's K and V tokens once, Q in and O out.  Page table / scores / partials are not counted."""
     import torch
@@ -78,7 +80,7 @@ def algorithmic_bytes(w, sel_count=None):
     b = s.page_size
     n = w.seq_lens.cpu().long()
     P = (n + b - 1) // b
-    summary = int(P.sum()) * s.num_kv_heads * 2 * s.qk_dim * esz
+    summary = int(P.sum()) * s.num_kv_heads * (1 if summary == "centroid" else 2) * s.qk_dim * esz
     k = torch.minimum(w.budget.cpu().long(), P)
     tokens = (k - 1) * b + (n - (P - 1) * b)          # the partial last page is always selected (n_local >= 1)
     per_tok = (s.qk_dim if s.kv_shared else s.qk_dim + s.v_dim) * esz
@@ -127,15 +129,17 @@ class ClockSampler(threading.Thread):
 class Runner:
     """One workload resident on one GPU: context, pools, summaries, outputs, L2 flush buffer."""
 
-    def __init__(self, cfg, device, seed_offset=0):
+    def __init__(self, cfg, device, seed_offset=0, summary="envelope"):
         import torch
         import paper_2606_06453_b200 as vx
         from paper_2606_06453_b200.workloads import make_workload
         self.torch, self.vx = torch, vx
         self.w = w = make_workload(cfg, device=device, seed_offset=seed_offset)
-        self.ctx = vx.context_for(w)
+        kind = vx.binding.VX_SUMMARY_CENTROID if summary == "centroid" else vx.binding.VX_SUMMARY_ENVELOPE
+        self.summary_name = summary
+        self.ctx = vx.context_for(w, summary_kind=kind)
         self.pool, self.pt = vx.tables_for(w)
-        self.summary = vx.alloc_summary(w)
+        self.summary = vx.alloc_summary(w, kind)
         self.ctx.page_summary_update(self.pool, self.pt, self.summary, first_new_pos=torch.zeros_like(w.seq_lens))
         s = w.spec
         self.out = torch.empty(s.batch, s.num_q_heads, s.v_dim, dtype=w.q.dtype, device=device)
@@ -216,7 +220,7 @@ class Runner:
         return out
 
 
-def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None):
+def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None, summary="envelope"):
     """Time the oracle (as it stands) on the first n_requests requests of the workload.
     Returns (seconds for score + top-k + attention on the sample, requests in sample, batch, threads)."""
     from oracle import vx_oracle as vo
@@ -227,10 +231,11 @@ def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=No
     sub = subproblem(w, range(n_requests))
     q, pool, pt = to_oracle(sub)
     s = sub.spec
-    summary = vo.page_summary(pool, pt, s.num_kv_heads, s.qk_dim)       # built outside the timed step
+    build = vo.page_centroid if summary == "centroid" else vo.page_summary
+    summ = build(pool, pt, s.num_kv_heads, s.qk_dim)                    # built outside the timed step
     t0 = time.perf_counter()
     vo.decode_step(q, pool, pt, vo.as_np(sub.budget), sub.max_budget, s.num_q_heads, s.num_kv_heads, s.qk_dim,
-                   s.v_dim, s.sm_scale, s.n_sink, s.n_local, summary=summary)
+                   s.v_dim, s.sm_scale, s.n_sink, s.n_local, summary=summ, kind=summary)
     return time.perf_counter() - t0, n_requests, w.spec.batch, vo.num_threads()
 
 
@@ -248,14 +253,14 @@ def run_reference(args):
     times = []
     steps = max(1, min(args.steps, 3))
     for it in range(min(args.warmup, 1) + steps):
-        t, n, batch, threads = oracle_sample_time(args.config, nreq, workload=w)
+        t, n, batch, threads = oracle_sample_time(args.config, nreq, workload=w, summary=args.summary)
         if it >= min(args.warmup, 1):
             times.append(t)
     us = statistics.mean(times) / n * batch * 1e6        # scaled from the sample to the whole batch
     line = {"impl": "reference", "metric": METRIC, "value": us, "unit": "us", "n_gpus": args.gpus, "steps": steps,
             "warmup": min(args.warmup, 1), "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.config, "l2": "n/a (CPU)"},
+            "config": {"workload": args.config, "summary": args.summary, "l2": "n/a (CPU)"},
             "cpu_baseline": {"value": us, "unit": "us", "cores": threads, "kind": "oracle",
                              "sample": f"{n} of {batch} requests per step, scaled by {batch}/{n}"},
             "e2e": {"value": us, "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -290,9 +295,9 @@ def main():
         dist.barrier()
 
     peak, peak_src = measured_peak()
-    r = Runner(args.config, device, seed_offset=rank)
+    r = Runner(args.config, device, seed_offset=rank, summary=args.summary)
     w, s = r.w, r.w.spec
-    bytes_ = algorithmic_bytes(w)
+    bytes_ = algorithmic_bytes(w, summary=args.summary)
 
     def barrier():
         if world > 1:
@@ -342,7 +347,7 @@ def main():
         step_gbs = bytes_["total"] / (ms * 1e-3) / 1e9
         cpu = None
         if not args.no_cpu_baseline:
-            t, n, batch, threads = oracle_sample_time(args.config, SAMPLE_REQUESTS.get(args.config, 1), workload=w)
+            t, n, batch, threads = oracle_sample_time(args.config, SAMPLE_REQUESTS.get(args.config, 1), workload=w, summary=args.summary)
             cpu = {"value": t / n * batch * 1e6, "unit": "us", "cores": threads, "kind": "oracle",
                    "sample": f"first {n} of {batch} requests, one pass (score + top-k + attention), scaled by {batch}/{n}"}
         also = {}
@@ -359,7 +364,7 @@ def main():
                 "vs_baseline": None, "dtype": s.dtype, "data": "synthetic",
                 "config": {"workload": args.config, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
                            "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
-                           "seq_len": list(s.seq_len), "budget_pages": w.max_budget,
+                           "seq_len": list(s.seq_len), "budget_pages": w.max_budget, "summary": args.summary,
                            "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"},
                 "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
                 "step_bytes": bytes_, "stage_us": stage, "roofline": roofline, "cpu_baseline": cpu,

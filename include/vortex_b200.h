@@ -60,6 +60,14 @@ typedef enum { VX_DT_BF16 = 0, VX_DT_F32 = 1 } vx_dtype;
  * MLA group vx_create returns VX_ERR_UNSUPPORTED. */
 typedef enum { VX_AGG_SUM = 0, VX_AGG_MAX = 1 } vx_agg;
 
+/* what a page summary is (the query-independent cache of the flow):
+ *  ENVELOPE  Quest: channel-wise min / max of the page's keys (:546); score = envelope upper bound (:552).
+ *            summary: [num_pool_pages, Hkv, 2, qk_dim], [..,0,:] = min, [..,1,:] = max.
+ *  CENTROID  block top-k (:85-99 section 3.1): mean of the page's valid keys, rounded to the KV dtype (:92 Eq.1);
+ *            score = sum over the head group of q_h . centroid (:92 Eq.2; ranks like the paper's mean).
+ *            summary: [num_pool_pages, Hkv, qk_dim] -- half the bytes.  VX_AGG_SUM only. */
+typedef enum { VX_SUMMARY_ENVELOPE = 0, VX_SUMMARY_CENTROID = 1 } vx_summary_kind;
+
 typedef struct {
   int32_t dtype;        /* vx_dtype of q, K, V, summaries and out */
   int32_t num_q_heads;  /* Hq */
@@ -72,6 +80,7 @@ typedef struct {
   int32_t n_sink;       /* first pages always selected (:280) */
   int32_t n_local;      /* last pages always selected (:280); precondition n_sink+n_local <= budget[i] */
   int32_t agg;          /* vx_agg */
+  int32_t summary_kind; /* vx_summary_kind */
 } vx_geom;
 
 typedef struct {
@@ -123,7 +132,9 @@ int32_t vx_last_launch_count(const vx_ctx *ctx);
  * the newest token fell into; first_new_pos[i] = 0 rebuilds all pages of the request):
  *   summary[p, h, 0, c] = min_t K[p, t, h, c],  summary[p, h, 1, c] = max_t K[p, t, h, c]
  * over the page's VALID tokens (position < seq_lens[i]).  Idempotent.
- * summary: dev [num_pool_pages, Hkv, 2, qk_dim] in the K dtype (min/max are exact). */
+ * summary: dev [num_pool_pages, Hkv, 2, qk_dim] in the K dtype (min/max are exact).
+ * VX_SUMMARY_CENTROID: summary[p, h, c] = mean_t K[p, t, h, c] over the valid tokens, computed exactly and rounded
+ * once (nearest even) to the K dtype; summary: dev [num_pool_pages, Hkv, qk_dim]. */
 vx_status vx_page_summary_update(vx_ctx *ctx, const vx_kv_pool *pool, const vx_page_table *pt,
                                  const int32_t *first_new_pos /* dev [B] or NULL */,
                                  void *summary, vx_stream stream);

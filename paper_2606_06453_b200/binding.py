@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_PKG, "libvortex_b200.so")
 VX_OK, VX_ERR_INVALID_ARG, VX_ERR_UNSUPPORTED, VX_ERR_WORKSPACE, VX_ERR_CUDA = range(5)
 VX_DT_BF16, VX_DT_F32 = 0, 1
 VX_AGG_SUM, VX_AGG_MAX = 0, 1
+VX_SUMMARY_ENVELOPE, VX_SUMMARY_CENTROID = 0, 1
 VX_STEP_UPDATE_SUMMARY = 1
 
 EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",
@@ -28,7 +29,7 @@ class VxGeom(C.Structure):
     _fields_ = [("dtype", C.c_int32), ("num_q_heads", C.c_int32), ("num_kv_heads", C.c_int32),
                 ("qk_dim", C.c_int32), ("v_dim", C.c_int32), ("page_size", C.c_int32),
                 ("kv_shared", C.c_int32), ("sm_scale", C.c_float), ("n_sink", C.c_int32),
-                ("n_local", C.c_int32), ("agg", C.c_int32)]
+                ("n_local", C.c_int32), ("agg", C.c_int32), ("summary_kind", C.c_int32)]
 
 
 class VxPageTable(C.Structure):
@@ -118,13 +119,14 @@ class Context:
     """One geometry on one device; owns its workspace tensor."""
 
     def __init__(self, *, dtype, num_q_heads, num_kv_heads, qk_dim, v_dim, page_size, sm_scale,
-                 n_sink, n_local, kv_shared=False, agg=VX_AGG_SUM, max_batch, max_total_pages,
+                 n_sink, n_local, kv_shared=False, agg=VX_AGG_SUM, summary_kind=VX_SUMMARY_ENVELOPE, max_batch,
+                 max_total_pages,
                  max_pages_per_req, max_budget, device="cuda:0"):
         self.lib = load_library()
         self.torch_dtype = dtype
         dt = {torch.bfloat16: VX_DT_BF16, torch.float32: VX_DT_F32}[dtype]
         self.geom = VxGeom(dt, num_q_heads, num_kv_heads, qk_dim, v_dim, page_size, int(kv_shared),
-                           float(sm_scale), n_sink, n_local, agg)
+                           float(sm_scale), n_sink, n_local, agg, summary_kind)
         self.device = torch.device(device)
         self.max = (int(max_batch), int(max_total_pages), int(max_pages_per_req), int(max_budget))
         need = self.lib.vx_workspace_bytes(C.byref(self.geom), *self.max)
@@ -216,7 +218,8 @@ def tables_for(w):
     return pool, pt
 
 
-def alloc_summary(w):
+def alloc_summary(w, summary_kind=VX_SUMMARY_ENVELOPE):
     s = w.spec
-    return torch.zeros(w.num_pool_pages, s.num_kv_heads, 2, s.qk_dim, dtype=w.k_pool.dtype,
-                       device=w.k_pool.device)
+    shape = (w.num_pool_pages, s.num_kv_heads, s.qk_dim) if summary_kind == VX_SUMMARY_CENTROID else \
+        (w.num_pool_pages, s.num_kv_heads, 2, s.qk_dim)
+    return torch.zeros(shape, dtype=w.k_pool.dtype, device=w.k_pool.device)

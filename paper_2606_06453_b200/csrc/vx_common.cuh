@@ -53,6 +53,18 @@ template <int N> __device__ __forceinline__ void cp_async_wait() {
   asm volatile("cp.async.wait_group %0;" ::"n"(N));
 }
 
+// round a double to the storage type once, to nearest even (the block top-k centroid, Eq.1).  The sum of
+// a page's bf16 / fp32 keys is exact in double for bf16 and correctly rounded pairwise for fp32; the oracle does the same.
+template <typename T> __device__ __forceinline__ T round_double(double x);
+template <> __device__ __forceinline__ float round_double<float>(double x) { return __double2float_rn(x); }
+template <> __device__ __forceinline__ __nv_bfloat16 round_double<__nv_bfloat16>(double x) {
+  // keep 8 significand bits of the double directly (going through float would round twice)
+  unsigned long long b = (unsigned long long)__double_as_longlong(x);
+  b += ((1ull << 44) - 1) + ((b >> 45) & 1ull);      // nearest, ties to even, at bit 45
+  b &= ~((1ull << 45) - 1);
+  return __float2bfloat16_rn(__double2float_rn(__longlong_as_double((long long)b)));   // both conversions are exact now
+}
+
 // ---- warp reductions --------------------------------------------------------------------------
 template <int WIDTH = 32> __device__ __forceinline__ float warp_sum(float v) {
 #pragma unroll

@@ -58,7 +58,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
                       const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ sel_phys,
                       const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count,
                       int max_budget, int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
-                      int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd,
+                      int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
                       __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0) {
   constexpr int ROWB = D * 2;                 // bytes per token row
   constexpr int CH = ROWB / 16;               // 16-byte chunks per row
@@ -161,6 +161,23 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
       // (exact in bf16).  Lane owns W consecutive 32-bit words (2 channels each) of the row.
       constexpr int W = ROWB / 128;
       const int byte0 = lane * W * 4, c = byte0 / 16, o16 = byte0 % 16;
+      if (summary_kind == VX_SUMMARY_CENTROID) {   // block top-k: exact mean of the valid keys, one rounding (Eq.1)
+        double sum[2 * W];
+#pragma unroll
+        for (int w = 0; w < 2 * W; ++w) sum[w] = 0.0;
+        for (int t = 0; t < valid; ++t) {
+#pragma unroll
+          for (int w = 0; w < W; ++w) {
+            const uint32_t x = *reinterpret_cast<const uint32_t*>(ring + (size_t)(p % kGqaStages) * 2 * PAGEB + t * ROWB +
+                                                                  ((c ^ (t & 7)) * 16) + o16 + w * 4);
+            sum[2 * w] += (double)__uint_as_float(x << 16);
+            sum[2 * w + 1] += (double)__uint_as_float(x & 0xffff0000u);
+          }
+        }
+        __nv_bfloat16* dstc = summary_upd + ((int64_t)phys_p * num_kv_heads + kvh) * D + lane * W * 2;
+#pragma unroll
+        for (int w = 0; w < 2 * W; ++w) dstc[w] = round_double<__nv_bfloat16>(sum[w] / (double)valid);
+      } else {
       __nv_bfloat162 lo[W], hi[W];
 #pragma unroll
       for (int w = 0; w < W; ++w) {
@@ -182,6 +199,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
       for (int w = 0; w < W; ++w) {
         *reinterpret_cast<__nv_bfloat162*>(dst + 2 * w) = lo[w];
         *reinterpret_cast<__nv_bfloat162*>(dst + D + 2 * w) = hi[w];
+      }
       }
     }
 
@@ -314,7 +332,7 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(pool.k),
       static_cast<const __nv_bfloat16*>(pool.v), pool.stride_page, pool.stride_token, pool.stride_head,
       g.num_q_heads, g.num_kv_heads, g.sm_scale * kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget,
-      splits, c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd),
+      splits, c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
       static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();

@@ -248,7 +248,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
                   float scale_log2, const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ sel_phys,
                   const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count, int max_budget,
                   int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
-                  int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd,
+                  int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
                   __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0) {
   using namespace mla;
   extern __shared__ uint8_t smem_raw[];
@@ -536,6 +536,22 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
         const int cc = hidx, a = cc >> 3;
         const uint8_t* atom = a < 8 ? sm + OFF_PAIR + ((pl * PAIRS_PER_PAGE + (a >> 1)) % N_PAIR) * PAIR_BYTES + (a & 1) * K_ATOM_BYTES
                                     : sm + OFF_ROPE + (pl % N_ROPE) * K_ATOM_BYTES;
+        if (summary_kind == VX_SUMMARY_CENTROID) {       // block top-k: exact mean of the valid latents, one rounding
+          double sum[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) sum[e] = 0.0;
+          for (int r = 0; r < valid; ++r) {
+            const uint4 v4 = *reinterpret_cast<const uint4*>(atom + (r >> 3) * 1024 + (r & 7) * 128 + (((cc & 7) ^ (r & 7)) << 4));
+            float f[8];
+            Elem<__nv_bfloat16>::unpack(v4, f);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) sum[e] += (double)f[e];
+          }
+          alignas(16) __nv_bfloat16 o8[8];
+#pragma unroll
+          for (int e = 0; e < 8; ++e) o8[e] = round_double<__nv_bfloat16>(sum[e] / (double)valid);
+          *reinterpret_cast<uint4*>(summary_upd + (int64_t)phys_list[pl] * D + cc * 8) = *reinterpret_cast<const uint4*>(o8);
+        } else {
         uint4 lo4 = *reinterpret_cast<const uint4*>(atom + ((cc & 7) << 4)), hi4 = lo4;     // token 0
         __nv_bfloat162* lo = reinterpret_cast<__nv_bfloat162*>(&lo4);
         __nv_bfloat162* hi = reinterpret_cast<__nv_bfloat162*>(&hi4);
@@ -548,6 +564,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
         __nv_bfloat16* dst = summary_upd + (int64_t)phys_list[pl] * 2 * D + cc * 8;
         *reinterpret_cast<uint4*>(dst) = lo4;
         *reinterpret_cast<uint4*>(dst + D) = hi4;
+        }
       }
     }
     // ---- epilogue (warps 2..5): O^T / l -> partial or final output ----------------------------------------
@@ -649,7 +666,7 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
   cudaError_t e = launch_kernel(decode_mla_kernel, grid, dim3(mla::THREADS), (size_t)mla::SMEM_BYTES, s, opt.pdl, kmap,
                                 static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens,
                                 sel_phys, sel_logical, sel_count, max_budget, best, c->ws.part_o, c->ws.part_lse,
-                                c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd),
+                                c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
                                 static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();

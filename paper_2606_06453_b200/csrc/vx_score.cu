@@ -70,13 +70,14 @@ struct GroupIter {
   }
 };
 
-template <typename T, int D, int PG, int HKV, int kScStages, int AGG>
+template <typename T, int D, int PG, int HKV, int kScStages, int AGG, int KIND>
 __global__ void __launch_bounds__(kScThreads, 2)
 score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int batch,
              const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices, int total_pages,
              float* __restrict__ scores, int req_begin, int req_end) {
   constexpr int PER = Elem<T>::kPerVec;
-  constexpr int ROW_ELEMS = 2 * D;               // [min | max] of one (page, KV head)
+  // envelope: [min | max] of one (page, KV head); centroid (block top-k): the mean key, d elements
+  constexpr int ROW_ELEMS = KIND == VX_SUMMARY_CENTROID ? D : 2 * D;
   constexpr int NCH = ROW_ELEMS / PER;           // 16-byte chunks per row
   constexpr int NIT = (NCH + kWarp - 1) / kWarp; // chunks per lane
   constexpr int RPW = PG * HKV / kScConsumerWarps;   // rows per warp per group
@@ -180,13 +181,19 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
             float f[PER];
             Elem<T>::unpack(v[k], f);
 #pragma unroll
-            for (int x = 0; x < PER; ++x) { qp[x] += fmaxf(f[x], 0.f); qm[x] += fminf(f[x], 0.f); }
+            for (int x = 0; x < PER; ++x) {
+              if constexpr (KIND == VX_SUMMARY_CENTROID) qp[x] += f[x];        // Eq.2: sum_h q_h . centroid = (sum_h q_h) . centroid
+              else { qp[x] += fmaxf(f[x], 0.f); qm[x] += fminf(f[x], 0.f); }
+            }
           }
         }
 #pragma unroll
         for (int x = 0; x < PER; ++x) {
-          s_q[h * ROW_ELEMS + c * PER + x] = qm[x];
-          s_q[h * ROW_ELEMS + D + c * PER + x] = qp[x];
+          if constexpr (KIND == VX_SUMMARY_CENTROID) s_q[h * ROW_ELEMS + c * PER + x] = qp[x];
+          else {
+            s_q[h * ROW_ELEMS + c * PER + x] = qm[x];
+            s_q[h * ROW_ELEMS + D + c * PER + x] = qp[x];
+          }
         }
       }
       }
@@ -306,23 +313,26 @@ bool score_geometry_supported(const vx_geom& g) {
   // MAX costs g flop per byte: CUDA cores carry it for GQA groups (g <= 8); the MLA group (g = 32) would need
   // the tensor cores for the scoring too -- not built (NEXT-1)
   if (g.agg == VX_AGG_MAX && (g.kv_shared || g.num_q_heads / hkv > 8)) return false;
+  if (g.summary_kind != VX_SUMMARY_ENVELOPE && g.summary_kind != VX_SUMMARY_CENTROID) return false;
+  if (g.summary_kind == VX_SUMMARY_CENTROID && g.agg != VX_AGG_SUM) return false;       // Eq.2 is a mean over the group
   if (hkv != 1 && hkv != 2 && hkv != 4 && hkv != 8) return false;   // a consumer warp owns one KV head
   if (g.dtype == VX_DT_BF16) return g.qk_dim == 128 || g.qk_dim == 64 || g.qk_dim == 576 || g.qk_dim == 256;
   return g.qk_dim == 64 || g.qk_dim == 128;
 }
 
-template <typename T, int D, int PG, int HKV, int AGG>
+template <typename T, int D, int PG, int HKV, int AGG, int KIND>
 static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
                                   float* scores, cudaStream_t s, const ReqRange& rr) {
   const vx_geom& g = c->g;
-  constexpr size_t page_bytes = (size_t)HKV * 2 * D * sizeof(T);
+  constexpr int ROW = KIND == VX_SUMMARY_CENTROID ? D : 2 * D;
+  constexpr size_t page_bytes = (size_t)HKV * ROW * sizeof(T);
   // as many ~16-32 KB stages as two CTAs per SM can hold (>= 3): the bytes in flight, not the math, set the rate
-  constexpr size_t q_bytes = AGG == VX_AGG_MAX ? (size_t)HKV * 8 * 2 * D * sizeof(T) : (size_t)HKV * 2 * D * sizeof(float);
+  constexpr size_t q_bytes = AGG == VX_AGG_MAX ? (size_t)HKV * 8 * ROW * sizeof(T) : (size_t)HKV * ROW * sizeof(float);
   constexpr int kScStages = (int)((110 * 1024 - q_bytes) / (PG * page_bytes)) < 3 ? 3 : ((int)((110 * 1024 - q_bytes) / (PG * page_bytes)) > 8 ? 8 : (int)((110 * 1024 - q_bytes) / (PG * page_bytes)));
   constexpr size_t smem = kScStages * PG * page_bytes + q_bytes;
   static bool attr_set = false;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(score_kernel<T, D, PG, HKV, kScStages, AGG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(score_kernel<T, D, PG, HKV, kScStages, AGG, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
@@ -331,33 +341,45 @@ static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summar
   const int64_t est_pages = rr.count < 0 ? pt.total_pages : (int64_t)pt.total_pages * rr.count / (pt.batch > 0 ? pt.batch : 1) + 1;
   if ((int64_t)ctas * min_pages > est_pages) ctas = (int)((est_pages + min_pages - 1) / min_pages);
   if (ctas < 1) ctas = 1;
-  score_kernel<T, D, PG, HKV, kScStages, AGG><<<ctas, kScThreads, smem, s>>>(
+  score_kernel<T, D, PG, HKV, kScStages, AGG, KIND><<<ctas, kScThreads, smem, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, pt.batch, pt.page_indptr,
       pt.page_indices, pt.total_pages, scores, rr.begin, rr.begin + (rr.count < 0 ? pt.batch : rr.count));
   c->launches += 1;
   return cudaGetLastError();
 }
 
-template <typename T, int D, int PG, int HKV>
+template <typename T, int D, int PG, int HKV, int KIND>
 static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
                                   float* scores, cudaStream_t s, const ReqRange& rr) {
-  if (c->g.agg == VX_AGG_MAX) return launch_score_agg<T, D, PG, HKV, VX_AGG_MAX>(c, q, summary, pt, scores, s, rr);
-  return launch_score_agg<T, D, PG, HKV, VX_AGG_SUM>(c, q, summary, pt, scores, s, rr);
+  if constexpr (KIND == VX_SUMMARY_ENVELOPE) {
+    if (c->g.agg == VX_AGG_MAX) return launch_score_agg<T, D, PG, HKV, VX_AGG_MAX, KIND>(c, q, summary, pt, scores, s, rr);
+  }
+  return launch_score_agg<T, D, PG, HKV, VX_AGG_SUM, KIND>(c, q, summary, pt, scores, s, rr);
 }
 
-// PG pages per stage so that a stage is ~32 KB and every consumer warp gets 1..8 rows of it
+constexpr int pow2_floor(int x) { int p = 1; while (2 * p <= x) p *= 2; return p; }
+constexpr int clamp_int(int x, int lo, int hi) { return x < lo ? lo : (x > hi ? hi : x); }
+
+// PG pages per stage so that a stage is ~32 KB and every consumer warp gets 1, 2, 4 or 8 rows of it
+template <typename T, int D, int KIND>
+static cudaError_t launch_score_k(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
+                                  float* scores, cudaStream_t s, const ReqRange& rr) {
+  constexpr int row_bytes = (KIND == VX_SUMMARY_CENTROID ? D : 2 * D) * (int)sizeof(T);
+  constexpr int rows32k = pow2_floor(32768 / row_bytes < 8 ? 8 : 32768 / row_bytes);     // rows per ~32 KB stage, >= 8
+  switch (c->g.num_kv_heads) {                   // rows per stage = PG * HKV in [8, 64] (1..8 rows per consumer warp)
+    case 8: return launch_score_t<T, D, clamp_int(rows32k, 8, 64) / 8, 8, KIND>(c, q, summary, pt, scores, s, rr);
+    case 4: return launch_score_t<T, D, clamp_int(rows32k, 8, 64) / 4, 4, KIND>(c, q, summary, pt, scores, s, rr);
+    case 2: return launch_score_t<T, D, clamp_int(rows32k, 8, 64) / 2, 2, KIND>(c, q, summary, pt, scores, s, rr);
+    case 1: return launch_score_t<T, D, clamp_int(rows32k, 8, 32), 1, KIND>(c, q, summary, pt, scores, s, rr);
+  }
+  return cudaErrorInvalidValue;
+}
+
 template <typename T, int D>
 static cudaError_t launch_score_d(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
                                   float* scores, cudaStream_t s, const ReqRange& rr) {
-  constexpr int row_bytes = 2 * D * (int)sizeof(T);
-  constexpr int pg8 = 32768 / (8 * row_bytes) < 1 ? 1 : 32768 / (8 * row_bytes);   // Hkv = 8
-  switch (c->g.num_kv_heads) {
-    case 8: return launch_score_t<T, D, (pg8 > 8 ? 8 : pg8), 8>(c, q, summary, pt, scores, s, rr);
-    case 4: return launch_score_t<T, D, (2 * pg8 > 16 ? 16 : 2 * pg8), 4>(c, q, summary, pt, scores, s, rr);
-    case 2: return launch_score_t<T, D, (4 * pg8 > 32 ? 32 : (4 * pg8 < 4 ? 4 : 4 * pg8)), 2>(c, q, summary, pt, scores, s, rr);
-    case 1: return launch_score_t<T, D, (8 * pg8 > 32 ? 32 : (8 * pg8 < 8 ? 8 : 8 * pg8)), 1>(c, q, summary, pt, scores, s, rr);
-  }
-  return cudaErrorInvalidValue;
+  if (c->g.summary_kind == VX_SUMMARY_CENTROID) return launch_score_k<T, D, VX_SUMMARY_CENTROID>(c, q, summary, pt, scores, s, rr);
+  return launch_score_k<T, D, VX_SUMMARY_ENVELOPE>(c, q, summary, pt, scores, s, rr);
 }
 
 cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,

@@ -10,7 +10,7 @@
 
 namespace vx {
 
-template <typename T, int UNROLL>
+template <typename T, int UNROLL, int KIND>
 __global__ void __launch_bounds__(256)
 summary_kernel(const T* __restrict__ k, int64_t stride_page, int64_t stride_token, int64_t stride_head,
                int num_kv_heads, int qk_dim, int page_size, int batch,
@@ -46,6 +46,36 @@ summary_kernel(const T* __restrict__ k, int64_t stride_page, int64_t stride_toke
     const int64_t phys = page_indices[page_indptr[i] + j];
     const T* src = k + phys * stride_page + h * stride_head + (int64_t)v * PER;
 
+    if constexpr (KIND == VX_SUMMARY_CENTROID) {       // mean of the valid keys, one rounding (exact double sums)
+      double sum[PER];
+#pragma unroll
+      for (int e = 0; e < PER; ++e) sum[e] = 0.0;
+      int t = 0;
+      for (; t + UNROLL <= valid; t += UNROLL) {
+        uint4 raw[UNROLL];
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u) raw[u] = ldg_stream(src + (int64_t)(t + u) * stride_token);
+#pragma unroll
+        for (int u = 0; u < UNROLL; ++u) {
+          float f[PER];
+          Elem<T>::unpack(raw[u], f);
+#pragma unroll
+          for (int e = 0; e < PER; ++e) sum[e] += (double)f[e];
+        }
+      }
+      for (; t < valid; ++t) {
+        float f[PER];
+        Elem<T>::unpack(ldg_stream(src + (int64_t)t * stride_token), f);
+#pragma unroll
+        for (int e = 0; e < PER; ++e) sum[e] += (double)f[e];
+      }
+      T* dst = summary + (phys * num_kv_heads + h) * (int64_t)qk_dim + (int64_t)v * PER;
+      alignas(16) T outv[PER];
+#pragma unroll
+      for (int e = 0; e < PER; ++e) outv[e] = round_double<T>(sum[e] / (double)valid);
+      *reinterpret_cast<uint4*>(dst) = *reinterpret_cast<const uint4*>(outv);
+      continue;
+    }
     float lo_v[PER], hi_v[PER];
 #pragma unroll
     for (int e = 0; e < PER; ++e) { lo_v[e] = INFINITY; hi_v[e] = -INFINITY; }
@@ -90,10 +120,16 @@ static cudaError_t launch_summary_t(vx_ctx* c, const vx_kv_pool& pool, const vx_
   int64_t blocks = (items + threads - 1) / threads;
   const int64_t cap = (int64_t)c->num_sms * 32;       // grid-stride beyond 32 CTAs per SM
   if (blocks > cap) blocks = cap;
-  summary_kernel<T, 8><<<(unsigned)blocks, threads, 0, s>>>(
-      static_cast<const T*>(pool.k), pool.stride_page, pool.stride_token, pool.stride_head,
-      g.num_kv_heads, g.qk_dim, g.page_size, pt.batch, pt.page_indptr, pt.page_indices, pt.seq_lens,
-      first_new_pos, append_only, slots, static_cast<T*>(summary));
+  if (g.summary_kind == VX_SUMMARY_CENTROID)
+    summary_kernel<T, 8, VX_SUMMARY_CENTROID><<<(unsigned)blocks, threads, 0, s>>>(
+        static_cast<const T*>(pool.k), pool.stride_page, pool.stride_token, pool.stride_head,
+        g.num_kv_heads, g.qk_dim, g.page_size, pt.batch, pt.page_indptr, pt.page_indices, pt.seq_lens,
+        first_new_pos, append_only, slots, static_cast<T*>(summary));
+  else
+    summary_kernel<T, 8, VX_SUMMARY_ENVELOPE><<<(unsigned)blocks, threads, 0, s>>>(
+        static_cast<const T*>(pool.k), pool.stride_page, pool.stride_token, pool.stride_head,
+        g.num_kv_heads, g.qk_dim, g.page_size, pt.batch, pt.page_indptr, pt.page_indices, pt.seq_lens,
+        first_new_pos, append_only, slots, static_cast<T*>(summary));
   c->launches += 1;
   return cudaGetLastError();
 }
