@@ -86,6 +86,10 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   constexpr int STAGE_BYTES = PG * PAGE_BYTES;
   static_assert(ROW_ELEMS % PER == 0 && kScConsumerWarps % HKV == 0, "shape");
   static_assert(RPW == 1 || RPW == 2 || RPW == 4 || RPW == 8, "rows per warp must be a power of two <= 8");
+  // rows narrower than a warp-wide 512-byte read (256 B centroid rows, d = 64 envelopes): NCH lanes per row, 32 / NCH
+  // rows per instruction, so that no lane idles
+  constexpr int RPI = NCH < kWarp ? kWarp / NCH : 1;
+  constexpr bool NARROW = AGG == VX_AGG_SUM && (NCH == 8 || NCH == 16) && RPW % RPI == 0;
 
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ __align__(8) uint64_t s_full[kScStages], s_empty[kScStages];
@@ -202,7 +206,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
       if constexpr (AGG == VX_AGG_SUM) {
 #pragma unroll
         for (int t = 0; t < NIT; ++t) {
-          const int c = lane + t * kWarp;
+          const int c = NARROW ? lane % NCH : lane + t * kWarp;
 #pragma unroll
           for (int e = 0; e < PER; ++e) qreg[t][e] = (NCH % kWarp == 0 || c < NCH) ? s_q[kvh * ROW_ELEMS + c * PER + e] : 0.f;
         }
@@ -210,6 +214,31 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     }
     sc_mbar_wait(smem_u32(&s_full[s]), (g / kScStages) & 1);
     const int rows = count * HKV;                // row r = page (r / HKV), head (r % HKV)
+    if constexpr (NARROW) {
+      constexpr int KIT = RPW / RPI;             // instructions per group; instruction i covers rows warp + 8 (i RPI + lane / NCH)
+      const uint8_t* st = smem + (size_t)s * STAGE_BYTES + (lane % NCH) * 16;
+      uint4 vn[KIT];
+#pragma unroll
+      for (int i = 0; i < KIT; ++i) {
+        const int r = warp + (i * RPI + lane / NCH) * kScConsumerWarps;
+        vn[i] = r < rows ? *reinterpret_cast<const uint4*>(st + r * ROW_BYTES) : make_uint4(0, 0, 0, 0);
+      }
+      __syncwarp();
+      if (lane == 0) sc_mbar_arrive(smem_u32(&s_empty[s]));  // stage consumed: its rows are in registers
+#pragma unroll
+      for (int i = 0; i < KIT; ++i) {
+        float f[PER];
+        Elem<T>::unpack(vn[i], f);
+        float acc = 0.f;
+#pragma unroll
+        for (int e = 0; e < PER; ++e) acc = fmaf(qreg[0][e], f[e], acc);
+#pragma unroll
+        for (int o = NCH / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);   // sum over the row's NCH lanes
+        const int r = warp + (i * RPI + lane / NCH) * kScConsumerWarps;
+        if (lane % NCH == 0 && r < rows) scores[(int64_t)kvh * total_pages + first + r / HKV] = acc;
+      }
+      continue;
+    }
     const uint8_t* stage = smem + (size_t)s * STAGE_BYTES + lane * 16;
     uint4 v[RPW][NIT];
 #pragma unroll
