@@ -110,7 +110,6 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   __syncthreads();
   pdl_trigger();                                // single-wave persistent grid: the selection kernel may queue up behind us
   if (begin >= end) return;
-  GroupIter it(begin, end, batch, page_indptr);
   int first, count, req;
 
   if (warp == kScConsumerWarps) {
@@ -120,6 +119,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     int chunk0 = begin;                                   // flat index of id_cur's lane 0
     int id_cur = chunk0 + lane < end ? page_indices[chunk0 + lane] : 0;
     int id_nxt = chunk0 + kWarp + lane < end ? page_indices[chunk0 + kWarp + lane] : 0;
+    GroupIter it(begin, end, batch, page_indptr);         // (its loads fly together with the id loads above)
     for (int g = 0; it.next(PG, first, count, req); ++g) {
       const int s = g % kScStages;
       if (g >= kScStages) sc_mbar_wait(smem_u32(&s_empty[s]), ((g / kScStages) - 1) & 1);
@@ -143,6 +143,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   }
 
   // ---- consumers: warp w owns KV head w % HKV and rows w + 8k of every group ---------------------
+  GroupIter it(begin, end, batch, page_indptr);
   const int grp = num_q_heads / HKV;
   const int kvh = warp % HKV;
   float qreg[NIT][PER];
@@ -165,6 +166,46 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
             s_qh[h * ROW_ELEMS + D + c * PER + x] = Elem<T>::from_float(fmaxf(f[x], 0.f));
           }
         }
+      } else if constexpr (HKV == 1) {
+        // one latent head shared by a large group (MLA, g = 32): three thread groups take a third of the heads each, so
+        // that every load of the rebuild is in flight at once (one memory latency, not g / 8); the partial sums are
+        // added in a fixed order (deterministic)
+        constexpr int NV1 = D / PER, GS = 3, HMAX = 11;              // up to 33 heads
+        float* s_part = s_q + ROW_ELEMS;                              // [GS][ROW_ELEMS]
+        const int e = threadIdx.x;
+        if (e < GS * NV1) {
+          const int gi = e / NV1, c = e % NV1;
+          const int per = (grp + GS - 1) / GS, h0 = gi * per, h1 = min(h0 + per, grp);
+          const T* qbase = q + ((int64_t)req * num_q_heads + h0) * D + c * PER;
+          uint4 v[HMAX];
+#pragma unroll
+          for (int k = 0; k < HMAX; ++k)
+            v[k] = h0 + k < h1 ? *reinterpret_cast<const uint4*>(qbase + (int64_t)k * D) : make_uint4(0, 0, 0, 0);
+          float qp[PER], qm[PER];
+#pragma unroll
+          for (int x = 0; x < PER; ++x) { qp[x] = 0.f; qm[x] = 0.f; }
+#pragma unroll
+          for (int k = 0; k < HMAX; ++k) {
+            float f[PER];
+            Elem<T>::unpack(v[k], f);
+#pragma unroll
+            for (int x = 0; x < PER; ++x) {
+              if constexpr (KIND == VX_SUMMARY_CENTROID) qp[x] += f[x];
+              else { qp[x] += fmaxf(f[x], 0.f); qm[x] += fminf(f[x], 0.f); }
+            }
+          }
+#pragma unroll
+          for (int x = 0; x < PER; ++x) {
+            if constexpr (KIND == VX_SUMMARY_CENTROID) s_part[gi * ROW_ELEMS + c * PER + x] = qp[x];
+            else {
+              s_part[gi * ROW_ELEMS + c * PER + x] = qm[x];
+              s_part[gi * ROW_ELEMS + D + c * PER + x] = qp[x];
+            }
+          }
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
+        for (int x = threadIdx.x; x < ROW_ELEMS; x += kScConsumerWarps * kWarp)
+          s_q[x] = (s_part[x] + s_part[ROW_ELEMS + x]) + s_part[2 * ROW_ELEMS + x];
       } else {
       // one thread per (KV head, 16-byte channel vector); the group's heads are read 8 at a time with all
       // loads of a batch in flight together (a head-by-head loop costs one memory latency per head)
@@ -356,7 +397,8 @@ static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summar
   constexpr int ROW = KIND == VX_SUMMARY_CENTROID ? D : 2 * D;
   constexpr size_t page_bytes = (size_t)HKV * ROW * sizeof(T);
   // as many ~16-32 KB stages as two CTAs per SM can hold (>= 3): the bytes in flight, not the math, set the rate
-  constexpr size_t q_bytes = AGG == VX_AGG_MAX ? (size_t)HKV * 8 * ROW * sizeof(T) : (size_t)HKV * ROW * sizeof(float);
+  constexpr size_t q_bytes = AGG == VX_AGG_MAX ? (size_t)HKV * 8 * ROW * sizeof(T)
+                                               : (size_t)HKV * ROW * sizeof(float) * (HKV == 1 ? 4 : 1);   // HKV 1: + 3 partial rows
   constexpr int kScStages = (int)((110 * 1024 - q_bytes) / (PG * page_bytes)) < 3 ? 3 : ((int)((110 * 1024 - q_bytes) / (PG * page_bytes)) > 8 ? 8 : (int)((110 * 1024 - q_bytes) / (PG * page_bytes)));
   constexpr size_t smem = kScStages * PG * page_bytes + q_bytes;
   static bool attr_set = false;
