@@ -53,7 +53,7 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
   __shared__ int s_wsum[WARPS];
   __shared__ int2 s_wcnt[WARPS];
   __shared__ int s_bin, s_above, s_cnt, s_nlist, s_need_eq;
-  __shared__ uint32_t s_thr;
+  __shared__ uint32_t s_thr, s_bmin, s_bmax;
 
   const int kvh = blockIdx.x, i = blockIdx.y + req0;
   const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
@@ -104,13 +104,21 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
     uint32_t lo = kmin;
     uint64_t width = (uint64_t)(kmax - kmin) + 1;
     int shift = max(0, (32 - __clz(kmax - kmin)) - kBinBits);     // ((kmax - kmin) >> shift) < kBins
+    // First pass in the FLOAT domain: bin = floor((score - min) * 2048 / (max - min)) is monotone in the score, and
+    // unlike the integer key it is linear across the sign change and across exponents -- a request whose scores
+    // straddle zero (centroid scores, bimodal distributions) would otherwise spend its first pass on a few coarse
+    // bins.  The members of one float bin are a contiguous key interval, so deeper passes continue on integer keys.
+    const float smin = key_to_float(kmin), smax = key_to_float(kmax);
+    const float fscale = (float)kBins / (smax - smin);
+    bool fpass = kmax > kmin && isfinite(fscale) && fscale > 0.f;
+    auto fbin = [&](uint32_t key) -> int { return min(kBins - 1, (int)((key_to_float(key) - smin) * fscale)); };
 #pragma unroll 1
     while (true) {
       for (int b = tid; b < kBins; b += THREADS) s_hist[b] = 0;
       __syncthreads();
       for (int j = tid; j < n_pages; j += THREADS) {
         const uint32_t key = key_at(j);
-        if (key != kForcedKey && key >= lo && (uint64_t)(key - lo) < width) atomicAdd(&s_hist[(key - lo) >> shift], 1);
+        if (key != kForcedKey && key >= lo && (uint64_t)(key - lo) < width) atomicAdd(&s_hist[fpass ? fbin(key) : (int)((key - lo) >> shift)], 1);
       }
       __syncthreads();
       // threshold bin: the highest b with  #keys in bins > b  <  need  <=  #keys in bins >= b
@@ -137,6 +145,40 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
       __syncthreads();
       const int bin = s_bin, cnt = s_cnt;
       need -= s_above;                          // still to take from the threshold bin
+      if (fpass) {                              // float pass: rank the bin's members, or continue on its key interval
+        if (tid == 0) { s_bmin = 0xFFFFFFFFu; s_bmax = 0u; }
+        __syncthreads();
+        for (int j = tid; j < n_pages; j += THREADS) {
+          const uint32_t key = key_at(j);
+          if (key != kForcedKey && fbin(key) == bin) {
+            if (cnt <= kList) s_list[atomicAdd(&s_nlist, 1)] = key;
+            else { atomicMin(&s_bmin, key); atomicMax(&s_bmax, key); }
+          }
+        }
+        __syncthreads();
+        if (cnt <= kList) {
+          if (tid < cnt) {
+            const uint32_t mykey = s_list[tid];
+            int gt = 0, ge = 0;
+            for (int j = 0; j < cnt; ++j) {
+              const uint32_t o = s_list[j];
+              gt += o > mykey;
+              ge += o >= mykey;
+            }
+            if (gt < need && need <= ge) { s_thr = mykey; s_need_eq = need - gt; }
+          }
+          __syncthreads();
+          thr = s_thr;
+          need_eq = s_need_eq;
+          break;
+        }
+        lo = s_bmin;                            // heavy bin: its members are exactly the keys in [bmin, bmax]
+        width = (uint64_t)(s_bmax - s_bmin) + 1;
+        shift = max(0, (32 - __clz(s_bmax - s_bmin)) - kBinBits);
+        fpass = false;
+        __syncthreads();
+        continue;
+      }
       const uint32_t bin_lo = lo + ((uint32_t)bin << shift);
       if (shift == 0) {                         // the bin is one key value: take the first `need` by index
         thr = bin_lo;

@@ -1,0 +1,91 @@
+"""Top-k microbenchmark on the score distributions of the paper's App. D.2/D.3 (bimodal,
+normal, lognormal, uniform): times vx_topk_pages alone on synthetic page scores and checks every result against
+torch.topk (set equality; ties are measure-zero for these draws).
+
+The paper reports its radix_topk as "highly sensitive to the score distribution" (:194); the select here bins
+the LIVE key range of each problem, so the four distributions should cost the same.
+
+    python -m paper_2606_06453_b200.topk_microbench [--batch 32] [--heads 8] [--iters 50]
+"""
+from __future__ import annotations
+
+import argparse
+import json
+
+import torch
+
+from . import binding as vx
+
+
+def draw(dist: str, shape, gen, device):
+    if dist == "normal":
+        return torch.randn(shape, generator=gen, device=device) * 32.0 + 900.0
+    if dist == "uniform":
+        return torch.rand(shape, generator=gen, device=device) * 100.0
+    if dist == "lognormal":
+        return torch.exp(torch.randn(shape, generator=gen, device=device) * 1.5)
+    if dist == "bimodal":
+        pick = torch.rand(shape, generator=gen, device=device) < 0.1
+        return torch.where(pick, torch.randn(shape, generator=gen, device=device) * 2.0 + 40.0,
+                           torch.randn(shape, generator=gen, device=device) * 2.0 - 10.0)
+    raise ValueError(dist)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--batch", type=int, default=32)
+    ap.add_argument("--heads", type=int, default=8)
+    ap.add_argument("--iters", type=int, default=50)
+    args = ap.parse_args()
+    dev = "cuda:0"
+    gen = torch.Generator(device=dev).manual_seed(77)
+    B, H = args.batch, args.heads
+    rows = []
+    for P in (2048, 8192, 32768):
+        for k in (32, 128, 256):
+            T = B * P
+            ctx = vx.Context(dtype=torch.bfloat16, num_q_heads=4 * H, num_kv_heads=H, qk_dim=128, v_dim=128, page_size=16,
+                             sm_scale=1.0, n_sink=1, n_local=2, max_batch=B, max_total_pages=T, max_pages_per_req=P,
+                             max_budget=k, device=dev)
+            indptr = (torch.arange(B + 1, dtype=torch.int32, device=dev) * P)
+            indices = torch.randperm(T, generator=gen, device=dev).to(torch.int32)
+            seq = torch.full((B,), P * 16, dtype=torch.int32, device=dev)
+            pt = vx.PageTable(indptr, indices, seq, T, P)
+            budget = torch.full((B,), k, dtype=torch.int32, device=dev)
+            sp = torch.empty(B, H, k, dtype=torch.int32, device=dev)
+            sl = torch.empty_like(sp)
+            sc = torch.empty(B, H, dtype=torch.int32, device=dev)
+            for dist in ("bimodal", "normal", "lognormal", "uniform"):
+                scores = draw(dist, (H, T), gen, dev)
+                ctx.topk_pages(scores, pt, budget, k, sp, sl, sc)
+                torch.cuda.synchronize()
+                # exactness: forced pages + the k - 3 best of the rest, as a set per problem
+                s3 = scores.view(H, B, P).permute(1, 0, 2).clone()
+                s3[:, :, 0] = float("inf"); s3[:, :, P - 2:] = float("inf")
+                want = torch.topk(s3, k, dim=-1).indices.sort(-1).values
+                assert torch.equal(sl.long(), want), (P, k, dist)
+                # device time: `iters` back-to-back launches replayed as ONE CUDA graph (the C ABI is capturable:
+                # no host sync, no device->host reads), so the host's per-call cost does not starve the GPU
+                graph = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(graph):
+                    for _ in range(args.iters):
+                        ctx.topk_pages(scores, pt, budget, k, sp, sl, sc)
+                graph.replay()
+                torch.cuda.synchronize()
+                a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a.record(); graph.replay(); b.record()
+                torch.cuda.synchronize()
+                us = a.elapsed_time(b) * 1e3 / args.iters
+                assert torch.equal(sl.long(), want), (P, k, dist, "after graph replay")
+                rows.append(dict(pages=P, k=k, dist=dist, problems=B * H, us=round(us, 2)))
+                print(json.dumps(rows[-1]))
+            ctx.close()
+    by = {}
+    for r in rows:
+        by.setdefault((r["pages"], r["k"]), []).append(r["us"])
+    worst = max(max(v) / min(v) for v in by.values())
+    print(json.dumps({"max_spread_across_distributions": round(worst, 3)}))
+
+
+if __name__ == "__main__":
+    main()
