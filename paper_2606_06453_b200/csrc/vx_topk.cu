@@ -78,10 +78,19 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
   const bool cached = n_pages <= smem_keys;
   // ---- keys, and the min / max key of the non-forced pages ------------------------------------
   uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
-  for (int j = tid; j < n_pages; j += THREADS) {
-    const uint32_t key = page_key(sc, j, n_pages, n_sink, n_local);
-    if (cached) s_keys[j] = key;
-    if (key != kForcedKey) { kmin = min(kmin, key); kmax = max(kmax, key); }
+  for (int j0 = tid; j0 < n_pages; j0 += 8 * THREADS) {          // 8 independent loads in flight per thread
+    float v[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) v[u] = j0 + u * THREADS < n_pages ? sc[j0 + u * THREADS] : 0.f;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) {
+      const int j = j0 + u * THREADS;
+      if (j < n_pages) {
+        const uint32_t key = page_forced(j, n_pages, n_sink, n_local) ? kForcedKey : float_to_key(v[u]);
+        if (cached) s_keys[j] = key;
+        if (key != kForcedKey) { kmin = min(kmin, key); kmax = max(kmax, key); }
+      }
+    }
   }
   kmin = __reduce_min_sync(0xffffffffu, kmin);
   kmax = __reduce_max_sync(0xffffffffu, kmax);
@@ -110,7 +119,9 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
     // bins.  The members of one float bin are a contiguous key interval, so deeper passes continue on integer keys.
     const float smin = key_to_float(kmin), smax = key_to_float(kmax);
     const float fscale = (float)kBins / (smax - smin);
-    bool fpass = kmax > kmin && isfinite(fscale) && fscale > 0.f;
+    // (only when the key range spans the sign change or several exponents -- >= 2^25 key steps; a narrow range is
+    //  already linear enough in the integer key and its pass is ~1 us cheaper)
+    bool fpass = kmax - kmin >= (1u << 25) && isfinite(fscale) && fscale > 0.f;
     auto fbin = [&](uint32_t key) -> int { return min(kBins - 1, (int)((key_to_float(key) - smin) * fscale)); };
 #pragma unroll 1
     while (true) {
