@@ -11,6 +11,10 @@
 // of the group on N = 8), which keeps the instruction stream ~8x below the CUDA-core formulation
 // and the kernel on the bandwidth roofline; the softmax (exp2, running max / sum) is fp32 in
 // registers, P is rounded to bf16 for the second MMA.
+// The splits of a (request, KV head) merge in-kernel: the last split CTA to arrive (a self-resetting
+// atomic counter) merges the partials by LSE.  In the fused step the warp that stages the request's
+// newest page also rebuilds that page's summary (min / max, or the block top-k centroid) from shared
+// memory (a1): the newest page is a forced local page, so no separate launch is needed.
 #include "vx_common.cuh"
 #include "vx_internal.h"
 

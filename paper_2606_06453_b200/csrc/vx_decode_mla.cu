@@ -18,17 +18,19 @@
 //               shared-memory layout both MMAs consume (K-major B operand of S, MN-major A operand of O^T).
 //               The ring is managed per BOX PAIR (16 KB = 128 value channels): 12 pair slots + 3 RoPE slots
 //               = 3 pages, each slot released by the tcgen05.commit of the last MMA that reads it.
-//   warp 1      MMA issuer (one elected lane, polling): PV(p) goes out the moment P(p) is ready, QK of the
-//               following pages box pair by box pair as the tiles land.  S (64 columns) and O^T
-//               (512 x 32 fp32) lives in TMEM for the whole CTA.
+//   warp 1      QK issuer (one elected lane): once S is free and page p has landed (ONE full barrier per page), the
+//               36 MMAs of S(p) go out back to back.  warp 6, the PV issuer, sends the 16 MMAs of O^T += V(p)^T P(p)^T
+//               the moment P(p) is written, and its commits free the page's slots.  Both wait on their mbarriers in a
+//               fixed order with blocking waits: one warp polling several barriers (~150 cycles per test_wait) was
+//               the kernel's bound.  S (64 columns), Q (288) and O^T (128 columns, 512 x 32 fp32) live in TMEM.
 //   warp 4      softmax (TMEM lanes 0..31 = heads): tcgen05.ld S, thread-local max / exp2 / sum, P row (bf16,
 //               128 B) to shared memory as the B operand of PV, double-buffered.  O^T is rescaled lazily (only
 //               when a head's running max grows by more than 2^8): the softmax warp publishes the factors,
 //               warps 2, 3, 5 rescale the TMEM lanes it cannot reach.
 //   warps 2..5  epilogue: O^T / l -> partial or final output.
 // Splits of a request merge in-kernel (the last split to arrive merges by LSE).  In the
-// fused step the CTA holding the request's newest page also rebuilds that page's min / max summary from
-// the staged tile (a1; the newest page is a forced local page).
+// fused step the CTA holding the request's newest page also rebuilds that page's summary (min / max, or the
+// block top-k centroid) from the staged tile (a1; the newest page is a forced local page).
 #include <cuda.h>
 
 #include "vx_common.cuh"

@@ -1,20 +1,23 @@
-// vx_score.cu -- (a2) query-to-page scores from the min/max summaries.
-// PAPER.md:552  u[h,j] = sum_c max(q_h[c]*M_j[c], q_h[c]*m_j[c]);  :92 / :119 aggregated over the
-// query heads of one KV head by SUM (reading G2).
+// vx_score.cu -- (a2) query-to-page scores from the page summaries.
+// Envelope summaries (Quest): PAPER.md:552  u[h,j] = sum_c max(q_h[c]*M_j[c], q_h[c]*m_j[c]);  :92 / :119 aggregated
+// over the query heads of one KV head by SUM (reading G2) or, for GQA groups, by MAX (:556).
+// Centroid summaries (block top-k): Eq.2  s[j] = sum_h q_h . centroid_j.
 //
 // With SUM the per-head maxima collapse exactly (max(q*M, q*m) = max(q,0)*M + min(q,0)*m, M >= m):
 //     S[kvh,j] = [Qm | Qp] . [m_j | M_j],   Qp = sum_h max(q_h,0),  Qm = sum_h min(q_h,0)
-// i.e. one fp32 dot product per summary row: 1 flop per byte, a pure HBM stream of 2*d*esz bytes per
-// (page, KV head), gathered through the page table.
+// i.e. one fp32 dot product per summary row (centroid: Qsum . centroid_j): 1 flop per byte, a pure HBM stream of
+// 2*d*esz (centroid: d*esz) bytes per (page, KV head), gathered through the page table.
 //
-// Persistent kernel, one CTA per SM.  The summary pool is [N_pool, Hkv, 2, d], so all KV heads of a
-// page are ONE contiguous chunk (4 KB at Hkv=8, d=128 bf16): a producer warp gathers PG pages per
-// stage with cp.async.bulk (TMA bulk copy, completion on an mbarrier) into a 4-stage shared-memory
-// ring (~128 KB in flight per SM, no registers or LSU slots spent on the gather); 8 consumer warps
-// read rows from shared memory conflict-free (a warp reads one whole row per instruction), multiply
-// with their register-resident slice of [Qm | Qp] and reduce with a transposed shuffle butterfly.
-// Every CTA walks a contiguous range of the flat (ragged) page list, cut into groups
-// that never straddle a request, so producer and consumers derive the same schedule independently.
+// Persistent kernel, two CTAs per SM.  All KV heads of a page are ONE contiguous chunk of the summary pool (4 KB
+// at Hkv=8, d=128 bf16): a producer warp gathers PG pages per stage with cp.async.bulk (TMA bulk copy, completion
+// on an mbarrier) into a 3..8-stage shared-memory ring sized to the shared-memory budget (no registers or LSU
+// slots spent on the gather; the physical ids are prefetched 32 at a time); 8 consumer warps read rows from
+// shared memory conflict-free (a warp reads one whole row per instruction -- two or four rows when a row is
+// narrower than 512 bytes), multiply with their register-resident slice of the query vector and reduce with a
+// shuffle butterfly.  Every CTA walks a contiguous range of the flat (ragged) page list, cut into
+// groups that never straddle a request, so producer and consumers derive the same schedule independently; the
+// request of the first page is found with independent strided loads (not a dependent binary search) and the
+// query vector of a request is rebuilt with all its loads in flight at once.
 #include "vx_common.cuh"
 #include "vx_internal.h"
 

@@ -1,4 +1,5 @@
-// vx_summary.cu -- (a1) page summaries: channel-wise min / max of the keys of a page.
+// vx_summary.cu -- (a1) page summaries: channel-wise min / max of the keys of a page (Quest envelope),
+// or their mean rounded once to the KV dtype (block top-k centroid, Eq.1).
 // PAPER.md:546 "feature-wise key envelope k_j^max, k_j^min"; :89 query-independent; :529 per block.
 //
 // HBM-bound streaming kernel.  One thread owns one 16-byte channel vector of one (page, KV head)

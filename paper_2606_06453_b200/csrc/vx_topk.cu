@@ -8,12 +8,16 @@
 // the min / max key of the non-forced pages and histograms (key - min) >> shift into 2048 bins that
 // span exactly that range, so one pass resolves 11 bits of the LIVE range (page scores of one request
 // cluster in a few exponent values; a fixed MSB-first digit would spend its first passes on bits that
-// are identical for every page).  The bin that holds the k-th key usually has a handful of members:
+// are identical for every page).  When the range spans the sign change or several exponents the first
+// pass bins in the float domain instead (monotone in the score, linear across exponents), and deeper
+// passes continue on the integer keys of the chosen bin.  The bin that holds the k-th key usually has a
+// handful of members:
 // they are ranked directly (all-pairs count in shared memory); only if it holds more than kList keys
 // (heavy ties) the select recurses into that bin, 11 more bits per pass, down to single key values.
 // The result is the exact threshold key and how many keys equal to it are taken; the ordered emission
 // then resolves ties to the lowest logical index and writes ids in ascending logical order (so the
-// partial last page comes last) together with the physical page ids.
+// partial last page comes last); the selected ids are staged in shared memory and the physical ids
+// gathered from the page table in one parallel pass.
 // Integer work on a few KB per problem -- latency-bound, not bandwidth-bound.
 #include <cstdlib>
 
