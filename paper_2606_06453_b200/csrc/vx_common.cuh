@@ -80,6 +80,7 @@ template <int WIDTH = 32> __device__ __forceinline__ float warp_max(float v) {
 // ---- order-preserving float <-> uint32 key (larger float <=> larger key) ---------------------
 __device__ __forceinline__ uint32_t float_to_key(float f) {
   uint32_t u = __float_as_uint(f);
+  if (u == 0x80000000u) u = 0u;                  // -0.0 == +0.0: one key, so the tie goes to the lower index
   return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
 }
 
