@@ -393,6 +393,9 @@ bool score_geometry_supported(const vx_geom& g) {
   return g.qk_dim == 64 || g.qk_dim == 128;
 }
 
+constexpr int pow2_floor(int x) { int p = 1; while (2 * p <= x) p *= 2; return p; }
+constexpr int clamp_int(int x, int lo, int hi) { return x < lo ? lo : (x > hi ? hi : x); }
+
 template <typename T, int D, int PG, int HKV, int AGG, int KIND>
 static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
                                   float* scores, cudaStream_t s, const ReqRange& rr) {
@@ -402,7 +405,10 @@ static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summar
   // as many ~16-32 KB stages as two CTAs per SM can hold (>= 3): the bytes in flight, not the math, set the rate
   constexpr size_t q_bytes = AGG == VX_AGG_MAX ? (size_t)HKV * 8 * ROW * sizeof(T)
                                                : (size_t)HKV * ROW * sizeof(float) * (HKV == 1 ? 4 : 1);   // HKV 1: + 3 partial rows
-  constexpr int kScStages = (int)((110 * 1024 - q_bytes) / (PG * page_bytes)) < 3 ? 3 : ((int)((110 * 1024 - q_bytes) / (PG * page_bytes)) > 8 ? 8 : (int)((110 * 1024 - q_bytes) / (PG * page_bytes)));
+  // measured (C2 / C3 / C4 sweep of stage size x footprint): GQA pools do best with ~16 KB stages in a 72 KB CTA,
+  // the single-head MLA pool with ~18 KB stages in 110 KB
+  constexpr int kFoot = (HKV == 1 ? 110 : 72) * 1024;
+  constexpr int kScStages = clamp_int((int)((kFoot - q_bytes) / (PG * page_bytes)), 3, 8);
   constexpr size_t smem = kScStages * PG * page_bytes + q_bytes;
   static bool attr_set = false;
   if (!attr_set) {
@@ -431,19 +437,17 @@ static cudaError_t launch_score_t(vx_ctx* c, const void* q, const void* summary,
   return launch_score_agg<T, D, PG, HKV, VX_AGG_SUM, KIND>(c, q, summary, pt, scores, s, rr);
 }
 
-constexpr int pow2_floor(int x) { int p = 1; while (2 * p <= x) p *= 2; return p; }
-constexpr int clamp_int(int x, int lo, int hi) { return x < lo ? lo : (x > hi ? hi : x); }
-
 // PG pages per stage so that a stage is ~32 KB and every consumer warp gets 1, 2, 4 or 8 rows of it
 template <typename T, int D, int KIND>
 static cudaError_t launch_score_k(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt,
                                   float* scores, cudaStream_t s, const ReqRange& rr) {
   constexpr int row_bytes = (KIND == VX_SUMMARY_CENTROID ? D : 2 * D) * (int)sizeof(T);
   constexpr int rows32k = pow2_floor(32768 / row_bytes < 8 ? 8 : 32768 / row_bytes);     // rows per ~32 KB stage, >= 8
+  constexpr int rows16k = pow2_floor(16384 / row_bytes < 8 ? 8 : 16384 / row_bytes);     // rows per ~16 KB stage, >= 8
   switch (c->g.num_kv_heads) {                   // rows per stage = PG * HKV in [8, 64] (1..8 rows per consumer warp)
-    case 8: return launch_score_t<T, D, clamp_int(rows32k, 8, 64) / 8, 8, KIND>(c, q, summary, pt, scores, s, rr);
-    case 4: return launch_score_t<T, D, clamp_int(rows32k, 8, 64) / 4, 4, KIND>(c, q, summary, pt, scores, s, rr);
-    case 2: return launch_score_t<T, D, clamp_int(rows32k, 8, 64) / 2, 2, KIND>(c, q, summary, pt, scores, s, rr);
+    case 8: return launch_score_t<T, D, clamp_int(rows16k, 8, 64) / 8, 8, KIND>(c, q, summary, pt, scores, s, rr);
+    case 4: return launch_score_t<T, D, clamp_int(rows16k, 8, 64) / 4, 4, KIND>(c, q, summary, pt, scores, s, rr);
+    case 2: return launch_score_t<T, D, clamp_int(rows16k, 8, 64) / 2, 2, KIND>(c, q, summary, pt, scores, s, rr);
     case 1: return launch_score_t<T, D, clamp_int(rows32k, 8, 32), 1, KIND>(c, q, summary, pt, scores, s, rr);
   }
   return cudaErrorInvalidValue;
