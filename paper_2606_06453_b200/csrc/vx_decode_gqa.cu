@@ -344,7 +344,8 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
 
 int decode_gqa_splits(const vx_ctx* c, int n_req, int max_budget) {
   const int units = n_req * c->g.num_kv_heads;
-  const int slots = c->num_sms * 2;              // 96 KB of shared memory per CTA -> 2 CTAs per SM
+  const int cta_smem = kGqaWarps * kGqaStages * 2 * kGqaPage * c->g.qk_dim * 2 + 1024;   // ring + static / reserved
+  const int slots = c->num_sms * (227 * 1024 / cta_smem > 0 ? 227 * 1024 / cta_smem : 1);    // resident CTAs
   int splits = 1, best_cost = 1 << 30;
   for (int sp = 1; sp <= kMaxSplits && sp <= max_budget; ++sp) {
     const int waves = (units * sp + slots - 1) / slots;
