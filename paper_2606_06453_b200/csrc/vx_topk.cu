@@ -317,15 +317,268 @@ static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_t
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+// ---- register-resident variant: requests of at most kKpt * THREADS pages ---------------------------------------
+// Same algorithm, but every thread keeps its kKpt keys in registers for all passes (no shared-memory key array, no
+// re-reads): warp w owns the contiguous run [w * 32 * kKpt, (w+1) * 32 * kKpt) of logical pages, lane-strided inside
+// it (coalesced score loads), so the ordered emission is one ballot per 32 pages.  Fewer, cheaper block-wide phases:
+// this kernel is latency-bound ("top-k selection becomes a bottleneck").
+constexpr int kKpt = 8;
+
+template <int THREADS>
+__global__ void __launch_bounds__(THREADS)
+topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
+                const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
+                const int32_t* __restrict__ seq_lens, int page_size, const int32_t* __restrict__ budget,
+                int n_sink, int n_local, int max_budget, int32_t* __restrict__ sel_phys,
+                int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count, int req0, const PrefetchPlan pf) {
+  constexpr int WARPS = THREADS / kWarp;
+  constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
+  static_assert(kBins % THREADS == 0, "shape");
+  __shared__ int s_hist[kBins];
+  __shared__ uint32_t s_list[kList];
+  __shared__ uint32_t s_wmin[WARPS], s_wmax[WARPS];
+  __shared__ int s_wsum[WARPS];
+  __shared__ int2 s_wcnt[WARPS];
+  __shared__ int s_bin, s_above, s_cnt, s_nlist, s_need_eq;
+  __shared__ uint32_t s_thr, s_bmin, s_bmax;
+
+  const int kvh = blockIdx.x, i = blockIdx.y + req0;
+  const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
+  const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
+  const int k = min(budget[i], max_budget);
+  const int row0 = page_indptr[i];
+  for (int b = tid; b < kBins; b += THREADS) s_hist[b] = 0;      // first pass's histogram, zeroed under the loads
+  pdl_wait();                                   // the scores (and, in a step, nothing else) come from the predecessor
+  const int64_t out0 = ((int64_t)i * num_kv_heads + kvh) * max_budget;
+  const int n_sel = min(k, n_pages);
+  if (tid == 0) sel_count[i * num_kv_heads + kvh] = n_sel;
+
+  if (k >= n_pages) {                           // G6: budget covers the request -> every page
+    for (int r = tid; r < max_budget; r += THREADS) {
+      const bool ok = r < n_pages;
+      sel_phys[out0 + r] = ok ? page_indices[row0 + r] : -1;
+      if (sel_logical) sel_logical[out0 + r] = ok ? r : -1;
+    }
+    return;
+  }
+
+  // ---- my keys: logical pages jbase + 32 u + lane ---------------------------------------------------------------
+  const float* sc = scores + (int64_t)kvh * total_pages + row0;
+  const int jbase = warp * kWarp * kKpt;
+  uint32_t key[kKpt];                           // 0 for pages past the request (never forced, never counted: see `live`)
+  float v[kKpt];
+#pragma unroll
+  for (int u = 0; u < kKpt; ++u) {
+    const int j = jbase + u * kWarp + lane;
+    v[u] = j < n_pages ? sc[j] : 0.f;
+  }
+  uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
+  unsigned live = 0;                            // bit u: my u-th page exists and is not forced
+#pragma unroll
+  for (int u = 0; u < kKpt; ++u) {
+    const int j = jbase + u * kWarp + lane;
+    const bool forced = j < n_pages && page_forced(j, n_pages, n_sink, n_local);
+    key[u] = forced ? kForcedKey : float_to_key(v[u]);
+    if (j < n_pages && !forced) { live |= 1u << u; kmin = min(kmin, key[u]); kmax = max(kmax, key[u]); }
+  }
+  kmin = __reduce_min_sync(0xffffffffu, kmin);
+  kmax = __reduce_max_sync(0xffffffffu, kmax);
+  if (lane == 0) { s_wmin[warp] = kmin; s_wmax[warp] = kmax; }
+  __syncthreads();
+#pragma unroll
+  for (int w = 0; w < WARPS; ++w) { kmin = min(kmin, s_wmin[w]); kmax = max(kmax, s_wmax[w]); }
+
+  const int sink = min(n_sink, n_pages), local = min(n_local, n_pages);
+  const int n_forced = min(n_pages, sink + local);
+  int need = k - n_forced;                      // non-forced pages still to take (precondition: >= 0)
+  uint32_t thr = kForcedKey;                    // take keys > thr, and the first need_eq keys == thr
+  int need_eq = 0;
+
+  if (need > 0) {
+    uint32_t lo = kmin;
+    uint64_t width = (uint64_t)(kmax - kmin) + 1;
+    int shift = max(0, (32 - __clz(kmax - kmin)) - kBinBits);     // ((kmax - kmin) >> shift) < kBins
+    const float smin = key_to_float(kmin), smax = key_to_float(kmax);
+    const float fscale = (float)kBins / (smax - smin);
+    bool fpass = kmax - kmin >= (1u << 25) && isfinite(fscale) && fscale > 0.f;   // float-domain first pass (see topk_kernel)
+    auto fbin = [&](uint32_t kk) -> int { return min(kBins - 1, (int)((key_to_float(kk) - smin) * fscale)); };
+    bool first = true;
+#pragma unroll 1
+    while (true) {
+      if (!first) {
+        for (int b = tid; b < kBins; b += THREADS) s_hist[b] = 0;
+        __syncthreads();
+      }
+      first = false;
+#pragma unroll
+      for (int u = 0; u < kKpt; ++u)
+        if (((live >> u) & 1u) && key[u] >= lo && (uint64_t)(key[u] - lo) < width)
+          atomicAdd(&s_hist[fpass ? fbin(key[u]) : (int)((key[u] - lo) >> shift)], 1);
+      __syncthreads();
+      // threshold bin: the highest b with  #keys in bins > b  <  need  <=  #keys in bins >= b
+      int h[BPT], mine = 0;
+#pragma unroll
+      for (int e = 0; e < BPT; ++e) { h[e] = s_hist[tid * BPT + e]; mine += h[e]; }
+      int inc = mine;                           // inclusive suffix sum over threads (tid' >= tid)
+#pragma unroll
+      for (int o = 1; o < kWarp; o <<= 1) {
+        const int a = __shfl_down_sync(0xffffffffu, inc, o);
+        if (lane + o < kWarp) inc += a;
+      }
+      if (lane == 0) s_wsum[warp] = inc;
+      __syncthreads();
+      int run = inc - mine;                     // keys in bins owned by higher threads
+#pragma unroll
+      for (int w = 0; w < WARPS; ++w) run += (w > warp) ? s_wsum[w] : 0;
+#pragma unroll
+      for (int e = BPT - 1; e >= 0; --e) {
+        if (run < need && run + h[e] >= need) { s_bin = tid * BPT + e; s_above = run; s_cnt = h[e]; }
+        run += h[e];
+      }
+      if (tid == 0) { s_nlist = 0; s_bmin = 0xFFFFFFFFu; s_bmax = 0u; }
+      __syncthreads();
+      const int bin = s_bin, cnt = s_cnt;
+      need -= s_above;                          // still to take from the threshold bin
+      const uint32_t bin_lo = lo + ((uint32_t)bin << shift);
+      if (!fpass && shift == 0) {               // the bin is one key value: take the first `need` by index
+        thr = bin_lo;
+        need_eq = need;
+        break;
+      }
+      // members of the threshold bin: rank them if they are few, else continue on their key interval
+      const uint64_t bin_w = (uint64_t)1 << shift;
+#pragma unroll
+      for (int u = 0; u < kKpt; ++u) {
+        const uint32_t kk = key[u];
+        const bool in_range = ((live >> u) & 1u) && kk >= lo && (uint64_t)(kk - lo) < width;
+        const bool member = in_range && (fpass ? fbin(kk) == bin : (kk >= bin_lo && (uint64_t)(kk - bin_lo) < bin_w));
+        if (member) {
+          if (cnt <= kList) s_list[atomicAdd(&s_nlist, 1)] = kk;
+          else if (fpass) { atomicMin(&s_bmin, kk); atomicMax(&s_bmax, kk); }
+        }
+      }
+      __syncthreads();
+      if (cnt <= kList) {
+        for (int m = tid; m < cnt; m += THREADS) {
+          const uint32_t mykey = s_list[m];
+          int gt = 0, ge = 0;
+          for (int j = 0; j < cnt; ++j) {
+            const uint32_t o = s_list[j];
+            gt += o > mykey;
+            ge += o >= mykey;
+          }
+          if (gt < need && need <= ge) { s_thr = mykey; s_need_eq = need - gt; }   // same values from every tie
+        }
+        __syncthreads();
+        thr = s_thr;
+        need_eq = s_need_eq;
+        break;
+      }
+      if (fpass) {                              // heavy float bin: its members are exactly the keys in [bmin, bmax]
+        lo = s_bmin;
+        width = (uint64_t)(s_bmax - s_bmin) + 1;
+        shift = max(0, (32 - __clz(s_bmax - s_bmin)) - kBinBits);
+        fpass = false;
+      } else {                                  // heavy ties: recurse into the bin, 11 more bits
+        lo = bin_lo;
+        width = bin_w;
+        shift = max(0, shift - kBinBits);
+      }
+      __syncthreads();                          // s_bmin / s_bmax / s_bin are read before the next pass rewrites them
+    }
+  }
+
+  pdl_trigger();
+  // ---- ordered emission: class of a page = sure (forced or key > thr) / tie (key == thr, first need_eq by index) --
+  unsigned m_sure[kKpt], m_tie[kKpt];
+  int n_sure = 0, n_tie = 0;                    // warp-uniform
+#pragma unroll
+  for (int u = 0; u < kKpt; ++u) {
+    const bool exists = jbase + u * kWarp + lane < n_pages;
+    const bool sure = exists && (key[u] == kForcedKey || key[u] > thr);
+    const bool tie = exists && key[u] != kForcedKey && key[u] == thr;
+    m_sure[u] = __ballot_sync(0xffffffffu, sure);
+    m_tie[u] = __ballot_sync(0xffffffffu, tie);
+    n_sure += __popc(m_sure[u]);
+    n_tie += __popc(m_tie[u]);
+  }
+  if (lane == 0) s_wcnt[warp] = make_int2(n_sure, n_tie);
+  __syncthreads();
+  int gt = 0, eq = 0;                           // sure / tie pages before this warp's run
+#pragma unroll
+  for (int w = 0; w < WARPS; ++w) {
+    const int2 c = s_wcnt[w];
+    gt += (w < warp) ? c.x : 0;
+    eq += (w < warp) ? c.y : 0;
+  }
+  const unsigned lt_mask = (1u << lane) - 1u;
+  const bool staged = n_sel <= kBins;           // the histogram is free now: stage the selected logical ids in it
+#pragma unroll
+  for (int u = 0; u < kKpt; ++u) {
+    const int j = jbase + u * kWarp + lane;
+    const bool sure = (m_sure[u] >> lane) & 1u, tie = (m_tie[u] >> lane) & 1u;
+    const int my_gt = gt + __popc(m_sure[u] & lt_mask), my_eq = eq + __popc(m_tie[u] & lt_mask);
+    const bool take = sure || (tie && my_eq < need_eq);
+    const int pos = my_gt + min(my_eq, need_eq);
+    if (take && pos < n_sel) {
+      if (staged) s_hist[pos] = j;
+      else {
+        sel_phys[out0 + pos] = page_indices[row0 + j];
+        if (sel_logical) sel_logical[out0 + pos] = j;
+      }
+    }
+    gt += __popc(m_sure[u]);
+    eq += __popc(m_tie[u]);
+  }
+  if (staged) {                                   // every selected page: one independent gather + two stores
+    __syncthreads();
+    const int per_split = (n_sel + pf.splits - 1) / pf.splits;
+    for (int r = tid; r < n_sel; r += THREADS) {
+      const int j = s_hist[r];
+      const int phys = page_indices[row0 + j];
+      sel_phys[out0 + r] = phys;
+      if (sel_logical) sel_logical[out0 + r] = j;
+      if (pf.k != nullptr && r % per_split < pf.pages_per_split) {
+        const int64_t off = (int64_t)phys * pf.page_bytes + (int64_t)kvh * pf.head_bytes;
+        l2_prefetch(static_cast<const uint8_t*>(pf.k) + off, pf.chunk_bytes);
+        if (pf.v != nullptr) l2_prefetch(static_cast<const uint8_t*>(pf.v) + off, pf.chunk_bytes);
+      }
+    }
+  }
+  for (int r = n_sel + tid; r < max_budget; r += THREADS) {
+    sel_phys[out0 + r] = -1;
+    if (sel_logical) sel_logical[out0 + r] = -1;
+  }
+}
+
+template <int THREADS>
+static cudaError_t launch_topk_reg(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
+                                   int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
+                                   cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf) {
+  const vx_geom& g = c->g;
+  dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
+  cudaError_t e = launch_kernel(topk_reg_kernel<THREADS>, grid, dim3(THREADS), 0, s, pdl, scores, g.num_kv_heads,
+                                pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
+                                g.n_sink, g.n_local, max_budget, sel_phys, sel_logical, sel_count, rr.begin, pf);
+  c->launches += 1;
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+
 cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
                               int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl, const ReqRange& rr,
                               const PrefetchPlan& pf) {
   if (pt.batch == 0) return cudaSuccess;
-  // block size by problem size (VX_TOPK_THREADS overrides, for tuning)
+  // block size by problem size (VX_TOPK_THREADS overrides, for tuning; it also selects the shared-memory-key kernel)
   static int force = -1;
   if (force < 0) { const char* e = getenv("VX_TOPK_THREADS"); force = e ? atoi(e) : 0; }
   const int n = pt.max_pages_per_req;
+  if (!force && n <= kKpt * 1024) {               // keys fit the registers of one CTA: 8 per thread
+    if (n <= kKpt * 128) return launch_topk_reg<128>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
+    if (n <= kKpt * 256) return launch_topk_reg<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
+    if (n <= kKpt * 512) return launch_topk_reg<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
+    return launch_topk_reg<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
+  }
   const int th = force ? force : (n <= 1024 ? 256 : n <= 4096 ? 512 : 1024);
   if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
   if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
