@@ -322,9 +322,7 @@ static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_t
 // re-reads): warp w owns the contiguous run [w * 32 * kKpt, (w+1) * 32 * kKpt) of logical pages, lane-strided inside
 // it (coalesced score loads), so the ordered emission is one ballot per 32 pages.  Fewer, cheaper block-wide phases:
 // this kernel is latency-bound ("top-k selection becomes a bottleneck").
-constexpr int kKpt = 8;
-
-template <int THREADS>
+template <int THREADS, int kKpt>
 __global__ void __launch_bounds__(THREADS)
 topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
                 const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
@@ -551,13 +549,13 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   }
 }
 
-template <int THREADS>
+template <int THREADS, int kKpt>
 static cudaError_t launch_topk_reg(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
                                    int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
                                    cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf) {
   const vx_geom& g = c->g;
   dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
-  cudaError_t e = launch_kernel(topk_reg_kernel<THREADS>, grid, dim3(THREADS), 0, s, pdl, scores, g.num_kv_heads,
+  cudaError_t e = launch_kernel(topk_reg_kernel<THREADS, kKpt>, grid, dim3(THREADS), 0, s, pdl, scores, g.num_kv_heads,
                                 pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
                                 g.n_sink, g.n_local, max_budget, sel_phys, sel_logical, sel_count, rr.begin, pf);
   c->launches += 1;
@@ -573,11 +571,13 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
   static int force = -1;
   if (force < 0) { const char* e = getenv("VX_TOPK_THREADS"); force = e ? atoi(e) : 0; }
   const int n = pt.max_pages_per_req;
-  if (!force && n <= kKpt * 1024) {               // keys fit the registers of one CTA: 8 per thread
-    if (n <= kKpt * 128) return launch_topk_reg<128>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
-    if (n <= kKpt * 256) return launch_topk_reg<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
-    if (n <= kKpt * 512) return launch_topk_reg<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
-    return launch_topk_reg<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
+  if (!force && n <= 8 * 1024) {                  // keys fit the registers of one CTA, 8 per thread (16 measured slower)
+#define VX_REG(T, K) return launch_topk_reg<T, K>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf)
+    if (n <= 1024) VX_REG(128, 8);
+    if (n <= 2048) VX_REG(256, 8);
+    if (n <= 4096) VX_REG(512, 8);
+    VX_REG(1024, 8);
+#undef VX_REG
   }
   const int th = force ? force : (n <= 1024 ? 256 : n <= 4096 ? 512 : 1024);
   if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
