@@ -269,6 +269,7 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   // launch, no extra HBM bytes).  Otherwise the summary kernel runs first.
   DecodeOpts opt;
   opt.pdl = c->use_pdl;
+  opt.budget = budget;
   if (flags & VX_STEP_UPDATE_SUMMARY) {
     if (c->g.n_local >= 1 && decode_folds_summary(c)) {
       opt.summary_upd = summary;

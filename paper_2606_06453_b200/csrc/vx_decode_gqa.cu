@@ -63,7 +63,8 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
                       const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count,
                       int max_budget, int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                       int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
-                      __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0) {
+                      __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0,
+                      const int32_t* __restrict__ budget_opt) {
   constexpr int ROWB = D * 2;                 // bytes per token row
   constexpr int CH = ROWB / 16;               // 16-byte chunks per row
   constexpr int PAGEB = kGqaPage * ROWB;      // bytes of one K (or V) page chunk
@@ -80,6 +81,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   const int grp = num_q_heads / num_kv_heads;
   const int n_tok = seq_lens[i];
   const int newest_page = (n_tok - 1) / kGqaPage;
+  const int cnt_known = budget_opt ? min(min(budget_opt[i], max_budget), newest_page + 1) : -1;
 
   // Q^T as the B operand: qb[ks] = Q[head lane/4][16*ks + 2*(lane%4) + {0,1}], [.. + 8 ..]
   uint32_t qb[KS][2];
@@ -95,7 +97,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   }
   pdl_wait();                                   // the selection lists come from the preceding kernel of the step
 
-  const int cnt = sel_count[i * num_kv_heads + kvh];
+  const int cnt = cnt_known >= 0 ? cnt_known : sel_count[i * num_kv_heads + kvh];
   const int per_split = (cnt + num_splits - 1) / num_splits;
   const int r_begin = min(split * per_split, cnt), r_end = min(r_begin + per_split, cnt);
   const int32_t* phys_list = sel_phys + ((int64_t)i * num_kv_heads + kvh) * max_budget;
@@ -337,7 +339,7 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const __nv_bfloat16*>(pool.v), pool.stride_page, pool.stride_token, pool.stride_head,
       g.num_q_heads, g.num_kv_heads, g.sm_scale * kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget,
       splits, c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
-      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin);
+      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

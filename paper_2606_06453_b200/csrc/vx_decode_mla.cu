@@ -251,7 +251,8 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
                   const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count, int max_budget,
                   int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                   int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
-                  __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0) {
+                  __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0,
+                  const int32_t* __restrict__ budget_opt) {
   using namespace mla;
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t s_bar[N_BARS];
@@ -270,6 +271,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   auto bar = [&](int idx) -> uint32_t { return bar0 + 8u * (uint32_t)idx; };
   const int n_tok = seq_lens[i];
   const int newest_page = (n_tok - 1) / PAGE;
+  const int cnt_known = budget_opt ? min(min(budget_opt[i], max_budget), newest_page + 1) : -1;
 
   // ---- prologue (overlaps the preceding kernel under PDL): barriers, TMEM, Q tile ---------------------
   if (warp == 1) {
@@ -333,7 +335,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   tc_fence_after();
   pdl_wait();                                          // the selection lists come from the preceding kernel of the step
 
-  const int cnt = sel_count[i];
+  const int cnt = cnt_known >= 0 ? cnt_known : sel_count[i];
   const int per_split = (cnt + num_splits - 1) / num_splits;
   const int r_begin = min(split * per_split, cnt), r_end = min(r_begin + per_split, cnt);
   const int n_pages = r_end - r_begin;
@@ -669,7 +671,7 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
                                 static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens,
                                 sel_phys, sel_logical, sel_count, max_budget, best, c->ws.part_o, c->ws.part_lse,
                                 c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
-                                static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin);
+                                static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -99,6 +99,8 @@ struct DecodeOpts {
   void* summary_upd = nullptr;   // non-null: also rebuild the summary of each request's newest page (a1), whose
                                  // keys the kernel stages anyway (it is a forced local page)
   bool pdl = false;              // launched as a programmatic dependent of the preceding kernel
+  const int32_t* budget = nullptr;   // fused step: sel_count[i, h] is known to be min(budget[i], max_budget, P_i), so the kernel
+                                 // need not wait for the selection kernel to read it (one L2 round trip less after the wait)
 };
 
 // every launcher returns cudaGetLastError() after its launches and adds to ctx->launches
