@@ -32,6 +32,7 @@
 // fused step the CTA holding the request's newest page also rebuilds that page's summary (min / max, or the
 // block top-k centroid) from the staged tile (a1; the newest page is a forced local page).
 #include <cuda.h>
+#include <cstdlib>
 
 #include "vx_common.cuh"
 #include "vx_internal.h"
@@ -164,6 +165,25 @@ __device__ __forceinline__ float ex2_approx(float x) {
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
+// thread-block cluster (the splits of one request): barrier over all threads of all CTAs, peer shared-memory reads
+__device__ __forceinline__ void cluster_sync() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ uint32_t dsmem_addr(uint32_t local, uint32_t rank) {
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(rank));
+  return r;
+}
+__device__ __forceinline__ float dsmem_ld_f32(uint32_t addr) {
+  float v;
+  asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ float4 dsmem_ld_f32x4(uint32_t addr) {
+  float4 v;
+  asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
+  return v;
+}
 __device__ __forceinline__ void softmax_barrier() { asm volatile("bar.sync 1, %0;" ::"n"(SOFTMAX_THREADS) : "memory"); }
 
 // barrier indices
@@ -245,6 +265,72 @@ __device__ __forceinline__ void merge_splits(const float* part_o, const float* p
   }
 }
 
+// (a5) LSE merge inside a thread-block cluster: the splits of a request are the CTAs of one cluster (rank = split).
+// Every CTA leaves its normalised partial O [channel][head] fp32 (64 KB, 16-byte columns XOR-swizzled by channel) and
+// its per-head LSE in its own shared memory; after a cluster barrier each CTA merges DV / n_part channels, reading
+// its peers' tiles through distributed shared memory, and writes that slice of the output rows.  No global
+// round trip, no arrival counter: the global-memory merge took 7 us of a 44 us kernel (profiles/r1e_trace.md).
+constexpr int kMaxClusterSplits = 8;
+__device__ __forceinline__ uint32_t stage_off(int d, int j4) { return (uint32_t)(d * 128 + ((j4 ^ (d & 7)) << 4)); }
+__device__ __forceinline__ void merge_cluster(uint8_t* stage, const float* s_lse, float (*s_w)[mla::NH], int i, int num_q_heads,
+                                              int n_part, int rank, __nv_bfloat16* out, float* lse) {
+  using namespace mla;
+  const int64_t row0 = (int64_t)i * num_q_heads;
+  const uint32_t stage_s = smem_u32(stage);
+  if (threadIdx.x < NH) {
+    const int j = threadIdx.x;
+    float l[kMaxClusterSplits];
+    float mx = -INFINITY;
+    for (int r = 0; r < n_part; ++r) { l[r] = dsmem_ld_f32(dsmem_addr(smem_u32(s_lse + j), r)); mx = fmaxf(mx, l[r]); }
+    float z = 0.f;
+    for (int r = 0; r < n_part; ++r) z += mx == -INFINITY ? 0.f : __expf(l[r] - mx);
+    const float inv = z > 0.f ? 1.f / z : 0.f;
+    for (int r = 0; r < n_part; ++r) s_w[r][j] = mx == -INFINITY ? 0.f : __expf(l[r] - mx) * inv;
+    if (rank == 0 && lse != nullptr && j < num_q_heads) lse[row0 + j] = z > 0.f ? mx + logf(z) : -INFINITY;
+  }
+  __syncthreads();
+  const int DS = DV / n_part, d0 = rank * DS;            // my channel slice
+  const int pitch = DS * 2 + 16;                         // bf16 row pitch of the transposed tile (bank spread)
+  uint8_t* tile = stage + NH * DV * 4;
+  constexpr int UNR = 4;
+  const int n_e = DS * (NH / 4);                         // e -> (channel d0 + e / 8, heads 4 (e % 8) ..)
+  for (int e0 = threadIdx.x; e0 < n_e; e0 += UNR * blockDim.x) {
+    float4 acc[UNR];
+#pragma unroll
+    for (int k = 0; k < UNR; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int r = 0; r < n_part; ++r) {
+      const uint32_t peer = dsmem_addr(stage_s, r);
+      float4 v[UNR];
+#pragma unroll
+      for (int k = 0; k < UNR; ++k) {
+        const int e = e0 + k * blockDim.x;
+        v[k] = e < n_e ? dsmem_ld_f32x4(peer + stage_off(d0 + e / (NH / 4), e % (NH / 4))) : make_float4(0.f, 0.f, 0.f, 0.f);
+      }
+#pragma unroll
+      for (int k = 0; k < UNR; ++k) {
+        const float4 w = *reinterpret_cast<const float4*>(&s_w[r][((e0 + k * blockDim.x) % (NH / 4)) * 4]);
+        acc[k].x += w.x * v[k].x; acc[k].y += w.y * v[k].y; acc[k].z += w.z * v[k].z; acc[k].w += w.w * v[k].w;
+      }
+    }
+#pragma unroll
+    for (int k = 0; k < UNR; ++k) {
+      const int e = e0 + k * blockDim.x;
+      if (e < n_e) {
+        const int dl = e / (NH / 4), j4 = (e % (NH / 4)) * 4;
+        *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 0) * pitch + dl * 2) = __float2bfloat16_rn(acc[k].x);
+        *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 1) * pitch + dl * 2) = __float2bfloat16_rn(acc[k].y);
+        *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 2) * pitch + dl * 2) = __float2bfloat16_rn(acc[k].z);
+        *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 3) * pitch + dl * 2) = __float2bfloat16_rn(acc[k].w);
+      }
+    }
+  }
+  __syncthreads();
+  for (int e = threadIdx.x; e < num_q_heads * (DS / 8); e += blockDim.x) {   // 16 bytes per thread, row slices contiguous
+    const int j = e / (DS / 8), c = e % (DS / 8);
+    *reinterpret_cast<uint4*>(out + (row0 + j) * DV + d0 + c * 8) = *reinterpret_cast<const uint4*>(tile + j * pitch + c * 16);
+  }
+}
+
 __global__ void __launch_bounds__(mla::THREADS, 1)
 decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16* __restrict__ q, int num_q_heads,
                   float scale_log2, const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ sel_phys,
@@ -252,7 +338,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
                   int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                   int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
                   __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0,
-                  const int32_t* __restrict__ budget_opt) {
+                  const int32_t* __restrict__ budget_opt, int cluster_merge) {
   using namespace mla;
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t s_bar[N_BARS];
@@ -261,6 +347,8 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   __shared__ int s_flag[2];                            // ... and whether any head needs them
   __shared__ float s_l[NH], s_m[NH], s_inv[NH];        // final denominators / references
   __shared__ int s_last;
+  __shared__ float s_lse[NH];                          // cluster merge: this split's per-head LSE
+  __shared__ __align__(16) float s_w[kMaxClusterSplits][NH];
 
   const int split = blockIdx.x, i = blockIdx.z + req0;
   const int tid = threadIdx.x, warp = tid / kWarp, lane = tid % kWarp;
@@ -343,7 +431,10 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   const int32_t* log_list = sel_logical + (int64_t)i * max_budget + r_begin;
   const uint32_t p_base = base + OFF_P;
 
-  if (n_pages == 0) {                                  // empty split: contributes nothing to the merge
+  if (n_pages == 0 && cluster_merge) {                 // empty split: a zero tile with weight zero
+    for (int e = tid; e < NH * DV / 4; e += THREADS) reinterpret_cast<float4*>(sm + OFF_PAIR)[e] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (tid < NH) s_lse[tid] = -INFINITY;
+  } else if (n_pages == 0) {                           // empty split: contributes nothing to the merge
     for (int e = tid; e < NH * DV; e += THREADS) {       // partial layout: [request][split][channel][head]
       const int h = e / DV, d = e % DV;
       if (num_splits > 1) part_o[(((int64_t)i * num_splits + split) * DV + d) * NH + h] = 0.f;
@@ -580,7 +671,14 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       float o[NH];
       tmem_ld32(t_lane + TM_O + 32 * mb, o);
       const int d = mb * 128 + sp * 32 + lane;
-      if (num_splits > 1) {                              // partial [request][split][channel][head]: 128 contiguous bytes per thread
+      if (cluster_merge) {                               // partial stays in shared memory (the ring is drained)
+        uint8_t* stage = sm + OFF_PAIR;
+#pragma unroll
+        for (int j4 = 0; j4 < NH / 4; ++j4)
+          *reinterpret_cast<float4*>(stage + stage_off(d, j4)) =
+              make_float4(o[4 * j4] * s_inv[4 * j4], o[4 * j4 + 1] * s_inv[4 * j4 + 1], o[4 * j4 + 2] * s_inv[4 * j4 + 2],
+                          o[4 * j4 + 3] * s_inv[4 * j4 + 3]);
+      } else if (num_splits > 1) {                       // partial [request][split][channel][head]: 128 contiguous bytes per thread
         float4* dst = reinterpret_cast<float4*>(part_o + (((int64_t)i * num_splits + split) * DV + d) * NH);
 #pragma unroll
         for (int j4 = 0; j4 < NH / 4; ++j4)
@@ -592,7 +690,9 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
           if (j < num_q_heads) out[((int64_t)i * num_q_heads + j) * DV + d] = __float2bfloat16_rn(o[j] * s_inv[j]);
       }
     }
-    if (warp == SOFTMAX_WARP && lane < num_q_heads) {
+    if (warp == SOFTMAX_WARP && cluster_merge) {
+      s_lse[lane] = lane < num_q_heads ? (s_m[lane] + log2f(s_l[lane])) * kLn2 : -INFINITY;
+    } else if (warp == SOFTMAX_WARP && lane < num_q_heads) {
       const float lse = (s_m[lane] + log2f(s_l[lane])) * kLn2;
       const int64_t orow = (int64_t)i * num_q_heads + lane;
       if (num_splits == 1) { if (lse_out) lse_out[orow] = lse; }
@@ -602,7 +702,11 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
 
   // ---- (a5) the last split of the request to arrive merges the partials; release TMEM -------------------
   tc_fence_before();
-  if (num_splits > 1) {
+  if (cluster_merge) {
+    cluster_sync();                                      // every split's tile and LSE are in place
+    merge_cluster(sm + OFF_PAIR, s_lse, s_w, i, num_q_heads, num_splits, split, out, lse_out);
+    cluster_sync();                                      // my tile stays until every peer has read it
+  } else if (num_splits > 1) {
     if (last_split_arrives(unit_counter + i, num_splits, &s_last))
       merge_splits(part_o, part_lse, i, num_q_heads, num_splits, out, lse_out, sm + OFF_PAIR);
   }
@@ -667,11 +771,15 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
   const int n_req = opt.rr.count < 0 ? pt.batch : opt.rr.count;
   const int best = decode_mla_splits(c, n_req, max_budget);
   dim3 grid(best, 1, n_req);
-  cudaError_t e = launch_kernel(decode_mla_kernel, grid, dim3(mla::THREADS), (size_t)mla::SMEM_BYTES, s, opt.pdl, kmap,
+  // splits of 2, 4 or 8: the splits of a request form a thread-block cluster and merge through shared memory
+  static int no_cluster = -1;
+  if (no_cluster < 0) { const char* ev = getenv("VX_NO_CLUSTER"); no_cluster = ev && atoi(ev) ? 1 : 0; }
+  const int cluster = (!no_cluster && (best == 2 || best == 4 || best == 8)) ? best : 1;
+  cudaError_t e = launch_kernel_cluster(decode_mla_kernel, grid, dim3(mla::THREADS), (size_t)mla::SMEM_BYTES, s, opt.pdl, cluster, kmap,
                                 static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens,
                                 sel_phys, sel_logical, sel_count, max_budget, best, c->ws.part_o, c->ws.part_lse,
                                 c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
-                                static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget);
+                                static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget, cluster > 1 ? 1 : 0);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }
