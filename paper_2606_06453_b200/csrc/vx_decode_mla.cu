@@ -179,6 +179,9 @@ __device__ __forceinline__ float dsmem_ld_f32(uint32_t addr) {
   asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
   return v;
 }
+__device__ __forceinline__ void dsmem_st_f32(uint32_t addr, float v) {
+  asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(addr), "f"(v) : "memory");
+}
 __device__ __forceinline__ float4 dsmem_ld_f32x4(uint32_t addr) {
   float4 v;
   asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr) : "memory");
@@ -267,65 +270,82 @@ __device__ __forceinline__ void merge_splits(const float* part_o, const float* p
 
 // (a5) LSE merge inside a thread-block cluster: the splits of a request are the CTAs of one cluster (rank = split).
 // Every CTA leaves its normalised partial O [channel][head] fp32 (64 KB, 16-byte columns XOR-swizzled by channel) and
-// its per-head LSE in its own shared memory; after a cluster barrier each CTA merges DV / n_part channels, reading
+// pushes its per-head LSE into every peer; after a cluster barrier each CTA merges DV / n_part channels, reading
 // its peers' tiles through distributed shared memory, and writes that slice of the output rows.  No global
 // round trip, no arrival counter: the global-memory merge took 7 us of a 44 us kernel (profiles/r1e_trace.md).
 constexpr int kMaxClusterSplits = 8;
 __device__ __forceinline__ uint32_t stage_off(int d, int j4) { return (uint32_t)(d * 128 + ((j4 ^ (d & 7)) << 4)); }
-__device__ __forceinline__ void merge_cluster(uint8_t* stage, const float* s_lse, float (*s_w)[mla::NH], int i, int num_q_heads,
-                                              int n_part, int rank, __nv_bfloat16* out, float* lse) {
+// s_lse_all[r][j]: split r's LSE of head j, pushed by its CTA into every CTA of the cluster before the barrier.
+// The code that runs once is kept small and rolled: after an L2 flush every first-touched instruction line is a
+// memory round trip that all CTAs wait for in lockstep (profiles/r1e_trace.md).
+__device__ __forceinline__ void merge_cluster(uint8_t* stage, const float (*s_lse_all)[mla::NH], float (*s_w)[mla::NH], int i,
+                                              int num_q_heads, int n_part, int rank, __nv_bfloat16* out, float* lse) {
   using namespace mla;
   const int64_t row0 = (int64_t)i * num_q_heads;
   const uint32_t stage_s = smem_u32(stage);
   if (threadIdx.x < NH) {
     const int j = threadIdx.x;
-    float l[kMaxClusterSplits];
     float mx = -INFINITY;
-    for (int r = 0; r < n_part; ++r) { l[r] = dsmem_ld_f32(dsmem_addr(smem_u32(s_lse + j), r)); mx = fmaxf(mx, l[r]); }
+#pragma unroll 1
+    for (int r = 0; r < n_part; ++r) mx = fmaxf(mx, s_lse_all[r][j]);
     float z = 0.f;
-    for (int r = 0; r < n_part; ++r) z += mx == -INFINITY ? 0.f : __expf(l[r] - mx);
+#pragma unroll 1
+    for (int r = 0; r < n_part; ++r) z += mx == -INFINITY ? 0.f : __expf(s_lse_all[r][j] - mx);
     const float inv = z > 0.f ? 1.f / z : 0.f;
-    for (int r = 0; r < n_part; ++r) s_w[r][j] = mx == -INFINITY ? 0.f : __expf(l[r] - mx) * inv;
+#pragma unroll 1
+    for (int r = 0; r < n_part; ++r) s_w[r][j] = mx == -INFINITY ? 0.f : __expf(s_lse_all[r][j] - mx) * inv;
     if (rank == 0 && lse != nullptr && j < num_q_heads) lse[row0 + j] = z > 0.f ? mx + logf(z) : -INFINITY;
   }
   __syncthreads();
   const int DS = DV / n_part, d0 = rank * DS;            // my channel slice
   const int pitch = DS * 2 + 16;                         // bf16 row pitch of the transposed tile (bank spread)
   uint8_t* tile = stage + NH * DV * 4;
-  constexpr int UNR = 4;
+  constexpr int UNR = 5;
   const int n_e = DS * (NH / 4);                         // e -> (channel d0 + e / 8, heads 4 (e % 8) ..)
-  for (int e0 = threadIdx.x; e0 < n_e; e0 += UNR * blockDim.x) {
+  const int j4 = threadIdx.x % (NH / 4);                 // (THREADS is a multiple of 8: the same heads for all my items)
+#pragma unroll 1
+  for (int e0 = threadIdx.x; e0 < n_e; e0 += UNR * THREADS) {
     float4 acc[UNR];
+    {                                                    // my own partial: plain shared-memory reads
+      const float4 w = *reinterpret_cast<const float4*>(&s_w[rank][j4 * 4]);
 #pragma unroll
-    for (int k = 0; k < UNR; ++k) acc[k] = make_float4(0.f, 0.f, 0.f, 0.f);
-    for (int r = 0; r < n_part; ++r) {
+      for (int k = 0; k < UNR; ++k) {
+        const int e = e0 + k * THREADS;
+        const float4 v = e < n_e ? *reinterpret_cast<const float4*>(stage + stage_off(d0 + e / (NH / 4), j4)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        acc[k] = make_float4(w.x * v.x, w.y * v.y, w.z * v.z, w.w * v.w);
+      }
+    }
+#pragma unroll 1
+    for (int rr = 1; rr < n_part; ++rr) {                // the peers' partials: distributed shared memory, UNR loads in flight
+      const int r = (rank + rr) % n_part;
       const uint32_t peer = dsmem_addr(stage_s, r);
+      const float4 w = *reinterpret_cast<const float4*>(&s_w[r][j4 * 4]);
       float4 v[UNR];
 #pragma unroll
       for (int k = 0; k < UNR; ++k) {
-        const int e = e0 + k * blockDim.x;
-        v[k] = e < n_e ? dsmem_ld_f32x4(peer + stage_off(d0 + e / (NH / 4), e % (NH / 4))) : make_float4(0.f, 0.f, 0.f, 0.f);
+        const int e = e0 + k * THREADS;
+        v[k] = e < n_e ? dsmem_ld_f32x4(peer + stage_off(d0 + e / (NH / 4), j4)) : make_float4(0.f, 0.f, 0.f, 0.f);
       }
 #pragma unroll
       for (int k = 0; k < UNR; ++k) {
-        const float4 w = *reinterpret_cast<const float4*>(&s_w[r][((e0 + k * blockDim.x) % (NH / 4)) * 4]);
         acc[k].x += w.x * v[k].x; acc[k].y += w.y * v[k].y; acc[k].z += w.z * v[k].z; acc[k].w += w.w * v[k].w;
       }
     }
 #pragma unroll
     for (int k = 0; k < UNR; ++k) {
-      const int e = e0 + k * blockDim.x;
+      const int e = e0 + k * THREADS;
       if (e < n_e) {
-        const int dl = e / (NH / 4), j4 = (e % (NH / 4)) * 4;
-        *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 0) * pitch + dl * 2) = __float2bfloat16_rn(acc[k].x);
-        *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 1) * pitch + dl * 2) = __float2bfloat16_rn(acc[k].y);
-        *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 2) * pitch + dl * 2) = __float2bfloat16_rn(acc[k].z);
-        *reinterpret_cast<__nv_bfloat16*>(tile + (j4 + 3) * pitch + dl * 2) = __float2bfloat16_rn(acc[k].w);
+        uint8_t* t = tile + (j4 * 4) * pitch + (e / (NH / 4)) * 2;
+        *reinterpret_cast<__nv_bfloat16*>(t) = __float2bfloat16_rn(acc[k].x);
+        *reinterpret_cast<__nv_bfloat16*>(t + pitch) = __float2bfloat16_rn(acc[k].y);
+        *reinterpret_cast<__nv_bfloat16*>(t + 2 * pitch) = __float2bfloat16_rn(acc[k].z);
+        *reinterpret_cast<__nv_bfloat16*>(t + 3 * pitch) = __float2bfloat16_rn(acc[k].w);
       }
     }
   }
   __syncthreads();
-  for (int e = threadIdx.x; e < num_q_heads * (DS / 8); e += blockDim.x) {   // 16 bytes per thread, row slices contiguous
+#pragma unroll 1
+  for (int e = threadIdx.x; e < num_q_heads * (DS / 8); e += THREADS) {      // 16 bytes per thread, row slices contiguous
     const int j = e / (DS / 8), c = e % (DS / 8);
     *reinterpret_cast<uint4*>(out + (row0 + j) * DV + d0 + c * 8) = *reinterpret_cast<const uint4*>(tile + j * pitch + c * 16);
   }
@@ -347,8 +367,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   __shared__ int s_flag[2];                            // ... and whether any head needs them
   __shared__ float s_l[NH], s_m[NH], s_inv[NH];        // final denominators / references
   __shared__ int s_last;
-  __shared__ float s_lse[NH];                          // cluster merge: this split's per-head LSE
-  __shared__ __align__(16) float s_w[kMaxClusterSplits][NH];
+  __shared__ float s_lse_all[kMaxClusterSplits][NH];   // cluster merge: every split's per-head LSE (pushed by its CTA)
 
   const int split = blockIdx.x, i = blockIdx.z + req0;
   const int tid = threadIdx.x, warp = tid / kWarp, lane = tid % kWarp;
@@ -433,7 +452,8 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
 
   if (n_pages == 0 && cluster_merge) {                 // empty split: a zero tile with weight zero
     for (int e = tid; e < NH * DV / 4; e += THREADS) reinterpret_cast<float4*>(sm + OFF_PAIR)[e] = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (tid < NH) s_lse[tid] = -INFINITY;
+    if (tid < NH)
+      for (int r = 0; r < num_splits; ++r) dsmem_st_f32(dsmem_addr(smem_u32(&s_lse_all[split][tid]), r), -INFINITY);
   } else if (n_pages == 0) {                           // empty split: contributes nothing to the merge
     for (int e = tid; e < NH * DV; e += THREADS) {       // partial layout: [request][split][channel][head]
       const int h = e / DV, d = e % DV;
@@ -691,7 +711,9 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       }
     }
     if (warp == SOFTMAX_WARP && cluster_merge) {
-      s_lse[lane] = lane < num_q_heads ? (s_m[lane] + log2f(s_l[lane])) * kLn2 : -INFINITY;
+      const float my_lse = lane < num_q_heads ? (s_m[lane] + log2f(s_l[lane])) * kLn2 : -INFINITY;
+#pragma unroll 1
+      for (int r = 0; r < num_splits; ++r) dsmem_st_f32(dsmem_addr(smem_u32(&s_lse_all[split][lane]), r), my_lse);
     } else if (warp == SOFTMAX_WARP && lane < num_q_heads) {
       const float lse = (s_m[lane] + log2f(s_l[lane])) * kLn2;
       const int64_t orow = (int64_t)i * num_q_heads + lane;
@@ -704,7 +726,8 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   tc_fence_before();
   if (cluster_merge) {
     cluster_sync();                                      // every split's tile and LSE are in place
-    merge_cluster(sm + OFF_PAIR, s_lse, s_w, i, num_q_heads, num_splits, split, out, lse_out);
+    merge_cluster(sm + OFF_PAIR, s_lse_all, reinterpret_cast<float (*)[NH]>(sm + OFF_PAIR + 96 * 1024), i, num_q_heads, num_splits, split,
+                  out, lse_out);
     cluster_sync();                                      // my tile stays until every peer has read it
   } else if (num_splits > 1) {
     if (last_split_arrives(unit_counter + i, num_splits, &s_last))
