@@ -77,7 +77,7 @@ template <typename T, int D, int PG, int HKV, int kScStages, int AGG, int KIND>
 __global__ void __launch_bounds__(kScThreads, 2)
 score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int batch,
              const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices, int total_pages,
-             float* __restrict__ scores, int req_begin, int req_end) {
+             float* __restrict__ scores, int req_begin, int req_end, int flat_lo_host, int flat_span_host) {
   constexpr int PER = Elem<T>::kPerVec;
   // envelope: [min | max] of one (page, KV head); centroid (block top-k): the mean key, d elements
   constexpr int ROW_ELEMS = KIND == VX_SUMMARY_CENTROID ? D : 2 * D;
@@ -100,7 +100,22 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   T* s_qh = reinterpret_cast<T*>(smem + (size_t)kScStages * STAGE_BYTES);          // MAX: [Hq][2*D] in T: min(q_h,0) | max(q_h,0)
 
   const int warp = threadIdx.x / kWarp, lane = threadIdx.x % kWarp;
-  const int flat_lo = page_indptr[req_begin], flat_span = page_indptr[req_end] - flat_lo;   // this launch's request window
+  // this launch's request window in the flat page list (known to the host when the window is the whole batch: one
+  // cold memory latency less at the head of every CTA)
+  const int flat_lo = flat_span_host >= 0 ? flat_lo_host : page_indptr[req_begin];
+  const int flat_span = flat_span_host >= 0 ? flat_span_host : page_indptr[req_end] - flat_lo;
+  // The window's queries -> L2, a slice per CTA, before the summary stream saturates HBM: a CTA whose range crosses
+  // into the next request rebuilds its query vector in mid-stream, and with the queries cold that stall was two
+  // loaded memory latencies (~2 us) on the CTAs that finish last (profiles/r1e_trace.md).  The attention kernel
+  // of the step reads the same queries later.
+  if (threadIdx.x >= kScConsumerWarps * kWarp) {
+    const int64_t q_bytes = (int64_t)(req_end - req_begin) * num_q_heads * D * (int)sizeof(T);
+    const int64_t per_cta = ((q_bytes + gridDim.x - 1) / gridDim.x + 127) / 128 * 128;
+    const int64_t off = per_cta * blockIdx.x + (int64_t)(threadIdx.x % kWarp) * 128;
+    const uint8_t* qb = reinterpret_cast<const uint8_t*>(q + (int64_t)req_begin * num_q_heads * D);
+    for (int64_t o = off; o < min(per_cta * (blockIdx.x + 1), q_bytes); o += kWarp * 128)
+      asm volatile("prefetch.global.L2 [%0];" ::"l"(qb + o));
+  }
   const int begin = flat_lo + (int)((int64_t)flat_span * blockIdx.x / gridDim.x);
   const int end = flat_lo + (int)((int64_t)flat_span * (blockIdx.x + 1) / gridDim.x);
   if (threadIdx.x == 0) {
@@ -423,7 +438,8 @@ static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summar
   if (ctas < 1) ctas = 1;
   score_kernel<T, D, PG, HKV, kScStages, AGG, KIND><<<ctas, kScThreads, smem, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, pt.batch, pt.page_indptr,
-      pt.page_indices, pt.total_pages, scores, rr.begin, rr.begin + (rr.count < 0 ? pt.batch : rr.count));
+      pt.page_indices, pt.total_pages, scores, rr.begin, rr.begin + (rr.count < 0 ? pt.batch : rr.count), 0,
+      rr.count < 0 ? pt.total_pages : -1);
   c->launches += 1;
   return cudaGetLastError();
 }
