@@ -48,3 +48,41 @@ def test_decode_on_random_unordered_selections(name, seed):
     q, opool, opt = to_oracle(w)
     o_ref, l_ref = vo.sparse_attention(q, opool, opt, sl, sc, s.num_q_heads, s.num_kv_heads, s.qk_dim, s.v_dim, s.sm_scale)
     check_attention(s.dtype, out.float().cpu().numpy(), lse.cpu().numpy(), o_ref, l_ref)
+
+
+@pytest.mark.parametrize("batch,splits", [(3, 8), (20, 4), (40, 3), (50, 2)])
+def test_mla_decode_cluster_merge_at_every_cluster_size(batch, splits):
+    """The MLA decode merges the splits of a request inside a thread-block cluster (2, 4 or 8 CTAs, DESIGN.md 7;
+    any other count goes through global partials and an arrival counter):
+    batches chosen so that the split heuristic picks each size, selections shorter than the split count included
+    (empty splits), the fused step against the oracle."""
+    from dataclasses import replace
+    import paper_2606_06453_b200 as vx
+    from paper_2606_06453_b200.workloads import make_workload, SPECS
+    from tests.oracle_io import oracle_step
+    from tests.parity import check_selection, oracle_attention_on
+    w = make_workload(replace(SPECS["C4-small"], name=f"C4-small-b{batch}", batch=batch, seq_len=(200, 3000)), device="cuda:0")
+    s = w.spec
+    ctx = vx.context_for(w)
+    pool, pt = vx.tables_for(w)
+    summary = vx.alloc_summary(w)
+    ctx.page_summary_update(pool, pt, summary, first_new_pos=torch.zeros_like(w.seq_lens))
+    dev = "cuda:0"
+    out = torch.full((s.batch, s.num_q_heads, s.v_dim), float("nan"), dtype=w.q.dtype, device=dev)
+    lse = torch.full((s.batch, s.num_q_heads), float("nan"), dtype=torch.float32, device=dev)
+    sp = torch.empty(s.batch, s.num_kv_heads, w.max_budget, dtype=torch.int32, device=dev)
+    sl = torch.empty_like(sp)
+    sc = torch.empty(s.batch, s.num_kv_heads, dtype=torch.int32, device=dev)
+    for _ in range(2):                            # twice: the kernel leaves no state behind
+        out.fill_(float("nan"))
+        ctx.sparse_decode_step(w.q, pool, summary, pt, w.budget, w.max_budget, out, lse, sp, sl, sc)
+    torch.cuda.synchronize()
+    # the split count the library picks for this batch (its heuristic, restated): whole waves of equal CTAs
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    cost = lambda sp: -(-s.batch * sp // sms) * (-(-w.max_budget // sp) + 2)
+    assert min(range(1, min(32, w.max_budget, s.num_q_heads) + 1), key=lambda sp: (cost(sp), sp)) == splits
+    ref = oracle_step(w)
+    sl_h, sc_h = sl.cpu().numpy(), sc.cpu().numpy()
+    check_selection(w, sl_h, sp.cpu().numpy(), sc_h, ref)
+    o_ref, l_ref = oracle_attention_on(w, sl_h, sc_h)
+    check_attention(s.dtype, out.float().cpu().numpy(), lse.cpu().numpy(), o_ref, l_ref)
