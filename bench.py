@@ -59,9 +59,9 @@ def measured_peak():
 
 def ncu_traffic(cfg, stage):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
-    `ncu --set full` capture (profiles/r1d_traffic.csv; commands in profiles/r1d_final.md), or None."""
+    `ncu --set full` capture (profiles/r1e_traffic.csv; commands in profiles/r1e_final.md), or None."""
     kernel = {"page_score": ("score_kernel",), "sparse_paged_decode": ("decode_gqa_mma_kernel", "decode_mla_kernel")}[stage]
-    path = os.path.join(ROOT, "profiles", "r1d_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "r1e_traffic.csv")
     if not os.path.exists(path):
         return None
     import csv
