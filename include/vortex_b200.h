@@ -126,6 +126,16 @@ const char *vx_last_error(const vx_ctx *ctx);
 /* Number of kernel launches the last compute call on this context enqueued (host counter). */
 int32_t vx_last_launch_count(const vx_ctx *ctx);
 
+/* Phase tracing (not part of the paper's method).  Only a library built with -DVX_TRACE
+ * (`python -m paper_2606_06453_b200.build --trace` -> libvortex_b200_trace.so) records anything; the
+ * product library returns VX_ERR_UNSUPPORTED.  `buffer` is a DEVICE pointer to max_ctas * 16 int64, owned
+ * by the caller and zeroed by it; from the next launch on, every CTA (linear block index < max_ctas) of the
+ * kernels named in `kernels` stores %globaltimer nanoseconds at its phase boundaries into its 16 slots
+ * (slot 15: SM id; slot meanings: paper_2606_06453_b200/trace.py).  buffer == NULL detaches.  Attach one kind
+ * at a time: the kinds share the slot numbering. */
+enum { VX_TRACE_SCORE = 1, VX_TRACE_TOPK = 2, VX_TRACE_DECODE = 4 };
+vx_status vx_trace_attach(vx_ctx *ctx, void *buffer, int32_t max_ctas, int32_t kernels);
+
 /* ---- (a1) summaries: PAPER.md:546 envelope, :89 query-independent, :529 per block ---- */
 /* For request i, rebuilds from the K pool the summary of every logical page
  * j >= first_new_pos[i] / page_size (first_new_pos == NULL: only the last page, i.e. the page

@@ -19,10 +19,11 @@ VX_DT_BF16, VX_DT_F32 = 0, 1
 VX_AGG_SUM, VX_AGG_MAX = 0, 1
 VX_SUMMARY_ENVELOPE, VX_SUMMARY_CENTROID = 0, 1
 VX_STEP_UPDATE_SUMMARY = 1
+VX_TRACE_SCORE, VX_TRACE_TOPK, VX_TRACE_DECODE = 1, 2, 4
 
 EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",
            "vx_page_summary_update", "vx_page_score", "vx_topk_pages", "vx_sparse_paged_decode",
-           "vx_sparse_decode_step", "vx_sparse_decode_step_host"]
+           "vx_sparse_decode_step", "vx_sparse_decode_step_host", "vx_trace_attach"]
 
 
 class VxGeom(C.Structure):
@@ -56,10 +57,12 @@ def load_library():
     global _lib
     if _lib is not None:
         return _lib
-    if not os.path.exists(LIB_PATH):
-        raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2606_06453_b200.build` "
+    # VX_B200_LIBRARY: another build of the same library (trace.py points it at libvortex_b200_trace.so)
+    path = os.environ.get("VX_B200_LIBRARY") or LIB_PATH
+    if not os.path.exists(path):
+        raise ImportError(f"{path} is missing: run `python -m paper_2606_06453_b200.build` "
                           "(there is no CPU fallback)")
-    lib = C.CDLL(LIB_PATH)
+    lib = C.CDLL(path)
     P, I32, U32, SZ = C.c_void_p, C.c_int32, C.c_uint32, C.c_size_t
     G, T, K = C.POINTER(VxGeom), C.POINTER(VxPageTable), C.POINTER(VxKvPool)
     sig = {
@@ -68,6 +71,7 @@ def load_library():
         "vx_destroy": (None, [P]),
         "vx_last_error": (C.c_char_p, [P]),
         "vx_last_launch_count": (I32, [P]),
+        "vx_trace_attach": (I32, [P, P, I32, I32]),
         "vx_page_summary_update": (I32, [P, K, T, P, P, P]),
         "vx_page_score": (I32, [P, P, P, T, P, P]),
         "vx_topk_pages": (I32, [P, P, T, P, I32, P, P, P, P]),
@@ -165,6 +169,11 @@ class Context:
     def page_score(self, q, summary, pt: PageTable, scores, stream=None):
         self._check(self.lib.vx_page_score(self._h, _ptr(q), _ptr(summary), C.byref(pt.c), _ptr(scores),
                                            _stream(stream)))
+
+    def trace_attach(self, buffer, kernels):
+        """buffer: int64 CUDA tensor [max_ctas, 16], zeroed by the caller (None detaches); trace builds only."""
+        n = 0 if buffer is None else buffer.shape[0]
+        self._check(self.lib.vx_trace_attach(self._h, _ptr(buffer), n, kernels))
 
     def topk_pages(self, scores, pt: PageTable, budget, max_budget, sel_phys, sel_logical, sel_count,
                    stream=None):

@@ -190,6 +190,20 @@ const char* vx_last_error(const vx_ctx* ctx) { return ctx ? ctx->err : g_create_
 
 int32_t vx_last_launch_count(const vx_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
+vx_status vx_trace_attach(vx_ctx* c, void* buffer, int32_t max_ctas, int32_t kernels) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  if (max_ctas < 0) return fail(c, VX_ERR_INVALID_ARG, "negative max_ctas");
+  if (cudaError_t e = cudaSetDevice(c->device)) return check_cuda(c, e, "vx_trace_attach");
+  long long* b = static_cast<long long*>(buffer);
+  const int n = buffer ? max_ctas : 0;
+  cudaError_t e = vx_trace_set_score((kernels & VX_TRACE_SCORE) ? b : nullptr, n);
+  if (e == cudaErrorNotSupported) return fail(c, VX_ERR_UNSUPPORTED, "this library was built without -DVX_TRACE");
+  if (e == cudaSuccess) e = vx_trace_set_topk((kernels & VX_TRACE_TOPK) ? b : nullptr, n);
+  if (e == cudaSuccess) e = vx_trace_set_decode_gqa((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
+  if (e == cudaSuccess) e = vx_trace_set_decode_mla((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
+  return check_cuda(c, e, "vx_trace_attach");
+}
+
 vx_status vx_page_summary_update(vx_ctx* c, const vx_kv_pool* pool, const vx_page_table* pt,
                                  const int32_t* first_new_pos, void* summary, vx_stream stream) {
   if (!c) return VX_ERR_INVALID_ARG;

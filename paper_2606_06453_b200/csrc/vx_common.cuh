@@ -108,6 +108,42 @@ __device__ __forceinline__ float ldcg_f32(const float* p) {
   return v;
 }
 
+// ---- phase tracing (builds with -DVX_TRACE only: `python -m paper_2606_06453_b200.build --trace`) ------------------
+// vx_trace_attach() hands the kernels of one kind a device buffer of 16 int64 slots per CTA; VX_TRACE_STAMP(cta, k)
+// stores %globaltimer (ns, one clock for the whole GPU) into slot k of CTA `cta`.  The slot meanings are listed in
+// paper_2606_06453_b200/trace.py, which prints the per-CTA timelines kept in profiles/.  Without -DVX_TRACE the
+// macro is empty and the product library contains none of this.
+#ifdef VX_TRACE
+static __device__ long long* g_vx_trace_buf;     // one copy per translation unit (set by its vx_trace_set_* below)
+static __device__ int g_vx_trace_ctas;
+#define VX_TRACE_STAMP(cta, k)                                                            \
+  do {                                                                                    \
+    if (g_vx_trace_buf != nullptr && (int)(cta) < g_vx_trace_ctas) {                      \
+      long long t_;                                                                       \
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                              \
+      g_vx_trace_buf[(long long)(cta) * 16 + (k)] = t_;                                   \
+    }                                                                                     \
+  } while (0)
+#define VX_TRACE_SMID(cta)                                                                \
+  do {                                                                                    \
+    if (g_vx_trace_buf != nullptr && (int)(cta) < g_vx_trace_ctas) {                      \
+      unsigned sm_;                                                                       \
+      asm volatile("mov.u32 %0, %%smid;" : "=r"(sm_));                                    \
+      g_vx_trace_buf[(long long)(cta) * 16 + 15] = sm_;                                   \
+    }                                                                                     \
+  } while (0)
+#define VX_TRACE_SETTER(name)                                                             \
+  cudaError_t name(long long* buf, int ctas) {                                            \
+    cudaError_t e = cudaMemcpyToSymbol(g_vx_trace_buf, &buf, sizeof(buf));                \
+    return e != cudaSuccess ? e : cudaMemcpyToSymbol(g_vx_trace_ctas, &ctas, sizeof(ctas)); \
+  }
+#else
+#define VX_TRACE_STAMP(cta, k) do {} while (0)
+#define VX_TRACE_SMID(cta) do {} while (0)
+#define VX_TRACE_SETTER(name) \
+  cudaError_t name(long long*, int) { return cudaErrorNotSupported; }
+#endif
+
 // thread-block cluster (the splits of one request / of one (request, KV head)): barrier over all threads of all CTAs, peer shared-memory reads
 __device__ __forceinline__ void cluster_sync() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");

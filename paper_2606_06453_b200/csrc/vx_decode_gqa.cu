@@ -78,6 +78,8 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
 
   const int split = blockIdx.x, kvh = blockIdx.y, i = blockIdx.z + req0;
   const int warp = threadIdx.x / kWarp, lane = threadIdx.x % kWarp;
+  [[maybe_unused]] const int cta = (blockIdx.z * gridDim.y + blockIdx.y) * gridDim.x + blockIdx.x;
+  if (threadIdx.x == 0) { VX_TRACE_STAMP(cta, 0); VX_TRACE_SMID(cta); }
   const int grp = num_q_heads / num_kv_heads;
   const int n_tok = seq_lens[i];
   const int newest_page = (n_tok - 1) / kGqaPage;
@@ -95,7 +97,9 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
       qb[ks][1] = h < grp ? *reinterpret_cast<const uint32_t*>(qrow + c + 8) : 0u;
     }
   }
+  if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 1);
   pdl_wait();                                   // the selection lists come from the preceding kernel of the step
+  if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 2);
 
   const int cnt = cnt_known >= 0 ? cnt_known : sel_count[i * num_kv_heads + kvh];
   const int per_split = (cnt + num_splits - 1) / num_splits;
@@ -147,10 +151,13 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     if (p < my_pages) issue(p);
     cp_async_commit();
   }
+  if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 3);
 
   for (int p = 0; p < my_pages; ++p) {
     cp_async_wait<kGqaStages - 2>();            // page p has landed (this lane's copies)
-    __syncwarp();                               // ... and every lane's; also: all lanes are done with page p-1
+    __syncwarp();
+    if (threadIdx.x == 0 && p == 0) VX_TRACE_STAMP(cta, 4);
+    if (threadIdx.x == 0 && p == my_pages - 1) VX_TRACE_STAMP(cta, 5);                               // ... and every lane's; also: all lanes are done with page p-1
     const int valid_enc = s_valid[warp][p % kGqaStages];
     const int valid = valid_enc & 255;
     const int phys_p = s_phys[warp][p % kGqaStages];
@@ -258,6 +265,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   }
   cp_async_wait<0>();
   pdl_trigger();
+  if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 6);
 
   // per-warp denominators: sum the lane partials of each head column
 #pragma unroll
@@ -270,6 +278,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     s_l[warp][2 * lane] = l_a; s_l[warp][2 * lane + 1] = l_b;
   }
   __syncthreads();                              // every warp is done with its ring: reuse it for the merge
+  if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 7);
   const int ha = 2 * (lane % 4);
   float mb_a = -INFINITY, mb_b = -INFINITY;
 #pragma unroll
@@ -305,12 +314,19 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
       if (d == 0) part_lse[head_row * num_splits + split] = lse;
     }
   }
+  if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 8);
   if (num_splits > 1) {                         // (a5) the last split of this (request, KV head) merges by LSE
-    if (last_split_arrives(unit_counter + i * num_kv_heads + kvh, num_splits, &s_last))
+    if (last_split_arrives(unit_counter + i * num_kv_heads + kvh, num_splits, &s_last)) {
+      if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 9);
       merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads + kvh * grp, grp, num_splits, D, out, lse_out,
                                      reinterpret_cast<float*>(smem));
+      if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 10);
+    }
   }
+  if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 11);
 }
+
+VX_TRACE_SETTER(vx_trace_set_decode_gqa)
 
 bool gqa_mma_supported(const vx_geom& g) {
   const int grp = g.num_q_heads / g.num_kv_heads;

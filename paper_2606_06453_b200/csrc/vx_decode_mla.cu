@@ -349,6 +349,8 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
 
   const int split = blockIdx.x, i = blockIdx.z + req0;
   const int tid = threadIdx.x, warp = tid / kWarp, lane = tid % kWarp;
+  [[maybe_unused]] const int cta = blockIdx.z * gridDim.x + blockIdx.x;
+  if (tid == 0) { VX_TRACE_STAMP(cta, 0); VX_TRACE_SMID(cta); }
   const uint32_t raw = smem_u32(smem_raw);
   const uint32_t base = (raw + 1023u) & ~1023u;        // swizzle atoms need 1024-byte alignment
   uint8_t* sm = smem_raw + (base - raw);
@@ -380,6 +382,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
+  if (tid == 0) VX_TRACE_STAMP(cta, 1);
   const uint32_t tmem = s_tmem;
   // Q[32 x 576] -> TMEM lanes 0..31 (heads), 288 columns (zero rows past Hq): coalesced through the (still
   // idle) ring, row pitch padded to 1168 B so that the per-head reads are bank-conflict free
@@ -418,7 +421,9 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   }
   __syncthreads();
   tc_fence_after();
-  pdl_wait();                                          // the selection lists come from the preceding kernel of the step
+  if (tid == 0) VX_TRACE_STAMP(cta, 2);
+  pdl_wait();
+  if (tid == 0) VX_TRACE_STAMP(cta, 3);                                          // the selection lists come from the preceding kernel of the step
 
   const int cnt = cnt_known >= 0 ? cnt_known : sel_count[i];
   const int per_split = (cnt + num_splits - 1) / num_splits;
@@ -464,6 +469,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
           tma_box(dst, &kmap, 128 * j, phys, full);
           tma_box(dst + K_ATOM_BYTES, &kmap, 128 * j + 64, phys, full);
         }
+        if (p == 0) VX_TRACE_STAMP(cta, 4);
       }
       __syncwarp();
     }
@@ -477,6 +483,8 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       mbar_wait(bar(B_PAGE_FULL + rs), (p / N_ROPE) & 1);
       tc_fence_after();
       if (elect_one()) {
+        if (p == 0) VX_TRACE_STAMP(cta, 5);
+        if (p == n_pages - 1) VX_TRACE_STAMP(cta, 6);
 #pragma unroll
         for (int j = 0; j < PAIRS_PER_PAGE; ++j)
 #pragma unroll
@@ -510,6 +518,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
 #pragma unroll
         for (int mb = 0; mb < PAIRS_PER_PAGE; ++mb) umma_commit(bar(B_PAIR_EMPTY + rs * PAIRS_PER_PAGE + mb));
         umma_commit(bar(B_PV_DONE + b));
+        if (p == n_pages - 1) VX_TRACE_STAMP(cta, 7);
       }
       __syncwarp();
     }
@@ -701,19 +710,25 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   }
 
   // ---- (a5) the last split of the request to arrive merges the partials; release TMEM -------------------
+  if (tid == 64) VX_TRACE_STAMP(cta, 8);                // epilogue stored
   tc_fence_before();
   if (cluster_merge) {
     cluster_sync();                                      // every split's tile and LSE are in place
+    if (tid == 0) VX_TRACE_STAMP(cta, 9);
     merge_cluster(sm + OFF_PAIR, s_lse_all, reinterpret_cast<float (*)[NH]>(sm + OFF_PAIR + 96 * 1024), i, num_q_heads, num_splits, split,
                   out, lse_out);
+    if (tid == 0) VX_TRACE_STAMP(cta, 10);
     cluster_sync();                                      // my tile stays until every peer has read it
   } else if (num_splits > 1) {
     if (last_split_arrives(unit_counter + i, num_splits, &s_last))
       merge_splits(part_o, part_lse, i, num_q_heads, num_splits, out, lse_out, sm + OFF_PAIR);
   }
   __syncthreads();
+  if (tid == 0) VX_TRACE_STAMP(cta, 11);
   if (warp == 1) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "n"(TMEM_COLS));
 }
+
+VX_TRACE_SETTER(vx_trace_set_decode_mla)
 
 bool mla_tc_supported(const vx_geom& g) {
   return g.kv_shared && g.dtype == VX_DT_BF16 && g.num_kv_heads == 1 && g.qk_dim == mla::D && g.v_dim == mla::DV &&

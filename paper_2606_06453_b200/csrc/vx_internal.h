@@ -118,6 +118,11 @@ struct PrefetchPlan {
   uint32_t chunk_bytes = 0;                      // page_size * row bytes, contiguous
   int splits = 1, pages_per_split = 0;
 };
+// phase tracing (-DVX_TRACE builds; cudaErrorNotSupported otherwise): one setter per kernel file
+cudaError_t vx_trace_set_score(long long* buf, int ctas);
+cudaError_t vx_trace_set_topk(long long* buf, int ctas);
+cudaError_t vx_trace_set_decode_gqa(long long* buf, int ctas);
+cudaError_t vx_trace_set_decode_mla(long long* buf, int ctas);
 int decode_gqa_splits(const vx_ctx* c, int n_req, int max_budget);
 int decode_mla_splits(const vx_ctx* c, int n_req, int max_budget);
 

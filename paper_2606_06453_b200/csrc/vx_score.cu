@@ -100,6 +100,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   T* s_qh = reinterpret_cast<T*>(smem + (size_t)kScStages * STAGE_BYTES);          // MAX: [Hq][2*D] in T: min(q_h,0) | max(q_h,0)
 
   const int warp = threadIdx.x / kWarp, lane = threadIdx.x % kWarp;
+  if (threadIdx.x == 0) { VX_TRACE_STAMP(blockIdx.x, 0); VX_TRACE_SMID(blockIdx.x); }
   // this launch's request window in the flat page list (known to the host when the window is the whole batch: one
   // cold memory latency less at the head of every CTA)
   const int flat_lo = flat_span_host >= 0 ? flat_lo_host : page_indptr[req_begin];
@@ -108,12 +109,12 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   // into the next request rebuilds its query vector in mid-stream, and with the queries cold that stall was two
   // loaded memory latencies (~2 us) on the CTAs that finish last (profiles/r1e_trace.md).  The attention kernel
   // of the step reads the same queries later.
-  if (threadIdx.x >= kScConsumerWarps * kWarp) {
+  if (threadIdx.x < kScConsumerWarps * kWarp) {    // (the consumers: the producer warp's first copies must not wait)
     const int64_t q_bytes = (int64_t)(req_end - req_begin) * num_q_heads * D * (int)sizeof(T);
     const int64_t per_cta = ((q_bytes + gridDim.x - 1) / gridDim.x + 127) / 128 * 128;
-    const int64_t off = per_cta * blockIdx.x + (int64_t)(threadIdx.x % kWarp) * 128;
+    const int64_t off = per_cta * blockIdx.x + (int64_t)threadIdx.x * 128;
     const uint8_t* qb = reinterpret_cast<const uint8_t*>(q + (int64_t)req_begin * num_q_heads * D);
-    for (int64_t o = off; o < min(per_cta * (blockIdx.x + 1), q_bytes); o += kWarp * 128)
+    for (int64_t o = off; o < min(per_cta * (blockIdx.x + 1), q_bytes); o += kScConsumerWarps * kWarp * 128)
       asm volatile("prefetch.global.L2 [%0];" ::"l"(qb + o));
   }
   const int begin = flat_lo + (int)((int64_t)flat_span * blockIdx.x / gridDim.x);
@@ -138,6 +139,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     int id_cur = chunk0 + lane < end ? page_indices[chunk0 + lane] : 0;
     int id_nxt = chunk0 + kWarp + lane < end ? page_indices[chunk0 + kWarp + lane] : 0;
     GroupIter it(begin, end, batch, page_indptr);         // (its loads fly together with the id loads above)
+    if (lane == 0) VX_TRACE_STAMP(blockIdx.x, 1);
     for (int g = 0; it.next(PG, first, count, req); ++g) {
       const int s = g % kScStages;
       if (g >= kScStages) sc_mbar_wait(smem_u32(&s_empty[s]), ((g / kScStages) - 1) & 1);
@@ -156,7 +158,10 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
       if (lane < count)
         bulk_g2s(smem_u32(smem + (size_t)s * STAGE_BYTES + (size_t)lane * PAGE_BYTES),
                  reinterpret_cast<const uint8_t*>(summary) + phys * PAGE_BYTES, (uint32_t)PAGE_BYTES, bar);
+      if (lane == 0 && g == 0) VX_TRACE_STAMP(blockIdx.x, 2);
+      if (lane == 0 && g == kScStages - 1) VX_TRACE_STAMP(blockIdx.x, 3);
     }
+    if (lane == 0) VX_TRACE_STAMP(blockIdx.x, 4);
     return;
   }
 
@@ -169,6 +174,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   for (int g = 0; it.next(PG, first, count, req); ++g) {
     const int s = g % kScStages;
     if (req != cur_req) {                        // new request: rebuild [Qm | Qp] for all KV heads (rare)
+      if (threadIdx.x == 0) VX_TRACE_STAMP(blockIdx.x, cur_req < 0 ? 5 : 7);
       asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
       if constexpr (AGG == VX_AGG_MAX) {
         // per-head vectors (PAPER.md:556 max_h variant): u[h] = [min(q_h,0) | max(q_h,0)] . [m | M], exact in T
@@ -261,6 +267,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
       }
       }
       asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
+      if (threadIdx.x == 0) VX_TRACE_STAMP(blockIdx.x, cur_req < 0 ? 6 : 8);
       cur_req = req;
       if constexpr (AGG == VX_AGG_SUM) {
 #pragma unroll
@@ -272,6 +279,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
       }
     }
     sc_mbar_wait(smem_u32(&s_full[s]), (g / kScStages) & 1);
+    if (threadIdx.x == 0 && g == 0) VX_TRACE_STAMP(blockIdx.x, 9);
     const int rows = count * HKV;                // row r = page (r / HKV), head (r % HKV)
     if constexpr (NARROW) {
       constexpr int KIT = RPW / RPI;             // instructions per group; instruction i covers rows warp + 8 (i RPI + lane / NCH)
@@ -393,7 +401,10 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     const int r = warp + (lane / LPR) * kScConsumerWarps;
     if ((lane % LPR) == 0 && r < rows) scores[(int64_t)kvh * total_pages + first + r / HKV] = tot;
   }
+  if (threadIdx.x == 0) VX_TRACE_STAMP(blockIdx.x, 11);
 }
+
+VX_TRACE_SETTER(vx_trace_set_score)
 
 bool score_geometry_supported(const vx_geom& g) {
   if (g.agg != VX_AGG_SUM && g.agg != VX_AGG_MAX) return false;

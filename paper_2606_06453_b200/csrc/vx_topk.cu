@@ -342,11 +342,15 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
 
   const int kvh = blockIdx.x, i = blockIdx.y + req0;
   const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
+  [[maybe_unused]] const int cta = blockIdx.y * gridDim.x + blockIdx.x;
+  if (tid == 0) { VX_TRACE_STAMP(cta, 0); VX_TRACE_SMID(cta); }
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
   const int k = min(budget[i], max_budget);
   const int row0 = page_indptr[i];
   for (int b = tid; b < kBins; b += THREADS) s_hist[b] = 0;      // first pass's histogram, zeroed under the loads
+  if (tid == 0) VX_TRACE_STAMP(cta, 1);
   pdl_wait();                                   // the scores (and, in a step, nothing else) come from the predecessor
+  if (tid == 0) VX_TRACE_STAMP(cta, 2);
   const int64_t out0 = ((int64_t)i * num_kv_heads + kvh) * max_budget;
   const int n_sel = min(k, n_pages);
   if (tid == 0) sel_count[i * num_kv_heads + kvh] = n_sel;
@@ -383,6 +387,7 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   kmax = __reduce_max_sync(0xffffffffu, kmax);
   if (lane == 0) { s_wmin[warp] = kmin; s_wmax[warp] = kmax; }
   __syncthreads();
+  if (tid == 0) VX_TRACE_STAMP(cta, 3);
 #pragma unroll
   for (int w = 0; w < WARPS; ++w) { kmin = min(kmin, s_wmin[w]); kmax = max(kmax, s_wmax[w]); }
 
@@ -413,6 +418,7 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
         if (((live >> u) & 1u) && key[u] >= lo && (uint64_t)(key[u] - lo) < width)
           atomicAdd(&s_hist[fpass ? fbin(key[u]) : (int)((key[u] - lo) >> shift)], 1);
       __syncthreads();
+      if (tid == 0) VX_TRACE_STAMP(cta, 4);           // (the last pass's, if the select recurses)
       // threshold bin: the highest b with  #keys in bins > b  <  need  <=  #keys in bins >= b
       int h[BPT], mine = 0;
 #pragma unroll
@@ -435,6 +441,7 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
       }
       if (tid == 0) { s_nlist = 0; s_bmin = 0xFFFFFFFFu; s_bmax = 0u; }
       __syncthreads();
+      if (tid == 0) VX_TRACE_STAMP(cta, 5);
       const int bin = s_bin, cnt = s_cnt;
       need -= s_above;                          // still to take from the threshold bin
       const uint32_t bin_lo = lo + ((uint32_t)bin << shift);
@@ -486,6 +493,7 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
     }
   }
 
+  if (tid == 0) VX_TRACE_STAMP(cta, 6);
   pdl_trigger();
   // ---- ordered emission: class of a page = sure (forced or key > thr) / tie (key == thr, first need_eq by index) --
   unsigned m_sure[kKpt], m_tie[kKpt];
@@ -502,6 +510,7 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   }
   if (lane == 0) s_wcnt[warp] = make_int2(n_sure, n_tie);
   __syncthreads();
+  if (tid == 0) VX_TRACE_STAMP(cta, 7);
   int gt = 0, eq = 0;                           // sure / tie pages before this warp's run
 #pragma unroll
   for (int w = 0; w < WARPS; ++w) {
@@ -530,6 +539,7 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   }
   if (staged) {                                   // every selected page: one independent gather + two stores
     __syncthreads();
+    if (tid == 0) VX_TRACE_STAMP(cta, 8);
     const int per_split = (n_sel + pf.splits - 1) / pf.splits;
     for (int r = tid; r < n_sel; r += THREADS) {
       const int j = s_hist[r];
@@ -547,7 +557,10 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
     sel_phys[out0 + r] = -1;
     if (sel_logical) sel_logical[out0 + r] = -1;
   }
+  if (tid == 0) VX_TRACE_STAMP(cta, 9);
 }
+
+VX_TRACE_SETTER(vx_trace_set_topk)
 
 template <int THREADS, int kKpt>
 static cudaError_t launch_topk_reg(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,

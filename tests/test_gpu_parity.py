@@ -5,6 +5,8 @@ last pages) where the oracle runs in seconds; full-size sampled parity is in tes
 """
 from dataclasses import replace
 
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -283,3 +285,23 @@ def test_empty_batch_and_bad_arguments():
     with pytest.raises(vx.VortexError) as e:
         vx.context_for(w, qk_dim=80, v_dim=80)
     assert e.value.status == 2
+
+
+def test_trace_attach_is_refused_by_the_product_library_and_works_in_the_trace_build():
+    """vx_trace_attach (include/vortex_b200.h): the product library carries no stamps and says so; the -DVX_TRACE
+    build records one timeline per CTA (paper_2606_06453_b200/trace.py, run here on a small config)."""
+    import subprocess
+    import sys
+    import paper_2606_06453_b200 as vxm
+    from paper_2606_06453_b200.binding import VortexError, VX_ERR_UNSUPPORTED, VX_TRACE_SCORE
+    vx, w, ctx, pool, pt = setup("C2-small")
+    buf = torch.zeros(64, 16, dtype=torch.int64, device="cuda:0")
+    with pytest.raises(VortexError) as e:
+        ctx.trace_attach(buf, VX_TRACE_SCORE)
+    assert e.value.status == VX_ERR_UNSUPPORTED
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for kernel in ("score", "topk", "decode"):
+        r = subprocess.run([sys.executable, "-m", "paper_2606_06453_b200.trace", "--config", "C2-small", "--kernel", kernel,
+                            "--iters", "1"], cwd=root, capture_output=True, text=True, timeout=600)
+        assert r.returncode == 0, r.stderr[-2000:]
+        assert "entry" in r.stdout and "CTAs on" in r.stdout, r.stdout
