@@ -203,3 +203,24 @@ def subproblem(w: Workload, requests) -> Workload:
                     max_budget=w.max_budget, total_pages=len(rows),
                     max_pages_per_req=int(counts.max()),
                     planted=[w.planted[r] for r in requests] if w.planted else [])
+
+
+APPD_DISTRIBUTIONS = ("bimodal", "normal", "lognormal", "uniform")
+
+
+def appd_scores(dist: str, shape, seed: int) -> torch.Tensor:
+    """Seeded fp32 page scores with the value distributions of the paper's top-k study (PAPER.md:485, :497:
+    bimodal, normal, lognormal, uniform; its parameters are not printed -- these are stand-ins).  CPU tensor;
+    inputs only, no arithmetic of the method."""
+    gen = torch.Generator(device="cpu").manual_seed(seed)
+    if dist == "normal":
+        return torch.randn(shape, generator=gen) * 32.0 + 900.0
+    if dist == "uniform":
+        return torch.rand(shape, generator=gen) * 100.0
+    if dist == "lognormal":
+        return torch.exp(torch.randn(shape, generator=gen) * 1.5)
+    if dist == "bimodal":
+        pick = torch.rand(shape, generator=gen) < 0.1
+        return torch.where(pick, torch.randn(shape, generator=gen) * 2.0 + 40.0,
+                           torch.randn(shape, generator=gen) * 2.0 - 10.0)
+    raise ValueError(dist)

@@ -1,0 +1,136 @@
+"""Pins for the approximate radix top-k oracle (oracle/vx_oracle_approx.py).
+
+The paper prints no worked example, so the pins are: tolerate_ratio 0 == the exact oracle (an independent
+full-sort implementation in vx_oracle.c) and == brute force; the published SplitMix64 vector; the error bound
+the method states (recall@k >= 1 - tolerate_ratio); structural invariants; the sampler's inclusion frequency.
+"""
+import os
+
+import numpy as np
+import pytest
+
+from oracle import vx_oracle as vo
+from oracle import vx_oracle_approx as va
+from paper_2606_06453_b200.workloads import APPD_DISTRIBUTIONS, appd_scores
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def exact_sets(scores, P_list, budget, n_sink, n_local, max_budget, page_size=16):
+    indptr = np.concatenate([[0], np.cumsum(P_list)]).astype(np.int32)
+    pt = vo.PageTable(indptr, np.arange(indptr[-1], dtype=np.int32),
+                      np.array([p * page_size for p in P_list], dtype=np.int32), page_size)
+    sl, _, sc, _ = vo.topk_pages(scores.astype(np.float64), pt, budget, n_sink, n_local, max_budget)
+    return indptr, pt, sl, sc
+
+
+def test_splitmix64_published_vector():
+    rows = [l.split() for l in open(os.path.join(HERE, "golden", "splitmix64.txt")) if not l.startswith("#")]
+    assert len(rows) == 5
+    for seed, idx, val in rows:
+        assert va.splitmix64(int(seed), int(idx)) == int(val)
+
+
+def test_keys_preserve_order_and_merge_zeros():
+    x = np.array([-np.inf, -3.5, -1e-40, -0.0, 0.0, 1e-40, 2.0, 900.0, np.inf], dtype=np.float32)
+    k = va.float_keys(x).astype(np.int64)
+    assert (np.diff(k) >= 0).all() and k[3] == k[4] and (np.diff(k)[[0, 1, 2, 4, 5, 6, 7]] > 0).all()
+    back = va.key_floats(va.float_keys(x))
+    assert np.array_equal(back[[0, 1, 2, 5, 6, 7, 8]], x[[0, 1, 2, 5, 6, 7, 8]])
+
+
+@pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
+def test_ratio_zero_is_the_exact_selection(dist):
+    hkv, P_list, k = 2, [700, 2048, 300], 64
+    T = sum(P_list)
+    scores = appd_scores(dist, (hkv, T), seed=11).numpy()
+    budget = np.full(len(P_list), k, dtype=np.int32)
+    indptr, pt, sl_e, sc_e = exact_sets(scores, P_list, budget, 1, 2, k)
+    sl, sp, sc, early = va.approx_topk_pages(scores, indptr, pt.page_indices, pt.seq_lens, 16, budget, 1, 2, k, 0.0, 5)
+    assert not early.any()
+    assert np.array_equal(sc, sc_e) and np.array_equal(sl, sl_e)
+
+
+def test_ratio_zero_heavy_ties_and_sign_spanning_ranges():
+    rng = np.random.default_rng(3)
+    for trial in range(30):
+        P = int(rng.integers(20, 900))
+        k = int(rng.integers(4, min(P, 200)))
+        kind = trial % 3
+        if kind == 0:
+            s = rng.integers(-3, 4, size=(1, P)).astype(np.float32)               # heavy ties, +-0
+        elif kind == 1:
+            s = (rng.standard_normal((1, P)) * 10.0 ** rng.integers(-20, 20)).astype(np.float32)
+        else:
+            s = np.round(rng.standard_normal((1, P)) * 4).astype(np.float32) / 4 + 1000.0
+        budget = np.array([k], dtype=np.int32)
+        indptr, pt, sl_e, sc_e = exact_sets(s, [P], budget, 1, 2, k)
+        sl, _, sc, _ = va.approx_topk_pages(s, indptr, pt.page_indices, pt.seq_lens, 16, budget, 1, 2, k, 0.0, trial)
+        assert np.array_equal(sl, sl_e), (trial, P, k)
+
+
+def test_ratio_zero_brute_force_tiny():
+    rng = np.random.default_rng(4)
+    for trial in range(200):
+        P = int(rng.integers(1, 13))
+        n_sink, n_local = int(rng.integers(0, 3)), int(rng.integers(0, 3))
+        k = int(rng.integers(n_sink + n_local, max(n_sink + n_local + 1, P + 3)))
+        if k == 0:
+            continue
+        s = rng.integers(0, 5, size=P).astype(np.float32) if trial % 2 else rng.standard_normal(P).astype(np.float32)
+        forced = [j for j in range(P) if j < n_sink or j >= P - n_local]
+        rest = sorted((j for j in range(P) if j not in forced), key=lambda j: (-float(s[j]), j))
+        want = sorted(set(forced) | set(rest[:max(0, k - len(forced))])) if k < P else list(range(P))
+        got, _ = va.select_one(s, k, n_sink, n_local, 0.0, 0, 0)
+        assert got.tolist() == want, (trial, P, k, n_sink, n_local)
+
+
+@pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
+@pytest.mark.parametrize("tau", [0.05, 0.25, 1.0])
+def test_invariants_and_error_bound(dist, tau):
+    P, k, n_sink, n_local = 4096, 128, 1, 2
+    scores = appd_scores(dist, (4, P), seed=21).numpy()
+    any_early = False
+    for h in range(4):
+        s = scores[h]
+        exact, _ = va.select_one(s, k, n_sink, n_local, 0.0, 0, h)
+        indptr, pt, sl_e, _ = exact_sets(s[None], [P], np.array([k], np.int32), n_sink, n_local, k)
+        assert exact.tolist() == sl_e[0, 0].tolist()
+        sel, info = va.select_one(s, k, n_sink, n_local, tau, 99, h)
+        any_early |= info["early"]
+        assert sel.shape[0] == k and len(set(sel.tolist())) == k and (np.diff(sel) > 0).all()
+        assert {0, P - 2, P - 1} <= set(sel.tolist())                       # PAPER.md:280 forced pages
+        ex = set(exact.tolist())
+        assert set(info["sure"].tolist()) <= ex                             # high-confidence candidates are exact
+        wrong = [j for j in sel.tolist() if j not in ex]
+        assert len(wrong) <= int(np.floor(np.float32(tau) * np.float32(k)))  # the method's error bound
+        assert va.recall_at_k(sel, exact) >= 1.0 - tau - 1e-12
+        if info["early"]:
+            assert set(wrong) <= set(info["members"].tolist())
+            if info["passes"] == 1:                                         # wrong picks: within one bin of the threshold
+                thr = min(float(s[j]) for j in ex if j not in (0, P - 2, P - 1))
+                w = info["bin_width"] * (1 + 1e-5) + 1e-30
+                assert all(abs(float(s[j]) - thr) <= w for j in wrong)
+        else:
+            assert sel.tolist() == exact.tolist()
+    if tau == 1.0:
+        assert any_early                                                    # ratio 1 stops after the first pass
+
+
+def test_sampler_inclusion_frequency_is_need_over_cnt():
+    P, k = 600, 40
+    s = np.zeros(P, dtype=np.float32)
+    s[:] = 5.0                                                              # one huge tie ... but not a single key:
+    s += (np.arange(P) % 7).astype(np.float32) * 1e-4                       # seven close values in one float bin
+    s[100] = 50.0                                                           # widen the range: all others share a bin
+    hits = np.zeros(P)
+    n = 400
+    for seed in range(n):
+        sel, info = va.select_one(s, k, 1, 2, 1.0, seed, 0)
+        assert info["early"] and 100 in sel.tolist()
+        hits[sel] += 1
+    members = info["members"]
+    need = info["need"]
+    freq = hits[members] / n
+    assert abs(freq.mean() - need / len(members)) < 1e-9                    # exactly need picks per draw
+    assert freq.max() < 3 * need / len(members) and freq.min() > 0          # no member favoured or starved
