@@ -168,6 +168,25 @@ vx_status vx_topk_pages(vx_ctx *ctx, const float *scores, const vx_page_table *p
                         int32_t *sel_phys, int32_t *sel_logical, int32_t *sel_count,
                         vx_stream stream);
 
+/* ---- NEXT-3: approximate radix top-k, PAPER.md:194-196 (stochastic early termination), :538 (`approxTopK`,
+ * "tolerate_ratio in [0,1] trades exactness for speed"), :495-509 (judged by recall@k) -----------------------
+ * Same inputs / outputs / layout as vx_topk_pages.  The radix select stops refining as soon as the pages still
+ * to be taken from the threshold bin number at most floor(tolerate_ratio * k): those are drawn from the bin's
+ * members as a cyclic window in page order whose start is SplitMix64(seed, problem = i * Hkv + kvh) >> 32 modulo
+ * the member count (every member equally likely; the same seed reproduces the selection bit for bit).  Forced
+ * pages and every page above the threshold bin are always taken, so at most floor(tolerate_ratio * k) selected
+ * pages differ from the exact set: recall@k >= 1 - tolerate_ratio.  tolerate_ratio = 0 is vx_topk_pages.
+ * The paper prints no pseudo-code; the choices made are readings G20-G23 of DESIGN.md section 12.
+ * VX_ERR_INVALID_ARG if tolerate_ratio is outside [0, 1]; VX_ERR_UNSUPPORTED if tolerate_ratio > 0 and
+ * pt->max_pages_per_req > 8192 (the selection kernel that implements it keeps a request's keys in registers). */
+vx_status vx_topk_pages_approx(vx_ctx *ctx, const float *scores, const vx_page_table *pt,
+                               const int32_t *budget /* dev [B] */, int32_t max_budget,
+                               float tolerate_ratio, uint64_t seed, int32_t *sel_phys,
+                               int32_t *sel_logical, int32_t *sel_count, vx_stream stream);
+/* tolerate_ratio and seed used by vx_sparse_decode_step when its flags carry VX_STEP_APPROX_TOPK
+ * (context state, host side; default 0 = exact).  VX_ERR_INVALID_ARG outside [0, 1]. */
+vx_status vx_set_topk_approx(vx_ctx *ctx, float tolerate_ratio, uint64_t seed);
+
 /* ---- (a4)+(a5) attention over the selected pages: PAPER.md:92 Eq.4, :200, :75 -------- */
 /* out[i,h,:] = softmax_t(sm_scale * q[i,h].K_t) V_t over the valid tokens of the pages listed
  * in sel_logical/sel_phys[i, h/g, 0:sel_count]; lse[i,h] = natural log of the softmax
@@ -180,6 +199,7 @@ vx_status vx_sparse_paged_decode(vx_ctx *ctx, const void *q, const vx_kv_pool *p
 
 /* ---- (a6) the fused step: (a1 append rows) -> a2 -> a3 -> a4 -> a5 in one call -------- */
 #define VX_STEP_UPDATE_SUMMARY 1u /* flags bit 0: first rebuild the last page's summary of each request */
+#define VX_STEP_APPROX_TOPK 2u    /* flags bit 1: select with vx_topk_pages_approx (vx_set_topk_approx's values) */
 /* sel_phys / sel_logical / sel_count are optional outputs (NULL = keep them in the workspace). */
 vx_status vx_sparse_decode_step(vx_ctx *ctx, const void *q, const vx_kv_pool *pool, void *summary,
                                 const vx_page_table *pt, const int32_t *budget, int32_t max_budget,

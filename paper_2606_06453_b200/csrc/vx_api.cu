@@ -237,6 +237,37 @@ vx_status vx_topk_pages(vx_ctx* c, const float* scores, const vx_page_table* pt,
                                          (cudaStream_t)stream), "vx_topk_pages");
 }
 
+vx_status vx_topk_pages_approx(vx_ctx* c, const float* scores, const vx_page_table* pt, const int32_t* budget,
+                               int32_t max_budget, float tolerate_ratio, uint64_t seed, int32_t* sel_phys,
+                               int32_t* sel_logical, int32_t* sel_count, vx_stream stream) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  c->launches = 0;
+  if (vx_status st = check_table(c, pt)) return st;
+  if (!scores || !budget || !sel_phys || !sel_count)
+    return fail(c, VX_ERR_INVALID_ARG, "scores / budget / sel_phys / sel_count is NULL");
+  if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
+  if (!(tolerate_ratio >= 0.f && tolerate_ratio <= 1.f))
+    return fail(c, VX_ERR_INVALID_ARG, "tolerate_ratio %g outside [0, 1]", (double)tolerate_ratio);
+  if (tolerate_ratio > 0.f && pt->max_pages_per_req > kTopkRegMaxPages)
+    return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (got %d)",
+                kTopkRegMaxPages, pt->max_pages_per_req);
+  ApproxPlan ap;
+  ap.tolerate_ratio = tolerate_ratio;
+  ap.seed = seed;
+  return check_cuda(c, launch_topk_pages(c, scores, *pt, budget, max_budget, sel_phys, sel_logical, sel_count,
+                                         (cudaStream_t)stream, false, ReqRange(), PrefetchPlan(), ap),
+                    "vx_topk_pages_approx");
+}
+
+vx_status vx_set_topk_approx(vx_ctx* c, float tolerate_ratio, uint64_t seed) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  if (!(tolerate_ratio >= 0.f && tolerate_ratio <= 1.f))
+    return fail(c, VX_ERR_INVALID_ARG, "tolerate_ratio %g outside [0, 1]", (double)tolerate_ratio);
+  c->approx.tolerate_ratio = tolerate_ratio;
+  c->approx.seed = seed;
+  return VX_OK;
+}
+
 static vx_status decode_dispatch(vx_ctx* c, const void* q, const vx_kv_pool* pool, const vx_page_table* pt,
                                  const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                                  int32_t max_budget, void* out, float* lse, cudaStream_t s,
@@ -274,6 +305,13 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   if (max_budget <= 0 || max_budget > c->max_budget)
     return fail(c, VX_ERR_WORKSPACE, "max_budget %d outside (0, %d]", max_budget, c->max_budget);
   if (pt->batch == 0) return VX_OK;
+  ApproxPlan ap;                                 // exact unless the caller asks for the lossy selection
+  if (flags & VX_STEP_APPROX_TOPK) {
+    ap = c->approx;
+    if (ap.tolerate_ratio > 0.f && pt->max_pages_per_req > kTopkRegMaxPages)
+      return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (got %d)",
+                  kTopkRegMaxPages, pt->max_pages_per_req);
+  }
   cudaStream_t s = (cudaStream_t)stream;
   int32_t* sp = sel_phys ? sel_phys : c->ws.sel_phys;
   int32_t* sl = sel_logical ? sel_logical : c->ws.sel_logical;
@@ -328,7 +366,7 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
       if (pf.pages_per_split < 1) pf.k = nullptr;
     }
     if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, cs,
-                                                       c->use_pdl, rr, pf), "top-k pages"))
+                                                       c->use_pdl, rr, pf, ap), "top-k pages"))
       return st;
     if (vx_status st = decode_dispatch(c, q, pool, pt, sp, sl, sc, max_budget, out, lse, cs, opt)) return st;
     total_launches = c->launches;

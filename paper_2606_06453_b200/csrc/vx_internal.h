@@ -32,6 +32,14 @@ struct Workspace {               // device pointers carved from the caller's wor
 Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32_t max_total_pages,
                           int32_t max_budget);
 
+// Approximate radix top-k (PAPER.md:196 stochastic early termination, :538 `approxTopK`):
+// tolerate_ratio <= 0 is the exact selection.
+struct ApproxPlan {
+  float tolerate_ratio = 0.f;
+  uint64_t seed = 0;
+};
+constexpr int kTopkRegMaxPages = 8 * 1024;       // register-resident selection kernel: pages per request
+
 }  // namespace vx
 
 struct vx_ctx {
@@ -48,6 +56,7 @@ struct vx_ctx {
   int chains;                    // request windows run as concurrent kernel chains inside a fused step (VX_CHAINS, 1 or 2)
   cudaStream_t aux_stream;       // second chain's stream; fork / join with the caller's stream by events
   cudaEvent_t ev_fork, ev_join;
+  vx::ApproxPlan approx;         // vx_set_topk_approx: used by a fused step with VX_STEP_APPROX_TOPK
   char err[512];
 };
 
@@ -144,7 +153,8 @@ cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, con
 cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
                               int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl = false,
-                              const ReqRange& rr = ReqRange(), const PrefetchPlan& pf = PrefetchPlan());
+                              const ReqRange& rr = ReqRange(), const PrefetchPlan& pf = PrefetchPlan(),
+                              const ApproxPlan& ap = ApproxPlan());
 cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,

@@ -322,13 +322,17 @@ static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_t
 // re-reads): warp w owns the contiguous run [w * 32 * kKpt, (w+1) * 32 * kKpt) of logical pages, lane-strided inside
 // it (coalesced score loads), so the ordered emission is one ballot per 32 pages.  Fewer, cheaper block-wide phases:
 // this kernel is latency-bound ("top-k selection becomes a bottleneck").
-template <int THREADS, int kKpt>
+// kApprox: the stochastic early termination of PAPER.md:196 (G20-G23): once the pages still to
+// take from the threshold bin number at most floor(tolerate_ratio * k), they are drawn from the bin's members as a
+// random cyclic window in page order instead of refining the bin (no member list, no ranking).
+template <int THREADS, int kKpt, bool kApprox>
 __global__ void __launch_bounds__(THREADS)
 topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
                 const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
                 const int32_t* __restrict__ seq_lens, int page_size, const int32_t* __restrict__ budget,
                 int n_sink, int n_local, int max_budget, int32_t* __restrict__ sel_phys,
-                int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count, int req0, const PrefetchPlan pf) {
+                int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count, int req0, const PrefetchPlan pf,
+                const ApproxPlan ap) {
   constexpr int WARPS = THREADS / kWarp;
   constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
   static_assert(kBins % THREADS == 0, "shape");
@@ -396,15 +400,21 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   int need = k - n_forced;                      // non-forced pages still to take (precondition: >= 0)
   uint32_t thr = kForcedKey;                    // take keys > thr, and the first need_eq keys == thr
   int need_eq = 0;
+  // early termination (kApprox): ties = the members of the threshold bin (key interval [m_lo, m_hi], or float bin
+  // t_bin), taken as the cyclic window of need_eq member ranks that starts at rot
+  bool early = false, fterm = false;
+  uint32_t m_lo = 0u, m_hi = 0u;
+  int t_bin = 0, rot = 0, wrap = 0;
+  const float smin = key_to_float(kmin), smax = key_to_float(kmax);
+  const float fscale = (float)kBins / (smax - smin);
+  auto fbin = [&](uint32_t kk) -> int { return min(kBins - 1, (int)((key_to_float(kk) - smin) * fscale)); };
 
   if (need > 0) {
     uint32_t lo = kmin;
     uint64_t width = (uint64_t)(kmax - kmin) + 1;
     int shift = max(0, (32 - __clz(kmax - kmin)) - kBinBits);     // ((kmax - kmin) >> shift) < kBins
-    const float smin = key_to_float(kmin), smax = key_to_float(kmax);
-    const float fscale = (float)kBins / (smax - smin);
     bool fpass = kmax - kmin >= (1u << 25) && isfinite(fscale) && fscale > 0.f;   // float-domain first pass (see topk_kernel)
-    auto fbin = [&](uint32_t kk) -> int { return min(kBins - 1, (int)((key_to_float(kk) - smin) * fscale)); };
+    [[maybe_unused]] const int tol = kApprox ? (int)(ap.tolerate_ratio * (float)k) : 0;   // floor: both factors >= 0
     bool first = true;
 #pragma unroll 1
     while (true) {
@@ -452,6 +462,23 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
       }
       // members of the threshold bin: rank them if they are few, else continue on their key interval
       const uint64_t bin_w = (uint64_t)1 << shift;
+      if constexpr (kApprox) {
+        if (need <= tol) {                      // enough high-confidence pages: sample the rest from the bin's members
+          early = true;
+          fterm = fpass;
+          t_bin = bin;
+          m_lo = bin_lo;
+          m_hi = (uint32_t)min((uint64_t)bin_lo + bin_w - 1, (uint64_t)lo + width - 1);
+          need_eq = need;
+          uint64_t z = ap.seed + 0x9E3779B97F4A7C15ull * (uint64_t)(i * num_kv_heads + kvh + 1);   // SplitMix64 draw
+          z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+          z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+          z ^= z >> 31;
+          rot = (int)((uint32_t)(z >> 32) % (uint32_t)cnt);
+          wrap = max(0, rot + need - cnt);      // member ranks [0, wrap) and [rot, rot + need - wrap) are taken
+          break;
+        }
+      }
 #pragma unroll
       for (int u = 0; u < kKpt; ++u) {
         const uint32_t kk = key[u];
@@ -501,8 +528,16 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
 #pragma unroll
   for (int u = 0; u < kKpt; ++u) {
     const bool exists = jbase + u * kWarp + lane < n_pages;
-    const bool sure = exists && (key[u] == kForcedKey || key[u] > thr);
-    const bool tie = exists && key[u] != kForcedKey && key[u] == thr;
+    bool sure = exists && (key[u] == kForcedKey || key[u] > thr);
+    bool tie = exists && key[u] != kForcedKey && key[u] == thr;
+    if constexpr (kApprox) {
+      if (early) {
+        const bool cand = exists && key[u] != kForcedKey;
+        const int fb = fterm && cand ? fbin(key[u]) : 0;
+        sure = exists && (key[u] == kForcedKey || (fterm ? fb > t_bin : key[u] > m_hi));
+        tie = cand && (fterm ? fb == t_bin : (key[u] >= m_lo && key[u] <= m_hi));
+      }
+    }
     m_sure[u] = __ballot_sync(0xffffffffu, sure);
     m_tie[u] = __ballot_sync(0xffffffffu, tie);
     n_sure += __popc(m_sure[u]);
@@ -525,8 +560,13 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
     const int j = jbase + u * kWarp + lane;
     const bool sure = (m_sure[u] >> lane) & 1u, tie = (m_tie[u] >> lane) & 1u;
     const int my_gt = gt + __popc(m_sure[u] & lt_mask), my_eq = eq + __popc(m_tie[u] & lt_mask);
-    const bool take = sure || (tie && my_eq < need_eq);
-    const int pos = my_gt + min(my_eq, need_eq);
+    bool take = sure || (tie && my_eq < need_eq);
+    int pos = my_gt + min(my_eq, need_eq);
+    if constexpr (kApprox) {                      // cyclic window of tie ranks (rot = wrap = 0: the same rule)
+      const int span = need_eq - wrap;
+      take = sure || (tie && (my_eq < wrap || (my_eq >= rot && my_eq < rot + span)));
+      pos = my_gt + min(my_eq, wrap) + min(max(my_eq - rot, 0), span);
+    }
     if (take && pos < n_sel) {
       if (staged) s_hist[pos] = j;
       else {
@@ -565,12 +605,14 @@ VX_TRACE_SETTER(vx_trace_set_topk)
 template <int THREADS, int kKpt>
 static cudaError_t launch_topk_reg(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
                                    int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
-                                   cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf) {
+                                   cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf,
+                                   const ApproxPlan& ap) {
   const vx_geom& g = c->g;
   dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
-  cudaError_t e = launch_kernel(topk_reg_kernel<THREADS, kKpt>, grid, dim3(THREADS), 0, s, pdl, scores, g.num_kv_heads,
+  auto kernel = ap.tolerate_ratio > 0.f ? topk_reg_kernel<THREADS, kKpt, true> : topk_reg_kernel<THREADS, kKpt, false>;
+  cudaError_t e = launch_kernel(kernel, grid, dim3(THREADS), 0, s, pdl, scores, g.num_kv_heads,
                                 pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
-                                g.n_sink, g.n_local, max_budget, sel_phys, sel_logical, sel_count, rr.begin, pf);
+                                g.n_sink, g.n_local, max_budget, sel_phys, sel_logical, sel_count, rr.begin, pf, ap);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -578,14 +620,15 @@ static cudaError_t launch_topk_reg(vx_ctx* c, const float* scores, const vx_page
 cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_table& pt,
                               const int32_t* budget, int32_t max_budget, int32_t* sel_phys,
                               int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl, const ReqRange& rr,
-                              const PrefetchPlan& pf) {
+                              const PrefetchPlan& pf, const ApproxPlan& ap) {
   if (pt.batch == 0) return cudaSuccess;
+  if (ap.tolerate_ratio > 0.f && pt.max_pages_per_req > kTopkRegMaxPages) return cudaErrorNotSupported;
   // block size by problem size (VX_TOPK_THREADS overrides, for tuning; it also selects the shared-memory-key kernel)
   static int force = -1;
   if (force < 0) { const char* e = getenv("VX_TOPK_THREADS"); force = e ? atoi(e) : 0; }
   const int n = pt.max_pages_per_req;
-  if (!force && n <= 8 * 1024) {                  // keys fit the registers of one CTA, 8 per thread (16 measured slower)
-#define VX_REG(T, K) return launch_topk_reg<T, K>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf)
+  if ((!force || ap.tolerate_ratio > 0.f) && n <= kTopkRegMaxPages) {                  // keys fit the registers of one CTA, 8 per thread (16 measured slower)
+#define VX_REG(T, K) return launch_topk_reg<T, K>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap)
     if (n <= 1024) VX_REG(128, 8);
     if (n <= 2048) VX_REG(256, 8);
     if (n <= 4096) VX_REG(512, 8);

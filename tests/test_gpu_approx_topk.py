@@ -1,0 +1,116 @@
+"""vx_topk_pages_approx against oracle/vx_oracle_approx.py (-m gpu): bit-exact ids, order, counts and padding.
+Both sides take every decision (keys, bins, the fp32 remap of the first pass, the termination test, the SplitMix64
+draw) on the same fp32 scores, so the lossy selection itself is reproducible and compared exactly
+(DESIGN.md section 12)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import vx_oracle as vo
+from oracle import vx_oracle_approx as va
+from paper_2606_06453_b200.workloads import APPD_DISTRIBUTIONS, appd_scores
+from tests.test_gpu_topk_fuzz import KINDS, draw_scores
+
+pytestmark = pytest.mark.gpu
+
+
+def run_both(scores, pages, seq, indices, budget, n_sink, n_local, tau, seed, b=16):
+    import paper_2606_06453_b200 as vx
+    hkv = scores.shape[0]
+    indptr = np.concatenate([[0], np.cumsum(pages)]).astype(np.int32)
+    T = int(indptr[-1])
+    mb = int(budget.max())
+    ref = va.approx_topk_pages(scores, indptr, indices, np.array(seq, np.int32), b, budget, n_sink, n_local, mb, tau, seed)
+    dev = "cuda:0"
+    ctx = vx.Context(dtype=torch.bfloat16, num_q_heads=4 * hkv, num_kv_heads=hkv, qk_dim=128, v_dim=128, page_size=b,
+                     sm_scale=1.0, n_sink=n_sink, n_local=n_local, max_batch=len(pages), max_total_pages=T,
+                     max_pages_per_req=max(pages), max_budget=mb, device=dev)
+    pt = vx.PageTable(torch.from_numpy(indptr).to(dev), torch.from_numpy(indices).to(dev),
+                      torch.tensor(seq, dtype=torch.int32, device=dev), T, max(pages))
+    sl = torch.full((len(pages), hkv, mb), -7, dtype=torch.int32, device=dev)
+    sp = torch.full_like(sl, -7)
+    sc = torch.full((len(pages), hkv), -7, dtype=torch.int32, device=dev)
+    ctx.topk_pages_approx(torch.from_numpy(scores).to(dev), pt, torch.from_numpy(budget).to(dev), mb, tau, seed,
+                          sp, sl, sc)
+    torch.cuda.synchronize()
+    ctx.close()
+    return ref, (sl.cpu().numpy(), sp.cpu().numpy(), sc.cpu().numpy())
+
+
+@pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
+@pytest.mark.parametrize("tau", [0.0, 0.05, 0.25, 1.0])
+def test_appd_distributions_bit_exact(dist, tau):
+    rng = np.random.default_rng(5)
+    pages = [2048, 777, 8192, 40, 4100]
+    hkv = 2
+    T = sum(pages)
+    seq = [p * 16 - int(rng.integers(0, 16)) for p in pages]
+    indices = rng.permutation(T + 9)[:T].astype(np.int32)
+    budget = np.array([128, 64, 256, 64, 200], np.int32)
+    scores = appd_scores(dist, (hkv, T), seed=31).numpy()
+    (sl_r, sp_r, sc_r, early), (sl, sp, sc) = run_both(scores, pages, seq, indices, budget, 1, 2, tau, 2024)
+    assert np.array_equal(sc, sc_r)
+    assert np.array_equal(sl, sl_r), (dist, tau)
+    assert np.array_equal(sp, sp_r), (dist, tau)
+    if tau == 1.0:
+        assert early[[0, 1, 2, 4]].all()          # budget < pages: one pass, then the sampler (request 3: k >= P)
+    if tau == 0.0:                                # ratio 0 is the exact selection (the C oracle's full sort)
+        indptr = np.concatenate([[0], np.cumsum(pages)]).astype(np.int32)
+        pt_o = vo.PageTable(indptr, indices, np.array(seq, np.int32), 16)
+        sl_e, _, _, _ = vo.topk_pages(scores.astype(np.float64), pt_o, budget, 1, 2, int(budget.max()))
+        assert np.array_equal(sl, sl_e)
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("tau", [0.1, 0.5])
+def test_fuzz_kinds_bit_exact(kind, tau):
+    rng = np.random.default_rng(77 + KINDS.index(kind))
+    n_sink, n_local = int(rng.integers(0, 3)), int(rng.integers(0, 4))
+    pages = [int(x) for x in rng.choice([1, 3, 40, 300, 1025, 2048, 5000, 8192], size=5)]
+    seq = [p * 16 - int(rng.integers(0, 16)) for p in pages]
+    T = sum(pages)
+    indices = rng.permutation(T + 17)[:T].astype(np.int32)
+    budget = np.array([max(n_sink + n_local, int(rng.integers(1, max(2, min(p + 3, 600))))) for p in pages], np.int32)
+    scores = np.stack([draw_scores(rng, kind, T) for _ in range(2)])
+    (sl_r, sp_r, sc_r, _), (sl, sp, sc) = run_both(scores, pages, seq, indices, budget, n_sink, n_local, tau, 9)
+    assert np.array_equal(sc, sc_r)
+    assert np.array_equal(sl, sl_r), kind
+    assert np.array_equal(sp, sp_r), kind
+
+
+def test_seed_changes_only_the_sampled_members_and_recall_holds():
+    pages, k, tau = [4096], 128, 0.25
+    scores = appd_scores("normal", (8, 4096), seed=41).numpy()
+    indices = np.arange(4096, dtype=np.int32)
+    budget = np.array([k], np.int32)
+    exact = run_both(scores, pages, [4096 * 16], indices, budget, 1, 2, 0.0, 0)[1][0]
+    a = run_both(scores, pages, [4096 * 16], indices, budget, 1, 2, tau, 1)[1][0]
+    b = run_both(scores, pages, [4096 * 16], indices, budget, 1, 2, tau, 2)[1][0]
+    assert not np.array_equal(a, b)
+    for h in range(8):
+        assert va.recall_at_k(a[0, h], exact[0, h]) >= 1 - tau
+        assert va.recall_at_k(b[0, h], exact[0, h]) >= 1 - tau
+
+
+def test_argument_checks():
+    import paper_2606_06453_b200 as vx
+    dev = "cuda:0"
+    P = 9000
+    ctx = vx.Context(dtype=torch.bfloat16, num_q_heads=8, num_kv_heads=2, qk_dim=128, v_dim=128, page_size=16,
+                     sm_scale=1.0, n_sink=1, n_local=2, max_batch=1, max_total_pages=P, max_pages_per_req=P,
+                     max_budget=64, device=dev)
+    pt = vx.PageTable(torch.tensor([0, P], dtype=torch.int32, device=dev), torch.arange(P, dtype=torch.int32, device=dev),
+                      torch.tensor([P * 16], dtype=torch.int32, device=dev), P, P)
+    scores = torch.randn(2, P, device=dev)
+    budget = torch.tensor([64], dtype=torch.int32, device=dev)
+    sl = torch.empty(1, 2, 64, dtype=torch.int32, device=dev)
+    sp, sc = torch.empty_like(sl), torch.empty(1, 2, dtype=torch.int32, device=dev)
+    with pytest.raises(vx.VortexError):           # more pages per request than the register kernel holds
+        ctx.topk_pages_approx(scores, pt, budget, 64, 0.25, 1, sp, sl, sc)
+    with pytest.raises(vx.VortexError):
+        ctx.topk_pages_approx(scores, pt, budget, 64, 1.5, 1, sp, sl, sc)
+    with pytest.raises(vx.VortexError):
+        ctx.set_topk_approx(-0.1, 1)
+    ctx.topk_pages_approx(scores, pt, budget, 64, 0.0, 1, sp, sl, sc)     # ratio 0: the exact kernel, any size
+    torch.cuda.synchronize()
+    ctx.close()
