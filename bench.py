@@ -44,6 +44,9 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--summary", default="envelope", choices=["envelope", "centroid"],
                     help="page summary / score flow: Quest envelope (default, the north star) or block top-k centroid")
+    ap.add_argument("--topk-approx", type=float, default=0.0, metavar="RATIO",
+                    help="select with vx_topk_pages_approx at this tolerate_ratio (PAPER.md:196; lossy, recall@k >= "
+                         "1 - RATIO).  Default 0: the exact selection, the north star's path")
     return ap.parse_args()
 
 
@@ -129,7 +132,7 @@ class ClockSampler(threading.Thread):
 class Runner:
     """One workload resident on one GPU: context, pools, summaries, outputs, L2 flush buffer."""
 
-    def __init__(self, cfg, device, seed_offset=0, summary="envelope"):
+    def __init__(self, cfg, device, seed_offset=0, summary="envelope", topk_approx=0.0):
         import torch
         import paper_2606_06453_b200 as vx
         from paper_2606_06453_b200.workloads import make_workload
@@ -138,6 +141,9 @@ class Runner:
         kind = vx.binding.VX_SUMMARY_CENTROID if summary == "centroid" else vx.binding.VX_SUMMARY_ENVELOPE
         self.summary_name = summary
         self.ctx = vx.context_for(w, summary_kind=kind)
+        self.tau = float(topk_approx)
+        self.step_flags = vx.VX_STEP_UPDATE_SUMMARY | (vx.VX_STEP_APPROX_TOPK if self.tau > 0 else 0)
+        self.ctx.set_topk_approx(self.tau, 20260604)
         self.pool, self.pt = vx.tables_for(w)
         self.summary = vx.alloc_summary(w, kind)
         self.ctx.page_summary_update(self.pool, self.pt, self.summary, first_new_pos=torch.zeros_like(w.seq_lens))
@@ -160,13 +166,13 @@ class Runner:
     def step(self):
         self.ctx.sparse_decode_step(self.w.q, self.pool, self.summary, self.pt, self.w.budget, self.w.max_budget,
                                     self.out, self.lse, self.sel_phys, self.sel_logical, self.sel_count,
-                                    flags=self.vx.VX_STEP_UPDATE_SUMMARY)
+                                    flags=self.step_flags)
 
     def step_host(self):
         h = self.h
         self.ctx.sparse_decode_step_host(h["q"], self.pool, self.summary, h["indptr"], h["indices"], h["seq"],
                                          h["budget"], self.w.max_budget, h["out"], h["lse"],
-                                         flags=self.vx.VX_STEP_UPDATE_SUMMARY)
+                                         flags=self.step_flags)
 
     def stage_summary(self):
         self.ctx.page_summary_update(self.pool, self.pt, self.summary, first_new_pos=None)
@@ -175,8 +181,8 @@ class Runner:
         self.ctx.page_score(self.w.q, self.summary, self.pt, self.scores)
 
     def stage_topk(self):
-        self.ctx.topk_pages(self.scores, self.pt, self.w.budget, self.w.max_budget, self.sel_phys,
-                            self.sel_logical, self.sel_count)
+        self.ctx.topk_pages_approx(self.scores, self.pt, self.w.budget, self.w.max_budget, self.tau, 20260604,
+                                   self.sel_phys, self.sel_logical, self.sel_count)   # ratio 0 = vx_topk_pages
 
     def stage_decode(self):
         self.ctx.sparse_paged_decode(self.w.q, self.pool, self.pt, self.sel_phys, self.sel_logical, self.sel_count,
@@ -295,7 +301,7 @@ def main():
         dist.barrier()
 
     peak, peak_src = measured_peak()
-    r = Runner(args.config, device, seed_offset=rank, summary=args.summary)
+    r = Runner(args.config, device, seed_offset=rank, summary=args.summary, topk_approx=args.topk_approx)
     w, s = r.w, r.w.spec
     bytes_ = algorithmic_bytes(w, summary=args.summary)
 
@@ -354,7 +360,7 @@ def main():
         for name in [c for c in args.also.split(",") if c and c != args.config]:
             del r
             torch.cuda.empty_cache()
-            r = Runner(name, device)
+            r = Runner(name, device, topk_approx=args.topk_approx)
             tt = statistics.mean(r.time_device(r.step, 20, 3))
             b2 = algorithmic_bytes(r.w)
             also[name] = {"us": tt * 1e3, "hbm_gbs": b2["total"] / (tt * 1e-3) / 1e9,
@@ -365,6 +371,7 @@ def main():
                 "config": {"workload": args.config, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
                            "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
                            "seq_len": list(s.seq_len), "budget_pages": w.max_budget, "summary": args.summary,
+                           "topk": "exact" if args.topk_approx <= 0 else f"approx tolerate_ratio={args.topk_approx} (lossy)",
                            "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"},
                 "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
                 "step_bytes": bytes_, "stage_us": stage, "roofline": roofline, "cpu_baseline": cpu,

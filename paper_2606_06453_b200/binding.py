@@ -19,6 +19,7 @@ VX_DT_BF16, VX_DT_F32 = 0, 1
 VX_AGG_SUM, VX_AGG_MAX = 0, 1
 VX_SUMMARY_ENVELOPE, VX_SUMMARY_CENTROID = 0, 1
 VX_STEP_UPDATE_SUMMARY = 1
+VX_STEP_APPROX_TOPK = 2
 VX_TRACE_SCORE, VX_TRACE_TOPK, VX_TRACE_DECODE = 1, 2, 4
 
 EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",

@@ -20,6 +20,7 @@
 // gathered from the page table in one parallel pass.
 // Integer work on a few KB per problem -- latency-bound, not bandwidth-bound.
 #include <cstdlib>
+#include <type_traits>
 
 #include "vx_common.cuh"
 #include "vx_internal.h"
@@ -525,24 +526,34 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   // ---- ordered emission: class of a page = sure (forced or key > thr) / tie (key == thr, first need_eq by index) --
   unsigned m_sure[kKpt], m_tie[kKpt];
   int n_sure = 0, n_tie = 0;                    // warp-uniform
+  // (the three rules are separate warp-uniform code paths: with 32 warps per SM every predicated-off instruction of
+  //  an unused rule would still cost an issue slot per warp)
+  auto classify = [&](auto rule) {                // rule 0: exact threshold key; 1: key interval of the bin; 2: float bin
 #pragma unroll
-  for (int u = 0; u < kKpt; ++u) {
-    const bool exists = jbase + u * kWarp + lane < n_pages;
-    bool sure = exists && (key[u] == kForcedKey || key[u] > thr);
-    bool tie = exists && key[u] != kForcedKey && key[u] == thr;
-    if constexpr (kApprox) {
-      if (early) {
-        const bool cand = exists && key[u] != kForcedKey;
-        const int fb = fterm && cand ? fbin(key[u]) : 0;
-        sure = exists && (key[u] == kForcedKey || (fterm ? fb > t_bin : key[u] > m_hi));
-        tie = cand && (fterm ? fb == t_bin : (key[u] >= m_lo && key[u] <= m_hi));
+    for (int u = 0; u < kKpt; ++u) {
+      const bool exists = jbase + u * kWarp + lane < n_pages;
+      const bool forced = key[u] == kForcedKey;
+      bool sure, tie;
+      if constexpr (decltype(rule)::value == 0) {
+        sure = exists && (forced || key[u] > thr);
+        tie = exists && !forced && key[u] == thr;
+      } else if constexpr (decltype(rule)::value == 1) {
+        sure = exists && (forced || key[u] > m_hi);
+        tie = exists && !forced && key[u] >= m_lo && key[u] <= m_hi;
+      } else {
+        const int fb = forced ? kBins : fbin(key[u]);
+        sure = exists && fb > t_bin;
+        tie = exists && fb == t_bin;
       }
+      m_sure[u] = __ballot_sync(0xffffffffu, sure);
+      m_tie[u] = __ballot_sync(0xffffffffu, tie);
+      n_sure += __popc(m_sure[u]);
+      n_tie += __popc(m_tie[u]);
     }
-    m_sure[u] = __ballot_sync(0xffffffffu, sure);
-    m_tie[u] = __ballot_sync(0xffffffffu, tie);
-    n_sure += __popc(m_sure[u]);
-    n_tie += __popc(m_tie[u]);
-  }
+  };
+  if (!kApprox || !early) classify(std::integral_constant<int, 0>());
+  else if (!fterm) classify(std::integral_constant<int, 1>());
+  else classify(std::integral_constant<int, 2>());
   if (lane == 0) s_wcnt[warp] = make_int2(n_sure, n_tie);
   __syncthreads();
   if (tid == 0) VX_TRACE_STAMP(cta, 7);
@@ -555,28 +566,35 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   }
   const unsigned lt_mask = (1u << lane) - 1u;
   const bool staged = n_sel <= kBins;           // the histogram is free now: stage the selected logical ids in it
+  auto emit = [&](auto rotated) {                 // rotated: the taken ties are a cyclic window of tie ranks
 #pragma unroll
-  for (int u = 0; u < kKpt; ++u) {
-    const int j = jbase + u * kWarp + lane;
-    const bool sure = (m_sure[u] >> lane) & 1u, tie = (m_tie[u] >> lane) & 1u;
-    const int my_gt = gt + __popc(m_sure[u] & lt_mask), my_eq = eq + __popc(m_tie[u] & lt_mask);
-    bool take = sure || (tie && my_eq < need_eq);
-    int pos = my_gt + min(my_eq, need_eq);
-    if constexpr (kApprox) {                      // cyclic window of tie ranks (rot = wrap = 0: the same rule)
-      const int span = need_eq - wrap;
-      take = sure || (tie && (my_eq < wrap || (my_eq >= rot && my_eq < rot + span)));
-      pos = my_gt + min(my_eq, wrap) + min(max(my_eq - rot, 0), span);
-    }
-    if (take && pos < n_sel) {
-      if (staged) s_hist[pos] = j;
-      else {
-        sel_phys[out0 + pos] = page_indices[row0 + j];
-        if (sel_logical) sel_logical[out0 + pos] = j;
+    for (int u = 0; u < kKpt; ++u) {
+      const int j = jbase + u * kWarp + lane;
+      const bool sure = (m_sure[u] >> lane) & 1u, tie = (m_tie[u] >> lane) & 1u;
+      const int my_gt = gt + __popc(m_sure[u] & lt_mask), my_eq = eq + __popc(m_tie[u] & lt_mask);
+      bool take;
+      int pos;
+      if constexpr (decltype(rotated)::value) {   // ranks [0, wrap) and [rot, rot + need_eq - wrap)
+        const int span = need_eq - wrap;
+        take = sure || (tie && (my_eq < wrap || (my_eq >= rot && my_eq < rot + span)));
+        pos = my_gt + min(my_eq, wrap) + min(max(my_eq - rot, 0), span);
+      } else {
+        take = sure || (tie && my_eq < need_eq);
+        pos = my_gt + min(my_eq, need_eq);
       }
+      if (take && pos < n_sel) {
+        if (staged) s_hist[pos] = j;
+        else {
+          sel_phys[out0 + pos] = page_indices[row0 + j];
+          if (sel_logical) sel_logical[out0 + pos] = j;
+        }
+      }
+      gt += __popc(m_sure[u]);
+      eq += __popc(m_tie[u]);
     }
-    gt += __popc(m_sure[u]);
-    eq += __popc(m_tie[u]);
-  }
+  };
+  if (kApprox && early) emit(std::true_type());
+  else emit(std::false_type());
   if (staged) {                                   // every selected page: one independent gather + two stores
     __syncthreads();
     if (tid == 0) VX_TRACE_STAMP(cta, 8);

@@ -5,7 +5,11 @@ torch.topk (set equality; ties are measure-zero for these draws).
 The paper reports its radix_topk as "highly sensitive to the score distribution" (:194); the select here bins
 the LIVE key range of each problem, so the four distributions should cost the same.
 
-    python -m paper_2606_06453_b200.topk_microbench [--batch 32] [--heads 8] [--iters 50]
+With --ratios the approximate selection (vx_topk_pages_approx, PAPER.md:196 stochastic early termination) is timed
+beside it at each tolerate_ratio, with its mean / min recall@k against the exact set (PAPER.md:497 reports latency at
+recall@k > 0.97).
+
+    python -m paper_2606_06453_b200.topk_microbench [--batch 32] [--heads 8] [--iters 50] [--ratios 0.05,0.1,0.25]
 """
 from __future__ import annotations
 
@@ -36,6 +40,7 @@ def main():
     ap.add_argument("--batch", type=int, default=32)
     ap.add_argument("--heads", type=int, default=8)
     ap.add_argument("--iters", type=int, default=50)
+    ap.add_argument("--ratios", default="0.05,0.1,0.25", help="tolerate_ratio values for vx_topk_pages_approx ('' = none)")
     args = ap.parse_args()
     dev = "cuda:0"
     gen = torch.Generator(device=dev).manual_seed(77)
@@ -77,7 +82,22 @@ def main():
                 torch.cuda.synchronize()
                 us = a.elapsed_time(b) * 1e3 / args.iters
                 assert torch.equal(sl.long(), want), (P, k, dist, "after graph replay")
-                rows.append(dict(pages=P, k=k, dist=dist, problems=B * H, us=round(us, 2)))
+                row = dict(pages=P, k=k, dist=dist, problems=B * H, us=round(us, 2))
+                for tau in [float(x) for x in args.ratios.split(",") if x] if P <= 8192 else []:
+                    ctx.topk_pages_approx(scores, pt, budget, k, tau, 7, sp, sl, sc)
+                    torch.cuda.synchronize()
+                    hit = (sl.long().unsqueeze(-1) == want.unsqueeze(-2)).any(-1).float().sum(-1) / k   # [B, H] recall@k
+                    g2 = torch.cuda.CUDAGraph()
+                    with torch.cuda.graph(g2):
+                        for _ in range(args.iters):
+                            ctx.topk_pages_approx(scores, pt, budget, k, tau, 7, sp, sl, sc)
+                    g2.replay()
+                    torch.cuda.synchronize()
+                    a.record(); g2.replay(); b.record()
+                    torch.cuda.synchronize()
+                    row[f"approx_{tau}"] = dict(us=round(a.elapsed_time(b) * 1e3 / args.iters, 2),
+                                                recall_mean=round(hit.mean().item(), 4), recall_min=round(hit.min().item(), 4))
+                rows.append(row)
                 print(json.dumps(rows[-1]))
             ctx.close()
     by = {}
