@@ -645,6 +645,11 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
   static int force = -1;
   if (force < 0) { const char* e = getenv("VX_TOPK_THREADS"); force = e ? atoi(e) : 0; }
   const int n = pt.max_pages_per_req;
+  static int pair = -1;
+  if (pair < 0) { const char* e = getenv("VX_TOPK_PAIR"); pair = e ? atoi(e) : 1; }
+  if (pair && !force && ap.tolerate_ratio <= 0.f &&
+      topk_pair_applies(c, c->g.num_kv_heads * (rr.count < 0 ? pt.batch : rr.count), n))
+    return launch_topk_pair(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
   if ((!force || ap.tolerate_ratio > 0.f) && n <= kTopkRegMaxPages) {                  // keys fit the registers of one CTA, 8 per thread (16 measured slower)
 #define VX_REG(T, K) return launch_topk_reg<T, K>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap)
     if (n <= 1024) VX_REG(128, 8);

@@ -70,3 +70,42 @@ def test_topk_fuzz_is_bit_exact(kind, seed):
     assert np.array_equal(sc.cpu().numpy(), sc_r)
     assert np.array_equal(sl.cpu().numpy(), sl_r), kind
     assert np.array_equal(sp.cpu().numpy(), sp_r), kind
+
+
+@pytest.mark.parametrize("kind", KINDS)
+@pytest.mark.parametrize("big", [2049, 4096, 4097, 8192])
+def test_topk_pair_kernel_fuzz_is_bit_exact(kind, big):
+    """Few problems of 2,049..8,192 pages run on clusters of two CTAs (vx_topk_pair.cu): same bit-exact contract."""
+    import paper_2606_06453_b200 as vx
+    rng = np.random.default_rng(7000 + 10 * KINDS.index(kind) + big)
+    b = 16
+    n_sink, n_local = int(rng.integers(0, 3)), int(rng.integers(0, 4))
+    pages = [big] + [int(x) for x in rng.choice([1, 3, 40, 300, 1025, 2048, 2100, big - 1, big], size=4)]
+    hkv = 2
+    seq = [p * b - int(rng.integers(0, b)) for p in pages]
+    indptr = np.concatenate([[0], np.cumsum(pages)]).astype(np.int32)
+    T = int(indptr[-1])
+    indices = rng.permutation(T + 17)[:T].astype(np.int32)
+    budget = np.array([max(n_sink + n_local, int(rng.integers(1, max(2, min(p + 3, 3000))))) for p in pages], np.int32)
+    mb = int(budget.max())
+    scores = np.stack([draw_scores(rng, kind, T) for _ in range(hkv)])
+    pt_o = vo.PageTable(indptr, indices, np.array(seq, np.int32), b)
+    sl_r, sp_r, sc_r, _ = vo.topk_pages(scores.astype(np.float64), pt_o, budget, n_sink, n_local, mb)
+    dev = "cuda:0"
+    ctx = vx.Context(dtype=torch.bfloat16, num_q_heads=8, num_kv_heads=hkv, qk_dim=128, v_dim=128, page_size=b,
+                     sm_scale=1.0, n_sink=n_sink, n_local=n_local, max_batch=len(pages), max_total_pages=T,
+                     max_pages_per_req=max(pages), max_budget=mb, device=dev)
+    pt = vx.PageTable(torch.from_numpy(indptr).to(dev), torch.from_numpy(indices).to(dev),
+                      torch.tensor(seq, dtype=torch.int32, device=dev), T, max(pages))
+    for with_logical in (True, False):
+        sl = torch.full((len(pages), hkv, mb), -7, dtype=torch.int32, device=dev)
+        sp = torch.full_like(sl, -7)
+        sc = torch.full((len(pages), hkv), -7, dtype=torch.int32, device=dev)
+        ctx.topk_pages(torch.from_numpy(scores).to(dev), pt, torch.from_numpy(budget).to(dev), mb, sp,
+                       sl if with_logical else None, sc)
+        torch.cuda.synchronize()
+        assert np.array_equal(sc.cpu().numpy(), sc_r)
+        assert np.array_equal(sp.cpu().numpy(), sp_r), kind
+        if with_logical:
+            assert np.array_equal(sl.cpu().numpy(), sl_r), kind
+    ctx.close()
