@@ -187,6 +187,19 @@ vx_status vx_topk_pages_approx(vx_ctx *ctx, const float *scores, const vx_page_t
  * (context state, host side; default 0 = exact).  VX_ERR_INVALID_ARG outside [0, 1]. */
 vx_status vx_set_topk_approx(vx_ctx *ctx, float tolerate_ratio, uint64_t seed);
 
+/* ---- NEXT-4: head-union block table, PAPER.md:538 (Table 1 "TopK, Union: block-table selection and its
+ * deduplicated union (trtllm backend)"), :200 (a paged decode backend that takes one table per request) ------
+ * union[i] = the set union over the KV heads of sel_logical[i, kvh, 0:sel_count[i, kvh]], duplicates removed,
+ * in ASCENDING logical order; union_phys holds the physical ids through the page table.
+ * sel_logical / sel_count: dev, as written by vx_topk_pages (entries outside [0, P_i) are ignored).
+ * union_phys / union_logical: dev [B, max_union], padded with -1; union_logical may be NULL.
+ * union_count: dev [B].  max_union (host) must be >= min(Hkv * max_budget, pt->max_pages_per_req), the largest
+ * union possible, else VX_ERR_INVALID_ARG.  VX_ERR_UNSUPPORTED above 393,184 pages per request. */
+vx_status vx_union_pages(vx_ctx *ctx, const vx_page_table *pt, const int32_t *sel_logical,
+                         const int32_t *sel_count, int32_t max_budget, int32_t max_union,
+                         int32_t *union_phys, int32_t *union_logical, int32_t *union_count,
+                         vx_stream stream);
+
 /* ---- (a4)+(a5) attention over the selected pages: PAPER.md:92 Eq.4, :200, :75 -------- */
 /* out[i,h,:] = softmax_t(sm_scale * q[i,h].K_t) V_t over the valid tokens of the pages listed
  * in sel_logical/sel_phys[i, h/g, 0:sel_count]; lse[i,h] = natural log of the softmax

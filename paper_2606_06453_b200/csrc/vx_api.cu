@@ -268,6 +268,25 @@ vx_status vx_set_topk_approx(vx_ctx* c, float tolerate_ratio, uint64_t seed) {
   return VX_OK;
 }
 
+vx_status vx_union_pages(vx_ctx* c, const vx_page_table* pt, const int32_t* sel_logical, const int32_t* sel_count,
+                         int32_t max_budget, int32_t max_union, int32_t* union_phys, int32_t* union_logical,
+                         int32_t* union_count, vx_stream stream) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  c->launches = 0;
+  if (vx_status st = check_table(c, pt)) return st;
+  if (!sel_logical || !sel_count || !union_phys || !union_count)
+    return fail(c, VX_ERR_INVALID_ARG, "sel_logical / sel_count / union_phys / union_count is NULL");
+  if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
+  const int64_t largest = (int64_t)c->g.num_kv_heads * max_budget;
+  const int64_t bound = largest < pt->max_pages_per_req ? largest : pt->max_pages_per_req;
+  if (max_union < bound)
+    return fail(c, VX_ERR_INVALID_ARG, "max_union %d below the largest possible union %lld", max_union, (long long)bound);
+  cudaError_t e = launch_union_pages(c, *pt, sel_logical, sel_count, max_budget, max_union, union_phys, union_logical,
+                                     union_count, (cudaStream_t)stream);
+  if (e == cudaErrorNotSupported) return fail(c, VX_ERR_UNSUPPORTED, "more than 393,184 pages per request");
+  return check_cuda(c, e, "vx_union_pages");
+}
+
 static vx_status decode_dispatch(vx_ctx* c, const void* q, const vx_kv_pool* pool, const vx_page_table* pt,
                                  const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                                  int32_t max_budget, void* out, float* lse, cudaStream_t s,

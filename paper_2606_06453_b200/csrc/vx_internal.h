@@ -155,6 +155,14 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
                               int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl = false,
                               const ReqRange& rr = ReqRange(), const PrefetchPlan& pf = PrefetchPlan(),
                               const ApproxPlan& ap = ApproxPlan());
+// the same selection with each problem on a cluster of two CTAs (vx_topk_pair.cu); VX_TOPK_PAIR=0 turns it off
+bool topk_pair_applies(const vx_ctx* c, int n_problems, int max_pages_per_req);
+cudaError_t launch_topk_pair(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
+                             int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
+                             cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf);
+cudaError_t launch_union_pages(vx_ctx* c, const vx_page_table& pt, const int32_t* sel_logical, const int32_t* sel_count,
+                               int32_t max_budget, int32_t max_union, int32_t* union_phys, int32_t* union_logical,
+                               int32_t* union_count, cudaStream_t s);
 cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical,
                               const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
