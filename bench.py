@@ -44,6 +44,8 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--summary", default="envelope", choices=["envelope", "centroid"],
                     help="page summary / score flow: Quest envelope (default, the north star) or block top-k centroid")
+    ap.add_argument("--agg", default="sum", choices=["sum", "max"],
+                    help="head-group aggregation of the envelope score: sum (default, the north star) or max_h (PAPER.md:556)")
     ap.add_argument("--topk-approx", type=float, default=0.0, metavar="RATIO",
                     help="select with vx_topk_pages_approx at this tolerate_ratio (PAPER.md:196; lossy, recall@k >= "
                          "1 - RATIO).  Default 0: the exact selection, the north star's path")
@@ -132,7 +134,7 @@ class ClockSampler(threading.Thread):
 class Runner:
     """One workload resident on one GPU: context, pools, summaries, outputs, L2 flush buffer."""
 
-    def __init__(self, cfg, device, seed_offset=0, summary="envelope", topk_approx=0.0):
+    def __init__(self, cfg, device, seed_offset=0, summary="envelope", topk_approx=0.0, agg="sum"):
         import torch
         import paper_2606_06453_b200 as vx
         from paper_2606_06453_b200.workloads import make_workload
@@ -140,7 +142,7 @@ class Runner:
         self.w = w = make_workload(cfg, device=device, seed_offset=seed_offset)
         kind = vx.binding.VX_SUMMARY_CENTROID if summary == "centroid" else vx.binding.VX_SUMMARY_ENVELOPE
         self.summary_name = summary
-        self.ctx = vx.context_for(w, summary_kind=kind)
+        self.ctx = vx.context_for(w, summary_kind=kind, agg=vx.binding.VX_AGG_MAX if agg == "max" else vx.binding.VX_AGG_SUM)
         self.tau = float(topk_approx)
         self.step_flags = vx.VX_STEP_UPDATE_SUMMARY | (vx.VX_STEP_APPROX_TOPK if self.tau > 0 else 0)
         self.ctx.set_topk_approx(self.tau, 20260604)
@@ -226,7 +228,7 @@ class Runner:
         return out
 
 
-def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None, summary="envelope"):
+def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None, summary="envelope", agg="sum"):
     """Time the oracle (as it stands) on the first n_requests requests of the workload.
     Returns (seconds for score + top-k + attention on the sample, requests in sample, batch, threads)."""
     from oracle import vx_oracle as vo
@@ -241,7 +243,8 @@ def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=No
     summ = build(pool, pt, s.num_kv_heads, s.qk_dim)                    # built outside the timed step
     t0 = time.perf_counter()
     vo.decode_step(q, pool, pt, vo.as_np(sub.budget), sub.max_budget, s.num_q_heads, s.num_kv_heads, s.qk_dim,
-                   s.v_dim, s.sm_scale, s.n_sink, s.n_local, summary=summ, kind=summary)
+                   s.v_dim, s.sm_scale, s.n_sink, s.n_local, agg=vo.AGG_MAX if agg == "max" else vo.AGG_SUM, summary=summ,
+                   kind=summary)
     return time.perf_counter() - t0, n_requests, w.spec.batch, vo.num_threads()
 
 
@@ -259,7 +262,7 @@ def run_reference(args):
     times = []
     steps = max(1, min(args.steps, 3))
     for it in range(min(args.warmup, 1) + steps):
-        t, n, batch, threads = oracle_sample_time(args.config, nreq, workload=w, summary=args.summary)
+        t, n, batch, threads = oracle_sample_time(args.config, nreq, workload=w, summary=args.summary, agg=args.agg)
         if it >= min(args.warmup, 1):
             times.append(t)
     us = statistics.mean(times) / n * batch * 1e6        # scaled from the sample to the whole batch
@@ -301,7 +304,7 @@ def main():
         dist.barrier()
 
     peak, peak_src = measured_peak()
-    r = Runner(args.config, device, seed_offset=rank, summary=args.summary, topk_approx=args.topk_approx)
+    r = Runner(args.config, device, seed_offset=rank, summary=args.summary, topk_approx=args.topk_approx, agg=args.agg)
     w, s = r.w, r.w.spec
     bytes_ = algorithmic_bytes(w, summary=args.summary)
 
@@ -353,7 +356,7 @@ def main():
         step_gbs = bytes_["total"] / (ms * 1e-3) / 1e9
         cpu = None
         if not args.no_cpu_baseline:
-            t, n, batch, threads = oracle_sample_time(args.config, SAMPLE_REQUESTS.get(args.config, 1), workload=w, summary=args.summary)
+            t, n, batch, threads = oracle_sample_time(args.config, SAMPLE_REQUESTS.get(args.config, 1), workload=w, summary=args.summary, agg=args.agg)
             cpu = {"value": t / n * batch * 1e6, "unit": "us", "cores": threads, "kind": "oracle",
                    "sample": f"first {n} of {batch} requests, one pass (score + top-k + attention), scaled by {batch}/{n}"}
         also = {}
@@ -370,7 +373,7 @@ def main():
                 "vs_baseline": None, "dtype": s.dtype, "data": "synthetic",
                 "config": {"workload": args.config, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
                            "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
-                           "seq_len": list(s.seq_len), "budget_pages": w.max_budget, "summary": args.summary,
+                           "seq_len": list(s.seq_len), "budget_pages": w.max_budget, "summary": args.summary, "agg": args.agg,
                            "topk": "exact" if args.topk_approx <= 0 else f"approx tolerate_ratio={args.topk_approx} (lossy)",
                            "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"},
                 "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,

@@ -67,7 +67,7 @@ static const char* check_geom(const vx_geom* g, vx_status* st) {
   if (g->agg != VX_AGG_SUM && g->agg != VX_AGG_MAX) return "agg must be VX_AGG_SUM or VX_AGG_MAX";
   if (g->summary_kind != VX_SUMMARY_ENVELOPE && g->summary_kind != VX_SUMMARY_CENTROID)
     return "summary_kind must be VX_SUMMARY_ENVELOPE or VX_SUMMARY_CENTROID";
-  if (!score_geometry_supported(*g)) return "qk_dim / dtype / aggregation not supported by the score kernel (VX_AGG_MAX: GQA groups of <= 8 heads)";
+  if (!score_geometry_supported(*g)) return "qk_dim / dtype / aggregation not supported by the score kernel (VX_AGG_MAX: GQA groups of <= 8 heads, or the bf16 MLA group of 16 / 32 heads)";
   if (g->kv_shared ? !mla_geometry_supported(*g) : !gqa_geometry_supported(*g))
     return "(dtype, qk_dim, v_dim, heads) not supported by the decode kernels";
   *st = VX_OK;

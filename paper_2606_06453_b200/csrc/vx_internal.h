@@ -160,6 +160,10 @@ bool topk_pair_applies(const vx_ctx* c, int n_problems, int max_pages_per_req);
 cudaError_t launch_topk_pair(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
                              int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
                              cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf);
+// VX_AGG_MAX over the MLA head group on the tensor cores (vx_score_mla_max.cu)
+bool score_mla_max_supported(const vx_geom& g);
+cudaError_t launch_score_mla_max(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt, float* scores,
+                                 cudaStream_t s, const ReqRange& rr);
 cudaError_t launch_union_pages(vx_ctx* c, const vx_page_table& pt, const int32_t* sel_logical, const int32_t* sel_count,
                                int32_t max_budget, int32_t max_union, int32_t* union_phys, int32_t* union_logical,
                                int32_t* union_count, cudaStream_t s);

@@ -409,8 +409,9 @@ VX_TRACE_SETTER(vx_trace_set_score)
 bool score_geometry_supported(const vx_geom& g) {
   if (g.agg != VX_AGG_SUM && g.agg != VX_AGG_MAX) return false;
   const int hkv = g.num_kv_heads;
-  // MAX costs g flop per byte: CUDA cores carry it for GQA groups (g <= 8); the MLA group (g = 32) would need
-  // the tensor cores for the scoring too -- not built (NEXT-1)
+  // MAX costs g flop per byte: CUDA cores carry it for GQA groups (g <= 8); the MLA group (16 or 32 heads on one
+  // latent head) is a contraction on the tensor cores (vx_score_mla_max.cu)
+  if (score_mla_max_supported(g)) return true;
   if (g.agg == VX_AGG_MAX && (g.kv_shared || g.num_q_heads / hkv > 8)) return false;
   if (g.summary_kind != VX_SUMMARY_ENVELOPE && g.summary_kind != VX_SUMMARY_CENTROID) return false;
   if (g.summary_kind == VX_SUMMARY_CENTROID && g.agg != VX_AGG_SUM) return false;       // Eq.2 is a mean over the group
@@ -491,6 +492,7 @@ cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, con
                               float* scores, cudaStream_t s, const ReqRange& rr) {
   if (pt.batch == 0 || pt.total_pages == 0) return cudaSuccess;
   const vx_geom& g = c->g;
+  if (score_mla_max_supported(g)) return launch_score_mla_max(c, q, summary, pt, scores, s, rr);
   if (g.dtype == VX_DT_BF16) {
     switch (g.qk_dim) {
       case 64: return launch_score_d<__nv_bfloat16, 64>(c, q, summary, pt, scores, s, rr);

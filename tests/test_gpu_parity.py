@@ -188,7 +188,7 @@ def test_fused_step_matches_oracle(name, flags):
         assert rec >= 0.99
 
 
-@pytest.mark.parametrize("name", ["C1", "C2-small", "C3-small", "C5-small"])
+@pytest.mark.parametrize("name", ["C1", "C2-small", "C3-small", "C5-small", "C4-small"])
 def test_max_aggregation_scores_and_step_match_oracle(name):
     """VX_AGG_MAX (the max_h envelope variant): scores and the fused step against the oracle."""
     import paper_2606_06453_b200 as vxm
