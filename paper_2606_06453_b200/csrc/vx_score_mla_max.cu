@@ -11,13 +11,14 @@
 // HBM rate -- a memory-bound use of them, which is why the warp-level instruction (no TMEM / TMA staging) is enough.
 //
 // One CTA serves one request: it splits the request's queries by sign into A in shared memory (rows padded to
-// 2,368 B so that a quarter-warp's 16-byte fragment loads cover all 32 banks once), then each warp takes 32-page
-// chunks: per 32-wide k block a thread loads one 16-byte piece of each of its 4 page rows straight from global
+// 2,368 B so that a quarter-warp's 16-byte fragment loads cover all 32 banks once), then each warp takes 16-page
+// chunks: per 32-wide k block a thread loads one 16-byte piece of each of its 2 page rows straight from global
 // memory (8 rows x 64 contiguous bytes per warp instruction) and the A fragments for both 16-head tiles from shared
 // memory.  The k order inside a block is permuted -- thread t owns elements 8t..8t+7 and feeds 8t..8t+3 to one
 // mma and 8t+4..8t+7 to the next -- identically for A and B, which a dot product does not notice; it turns every
 // fragment load into one 128-bit access.  The head maximum is taken over the accumulator rows in registers and by
-// three shuffles; scores leave as fp32.
+// three shuffles; scores leave as fp32.  The page rows go global -> registers through a 6-deep register pipeline
+// (loads of k blocks kb+1 .. kb+5 in flight under block kb's mma).
 #include <cuda_bf16.h>
 
 #include "vx_common.cuh"
@@ -32,25 +33,26 @@ constexpr int kKBlocks = kK / 32;               // 36 blocks of 32
 constexpr int kARowBytes = kK * 2 + 64;         // 2,368: consecutive rows start 64 B apart modulo 128
 constexpr int kThreads = 256;
 constexpr int kWarps = kThreads / kWarp;
-constexpr int kNT = 4;                          // n tiles of 8 pages per warp item
+constexpr int kNT = 2;                          // n tiles of 8 pages per warp item
+constexpr int kDepth = 6;                       // k blocks in the register pipeline (bytes in flight set the rate)
 constexpr int kChunk = 8 * kNT;                 // pages per warp item
 
 __device__ __forceinline__ uint4 ldg_stream_v4(const void* p) {
   uint4 v;
-  asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
+  asm("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
                : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
   return v;
 }
 __device__ __forceinline__ void mma_bf16_16816(float (&c)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
                                                uint32_t b0, uint32_t b1) {
-  asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
+  asm("mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, "
                "{%0, %1, %2, %3};"
                : "+f"(c[0]), "+f"(c[1]), "+f"(c[2]), "+f"(c[3]) : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 }  // namespace
 
 template <int MT>                               // 16-head tiles: Hq = 16 * MT
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 2)
 score_mla_max_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ summary,
                      const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
                      float* __restrict__ scores, int req0) {
@@ -61,17 +63,30 @@ score_mla_max_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* _
   const int g = lane >> 2, t = lane & 3;
   pdl_trigger();                                // the selection kernel may queue up behind us
   const int row0 = page_indptr[i], n_pages = page_indptr[i + 1] - row0;
+  if (blockIdx.x * kWarps * kChunk >= n_pages) return;          // a short request needs fewer CTAs than the grid has
 
   // ---- A = [q- | q+] of this request's heads -------------------------------------------------------------------
   const __nv_bfloat16* qi = q + (int64_t)i * HQ * kD;
-  const __nv_bfloat16 zero = __float2bfloat16(0.f);
-  for (int e = tid; e < HQ * kD; e += kThreads) {
-    const int h = e / kD, c = e - h * kD;
-    const __nv_bfloat16 x = qi[e];
-    const bool neg = __bfloat162float(x) < 0.f;
-    __nv_bfloat16* row = reinterpret_cast<__nv_bfloat16*>(s_a + (size_t)h * kARowBytes);
-    row[c] = neg ? x : zero;                    // pairs with m (summary row [0, 576))
-    row[kD + c] = neg ? zero : x;               // pairs with M (summary row [576, 1152))
+  // (8 elements per thread and step, all loads of a thread independent: the 36 KB of queries come from L2 once)
+  constexpr int kVecs = HQ * kD / 8;
+#pragma unroll
+  for (int v0 = 0; v0 < kVecs; v0 += kThreads) {
+    const int v = v0 + tid;
+    if (v < kVecs) {
+      const int h = v / (kD / 8), c = (v - h * (kD / 8)) * 8;
+      const uint4 x = *reinterpret_cast<const uint4*>(qi + (size_t)v * 8);
+      const uint32_t w[4] = {x.x, x.y, x.z, x.w};
+      uint32_t neg[4], pos[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {             // bf16 pairs: the sign bit decides (-0.0 goes to q-, which adds 0 either way)
+        const uint32_t m = ((w[e] & 0x00008000u) ? 0x0000FFFFu : 0u) | ((w[e] & 0x80000000u) ? 0xFFFF0000u : 0u);
+        neg[e] = w[e] & m;
+        pos[e] = w[e] & ~m;
+      }
+      uint8_t* row = s_a + (size_t)h * kARowBytes;
+      *reinterpret_cast<uint4*>(row + c * 2) = make_uint4(neg[0], neg[1], neg[2], neg[3]);              // pairs with m
+      *reinterpret_cast<uint4*>(row + (kD + c) * 2) = make_uint4(pos[0], pos[1], pos[2], pos[3]);       // pairs with M
+    }
   }
   __syncthreads();
 
@@ -92,20 +107,34 @@ score_mla_max_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* _
 #pragma unroll
         for (int e = 0; e < 4; ++e) acc[mt][nt][e] = 0.f;
     const uint8_t* arow = s_a + (size_t)g * kARowBytes + t * 16;
-#pragma unroll 2
-    for (int kb = 0; kb < kKBlocks; ++kb) {
-      uint4 b[kNT];
+    // register pipeline, kDepth k blocks deep: the loads of blocks kb + 1 .. kb + kDepth - 1 are in flight under block kb's mma
+    uint4 b[kDepth][kNT];
+    auto load_b = [&](uint4 (&dst)[kNT], int kb) {
+      const int off = min(kb, kKBlocks - 1) * 64;               // (past the end: a harmless repeat of the last block)
 #pragma unroll
-      for (int nt = 0; nt < kNT; ++nt) b[nt] = ldg_stream_v4(brow[nt] + kb * 64);
+      for (int nt = 0; nt < kNT; ++nt) dst[nt] = ldg_stream_v4(brow[nt] + off);
+    };
+    auto compute = [&](const uint4 (&bb)[kNT], int kb) {
 #pragma unroll
       for (int mt = 0; mt < MT; ++mt) {
         const uint4 lo = *reinterpret_cast<const uint4*>(arow + (size_t)(mt * 16) * kARowBytes + kb * 64);      // head 16 mt + g
         const uint4 hi = *reinterpret_cast<const uint4*>(arow + (size_t)(mt * 16 + 8) * kARowBytes + kb * 64);  // head 16 mt + g + 8
 #pragma unroll
         for (int nt = 0; nt < kNT; ++nt) {
-          mma_bf16_16816(acc[mt][nt], lo.x, hi.x, lo.y, hi.y, b[nt].x, b[nt].y);
-          mma_bf16_16816(acc[mt][nt], lo.z, hi.z, lo.w, hi.w, b[nt].z, b[nt].w);
+          mma_bf16_16816(acc[mt][nt], lo.x, hi.x, lo.y, hi.y, bb[nt].x, bb[nt].y);
+          mma_bf16_16816(acc[mt][nt], lo.z, hi.z, lo.w, hi.w, bb[nt].z, bb[nt].w);
         }
+      }
+    };
+    static_assert(kKBlocks % kDepth == 0, "pipeline depth");
+#pragma unroll
+    for (int st = 0; st < kDepth - 1; ++st) load_b(b[st], st);
+#pragma unroll 1
+    for (int kb = 0; kb < kKBlocks; kb += kDepth) {
+#pragma unroll
+      for (int st = 0; st < kDepth; ++st) {
+        load_b(b[(st + kDepth - 1) % kDepth], kb + st + kDepth - 1);
+        compute(b[st], kb + st);
       }
     }
     // ---- max over the heads: accumulator rows g, g + 8 of every tile, then the 8 lanes that share t -----------
@@ -147,7 +176,9 @@ static cudaError_t launch_mt(vx_ctx* c, const void* q, const void* summary, cons
     attr_set = true;
   }
   const int n_req = rr.count < 0 ? pt.batch : rr.count;
-  // CTAs per request: enough warps for the longest request's chunks, at most ~2 resident CTAs per SM over the batch
+  // CTAs per request: enough warps for the longest request's chunks, capped at ~2 resident CTAs per SM over the batch
+  // (one chunk per warp whatever the batch -- 512 CTAs on C4 -- measured 35.0 us against 32.5: every CTA rebuilds A);
+  // CTAs beyond a shorter request's chunks leave at once
   const int chunks = (pt.max_pages_per_req + kChunk - 1) / kChunk;
   int per_req = (chunks + kWarps - 1) / kWarps;
   const int cap = (2 * c->num_sms + n_req - 1) / n_req;
