@@ -58,7 +58,9 @@ def test_workspace_bytes_and_geometry_validation(vx):
     assert ws(geom(vx, dtype=0, num_q_heads=32, num_kv_heads=1, qk_dim=576, v_dim=512, page_size=64,
                    kv_shared=1), 64, 50000, 1024, 32) > 0              # MLA geometry
     assert ws(geom(vx, dtype=0, num_q_heads=32, num_kv_heads=1, qk_dim=576, v_dim=512, page_size=64,
-                   kv_shared=1, agg=1), 64, 50000, 1024, 32) == 0      # max_h over the 32-head MLA group: not built
+                   kv_shared=1, agg=1), 64, 50000, 1024, 32) > 0       # max_h over the 32-head MLA group: tensor-core scoring
+    assert ws(geom(vx, dtype=0, num_q_heads=8, num_kv_heads=1, qk_dim=576, v_dim=512, page_size=64,
+                   kv_shared=1, agg=1), 64, 50000, 1024, 32) == 0      # ... which takes 16 or 32 heads only
     assert ws(geom(vx, dtype=1, num_q_heads=4, num_kv_heads=1, qk_dim=64, v_dim=64), 1, 64, 64, 8) > 0
 
 
