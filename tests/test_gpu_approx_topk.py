@@ -114,3 +114,40 @@ def test_argument_checks():
     ctx.topk_pages_approx(scores, pt, budget, 64, 0.0, 1, sp, sl, sc)     # ratio 0: the exact kernel, any size
     torch.cuda.synchronize()
     ctx.close()
+
+
+@pytest.mark.parametrize("name", ["C2-small", "C4-small", "C5-small"])
+def test_fused_step_with_approximate_selection(name):
+    """VX_STEP_APPROX_TOPK: the fused step selects with the approximate kernel (vx_set_topk_approx's ratio and seed):
+    its selection equals the approximate oracle's on the GPU's own fp32 scores bit for bit, and its attention output
+    matches the fp64 oracle evaluated on that selection within the bf16 tolerances."""
+    import paper_2606_06453_b200 as vx
+    from paper_2606_06453_b200.workloads import make_workload
+    from tests.parity import check_attention, oracle_attention_on
+    w = make_workload(name, device="cuda:0")
+    s = w.spec
+    dev = "cuda:0"
+    ctx = vx.context_for(w)
+    pool, pt = vx.tables_for(w)
+    summary = vx.alloc_summary(w)
+    ctx.page_summary_update(pool, pt, summary, first_new_pos=torch.zeros_like(w.seq_lens))
+    scores = torch.empty(s.num_kv_heads, w.total_pages, dtype=torch.float32, device=dev)
+    ctx.page_score(w.q, summary, pt, scores)
+    tau, seed = 0.25, 123
+    ctx.set_topk_approx(tau, seed)
+    out = torch.full((s.batch, s.num_q_heads, s.v_dim), float("nan"), dtype=w.q.dtype, device=dev)
+    lse = torch.full((s.batch, s.num_q_heads), float("nan"), dtype=torch.float32, device=dev)
+    sl = torch.full((s.batch, s.num_kv_heads, w.max_budget), -7, dtype=torch.int32, device=dev)
+    sp, sc = torch.full_like(sl, -7), torch.full((s.batch, s.num_kv_heads), -7, dtype=torch.int32, device=dev)
+    ctx.sparse_decode_step(w.q, pool, summary, pt, w.budget, w.max_budget, out, lse, sp, sl, sc,
+                           flags=vx.VX_STEP_UPDATE_SUMMARY | vx.VX_STEP_APPROX_TOPK)
+    torch.cuda.synchronize()
+    sl_r, sp_r, sc_r, early = va.approx_topk_pages(scores.cpu().numpy(), w.page_indptr.cpu().numpy(),
+                                                   w.page_indices.cpu().numpy(), w.seq_lens.cpu().numpy(), s.page_size,
+                                                   w.budget.cpu().numpy(), s.n_sink, s.n_local, w.max_budget, tau, seed)
+    assert early.any()                                                  # the lossy path was actually taken
+    assert np.array_equal(sc.cpu().numpy(), sc_r)
+    assert np.array_equal(sl.cpu().numpy(), sl_r) and np.array_equal(sp.cpu().numpy(), sp_r)
+    o_ref, l_ref = oracle_attention_on(w, sl.cpu().numpy(), sc.cpu().numpy())
+    check_attention(s.dtype, out.float().cpu().numpy(), lse.cpu().numpy(), o_ref, l_ref)
+    ctx.close()
