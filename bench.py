@@ -64,7 +64,8 @@ def measured_peak():
 
 def ncu_traffic(cfg, stage):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
-    `ncu --set full` capture (profiles/r1e_traffic.csv; commands in profiles/r1e_final.md), or None."""
+    `ncu --set full` capture (profiles/r1e_traffic.csv; commands in profiles/r1e_final.md; those kernels are unchanged in
+    snapshot r1f, profiles/r1f_final.md), or None."""
     kernel = {"page_score": ("score_kernel",), "sparse_paged_decode": ("decode_gqa_mma_kernel", "decode_mla_kernel")}[stage]
     path = os.path.join(ROOT, "profiles", "r1e_traffic.csv")
     if not os.path.exists(path):
