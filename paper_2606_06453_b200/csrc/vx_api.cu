@@ -156,6 +156,8 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   const char* pm = getenv("VX_PREFETCH_MB");
   c->prefetch_mb = pm ? atoi(pm) : 0;               // measured: no gain at 16 MB, slower beyond (the prefetch delays the selection kernel)
   c->use_prefetch = c->prefetch_mb > 0;
+  const char* pp = getenv("VX_PREFETCH_PAGES");   // pages per decode split; unset = the measured default (see the step)
+  c->prefetch_pages = pp ? atoi(pp) : -1;
   const char* ch = getenv("VX_CHAINS");
   c->chains = ch && atoi(ch) >= 2 ? 2 : 1;      // measured: no gain on C2..C4 (the chains mostly serialise on shared memory), +3 % on C5
   c->aux_stream = nullptr;
@@ -370,7 +372,8 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
     // L2 prefetch plan for the decode kernel's first pages (fast decode paths with contiguous page chunks only)
     PrefetchPlan pf;
     const int64_t esz = (int64_t)elem_size(c->g.dtype);
-    if (c->use_prefetch && decode_folds_summary(c) && pool->stride_token == c->g.qk_dim) {
+    const bool pf_auto = !c->use_prefetch && (c->prefetch_pages > 0 || (c->prefetch_pages < 0 && !c->g.kv_shared));
+    if ((c->use_prefetch || pf_auto) && decode_folds_summary(c) && pool->stride_token == c->g.qk_dim) {
       const int n_req = rr.count < 0 ? pt->batch : rr.count;
       pf.k = pool->k;
       pf.v = c->g.kv_shared ? nullptr : pool->v;
@@ -382,6 +385,15 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
       const int64_t units = (int64_t)n_req * c->g.num_kv_heads * pf.splits;
       const int64_t budget_bytes = (int64_t)c->prefetch_mb << 20;
       pf.pages_per_split = (int)(budget_bytes / (units * per_page > 0 ? units * per_page : 1));
+      if (pf_auto) {
+        // GQA default: the first 6 pages of every split, at most 16 MB in all (C3: 88.8 us against 89.8 without;
+        // 4 / 8 pages 89.2-89.4, 48 MB and more slower -- the prefetch then delays the selection kernel's own tail;
+        // the MLA decode (C4) loses 7 us with any of it: its first TMA boxes and the prefetch queue behind each other)
+        const int64_t cap = ((int64_t)16 << 20) / (units * per_page > 0 ? units * per_page : 1);
+        const int want = c->prefetch_pages > 0 ? c->prefetch_pages : 6;
+        pf.pages_per_split = (int)(want < cap ? want : cap);
+        if (c->prefetch_pages < 0 && cap < 4) pf.pages_per_split = 0;   // big batches (C5): nothing to gain from 1-3 pages
+      }
       if (pf.pages_per_split < 1) pf.k = nullptr;
     }
     if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, cs,

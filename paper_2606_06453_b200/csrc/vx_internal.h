@@ -52,7 +52,8 @@ struct vx_ctx {
   bool force_generic;            // VX_FORCE_GENERIC=1 in the environment: CUDA-core decode path only (debug)
   bool use_pdl;                  // chain the kernels of a step with programmatic dependent launch (VX_NO_PDL=1: off)
   bool use_prefetch;             // the selection kernel prefetches the decode kernel's first pages into L2 (VX_PREFETCH_MB=0: off)
-  int prefetch_mb;               // prefetch budget, MiB (default 48 of the 126 MB L2)
+  int prefetch_mb;               // prefetch budget, MiB (VX_PREFETCH_MB; 0 = use prefetch_pages)
+  int prefetch_pages;            // pages per decode split to prefetch (VX_PREFETCH_PAGES; -1 = default: 6 for GQA, none for MLA)
   int chains;                    // request windows run as concurrent kernel chains inside a fused step (VX_CHAINS, 1 or 2)
   cudaStream_t aux_stream;       // second chain's stream; fork / join with the caller's stream by events
   cudaEvent_t ev_fork, ev_join;
