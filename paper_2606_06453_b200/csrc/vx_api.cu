@@ -372,7 +372,7 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
     // L2 prefetch plan for the decode kernel's first pages (fast decode paths with contiguous page chunks only)
     PrefetchPlan pf;
     const int64_t esz = (int64_t)elem_size(c->g.dtype);
-    const bool pf_auto = !c->use_prefetch && (c->prefetch_pages > 0 || (c->prefetch_pages < 0 && !c->g.kv_shared));
+    const bool pf_auto = !c->use_prefetch && c->prefetch_pages != 0;
     if ((c->use_prefetch || pf_auto) && decode_folds_summary(c) && pool->stride_token == c->g.qk_dim) {
       const int n_req = rr.count < 0 ? pt->batch : rr.count;
       pf.k = pool->k;
@@ -388,11 +388,12 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
       if (pf_auto) {
         // GQA default: the first 6 pages of every split, at most 16 MB in all (C3: 88.8 us against 89.8 without;
         // 4 / 8 pages 89.2-89.4, 48 MB and more slower -- the prefetch then delays the selection kernel's own tail;
-        // the MLA decode (C4) loses 7 us with any of it: its first TMA boxes and the prefetch queue behind each other)
+        // MLA default: the first page only (73.7 KB pages: C4 71.0 -> 70.1 us with 1 page, 72.1 / 74.0 / 75.8 with 2 / 3 / 4 --
+        // the decode kernel's first TMA boxes queue behind the prefetches)
         const int64_t cap = ((int64_t)16 << 20) / (units * per_page > 0 ? units * per_page : 1);
-        const int want = c->prefetch_pages > 0 ? c->prefetch_pages : 6;
+        const int want = c->prefetch_pages > 0 ? c->prefetch_pages : (c->g.kv_shared ? 1 : 6);
         pf.pages_per_split = (int)(want < cap ? want : cap);
-        if (c->prefetch_pages < 0 && cap < 4) pf.pages_per_split = 0;   // big batches (C5): nothing to gain from 1-3 pages
+        if (c->prefetch_pages < 0 && !c->g.kv_shared && cap < 4) pf.pages_per_split = 0;   // big GQA batches (C5): nothing to gain from 1-3 pages
       }
       if (pf.pages_per_split < 1) pf.k = nullptr;
     }
