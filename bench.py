@@ -234,7 +234,7 @@ def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=No
     Returns (seconds for score + top-k + attention on the sample, requests in sample, batch, threads)."""
     from oracle import vx_oracle as vo
     from paper_2606_06453_b200.workloads import make_workload, subproblem
-    from tests.oracle_io import to_oracle
+    from oracle.workload_io import to_oracle
     w = workload if workload is not None else make_workload(cfg, device=device, seed_offset=seed_offset)
     n_requests = min(n_requests, w.spec.batch)
     sub = subproblem(w, range(n_requests))

@@ -56,8 +56,9 @@ typedef enum { VX_DT_BF16 = 0, VX_DT_F32 = 1 } vx_dtype;
 
 /* aggregation of per-head envelope scores over the heads of one KV head.
  * SUM ranks like the paper's mean ("topK(Sum(s))"); MAX is the max_h variant of
- * App. G (:556), built for GQA groups of <= 8 heads (g flop per byte on CUDA cores); for the 32-head
- * MLA group vx_create returns VX_ERR_UNSUPPORTED. */
+ * App. G (:556): built for GQA groups of <= 8 heads (g flop per byte on CUDA cores) and, as a tensor-core
+ * contraction, for the bf16 MLA group of 16 or 32 heads on one 576-wide latent head with envelope summaries;
+ * any other (geometry, MAX) pair makes vx_create return VX_ERR_UNSUPPORTED. */
 typedef enum { VX_AGG_SUM = 0, VX_AGG_MAX = 1 } vx_agg;
 
 /* what a page summary is (the query-independent cache of the flow):
@@ -126,16 +127,6 @@ const char *vx_last_error(const vx_ctx *ctx);
 /* Number of kernel launches the last compute call on this context enqueued (host counter). */
 int32_t vx_last_launch_count(const vx_ctx *ctx);
 
-/* Phase tracing (not part of the paper's method).  Only a library built with -DVX_TRACE
- * (`python -m paper_2606_06453_b200.build --trace` -> libvortex_b200_trace.so) records anything; the
- * product library returns VX_ERR_UNSUPPORTED.  `buffer` is a DEVICE pointer to max_ctas * 16 int64, owned
- * by the caller and zeroed by it; from the next launch on, every CTA (linear block index < max_ctas) of the
- * kernels named in `kernels` stores %globaltimer nanoseconds at its phase boundaries into its 16 slots
- * (slot 15: SM id; slot meanings: paper_2606_06453_b200/trace.py).  buffer == NULL detaches.  Attach one kind
- * at a time: the kinds share the slot numbering. */
-enum { VX_TRACE_SCORE = 1, VX_TRACE_TOPK = 2, VX_TRACE_DECODE = 4 };
-vx_status vx_trace_attach(vx_ctx *ctx, void *buffer, int32_t max_ctas, int32_t kernels);
-
 /* ---- (a1) summaries: PAPER.md:546 envelope, :89 query-independent, :529 per block ---- */
 /* For request i, rebuilds from the K pool the summary of every logical page
  * j >= first_new_pos[i] / page_size (first_new_pos == NULL: only the last page, i.e. the page
@@ -162,7 +153,10 @@ vx_status vx_page_score(vx_ctx *ctx, const void *q, const void *summary, const v
  * the k - #forced best-scoring of the rest (ties: lower logical index).  Exact.
  * sel_phys / sel_logical: dev [B, Hkv, max_budget], entries in ASCENDING logical order,
  * padded with -1; sel_logical may be NULL.  sel_count: dev [B, Hkv] = min(k, P_i).
- * max_budget (host) >= every budget[i]. */
+ * max_budget (host) >= every budget[i].  budget[i] lives on the device and is not validated on the host:
+ * a value above max_budget is clamped to it, a negative one selects nothing, and budget[i] < n_sink + n_local
+ * breaks the precondition of vx_geom.n_local (the first budget[i] forced pages in logical order are taken, so the
+ * newest page may be dropped and vx_sparse_decode_step then leaves its summary as it was). */
 vx_status vx_topk_pages(vx_ctx *ctx, const float *scores, const vx_page_table *pt,
                         const int32_t *budget /* dev [B] */, int32_t max_budget,
                         int32_t *sel_phys, int32_t *sel_logical, int32_t *sel_count,

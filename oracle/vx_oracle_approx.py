@@ -147,7 +147,8 @@ def select_one(scores_f32: np.ndarray, k: int, n_sink: int, n_local: int, tolera
             shift = max(0, _bitlen(width - 1) - K_BIN_BITS)
             fpass = False
         else:
-            lo, width = lo + (t << shift), 1 << shift
+            blo = lo + (t << shift)
+            lo, width = blo, min(1 << shift, lo + width - blo)    # the window never leaves [lo, lo + width)
             shift = max(0, shift - K_BIN_BITS)
     info["sure"] = cand[taken_above].astype(np.int64)
     sel = np.concatenate([j[forced], cand[taken_above], cand[chosen]]).astype(np.int64)

@@ -1,4 +1,5 @@
-"""Test-side glue: hand a workloads.Workload (torch tensors) to oracle/vx_oracle.py (numpy)."""
+"""Oracle-side glue (test infrastructure, like everything under oracle/): hand a workloads.Workload (torch tensors) to
+oracle/vx_oracle.py (numpy).  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import it."""
 import numpy as np
 
 from oracle import vx_oracle as vo

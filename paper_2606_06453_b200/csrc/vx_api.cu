@@ -4,7 +4,10 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <set>
+#include <utility>
 
 #include "vx_internal.h"
 
@@ -45,6 +48,16 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
 
 static char g_create_err[512] = "";
 
+cudaError_t ensure_dyn_smem(const void* kernel, int device, int bytes) {
+  static std::mutex mu;
+  static std::set<std::pair<const void*, int>> done;
+  std::lock_guard<std::mutex> lock(mu);
+  if (done.count({kernel, device})) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+  if (e == cudaSuccess) done.insert({kernel, device});
+  return e;
+}
+
 static vx_status fail(vx_ctx* c, vx_status st, const char* fmt, ...) {
   char* dst = c ? c->err : g_create_err;
   va_list ap;
@@ -79,7 +92,19 @@ static vx_status check_cuda(vx_ctx* c, cudaError_t e, const char* what) {
   return fail(c, VX_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
 }
 
+// every compute call: the context's kernels, workspace and per-device attributes belong to c->device
+static vx_status check_device(vx_ctx* c) {
+  int cur = -1;
+  const cudaError_t e = cudaGetDevice(&cur);
+  if (e != cudaSuccess) return fail(c, VX_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+  if (cur != c->device)
+    return fail(c, VX_ERR_INVALID_ARG, "the context is bound to device %d but the calling thread's current device is %d",
+                c->device, cur);
+  return VX_OK;
+}
+
 static vx_status check_table(vx_ctx* c, const vx_page_table* pt) {
+  if (vx_status st = check_device(c)) return st;
   if (!pt) return fail(c, VX_ERR_INVALID_ARG, "page table is NULL");
   if (pt->batch < 0 || pt->total_pages < 0 || pt->max_pages_per_req < 0)
     return fail(c, VX_ERR_INVALID_ARG, "negative size in page table");
@@ -149,26 +174,6 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->ws = carve_workspace(*g, workspace, max_batch, max_total_pages, max_budget);
   c->launches = 0;
   c->err[0] = 0;
-  const char* fg = getenv("VX_FORCE_GENERIC");
-  c->force_generic = fg && fg[0] == '1';
-  const char* np = getenv("VX_NO_PDL");
-  c->use_pdl = !(np && np[0] == '1');
-  const char* pm = getenv("VX_PREFETCH_MB");
-  c->prefetch_mb = pm ? atoi(pm) : 0;               // measured: no gain at 16 MB, slower beyond (the prefetch delays the selection kernel)
-  c->use_prefetch = c->prefetch_mb > 0;
-  const char* pp = getenv("VX_PREFETCH_PAGES");   // pages per decode split; unset = the measured default (see the step)
-  c->prefetch_pages = pp ? atoi(pp) : -1;
-  const char* ch = getenv("VX_CHAINS");
-  c->chains = ch && atoi(ch) >= 2 ? 2 : 1;      // measured: no gain on C2..C4 (the chains mostly serialise on shared memory), +3 % on C5
-  c->aux_stream = nullptr;
-  c->ev_fork = c->ev_join = nullptr;
-  e = cudaStreamCreateWithFlags(&c->aux_stream, cudaStreamNonBlocking);
-  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming);
-  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming);
-  if (e != cudaSuccess) {
-    delete c;
-    return fail(nullptr, VX_ERR_CUDA, "stream / event creation: %s", cudaGetErrorString(e));
-  }
   // split-arrival counters start at zero and every step leaves them at zero
   e = cudaMemset(c->ws.unit_counter, 0, (size_t)(max_batch > 0 ? max_batch : 1) * g->num_kv_heads * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -181,10 +186,6 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
 }
 
 void vx_destroy(vx_ctx* ctx) {
-  if (!ctx) return;
-  if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
-  if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
-  if (ctx->aux_stream) cudaStreamDestroy(ctx->aux_stream);
   delete ctx;
 }
 
@@ -341,7 +342,7 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   // are staged by the decode kernel anyway, so the decode kernel rebuilds its summary (same result, no extra
   // launch, no extra HBM bytes).  Otherwise the summary kernel runs first.
   DecodeOpts opt;
-  opt.pdl = c->use_pdl;
+  opt.pdl = true;                                // the kernels of a step are chained by programmatic dependent launch
   opt.budget = budget;
   if (flags & VX_STEP_UPDATE_SUMMARY) {
     if (c->g.n_local >= 1 && decode_folds_summary(c)) {
@@ -350,66 +351,34 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
       return st;
     }
   }
-  // Two request windows run as independent score -> top-k -> decode chains on two streams (fork / join by events,
-  // graph-capturable): every kernel has a few microseconds of start-up and tail that stream nothing, and the
-  // other chain's kernels fill them.  Results are identical: the path is independent per request.
-  const bool two = c->chains == 2 && pt->batch >= 2 && decode_folds_summary(c);
-  const int n0 = two ? (pt->batch + 1) / 2 : pt->batch;
-  cudaStream_t s1 = c->aux_stream;
-  if (two) {
-    cudaError_t e = cudaEventRecord(c->ev_fork, s);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(s1, c->ev_fork, 0);
-    if (vx_status st = check_cuda(c, e, "fork")) return st;
+  if (vx_status st = check_cuda(c, launch_page_score(c, q, summary, *pt, c->ws.scores, s), "page score")) return st;
+  // L2 prefetch plan for the decode kernel's first pages (fast decode paths with contiguous page chunks only): the
+  // selection kernel's emission issues it while HBM would otherwise idle between the two kernels.
+  // GQA: the first 6 pages of every split, at most 16 MB in all (measured on C3: 88.8 us against 89.8 without;
+  // 4 / 8 pages 89.2-89.4, 48 MB and more slower -- the prefetch then delays the selection kernel's own tail), none
+  // when a big batch leaves fewer than 4 (C5).  MLA (73.7 KB pages): the first page only (C4 71.0 -> 70.1 us with 1
+  // page, 72.1 / 74.0 / 75.8 with 2 / 3 / 4 -- the decode kernel's first TMA boxes queue behind the prefetches).
+  PrefetchPlan pf;
+  const int64_t esz = (int64_t)elem_size(c->g.dtype);
+  if (decode_folds_summary(c) && pool->stride_token == c->g.qk_dim) {
+    pf.k = pool->k;
+    pf.v = c->g.kv_shared ? nullptr : pool->v;
+    pf.page_bytes = pool->stride_page * esz;
+    pf.head_bytes = pool->stride_head * esz;
+    pf.chunk_bytes = (uint32_t)(c->g.page_size * c->g.qk_dim * esz);
+    pf.splits = c->g.kv_shared ? decode_mla_splits(c, pt->batch, max_budget) : decode_gqa_splits(c, pt->batch, max_budget);
+    const int64_t per_page = (int64_t)pf.chunk_bytes * (pf.v ? 2 : 1);
+    const int64_t units = (int64_t)pt->batch * c->g.num_kv_heads * pf.splits;
+    const int64_t cap = ((int64_t)16 << 20) / (units * per_page > 0 ? units * per_page : 1);
+    const int want = c->g.kv_shared ? 1 : 6;
+    pf.pages_per_split = (int)(want < cap ? want : cap);
+    if (!c->g.kv_shared && cap < 4) pf.pages_per_split = 0;
+    if (pf.pages_per_split < 1) pf.k = nullptr;
   }
-  int total_launches = 0;
-  for (int ch = 0; ch < (two ? 2 : 1); ++ch) {
-    cudaStream_t cs = ch == 0 ? s : s1;
-    ReqRange rr;
-    rr.begin = ch == 0 ? 0 : n0;
-    rr.count = two ? (ch == 0 ? n0 : pt->batch - n0) : -1;
-    opt.rr = rr;
-    if (vx_status st = check_cuda(c, launch_page_score(c, q, summary, *pt, c->ws.scores, cs, rr), "page score")) return st;
-    // L2 prefetch plan for the decode kernel's first pages (fast decode paths with contiguous page chunks only)
-    PrefetchPlan pf;
-    const int64_t esz = (int64_t)elem_size(c->g.dtype);
-    const bool pf_auto = !c->use_prefetch && c->prefetch_pages != 0;
-    if ((c->use_prefetch || pf_auto) && decode_folds_summary(c) && pool->stride_token == c->g.qk_dim) {
-      const int n_req = rr.count < 0 ? pt->batch : rr.count;
-      pf.k = pool->k;
-      pf.v = c->g.kv_shared ? nullptr : pool->v;
-      pf.page_bytes = pool->stride_page * esz;
-      pf.head_bytes = pool->stride_head * esz;
-      pf.chunk_bytes = (uint32_t)(c->g.page_size * c->g.qk_dim * esz);
-      pf.splits = c->g.kv_shared ? decode_mla_splits(c, n_req, max_budget) : decode_gqa_splits(c, n_req, max_budget);
-      const int64_t per_page = (int64_t)pf.chunk_bytes * (pf.v ? 2 : 1);
-      const int64_t units = (int64_t)n_req * c->g.num_kv_heads * pf.splits;
-      const int64_t budget_bytes = (int64_t)c->prefetch_mb << 20;
-      pf.pages_per_split = (int)(budget_bytes / (units * per_page > 0 ? units * per_page : 1));
-      if (pf_auto) {
-        // GQA default: the first 6 pages of every split, at most 16 MB in all (C3: 88.8 us against 89.8 without;
-        // 4 / 8 pages 89.2-89.4, 48 MB and more slower -- the prefetch then delays the selection kernel's own tail;
-        // MLA default: the first page only (73.7 KB pages: C4 71.0 -> 70.1 us with 1 page, 72.1 / 74.0 / 75.8 with 2 / 3 / 4 --
-        // the decode kernel's first TMA boxes queue behind the prefetches)
-        const int64_t cap = ((int64_t)16 << 20) / (units * per_page > 0 ? units * per_page : 1);
-        const int want = c->prefetch_pages > 0 ? c->prefetch_pages : (c->g.kv_shared ? 1 : 6);
-        pf.pages_per_split = (int)(want < cap ? want : cap);
-        if (c->prefetch_pages < 0 && !c->g.kv_shared && cap < 4) pf.pages_per_split = 0;   // big GQA batches (C5): nothing to gain from 1-3 pages
-      }
-      if (pf.pages_per_split < 1) pf.k = nullptr;
-    }
-    if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, cs,
-                                                       c->use_pdl, rr, pf, ap), "top-k pages"))
-      return st;
-    if (vx_status st = decode_dispatch(c, q, pool, pt, sp, sl, sc, max_budget, out, lse, cs, opt)) return st;
-    total_launches = c->launches;
-  }
-  (void)total_launches;
-  if (two) {
-    cudaError_t e = cudaEventRecord(c->ev_join, s1);
-    if (e == cudaSuccess) e = cudaStreamWaitEvent(s, c->ev_join, 0);
-    if (vx_status st = check_cuda(c, e, "join")) return st;
-  }
-  return VX_OK;
+  if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, s, true,
+                                                     ReqRange(), pf, ap), "top-k pages"))
+    return st;
+  return decode_dispatch(c, q, pool, pt, sp, sl, sc, max_budget, out, lse, s, opt);
 }
 
 vx_status vx_sparse_decode_step_host(vx_ctx* c, const void* h_q, const vx_kv_pool* pool, void* summary,

@@ -211,7 +211,7 @@ cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
                               const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                               int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
   const vx_geom& g = c->g;
-  if (gqa_mma_supported(g) && !c->force_generic)
+  if (gqa_mma_supported(g))
     return launch_decode_gqa_mma(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt);
 #define VX_GO(T, D, HPW, WT) \
   return launch_generic_t<T, D, D, HPW, WT>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s)
@@ -229,7 +229,7 @@ cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
 cudaError_t launch_decode_mla(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                               int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
-  if (mla_tc_supported(c->g) && !c->force_generic)
+  if (mla_tc_supported(c->g))
     return launch_decode_mla_tc(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt);
   // CUDA-core fallback: 32 heads = 8 head-groups of 4 per CTA, one token slice: 8 warps
   return launch_generic_t<__nv_bfloat16, 576, 512, 4, 1>(c, q, pool, pt, sel_phys, sel_logical, sel_count,

@@ -83,7 +83,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   const int grp = num_q_heads / num_kv_heads;
   const int n_tok = seq_lens[i];
   const int newest_page = (n_tok - 1) / kGqaPage;
-  const int cnt_known = budget_opt ? min(min(budget_opt[i], max_budget), newest_page + 1) : -1;
+  const int cnt_known = budget_opt ? max(0, min(min(budget_opt[i], max_budget), newest_page + 1)) : -1;
 
   // Q^T as the B operand: qb[ks] = Q[head lane/4][16*ks + 2*(lane%4) + {0,1}], [.. + 8 ..]
   uint32_t qb[KS][2];
@@ -340,12 +340,7 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
                                     int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
   const vx_geom& g = c->g;
   constexpr int smem = kGqaWarps * kGqaStages * 2 * kGqaPage * D * 2;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(decode_gqa_mma_kernel<D>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_gqa_mma_kernel<D>), c->device, smem)) return e;
   // splits: whole waves of equal CTAs.  cost(sp) = waves x (pages per warp + ~3 pages of pipeline fill)
   const int n_req = opt.rr.count < 0 ? pt.batch : opt.rr.count;
   const int splits = decode_gqa_splits(c, n_req, max_budget);
@@ -373,7 +368,7 @@ int decode_gqa_splits(const vx_ctx* c, int n_req, int max_budget) {
   return splits;
 }
 
-bool decode_folds_summary(const vx_ctx* c) { return !c->force_generic && (gqa_mma_supported(c->g) || mla_tc_supported(c->g)); }
+bool decode_folds_summary(const vx_ctx* c) { return (gqa_mma_supported(c->g) || mla_tc_supported(c->g)); }
 
 cudaError_t launch_decode_gqa_mma(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,

@@ -32,7 +32,6 @@
 // fused step the CTA holding the request's newest page also rebuilds that page's summary (min / max, or the
 // block top-k centroid) from the staged tile (a1; the newest page is a forced local page).
 #include <cuda.h>
-#include <cstdlib>
 
 #include "vx_common.cuh"
 #include "vx_internal.h"
@@ -358,7 +357,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
   auto bar = [&](int idx) -> uint32_t { return bar0 + 8u * (uint32_t)idx; };
   const int n_tok = seq_lens[i];
   const int newest_page = (n_tok - 1) / PAGE;
-  const int cnt_known = budget_opt ? min(min(budget_opt[i], max_budget), newest_page + 1) : -1;
+  const int cnt_known = budget_opt ? max(0, min(min(budget_opt[i], max_budget), newest_page + 1)) : -1;
 
   // ---- prologue (overlaps the preceding kernel under PDL): barriers, TMEM, Q tile ---------------------
   if (warp == 1) {
@@ -774,12 +773,7 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
                                  const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                                  int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
   const vx_geom& g = c->g;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(decode_mla_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, mla::SMEM_BYTES);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_mla_kernel), c->device, mla::SMEM_BYTES)) return e;
   CUtensorMap kmap;
   if (cudaError_t e = make_latent_map(&kmap, pool)) return e;
   // one CTA per SM (221 KB of shared memory): whole waves of equal CTAs,
@@ -788,9 +782,7 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
   const int best = decode_mla_splits(c, n_req, max_budget);
   dim3 grid(best, 1, n_req);
   // splits of 2, 4 or 8: the splits of a request form a thread-block cluster and merge through shared memory
-  static int no_cluster = -1;
-  if (no_cluster < 0) { const char* ev = getenv("VX_NO_CLUSTER"); no_cluster = ev && atoi(ev) ? 1 : 0; }
-  const int cluster = (!no_cluster && (best == 2 || best == 4 || best == 8)) ? best : 1;
+  const int cluster = (best == 2 || best == 4 || best == 8) ? best : 1;
   cudaError_t e = launch_kernel_cluster(decode_mla_kernel, grid, dim3(mla::THREADS), (size_t)mla::SMEM_BYTES, s, opt.pdl, cluster, kmap,
                                 static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens,
                                 sel_phys, sel_logical, sel_count, max_budget, best, c->ws.part_o, c->ws.part_lse,

@@ -4,6 +4,7 @@
 #include <stdint.h>
 
 #include "../../include/vortex_b200.h"
+#include "../../include/vortex_b200_trace.h"
 
 namespace vx {
 
@@ -49,19 +50,15 @@ struct vx_ctx {
   int32_t max_batch, max_total_pages, max_pages_per_req, max_budget;
   vx::Workspace ws;
   int32_t launches;              // kernels enqueued by the last compute call
-  bool force_generic;            // VX_FORCE_GENERIC=1 in the environment: CUDA-core decode path only (debug)
-  bool use_pdl;                  // chain the kernels of a step with programmatic dependent launch (VX_NO_PDL=1: off)
-  bool use_prefetch;             // the selection kernel prefetches the decode kernel's first pages into L2 (VX_PREFETCH_MB=0: off)
-  int prefetch_mb;               // prefetch budget, MiB (VX_PREFETCH_MB; 0 = use prefetch_pages)
-  int prefetch_pages;            // pages per decode split to prefetch (VX_PREFETCH_PAGES; -1 = default: 6 for GQA, none for MLA)
-  int chains;                    // request windows run as concurrent kernel chains inside a fused step (VX_CHAINS, 1 or 2)
-  cudaStream_t aux_stream;       // second chain's stream; fork / join with the caller's stream by events
-  cudaEvent_t ev_fork, ev_join;
   vx::ApproxPlan approx;         // vx_set_topk_approx: used by a fused step with VX_STEP_APPROX_TOPK
   char err[512];
 };
 
 namespace vx {
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) holds per DEVICE: the opt-in is remembered per (kernel, device),
+// so contexts on several GPUs of one process each get it (a process-wide flag would skip the second device).
+cudaError_t ensure_dyn_smem(const void* kernel, int device, int bytes);
 
 // One kernel launch; pdl = allow it to start while its predecessor in the stream drains (the kernel
 // itself calls pdl_wait() before touching what the predecessor wrote).
@@ -109,9 +106,7 @@ inline cudaError_t launch_kernel_cluster(void (*kernel)(KArgs...), dim3 grid, di
   return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
-// a window of requests [begin, begin + count) of the page table; count < 0 = the whole batch.  The fused step runs
-// two such windows as independent kernel chains on two streams so that one chain's start-up and tail latencies
-// (index chains, first-stage latency, selection phases, split merge) overlap the other chain's streaming.
+// a window of requests [begin, begin + count) of the page table; count < 0 = the whole batch
 struct ReqRange {
   int begin = 0;
   int count = -1;
@@ -120,7 +115,7 @@ struct ReqRange {
 // What the selection kernel prefetches into L2 for the decode kernel that follows it in a step: the first
 // `pages_per_split` pages of every split of every (request, KV head), K and V chunks (`chunk_bytes` contiguous
 // bytes each).  Between the end of the selection and the decode kernel's first loads HBM would sit idle; the
-// prefetch moves up to ~48 MB of the decode kernel's stream into that gap.  k == nullptr: no prefetch.
+// prefetch moves a few MB of the decode kernel's stream into that gap.  k == nullptr: no prefetch.
 struct PrefetchPlan {
   const void* k = nullptr;
   const void* v = nullptr;                       // nullptr: K only (MLA latent)
@@ -156,7 +151,7 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
                               int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl = false,
                               const ReqRange& rr = ReqRange(), const PrefetchPlan& pf = PrefetchPlan(),
                               const ApproxPlan& ap = ApproxPlan());
-// the same selection with each problem on a cluster of two CTAs (vx_topk_pair.cu); VX_TOPK_PAIR=0 turns it off
+// the same selection with each problem on a cluster of two CTAs (vx_topk_pair.cu)
 bool topk_pair_applies(const vx_ctx* c, int n_problems, int max_pages_per_req);
 cudaError_t launch_topk_pair(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
                              int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,

@@ -437,12 +437,7 @@ static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summar
   constexpr int kFoot = (HKV == 1 ? 110 : 72) * 1024;
   constexpr int kScStages = clamp_int((int)((kFoot - q_bytes) / (PG * page_bytes)), 3, 8);
   constexpr size_t smem = kScStages * PG * page_bytes + q_bytes;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(score_kernel<T, D, PG, HKV, kScStages, AGG, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(score_kernel<T, D, PG, HKV, kScStages, AGG, KIND>), c->device, (int)smem)) return e;
   int ctas = c->num_sms * (2 * smem + 4096 <= 227 * 1024 ? 2 : 1);   // two CTAs per SM when they fit
   const int min_pages = 2 * PG;                  // do not spread tiny inputs over every SM
   const int64_t est_pages = rr.count < 0 ? pt.total_pages : (int64_t)pt.total_pages * rr.count / (pt.batch > 0 ? pt.batch : 1) + 1;

@@ -169,12 +169,7 @@ template <int MT>
 static cudaError_t launch_mt(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt, float* scores,
                              cudaStream_t s, const ReqRange& rr) {
   constexpr int smem = 16 * MT * kARowBytes;
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(score_mla_max_kernel<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(score_mla_max_kernel<MT>), c->device, smem)) return e;
   const int n_req = rr.count < 0 ? pt.batch : rr.count;
   // CTAs per request: enough warps for the longest request's chunks, capped at ~2 resident CTAs per SM over the batch
   // (one chunk per warp whatever the batch -- 512 CTAs on C4 -- measured 35.0 us against 32.5: every CTA rebuilds A);

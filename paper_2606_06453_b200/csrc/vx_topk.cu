@@ -19,7 +19,6 @@
 // partial last page comes last); the selected ids are staged in shared memory and the physical ids
 // gathered from the page table in one parallel pass.
 // Integer work on a few KB per problem -- latency-bound, not bandwidth-bound.
-#include <cstdlib>
 #include <type_traits>
 
 #include "vx_common.cuh"
@@ -63,7 +62,7 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
   const int kvh = blockIdx.x, i = blockIdx.y + req0;
   const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
-  const int k = min(budget[i], max_budget);
+  const int k = max(0, min(budget[i], max_budget));   // a negative budget selects nothing (never indexes below the row)
   const int row0 = page_indptr[i];
   pdl_wait();                                   // the scores (and, in a step, nothing else) come from the predecessor
   const int64_t out0 = ((int64_t)i * num_kv_heads + kvh) * max_budget;
@@ -224,8 +223,11 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
         need_eq = s_need_eq;
         break;
       }
-      lo = bin_lo;                              // heavy ties: recurse into the bin, 11 more bits
-      width = (uint64_t)1 << shift;
+      // heavy ties: recurse into the bin, 11 more bits.  The window stays inside [lo, lo + width): after a float pass the
+      // interval [bmin, bmax] is unaligned, so its last sub-bin ends at bmax, not at bin_lo + 2^shift (keys above bmax
+      // belong to a higher float bin and are already counted)
+      width = min((uint64_t)1 << shift, (uint64_t)lo + width - bin_lo);
+      lo = bin_lo;
       shift = max(0, shift - kBinBits);
     }
   }
@@ -303,13 +305,7 @@ static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_t
   const vx_geom& g = c->g;
   const int keys = pt.max_pages_per_req <= kTopkSmemKeys ? pt.max_pages_per_req : 0;
   const size_t smem = (size_t)(keys > 0 ? keys : 1) * sizeof(uint32_t);
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(topk_kernel<THREADS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         kTopkSmemKeys * (int)sizeof(uint32_t));
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(topk_kernel<THREADS>), c->device, kTopkSmemKeys * (int)sizeof(uint32_t))) return e;
   dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
   cudaError_t e = launch_kernel(topk_kernel<THREADS>, grid, dim3(THREADS), smem, s, pdl, scores, g.num_kv_heads,
                                 pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
@@ -350,7 +346,7 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   [[maybe_unused]] const int cta = blockIdx.y * gridDim.x + blockIdx.x;
   if (tid == 0) { VX_TRACE_STAMP(cta, 0); VX_TRACE_SMID(cta); }
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
-  const int k = min(budget[i], max_budget);
+  const int k = max(0, min(budget[i], max_budget));   // a negative budget selects nothing (never indexes below the row)
   const int row0 = page_indptr[i];
   for (int b = tid; b < kBins; b += THREADS) s_hist[b] = 0;      // first pass's histogram, zeroed under the loads
   if (tid == 0) VX_TRACE_STAMP(cta, 1);
@@ -513,8 +509,8 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
         shift = max(0, (32 - __clz(s_bmax - s_bmin)) - kBinBits);
         fpass = false;
       } else {                                  // heavy ties: recurse into the bin, 11 more bits
+        width = min(bin_w, (uint64_t)lo + width - bin_lo);   // never past the live window (unaligned after a float pass)
         lo = bin_lo;
-        width = bin_w;
         shift = max(0, shift - kBinBits);
       }
       __syncthreads();                          // s_bmin / s_bmax / s_bin are read before the next pass rewrites them
@@ -641,34 +637,21 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
                               const PrefetchPlan& pf, const ApproxPlan& ap) {
   if (pt.batch == 0) return cudaSuccess;
   if (ap.tolerate_ratio > 0.f && pt.max_pages_per_req > kTopkRegMaxPages) return cudaErrorNotSupported;
-  // block size by problem size (VX_TOPK_THREADS overrides, for tuning; it also selects the shared-memory-key kernel)
-  static int force = -1;
-  if (force < 0) { const char* e = getenv("VX_TOPK_THREADS"); force = e ? atoi(e) : 0; }
+  // block size by problem size
   const int n = pt.max_pages_per_req;
-  static int pair = -1;
-  if (pair < 0) { const char* e = getenv("VX_TOPK_PAIR"); pair = e ? atoi(e) : 1; }
-  if (pair && !force && ap.tolerate_ratio <= 0.f &&
-      topk_pair_applies(c, c->g.num_kv_heads * (rr.count < 0 ? pt.batch : rr.count), n))
+  if (ap.tolerate_ratio <= 0.f && topk_pair_applies(c, c->g.num_kv_heads * (rr.count < 0 ? pt.batch : rr.count), n))
     return launch_topk_pair(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
-  if ((!force || ap.tolerate_ratio > 0.f) && n <= kTopkRegMaxPages) {                  // keys fit the registers of one CTA, 8 per thread (16 measured slower)
+  if (n <= kTopkRegMaxPages) {                   // keys fit the registers of one CTA
 #define VX_REG(T, K) return launch_topk_reg<T, K>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap)
-    // short requests: 4 keys per thread on twice the threads (C4 71.5 -> 70.9 us, C2 106.8 -> 106.2; VX_TOPK_KPT=8 / 2 for the A/B)
-    static int kpt = -1;
-    if (kpt < 0) { const char* e = getenv("VX_TOPK_KPT"); kpt = e ? atoi(e) : 4; }
-    if (kpt == 4) {
-      if (n <= 1024) VX_REG(256, 4);
-      if (n <= 2048) VX_REG(512, 4);
-    } else if (kpt == 2) {
-      if (n <= 1024) VX_REG(512, 2);
-      if (n <= 2048) VX_REG(1024, 2);
-    }
-    if (n <= 1024) VX_REG(128, 8);
-    if (n <= 2048) VX_REG(256, 8);
+    // short requests: 4 keys per thread on twice the threads (measured: C4 71.5 -> 70.9 us, C2 106.8 -> 106.2 against 8
+    // keys per thread; 2 keys on four times the threads and 16 keys per thread were slower)
+    if (n <= 1024) VX_REG(256, 4);
+    if (n <= 2048) VX_REG(512, 4);
     if (n <= 4096) VX_REG(512, 8);
     VX_REG(1024, 8);
 #undef VX_REG
   }
-  const int th = force ? force : (n <= 1024 ? 256 : n <= 4096 ? 512 : 1024);
+  const int th = n <= 1024 ? 256 : n <= 4096 ? 512 : 1024;
   if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
   if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
   return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);

@@ -54,7 +54,7 @@ topk_pair_kernel(const float* __restrict__ scores, int num_kv_heads, int total_p
   const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
   const int gw = crank * WARPS + warp;
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
-  const int k = min(budget[i], max_budget);
+  const int k = max(0, min(budget[i], max_budget));   // a negative budget selects nothing (never indexes below the row)
   const int row0 = page_indptr[i];
   for (int b = tid; b < kBins; b += THREADS) s_hist[b] = 0;      // first pass's histogram, zeroed under the loads
   pdl_wait();                                   // the scores come from the predecessor
@@ -208,8 +208,8 @@ topk_pair_kernel(const float* __restrict__ scores, int num_kv_heads, int total_p
         shift = max(0, (32 - __clz(bmax - bmin)) - kBinBits);
         fpass = false;
       } else {                                  // heavy ties: recurse into the bin, 11 more bits
+        width = min(bin_w, (uint64_t)lo + width - bin_lo);   // never past the live window (unaligned after a float pass)
         lo = bin_lo;
-        width = bin_w;
         shift = max(0, shift - kBinBits);
       }
       // (the next pass starts with a cluster barrier after zeroing: the peer has read my s_bmin / s_bmax by then,

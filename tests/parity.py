@@ -9,7 +9,7 @@ attention : compared with the oracle evaluated on the GPU's own selected set:
 import numpy as np
 
 from oracle import vx_oracle as vo
-from tests.oracle_io import to_oracle
+from oracle.workload_io import to_oracle
 
 TOL = {"bf16": dict(abs=2e-2, rel=1e-2, lse=1e-3), "f32": dict(abs=1e-4, rel=1e-4, lse=1e-5)}
 

@@ -20,9 +20,12 @@ def vx():
 
 
 def declared_functions():
-    text = open(os.path.join(ROOT, "include", "vortex_b200.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(vx_[a-z_]+)\s*\(", text)))
+    names = set()
+    for header in sorted(os.listdir(os.path.join(ROOT, "include"))):      # every include/*.h
+        text = open(os.path.join(ROOT, "include", header)).read()
+        text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+        names |= set(re.findall(r"\b(vx_[a-z_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_header_symbols_are_exported(vx):

@@ -1,7 +1,14 @@
-"""vx_topk_pages_approx against oracle/vx_oracle_approx.py (-m gpu): bit-exact ids, order, counts and padding.
-Both sides take every decision (keys, bins, the fp32 remap of the first pass, the termination test, the SplitMix64
-draw) on the same fp32 scores, so the lossy selection itself is reproducible and compared exactly
-(DESIGN.md section 12)."""
+"""vx_topk_pages_approx (-m gpu).
+
+THE PARITY GATE is `check_against_exact`: every case's GPU output is held against the EXACT C oracle
+(oracle/vx_oracle.c, a full sort -- code that shares nothing with the kernel) by the properties the paper fixes for a
+lossy selection: recall@k >= 1 - tolerate_ratio (|exact minus gpu| <= floor(tolerate_ratio * k), :196, :538), forced pages
+present (:280), sel_count = min(k, P), strictly ascending in-range ids, physical ids through the page table, the same
+seed gives the same set, and tolerate_ratio = 0 gives the exact set.
+
+The bit-equality with oracle/vx_oracle_approx.py that the tests also assert is a REGRESSION check only: that file
+follows the kernel's encoding (bin count, remap, sampler; readings G20-G23), so agreeing with it shows that the
+encoding did not drift, not that it is right."""
 import numpy as np
 import pytest
 import torch
@@ -12,6 +19,37 @@ from paper_2606_06453_b200.workloads import APPD_DISTRIBUTIONS, appd_scores
 from tests.test_gpu_topk_fuzz import KINDS, draw_scores
 
 pytestmark = pytest.mark.gpu
+
+
+def check_against_exact(scores, pages, seq, indices, budget, n_sink, n_local, tau, gpu, b=16):
+    """the structure-independent gate: GPU output vs the exact C oracle (see the module docstring)"""
+    sl, sp, sc = gpu
+    indptr = np.concatenate([[0], np.cumsum(pages)]).astype(np.int64)
+    pt_o = vo.PageTable(indptr.astype(np.int32), indices, np.array(seq, np.int32), b)
+    mb = int(budget.max())
+    sl_e, _, sc_e, _ = vo.topk_pages(scores.astype(np.float64), pt_o, budget, n_sink, n_local, mb)
+    assert np.array_equal(sc, sc_e), "sel_count != min(k, P)"
+    worst = 1.0
+    for i, P in enumerate(pages):
+        k = min(int(budget[i]), mb)
+        for h in range(scores.shape[0]):
+            n = int(sc_e[i, h])
+            assert n == min(k, P)
+            got = sl[i, h, :n]
+            assert (sl[i, h, n:] == -1).all() and (sp[i, h, n:] == -1).all(), "padding"
+            assert got.min(initial=0) >= 0 and got.max(initial=0) < P and (np.diff(got) > 0).all(), "ascending in-range ids"
+            assert np.array_equal(sp[i, h, :n], indices[indptr[i] + got]), "physical ids follow the page table"
+            forced = [j for j in range(P) if j < n_sink or j >= P - n_local]
+            if k >= len(forced):
+                assert set(forced) <= set(got.tolist()), "forced pages (PAPER.md:280)"
+            missed = len(set(sl_e[i, h, :n].tolist()) - set(got.tolist()))
+            allowed = int(np.floor(np.float32(tau) * np.float32(k)))
+            assert missed <= allowed, f"request {i} head {h}: {missed} exact pages missed, {allowed} allowed at ratio {tau}"
+            if n:
+                worst = min(worst, 1.0 - missed / n)
+            if tau == 0.0:
+                assert np.array_equal(got, sl_e[i, h, :n]), "ratio 0 is the exact selection"
+    return worst
 
 
 def run_both(scores, pages, seq, indices, budget, n_sink, n_local, tau, seed, b=16):
@@ -33,13 +71,20 @@ def run_both(scores, pages, seq, indices, budget, n_sink, n_local, tau, seed, b=
     ctx.topk_pages_approx(torch.from_numpy(scores).to(dev), pt, torch.from_numpy(budget).to(dev), mb, tau, seed,
                           sp, sl, sc)
     torch.cuda.synchronize()
+    gpu = (sl.cpu().numpy(), sp.cpu().numpy(), sc.cpu().numpy())
+    sl2, sp2 = torch.full_like(sl, -7), torch.full_like(sl, -7)         # the same seed reproduces the selection
+    ctx.topk_pages_approx(torch.from_numpy(scores).to(dev), pt, torch.from_numpy(budget).to(dev), mb, tau, seed,
+                          sp2, sl2, sc)
+    torch.cuda.synchronize()
+    assert torch.equal(sl2, sl) and torch.equal(sp2, sp)
     ctx.close()
-    return ref, (sl.cpu().numpy(), sp.cpu().numpy(), sc.cpu().numpy())
+    check_against_exact(scores, pages, seq, indices, budget, n_sink, n_local, tau, gpu, b)     # the parity gate
+    return ref, gpu
 
 
 @pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
 @pytest.mark.parametrize("tau", [0.0, 0.05, 0.25, 1.0])
-def test_appd_distributions_bit_exact(dist, tau):
+def test_appd_distributions(dist, tau):
     rng = np.random.default_rng(5)
     pages = [2048, 777, 8192, 40, 4100]
     hkv = 2
@@ -63,7 +108,7 @@ def test_appd_distributions_bit_exact(dist, tau):
 
 @pytest.mark.parametrize("kind", KINDS)
 @pytest.mark.parametrize("tau", [0.1, 0.5])
-def test_fuzz_kinds_bit_exact(kind, tau):
+def test_fuzz_kinds(kind, tau):
     rng = np.random.default_rng(77 + KINDS.index(kind))
     n_sink, n_local = int(rng.integers(0, 3)), int(rng.integers(0, 4))
     pages = [int(x) for x in rng.choice([1, 3, 40, 300, 1025, 2048, 5000, 8192], size=5)]
@@ -78,18 +123,23 @@ def test_fuzz_kinds_bit_exact(kind, tau):
     assert np.array_equal(sp, sp_r), kind
 
 
-def test_seed_changes_only_the_sampled_members_and_recall_holds():
-    pages, k, tau = [4096], 128, 0.25
-    scores = appd_scores("normal", (8, 4096), seed=41).numpy()
+@pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
+@pytest.mark.parametrize("tau", [0.05, 0.25])
+def test_seed_changes_only_the_sampled_members_and_recall_holds(dist, tau):
+    pages, k = [4096], 128
+    scores = appd_scores(dist, (8, 4096), seed=41).numpy()
     indices = np.arange(4096, dtype=np.int32)
     budget = np.array([k], np.int32)
     exact = run_both(scores, pages, [4096 * 16], indices, budget, 1, 2, 0.0, 0)[1][0]
-    a = run_both(scores, pages, [4096 * 16], indices, budget, 1, 2, tau, 1)[1][0]
+    (_, _, _, early), (a, _, _) = run_both(scores, pages, [4096 * 16], indices, budget, 1, 2, tau, 1)
     b = run_both(scores, pages, [4096 * 16], indices, budget, 1, 2, tau, 2)[1][0]
-    assert not np.array_equal(a, b)
-    for h in range(8):
+    if early.any():
+        assert not np.array_equal(a, b)
+    for h in range(8):                                  # (run_both has already held a and b against the exact oracle)
         assert va.recall_at_k(a[0, h], exact[0, h]) >= 1 - tau
         assert va.recall_at_k(b[0, h], exact[0, h]) >= 1 - tau
+        if not early[0, h]:
+            assert np.array_equal(a[0, h], exact[0, h])
 
 
 def test_argument_checks():
@@ -146,6 +196,10 @@ def test_fused_step_with_approximate_selection(name):
                                                    w.page_indices.cpu().numpy(), w.seq_lens.cpu().numpy(), s.page_size,
                                                    w.budget.cpu().numpy(), s.n_sink, s.n_local, w.max_budget, tau, seed)
     assert early.any()                                                  # the lossy path was actually taken
+    pages = [int(x) for x in np.diff(w.page_indptr.cpu().numpy())]
+    check_against_exact(scores.cpu().numpy(), pages, w.seq_lens.cpu().numpy().tolist(), w.page_indices.cpu().numpy(),
+                        w.budget.cpu().numpy(), s.n_sink, s.n_local, tau,
+                        (sl.cpu().numpy(), sp.cpu().numpy(), sc.cpu().numpy()), b=s.page_size)   # the parity gate
     assert np.array_equal(sc.cpu().numpy(), sc_r)
     assert np.array_equal(sl.cpu().numpy(), sl_r) and np.array_equal(sp.cpu().numpy(), sp_r)
     o_ref, l_ref = oracle_attention_on(w, sl.cpu().numpy(), sc.cpu().numpy())

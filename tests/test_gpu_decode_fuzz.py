@@ -5,7 +5,7 @@ import numpy as np
 import pytest
 import torch
 
-from tests.oracle_io import to_oracle
+from oracle.workload_io import to_oracle
 from tests.parity import check_attention
 from oracle import vx_oracle as vo
 
@@ -59,7 +59,7 @@ def test_mla_decode_cluster_merge_at_every_cluster_size(batch, splits):
     from dataclasses import replace
     import paper_2606_06453_b200 as vx
     from paper_2606_06453_b200.workloads import make_workload, SPECS
-    from tests.oracle_io import oracle_step
+    from oracle.workload_io import oracle_step
     from tests.parity import check_selection, oracle_attention_on
     w = make_workload(replace(SPECS["C4-small"], name=f"C4-small-b{batch}", batch=batch, seq_len=(200, 3000)), device="cuda:0")
     s = w.spec

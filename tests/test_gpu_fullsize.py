@@ -7,7 +7,7 @@ import pytest
 import torch
 
 from oracle import vx_oracle as vo
-from tests.oracle_io import oracle_step, to_oracle
+from oracle.workload_io import oracle_step, to_oracle
 from tests.parity import check_attention, check_selection
 
 pytestmark = pytest.mark.gpu

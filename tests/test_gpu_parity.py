@@ -12,7 +12,7 @@ import pytest
 import torch
 
 from oracle import vx_oracle as vo
-from tests.oracle_io import bf16_bits_to_f64, oracle_step, to_oracle
+from oracle.workload_io import bf16_bits_to_f64, oracle_step, to_oracle
 from tests.parity import check_attention, check_selection, oracle_attention_on
 
 pytestmark = pytest.mark.gpu

@@ -61,7 +61,7 @@ def test_decode_over_the_union_table(name):
     union set within the bf16 tolerances."""
     import paper_2606_06453_b200 as vx
     from paper_2606_06453_b200.workloads import make_workload
-    from tests.oracle_io import oracle_step
+    from oracle.workload_io import oracle_step
     from tests.parity import check_attention, oracle_attention_on
     w = make_workload(name, device="cuda:0")
     s = w.spec

@@ -69,6 +69,34 @@ def test_ratio_zero_heavy_ties_and_sign_spanning_ranges():
         assert np.array_equal(sl, sl_e), (trial, P, k)
 
 
+def test_ratio_zero_ties_at_the_top_edge_of_a_float_bin():
+    """Round-1 advisor finding: a heavy float-pass bin is handed over as the UNALIGNED key interval [bmin, bmax]; when
+    its last integer sub-bin is heavy again the recursion window must end at bmax, or the first key of the next
+    float bin is counted twice.  Scores {-1, 3, b + 1 ulp, b - 3000 ulp, 300 x b}, b = 1 - 2^-23 = the last fp32 value
+    of float bin 1023 of the range [-1, 3].  Expected value: the exact C oracle (full sort)."""
+    b = np.float32(1.0) - np.float32(2.0 ** -23)
+    up = np.nextafter(b, np.float32(2.0))
+    down = (b.view(np.uint32) - np.uint32(3000)).view(np.float32)
+    s = np.array([-1.0, 3.0, up, down] + [b] * 300, dtype=np.float32)[None]
+    for k in (3, 50, 102, 200, 302):
+        budget = np.array([k], dtype=np.int32)
+        indptr, pt, sl_e, sc_e = exact_sets(s, [s.shape[1]], budget, 0, 0, k)
+        sel, info = va.select_one(s[0], k, 0, 0, 0.0, 0, 0)
+        assert sel.shape[0] == k and len(set(sel.tolist())) == k
+        assert sel.tolist() == sl_e[0, 0, :k].tolist(), k
+        if 3 <= k <= 302:
+            assert info["passes"] >= 3                                    # float pass -> integer pass -> recursion
+    rng = np.random.default_rng(9)
+    for trial in range(20):                                               # the same values in random order and counts
+        n = int(rng.integers(300, 1500))
+        row = rng.choice(np.array([-1.0, 3.0, up, down, b], np.float32), size=n, p=[0.05, 0.05, 0.1, 0.1, 0.7])
+        k = int(rng.integers(3, n))
+        budget = np.array([k], dtype=np.int32)
+        indptr, pt, sl_e, _ = exact_sets(row[None], [n], budget, 1, 2, k)
+        sel, _ = va.select_one(row, k, 1, 2, 0.0, 0, 0)
+        assert sel.tolist() == sl_e[0, 0, :k].tolist(), (trial, n, k)
+
+
 def test_ratio_zero_brute_force_tiny():
     rng = np.random.default_rng(4)
     for trial in range(200):

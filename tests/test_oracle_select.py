@@ -225,7 +225,7 @@ def test_full_budget_step_equals_dense_attention():
     import torch
     from paper_2606_06453_b200.workloads import SPECS, make_workload
     from dataclasses import replace
-    from tests.oracle_io import oracle_step, to_oracle
+    from oracle.workload_io import oracle_step, to_oracle
     spec = replace(SPECS["C1"], budget=64)
     w = make_workload(spec)
     r = oracle_step(w)

@@ -11,7 +11,7 @@ import torch
 import torch.distributed as dist
 import torch.multiprocessing as mp
 
-from tests.oracle_io import oracle_step
+from oracle.workload_io import oracle_step
 
 
 def shard_requests(batch, rank, world):
