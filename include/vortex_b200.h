@@ -127,6 +127,17 @@ const char *vx_last_error(const vx_ctx *ctx);
 /* Number of kernel launches the last compute call on this context enqueued (host counter). */
 int32_t vx_last_launch_count(const vx_ctx *ctx);
 
+/* Context options (host side, persistent until changed).  VX_ERR_INVALID_ARG for an unknown option or value.
+ *  VX_OPT_MLA_STEP   how vx_sparse_decode_step schedules the MLA geometry:
+ *      VX_MLA_STEP_AUTO     (default) the faster of the two for the batch at hand
+ *      VX_MLA_STEP_FUSED    one kernel: a thread-block cluster per request runs score -> select -> decode -> merge
+ *                           (falls back to CHAINED when the request / budget sizes exceed what it keeps on chip)
+ *      VX_MLA_STEP_CHAINED  three kernels chained by programmatic dependent launch (score, select, decode)
+ *    Both schedules compute the same selection bit for bit; outputs agree to rounding (different split sizes). */
+enum { VX_OPT_MLA_STEP = 1 };
+enum { VX_MLA_STEP_AUTO = 0, VX_MLA_STEP_FUSED = 1, VX_MLA_STEP_CHAINED = 2 };
+vx_status vx_set_option(vx_ctx *ctx, int32_t option, int32_t value);
+
 /* ---- (a1) summaries: PAPER.md:546 envelope, :89 query-independent, :529 per block ---- */
 /* For request i, rebuilds from the K pool the summary of every logical page
  * j >= first_new_pos[i] / page_size (first_new_pos == NULL: only the last page, i.e. the page

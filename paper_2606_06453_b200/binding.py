@@ -21,11 +21,13 @@ VX_SUMMARY_ENVELOPE, VX_SUMMARY_CENTROID = 0, 1
 VX_STEP_UPDATE_SUMMARY = 1
 VX_STEP_APPROX_TOPK = 2
 VX_TRACE_SCORE, VX_TRACE_TOPK, VX_TRACE_DECODE = 1, 2, 4
+VX_OPT_MLA_STEP = 1
+VX_MLA_STEP_AUTO, VX_MLA_STEP_FUSED, VX_MLA_STEP_CHAINED = 0, 1, 2
 
 EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",
            "vx_page_summary_update", "vx_page_score", "vx_topk_pages", "vx_sparse_paged_decode",
            "vx_sparse_decode_step", "vx_sparse_decode_step_host", "vx_trace_attach",
-           "vx_topk_pages_approx", "vx_set_topk_approx", "vx_union_pages"]
+           "vx_topk_pages_approx", "vx_set_topk_approx", "vx_union_pages", "vx_set_option"]
 
 
 class VxGeom(C.Structure):
@@ -79,6 +81,7 @@ def load_library():
         "vx_topk_pages": (I32, [P, P, T, P, I32, P, P, P, P]),
         "vx_topk_pages_approx": (I32, [P, P, T, P, I32, C.c_float, C.c_uint64, P, P, P, P]),
         "vx_set_topk_approx": (I32, [P, C.c_float, C.c_uint64]),
+        "vx_set_option": (I32, [P, I32, I32]),
         "vx_union_pages": (I32, [P, T, P, P, I32, I32, P, P, P, P]),
         "vx_sparse_paged_decode": (I32, [P, P, K, T, P, P, P, I32, P, P, P]),
         "vx_sparse_decode_step": (I32, [P, P, K, P, T, P, I32, U32, P, P, P, P, P, P]),
@@ -197,6 +200,9 @@ class Context:
         self._check(self.lib.vx_union_pages(self._h, C.byref(pt.c), _ptr(sel_logical), _ptr(sel_count), max_budget,
                                             max_union, _ptr(union_phys), _ptr(union_logical), _ptr(union_count),
                                             _stream(stream)))
+
+    def set_option(self, option, value):
+        self._check(self.lib.vx_set_option(self._h, int(option), int(value)))
 
     def set_topk_approx(self, tolerate_ratio, seed):
         self._check(self.lib.vx_set_topk_approx(self._h, float(tolerate_ratio), int(seed)))

@@ -174,6 +174,7 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->ws = carve_workspace(*g, workspace, max_batch, max_total_pages, max_budget);
   c->launches = 0;
   c->err[0] = 0;
+  c->mla_step = VX_MLA_STEP_AUTO;
   // split-arrival counters start at zero and every step leaves them at zero
   e = cudaMemset(c->ws.unit_counter, 0, (size_t)(max_batch > 0 ? max_batch : 1) * g->num_kv_heads * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
@@ -204,6 +205,7 @@ vx_status vx_trace_attach(vx_ctx* c, void* buffer, int32_t max_ctas, int32_t ker
   if (e == cudaSuccess) e = vx_trace_set_topk((kernels & VX_TRACE_TOPK) ? b : nullptr, n);
   if (e == cudaSuccess) e = vx_trace_set_decode_gqa((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
   if (e == cudaSuccess) e = vx_trace_set_decode_mla((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
+  if (e == cudaSuccess) e = vx_trace_set_step_mla((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
   return check_cuda(c, e, "vx_trace_attach");
 }
 
@@ -269,6 +271,15 @@ vx_status vx_set_topk_approx(vx_ctx* c, float tolerate_ratio, uint64_t seed) {
   c->approx.tolerate_ratio = tolerate_ratio;
   c->approx.seed = seed;
   return VX_OK;
+}
+
+vx_status vx_set_option(vx_ctx* c, int32_t option, int32_t value) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  if (option == VX_OPT_MLA_STEP && value >= VX_MLA_STEP_AUTO && value <= VX_MLA_STEP_CHAINED) {
+    c->mla_step = value;
+    return VX_OK;
+  }
+  return fail(c, VX_ERR_INVALID_ARG, "unknown option %d / value %d", option, value);
 }
 
 vx_status vx_union_pages(vx_ctx* c, const vx_page_table* pt, const int32_t* sel_logical, const int32_t* sel_count,
@@ -341,6 +352,13 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   // (a1) With n_local >= 1 the newest page is a forced page: its score never decides the selection and its keys
   // are staged by the decode kernel anyway, so the decode kernel rebuilds its summary (same result, no extra
   // launch, no extra HBM bytes).  Otherwise the summary kernel runs first.
+  // MLA: the whole step of a request runs in one kernel on the cluster that owns it (vx_decode_mla.cu, FUSED)
+  // MLA, small batches: the whole step of a request runs in one kernel on the cluster that owns it (vx_step_mla.cu)
+  if (c->g.kv_shared && !(flags & VX_STEP_APPROX_TOPK) && c->mla_step != VX_MLA_STEP_CHAINED &&
+      step_mla_fused_applies(c, *pt, *pool, max_budget) && (c->mla_step == VX_MLA_STEP_FUSED || step_mla_fused_pays(c, *pt)))
+    return check_cuda(c, launch_step_mla_fused(c, q, *pool, summary, *pt, budget, max_budget,
+                                               (flags & VX_STEP_UPDATE_SUMMARY) != 0, sp, sl, sc, out, lse, s),
+                      "fused MLA step");
   DecodeOpts opt;
   opt.pdl = true;                                // the kernels of a step are chained by programmatic dependent launch
   opt.budget = budget;

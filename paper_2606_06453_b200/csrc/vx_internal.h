@@ -51,6 +51,7 @@ struct vx_ctx {
   vx::Workspace ws;
   int32_t launches;              // kernels enqueued by the last compute call
   vx::ApproxPlan approx;         // vx_set_topk_approx: used by a fused step with VX_STEP_APPROX_TOPK
+  int32_t mla_step;              // VX_OPT_MLA_STEP
   char err[512];
 };
 
@@ -128,6 +129,7 @@ cudaError_t vx_trace_set_score(long long* buf, int ctas);
 cudaError_t vx_trace_set_topk(long long* buf, int ctas);
 cudaError_t vx_trace_set_decode_gqa(long long* buf, int ctas);
 cudaError_t vx_trace_set_decode_mla(long long* buf, int ctas);
+cudaError_t vx_trace_set_step_mla(long long* buf, int ctas);
 int decode_gqa_splits(const vx_ctx* c, int n_req, int max_budget);
 int decode_mla_splits(const vx_ctx* c, int n_req, int max_budget);
 
@@ -182,6 +184,13 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
                                  const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
                                  cudaStream_t s, const DecodeOpts& opt = DecodeOpts());
 bool mla_tc_supported(const vx_geom& g);
+// the whole step of a request (score -> select -> decode -> merge) in one kernel on the cluster that owns it
+bool step_mla_fused_applies(const vx_ctx* c, const vx_page_table& pt, const vx_kv_pool& pool, int32_t max_budget);   // it can run
+bool step_mla_fused_pays(const vx_ctx* c, const vx_page_table& pt);                                                  // ... and is the faster schedule
+cudaError_t launch_step_mla_fused(vx_ctx* c, const void* q, const vx_kv_pool& pool, const void* summary,
+                                  const vx_page_table& pt, const int32_t* budget, int32_t max_budget, bool update_summary,
+                                  int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count, void* out, float* lse,
+                                  cudaStream_t s);
 cudaError_t launch_combine(vx_ctx* c, int32_t batch, int num_splits, void* out, float* lse,
                            cudaStream_t s);
 

@@ -23,18 +23,12 @@
 
 #include "vx_common.cuh"
 #include "vx_internal.h"
+#include "vx_select.cuh"
 
 namespace vx {
 
 constexpr int kTopkSmemKeys = 48 * 1024;        // keys cached in shared memory (192 KB); more -> re-read scores
-constexpr int kBins = 2048;                     // 11 bits per pass
-constexpr int kBinBits = 11;
-constexpr int kList = 256;                      // threshold-bin members ranked directly
-constexpr uint32_t kForcedKey = 0xFFFFFFFFu;    // not the key of any finite float
 
-__device__ __forceinline__ bool page_forced(int j, int n_pages, int n_sink, int n_local) {
-  return (j < n_sink) || (j >= n_pages - n_local);
-}
 __device__ __forceinline__ uint32_t page_key(const float* __restrict__ sc, int j, int n_pages, int n_sink,
                                              int n_local) {
   return page_forced(j, n_pages, n_sink, n_local) ? kForcedKey : float_to_key(sc[j]);
@@ -80,7 +74,42 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
 
   const float* sc = scores + (int64_t)kvh * total_pages + row0;
   const bool cached = n_pages <= smem_keys;
-  // ---- keys, and the min / max key of the non-forced pages ------------------------------------
+  if (cached && n_sel <= kBins) {
+    // the usual case: the request's keys fit shared memory -> the CTA-wide selection of vx_select.cuh (the same
+    // device function the fused MLA step kernel runs), then the page-table gather as one parallel pass
+    __shared__ SelectScratch scratch;
+    for (int j0 = tid; j0 < n_pages; j0 += 8 * THREADS) {        // 8 independent loads in flight per thread
+      float v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) v[u] = j0 + u * THREADS < n_pages ? sc[j0 + u * THREADS] : 0.f;
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        if (j0 + u * THREADS < n_pages) s_keys[j0 + u * THREADS] = __float_as_uint(v[u]);
+    }
+    __syncthreads();
+    cta_select_pages<THREADS>(scratch, s_keys, n_pages, k, n_sink, n_local);
+    pdl_trigger();
+    const int per_split = (n_sel + pf.splits - 1) / pf.splits;
+    for (int r = tid; r < n_sel; r += THREADS) {
+      const int j = scratch.hist[r];
+      const int phys = page_indices[row0 + j];
+      sel_phys[out0 + r] = phys;
+      if (sel_logical) sel_logical[out0 + r] = j;
+      // the decode kernel starts every split at its first pages: pull those into L2 while HBM is idle
+      if (pf.k != nullptr && r % per_split < pf.pages_per_split) {
+        const int64_t off = (int64_t)phys * pf.page_bytes + (int64_t)kvh * pf.head_bytes;
+        l2_prefetch(static_cast<const uint8_t*>(pf.k) + off, pf.chunk_bytes);
+        if (pf.v != nullptr) l2_prefetch(static_cast<const uint8_t*>(pf.v) + off, pf.chunk_bytes);
+      }
+    }
+    for (int r = n_sel + tid; r < max_budget; r += THREADS) {
+      sel_phys[out0 + r] = -1;
+      if (sel_logical) sel_logical[out0 + r] = -1;
+    }
+    return;
+  }
+  // ---- requests beyond the shared-memory key cache, or budgets beyond the staging area: the general form -------
+  // keys, and the min / max key of the non-forced pages
   uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
   for (int j0 = tid; j0 < n_pages; j0 += 8 * THREADS) {          // 8 independent loads in flight per thread
     float v[8];

@@ -16,19 +16,9 @@
 
 #include "vx_common.cuh"
 #include "vx_internal.h"
+#include "vx_select.cuh"
 
 namespace vx {
-
-namespace {
-constexpr int kBins = 2048;                     // 11 bits per pass (as vx_topk.cu)
-constexpr int kBinBits = 11;
-constexpr int kList = 256;                      // threshold-bin members ranked directly
-constexpr uint32_t kForcedKey = 0xFFFFFFFFu;    // not the key of any finite float
-
-__device__ __forceinline__ bool page_forced(int j, int n_pages, int n_sink, int n_local) {
-  return (j < n_sink) || (j >= n_pages - n_local);
-}
-}  // namespace
 
 template <int THREADS, int kKpt>
 __global__ void __launch_bounds__(THREADS)

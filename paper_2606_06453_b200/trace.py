@@ -31,6 +31,12 @@ SLOTS = {
                    4: "prod: page 0 issued", 5: "QK: page 0 landed", 6: "QK: last page landed",
                    7: "PV: last issued", 8: "epilogue stored", 9: "cluster barrier passed", 10: "merge done",
                    11: "exit"},
+    # the fused MLA step (decode_mla_kernel<FUSED>): `--kernel decode --mode step` on an MLA config
+    "step_mla": {0: "entry", 1: "barriers + TMEM ready", 12: "prod: first summary rows issued",
+                 13: "cons: first summary stage landed", 14: "scores complete (cluster barrier passed)",
+                 2: "selection done", 3: "block table written, decode barriers ready", 4: "prod: page 0 issued",
+                 5: "QK: page 0 landed", 6: "QK: last page landed", 7: "PV: last issued", 8: "epilogue stored",
+                 9: "cluster barrier passed", 10: "merge done", 11: "exit"},
 }
 
 
@@ -72,6 +78,8 @@ def main():
              "decode": lambda: ctx.sparse_paged_decode(w.q, pool, pt, sp, sl, sc, w.max_budget, out, lse)}[args.kernel]
     kind = {"score": binding.VX_TRACE_SCORE, "topk": binding.VX_TRACE_TOPK, "decode": binding.VX_TRACE_DECODE}[args.kernel]
     names = SLOTS[args.kernel if args.kernel != "decode" else ("decode_mla" if s.kv_shared else "decode_gqa")]
+    if args.kernel == "decode" and args.mode == "step" and s.kv_shared:
+        names = SLOTS["step_mla"]
     buf = torch.zeros(8192, 16, dtype=torch.int64, device=dev)
     ctx.trace_attach(buf, kind)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
@@ -93,8 +101,35 @@ def main():
             if not ok.any():
                 continue
             v = (col[ok] - t0) / 1e3
-            print(f"{n:38s} n {ok.sum():4d}  min {v.min():6.1f}  p10 {np.percentile(v, 10):6.1f}  med {np.median(v):6.1f}"
+            print(f"{n:44s} n {ok.sum():4d}  min {v.min():6.1f}  p10 {np.percentile(v, 10):6.1f}  med {np.median(v):6.1f}"
                   f"  p90 {np.percentile(v, 90):6.1f}  max {v.max():6.1f}")
+        keys = [k for k in names if (b[:, k] > 0).all()]
+        print("    per-CTA durations between consecutive stamps:")
+        for k0, k1 in zip(keys[:-1], keys[1:]):
+            d = (b[:, k1] - b[:, k0]) / 1e3
+            print(f"    {names[k0][:30]:30s} -> {names[k1][:30]:30s} min {d.min():6.1f}  med {np.median(d):6.1f}  max {d.max():6.1f}")
+        if names is SLOTS["step_mla"]:
+            # aggregate HBM rate over time, assuming every CTA streams its summary share evenly between stamps 13 and 14
+            # and its pages evenly between stamps 4 and 6 (grid = (splits, 1, batch): CTA index = request * splits + split)
+            splits = len(b) // B
+            Pn = ((w.seq_lens.cpu().numpy() + s.page_size - 1) // s.page_size)
+            kk = np.minimum(w.budget.cpu().numpy(), Pn)
+            edges = np.arange(0.0, (b[:, last].max() - t0) / 1e3 + 2.0, 2.0)
+            rate = np.zeros(len(edges) - 1)
+            row_bytes = 2 * s.qk_dim * 2
+            for c in range(len(b)):
+                req, sp_ = c // splits, c % splits
+                rows = Pn[req] * (sp_ + 1) // splits - Pn[req] * sp_ // splits
+                per = -(-kk[req] // splits)
+                pages = max(0, min(kk[req], (sp_ + 1) * per) - min(kk[req], sp_ * per))
+                for (k0, k1, nbytes) in ((12, 14, rows * row_bytes), (4, 6, pages * s.page_size * s.qk_dim * 2)):
+                    a, e = (b[c, k0] - t0) / 1e3, (b[c, k1] - t0) / 1e3
+                    if e <= a:
+                        continue
+                    lo, hi = np.maximum(edges[:-1], a), np.minimum(edges[1:], e)
+                    rate += np.clip(hi - lo, 0, None) / (e - a) * nbytes
+            print("    aggregate stream rate, TB/s per 2 us bin (summary rows between stamps 12-14, pages between 4-6):")
+            print("    " + " ".join(f"{x / 2e-6 / 1e12:4.1f}" for x in rate))
     ctx.trace_attach(None, 0)
 
 

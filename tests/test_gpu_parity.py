@@ -176,7 +176,7 @@ def test_fused_step_matches_oracle(name, flags):
     ctx.sparse_decode_step(w.q, pool, summary, pt, w.budget, w.max_budget, o["out"], o["lse"], o["sel_phys"],
                            o["sel_logical"], o["sel_count"], flags=flags)
     torch.cuda.synchronize()
-    assert ctx.last_launch_count >= 3
+    assert ctx.last_launch_count >= (1 if w.spec.kv_shared else 3)     # MLA, small batch: one fused kernel; else score, select, decode
     ref = oracle_step(w)
     sl, sc = o["sel_logical"].cpu().numpy(), o["sel_count"].cpu().numpy()
     check_selection(w, sl, o["sel_phys"].cpu().numpy(), sc, ref)
