@@ -133,9 +133,14 @@ int32_t vx_last_launch_count(const vx_ctx *ctx);
  *      VX_MLA_STEP_FUSED    one kernel: a thread-block cluster per request runs score -> select -> decode -> merge
  *                           (falls back to CHAINED when the request / budget sizes exceed what it keeps on chip)
  *      VX_MLA_STEP_CHAINED  three kernels chained by programmatic dependent launch (score, select, decode)
- *    Both schedules compute the same selection bit for bit; outputs agree to rounding (different split sizes). */
-enum { VX_OPT_MLA_STEP = 1 };
-enum { VX_MLA_STEP_AUTO = 0, VX_MLA_STEP_FUSED = 1, VX_MLA_STEP_CHAINED = 2 };
+ *      VX_MLA_STEP_FLAT     one persistent kernel for the whole batch: the summary stream cut flat over the SMs, a
+ *                           selection warpgroup per request running beside the stream, decode shares taken from a
+ *                           counter (falls back to CHAINED for batches / requests beyond what it keeps on chip)
+ *    All schedules compute the same selection bit for bit; outputs agree to rounding (different split sizes).
+ *  VX_OPT_MLA_FLAT_SPLITS / VX_OPT_MLA_FLAT_WAVES   0 (default) = chosen by the library; > 0 = decode shares per request /
+ *                           interleaved waves of the summary stream of the FLAT schedule (tuning knobs) */
+enum { VX_OPT_MLA_STEP = 1, VX_OPT_MLA_FLAT_SPLITS = 2, VX_OPT_MLA_FLAT_WAVES = 3 };
+enum { VX_MLA_STEP_AUTO = 0, VX_MLA_STEP_FUSED = 1, VX_MLA_STEP_CHAINED = 2, VX_MLA_STEP_FLAT = 3 };
 vx_status vx_set_option(vx_ctx *ctx, int32_t option, int32_t value);
 
 /* ---- (a1) summaries: PAPER.md:546 envelope, :89 query-independent, :529 per block ---- */

@@ -21,8 +21,8 @@ VX_SUMMARY_ENVELOPE, VX_SUMMARY_CENTROID = 0, 1
 VX_STEP_UPDATE_SUMMARY = 1
 VX_STEP_APPROX_TOPK = 2
 VX_TRACE_SCORE, VX_TRACE_TOPK, VX_TRACE_DECODE = 1, 2, 4
-VX_OPT_MLA_STEP = 1
-VX_MLA_STEP_AUTO, VX_MLA_STEP_FUSED, VX_MLA_STEP_CHAINED = 0, 1, 2
+VX_OPT_MLA_STEP, VX_OPT_MLA_FLAT_SPLITS, VX_OPT_MLA_FLAT_WAVES = 1, 2, 3
+VX_MLA_STEP_AUTO, VX_MLA_STEP_FUSED, VX_MLA_STEP_CHAINED, VX_MLA_STEP_FLAT = 0, 1, 2, 3
 
 EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",
            "vx_page_summary_update", "vx_page_score", "vx_topk_pages", "vx_sparse_paged_decode",

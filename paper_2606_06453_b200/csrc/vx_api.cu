@@ -42,6 +42,9 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   w.h_budget = static_cast<int32_t*>(take(B * 4));
   w.h_out = take(B * Hq * (size_t)g.v_dim * esz);
   w.h_lse = static_cast<float*>(take(B * Hq * 4));
+  const bool mla = g.kv_shared != 0;
+  w.flat_qvec = static_cast<float*>(take(mla ? step_mla_flat_qvec_floats(max_batch) * 4 : 0));
+  w.flat_sync = static_cast<int32_t*>(take(mla ? step_mla_flat_workspace_ints(max_batch) * 4 : 0));
   w.bytes = off;
   return w;
 }
@@ -175,8 +178,10 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->launches = 0;
   c->err[0] = 0;
   c->mla_step = VX_MLA_STEP_AUTO;
+  c->flat_splits = c->flat_waves = 0;
   // split-arrival counters start at zero and every step leaves them at zero
   e = cudaMemset(c->ws.unit_counter, 0, (size_t)(max_batch > 0 ? max_batch : 1) * g->num_kv_heads * 4);
+  if (e == cudaSuccess && g->kv_shared) e = cudaMemset(c->ws.flat_sync, 0, step_mla_flat_workspace_ints(max_batch) * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (e != cudaSuccess) {
     delete c;
@@ -206,6 +211,7 @@ vx_status vx_trace_attach(vx_ctx* c, void* buffer, int32_t max_ctas, int32_t ker
   if (e == cudaSuccess) e = vx_trace_set_decode_gqa((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
   if (e == cudaSuccess) e = vx_trace_set_decode_mla((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
   if (e == cudaSuccess) e = vx_trace_set_step_mla((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
+  if (e == cudaSuccess) e = vx_trace_set_step_mla_flat((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
   return check_cuda(c, e, "vx_trace_attach");
 }
 
@@ -275,10 +281,12 @@ vx_status vx_set_topk_approx(vx_ctx* c, float tolerate_ratio, uint64_t seed) {
 
 vx_status vx_set_option(vx_ctx* c, int32_t option, int32_t value) {
   if (!c) return VX_ERR_INVALID_ARG;
-  if (option == VX_OPT_MLA_STEP && value >= VX_MLA_STEP_AUTO && value <= VX_MLA_STEP_CHAINED) {
+  if (option == VX_OPT_MLA_STEP && value >= VX_MLA_STEP_AUTO && value <= VX_MLA_STEP_FLAT) {
     c->mla_step = value;
     return VX_OK;
   }
+  if (option == VX_OPT_MLA_FLAT_SPLITS && value >= 0 && value <= kMaxSplits) { c->flat_splits = value; return VX_OK; }
+  if (option == VX_OPT_MLA_FLAT_WAVES && value >= 0 && value <= 8) { c->flat_waves = value; return VX_OK; }
   return fail(c, VX_ERR_INVALID_ARG, "unknown option %d / value %d", option, value);
 }
 
@@ -354,7 +362,12 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   // launch, no extra HBM bytes).  Otherwise the summary kernel runs first.
   // MLA: the whole step of a request runs in one kernel on the cluster that owns it (vx_decode_mla.cu, FUSED)
   // MLA, small batches: the whole step of a request runs in one kernel on the cluster that owns it (vx_step_mla.cu)
-  if (c->g.kv_shared && !(flags & VX_STEP_APPROX_TOPK) && c->mla_step != VX_MLA_STEP_CHAINED &&
+  if (c->g.kv_shared && !(flags & VX_STEP_APPROX_TOPK) && c->mla_step == VX_MLA_STEP_FLAT &&
+      step_mla_flat_applies(c, *pt, *pool, max_budget))
+    return check_cuda(c, launch_step_mla_flat(c, q, *pool, summary, *pt, budget, max_budget,
+                                              (flags & VX_STEP_UPDATE_SUMMARY) != 0, sp, sl, sc, out, lse, s),
+                      "flat MLA step");
+  if (c->g.kv_shared && !(flags & VX_STEP_APPROX_TOPK) && c->mla_step != VX_MLA_STEP_CHAINED && c->mla_step != VX_MLA_STEP_FLAT &&
       step_mla_fused_applies(c, *pt, *pool, max_budget) && (c->mla_step == VX_MLA_STEP_FUSED || step_mla_fused_pays(c, *pt)))
     return check_cuda(c, launch_step_mla_fused(c, q, *pool, summary, *pt, budget, max_budget,
                                                (flags & VX_STEP_UPDATE_SUMMARY) != 0, sp, sl, sc, out, lse, s),

@@ -26,6 +26,9 @@ struct Workspace {               // device pointers carved from the caller's wor
   int32_t* h_budget;             // [max_batch]
   void* h_out;                   // [max_batch, Hq, v_dim] elements
   float* h_lse;                  // [max_batch, Hq]
+  // the flat MLA step kernel (vx_step_mla_flat.cu)
+  float* flat_qvec;              // [max_batch, 2 qk_dim] query vectors [Qm | Qp]
+  int32_t* flat_sync;            // counters and per-request flags; zero between steps
   size_t bytes;                  // total
 };
 
@@ -52,6 +55,7 @@ struct vx_ctx {
   int32_t launches;              // kernels enqueued by the last compute call
   vx::ApproxPlan approx;         // vx_set_topk_approx: used by a fused step with VX_STEP_APPROX_TOPK
   int32_t mla_step;              // VX_OPT_MLA_STEP
+  int32_t flat_splits, flat_waves;   // VX_OPT_MLA_FLAT_*: 0 = the library's choice
   char err[512];
 };
 
@@ -191,6 +195,15 @@ cudaError_t launch_step_mla_fused(vx_ctx* c, const void* q, const vx_kv_pool& po
                                   const vx_page_table& pt, const int32_t* budget, int32_t max_budget, bool update_summary,
                                   int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count, void* out, float* lse,
                                   cudaStream_t s);
+// the whole step of the batch in one persistent kernel (flat summary stream, selection warpgroups, decode items from a counter)
+bool step_mla_flat_applies(const vx_ctx* c, const vx_page_table& pt, const vx_kv_pool& pool, int32_t max_budget);
+size_t step_mla_flat_workspace_ints(int max_batch);
+size_t step_mla_flat_qvec_floats(int max_batch);
+cudaError_t launch_step_mla_flat(vx_ctx* c, const void* q, const vx_kv_pool& pool, const void* summary,
+                                 const vx_page_table& pt, const int32_t* budget, int32_t max_budget, bool update_summary,
+                                 int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count, void* out, float* lse,
+                                 cudaStream_t s);
+cudaError_t vx_trace_set_step_mla_flat(long long* buf, int ctas);
 cudaError_t launch_combine(vx_ctx* c, int32_t batch, int num_splits, void* out, float* lse,
                            cudaStream_t s);
 

@@ -36,18 +36,25 @@ struct SelectScratch {                          // ~10 KB of shared memory
 // keys[0 .. n_pages): on entry the BIT PATTERNS of the fp32 scores of logical pages 0 .. n_pages-1, on return their
 // order-preserving keys (forced pages: kForcedKey).  k = the budget including forced pages (>= 0).
 // Returns n_sel = min(k, n_pages) and leaves the selected logical pages in sc.hist[0 .. n_sel), ascending.
-// Requires n_sel <= kBins.  Every one of the CTA's THREADS threads calls it (it synchronises the block); the caller
-// has synchronised after writing keys[].
-template <int THREADS>
+// Requires n_sel <= kBins.  Every one of the THREADS threads of the selecting group calls it (it synchronises the group);
+// the caller has synchronised after writing keys[].  The group is the whole CTA (BAR = 0: __syncthreads) or the THREADS
+// consecutive threads starting at thread TID0, which synchronise on the named barrier BAR while the rest of the CTA does
+// something else (the flat MLA step kernel selects on one warpgroup while the other warps stream summaries).
+template <int THREADS, int BAR>
+__device__ __forceinline__ void select_sync() {
+  if constexpr (BAR == 0) __syncthreads();
+  else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(THREADS) : "memory");
+}
+template <int THREADS, int BAR = 0, int TID0 = 0>
 __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, int k, int n_sink, int n_local) {
   constexpr int WARPS = THREADS / kWarp;
   constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
-  static_assert(kBins % THREADS == 0 && THREADS >= kList && WARPS <= 32, "shape");
-  const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
+  static_assert(kBins % THREADS == 0 && WARPS <= 32, "shape");
+  const int tid = (int)threadIdx.x - TID0, lane = tid % kWarp, warp = tid / kWarp;
   const int n_sel = min(k, n_pages);
   if (k >= n_pages) {                           // G6: the budget covers the request -> every page
     for (int r = tid; r < n_pages; r += THREADS) sc.hist[r] = r;
-    __syncthreads();
+    select_sync<THREADS, BAR>();
     return n_sel;
   }
 
@@ -62,7 +69,7 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
   kmin = __reduce_min_sync(0xffffffffu, kmin);
   kmax = __reduce_max_sync(0xffffffffu, kmax);
   if (lane == 0) { sc.wmin[warp] = kmin; sc.wmax[warp] = kmax; }
-  __syncthreads();
+  select_sync<THREADS, BAR>();
 #pragma unroll
   for (int w = 0; w < WARPS; ++w) { kmin = min(kmin, sc.wmin[w]); kmax = max(kmax, sc.wmax[w]); }
 
@@ -88,13 +95,13 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
 #pragma unroll 1
     while (true) {
       for (int b = tid; b < kBins; b += THREADS) sc.hist[b] = 0;
-      __syncthreads();
+      select_sync<THREADS, BAR>();
       for (int j = tid; j < n_pages; j += THREADS) {
         const uint32_t key = keys[j];
         if (key != kForcedKey && key >= lo && (uint64_t)(key - lo) < width)
           atomicAdd(&sc.hist[fpass ? fbin(key) : (int)((key - lo) >> shift)], 1);
       }
-      __syncthreads();
+      select_sync<THREADS, BAR>();
       // threshold bin: the highest b with  #keys in bins > b  <  need  <=  #keys in bins >= b
       int h[BPT], mine = 0;
 #pragma unroll
@@ -106,7 +113,7 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
         if (lane + o < kWarp) inc += a;
       }
       if (lane == 0) sc.wsum[warp] = inc;
-      __syncthreads();
+      select_sync<THREADS, BAR>();
       int run = inc - mine;                     // keys in bins owned by higher threads
 #pragma unroll
       for (int w = 0; w < WARPS; ++w) run += (w > warp) ? sc.wsum[w] : 0;
@@ -116,7 +123,7 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
         run += h[e];
       }
       if (tid == 0) { sc.nlist = 0; sc.bmin = 0xFFFFFFFFu; sc.bmax = 0u; }
-      __syncthreads();
+      select_sync<THREADS, BAR>();
       const int bin = sc.bin, cnt = sc.cnt;
       need -= sc.above;                         // still to take from the threshold bin
       const uint32_t bin_lo = lo + ((uint32_t)bin << shift);
@@ -136,10 +143,10 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
           else if (fpass) { atomicMin(&sc.bmin, key); atomicMax(&sc.bmax, key); }
         }
       }
-      __syncthreads();
+      select_sync<THREADS, BAR>();
       if (cnt <= kList) {
-        if (tid < cnt) {
-          const uint32_t mykey = sc.list[tid];
+        for (int t = tid; t < cnt; t += THREADS) {
+          const uint32_t mykey = sc.list[t];
           int gt = 0, ge = 0;
           for (int j = 0; j < cnt; ++j) {
             const uint32_t o = sc.list[j];
@@ -148,7 +155,7 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
           }
           if (gt < need && need <= ge) { sc.thr = mykey; sc.need_eq = need - gt; }   // same values from every tie
         }
-        __syncthreads();
+        select_sync<THREADS, BAR>();
         thr = sc.thr;
         need_eq = sc.need_eq;
         break;
@@ -163,7 +170,7 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
         lo = bin_lo;
         shift = max(0, shift - kBinBits);
       }
-      __syncthreads();                          // bmin / bmax / bin are read before the next pass rewrites them
+      select_sync<THREADS, BAR>();                          // bmin / bmax / bin are read before the next pass rewrites them
     }
   }
 
@@ -181,7 +188,7 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
     n_tie += __popc(__ballot_sync(0xffffffffu, tie));
   }
   if (lane == 0) sc.wcnt[warp] = make_int2(n_sure, n_tie);
-  __syncthreads();
+  select_sync<THREADS, BAR>();
   int gt = 0, eq = 0;                           // sure / tie pages before this warp's run
 #pragma unroll
   for (int w = 0; w < WARPS; ++w) {
@@ -203,7 +210,7 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
     gt += __popc(b_sure);
     eq += __popc(b_tie);
   }
-  __syncthreads();
+  select_sync<THREADS, BAR>();
   return n_sel;
 }
 

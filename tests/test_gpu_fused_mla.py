@@ -18,14 +18,17 @@ from tests.parity import check_attention, check_selection, oracle_attention_on
 pytestmark = pytest.mark.gpu
 
 
-def run_fused(spec, flags=None):
+SCHEDULES = ["fused", "flat"]
+
+
+def run_fused(spec, flags=None, schedule="fused"):
     import paper_2606_06453_b200 as vx
     from paper_2606_06453_b200.workloads import make_workload
     w = make_workload(spec, device="cuda:0")
     s = w.spec
     dev = w.q.device
     ctx = vx.context_for(w)
-    ctx.set_option(vx.VX_OPT_MLA_STEP, vx.VX_MLA_STEP_FUSED)      # (AUTO takes it for batches of up to 8 requests only)
+    ctx.set_option(vx.VX_OPT_MLA_STEP, vx.VX_MLA_STEP_FLAT if schedule == "flat" else vx.VX_MLA_STEP_FUSED)
     pool, pt = vx.tables_for(w)
     summary = vx.alloc_summary(w)
     ctx.page_summary_update(pool, pt, summary, first_new_pos=torch.zeros_like(w.seq_lens))
@@ -56,12 +59,13 @@ CASES = {
 }
 
 
+@pytest.mark.parametrize("schedule", SCHEDULES)
 @pytest.mark.parametrize("case", list(CASES))
-def test_fused_step_matches_oracle_and_the_separate_calls(case):
+def test_fused_step_matches_oracle_and_the_separate_calls(case, schedule):
     from paper_2606_06453_b200.workloads import SPECS
     batch, seq, budget = CASES[case]
     spec = replace(SPECS["C4"], name=case, batch=batch, seq_len=seq, budget=budget, cfg_id=40 + list(CASES).index(case))
-    vx, w, ctx, pool, pt, summary, clean, out, lse, sp, sl, sc, launches = run_fused(spec)
+    vx, w, ctx, pool, pt, summary, clean, out, lse, sp, sl, sc, launches = run_fused(spec, schedule=schedule)
     s = w.spec
     assert launches == 1, "the MLA step is one kernel"
     ref = oracle_step(w)
@@ -93,10 +97,11 @@ def test_fused_step_matches_oracle_and_the_separate_calls(case):
     ctx.close()
 
 
-def test_fused_step_without_summary_update_leaves_the_pool_alone():
+@pytest.mark.parametrize("schedule", SCHEDULES)
+def test_fused_step_without_summary_update_leaves_the_pool_alone(schedule):
     from paper_2606_06453_b200.workloads import SPECS
     spec = replace(SPECS["C4"], name="no-update", batch=9, seq_len=(100, 5000), budget=7, cfg_id=48)
-    vx, w, ctx, pool, pt, summary, clean, out, lse, sp, sl, sc, launches = run_fused(spec, flags=0)
+    vx, w, ctx, pool, pt, summary, clean, out, lse, sp, sl, sc, launches = run_fused(spec, flags=0, schedule=schedule)
     last = w.page_indices[(w.page_indptr[1:] - 1).long()].long()
     assert launches == 1 and bool((summary[last] == 0).all())          # poisoned rows stay as they were
     o_ref, l_ref = oracle_attention_on(w, sl.cpu().numpy(), sc.cpu().numpy())
@@ -104,7 +109,8 @@ def test_fused_step_without_summary_update_leaves_the_pool_alone():
     ctx.close()
 
 
-def test_fused_step_centroid_flow():
+@pytest.mark.parametrize("schedule", SCHEDULES)
+def test_fused_step_centroid_flow(schedule):
     """block top-k summaries (Eq.1-2) through the fused kernel: 1,152-byte rows, [Qsum] query vector"""
     import paper_2606_06453_b200 as vx
     from paper_2606_06453_b200.workloads import SPECS, make_workload
@@ -113,7 +119,7 @@ def test_fused_step_centroid_flow():
     s = w.spec
     kind = vx.binding.VX_SUMMARY_CENTROID
     ctx = vx.context_for(w, summary_kind=kind)
-    ctx.set_option(vx.VX_OPT_MLA_STEP, vx.VX_MLA_STEP_FUSED)
+    ctx.set_option(vx.VX_OPT_MLA_STEP, vx.VX_MLA_STEP_FLAT if schedule == "flat" else vx.VX_MLA_STEP_FUSED)
     pool, pt = vx.tables_for(w)
     summary = vx.alloc_summary(w, kind)
     ctx.page_summary_update(pool, pt, summary, first_new_pos=torch.zeros_like(w.seq_lens))
