@@ -2,7 +2,7 @@
 """bench.py -- times the fused sparse decode step (all hot-path rows a1..a5) on synthetic, seeded
 decode workloads shaped like BASELINE.json's configs, and prints ONE JSON line.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C2|C3|C4|C5|C1] [--impl reference]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C4|C3|C2|C5|C1] [--impl reference]
 
 metric : sparse decode step time in microseconds (lower is better), with the achieved HBM GB/s and
          the fraction of the bytes roofline (summary bytes + selected-KV bytes + Q/O bytes).
@@ -38,9 +38,14 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
-    ap.add_argument("--config", default="C2", help="workload: C1..C5 (default C2 = BASELINE.json configs[1])")
+    ap.add_argument("--config", default="C4", help="workload: C1..C5 (default C4, the MLA config the north star's >= 70 %% target "
+                    "names and the one furthest from it; C3 is the other target config)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--also", default="C3,C4", help="extra configs timed briefly and reported under 'also'")
+    ap.add_argument("--also", default="C3,C2,C5,C1", help="further configs, each a full record (step, stages, roofline, e2e, "
+                    "clocks) under 'also'")
+    ap.add_argument("--also-steps", type=int, default=50)
+    ap.add_argument("--mla-step", default="auto", choices=["auto", "chained", "fused", "flat"],
+                    help="schedule of the MLA step (VX_OPT_MLA_STEP); auto = the library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--summary", default="envelope", choices=["envelope", "centroid"],
                     help="page summary / score flow: Quest envelope (default, the north star) or block top-k centroid")
@@ -63,18 +68,19 @@ def measured_peak():
 
 
 def ncu_traffic(cfg, stage):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
-    `ncu --set full` capture (profiles/r1e_traffic.csv; commands in profiles/r1e_final.md; those kernels are unchanged in
-    snapshot r1f, profiles/r1f_final.md), or None."""
-    kernel = {"page_score": ("score_kernel",), "sparse_paged_decode": ("decode_gqa_mma_kernel", "decode_mla_kernel")}[stage]
-    path = os.path.join(ROOT, "profiles", "r1e_traffic.csv")
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, source) from the committed
+    `ncu --set full` captures of this round (profiles/r2_traffic.csv: one row per config and kernel, each naming the
+    raw export it was read from and the git revision of the library that was profiled), or (None, None)."""
+    kernels = {"page_score": ("score_kernel", "score_mla_max_kernel"),
+               "sparse_paged_decode": ("decode_gqa_mma_kernel", "decode_mla_kernel", "decode_generic_kernel")}[stage]
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
     if not os.path.exists(path):
-        return None
+        return None, None
     import csv
     for row in csv.DictReader(open(path)):
-        if row["config"] == cfg and row["kernel"] in kernel:
-            return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"])
-    return None
+        if row["config"] == cfg and row["kernel"] in kernels:
+            return int(row["dram_bytes_read"]) + int(row["dram_bytes_write"]), f"profiles/{row['source']} (library at {row['lib_rev']})"
+    return None, None
 
 
 def algorithmic_bytes(w, sel_count=None, summary="envelope"):
@@ -135,7 +141,7 @@ class ClockSampler(threading.Thread):
 class Runner:
     """One workload resident on one GPU: context, pools, summaries, outputs, L2 flush buffer."""
 
-    def __init__(self, cfg, device, seed_offset=0, summary="envelope", topk_approx=0.0, agg="sum"):
+    def __init__(self, cfg, device, seed_offset=0, summary="envelope", topk_approx=0.0, agg="sum", mla_step="auto"):
         import torch
         import paper_2606_06453_b200 as vx
         from paper_2606_06453_b200.workloads import make_workload
@@ -144,6 +150,9 @@ class Runner:
         kind = vx.binding.VX_SUMMARY_CENTROID if summary == "centroid" else vx.binding.VX_SUMMARY_ENVELOPE
         self.summary_name = summary
         self.ctx = vx.context_for(w, summary_kind=kind, agg=vx.binding.VX_AGG_MAX if agg == "max" else vx.binding.VX_AGG_SUM)
+        if w.spec.kv_shared:
+            self.ctx.set_option(vx.VX_OPT_MLA_STEP, {"auto": vx.VX_MLA_STEP_AUTO, "chained": vx.VX_MLA_STEP_CHAINED,
+                                                     "fused": vx.VX_MLA_STEP_FUSED, "flat": vx.VX_MLA_STEP_FLAT}[mla_step])
         self.tau = float(topk_approx)
         self.step_flags = vx.VX_STEP_UPDATE_SUMMARY | (vx.VX_STEP_APPROX_TOPK if self.tau > 0 else 0)
         self.ctx.set_topk_approx(self.tau, 20260604)
@@ -229,9 +238,10 @@ class Runner:
         return out
 
 
-def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None, summary="envelope", agg="sum"):
-    """Time the oracle (as it stands) on the first n_requests requests of the workload.
-    Returns (seconds for score + top-k + attention on the sample, requests in sample, batch, threads)."""
+def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None, summary="envelope", agg="sum", passes=3):
+    """Time the oracle (as it stands) on the first n_requests requests of the workload: one untimed warm-up pass, then
+    the MEDIAN of `passes` timed passes.  Returns (seconds for score + top-k + attention on the sample, requests in sample,
+    batch, threads)."""
     from oracle import vx_oracle as vo
     from paper_2606_06453_b200.workloads import make_workload, subproblem
     from oracle.workload_io import to_oracle
@@ -242,14 +252,19 @@ def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=No
     s = sub.spec
     build = vo.page_centroid if summary == "centroid" else vo.page_summary
     summ = build(pool, pt, s.num_kv_heads, s.qk_dim)                    # built outside the timed step
-    t0 = time.perf_counter()
-    vo.decode_step(q, pool, pt, vo.as_np(sub.budget), sub.max_budget, s.num_q_heads, s.num_kv_heads, s.qk_dim,
-                   s.v_dim, s.sm_scale, s.n_sink, s.n_local, agg=vo.AGG_MAX if agg == "max" else vo.AGG_SUM, summary=summ,
-                   kind=summary)
-    return time.perf_counter() - t0, n_requests, w.spec.batch, vo.num_threads()
+    times = []
+    for it in range(1 + passes):
+        t0 = time.perf_counter()
+        vo.decode_step(q, pool, pt, vo.as_np(sub.budget), sub.max_budget, s.num_q_heads, s.num_kv_heads, s.qk_dim,
+                       s.v_dim, s.sm_scale, s.n_sink, s.n_local, agg=vo.AGG_MAX if agg == "max" else vo.AGG_SUM, summary=summ,
+                       kind=summary)
+        if it > 0:
+            times.append(time.perf_counter() - t0)
+    return statistics.median(times), n_requests, w.spec.batch, vo.num_threads()
 
 
-SAMPLE_REQUESTS = {"C1": 1, "C2": 4, "C3": 1, "C4": 8, "C5": 8}
+SAMPLE_REQUESTS = {"C1": 1, "C2": 4, "C3": 1, "C4": 8, "C5": 8}     # cpu_baseline: requests per oracle pass
+PARITY_REQUESTS = {"C1": [0], "C2": [5, 27], "C3": [6], "C4": [7, 50], "C5": [33, 90]}   # post-timing sampled parity check
 
 
 def run_reference(args):
@@ -262,17 +277,16 @@ def run_reference(args):
     w = make_workload(args.config, device=_gen_device())     # inputs only; the oracle runs on the host cores
     times = []
     steps = max(1, min(args.steps, 3))
-    for it in range(min(args.warmup, 1) + steps):
-        t, n, batch, threads = oracle_sample_time(args.config, nreq, workload=w, summary=args.summary, agg=args.agg)
-        if it >= min(args.warmup, 1):
-            times.append(t)
+    for it in range(steps):
+        t, n, batch, threads = oracle_sample_time(args.config, nreq, workload=w, summary=args.summary, agg=args.agg, passes=1)
+        times.append(t)
     us = statistics.mean(times) / n * batch * 1e6        # scaled from the sample to the whole batch
     line = {"impl": "reference", "metric": METRIC, "value": us, "unit": "us", "n_gpus": args.gpus, "steps": steps,
-            "warmup": min(args.warmup, 1), "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
+            "warmup": 1, "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": args.config, "summary": args.summary, "l2": "n/a (CPU)"},
             "cpu_baseline": {"value": us, "unit": "us", "cores": threads, "kind": "oracle",
-                             "sample": f"{n} of {batch} requests per step, scaled by {batch}/{n}"},
+                             "sample": f"{n} of {batch} requests per step (one untimed warm-up pass before each), scaled by {batch}/{n}"},
             "e2e": {"value": us, "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -283,10 +297,109 @@ def _gen_device():
     return "cuda:0" if torch.cuda.is_available() else "cpu"
 
 
+def spawn_ranks(args):
+    """`python bench.py --gpus N` without torchrun in front: start the N ranks ourselves (one process per GPU)."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    os.execv(sys.executable, cmd)
+
+
+def measure(cfg, args, device, local, rank, world, steps, warmup, peak, peak_src, seed_offset):
+    """One full record for one workload: K device-timed fused steps (max over ranks), the end-to-end leg, and on rank 0
+    the per-stage times, the dominant kernel's roofline, the oracle beside it and a sampled parity check."""
+    import torch
+    import torch.distributed as dist
+    is_main = cfg == args.config
+    r = Runner(cfg, device, seed_offset=seed_offset, summary=args.summary if is_main else "envelope",
+               topk_approx=args.topk_approx, agg=args.agg if is_main else "sum", mla_step=args.mla_step)
+    summary_kind = args.summary if is_main else "envelope"
+    w, s = r.w, r.w.spec
+    bytes_ = algorithmic_bytes(w, summary=summary_kind)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x):
+        if world > 1:
+            t = torch.tensor([x], device=device, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            return float(t.item())
+        return x
+
+    # ---- the timed region: K fused steps, device-timed, max over ranks --------------------------
+    barrier()
+    sampler = ClockSampler(local)
+    sampler.start()
+    sampler.ready.wait(timeout=10)          # NVML is up and the first sample is in before the timed region
+    times = r.time_device(r.step, steps, warmup)
+    launches_per_step = r.ctx.last_launch_count
+    barrier()
+    clocks = sampler.result()
+    ms = max_over_ranks(statistics.mean(times))
+    # ---- end to end through the host-buffer entry point ------------------------------------------
+    e2e_ms = max_over_ranks(statistics.mean(r.time_host(r.step_host, min(steps, 30), 3)))
+    esz = 2 if s.dtype == "bf16" else 4
+    h2d = s.batch * s.num_q_heads * s.qk_dim * esz + 4 * (s.batch + 1 + w.total_pages + 2 * s.batch)
+    d2h = s.batch * s.num_q_heads * s.v_dim * esz + 4 * s.batch * s.num_q_heads
+    rec = None
+    if rank == 0:
+        # ---- per-stage times (each C-ABI call alone) and the dominant kernel's roofline -------------------
+        r.step()
+        stage = {}
+        for name, fn in (("summary_append", r.stage_summary), ("page_score", r.stage_score),
+                         ("topk_pages", r.stage_topk), ("sparse_paged_decode", r.stage_decode)):
+            stage[name] = statistics.mean(r.time_device(fn, min(steps, 30), 3)) * 1e3      # us
+        stage_bytes = {"page_score": bytes_["summary"], "sparse_paged_decode": bytes_["kv"] + bytes_["qo"]}
+        dom = max(stage_bytes, key=lambda k: stage[k])
+        achieved = stage_bytes[dom] / (stage[dom] * 1e-6) / 1e9
+        traffic, traffic_src = ncu_traffic(cfg, dom)
+        roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
+                    "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                    "algorithmic_bytes": stage_bytes[dom], "us": stage[dom]}
+        step_gbs = bytes_["total"] / (ms * 1e-3) / 1e9
+        cpu = None
+        if not args.no_cpu_baseline:
+            t, n, batch, threads = oracle_sample_time(cfg, SAMPLE_REQUESTS.get(cfg, 1), workload=w, summary=summary_kind,
+                                                      agg=args.agg if is_main else "sum")
+            cpu = {"value": t / n * batch * 1e6, "unit": "us", "cores": threads, "kind": "oracle",
+                   "sample": f"first {n} of {batch} requests (score + top-k + attention), one warm-up pass then the median of "
+                             f"3 passes, scaled by {batch}/{n}"}
+        # ---- sampled parity of the very outputs the timed step produced (outside every timed region) ----------
+        parity = None
+        if not args.no_cpu_baseline and summary_kind == "envelope" and args.agg == "sum" and args.topk_approx <= 0:
+            from oracle.workload_io import parity_sample
+            r.step()
+            torch.cuda.synchronize()
+            parity = parity_sample(w, PARITY_REQUESTS.get(cfg, [0]), r.sel_logical, r.sel_count, r.out, r.lse)
+        rec = {"value": ms * 1e3, "unit": "us", "steps": steps, "warmup": warmup, "ms_per_step": ms, "dtype": s.dtype,
+               "config": {"workload": cfg, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
+                          "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
+                          "seq_len": list(s.seq_len), "budget_pages": w.max_budget, "summary": summary_kind,
+                          "agg": args.agg if is_main else "sum",
+                          "topk": "exact" if args.topk_approx <= 0 else f"approx tolerate_ratio={args.topk_approx} (lossy)",
+                          "mla_step": args.mla_step if s.kv_shared else "n/a",
+                          "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"},
+               "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
+               "step_bytes": bytes_, "stage_us": stage, "roofline": roofline, "cpu_baseline": cpu, "parity": parity,
+               "e2e": {"value": e2e_ms * 1e3, "unit": "us", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+               "gpu_launches": launches_per_step * steps, "launches_per_step": launches_per_step, "clocks": clocks}
+    del r
+    torch.cuda.empty_cache()
+    return rec
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return spawn_ranks(args)
     import torch
     import torch.distributed as dist
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -303,89 +416,21 @@ def main():
         __graft_entry__.build()
     if world > 1:
         dist.barrier()
-
     peak, peak_src = measured_peak()
-    r = Runner(args.config, device, seed_offset=rank, summary=args.summary, topk_approx=args.topk_approx, agg=args.agg)
-    w, s = r.w, r.w.spec
-    bytes_ = algorithmic_bytes(w, summary=args.summary)
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    # ---- the timed region: K fused steps, device-timed, max over ranks --------------------------
-    barrier()
-    sampler = ClockSampler(local)
-    sampler.start()
-    sampler.ready.wait(timeout=10)          # NVML is up and the first sample is in before the timed region
-    times = r.time_device(r.step, args.steps, max(args.warmup, 3))
-    launches_per_step = r.ctx.last_launch_count
-    barrier()
-    clocks = sampler.result()
-    ms = statistics.mean(times)
-    if world > 1:
-        t = torch.tensor([ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-
-    # ---- end to end through the host-buffer entry point ------------------------------------------
-    e2e_times = r.time_host(r.step_host, min(args.steps, 30), 3)
-    e2e_ms = statistics.mean(e2e_times)
-    if world > 1:
-        t = torch.tensor([e2e_ms], device=device, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
-    esz = 2 if s.dtype == "bf16" else 4
-    h2d = s.batch * s.num_q_heads * s.qk_dim * esz + 4 * (s.batch + 1 + w.total_pages + 2 * s.batch)
-    d2h = s.batch * s.num_q_heads * s.v_dim * esz + 4 * s.batch * s.num_q_heads
-
-    # ---- per-stage times and the dominant kernel's roofline (rank 0) ------------------------------
-    line = None
-    if rank == 0:
-        r.step()
-        stage = {}
-        for name, fn in (("summary_append", r.stage_summary), ("page_score", r.stage_score),
-                         ("topk_pages", r.stage_topk), ("sparse_paged_decode", r.stage_decode)):
-            stage[name] = statistics.mean(r.time_device(fn, min(args.steps, 30), 3)) * 1e3      # us
-        stage_bytes = {"page_score": bytes_["summary"], "sparse_paged_decode": bytes_["kv"] + bytes_["qo"]}
-        dom = max(stage_bytes, key=lambda k: stage[k])
-        achieved = stage_bytes[dom] / (stage[dom] * 1e-6) / 1e9
-        roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
-                    "frac": achieved / peak, "traffic": ncu_traffic(args.config, dom), "peak_source": peak_src,
-                    "algorithmic_bytes": stage_bytes[dom], "us": stage[dom]}
-        step_gbs = bytes_["total"] / (ms * 1e-3) / 1e9
-        cpu = None
-        if not args.no_cpu_baseline:
-            t, n, batch, threads = oracle_sample_time(args.config, SAMPLE_REQUESTS.get(args.config, 1), workload=w, summary=args.summary, agg=args.agg)
-            cpu = {"value": t / n * batch * 1e6, "unit": "us", "cores": threads, "kind": "oracle",
-                   "sample": f"first {n} of {batch} requests, one pass (score + top-k + attention), scaled by {batch}/{n}"}
-        also = {}
-        for name in [c for c in args.also.split(",") if c and c != args.config]:
-            del r
-            torch.cuda.empty_cache()
-            r = Runner(name, device, topk_approx=args.topk_approx)
-            tt = statistics.mean(r.time_device(r.step, 20, 3))
-            b2 = algorithmic_bytes(r.w)
-            also[name] = {"us": tt * 1e3, "hbm_gbs": b2["total"] / (tt * 1e-3) / 1e9,
-                          "roofline_frac": b2["total"] / (tt * 1e-3) / 1e9 / peak, "bytes": b2["total"]}
-        line = {"metric": METRIC, "value": ms * 1e3, "unit": "us", "n_gpus": world, "steps": args.steps,
-                "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": False, "scaling": "weak",
-                "vs_baseline": None, "dtype": s.dtype, "data": "synthetic",
-                "config": {"workload": args.config, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
-                           "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
-                           "seq_len": list(s.seq_len), "budget_pages": w.max_budget, "summary": args.summary, "agg": args.agg,
-                           "topk": "exact" if args.topk_approx <= 0 else f"approx tolerate_ratio={args.topk_approx} (lossy)",
-                           "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"},
-                "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
-                "step_bytes": bytes_, "stage_us": stage, "roofline": roofline, "cpu_baseline": cpu,
-                "e2e": {"value": e2e_ms * 1e3, "unit": "us", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
-                "gpu_launches": launches_per_step * args.steps, "launches_per_step": launches_per_step,
-                "clocks": clocks, "also": also}
+    main_rec = measure(args.config, args, device, local, rank, world, args.steps, max(args.warmup, 3), peak, peak_src, rank)
+    also = {}
+    for name in [c for c in args.also.split(",") if c and c != args.config]:
+        rec = measure(name, args, device, local, rank, world, args.also_steps, 3, peak, peak_src, rank)
+        if rec is not None:
+            also[name] = rec
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
-    if line is not None:
+    if rank == 0:
+        line = {"metric": METRIC, "n_gpus": world, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+                "data": "synthetic"}
+        line.update(main_rec)
+        line["also"] = also
         print(json.dumps(line))
 
 

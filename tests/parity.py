@@ -14,31 +14,65 @@ from oracle.workload_io import to_oracle
 TOL = {"bf16": dict(abs=2e-2, rel=1e-2, lse=1e-3), "f32": dict(abs=1e-4, rel=1e-4, lse=1e-5)}
 
 
-def check_selection(w, gpu_logical, gpu_phys, gpu_count, ref):
-    """returns the number of (request, head) problems that needed the near-tie exception."""
+NEAR_TIE = 1e-3          # north star: a differing page must score within this (relative) of the oracle's k-th score
+FP32_BAND = 1e-4         # worst-case fp32 rounding of a 1,152-term score sum (n * 2^-24), rounded up
+PARITY_LOG = []          # one record per check_selection call; conftest.py prints the totals and writes gpurun_out/parity_counts.json
+
+
+class SelectionStats(dict):
+    """problems, excepted (problems that needed the near-tie rule), swapped_pages (pages in the symmetric difference),
+    fp32_band_pages (oracle pages within FP32_BAND of the threshold: the ceiling for swapped_pages), max_rel."""
+
+    def __int__(self):
+        return self["excepted"]
+
+    def __radd__(self, other):
+        return other + self["excepted"]
+
+    def __add__(self, other):
+        return self["excepted"] + int(other)
+
+
+def check_selection(w, gpu_logical, gpu_phys, gpu_count, ref, label=None):
+    """Selection parity per (request, KV head); returns SelectionStats (int(stats) = problems that needed the near-tie rule).
+    The stated rule: a page in the symmetric difference must score within 1e-3 relative of the oracle's threshold.  On top
+    of it the exception is BOUNDED: a problem may not swap more pages than the oracle itself finds inside the fp32 rounding
+    band (FP32_BAND) around its threshold -- a kernel that mis-ranks pages 5e-4 apart passes the rule but not the ceiling."""
     sl, sp, sc = (np.asarray(t) for t in (gpu_logical, gpu_phys, gpu_count))
     indptr = np.asarray(w.page_indptr.cpu())
     indices = np.asarray(w.page_indices.cpu())
     assert np.array_equal(sc, ref["sel_count"]), "sel_count differs"
-    excepted = 0
+    st = SelectionStats(problems=0, excepted=0, swapped_pages=0, fp32_band_pages=0, max_rel=0.0)
     for i in range(sc.shape[0]):
         for h in range(sc.shape[1]):
             n = sc[i, h]
             got = sl[i, h, :n]
+            st["problems"] += 1
             assert (sl[i, h, n:] == -1).all() and (sp[i, h, n:] == -1).all(), "padding must be -1"
             assert (np.diff(got) > 0).all(), "logical ids must be strictly ascending (no duplicates)"
             assert np.array_equal(sp[i, h, :n], indices[indptr[i] + got]), "physical ids do not match the page table"
             want = ref["sel_logical"][i, h, :n]
+            thr = ref["thr"][i, h]
+            if np.isfinite(thr):
+                allp = ref["scores"][h, indptr[i]:indptr[i + 1]]
+                band = int((np.abs(allp - thr) / np.maximum(np.abs(allp), np.abs(thr)) < FP32_BAND).sum())
+            else:
+                band = 0
+            st["fp32_band_pages"] += band
             if np.array_equal(got, want):
                 continue
             diff = np.setxor1d(got, want)
-            thr = ref["thr"][i, h]
             s = ref["scores"][h, indptr[i] + diff]
             rel = np.abs(s - thr) / np.maximum(np.abs(s), np.abs(thr))
-            assert np.isfinite(thr) and (rel < 1e-3).all(), \
+            assert np.isfinite(thr) and (rel < NEAR_TIE).all(), \
                 f"selection differs beyond the 1e-3 near-tie rule at request {i} head {h}: pages {diff}, rel {rel}"
-            excepted += 1
-    return excepted
+            assert len(diff) <= band, \
+                f"request {i} head {h}: {len(diff)} pages swapped but only {band} oracle scores lie within {FP32_BAND} of the threshold"
+            st["excepted"] += 1
+            st["swapped_pages"] += len(diff)
+            st["max_rel"] = max(st["max_rel"], float(rel.max()))
+    PARITY_LOG.append(dict(st, label=label or getattr(w.spec, "name", "?")))
+    return st
 
 
 def oracle_attention_on(w, sel_logical, sel_count):

@@ -12,7 +12,7 @@ from tests.parity import check_attention, check_selection
 
 pytestmark = pytest.mark.gpu
 
-SAMPLES = {"C2": [0, 17, 31], "C3": [3], "C4": [0, 21, 42, 63], "C5": [1, 64, 127]}
+SAMPLES = {"C2": [0, 4, 9, 13, 17, 22, 26, 31], "C3": [0, 3, 5, 7], "C4": [0, 9, 18, 21, 33, 42, 55, 63], "C5": [1, 40, 64, 127]}
 
 
 def run_step(name):
@@ -40,7 +40,7 @@ def run_step(name):
 
 
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
-def test_fullsize_fused_step_sampled_against_oracle(name):
+def test_fullsize_fused_step_sampled_against_oracle(name, record_property):
     from paper_2606_06453_b200.workloads import subproblem
     w, summary, out, lse, sp, sl, sc = run_step(name)
     s = w.spec
@@ -63,13 +63,14 @@ def test_fullsize_fused_step_sampled_against_oracle(name):
     assert bool((w.page_indices.cpu().long()[flat][live] == spc[live]).all()), "physical ids follow the page table"
     assert bool(torch.isfinite(out.float()).all()) and bool(torch.isfinite(lse).all())
     # ---- sampled requests against the oracle ---------------------------------------------------------
-    excepted = 0
+    excepted = swapped = problems = 0
     for r in SAMPLES[name]:
         sub = subproblem(w, [r])
         ref = oracle_step(sub)
         # the sub-problem renumbers physical pages 0..P-1 in logical order
-        excepted += check_selection(sub, sl[r:r + 1].cpu().numpy(), sl[r:r + 1].cpu().numpy(), sc[r:r + 1].cpu().numpy(),
-                                    ref)
+        st = check_selection(sub, sl[r:r + 1].cpu().numpy(), sl[r:r + 1].cpu().numpy(), sc[r:r + 1].cpu().numpy(),
+                             ref, label=f"{name} full size, request {r}")
+        excepted, swapped, problems = excepted + st["excepted"], swapped + st["swapped_pages"], problems + st["problems"]
         q, opool, opt = to_oracle(sub)
         o_ref, l_ref = vo.sparse_attention(q, opool, opt, sl[r:r + 1].cpu().numpy(), sc[r:r + 1].cpu().numpy(),
                                            s.num_q_heads, s.num_kv_heads, s.qk_dim, s.v_dim, s.sm_scale)
@@ -79,7 +80,8 @@ def test_fullsize_fused_step_sampled_against_oracle(name):
         got = summary[last].float().cpu().numpy().astype(np.float64)
         want = ref["summary"][int(sub.page_indptr[1]) - 1]
         assert np.array_equal(got, want), "append summary update inside the fused step"
-    print(f"{name}: near-tie exception used in {excepted} sampled (request, head) problems")
+    record_property("near_tie", dict(problems=problems, excepted=excepted, swapped_pages=swapped))
+    print(f"{name}: near-tie exception used in {excepted} of {problems} sampled (request, head) problems, {swapped} pages swapped")
 
 
 def test_c3_planted_pages_are_recalled():
