@@ -239,6 +239,25 @@ vx_status vx_sparse_decode_step_host(vx_ctx *ctx, const void *h_q, const vx_kv_p
                                      const int32_t *h_budget, int32_t max_budget, uint32_t flags,
                                      void *h_out, float *h_lse, vx_stream stream);
 
+/* ---- (a4)+(a5) without a context, a workspace or any allocation ------------------------------------------------
+ * vx_sparse_paged_decode_static computes what vx_sparse_paged_decode computes (Eq.4 over the selected pages,
+ * :75 split + LSE merge) for callers that cannot call cudaMalloc -- code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid it.  It takes the geometry by value instead of a context, and its split-KV partials live in a
+ * file-scope device array of vx_static_scratch_bytes() = 8 MiB that every GPU loading the library holds until the
+ * process exits; the call itself performs no cudaMalloc / cudaFree and calls no allocating routine.  It runs the
+ * geometry-agnostic CUDA-core kernels (every geometry vx_create accepts; not the tensor-core paths), on the calling
+ * thread's current device, asynchronously on `stream`.
+ * Limits and hazards: batch * num_q_heads * 4 (GQA; 1 for MLA) * (v_dim + 1) * 4 bytes must fit the array, else
+ * VX_ERR_WORKSPACE (the split count shrinks to fit first); all calls share the array, which keeps the last call's
+ * contents (nothing in it needs clearing), so calls that overlap on the GPU -- different streams -- race: serialise them.
+ * Arguments as vx_sparse_paged_decode.  Errors: text in vx_static_last_error() (process-wide, not thread-safe). */
+vx_status vx_sparse_paged_decode_static(const vx_geom *geom, const void *q, const vx_kv_pool *pool,
+                                        const vx_page_table *pt, const int32_t *sel_phys, const int32_t *sel_logical,
+                                        const int32_t *sel_count, int32_t max_budget, void *out, float *lse,
+                                        vx_stream stream);
+size_t vx_static_scratch_bytes(void);
+const char *vx_static_last_error(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -27,7 +27,8 @@ VX_MLA_STEP_AUTO, VX_MLA_STEP_FUSED, VX_MLA_STEP_CHAINED, VX_MLA_STEP_FLAT = 0, 
 EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",
            "vx_page_summary_update", "vx_page_score", "vx_topk_pages", "vx_sparse_paged_decode",
            "vx_sparse_decode_step", "vx_sparse_decode_step_host", "vx_trace_attach",
-           "vx_topk_pages_approx", "vx_set_topk_approx", "vx_union_pages", "vx_set_option"]
+           "vx_topk_pages_approx", "vx_set_topk_approx", "vx_union_pages", "vx_set_option",
+           "vx_sparse_paged_decode_static", "vx_static_scratch_bytes", "vx_static_last_error"]
 
 
 class VxGeom(C.Structure):
@@ -82,6 +83,9 @@ def load_library():
         "vx_topk_pages_approx": (I32, [P, P, T, P, I32, C.c_float, C.c_uint64, P, P, P, P]),
         "vx_set_topk_approx": (I32, [P, C.c_float, C.c_uint64]),
         "vx_set_option": (I32, [P, I32, I32]),
+        "vx_sparse_paged_decode_static": (I32, [G, P, K, T, P, P, P, I32, P, P, P]),
+        "vx_static_scratch_bytes": (C.c_size_t, []),
+        "vx_static_last_error": (C.c_char_p, []),
         "vx_union_pages": (I32, [P, T, P, P, I32, I32, P, P, P, P]),
         "vx_sparse_paged_decode": (I32, [P, P, K, T, P, P, P, I32, P, P, P]),
         "vx_sparse_decode_step": (I32, [P, P, K, P, T, P, I32, U32, P, P, P, P, P, P]),
@@ -231,6 +235,17 @@ class Context:
             self._h, _ptr(h_q), C.byref(pool.c), _ptr(summary), h_seq_lens.numel(), _ptr(h_page_indptr),
             _ptr(h_page_indices), _ptr(h_seq_lens), _ptr(h_budget), max_budget, flags, _ptr(h_out),
             _ptr(h_lse), _stream(stream)))
+
+
+def sparse_paged_decode_static(geom: VxGeom, q, pool: KvPool, pt: PageTable, sel_phys, sel_logical, sel_count, max_budget,
+                               out, lse=None, stream=None):
+    """vx_sparse_paged_decode_static: no context, no workspace, no allocation (scratch in a static device array)."""
+    lib = load_library()
+    st = lib.vx_sparse_paged_decode_static(C.byref(geom), _ptr(q), C.byref(pool.c), C.byref(pt.c), _ptr(sel_phys),
+                                           _ptr(sel_logical), _ptr(sel_count), max_budget, _ptr(out), _ptr(lse),
+                                           _stream(stream))
+    if st != VX_OK:
+        raise VortexError(st, lib.vx_static_last_error().decode())
 
 
 # ---- conveniences used by tests / bench (allocation + marshalling only) -----------------------

@@ -8,6 +8,10 @@
 // online softmax state and the output accumulators live in registers.  Work is split over
 // (request, KV head, page split, token slice); every (split, slice) writes one partial (o, lse)
 // that the combine kernel merges.
+#include <cstdarg>
+#include <cstdio>
+#include <mutex>
+
 #include "vx_common.cuh"
 #include "vx_internal.h"
 
@@ -236,4 +240,132 @@ cudaError_t launch_decode_mla(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
                                                          max_budget, out, lse, s);
 }
 
+
+// ---- vx_sparse_paged_decode_static: (a4)+(a5) with NO allocation and no context ---------------------------------------
+// For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it):
+// the split-KV partials of decode_generic_kernel / combine_kernel live in the file-scope device array below instead of a
+// caller workspace.  Every GPU that loads the library holds the array (kStaticScratchBytes) until the process exits.
+// Every call shares it and it keeps the last call's contents; nothing in it has to start at zero (each (split, slice)
+// writes its whole partial, weight -inf when empty, before the combine kernel reads it), but two calls that overlap on
+// the GPU (different streams) race on it.  Same arithmetic as the generic path of vx_sparse_paged_decode.
+constexpr size_t kStaticScratchBytes = (size_t)8 << 20;          // 8 MiB: partial o + partial lse of one call
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+constexpr int kStaticMaxDevices = 64;
+static std::mutex g_static_mu;
+static void* g_static_ptr[kStaticMaxDevices];                   // device address of the array, per device
+static int g_static_sms[kStaticMaxDevices];
+static char g_static_err[512] = "";
+
+static vx_status static_fail(vx_status st, const char* fmt, ...) {
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(g_static_err, sizeof g_static_err, fmt, ap);
+  va_end(ap);
+  return st;
+}
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the address the kernels get comes from
+// cudaGetSymbolAddress, once per device, with that device current.
+static vx_status static_scratch_for_current_device(void** ptr, int* num_sms) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return static_fail(VX_ERR_CUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+  if (dev < 0 || dev >= kStaticMaxDevices) return static_fail(VX_ERR_UNSUPPORTED, "device index %d beyond %d", dev, kStaticMaxDevices);
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (g_static_ptr[dev] == nullptr) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || p == nullptr)
+      return static_fail(VX_ERR_CUDA, "cudaGetSymbolAddress(static scratch): %s", cudaGetErrorString(e));
+    int sms = 0;
+    e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return static_fail(VX_ERR_CUDA, "cudaDeviceGetAttribute: %s", cudaGetErrorString(e));
+    g_static_sms[dev] = sms;
+    g_static_ptr[dev] = p;
+  }
+  *ptr = g_static_ptr[dev];
+  *num_sms = g_static_sms[dev];
+  return VX_OK;
+}
+
+template <typename T, int D, int DV, int HPW, int WT>
+static vx_status launch_generic_static_t(const vx_geom& g, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                                         const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
+                                         int32_t max_budget, void* out, float* lse, cudaStream_t s, void* scratch, int num_sms) {
+  const int grp = g.num_q_heads / g.num_kv_heads;
+  const int wh = (grp + HPW - 1) / HPW;
+  const size_t rows = (size_t)pt.batch * g.num_q_heads;
+  const size_t per_part = rows * ((size_t)DV + 1) * 4;           // bytes of partial o + lse per (split, slice)
+  // splits: cover the SMs a few times over (as the workspace path), at least 2 pages per split, and within the array
+  const int units = pt.batch * g.num_kv_heads;
+  int splits = (num_sms * 4 + units - 1) / (units > 0 ? units : 1);
+  if (splits > (max_budget + 1) / 2) splits = (max_budget + 1) / 2;
+  if (splits > kMaxSplits / WT) splits = kMaxSplits / WT;
+  if (splits < 1) splits = 1;
+  const size_t fit = kStaticScratchBytes / (per_part * WT + 512);      // (+512: the lse block starts 256-byte aligned)
+  if (fit < 1)
+    return static_fail(VX_ERR_WORKSPACE, "batch %d x %d query heads x v_dim %d needs %zu bytes of split partials; the static "
+                       "scratch of vx_sparse_paged_decode_static holds %zu (use vx_sparse_paged_decode with a workspace)",
+                       pt.batch, g.num_q_heads, DV, per_part * WT, kStaticScratchBytes);
+  if ((size_t)splits > fit) splits = (int)fit;
+  const int n_part = splits * WT;
+  float* part_o = static_cast<float*>(scratch);
+  const size_t o_bytes = (rows * n_part * DV * 4 + 255) / 256 * 256;
+  float* part_lse = reinterpret_cast<float*>(static_cast<unsigned char*>(scratch) + o_bytes);
+  dim3 grid(splits, g.num_kv_heads, pt.batch);
+  const void* v = g.kv_shared ? pool.k : pool.v;
+  decode_generic_kernel<T, D, DV, HPW, WT><<<grid, wh * WT * kWarp, 0, s>>>(
+      static_cast<const T*>(q), static_cast<const T*>(pool.k), static_cast<const T*>(v), pool.stride_page,
+      pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads, g.page_size, g.sm_scale,
+      pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits, part_o, part_lse);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) {
+    combine_kernel<T><<<(unsigned)rows, 128, 0, s>>>(part_o, part_lse, n_part, g.v_dim, static_cast<T*>(out), lse);
+    e = cudaGetLastError();
+  }
+  if (e != cudaSuccess) return static_fail(VX_ERR_CUDA, "vx_sparse_paged_decode_static: %s", cudaGetErrorString(e));
+  return VX_OK;
+}
+
 }  // namespace vx
+
+extern "C" {
+
+size_t vx_static_scratch_bytes(void) { return vx::kStaticScratchBytes; }
+
+const char* vx_static_last_error(void) { return vx::g_static_err; }
+
+vx_status vx_sparse_paged_decode_static(const vx_geom* g, const void* q, const vx_kv_pool* pool, const vx_page_table* pt,
+                                        const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
+                                        int32_t max_budget, void* out, float* lse, vx_stream stream) {
+  using namespace vx;
+  if (!g || !q || !pool || !pool->k || !pt || !sel_phys || !sel_logical || !sel_count || !out)
+    return static_fail(VX_ERR_INVALID_ARG, "geom / q / pool / page table / sel_* / out is NULL");
+  if (g->num_q_heads <= 0 || g->num_kv_heads <= 0 || g->num_q_heads % g->num_kv_heads != 0 || g->page_size <= 0)
+    return static_fail(VX_ERR_INVALID_ARG, "num_q_heads must be a positive multiple of num_kv_heads, page_size positive");
+  if (!g->kv_shared && !pool->v) return static_fail(VX_ERR_INVALID_ARG, "kv pool v is NULL");
+  if (pt->batch < 0 || (pt->batch > 0 && !pt->seq_lens)) return static_fail(VX_ERR_INVALID_ARG, "bad page table");
+  if (max_budget <= 0) return static_fail(VX_ERR_INVALID_ARG, "max_budget must be positive");
+  if (g->kv_shared ? !mla_geometry_supported(*g) : !gqa_geometry_supported(*g))
+    return static_fail(VX_ERR_UNSUPPORTED, "(dtype, qk_dim, v_dim, heads) not supported by the decode kernels");
+  if (pt->batch == 0) return VX_OK;
+  void* scratch = nullptr;
+  int sms = 0;
+  if (vx_status st = static_scratch_for_current_device(&scratch, &sms)) return st;
+  cudaStream_t s = (cudaStream_t)stream;
+#define VX_GO(T, D, DV, HPW, WT) \
+  return launch_generic_static_t<T, D, DV, HPW, WT>(*g, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, scratch, sms)
+  if (g->kv_shared) VX_GO(__nv_bfloat16, 576, 512, 4, 1);
+  if (g->dtype == VX_DT_F32) {
+    if (g->qk_dim == 64) VX_GO(float, 64, 64, 8, 4);
+    if (g->qk_dim == 128) VX_GO(float, 128, 128, 8, 4);
+  } else {
+    if (g->qk_dim == 64) VX_GO(__nv_bfloat16, 64, 64, 8, 4);
+    if (g->qk_dim == 128) VX_GO(__nv_bfloat16, 128, 128, 8, 4);
+  }
+#undef VX_GO
+  return static_fail(VX_ERR_UNSUPPORTED, "qk_dim %d not supported", g->qk_dim);
+}
+
+}  // extern "C"
