@@ -36,10 +36,11 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   w.part_lse = static_cast<float*>(take(B * Hq * kMaxSplits * 4));
   w.unit_counter = static_cast<int32_t*>(take(B * Hkv * 4));
   w.h_q = take(B * Hq * (size_t)g.qk_dim * esz);
-  w.h_indptr = static_cast<int32_t*>(take((B + 1) * 4));
+  // page_indptr | seq_lens | budget are one contiguous block (one host->device copy), each part 4-byte aligned
+  w.h_indptr = static_cast<int32_t*>(take((3 * B + 1) * 4));
+  w.h_seq_lens = w.h_indptr ? w.h_indptr + (B + 1) : nullptr;
+  w.h_budget = w.h_indptr ? w.h_indptr + (2 * B + 1) : nullptr;
   w.h_indices = static_cast<int32_t*>(take((size_t)max_total_pages * 4));
-  w.h_seq_lens = static_cast<int32_t*>(take(B * 4));
-  w.h_budget = static_cast<int32_t*>(take(B * 4));
   w.h_out = take(B * Hq * (size_t)g.v_dim * esz);
   w.h_lse = static_cast<float*>(take(B * Hq * 4));
   const bool mla = g.kv_shared != 0;
@@ -178,12 +179,19 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->launches = 0;
   c->err[0] = 0;
   c->mla_step = VX_MLA_STEP_AUTO;
+  c->pinned_small = nullptr;
+  e = cudaHostAlloc(reinterpret_cast<void**>(&c->pinned_small), (3 * (size_t)(max_batch > 0 ? max_batch : 1) + 1) * 4, cudaHostAllocDefault);
+  if (e != cudaSuccess) {
+    delete c;
+    return fail(nullptr, VX_ERR_CUDA, "pinned staging for the host entry point: %s", cudaGetErrorString(e));
+  }
   c->flat_splits = c->flat_waves = 0;
   // split-arrival counters start at zero and every step leaves them at zero
   e = cudaMemset(c->ws.unit_counter, 0, (size_t)(max_batch > 0 ? max_batch : 1) * g->num_kv_heads * 4);
   if (e == cudaSuccess && g->kv_shared) e = cudaMemset(c->ws.flat_sync, 0, step_mla_flat_workspace_ints(max_batch) * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (e != cudaSuccess) {
+    cudaFreeHost(c->pinned_small);
     delete c;
     return fail(nullptr, VX_ERR_CUDA, "workspace initialisation: %s", cudaGetErrorString(e));
   }
@@ -192,6 +200,7 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
 }
 
 void vx_destroy(vx_ctx* ctx) {
+  if (ctx && ctx->pinned_small) cudaFreeHost(ctx->pinned_small);
   delete ctx;
 }
 
@@ -437,14 +446,22 @@ vx_status vx_sparse_decode_step_host(vx_ctx* c, const void* h_q, const vx_kv_poo
   Workspace& w = c->ws;
   const size_t q_bytes = (size_t)batch * g.num_q_heads * g.qk_dim * esz;
   const size_t o_bytes = (size_t)batch * g.num_q_heads * g.v_dim * esz;
-  cudaError_t e = cudaMemcpyAsync(w.h_q, h_q, q_bytes, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_indptr, h_page_indptr, (size_t)(batch + 1) * 4, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_indices, h_page_indices, (size_t)total * 4, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_seq_lens, h_seq_lens, (size_t)batch * 4, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_budget, h_budget, (size_t)batch * 4, cudaMemcpyHostToDevice, s);
+  // three copies in: the page ids first (the score kernel's first loads), then the three small arrays packed into the
+  // context's pinned staging block (a few hundred bytes; one transfer instead of three), then the queries.  The call is
+  // synchronous, so the staging block is free again when it returns.
+  const size_t B = (size_t)batch;
+  memcpy(c->pinned_small, h_page_indptr, (B + 1) * 4);
+  memcpy(c->pinned_small + (B + 1), h_seq_lens, B * 4);
+  memcpy(c->pinned_small + (2 * B + 1), h_budget, B * 4);
+  int32_t* d_indptr = w.h_indptr;                       // device block laid out like the staging block for THIS batch
+  int32_t* d_seq = d_indptr + (B + 1);
+  int32_t* d_budget = d_indptr + (2 * B + 1);
+  cudaError_t e = cudaMemcpyAsync(w.h_indices, h_page_indices, (size_t)total * 4, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(d_indptr, c->pinned_small, (3 * B + 1) * 4, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(w.h_q, h_q, q_bytes, cudaMemcpyHostToDevice, s);
   if (vx_status st = check_cuda(c, e, "host->device copies")) return st;
-  vx_page_table pt{batch, w.h_indptr, w.h_indices, w.h_seq_lens, total, max_pages};
-  vx_status st = vx_sparse_decode_step(c, w.h_q, pool, summary, &pt, w.h_budget, max_budget, flags, w.h_out,
+  vx_page_table pt{batch, d_indptr, w.h_indices, d_seq, total, max_pages};
+  vx_status st = vx_sparse_decode_step(c, w.h_q, pool, summary, &pt, d_budget, max_budget, flags, w.h_out,
                                        w.h_lse, nullptr, nullptr, nullptr, stream);
   if (st != VX_OK) return st;
   e = cudaMemcpyAsync(h_out, w.h_out, o_bytes, cudaMemcpyDeviceToHost, s);

@@ -55,6 +55,7 @@ struct vx_ctx {
   int32_t launches;              // kernels enqueued by the last compute call
   vx::ApproxPlan approx;         // vx_set_topk_approx: used by a fused step with VX_STEP_APPROX_TOPK
   int32_t mla_step;              // VX_OPT_MLA_STEP
+  int32_t* pinned_small;         // pinned host staging [3 max_batch + 1] for vx_sparse_decode_step_host's small arrays
   int32_t flat_splits, flat_waves;   // VX_OPT_MLA_FLAT_*: 0 = the library's choice
   char err[512];
 };
