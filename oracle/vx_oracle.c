@@ -24,7 +24,7 @@
  *
  * Every function is the plain definition: no blocking, no fusion, no reordering.
  * All arithmetic is double.  Inputs are read in their storage dtype (bf16 bits or
- * fp32) and widened exactly.
+ * fp32) and widened exactly; fp8 KV pools arrive as the doubles scale * decode(code) (vx_oracle_fp8.py).
  *
  * Pins (tests/test_oracle_*.py, -m "not gpu"): closed forms of softmax attention,
  * dense == sparse when the budget covers all pages, split+combine == unsplit,
@@ -47,9 +47,11 @@
 
 #define VXO_BF16 0
 #define VXO_F32 1
+#define VXO_F64 2 /* values that are already doubles: fp8 pools widened and scaled by oracle/vx_oracle_fp8.py (readings G25-G27) */
 
 /* exact widening of one stored element to double */
 static double ld_elem(const void *base, int dtype, int64_t idx) {
+  if (dtype == VXO_F64) return ((const double *)base)[idx];
   if (dtype == VXO_F32) return (double)((const float *)base)[idx];
   uint32_t bits = ((uint32_t)((const uint16_t *)base)[idx]) << 16;
   float f;
@@ -159,6 +161,7 @@ void vxo_page_score(const void *q, int dtype, const double *summary, int num_q_h
 static double round_to_storage(double x, int dtype) {
   float f = (float)x;                         /* fp32 storage: one rounding */
   if (dtype == VXO_F32) return (double)f;
+  if (dtype == VXO_F64) return x;             /* (fp8 pools have no centroid flow; doubles pass through) */
   /* bf16: round the DOUBLE to 8 significand bits directly (no double rounding through float) */
   if (x == 0.0 || x != x) return x;
   int e;

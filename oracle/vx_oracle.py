@@ -21,7 +21,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "vx_oracle.c")
 _LIB = os.path.join(_HERE, "libvx_oracle.so")
 
-BF16, F32 = 0, 1
+BF16, F32, F64 = 0, 1, 2   # F64: values that are already doubles (fp8 pools widened by vx_oracle_fp8.py)
 AGG_SUM, AGG_MAX = 0, 1
 
 
@@ -67,7 +67,9 @@ def _dt(a: np.ndarray) -> int:
         return BF16
     if a.dtype == np.float32:
         return F32
-    raise TypeError(f"oracle takes bf16 bits (uint16) or float32, got {a.dtype}")
+    if a.dtype == np.float64:
+        return F64
+    raise TypeError(f"oracle takes bf16 bits (uint16), float32 or float64, got {a.dtype}")
 
 
 def _p(a):

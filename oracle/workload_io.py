@@ -8,6 +8,12 @@ from oracle import vx_oracle as vo
 def to_oracle(w):
     """Workload (any device) -> (q, Pool, PageTable) numpy views on CPU copies."""
     sp, st, sh = w.strides
+    if getattr(w.spec, "kv_dtype", ""):                  # fp8 KV cache: the doubles scale * decode(code) (vx_oracle_fp8.py)
+        from oracle.vx_oracle_fp8 import pool_fp8
+        pool = pool_fp8(vo.as_np(w.k_pool), None if w.v_pool is None else vo.as_np(w.v_pool), w.spec.kv_dtype,
+                        w.k_scale, w.v_scale, sp, st, sh, w.num_pool_pages)
+        pt = vo.PageTable(vo.as_np(w.page_indptr), vo.as_np(w.page_indices), vo.as_np(w.seq_lens), w.spec.page_size)
+        return vo.as_np(w.q), pool, pt
     pool = vo.Pool(k=vo.as_np(w.k_pool), v=None if w.v_pool is None else vo.as_np(w.v_pool),
                    stride_page=sp, stride_token=st, stride_head=sh, num_pool_pages=w.num_pool_pages)
     pt = vo.PageTable(vo.as_np(w.page_indptr), vo.as_np(w.page_indices), vo.as_np(w.seq_lens),

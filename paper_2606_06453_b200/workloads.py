@@ -41,6 +41,7 @@ class Spec:
     pool_slack: int = 64       # unused physical pages in the pool
     pool_pages: int = 0        # fixed pool size (C1: 128), 0 -> total + slack
     cfg_id: int = 0            # seeds: 1000+id data, 2000+id permutation, 3000+id lengths, 4000+id planted
+    kv_dtype: str = ""         # "" = pools in `dtype`; "e4m3" / "e5m2" = fp8 KV cache: uint8 code pools
 
     @property
     def sm_scale(self) -> float:
@@ -68,6 +69,14 @@ SPECS["C4-small"] = replace(SPECS["C4"], name="C4-small", batch=3, seq_len=(1000
 SPECS["C5-small"] = replace(SPECS["C5"], name="C5-small", batch=6, seq_len=(600, 6000))
 
 
+def with_fp8(spec: "Spec | str", fmt: str = "e4m3") -> Spec:
+    """the same workload with an fp8 KV cache: the pools are drawn as before, then stored as fp8 codes with one scale
+    per pool tensor (scale = max |x| / largest fp8 value, so nothing saturates)"""
+    spec = SPECS[spec] if isinstance(spec, str) else spec
+    assert fmt in ("e4m3", "e5m2") and spec.dtype == "bf16"
+    return replace(spec, name=f"{spec.name}-{fmt}", kv_dtype=fmt)
+
+
 @dataclass
 class Workload:
     spec: Spec
@@ -82,6 +91,8 @@ class Workload:
     total_pages: int
     max_pages_per_req: int
     planted: list = field(default_factory=list)  # per request: logical ids of planted pages
+    k_scale: float = 1.0        # fp8 pools: a code c stands for scale * decode(c)
+    v_scale: float = 1.0
 
     @property
     def num_pool_pages(self) -> int:
@@ -172,11 +183,33 @@ def make_workload(spec: Spec | str, device="cpu", seed_offset: int = 0) -> Workl
             blk = k_pool[phys].float() + spec.planted_alpha * qhat[i].view(1, spec.num_kv_heads, 1, -1)
             k_pool[phys] = blk.to(dt)
 
+    k_scale = v_scale = 1.0
+    if spec.kv_dtype:
+        k_pool, k_scale = _to_fp8_codes(k_pool, spec.kv_dtype)
+        if v_pool is not None:
+            v_pool, v_scale = _to_fp8_codes(v_pool, spec.kv_dtype)
+        else:
+            v_scale = k_scale
+
     return Workload(spec=spec, q=q, k_pool=k_pool, v_pool=v_pool,
                     page_indptr=indptr.to(torch.int32).to(dev), page_indices=indices.to(dev),
                     seq_lens=seq.to(torch.int32).to(dev), budget=budget.to(torch.int32).to(dev),
                     max_budget=max_budget, total_pages=total, max_pages_per_req=int(pages.max()),
-                    planted=planted)
+                    planted=planted, k_scale=k_scale, v_scale=v_scale)
+
+
+_FP8 = {"e4m3": (torch.float8_e4m3fn, 448.0), "e5m2": (torch.float8_e5m2, 57344.0)}
+
+
+def _to_fp8_codes(pool: torch.Tensor, fmt: str):
+    """(uint8 codes of the pool stored as fp8, fp32 scale): storage conversion of the drawn data, not the method"""
+    tdt, fmax = _FP8[fmt]
+    scale = float(torch.tensor(float(pool.abs().max()) / fmax, dtype=torch.float32))
+    codes = torch.empty(pool.shape, dtype=torch.uint8, device=pool.device)
+    step = max(1, (1 << 27) // max(1, pool[0].numel()))
+    for p0 in range(0, pool.shape[0], step):
+        codes[p0:p0 + step] = (pool[p0:p0 + step].float() / scale).to(tdt).view(torch.uint8)
+    return codes, scale
 
 
 def subproblem(w: Workload, requests) -> Workload:
@@ -202,7 +235,7 @@ def subproblem(w: Workload, requests) -> Workload:
                     seq_lens=w.seq_lens.cpu()[sel].contiguous(), budget=budget.contiguous(),
                     max_budget=w.max_budget, total_pages=len(rows),
                     max_pages_per_req=int(counts.max()),
-                    planted=[w.planted[r] for r in requests] if w.planted else [])
+                    planted=[w.planted[r] for r in requests] if w.planted else [], k_scale=w.k_scale, v_scale=w.v_scale)
 
 
 APPD_DISTRIBUTIONS = ("bimodal", "normal", "lognormal", "uniform")
