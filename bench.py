@@ -44,6 +44,9 @@ def parse_args():
     ap.add_argument("--also", default="C3,C2,C5,C1", help="further configs, each a full record (step, stages, roofline, e2e, "
                     "clocks) under 'also'")
     ap.add_argument("--also-steps", type=int, default=50)
+    ap.add_argument("--kv-dtype", default="same", choices=["same", "e4m3", "e5m2"],
+                    help="storage of the KV cache and the summaries: the config's dtype (default, the north star) or fp8 codes "
+                         "with per-tensor scales (PAPER.md:200, :520; the bytes roofline is recomputed: summary and KV bytes halve)")
     ap.add_argument("--mla-step", default="auto", choices=["auto", "chained", "fused", "flat"],
                     help="schedule of the MLA step (VX_OPT_MLA_STEP); auto = the library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -88,14 +91,15 @@ def algorithmic_bytes(w, sel_count=None, summary="envelope"):
     page's K and V tokens once, Q in and O out.  Page table / scores / partials are not counted."""
     import torch
     s = w.spec
-    esz = 2 if s.dtype == "bf16" else 4
+    esz = 2 if s.dtype == "bf16" else 4                # q and out
+    kv_esz = 1 if getattr(s, "kv_dtype", "") else esz   # K, V and the summaries (fp8 KV cache: one byte)
     b = s.page_size
     n = w.seq_lens.cpu().long()
     P = (n + b - 1) // b
-    summary = int(P.sum()) * s.num_kv_heads * (1 if summary == "centroid" else 2) * s.qk_dim * esz
+    summary = int(P.sum()) * s.num_kv_heads * (1 if summary == "centroid" else 2) * s.qk_dim * kv_esz
     k = torch.minimum(w.budget.cpu().long(), P)
     tokens = (k - 1) * b + (n - (P - 1) * b)          # the partial last page is always selected (n_local >= 1)
-    per_tok = (s.qk_dim if s.kv_shared else s.qk_dim + s.v_dim) * esz
+    per_tok = (s.qk_dim if s.kv_shared else s.qk_dim + s.v_dim) * kv_esz
     kv = int(tokens.sum()) * s.num_kv_heads * per_tok
     qo = s.batch * s.num_q_heads * (s.qk_dim + s.v_dim) * esz
     return dict(summary=summary, kv=kv, qo=qo, total=summary + kv + qo)
@@ -141,12 +145,14 @@ class ClockSampler(threading.Thread):
 class Runner:
     """One workload resident on one GPU: context, pools, summaries, outputs, L2 flush buffer."""
 
-    def __init__(self, cfg, device, seed_offset=0, summary="envelope", topk_approx=0.0, agg="sum", mla_step="auto"):
+    def __init__(self, cfg, device, seed_offset=0, summary="envelope", topk_approx=0.0, agg="sum", mla_step="auto",
+                 kv_dtype="same"):
         import torch
         import paper_2606_06453_b200 as vx
-        from paper_2606_06453_b200.workloads import make_workload
+        from paper_2606_06453_b200.workloads import make_workload, with_fp8
         self.torch, self.vx = torch, vx
-        self.w = w = make_workload(cfg, device=device, seed_offset=seed_offset)
+        spec = cfg if kv_dtype == "same" else with_fp8(cfg, kv_dtype)
+        self.w = w = make_workload(spec, device=device, seed_offset=seed_offset)
         kind = vx.binding.VX_SUMMARY_CENTROID if summary == "centroid" else vx.binding.VX_SUMMARY_ENVELOPE
         self.summary_name = summary
         self.ctx = vx.context_for(w, summary_kind=kind, agg=vx.binding.VX_AGG_MAX if agg == "max" else vx.binding.VX_AGG_SUM)
@@ -315,7 +321,8 @@ def measure(cfg, args, device, local, rank, world, steps, warmup, peak, peak_src
     import torch.distributed as dist
     is_main = cfg == args.config
     r = Runner(cfg, device, seed_offset=seed_offset, summary=args.summary if is_main else "envelope",
-               topk_approx=args.topk_approx, agg=args.agg if is_main else "sum", mla_step=args.mla_step)
+               topk_approx=args.topk_approx, agg=args.agg if is_main else "sum", mla_step=args.mla_step,
+               kv_dtype=args.kv_dtype if cfg != "C1" else "same")
     summary_kind = args.summary if is_main else "envelope"
     w, s = r.w, r.w.spec
     bytes_ = algorithmic_bytes(w, summary=summary_kind)
@@ -358,7 +365,7 @@ def measure(cfg, args, device, local, rank, world, steps, warmup, peak, peak_src
         stage_bytes = {"page_score": bytes_["summary"], "sparse_paged_decode": bytes_["kv"] + bytes_["qo"]}
         dom = max(stage_bytes, key=lambda k: stage[k])
         achieved = stage_bytes[dom] / (stage[dom] * 1e-6) / 1e9
-        traffic, traffic_src = ncu_traffic(cfg, dom)
+        traffic, traffic_src = ncu_traffic(cfg, dom) if not getattr(s, "kv_dtype", "") else (None, None)
         roofline = {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": "GB/s",
                     "frac": achieved / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
                     "algorithmic_bytes": stage_bytes[dom], "us": stage[dom]}
@@ -384,6 +391,7 @@ def measure(cfg, args, device, local, rank, world, steps, warmup, peak, peak_src
                           "agg": args.agg if is_main else "sum",
                           "topk": "exact" if args.topk_approx <= 0 else f"approx tolerate_ratio={args.topk_approx} (lossy)",
                           "mla_step": args.mla_step if s.kv_shared else "n/a",
+                          "kv_dtype": getattr(s, "kv_dtype", "") or s.dtype,
                           "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"},
                "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
                "step_bytes": bytes_, "stage_us": stage, "roofline": roofline, "cpu_baseline": cpu, "parity": parity,

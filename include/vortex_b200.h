@@ -69,6 +69,17 @@ typedef enum { VX_AGG_SUM = 0, VX_AGG_MAX = 1 } vx_agg;
  *            summary: [num_pool_pages, Hkv, qk_dim] -- half the bytes.  VX_AGG_SUM only. */
 typedef enum { VX_SUMMARY_ENVELOPE = 0, VX_SUMMARY_CENTROID = 1 } vx_summary_kind;
 
+/* storage format of the KV cache (PAPER.md:200 "fp8 KV cache", :520 / :525 kv_cache_dtype "fp8_e4m3", "fp8_e5m2"):
+ *  SAME      K, V pools and summaries hold elements of geom.dtype.
+ *  FP8_E4M3  OCP E4M3 (bias 7, no infinities, S.1111.111 = NaN, max 448) / FP8_E5M2  OCP E5M2 (bias 15, IEEE-like):
+ *            K, V pools and the summary pool hold one-byte codes; a code c stands for  scale * decode(c)  with one
+ *            fp32 scale per pool tensor (vx_kv_pool.k_scale / .v_scale; the MLA latent pool uses k_scale for both
+ *            roles).  q, out and lse stay in geom.dtype, which must be VX_DT_BF16.  Summaries are the min / max CODES
+ *            (exact); page scores are computed on decoded codes without k_scale -- a positive factor common to every
+ *            page changes no selection -- so vx_page_score returns  oracle score / k_scale  (G25-G27).
+ *            Envelope summaries and VX_AGG_SUM only; pool strides are in one-byte elements. */
+typedef enum { VX_KV_SAME = 0, VX_KV_FP8_E4M3 = 1, VX_KV_FP8_E5M2 = 2 } vx_kv_format;
+
 typedef struct {
   int32_t dtype;        /* vx_dtype of q, K, V, summaries and out */
   int32_t num_q_heads;  /* Hq */
@@ -82,6 +93,7 @@ typedef struct {
   int32_t n_local;      /* last pages always selected (:280); precondition n_sink+n_local <= budget[i] */
   int32_t agg;          /* vx_agg */
   int32_t summary_kind; /* vx_summary_kind */
+  int32_t kv_format;    /* vx_kv_format: storage of the K, V and summary pools (0 = elements of dtype) */
 } vx_geom;
 
 typedef struct {
@@ -102,6 +114,7 @@ typedef struct {
   const void *v; /* ignored when geom.kv_shared */
   int64_t stride_page, stride_token, stride_head;
   int32_t num_pool_pages;
+  float k_scale, v_scale; /* fp8 pools only (geom.kv_format != VX_KV_SAME): value = scale * decode(code); must be > 0 */
 } vx_kv_pool;
 
 /* ---- context ------------------------------------------------------------------------ */

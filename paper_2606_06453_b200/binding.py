@@ -21,6 +21,7 @@ VX_SUMMARY_ENVELOPE, VX_SUMMARY_CENTROID = 0, 1
 VX_STEP_UPDATE_SUMMARY = 1
 VX_STEP_APPROX_TOPK = 2
 VX_TRACE_SCORE, VX_TRACE_TOPK, VX_TRACE_DECODE = 1, 2, 4
+VX_KV_SAME, VX_KV_FP8_E4M3, VX_KV_FP8_E5M2 = 0, 1, 2
 VX_OPT_MLA_STEP, VX_OPT_MLA_FLAT_SPLITS, VX_OPT_MLA_FLAT_WAVES = 1, 2, 3
 VX_MLA_STEP_AUTO, VX_MLA_STEP_FUSED, VX_MLA_STEP_CHAINED, VX_MLA_STEP_FLAT = 0, 1, 2, 3
 
@@ -35,7 +36,7 @@ class VxGeom(C.Structure):
     _fields_ = [("dtype", C.c_int32), ("num_q_heads", C.c_int32), ("num_kv_heads", C.c_int32),
                 ("qk_dim", C.c_int32), ("v_dim", C.c_int32), ("page_size", C.c_int32),
                 ("kv_shared", C.c_int32), ("sm_scale", C.c_float), ("n_sink", C.c_int32),
-                ("n_local", C.c_int32), ("agg", C.c_int32), ("summary_kind", C.c_int32)]
+                ("n_local", C.c_int32), ("agg", C.c_int32), ("summary_kind", C.c_int32), ("kv_format", C.c_int32)]
 
 
 class VxPageTable(C.Structure):
@@ -45,7 +46,8 @@ class VxPageTable(C.Structure):
 
 class VxKvPool(C.Structure):
     _fields_ = [("k", C.c_void_p), ("v", C.c_void_p), ("stride_page", C.c_int64),
-                ("stride_token", C.c_int64), ("stride_head", C.c_int64), ("num_pool_pages", C.c_int32)]
+                ("stride_token", C.c_int64), ("stride_head", C.c_int64), ("num_pool_pages", C.c_int32),
+                ("k_scale", C.c_float), ("v_scale", C.c_float)]
 
 
 class VortexError(RuntimeError):
@@ -125,24 +127,25 @@ class PageTable:
 class KvPool:
     """K/V pools [N_pool, Hkv, page, d] (or any layout expressed by element strides)."""
 
-    def __init__(self, k, v, stride_page: int, stride_token: int, stride_head: int):
+    def __init__(self, k, v, stride_page: int, stride_token: int, stride_head: int, k_scale: float = 1.0,
+                 v_scale: float = 1.0):
         self.tensors = (k, v)
         self.c = VxKvPool(k.data_ptr(), 0 if v is None else v.data_ptr(), stride_page, stride_token,
-                          stride_head, k.shape[0])
+                          stride_head, k.shape[0], float(k_scale), float(v_scale))
 
 
 class Context:
     """One geometry on one device; owns its workspace tensor."""
 
     def __init__(self, *, dtype, num_q_heads, num_kv_heads, qk_dim, v_dim, page_size, sm_scale,
-                 n_sink, n_local, kv_shared=False, agg=VX_AGG_SUM, summary_kind=VX_SUMMARY_ENVELOPE, max_batch,
+                 n_sink, n_local, kv_shared=False, agg=VX_AGG_SUM, summary_kind=VX_SUMMARY_ENVELOPE, kv_format=0, max_batch,
                  max_total_pages,
                  max_pages_per_req, max_budget, device="cuda:0"):
         self.lib = load_library()
         self.torch_dtype = dtype
         dt = {torch.bfloat16: VX_DT_BF16, torch.float32: VX_DT_F32}[dtype]
         self.geom = VxGeom(dt, num_q_heads, num_kv_heads, qk_dim, v_dim, page_size, int(kv_shared),
-                           float(sm_scale), n_sink, n_local, agg, summary_kind)
+                           float(sm_scale), n_sink, n_local, agg, summary_kind, int(kv_format))
         self.device = torch.device(device)
         self.max = (int(max_batch), int(max_total_pages), int(max_pages_per_req), int(max_budget))
         need = self.lib.vx_workspace_bytes(C.byref(self.geom), *self.max)
@@ -256,14 +259,15 @@ def context_for(w, device=None, **over) -> Context:
               num_kv_heads=s.num_kv_heads, qk_dim=s.qk_dim, v_dim=s.v_dim, page_size=s.page_size,
               sm_scale=s.sm_scale, n_sink=s.n_sink, n_local=s.n_local, kv_shared=s.kv_shared,
               max_batch=s.batch, max_total_pages=w.total_pages, max_pages_per_req=w.max_pages_per_req,
-              max_budget=w.max_budget, device=device or w.q.device)
+              max_budget=w.max_budget, device=device or w.q.device,
+              kv_format={"": VX_KV_SAME, "e4m3": VX_KV_FP8_E4M3, "e5m2": VX_KV_FP8_E5M2}[getattr(s, "kv_dtype", "")])
     kw.update(over)
     return Context(**kw)
 
 
 def tables_for(w):
     sp, st, sh = w.strides
-    pool = KvPool(w.k_pool, w.v_pool, sp, st, sh)
+    pool = KvPool(w.k_pool, w.v_pool, sp, st, sh, getattr(w, "k_scale", 1.0), getattr(w, "v_scale", 1.0))
     pt = PageTable(w.page_indptr, w.page_indices, w.seq_lens, w.total_pages, w.max_pages_per_req)
     return pool, pt
 

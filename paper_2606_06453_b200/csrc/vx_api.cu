@@ -46,6 +46,7 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   const bool mla = g.kv_shared != 0;
   w.flat_qvec = static_cast<float*>(take(mla ? step_mla_flat_qvec_floats(max_batch) * 4 : 0));
   w.flat_sync = static_cast<int32_t*>(take(mla ? step_mla_flat_workspace_ints(max_batch) * 4 : 0));
+  w.fp8_qvec = static_cast<float*>(take(kv_is_fp8(g) ? B * Hkv * 2 * (size_t)g.qk_dim * 4 : 0));
   w.bytes = off;
   return w;
 }
@@ -84,6 +85,13 @@ static const char* check_geom(const vx_geom* g, vx_status* st) {
   if (g->agg != VX_AGG_SUM && g->agg != VX_AGG_MAX) return "agg must be VX_AGG_SUM or VX_AGG_MAX";
   if (g->summary_kind != VX_SUMMARY_ENVELOPE && g->summary_kind != VX_SUMMARY_CENTROID)
     return "summary_kind must be VX_SUMMARY_ENVELOPE or VX_SUMMARY_CENTROID";
+  if (g->kv_format != VX_KV_SAME) {            // fp8 KV cache: its own kernels (vx_score_fp8.cu, the generic decode path)
+    if (g->kv_format != VX_KV_FP8_E4M3 && g->kv_format != VX_KV_FP8_E5M2) return "kv_format must be VX_KV_SAME, VX_KV_FP8_E4M3 or VX_KV_FP8_E5M2";
+    if (!fp8_geometry_supported(*g))
+      return "fp8 KV cache: bf16 queries, envelope summaries, VX_AGG_SUM; GQA head widths 64 / 128 (groups of <= 8 heads) or the 576 / 512 MLA latent";
+    *st = VX_OK;
+    return nullptr;
+  }
   if (!score_geometry_supported(*g)) return "qk_dim / dtype / aggregation not supported by the score kernel (VX_AGG_MAX: GQA groups of <= 8 heads, or the bf16 MLA group of 16 / 32 heads)";
   if (g->kv_shared ? !mla_geometry_supported(*g) : !gqa_geometry_supported(*g))
     return "(dtype, qk_dim, v_dim, heads) not supported by the decode kernels";
@@ -123,7 +131,9 @@ static vx_status check_table(vx_ctx* c, const vx_page_table* pt) {
 static vx_status check_pool(vx_ctx* c, const vx_kv_pool* pool) {
   if (!pool || !pool->k) return fail(c, VX_ERR_INVALID_ARG, "kv pool / k is NULL");
   if (!c->g.kv_shared && !pool->v) return fail(c, VX_ERR_INVALID_ARG, "kv pool v is NULL");
-  const int64_t per16 = 16 / (int64_t)elem_size(c->g.dtype);
+  const int64_t per16 = 16 / (int64_t)kv_elem_size(c->g);
+  if (kv_is_fp8(c->g) && !(pool->k_scale > 0.f && (c->g.kv_shared || pool->v_scale > 0.f)))
+    return fail(c, VX_ERR_INVALID_ARG, "fp8 KV cache: k_scale / v_scale must be positive");
   if (pool->stride_page % per16 || pool->stride_token % per16 || pool->stride_head % per16 ||
       ((uintptr_t)pool->k & 15) || (!c->g.kv_shared && ((uintptr_t)pool->v & 15)))
     return fail(c, VX_ERR_INVALID_ARG, "pool pointers and strides must be multiples of 16 bytes");
@@ -322,6 +332,9 @@ static vx_status decode_dispatch(vx_ctx* c, const void* q, const vx_kv_pool* poo
                                  const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                                  int32_t max_budget, void* out, float* lse, cudaStream_t s,
                                  const DecodeOpts& opt = DecodeOpts()) {
+  if (kv_is_fp8(c->g))
+    return check_cuda(c, launch_decode_fp8(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s),
+                      "vx_sparse_paged_decode (fp8 KV cache)");
   cudaError_t e = c->g.kv_shared
                       ? launch_decode_mla(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt)
                       : launch_decode_gqa(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt);

@@ -2,6 +2,8 @@
 // (Not shared with oracle/: the oracle is plain C and includes nothing from here.)
 #pragma once
 #include <cuda_bf16.h>
+#include <cuda_fp16.h>
+#include <cuda_fp8.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -32,6 +34,37 @@ template <> struct Elem<float> {
   __device__ __forceinline__ static float to_float(float x) { return x; }
   __device__ __forceinline__ static float from_float(float x) { return x; }
 };
+
+// fp8 KV cache (include/vortex_b200.h vx_kv_format): one-byte codes, OCP E4M3 / E5M2.
+// Decoding goes through the hardware conversion to f16 (cvt.rn.f16x2.e4m3x2 / .e5m2x2: every fp8 value is exact in
+// f16), encoding through cvt.rn.satfinite (exact for values that are already representable: min / max of codes).
+struct fp8_e4m3 { uint8_t bits; };
+struct fp8_e5m2 { uint8_t bits; };
+template <typename T> struct Fp8Interp;
+template <> struct Fp8Interp<fp8_e4m3> { static constexpr __nv_fp8_interpretation_t kind = __NV_E4M3; };
+template <> struct Fp8Interp<fp8_e5m2> { static constexpr __nv_fp8_interpretation_t kind = __NV_E5M2; };
+template <typename T> __device__ __forceinline__ float2 fp8x2_to_float2(uint16_t two) {     // low byte = element 0
+  const __half2_raw h = __nv_cvt_fp8x2_to_halfraw2((__nv_fp8x2_storage_t)two, Fp8Interp<T>::kind);
+  return __half22float2(*reinterpret_cast<const __half2*>(&h));
+}
+template <typename T> struct ElemFp8 {
+  static constexpr int kPerVec = 16;  // elements per 16 B
+  __device__ __forceinline__ static void unpack(const uint4& v, float (&f)[16]) {
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const float2 a = fp8x2_to_float2<T>((uint16_t)(w[i] & 0xffffu)), b = fp8x2_to_float2<T>((uint16_t)(w[i] >> 16));
+      f[4 * i] = a.x; f[4 * i + 1] = a.y; f[4 * i + 2] = b.x; f[4 * i + 3] = b.y;
+    }
+  }
+  __device__ __forceinline__ static T from_float(float x) {
+    T r;
+    r.bits = (uint8_t)__nv_cvt_float_to_fp8(x, __NV_SATFINITE, Fp8Interp<T>::kind);
+    return r;
+  }
+};
+template <> struct Elem<fp8_e4m3> : ElemFp8<fp8_e4m3> {};
+template <> struct Elem<fp8_e5m2> : ElemFp8<fp8_e5m2> {};
 
 // ---- global / shared access -----------------------------------------------------------------
 // streaming 16-byte load: read once, do not keep in L1
@@ -64,6 +97,10 @@ template <> __device__ __forceinline__ __nv_bfloat16 round_double<__nv_bfloat16>
   b &= ~((1ull << 45) - 1);
   return __float2bfloat16_rn(__double2float_rn(__longlong_as_double((long long)b)));   // both conversions are exact now
 }
+
+// (fp8 pools have no centroid flow -- vx_create rejects the pair -- these only let the summary kernel's template instantiate)
+template <> __device__ __forceinline__ fp8_e4m3 round_double<fp8_e4m3>(double x) { return Elem<fp8_e4m3>::from_float((float)x); }
+template <> __device__ __forceinline__ fp8_e5m2 round_double<fp8_e5m2>(double x) { return Elem<fp8_e5m2>::from_float((float)x); }
 
 // ---- warp reductions --------------------------------------------------------------------------
 template <int WIDTH = 32> __device__ __forceinline__ float warp_sum(float v) {

@@ -26,22 +26,36 @@ template <> struct Pair<__nv_bfloat16> {
     f[1] = __uint_as_float(w & 0xffff0000u);
   }
 };
+template <typename T> struct PairFp8 {       // fp8 KV cache: two one-byte codes per lane access (the same channels as a bf16 pair)
+  static constexpr int kElems = 2;
+  __device__ __forceinline__ static void load(const T* p, float (&f)[2]) {
+    const float2 v = fp8x2_to_float2<T>(*reinterpret_cast<const uint16_t*>(p));
+    f[0] = v.x;
+    f[1] = v.y;
+  }
+};
+template <> struct Pair<fp8_e4m3> : PairFp8<fp8_e4m3> {};
+template <> struct Pair<fp8_e5m2> : PairFp8<fp8_e5m2> {};
 template <> struct Pair<float> {
   static constexpr int kElems = 1;
   __device__ __forceinline__ static void load(const float* p, float (&f)[1]) { f[0] = *p; }
 };
 
 // block = WH head-groups x WT token slices (warps); HPW query heads per warp
-template <typename T, int D, int DV, int HPW, int WT>
+// T = element type of q (and of out, through the combine kernel); TKV = element type of the pools (T, or an fp8 code type:
+// then a code stands for k_scale / v_scale times its decoded value, G26)
+template <typename T, typename TKV, int D, int DV, int HPW, int WT>
 __global__ void __launch_bounds__(256)
-decode_generic_kernel(const T* __restrict__ q, const T* __restrict__ kpool, const T* __restrict__ vpool,
+decode_generic_kernel(const T* __restrict__ q, const TKV* __restrict__ kpool, const TKV* __restrict__ vpool,
                       int64_t stride_page, int64_t stride_token, int64_t stride_head, int num_q_heads,
                       int num_kv_heads, int page_size, float sm_scale,
                       const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ sel_phys,
                       const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count,
                       int max_budget, int num_splits, float* __restrict__ part_o,
-                      float* __restrict__ part_lse) {
+                      float* __restrict__ part_lse, float k_scale, float v_scale) {
   constexpr int E = Pair<T>::kElems;
+  static_assert(Pair<TKV>::kElems == E, "q and the pools are read with the same channels per lane");
+  sm_scale *= k_scale;                           // logits = sm_scale * q . (k_scale * decode(code))
   constexpr int NK = D / (kWarp * E);            // 4-byte loads per lane per K row
   constexpr int NV = DV / (kWarp * E);
   static_assert(D % (kWarp * E) == 0 && DV % (kWarp * E) == 0, "row width must be a multiple of 128 B / 64 B");
@@ -82,14 +96,14 @@ decode_generic_kernel(const T* __restrict__ q, const T* __restrict__ kpool, cons
   for (int r = r_begin; r < r_end; ++r) {
     const int64_t phys = phys_list[r];
     const int valid = min(page_size, n_tok - log_list[r] * page_size);
-    const T* kbase = kpool + phys * stride_page + kvh * stride_head;
-    const T* vbase = vpool + phys * stride_page + kvh * stride_head;
+    const TKV* kbase = kpool + phys * stride_page + kvh * stride_head;
+    const TKV* vbase = vpool + phys * stride_page + kvh * stride_head;
     for (int t = wt; t < valid; t += WT) {
       float kf[NK * E];
 #pragma unroll
       for (int c = 0; c < NK; ++c) {
         float f[E];
-        Pair<T>::load(kbase + t * stride_token + (c * kWarp + lane) * E, f);
+        Pair<TKV>::load(kbase + t * stride_token + (c * kWarp + lane) * E, f);
 #pragma unroll
         for (int e = 0; e < E; ++e) kf[c * E + e] = f[e];
       }
@@ -97,7 +111,7 @@ decode_generic_kernel(const T* __restrict__ q, const T* __restrict__ kpool, cons
 #pragma unroll
       for (int c = 0; c < NV; ++c) {
         float f[E];
-        Pair<T>::load(vbase + t * stride_token + (c * kWarp + lane) * E, f);
+        Pair<TKV>::load(vbase + t * stride_token + (c * kWarp + lane) * E, f);
 #pragma unroll
         for (int e = 0; e < E; ++e) vf[c * E + e] = f[e];
       }
@@ -123,7 +137,7 @@ decode_generic_kernel(const T* __restrict__ q, const T* __restrict__ kpool, cons
   for (int h = 0; h < HPW; ++h) {
     if (h >= n_heads) break;
     const int64_t row = ((int64_t)i * num_q_heads + h0 + h) * n_part + part;
-    const float inv = l[h] > 0.f ? 1.f / l[h] : 0.f;
+    const float inv = l[h] > 0.f ? v_scale / l[h] : 0.f;
 #pragma unroll
     for (int c = 0; c < NV; ++c)
 #pragma unroll
@@ -178,7 +192,7 @@ static int pick_splits(const vx_ctx* c, int batch, int max_budget, int wt, int m
   return s < 1 ? 1 : s;
 }
 
-template <typename T, int D, int DV, int HPW, int WT>
+template <typename T, typename TKV, int D, int DV, int HPW, int WT>
 static cudaError_t launch_generic_t(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                     const int32_t* sel_phys, const int32_t* sel_logical,
                                     const int32_t* sel_count, int32_t max_budget, void* out, float* lse,
@@ -189,10 +203,12 @@ static cudaError_t launch_generic_t(vx_ctx* c, const void* q, const vx_kv_pool& 
   const int splits = pick_splits(c, pt.batch, max_budget, WT, 2);
   dim3 grid(splits, g.num_kv_heads, pt.batch);
   const void* v = g.kv_shared ? pool.k : pool.v;
-  decode_generic_kernel<T, D, DV, HPW, WT><<<grid, wh * WT * kWarp, 0, s>>>(
-      static_cast<const T*>(q), static_cast<const T*>(pool.k), static_cast<const T*>(v), pool.stride_page,
+  const bool fp8 = kv_is_fp8(g);
+  decode_generic_kernel<T, TKV, D, DV, HPW, WT><<<grid, wh * WT * kWarp, 0, s>>>(
+      static_cast<const T*>(q), static_cast<const TKV*>(pool.k), static_cast<const TKV*>(v), pool.stride_page,
       pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads, g.page_size, g.sm_scale,
-      pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits, c->ws.part_o, c->ws.part_lse);
+      pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits, c->ws.part_o, c->ws.part_lse,
+      fp8 ? pool.k_scale : 1.f, fp8 ? (g.kv_shared ? pool.k_scale : pool.v_scale) : 1.f);
   c->launches += 1;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
@@ -218,7 +234,7 @@ cudaError_t launch_decode_gqa(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
   if (gqa_mma_supported(g))
     return launch_decode_gqa_mma(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt);
 #define VX_GO(T, D, HPW, WT) \
-  return launch_generic_t<T, D, D, HPW, WT>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s)
+  return launch_generic_t<T, T, D, D, HPW, WT>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s)
   if (g.dtype == VX_DT_F32) {
     if (g.qk_dim == 64) VX_GO(float, 64, 8, 4);
     if (g.qk_dim == 128) VX_GO(float, 128, 8, 4);
@@ -236,8 +252,28 @@ cudaError_t launch_decode_mla(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
   if (mla_tc_supported(c->g))
     return launch_decode_mla_tc(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt);
   // CUDA-core fallback: 32 heads = 8 head-groups of 4 per CTA, one token slice: 8 warps
-  return launch_generic_t<__nv_bfloat16, 576, 512, 4, 1>(c, q, pool, pt, sel_phys, sel_logical, sel_count,
-                                                         max_budget, out, lse, s);
+  return launch_generic_t<__nv_bfloat16, __nv_bfloat16, 576, 512, 4, 1>(c, q, pool, pt, sel_phys, sel_logical, sel_count,
+                                                                        max_budget, out, lse, s);
+}
+
+// fp8 KV cache (vx_kv_format): the generic kernels with one-byte pool elements converted in registers
+template <typename TKV>
+static cudaError_t launch_decode_fp8_t(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                                       const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
+                                       int32_t max_budget, void* out, float* lse, cudaStream_t s) {
+  const vx_geom& g = c->g;
+  typedef __nv_bfloat16 B;
+  if (g.kv_shared) return launch_generic_t<B, TKV, 576, 512, 4, 1>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
+  if (g.qk_dim == 64) return launch_generic_t<B, TKV, 64, 64, 8, 4>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
+  if (g.qk_dim == 128) return launch_generic_t<B, TKV, 128, 128, 8, 4>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
+  return cudaErrorInvalidValue;
+}
+cudaError_t launch_decode_fp8(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                              const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
+                              int32_t max_budget, void* out, float* lse, cudaStream_t s) {
+  return c->g.kv_format == VX_KV_FP8_E4M3
+             ? launch_decode_fp8_t<fp8_e4m3>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s)
+             : launch_decode_fp8_t<fp8_e5m2>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s);
 }
 
 
@@ -315,10 +351,10 @@ static vx_status launch_generic_static_t(const vx_geom& g, const void* q, const 
   float* part_lse = reinterpret_cast<float*>(static_cast<unsigned char*>(scratch) + o_bytes);
   dim3 grid(splits, g.num_kv_heads, pt.batch);
   const void* v = g.kv_shared ? pool.k : pool.v;
-  decode_generic_kernel<T, D, DV, HPW, WT><<<grid, wh * WT * kWarp, 0, s>>>(
+  decode_generic_kernel<T, T, D, DV, HPW, WT><<<grid, wh * WT * kWarp, 0, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(pool.k), static_cast<const T*>(v), pool.stride_page,
       pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads, g.page_size, g.sm_scale,
-      pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits, part_o, part_lse);
+      pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits, part_o, part_lse, 1.f, 1.f);
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) {
     combine_kernel<T><<<(unsigned)rows, 128, 0, s>>>(part_o, part_lse, n_part, g.v_dim, static_cast<T*>(out), lse);
@@ -347,6 +383,7 @@ vx_status vx_sparse_paged_decode_static(const vx_geom* g, const void* q, const v
   if (!g->kv_shared && !pool->v) return static_fail(VX_ERR_INVALID_ARG, "kv pool v is NULL");
   if (pt->batch < 0 || (pt->batch > 0 && !pt->seq_lens)) return static_fail(VX_ERR_INVALID_ARG, "bad page table");
   if (max_budget <= 0) return static_fail(VX_ERR_INVALID_ARG, "max_budget must be positive");
+  if (g->kv_format != VX_KV_SAME) return static_fail(VX_ERR_UNSUPPORTED, "vx_sparse_paged_decode_static takes pools of geom.dtype only");
   if (g->kv_shared ? !mla_geometry_supported(*g) : !gqa_geometry_supported(*g))
     return static_fail(VX_ERR_UNSUPPORTED, "(dtype, qk_dim, v_dim, heads) not supported by the decode kernels");
   if (pt->batch == 0) return VX_OK;

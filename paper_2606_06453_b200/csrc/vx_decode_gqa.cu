@@ -330,7 +330,7 @@ VX_TRACE_SETTER(vx_trace_set_decode_gqa)
 
 bool gqa_mma_supported(const vx_geom& g) {
   const int grp = g.num_q_heads / g.num_kv_heads;
-  return g.dtype == VX_DT_BF16 && !g.kv_shared && g.page_size == kGqaPage && g.qk_dim == g.v_dim &&
+  return g.dtype == VX_DT_BF16 && g.kv_format == VX_KV_SAME && !g.kv_shared && g.page_size == kGqaPage && g.qk_dim == g.v_dim &&
          (g.qk_dim == 128 || g.qk_dim == 64) && grp <= 8;
 }
 

@@ -440,7 +440,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
 VX_TRACE_SETTER(vx_trace_set_decode_mla)
 
 bool mla_tc_supported(const vx_geom& g) {
-  return g.kv_shared && g.dtype == VX_DT_BF16 && g.num_kv_heads == 1 && g.qk_dim == mla::D && g.v_dim == mla::DV &&
+  return g.kv_shared && g.dtype == VX_DT_BF16 && g.kv_format == VX_KV_SAME && g.num_kv_heads == 1 && g.qk_dim == mla::D && g.v_dim == mla::DV &&
          g.page_size == mla::PAGE && g.num_q_heads <= mla::NH;
 }
 

@@ -29,6 +29,7 @@ struct Workspace {               // device pointers carved from the caller's wor
   // the flat MLA step kernel (vx_step_mla_flat.cu)
   float* flat_qvec;              // [max_batch, 2 qk_dim] query vectors [Qm | Qp]
   int32_t* flat_sync;            // counters and per-request flags; zero between steps
+  float* fp8_qvec;               // fp8 KV cache: [max_batch, Hkv, 2 qk_dim] query vectors [Qm | Qp] of the score kernel (vx_score_fp8.cu)
   size_t bytes;                  // total
 };
 
@@ -207,6 +208,15 @@ cudaError_t launch_step_mla_flat(vx_ctx* c, const void* q, const vx_kv_pool& poo
 cudaError_t vx_trace_set_step_mla_flat(long long* buf, int ctas);
 cudaError_t launch_combine(vx_ctx* c, int32_t batch, int num_splits, void* out, float* lse,
                            cudaStream_t s);
+
+// fp8 KV cache (vx_kv_format): one-byte K / V / summary elements
+inline bool kv_is_fp8(const vx_geom& g) { return g.kv_format != VX_KV_SAME; }
+inline size_t kv_elem_size(const vx_geom& g) { return kv_is_fp8(g) ? 1 : (g.dtype == VX_DT_BF16 ? 2 : 4); }
+bool fp8_geometry_supported(const vx_geom& g);
+cudaError_t launch_score_fp8(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt, float* scores, cudaStream_t s);
+cudaError_t launch_decode_fp8(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                              const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
+                              int32_t max_budget, void* out, float* lse, cudaStream_t s);
 
 // geometry support predicates (used by vx_create validation)
 bool gqa_geometry_supported(const vx_geom& g);

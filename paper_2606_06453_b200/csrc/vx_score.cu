@@ -487,6 +487,7 @@ cudaError_t launch_page_score(vx_ctx* c, const void* q, const void* summary, con
                               float* scores, cudaStream_t s, const ReqRange& rr) {
   if (pt.batch == 0 || pt.total_pages == 0) return cudaSuccess;
   const vx_geom& g = c->g;
+  if (kv_is_fp8(g)) return launch_score_fp8(c, q, summary, pt, scores, s);
   if (score_mla_max_supported(g)) return launch_score_mla_max(c, q, summary, pt, scores, s, rr);
   if (g.dtype == VX_DT_BF16) {
     switch (g.qk_dim) {

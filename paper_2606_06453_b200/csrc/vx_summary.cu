@@ -137,6 +137,8 @@ static cudaError_t launch_summary_t(vx_ctx* c, const vx_kv_pool& pool, const vx_
 
 cudaError_t launch_summary_update(vx_ctx* c, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* first_new_pos, void* summary, cudaStream_t s) {
+  if (c->g.kv_format == VX_KV_FP8_E4M3) return launch_summary_t<fp8_e4m3>(c, pool, pt, first_new_pos, summary, s);
+  if (c->g.kv_format == VX_KV_FP8_E5M2) return launch_summary_t<fp8_e5m2>(c, pool, pt, first_new_pos, summary, s);
   if (c->g.dtype == VX_DT_BF16) return launch_summary_t<__nv_bfloat16>(c, pool, pt, first_new_pos, summary, s);
   return launch_summary_t<float>(c, pool, pt, first_new_pos, summary, s);
 }
