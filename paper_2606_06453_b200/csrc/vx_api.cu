@@ -332,6 +332,9 @@ static vx_status decode_dispatch(vx_ctx* c, const void* q, const vx_kv_pool* poo
                                  const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                                  int32_t max_budget, void* out, float* lse, cudaStream_t s,
                                  const DecodeOpts& opt = DecodeOpts()) {
+  if (gqa_fp8_fast_supported(c->g))
+    return check_cuda(c, launch_decode_gqa_fp8(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s,
+                                               opt.pdl, opt.budget), "vx_sparse_paged_decode (fp8 KV cache)");
   if (kv_is_fp8(c->g))
     return check_cuda(c, launch_decode_fp8(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s),
                       "vx_sparse_paged_decode (fp8 KV cache)");

@@ -36,18 +36,37 @@ qvec_fp8_kernel(const __nv_bfloat16* __restrict__ q, int batch, int num_q_heads,
   }
 }
 
-// NT16 = 16-byte vectors per lane per page = ceil(Hkv * (2 d / 16) / 32)
+// NT16 = 16-byte vectors per lane per page = ceil(Hkv * (2 d / 16) / 32).  Every warp streams its own pages (begin + warp,
+// + 8, ..) through a private ring of STAGES page slots filled by 16-byte cp.async copies -- the bytes in flight cost
+// shared memory, not registers -- with the page ids fetched 32 at a time (one coalesced load per warp).
+constexpr int kS8Warps = 8, kS8Stages = 4;
 template <typename T, int NT16>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(kS8Warps * kWarp, 3)
 score_fp8_kernel(const uint8_t* __restrict__ summary, const float* __restrict__ qvec, const int32_t* __restrict__ page_indptr,
                  const int32_t* __restrict__ page_indices, int batch, int total_pages, int num_kv_heads, int d,
                  float* __restrict__ scores) {
-  const int lane = threadIdx.x % kWarp, warp = threadIdx.x / kWarp, nwarp = blockDim.x / kWarp;
+  extern __shared__ __align__(128) uint8_t s8_smem[];
+  const int lane = threadIdx.x % kWarp, warp = threadIdx.x / kWarp;
   const int rowv = 2 * d / 16;                           // vectors per (page, head) row
   const int pagev = num_kv_heads * rowv;                 // vectors per page
   const int64_t page_bytes = (int64_t)pagev * 16;
+  constexpr int SLOT = NT16 * kWarp * 16;                // bytes of a page slot
   const int begin = (int)((int64_t)total_pages * blockIdx.x / gridDim.x);
   const int end = (int)((int64_t)total_pages * (blockIdx.x + 1) / gridDim.x);
+  const int my_pages = end - begin > warp ? (end - begin - warp + kS8Warps - 1) / kS8Warps : 0;
+  uint8_t* ring = s8_smem + (size_t)warp * kS8Stages * SLOT;
+  int ids = 0;                                           // lane l: physical id of my (base + l)-th page
+  auto fetch_ids = [&](int base) {
+    const int p = base + lane;
+    if (p < my_pages) ids = page_indices[begin + warp + p * kS8Warps];
+  };
+  auto issue = [&](int p) {
+    const int phys = __shfl_sync(0xffffffffu, ids, p & 31);
+    const uint8_t* src = summary + (int64_t)phys * page_bytes + lane * 16;
+#pragma unroll
+    for (int t = 0; t < NT16; ++t)
+      if (lane + t * kWarp < pagev) cp_async16(ring + (size_t)(p % kS8Stages) * SLOT + (lane + t * kWarp) * 16, src + t * kWarp * 16);
+  };
   float qreg[NT16][16];
   int cur_req = -1, cur_end = 0;                         // the request whose query vector is in qreg; its last flat page + 1
   auto load_qreg = [&](int flat) {
@@ -74,23 +93,33 @@ score_fp8_kernel(const uint8_t* __restrict__ summary, const float* __restrict__ 
       }
     }
   };
-  auto load_page = [&](int flat, uint4 (&v)[NT16]) {
-    const uint8_t* src = summary + (int64_t)page_indices[flat] * page_bytes;
+  fetch_ids(0);
 #pragma unroll
-    for (int t = 0; t < NT16; ++t)
-      v[t] = lane + t * kWarp < pagev ? ldg_stream(src + (lane + t * kWarp) * 16) : make_uint4(0, 0, 0, 0);
-  };
-  auto finish_page = [&](int flat, const uint4 (&v)[NT16]) {
-    if (flat >= cur_end || cur_req < 0) load_qreg(flat);         // (warp-uniform)
+  for (int p = 0; p < kS8Stages - 1; ++p) {
+    if (p < my_pages) issue(p);
+    cp_async_commit();
+  }
+  for (int p = 0; p < my_pages; ++p) {
+    const int flat = begin + warp + p * kS8Warps;
+    if (flat >= cur_end || cur_req < 0) load_qreg(flat);          // (warp-uniform)
+    cp_async_wait<kS8Stages - 2>();                      // page p has landed (this lane's copies; a lane reads only its own)
     float part[NT16];
 #pragma unroll
     for (int t = 0; t < NT16; ++t) {
+      const uint4 v = lane + t * kWarp < pagev ? *reinterpret_cast<const uint4*>(ring + (size_t)(p % kS8Stages) * SLOT + (lane + t * kWarp) * 16)
+                                              : make_uint4(0, 0, 0, 0);
       float f[16];
-      Elem<T>::unpack(v[t], f);
+      Elem<T>::unpack(v, f);
       float acc = 0.f;
 #pragma unroll
       for (int e = 0; e < 16; ++e) acc = fmaf(qreg[t][e], f[e], acc);
       part[t] = acc;
+    }
+    {
+      const int nxt = p + kS8Stages - 1;                 // refill the slot page p - 1 used (this lane read it an iteration ago)
+      if ((nxt & 31) == 0 && nxt < my_pages) fetch_ids(nxt);
+      if (nxt < my_pages) issue(nxt);
+      cp_async_commit();
     }
     if (num_kv_heads == 1) {                             // one (latent) head: the whole page is one row
       float tot = 0.f;
@@ -107,15 +136,160 @@ score_fp8_kernel(const uint8_t* __restrict__ summary, const float* __restrict__ 
         if (v0 < pagev && v0 % rowv == 0) scores[(int64_t)(v0 / rowv) * total_pages + flat] = x;
       }
     }
-  };
-  for (int p0 = begin + warp; p0 < end; p0 += 2 * nwarp) {       // two pages in flight per warp
-    const int p1 = p0 + nwarp;
-    uint4 va[NT16], vb[NT16];
-    load_page(p0, va);
-    if (p1 < end) load_page(p1, vb);
-    finish_page(p0, va);
-    if (p1 < end) finish_page(p1, vb);
   }
+  cp_async_wait<0>();
+}
+
+// ---- the same scores on the tensor cores, for the GQA geometry the configs use (8 KV heads, d = 128: a page's summary chunk
+// is [8 heads][256 B]).  The CUDA-core kernel above is ISSUE-bound on this format (ncu: 67 % issue slots busy at 26 % of
+// the DRAM peak -- every byte is an element that costs a conversion and an FMA), so the dot products go to
+// mma.m16n8k16: an A tile is 16 rows = 2 pages x 8 heads of one 16-channel chunk (ldmatrix straight from the staged
+// codes, widened to f16 by cvt.rn.f16x2.*: 0.5 LDSM + 4 F2FP + 2 HMMA per 256 elements against ~20 instructions), the B
+// operand holds the 8 heads' query vectors as the 8 columns, split into an f16 high and low part (q = hi + lo to 2^-22;
+// a power-of-two pre-scale keeps it inside the f16 range), and row r reads its score from column r % 8 of fp32 D.
+constexpr int kM8Warps = 8, kM8Stages = 3, kM8TileBytes = 2 * 2048;
+template <typename T> __device__ __forceinline__ void s8_cvt4(uint32_t four, uint32_t& lo, uint32_t& hi);
+template <> __device__ __forceinline__ void s8_cvt4<fp8_e4m3>(uint32_t four, uint32_t& lo, uint32_t& hi) {
+  asm("{\n\t.reg .b16 l, h;\n\tmov.b32 {l, h}, %2;\n\tcvt.rn.f16x2.e4m3x2 %0, l;\n\tcvt.rn.f16x2.e4m3x2 %1, h;\n\t}"
+      : "=r"(lo), "=r"(hi) : "r"(four));
+}
+template <> __device__ __forceinline__ void s8_cvt4<fp8_e5m2>(uint32_t four, uint32_t& lo, uint32_t& hi) {
+  asm("{\n\t.reg .b16 l, h;\n\tmov.b32 {l, h}, %2;\n\tcvt.rn.f16x2.e5m2x2 %0, l;\n\tcvt.rn.f16x2.e5m2x2 %1, h;\n\t}"
+      : "=r"(lo), "=r"(hi) : "r"(four));
+}
+template <typename T>
+__global__ void __launch_bounds__(kM8Warps * kWarp, 2)
+score_fp8_mma_kernel(const uint8_t* __restrict__ summary, const float* __restrict__ qvec, const int32_t* __restrict__ page_indptr,
+                     const int32_t* __restrict__ page_indices, int batch, int total_pages, float* __restrict__ scores) {
+  constexpr int HKV = 8, ROW = 256, PAGEB = HKV * ROW, NCH = ROW / 16;      // 16 chunks of 16 codes per row
+  extern __shared__ __align__(128) uint8_t s8_smem[];
+  const int lane = threadIdx.x % kWarp, warp = threadIdx.x / kWarp;
+  const int g = lane >> 2, j = lane & 3;
+  const int begin = (int)((int64_t)total_pages * blockIdx.x / gridDim.x);
+  const int end = (int)((int64_t)total_pages * (blockIdx.x + 1) / gridDim.x);
+  const int n_tiles = (end - begin + 1) / 2;              // tiles of 2 consecutive flat pages
+  const int my_tiles = n_tiles > warp ? (n_tiles - warp + kM8Warps - 1) / kM8Warps : 0;
+  auto tile_page0 = [&](int p) -> int { return begin + 2 * (warp + kM8Warps * p); };
+  const uint32_t ring = smem_u32(s8_smem) + (uint32_t)warp * kM8Stages * kM8TileBytes;
+  int ids = 0;                                            // lane l: page l % 2 of my (base + l / 2)-th tile
+  auto fetch_ids = [&](int base) {
+    const int flat = tile_page0(base + (lane >> 1)) + (lane & 1);
+    ids = (base + (lane >> 1) < my_tiles && flat < end) ? page_indices[flat] : -1;
+  };
+  auto issue = [&](int p) {
+    const uint32_t dst = ring + (uint32_t)(p % kM8Stages) * kM8TileBytes;
+#pragma unroll
+    for (int pg = 0; pg < 2; ++pg) {
+      const int phys = __shfl_sync(0xffffffffu, ids, 2 * (p & 15) + pg);
+      if (phys >= 0) {
+        const uint8_t* src = summary + (int64_t)phys * PAGEB;
+#pragma unroll
+        for (int it = 0; it < 4; ++it) {                  // 128 granules of 16 B per page
+          const int x = lane + it * kWarp, head = x >> 4, c = x & 15;
+          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + pg * PAGEB + head * ROW + ((c ^ head) << 4)), "l"(src + x * 16));
+        }
+      }
+    }
+  };
+  // B operand: thread (column = head g, j) holds for chunk c the channels 16 c + 4 j .. + 3 of head g's [Qm | Qp]
+  uint32_t qh[NCH][2], ql[NCH][2];
+  float q_up = 1.f;
+  int cur_req = -1, cur_end = 0;
+  auto load_qreg = [&](int flat) {
+    int lo = 0, hi = batch;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (page_indptr[mid] <= flat) lo = mid; else hi = mid;
+    }
+    cur_req = lo;
+    cur_end = page_indptr[lo + 1];
+    const float4* src = reinterpret_cast<const float4*>(qvec + ((int64_t)lo * HKV + g) * ROW) + j;
+    float mx = 0.f;
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+      const float4 x = src[4 * c];
+      mx = fmaxf(fmaxf(mx, fmaxf(fabsf(x.x), fabsf(x.y))), fmaxf(fabsf(x.z), fabsf(x.w)));
+    }
+    mx = warp_max(mx);
+    const int e2 = mx > 16384.f ? ilogbf(mx) - 13 : 0;
+    const float down = exp2f((float)-e2);
+    q_up = exp2f((float)e2);
+#pragma unroll
+    for (int c = 0; c < NCH; ++c) {
+      const float4 x = src[4 * c];
+      const float v[4] = {x.x * down, x.y * down, x.z * down, x.w * down};
+      __half h[4], l[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        h[e] = __float2half_rn(v[e]);
+        l[e] = __float2half_rn(v[e] - __half2float(h[e]));
+      }
+      qh[c][0] = (uint32_t)__half_as_ushort(h[0]) | ((uint32_t)__half_as_ushort(h[1]) << 16);
+      qh[c][1] = (uint32_t)__half_as_ushort(h[2]) | ((uint32_t)__half_as_ushort(h[3]) << 16);
+      ql[c][0] = (uint32_t)__half_as_ushort(l[0]) | ((uint32_t)__half_as_ushort(l[1]) << 16);
+      ql[c][1] = (uint32_t)__half_as_ushort(l[2]) | ((uint32_t)__half_as_ushort(l[3]) << 16);
+    }
+  };
+  // rows of the A tile: r = lane & 15 -> page r / 8, head r % 8; lanes 16..31 address the odd chunk of a pair
+  const uint32_t row_off = (uint32_t)(((lane & 15) >> 3) * PAGEB + (lane & 7) * ROW);
+  auto compute = [&](int p, float& s_page0, float& s_page1) {
+    const uint32_t slot = ring + (uint32_t)(p % kM8Stages) * kM8TileBytes + row_off;
+    float dh[4] = {0.f, 0.f, 0.f, 0.f}, dl[4] = {0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+    for (int cc = 0; cc < NCH / 2; ++cc) {
+      uint32_t r[4];
+      const int c = 2 * cc + (lane >> 4);
+      asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                   : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]) : "r"(slot + (uint32_t)((c ^ (lane & 7)) << 4)));
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {                       // chunk 2 cc + u: r[2u] = rows 0..7, r[2u + 1] = rows 8..15
+        uint32_t a0, a1, a2, a3;
+        s8_cvt4<T>(r[2 * u], a0, a2);
+        s8_cvt4<T>(r[2 * u + 1], a1, a3);
+        asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                     : "+f"(dh[0]), "+f"(dh[1]), "+f"(dh[2]), "+f"(dh[3])
+                     : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(qh[2 * cc + u][0]), "r"(qh[2 * cc + u][1]));
+        asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                     : "+f"(dl[0]), "+f"(dl[1]), "+f"(dl[2]), "+f"(dl[3])
+                     : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(ql[2 * cc + u][0]), "r"(ql[2 * cc + u][1]));
+      }
+    }
+    // D[row][col]: this thread holds rows g, g + 8 x columns 2 j, 2 j + 1; row g / g + 8 = head g wants column g
+    const bool odd = g & 1;
+    s_page0 = ((odd ? dh[1] : dh[0]) + (odd ? dl[1] : dl[0])) * q_up;
+    s_page1 = ((odd ? dh[3] : dh[2]) + (odd ? dl[3] : dl[2])) * q_up;
+  };
+  fetch_ids(0);
+#pragma unroll
+  for (int p = 0; p < kM8Stages - 1; ++p) {
+    if (p < my_tiles) issue(p);
+    cp_async_commit();
+  }
+  for (int p = 0; p < my_tiles; ++p) {
+    const int flat0 = tile_page0(p), flat1 = flat0 + 1;
+    if (flat0 >= cur_end || cur_req < 0) load_qreg(flat0);         // (warp-uniform)
+    cp_async_wait<kM8Stages - 2>();
+    __syncwarp();                                         // every lane's copies of tile p have landed
+    float s0, s1;
+    compute(p, s0, s1);
+    const bool mine = j == (g >> 1);                      // the thread that holds column g of rows g, g + 8
+    if (mine) scores[(int64_t)g * total_pages + flat0] = s0;
+    if (flat1 < end) {
+      if (flat1 >= cur_end) {                             // the tile straddles two requests: page 1 again with its own query
+        load_qreg(flat1);
+        compute(p, s0, s1);
+      }
+      if (mine) scores[(int64_t)g * total_pages + flat1] = s1;
+    }
+    __syncwarp();                                         // all lanes are done with tile p's slot group before it is refilled
+    {
+      const int nxt = p + kM8Stages - 1;
+      if ((nxt & 15) == 0 && nxt < my_tiles) fetch_ids(nxt);
+      if (nxt < my_tiles) issue(nxt);
+      cp_async_commit();
+    }
+  }
+  cp_async_wait<0>();
 }
 
 bool fp8_geometry_supported(const vx_geom& g) {
@@ -139,13 +313,28 @@ static cudaError_t launch_score_fp8_t(vx_ctx* c, const void* q, const void* summ
                                      c->ws.fp8_qvec);
   c->launches += 1;
   if (cudaError_t e = cudaGetLastError()) return e;
+  if (g.num_kv_heads == 8 && g.qk_dim == 128) {         // the tensor-core kernel
+    constexpr int smem_bytes = kM8Warps * kM8Stages * kM8TileBytes;
+    if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(score_fp8_mma_kernel<T>), c->device, smem_bytes)) return e;
+    int grid = c->num_sms * 2;
+    if (grid > (pt.total_pages + 1) / 2) grid = (pt.total_pages + 1) / 2;
+    score_fp8_mma_kernel<T><<<grid, kM8Warps * kWarp, smem_bytes, s>>>(static_cast<const uint8_t*>(summary), c->ws.fp8_qvec,
+                                                                      pt.page_indptr, pt.page_indices, pt.batch, pt.total_pages, scores);
+    c->launches += 1;
+    return cudaGetLastError();
+  }
   const int pagev = g.num_kv_heads * (2 * g.qk_dim / 16);
   const int nt16 = (pagev + kWarp - 1) / kWarp;
-  int grid = c->num_sms * 4;                             // 4 CTAs of 8 warps per SM: 64 pages in flight per SM
+  int grid = c->num_sms * 3;                             // 3 CTAs of 8 warps per SM, 3 pages in flight per warp
   if (grid > pt.total_pages) grid = pt.total_pages;
   const uint8_t* sm = static_cast<const uint8_t*>(summary);
-#define VX_GO(N) score_fp8_kernel<T, N><<<grid, 256, 0, s>>>(sm, c->ws.fp8_qvec, pt.page_indptr, pt.page_indices, pt.batch, \
-                                                             pt.total_pages, g.num_kv_heads, g.qk_dim, scores)
+#define VX_GO(N)                                                                                                            \
+  do {                                                                                                                      \
+    constexpr int smem_bytes = kS8Warps * kS8Stages * N * kWarp * 16;                                                       \
+    if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(score_fp8_kernel<T, N>), c->device, smem_bytes)) return e; \
+    score_fp8_kernel<T, N><<<grid, kS8Warps * kWarp, smem_bytes, s>>>(sm, c->ws.fp8_qvec, pt.page_indptr, pt.page_indices,  \
+                                                                     pt.batch, pt.total_pages, g.num_kv_heads, g.qk_dim, scores); \
+  } while (0)
   switch (nt16) {
     case 1: VX_GO(1); break;
     case 2: VX_GO(2); break;
