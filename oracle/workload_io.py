@@ -6,7 +6,27 @@ from oracle import vx_oracle as vo
 
 
 def to_oracle(w):
-    """Workload (any device) -> (q, Pool, PageTable) numpy views on CPU copies."""
+    """Workload (any device) -> (q, Pool, PageTable) numpy views on CPU copies.  With selection blocks finer than the page
+    (spec.block_size) the pool and the table are the BLOCK-level ones of oracle/vx_oracle_blocks.py (page_size = block size)."""
+    q, pool, pt = _to_oracle_pages(w)
+    bs = getattr(w.spec, "block_size", 0)
+    if bs and bs != w.spec.page_size:
+        from oracle.vx_oracle_blocks import block_problem
+        pool, pt = block_problem(pool, pt, bs, w.spec.num_kv_heads, w.spec.qk_dim, w.spec.v_dim)
+    return q, pool, pt
+
+
+def block_table(w):
+    """(indptr, indices) of the selection units of a workload: the page table, or its expansion into blocks (G28)"""
+    indptr, indices = vo.as_np(w.page_indptr).astype(np.int64), vo.as_np(w.page_indices).astype(np.int64)
+    bs = getattr(w.spec, "block_size", 0)
+    if bs and bs != w.spec.page_size:
+        bpp = w.spec.page_size // bs
+        return indptr * bpp, (indices[:, None] * bpp + np.arange(bpp)[None, :]).reshape(-1)
+    return indptr, indices
+
+
+def _to_oracle_pages(w):
     sp, st, sh = w.strides
     if getattr(w.spec, "kv_dtype", ""):                  # fp8 KV cache: the doubles scale * decode(code) (vx_oracle_fp8.py)
         from oracle.vx_oracle_fp8 import pool_fp8

@@ -13,7 +13,6 @@
 //   * Q is converted bf16 -> f16 once (exact in the f16 normal range; a power-of-two pre-scale, folded back into the
 //     softmax scale, keeps |q| below 2^15 whatever the queries are);  P is rounded to f16 (11 bits) for the second MMA;
 //   * k_scale rides in the softmax scale, v_scale in the final normalisation.
-#include <cstdlib>
 #include "vx_common.cuh"
 #include "vx_internal.h"
 
@@ -299,11 +298,12 @@ static int decode_gqa_fp8_splits(const vx_ctx* c, int n_req, int max_budget) {
   const int units = n_req * c->g.num_kv_heads;
   const int per_sm = 227 * 1024 / (gq8::SMEM + 1024);
   const int slots = c->num_sms * (per_sm > 0 ? per_sm : 1);
-  if (const char* ev = getenv("VX_TMP_FP8_SPLITS")) return atoi(ev);
   int splits = 1, best_cost = 1 << 30;
   for (int sp = 1; sp <= kMaxSplits && sp <= max_budget; ++sp) {
     const int waves = (units * sp + slots - 1) / slots;
-    const int cost = waves * (((max_budget + sp - 1) / sp + gq8::WARPS - 1) / gq8::WARPS + 3);
+    // a wave costs its pages per warp plus ~30 page times that stream nothing (measured on C2 / C3: launch, Q and id
+    // loads, first-page latency, in-CTA and cross-split merge ~ 15 us against 0.5 us per page and warp)
+    const int cost = waves * (((max_budget + sp - 1) / sp + gq8::WARPS - 1) / gq8::WARPS + 30);
     if (cost < best_cost) { best_cost = cost; splits = sp; }
   }
   return splits;

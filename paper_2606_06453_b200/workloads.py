@@ -41,6 +41,8 @@ class Spec:
     pool_slack: int = 64       # unused physical pages in the pool
     pool_pages: int = 0        # fixed pool size (C1: 128), 0 -> total + slack
     cfg_id: int = 0            # seeds: 1000+id data, 2000+id permutation, 3000+id lengths, 4000+id planted
+    block_size: int = 0        # selection block finer than the page: 0 = the page; must divide page_size.
+                               # budget, n_sink and n_local then count BLOCKS
     kv_dtype: str = ""         # "" = pools in `dtype`; "e4m3" / "e5m2" = fp8 KV cache: uint8 code pools
 
     @property
@@ -134,10 +136,11 @@ def make_workload(spec: Spec | str, device="cpu", seed_offset: int = 0) -> Workl
     indptr = torch.zeros(spec.batch + 1, dtype=torch.int64)
     indptr[1:] = torch.cumsum(pages, 0)
     total = int(indptr[-1])
+    units = pages if not spec.block_size else (seq + spec.block_size - 1) // spec.block_size     # what the budget counts
     if spec.budget > 0:
         budget = torch.full((spec.batch,), spec.budget, dtype=torch.int64)
     else:
-        budget = torch.clamp((pages.double() * spec.budget_frac).floor().long(), min=spec.budget_min)
+        budget = torch.clamp((units.double() * spec.budget_frac).floor().long(), min=spec.budget_min)
     max_budget = int(budget.max())
 
     # shuffled shared pool: a global seeded permutation dealt to requests in order

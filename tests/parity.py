@@ -39,8 +39,8 @@ def check_selection(w, gpu_logical, gpu_phys, gpu_count, ref, label=None):
     of it the exception is BOUNDED: a problem may not swap more pages than the oracle itself finds inside the fp32 rounding
     band (FP32_BAND) around its threshold -- a kernel that mis-ranks pages 5e-4 apart passes the rule but not the ceiling."""
     sl, sp, sc = (np.asarray(t) for t in (gpu_logical, gpu_phys, gpu_count))
-    indptr = np.asarray(w.page_indptr.cpu())
-    indices = np.asarray(w.page_indices.cpu())
+    from oracle.workload_io import block_table
+    indptr, indices = block_table(w)                     # pages, or blocks finer than the page (physical block ids)
     assert np.array_equal(sc, ref["sel_count"]), "sel_count differs"
     st = SelectionStats(problems=0, excepted=0, swapped_pages=0, fp32_band_pages=0, max_rel=0.0)
     for i in range(sc.shape[0]):
