@@ -94,6 +94,14 @@ typedef struct {
   int32_t agg;          /* vx_agg */
   int32_t summary_kind; /* vx_summary_kind */
   int32_t kv_format;    /* vx_kv_format: storage of the K, V and summary pools (0 = elements of dtype) */
+  int32_t block_size;   /* selection block b_s in tokens (PAPER.md:518-519 `block_size: 16` inside `page_size: 32`; :202):
+                         * 0 or page_size = the page; otherwise it must divide page_size.  A block is b_s consecutive tokens
+                         * inside one physical page; everything the calls below do per page they then do per BLOCK:
+                         * summaries are [num_pool_pages * (page_size / b_s), Hkv, ..] addressed by the physical block id
+                         * page id * (page_size / b_s) + block in page, scores are [Hkv, total_pages * (page_size / b_s)]
+                         * (request i's blocks start at page_indptr[i] * page_size / b_s), budget / n_sink / n_local count
+                         * blocks, sel_logical / sel_phys hold logical / physical block ids.  The page table stays the
+                         * caller's page table (G28).  Fast decode kernels: GQA with b_s = 16. */
 } vx_geom;
 
 typedef struct {

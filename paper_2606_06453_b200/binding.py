@@ -36,7 +36,7 @@ class VxGeom(C.Structure):
     _fields_ = [("dtype", C.c_int32), ("num_q_heads", C.c_int32), ("num_kv_heads", C.c_int32),
                 ("qk_dim", C.c_int32), ("v_dim", C.c_int32), ("page_size", C.c_int32),
                 ("kv_shared", C.c_int32), ("sm_scale", C.c_float), ("n_sink", C.c_int32),
-                ("n_local", C.c_int32), ("agg", C.c_int32), ("summary_kind", C.c_int32), ("kv_format", C.c_int32)]
+                ("n_local", C.c_int32), ("agg", C.c_int32), ("summary_kind", C.c_int32), ("kv_format", C.c_int32), ("block_size", C.c_int32)]
 
 
 class VxPageTable(C.Structure):
@@ -138,14 +138,14 @@ class Context:
     """One geometry on one device; owns its workspace tensor."""
 
     def __init__(self, *, dtype, num_q_heads, num_kv_heads, qk_dim, v_dim, page_size, sm_scale,
-                 n_sink, n_local, kv_shared=False, agg=VX_AGG_SUM, summary_kind=VX_SUMMARY_ENVELOPE, kv_format=0, max_batch,
+                 n_sink, n_local, kv_shared=False, agg=VX_AGG_SUM, summary_kind=VX_SUMMARY_ENVELOPE, kv_format=0, block_size=0, max_batch,
                  max_total_pages,
                  max_pages_per_req, max_budget, device="cuda:0"):
         self.lib = load_library()
         self.torch_dtype = dtype
         dt = {torch.bfloat16: VX_DT_BF16, torch.float32: VX_DT_F32}[dtype]
         self.geom = VxGeom(dt, num_q_heads, num_kv_heads, qk_dim, v_dim, page_size, int(kv_shared),
-                           float(sm_scale), n_sink, n_local, agg, summary_kind, int(kv_format))
+                           float(sm_scale), n_sink, n_local, agg, summary_kind, int(kv_format), int(block_size))
         self.device = torch.device(device)
         self.max = (int(max_batch), int(max_total_pages), int(max_pages_per_req), int(max_budget))
         need = self.lib.vx_workspace_bytes(C.byref(self.geom), *self.max)
@@ -260,6 +260,7 @@ def context_for(w, device=None, **over) -> Context:
               sm_scale=s.sm_scale, n_sink=s.n_sink, n_local=s.n_local, kv_shared=s.kv_shared,
               max_batch=s.batch, max_total_pages=w.total_pages, max_pages_per_req=w.max_pages_per_req,
               max_budget=w.max_budget, device=device or w.q.device,
+              block_size=getattr(s, "block_size", 0),
               kv_format={"": VX_KV_SAME, "e4m3": VX_KV_FP8_E4M3, "e5m2": VX_KV_FP8_E5M2}[getattr(s, "kv_dtype", "")])
     kw.update(over)
     return Context(**kw)
@@ -274,6 +275,7 @@ def tables_for(w):
 
 def alloc_summary(w, summary_kind=VX_SUMMARY_ENVELOPE):
     s = w.spec
-    shape = (w.num_pool_pages, s.num_kv_heads, s.qk_dim) if summary_kind == VX_SUMMARY_CENTROID else \
-        (w.num_pool_pages, s.num_kv_heads, 2, s.qk_dim)
+    bs = getattr(s, "block_size", 0)
+    n = w.num_pool_pages * (s.page_size // bs if bs else 1)       # one summary per selection block (= page unless finer)
+    shape = (n, s.num_kv_heads, s.qk_dim) if summary_kind == VX_SUMMARY_CENTROID else (n, s.num_kv_heads, 2, s.qk_dim)
     return torch.zeros(shape, dtype=w.k_pool.dtype, device=w.k_pool.device)

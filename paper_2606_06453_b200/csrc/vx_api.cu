@@ -28,7 +28,9 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   };
   const size_t B = (size_t)max_batch, Hq = (size_t)g.num_q_heads, Hkv = (size_t)g.num_kv_heads;
   const size_t esz = elem_size(g.dtype);
-  w.scores = static_cast<float*>(take(Hkv * (size_t)max_total_pages * 4));
+  // (carved from the CALLER's geometry: page_size is the physical page, block_size the selection block)
+  const size_t bpp = (g.block_size > 0 && g.block_size < g.page_size) ? (size_t)(g.page_size / g.block_size) : 1;
+  w.scores = static_cast<float*>(take(Hkv * (size_t)max_total_pages * bpp * 4));
   w.sel_phys = static_cast<int32_t*>(take(B * Hkv * (size_t)max_budget * 4));
   w.sel_logical = static_cast<int32_t*>(take(B * Hkv * (size_t)max_budget * 4));
   w.sel_count = static_cast<int32_t*>(take(B * Hkv * 4));
@@ -46,6 +48,8 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   const bool mla = g.kv_shared != 0;
   w.flat_qvec = static_cast<float*>(take(mla ? step_mla_flat_qvec_floats(max_batch) * 4 : 0));
   w.flat_sync = static_cast<int32_t*>(take(mla ? step_mla_flat_workspace_ints(max_batch) * 4 : 0));
+  w.blk_indptr = static_cast<int32_t*>(take(bpp > 1 ? (B + 1) * 4 : 0));
+  w.blk_indices = static_cast<int32_t*>(take(bpp > 1 ? (size_t)max_total_pages * bpp * 4 : 0));
   w.fp8_qvec = static_cast<float*>(take(kv_is_fp8(g) ? B * Hkv * 2 * (size_t)g.qk_dim * 4 : 0));
   w.bytes = off;
   return w;
@@ -81,6 +85,8 @@ static const char* check_geom(const vx_geom* g, vx_status* st) {
   if (g->qk_dim <= 0 || g->v_dim <= 0 || g->page_size <= 0) return "qk_dim, v_dim, page_size must be positive";
   if (g->n_sink < 0 || g->n_local < 0) return "n_sink, n_local must be >= 0";
   if (g->kv_shared && g->v_dim > g->qk_dim) return "kv_shared needs v_dim <= qk_dim";
+  if (g->block_size < 0 || (g->block_size > 0 && g->page_size % g->block_size != 0))
+    return "block_size must be 0 (= page_size) or divide page_size";
   *st = VX_ERR_UNSUPPORTED;
   if (g->agg != VX_AGG_SUM && g->agg != VX_AGG_MAX) return "agg must be VX_AGG_SUM or VX_AGG_MAX";
   if (g->summary_kind != VX_SUMMARY_ENVELOPE && g->summary_kind != VX_SUMMARY_CENTROID)
@@ -140,6 +146,33 @@ static vx_status check_pool(vx_ctx* c, const vx_kv_pool* pool) {
   return VX_OK;
 }
 
+// the page table the kernels work on: the caller's, or (blocks finer than the page) its expansion into a block table in
+// the workspace -- request i's blocks are page_indptr[i] * bpp .., block (page, s) has the physical id page id * bpp + s
+__global__ void expand_block_table_kernel(const int32_t* __restrict__ indptr, const int32_t* __restrict__ indices, int batch,
+                                          int total_pages, int bpp, int32_t* __restrict__ out_indptr, int32_t* __restrict__ out_indices) {
+  const int n = total_pages * bpp;
+  for (int x = blockIdx.x * blockDim.x + threadIdx.x; x < n; x += gridDim.x * blockDim.x) out_indices[x] = indices[x / bpp] * bpp + x % bpp;
+  for (int x = blockIdx.x * blockDim.x + threadIdx.x; x <= batch; x += gridDim.x * blockDim.x) out_indptr[x] = indptr[x] * bpp;
+}
+
+static vx_status effective_table(vx_ctx* c, const vx_page_table* pt, cudaStream_t s, vx_page_table* out) {
+  *out = *pt;
+  if (c->bpp == 1 || pt->batch == 0) return VX_OK;
+  const int n = pt->total_pages * c->bpp;
+  int blocks = (n + 255) / 256;
+  if (blocks < 1) blocks = 1;
+  if (blocks > c->num_sms * 8) blocks = c->num_sms * 8;
+  expand_block_table_kernel<<<blocks, 256, 0, s>>>(pt->page_indptr, pt->page_indices, pt->batch, pt->total_pages, c->bpp,
+                                                   c->ws.blk_indptr, c->ws.blk_indices);
+  c->launches += 1;
+  if (vx_status st = check_cuda(c, cudaGetLastError(), "block table")) return st;
+  out->page_indptr = c->ws.blk_indptr;
+  out->page_indices = c->ws.blk_indices;
+  out->total_pages = n;
+  out->max_pages_per_req = pt->max_pages_per_req * c->bpp;
+  return VX_OK;
+}
+
 }  // namespace vx
 
 using namespace vx;
@@ -179,6 +212,12 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   vx_ctx* c = new (std::nothrow) vx_ctx();
   if (!c) return fail(nullptr, VX_ERR_INVALID_ARG, "out of host memory");
   c->g = *g;
+  // blocks finer than the page: from here on the kernels' "page" is the selection block (G28); the physical page survives
+  // in user_page_size / bpp, which only the kernels that address the KV pool need
+  c->user_page_size = g->page_size;
+  c->bpp = (g->block_size > 0 && g->block_size < g->page_size) ? g->page_size / g->block_size : 1;
+  c->g.page_size = g->page_size / c->bpp;
+  c->g.block_size = c->g.page_size;
   c->device = device;
   c->num_sms = prop.multiProcessorCount;
   c->max_batch = max_batch;
@@ -239,6 +278,9 @@ vx_status vx_page_summary_update(vx_ctx* c, const vx_kv_pool* pool, const vx_pag
   if (!c) return VX_ERR_INVALID_ARG;
   c->launches = 0;
   if (vx_status st = check_table(c, pt)) return st;
+  vx_page_table pt_eff;                          // (the block table when blocks are finer than the page)
+  if (vx_status st = effective_table(c, pt, (cudaStream_t)stream, &pt_eff)) return st;
+  pt = &pt_eff;
   if (vx_status st = check_pool(c, pool)) return st;
   if (!summary) return fail(c, VX_ERR_INVALID_ARG, "summary is NULL");
   return check_cuda(c, launch_summary_update(c, *pool, *pt, first_new_pos, summary, (cudaStream_t)stream),
@@ -250,6 +292,9 @@ vx_status vx_page_score(vx_ctx* c, const void* q, const void* summary, const vx_
   if (!c) return VX_ERR_INVALID_ARG;
   c->launches = 0;
   if (vx_status st = check_table(c, pt)) return st;
+  vx_page_table pt_eff;                          // (the block table when blocks are finer than the page)
+  if (vx_status st = effective_table(c, pt, (cudaStream_t)stream, &pt_eff)) return st;
+  pt = &pt_eff;
   if (!q || !summary || !scores) return fail(c, VX_ERR_INVALID_ARG, "q / summary / scores is NULL");
   return check_cuda(c, launch_page_score(c, q, summary, *pt, scores, (cudaStream_t)stream), "vx_page_score");
 }
@@ -260,6 +305,9 @@ vx_status vx_topk_pages(vx_ctx* c, const float* scores, const vx_page_table* pt,
   if (!c) return VX_ERR_INVALID_ARG;
   c->launches = 0;
   if (vx_status st = check_table(c, pt)) return st;
+  vx_page_table pt_eff;                          // (the block table when blocks are finer than the page)
+  if (vx_status st = effective_table(c, pt, (cudaStream_t)stream, &pt_eff)) return st;
+  pt = &pt_eff;
   if (!scores || !budget || !sel_phys || !sel_count)
     return fail(c, VX_ERR_INVALID_ARG, "scores / budget / sel_phys / sel_count is NULL");
   if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
@@ -273,6 +321,9 @@ vx_status vx_topk_pages_approx(vx_ctx* c, const float* scores, const vx_page_tab
   if (!c) return VX_ERR_INVALID_ARG;
   c->launches = 0;
   if (vx_status st = check_table(c, pt)) return st;
+  vx_page_table pt_eff;                          // (the block table when blocks are finer than the page)
+  if (vx_status st = effective_table(c, pt, (cudaStream_t)stream, &pt_eff)) return st;
+  pt = &pt_eff;
   if (!scores || !budget || !sel_phys || !sel_count)
     return fail(c, VX_ERR_INVALID_ARG, "scores / budget / sel_phys / sel_count is NULL");
   if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
@@ -315,6 +366,9 @@ vx_status vx_union_pages(vx_ctx* c, const vx_page_table* pt, const int32_t* sel_
   if (!c) return VX_ERR_INVALID_ARG;
   c->launches = 0;
   if (vx_status st = check_table(c, pt)) return st;
+  vx_page_table pt_eff;                          // (the block table when blocks are finer than the page)
+  if (vx_status st = effective_table(c, pt, (cudaStream_t)stream, &pt_eff)) return st;
+  pt = &pt_eff;
   if (!sel_logical || !sel_count || !union_phys || !union_count)
     return fail(c, VX_ERR_INVALID_ARG, "sel_logical / sel_count / union_phys / union_count is NULL");
   if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
@@ -350,6 +404,9 @@ vx_status vx_sparse_paged_decode(vx_ctx* c, const void* q, const vx_kv_pool* poo
   if (!c) return VX_ERR_INVALID_ARG;
   c->launches = 0;
   if (vx_status st = check_table(c, pt)) return st;
+  vx_page_table pt_eff;                          // (the block table when blocks are finer than the page)
+  if (vx_status st = effective_table(c, pt, (cudaStream_t)stream, &pt_eff)) return st;
+  pt = &pt_eff;
   if (vx_status st = check_pool(c, pool)) return st;
   if (!q || !sel_phys || !sel_logical || !sel_count || !out)
     return fail(c, VX_ERR_INVALID_ARG, "q / sel_phys / sel_logical / sel_count / out is NULL");
@@ -366,6 +423,9 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   if (!c) return VX_ERR_INVALID_ARG;
   c->launches = 0;
   if (vx_status st = check_table(c, pt)) return st;
+  vx_page_table pt_eff;                          // (the block table when blocks are finer than the page)
+  if (vx_status st = effective_table(c, pt, (cudaStream_t)stream, &pt_eff)) return st;
+  pt = &pt_eff;
   if (vx_status st = check_pool(c, pool)) return st;
   if (!q || !summary || !budget || !out) return fail(c, VX_ERR_INVALID_ARG, "q / summary / budget / out is NULL");
   if (max_budget <= 0 || max_budget > c->max_budget)
@@ -416,7 +476,7 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   // page, 72.1 / 74.0 / 75.8 with 2 / 3 / 4 -- the decode kernel's first TMA boxes queue behind the prefetches).
   PrefetchPlan pf;
   const int64_t esz = (int64_t)elem_size(c->g.dtype);
-  if (decode_folds_summary(c) && pool->stride_token == c->g.qk_dim) {
+  if (decode_folds_summary(c) && pool->stride_token == c->g.qk_dim && c->bpp == 1) {
     pf.k = pool->k;
     pf.v = c->g.kv_shared ? nullptr : pool->v;
     pf.page_bytes = pool->stride_page * esz;

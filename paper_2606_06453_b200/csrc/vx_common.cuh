@@ -127,6 +127,13 @@ __device__ __forceinline__ float key_to_float(uint32_t k) {
 
 __device__ __forceinline__ int ceil_div(int a, int b) { return (a + b - 1) / b; }
 
+// Selection blocks finer than the physical page (include/vortex_b200.h vx_geom.block_size): the kernels see
+// blocks as their "pages"; physical block id = page id * bpp + block in page, so a block's first token row sits at
+// page * stride_page + (block in page) * block_tokens * stride_token.  bpp = 1: the page itself.
+__device__ __forceinline__ int64_t pool_block_base(int64_t phys, int64_t stride_page, int bpp, int64_t block_tokens_stride) {
+  return bpp == 1 ? phys * stride_page : (phys / bpp) * stride_page + (phys % bpp) * block_tokens_stride;
+}
+
 // ---- programmatic dependent launch (PDL): the kernels of one decode step are chained so that a
 // kernel's prologue (index loads, barrier / TMEM set-up, Q staging) overlaps its predecessor's tail.
 // pdl_wait(): everything the preceding kernel wrote is visible after it (no-op without the attribute).

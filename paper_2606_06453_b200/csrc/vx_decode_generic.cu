@@ -52,7 +52,7 @@ decode_generic_kernel(const T* __restrict__ q, const TKV* __restrict__ kpool, co
                       const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ sel_phys,
                       const int32_t* __restrict__ sel_logical, const int32_t* __restrict__ sel_count,
                       int max_budget, int num_splits, float* __restrict__ part_o,
-                      float* __restrict__ part_lse, float k_scale, float v_scale) {
+                      float* __restrict__ part_lse, float k_scale, float v_scale, int bpp) {
   constexpr int E = Pair<T>::kElems;
   static_assert(Pair<TKV>::kElems == E, "q and the pools are read with the same channels per lane");
   sm_scale *= k_scale;                           // logits = sm_scale * q . (k_scale * decode(code))
@@ -96,8 +96,9 @@ decode_generic_kernel(const T* __restrict__ q, const TKV* __restrict__ kpool, co
   for (int r = r_begin; r < r_end; ++r) {
     const int64_t phys = phys_list[r];
     const int valid = min(page_size, n_tok - log_list[r] * page_size);
-    const TKV* kbase = kpool + phys * stride_page + kvh * stride_head;
-    const TKV* vbase = vpool + phys * stride_page + kvh * stride_head;
+    const int64_t pbase = pool_block_base(phys, stride_page, bpp, page_size * stride_token) + kvh * stride_head;
+    const TKV* kbase = kpool + pbase;
+    const TKV* vbase = vpool + pbase;
     for (int t = wt; t < valid; t += WT) {
       float kf[NK * E];
 #pragma unroll
@@ -208,7 +209,7 @@ static cudaError_t launch_generic_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const T*>(q), static_cast<const TKV*>(pool.k), static_cast<const TKV*>(v), pool.stride_page,
       pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads, g.page_size, g.sm_scale,
       pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits, c->ws.part_o, c->ws.part_lse,
-      fp8 ? pool.k_scale : 1.f, fp8 ? (g.kv_shared ? pool.k_scale : pool.v_scale) : 1.f);
+      fp8 ? pool.k_scale : 1.f, fp8 ? (g.kv_shared ? pool.k_scale : pool.v_scale) : 1.f, c->bpp);
   c->launches += 1;
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return e;
@@ -354,7 +355,7 @@ static vx_status launch_generic_static_t(const vx_geom& g, const void* q, const 
   decode_generic_kernel<T, T, D, DV, HPW, WT><<<grid, wh * WT * kWarp, 0, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(pool.k), static_cast<const T*>(v), pool.stride_page,
       pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads, g.page_size, g.sm_scale,
-      pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits, part_o, part_lse, 1.f, 1.f);
+      pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits, part_o, part_lse, 1.f, 1.f, 1);
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) {
     combine_kernel<T><<<(unsigned)rows, 128, 0, s>>>(part_o, part_lse, n_part, g.v_dim, static_cast<T*>(out), lse);

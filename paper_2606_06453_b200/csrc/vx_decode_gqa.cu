@@ -64,7 +64,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
                       int max_budget, int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                       int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
                       __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0,
-                      const int32_t* __restrict__ budget_opt) {
+                      const int32_t* __restrict__ budget_opt, int bpp) {
   constexpr int ROWB = D * 2;                 // bytes per token row
   constexpr int CH = ROWB / 16;               // 16-byte chunks per row
   constexpr int PAGEB = kGqaPage * ROWB;      // bytes of one K (or V) page chunk
@@ -125,7 +125,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   auto issue = [&](int p) {                     // all lanes: copy page p of this warp into slot p % stages
     const int phys = __shfl_sync(0xffffffffu, id_phys, p & 31);
     const int valid = __shfl_sync(0xffffffffu, id_valid, p & 31);
-    const int64_t base = (int64_t)phys * stride_page + (int64_t)kvh * stride_head;
+    const int64_t base = pool_block_base(phys, stride_page, bpp, kGqaPage * stride_token) + (int64_t)kvh * stride_head;
     const uint32_t dst = ring_u32 + (uint32_t)(p % kGqaStages) * 2 * PAGEB;
     if (lane == 0) { s_valid[warp][p % kGqaStages] = valid; s_phys[warp][p % kGqaStages] = phys; }
     const int nv = valid & 255;
@@ -350,7 +350,7 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const __nv_bfloat16*>(pool.v), pool.stride_page, pool.stride_token, pool.stride_head,
       g.num_q_heads, g.num_kv_heads, g.sm_scale * kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget,
       splits, c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
-      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget);
+      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget, c->bpp);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -74,7 +74,7 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
                       const int32_t* __restrict__ sel_phys, const int32_t* __restrict__ sel_logical,
                       const int32_t* __restrict__ sel_count, int max_budget, int num_splits, float* __restrict__ part_o,
                       float* __restrict__ part_lse, int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ out,
-                      float* __restrict__ lse_out, const int32_t* __restrict__ budget_opt) {
+                      float* __restrict__ lse_out, const int32_t* __restrict__ budget_opt, int bpp) {
   using namespace gq8;
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float s_m[WARPS][8], s_l[WARPS][8];
@@ -138,7 +138,7 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
   auto issue = [&](int p) {                     // all lanes: copy page p of this warp into slot p % STAGES
     const int phys = __shfl_sync(0xffffffffu, id_phys, p & 31);
     const int nv = __shfl_sync(0xffffffffu, id_valid, p & 31);
-    const int64_t base = (int64_t)phys * stride_page + (int64_t)kvh * stride_head;
+    const int64_t base = pool_block_base(phys, stride_page, bpp, PAGE * stride_token) + (int64_t)kvh * stride_head;
     const uint32_t dst = ring_u32 + (uint32_t)(p % STAGES) * 2 * PAGEB;
     if (lane == 0) s_valid[warp][p % STAGES] = nv;
 #pragma unroll
@@ -321,7 +321,7 @@ static cudaError_t launch_gqa_fp8_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const __nv_bfloat16*>(q), static_cast<const uint8_t*>(pool.k), static_cast<const uint8_t*>(pool.v),
       pool.stride_page, pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads,
       g.sm_scale * pool.k_scale * gq8::kLog2e, pool.v_scale, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits,
-      c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(out), lse, budget);
+      c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(out), lse, budget, c->bpp);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

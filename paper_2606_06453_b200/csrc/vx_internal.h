@@ -29,6 +29,8 @@ struct Workspace {               // device pointers carved from the caller's wor
   // the flat MLA step kernel (vx_step_mla_flat.cu)
   float* flat_qvec;              // [max_batch, 2 qk_dim] query vectors [Qm | Qp]
   int32_t* flat_sync;            // counters and per-request flags; zero between steps
+  int32_t* blk_indptr;           // blocks finer than the page: the page table expanded into a block table, [max_batch + 1]
+  int32_t* blk_indices;          // [max_total_pages * bpp] physical block ids
   float* fp8_qvec;               // fp8 KV cache: [max_batch, Hkv, 2 qk_dim] query vectors [Qm | Qp] of the score kernel (vx_score_fp8.cu)
   size_t bytes;                  // total
 };
@@ -56,6 +58,8 @@ struct vx_ctx {
   int32_t launches;              // kernels enqueued by the last compute call
   vx::ApproxPlan approx;         // vx_set_topk_approx: used by a fused step with VX_STEP_APPROX_TOPK
   int32_t mla_step;              // VX_OPT_MLA_STEP
+  int32_t bpp;                   // selection blocks per physical page (vx_geom.block_size); g.page_size holds the BLOCK size
+  int32_t user_page_size;        // tokens per physical page as the caller gave it
   int32_t* pinned_small;         // pinned host staging [3 max_batch + 1] for vx_sparse_decode_step_host's small arrays
   int32_t flat_splits, flat_waves;   // VX_OPT_MLA_FLAT_*: 0 = the library's choice
   char err[512];

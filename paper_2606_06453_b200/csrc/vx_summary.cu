@@ -17,7 +17,7 @@ summary_kernel(const T* __restrict__ k, int64_t stride_page, int64_t stride_toke
                int num_kv_heads, int qk_dim, int page_size, int batch,
                const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
                const int32_t* __restrict__ seq_lens, const int32_t* __restrict__ first_new_pos,
-               int append_only, int64_t num_slots, T* __restrict__ summary) {
+               int append_only, int64_t num_slots, T* __restrict__ summary, int bpp) {
   constexpr int PER = Elem<T>::kPerVec;
   const int nvec = qk_dim / PER;
   const int64_t items = num_slots * num_kv_heads * nvec;
@@ -45,7 +45,7 @@ summary_kernel(const T* __restrict__ k, int64_t stride_page, int64_t stride_toke
     if (j >= n_pages) continue;   // slack entries of an over-allocated table
     const int valid = min(page_size, n - j * page_size);
     const int64_t phys = page_indices[page_indptr[i] + j];
-    const T* src = k + phys * stride_page + h * stride_head + (int64_t)v * PER;
+    const T* src = k + pool_block_base(phys, stride_page, bpp, page_size * stride_token) + h * stride_head + (int64_t)v * PER;
 
     if constexpr (KIND == VX_SUMMARY_CENTROID) {       // mean of the valid keys, one rounding (exact double sums)
       double sum[PER];
@@ -125,12 +125,12 @@ static cudaError_t launch_summary_t(vx_ctx* c, const vx_kv_pool& pool, const vx_
     summary_kernel<T, 8, VX_SUMMARY_CENTROID><<<(unsigned)blocks, threads, 0, s>>>(
         static_cast<const T*>(pool.k), pool.stride_page, pool.stride_token, pool.stride_head,
         g.num_kv_heads, g.qk_dim, g.page_size, pt.batch, pt.page_indptr, pt.page_indices, pt.seq_lens,
-        first_new_pos, append_only, slots, static_cast<T*>(summary));
+        first_new_pos, append_only, slots, static_cast<T*>(summary), c->bpp);
   else
     summary_kernel<T, 8, VX_SUMMARY_ENVELOPE><<<(unsigned)blocks, threads, 0, s>>>(
         static_cast<const T*>(pool.k), pool.stride_page, pool.stride_token, pool.stride_head,
         g.num_kv_heads, g.qk_dim, g.page_size, pt.batch, pt.page_indptr, pt.page_indices, pt.seq_lens,
-        first_new_pos, append_only, slots, static_cast<T*>(summary));
+        first_new_pos, append_only, slots, static_cast<T*>(summary), c->bpp);
   c->launches += 1;
   return cudaGetLastError();
 }

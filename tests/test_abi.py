@@ -41,7 +41,7 @@ def test_header_symbols_are_exported(vx):
 def geom(vx, **kw):
     from paper_2606_06453_b200.binding import VxGeom
     base = dict(dtype=0, num_q_heads=32, num_kv_heads=8, qk_dim=128, v_dim=128, page_size=16, kv_shared=0,
-                sm_scale=0.088, n_sink=1, n_local=2, agg=0, summary_kind=0, kv_format=0)
+                sm_scale=0.088, n_sink=1, n_local=2, agg=0, summary_kind=0, kv_format=0, block_size=0)
     base.update(kw)
     return VxGeom(*[base[f[0]] for f in VxGeom._fields_])
 
