@@ -150,7 +150,7 @@ int32_t vx_last_launch_count(const vx_ctx *ctx);
 
 /* Context options (host side, persistent until changed).  VX_ERR_INVALID_ARG for an unknown option or value.
  *  VX_OPT_MLA_STEP   how vx_sparse_decode_step schedules the MLA geometry:
- *      VX_MLA_STEP_AUTO     (default) the faster of the two for the batch at hand (DESIGN.md section 17)
+ *      VX_MLA_STEP_AUTO     (default) the faster of the two for the batch at hand (DESIGN.md section 16)
  *      VX_MLA_STEP_FUSED    one kernel: a thread-block cluster per request runs score -> select -> decode -> merge
  *                           (falls back to CHAINED when the request / budget sizes exceed what it keeps on chip)
  *      VX_MLA_STEP_CHAINED  three kernels chained by programmatic dependent launch (score, select, decode)
@@ -159,7 +159,7 @@ int32_t vx_last_launch_count(const vx_ctx *ctx);
  *                           counter (falls back to CHAINED for batches / requests beyond what it keeps on chip)
  *    All schedules compute the same selection bit for bit; outputs agree to rounding (different split sizes).
  *  VX_OPT_MLA_FLAT_SPLITS / VX_OPT_MLA_FLAT_WAVES   0 (default) = chosen by the library; > 0 = decode shares per request /
- *                           interleaved waves of the summary stream of the FLAT schedule (tuning knobs, DESIGN.md section 17) */
+ *                           interleaved waves of the summary stream of the FLAT schedule (tuning knobs, DESIGN.md section 16) */
 enum { VX_OPT_MLA_STEP = 1, VX_OPT_MLA_FLAT_SPLITS = 2, VX_OPT_MLA_FLAT_WAVES = 3 };
 enum { VX_MLA_STEP_AUTO = 0, VX_MLA_STEP_FUSED = 1, VX_MLA_STEP_CHAINED = 2, VX_MLA_STEP_FLAT = 3 };
 vx_status vx_set_option(vx_ctx *ctx, int32_t option, int32_t value);

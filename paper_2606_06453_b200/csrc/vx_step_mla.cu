@@ -652,7 +652,7 @@ bool step_mla_fused_applies(const vx_ctx* c, const vx_page_table& pt, const vx_k
          pt.max_pages_per_req <= mla::F_MAX_PAGES && max_budget <= 8 * mla::F_MAX_LIST && pool.num_pool_pages > 0;
 }
 
-// Where it pays (measured on the C4 geometry, DESIGN.md section 17): batches of up to 8 requests, which run as 8 CTAs per
+// Where it pays (measured on the C4 geometry, DESIGN.md section 16): batches of up to 8 requests, which run as 8 CTAs per
 // request in one wave -- 47-49 us against 70-79 us for the three chained kernels.  From 16 requests on the chained kernels
 // win: their score and decode kernels split the BATCH's pages evenly over all SMs, while a cluster streams its own
 // request's summaries, so the longest request sets the pace (B = 64: 71.5 against 68.5 us).
