@@ -7,6 +7,8 @@
 
 #include "vortex_b200.h"
 
+/* `kernels` with ONE kind set: that kind's CTA c writes row c.  With several kinds set (a whole step on one time line) the
+ * score kernel's rows start at 0, the selection kernels' at 1024, the decode kernels' at 4096. */
 #ifdef __cplusplus
 extern "C" {
 #endif

@@ -263,13 +263,19 @@ vx_status vx_trace_attach(vx_ctx* c, void* buffer, int32_t max_ctas, int32_t ker
   if (cudaError_t e = cudaSetDevice(c->device)) return check_cuda(c, e, "vx_trace_attach");
   long long* b = static_cast<long long*>(buffer);
   const int n = buffer ? max_ctas : 0;
+  // one kind: its CTAs' rows start at row 0.  Several kinds at once (a whole step on one time line): the score kernel's
+  // rows start at 0, the selection kernels' at 1024, the decode kernels' at 4096
+  const bool many = (kernels & (kernels - 1)) != 0;
+  const int o_topk = many ? 1024 : 0, o_dec = many ? 4096 : 0;
+  auto at = [&](int off) -> long long* { return b ? b + (long long)off * 16 : nullptr; };
+  auto left = [&](int off) -> int { return n > off ? n - off : 0; };
   cudaError_t e = vx_trace_set_score((kernels & VX_TRACE_SCORE) ? b : nullptr, n);
   if (e == cudaErrorNotSupported) return fail(c, VX_ERR_UNSUPPORTED, "this library was built without -DVX_TRACE");
-  if (e == cudaSuccess) e = vx_trace_set_topk((kernels & VX_TRACE_TOPK) ? b : nullptr, n);
-  if (e == cudaSuccess) e = vx_trace_set_decode_gqa((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
-  if (e == cudaSuccess) e = vx_trace_set_decode_mla((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
-  if (e == cudaSuccess) e = vx_trace_set_step_mla((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
-  if (e == cudaSuccess) e = vx_trace_set_step_mla_flat((kernels & VX_TRACE_DECODE) ? b : nullptr, n);
+  if (e == cudaSuccess) e = vx_trace_set_topk((kernels & VX_TRACE_TOPK) ? at(o_topk) : nullptr, left(o_topk));
+  if (e == cudaSuccess) e = vx_trace_set_decode_gqa((kernels & VX_TRACE_DECODE) ? at(o_dec) : nullptr, left(o_dec));
+  if (e == cudaSuccess) e = vx_trace_set_decode_mla((kernels & VX_TRACE_DECODE) ? at(o_dec) : nullptr, left(o_dec));
+  if (e == cudaSuccess) e = vx_trace_set_step_mla((kernels & VX_TRACE_DECODE) ? at(o_dec) : nullptr, left(o_dec));
+  if (e == cudaSuccess) e = vx_trace_set_step_mla_flat((kernels & VX_TRACE_DECODE) ? at(o_dec) : nullptr, left(o_dec));
   return check_cuda(c, e, "vx_trace_attach");
 }
 
