@@ -21,18 +21,10 @@ import torch
 from . import binding as vx
 
 
-def draw(dist: str, shape, gen, device):
-    if dist == "normal":
-        return torch.randn(shape, generator=gen, device=device) * 32.0 + 900.0
-    if dist == "uniform":
-        return torch.rand(shape, generator=gen, device=device) * 100.0
-    if dist == "lognormal":
-        return torch.exp(torch.randn(shape, generator=gen, device=device) * 1.5)
-    if dist == "bimodal":
-        pick = torch.rand(shape, generator=gen, device=device) < 0.1
-        return torch.where(pick, torch.randn(shape, generator=gen, device=device) * 2.0 + 40.0,
-                           torch.randn(shape, generator=gen, device=device) * 2.0 - 10.0)
-    raise ValueError(dist)
+def draw(dist: str, shape, seed, device):
+    """the App. D stand-in distributions: workloads.appd_scores (the one generator the tests use too), moved to the GPU"""
+    from .workloads import appd_scores
+    return appd_scores(dist, shape, seed).to(device)
 
 
 def main():
@@ -61,7 +53,7 @@ def main():
             sl = torch.empty_like(sp)
             sc = torch.empty(B, H, dtype=torch.int32, device=dev)
             for dist in ("bimodal", "normal", "lognormal", "uniform"):
-                scores = draw(dist, (H, T), gen, dev)
+                scores = draw(dist, (H, T), 7700 + P + k, dev)
                 ctx.topk_pages(scores, pt, budget, k, sp, sl, sc)
                 torch.cuda.synchronize()
                 # exactness: forced pages + the k - 3 best of the rest, as a set per problem
