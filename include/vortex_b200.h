@@ -209,7 +209,8 @@ vx_status vx_topk_pages(vx_ctx *ctx, const float *scores, const vx_page_table *p
  * pages differ from the exact set: recall@k >= 1 - tolerate_ratio.  tolerate_ratio = 0 is vx_topk_pages.
  * The paper prints no pseudo-code; the choices made are readings G20-G23 of DESIGN.md section 12.
  * VX_ERR_INVALID_ARG if tolerate_ratio is outside [0, 1]; VX_ERR_UNSUPPORTED if tolerate_ratio > 0 and
- * pt->max_pages_per_req > 8192 (the selection kernel that implements it keeps a request's keys in registers). */
+ * pt->max_pages_per_req > 49152, or > 8192 with max_budget > 2048 (requests of up to 8,192 pages are selected with their
+ * keys in registers, longer ones with their keys in shared memory, which stages at most 2,048 selected pages). */
 vx_status vx_topk_pages_approx(vx_ctx *ctx, const float *scores, const vx_page_table *pt,
                                const int32_t *budget /* dev [B] */, int32_t max_budget,
                                float tolerate_ratio, uint64_t seed, int32_t *sel_phys,

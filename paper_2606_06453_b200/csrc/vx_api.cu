@@ -335,9 +335,9 @@ vx_status vx_topk_pages_approx(vx_ctx* c, const float* scores, const vx_page_tab
   if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
   if (!(tolerate_ratio >= 0.f && tolerate_ratio <= 1.f))
     return fail(c, VX_ERR_INVALID_ARG, "tolerate_ratio %g outside [0, 1]", (double)tolerate_ratio);
-  if (tolerate_ratio > 0.f && pt->max_pages_per_req > kTopkRegMaxPages)
-    return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (got %d)",
-                kTopkRegMaxPages, pt->max_pages_per_req);
+  if (tolerate_ratio > 0.f && !approx_topk_supported(pt->max_pages_per_req, max_budget))
+    return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (budgets above %d: %d pages); got %d",
+                kTopkApproxMaxPages, kTopkApproxMaxBudgetLong, kTopkRegMaxPages, pt->max_pages_per_req);
   ApproxPlan ap;
   ap.tolerate_ratio = tolerate_ratio;
   ap.seed = seed;
@@ -440,9 +440,9 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   ApproxPlan ap;                                 // exact unless the caller asks for the lossy selection
   if (flags & VX_STEP_APPROX_TOPK) {
     ap = c->approx;
-    if (ap.tolerate_ratio > 0.f && pt->max_pages_per_req > kTopkRegMaxPages)
-      return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (got %d)",
-                  kTopkRegMaxPages, pt->max_pages_per_req);
+    if (ap.tolerate_ratio > 0.f && !approx_topk_supported(pt->max_pages_per_req, max_budget))
+      return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (budgets above %d: %d pages); got %d",
+                  kTopkApproxMaxPages, kTopkApproxMaxBudgetLong, kTopkRegMaxPages, pt->max_pages_per_req);
   }
   cudaStream_t s = (cudaStream_t)stream;
   int32_t* sp = sel_phys ? sel_phys : c->ws.sel_phys;

@@ -46,6 +46,11 @@ struct ApproxPlan {
   uint64_t seed = 0;
 };
 constexpr int kTopkRegMaxPages = 8 * 1024;       // register-resident selection kernel: pages per request
+constexpr int kTopkApproxMaxPages = 48 * 1024;   // the lossy selection beyond that: the shared-memory-key kernel's key cache
+constexpr int kTopkApproxMaxBudgetLong = 2048;   // ... which stages at most this many selected pages
+inline bool approx_topk_supported(int max_pages_per_req, int max_budget) {
+  return max_pages_per_req <= kTopkRegMaxPages || (max_pages_per_req <= kTopkApproxMaxPages && max_budget <= kTopkApproxMaxBudgetLong);
+}
 
 }  // namespace vx
 

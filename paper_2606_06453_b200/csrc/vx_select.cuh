@@ -45,8 +45,13 @@ __device__ __forceinline__ void select_sync() {
   if constexpr (BAR == 0) __syncthreads();
   else asm volatile("bar.sync %0, %1;" ::"n"(BAR), "n"(THREADS) : "memory");
 }
-template <int THREADS, int BAR = 0, int TID0 = 0>
-__device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, int k, int n_sink, int n_local) {
+// kApprox (PAPER.md:196 stochastic early termination, readings G20-G23): after a pass, when the pages
+// still to take from the threshold bin number at most floor(tolerate_ratio * k), they are drawn from the bin's members as
+// the cyclic window of member ranks (page order) that starts at a SplitMix64 draw of (seed, problem) -- the same rule,
+// constants and order of tests as topk_reg_kernel<.., true>, so both kernels and oracle/vx_oracle_approx.py agree bit for bit.
+template <int THREADS, int BAR = 0, int TID0 = 0, bool kApprox = false>
+__device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, int k, int n_sink, int n_local,
+                                float tolerate_ratio = 0.f, uint64_t seed = 0, int problem = 0) {
   constexpr int WARPS = THREADS / kWarp;
   constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
   static_assert(kBins % THREADS == 0 && WARPS <= 32, "shape");
@@ -78,20 +83,26 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
   int need = k - n_forced;                      // non-forced pages still to take (precondition: >= 0)
   uint32_t thr = kForcedKey;                    // take keys > thr, and the first need_eq keys == thr
   int need_eq = 0;
+  // early termination (kApprox): ties = the members of the threshold bin (key interval [m_lo, m_hi], or float bin t_bin),
+  // taken as the cyclic window of need_eq member ranks that starts at rot
+  [[maybe_unused]] bool early = false, fterm = false;
+  [[maybe_unused]] uint32_t m_lo = 0u, m_hi = 0u;
+  [[maybe_unused]] int t_bin = 0, rot = 0, wrap = 0;
+  const float smin = key_to_float(kmin), smax = key_to_float(kmax);
+  const float fscale = (float)kBins / (smax - smin);
+  auto fbin = [&](uint32_t key) -> int { return min(kBins - 1, (int)((key_to_float(key) - smin) * fscale)); };
 
   if (need > 0) {
     // ---- radix select over the live key range [lo, lo + width) ----------------------------------
     uint32_t lo = kmin;
     uint64_t width = (uint64_t)(kmax - kmin) + 1;
     int shift = max(0, (32 - __clz(kmax - kmin)) - kBinBits);     // ((kmax - kmin) >> shift) < kBins
+    [[maybe_unused]] const int tol = kApprox ? (int)(tolerate_ratio * (float)k) : 0;   // floor: both factors >= 0
     // First pass in the FLOAT domain: bin = floor((score - min) * 2048 / (max - min)) is monotone in the score, and
     // unlike the integer key it is linear across the sign change and across exponents.  The members of one float bin
     // are a contiguous key interval, so deeper passes continue on integer keys.  Only when the key range spans the
     // sign change or several exponents (>= 2^25 key steps): a narrow range is linear enough in the integer key.
-    const float smin = key_to_float(kmin), smax = key_to_float(kmax);
-    const float fscale = (float)kBins / (smax - smin);
     bool fpass = kmax - kmin >= (1u << 25) && isfinite(fscale) && fscale > 0.f;
-    auto fbin = [&](uint32_t key) -> int { return min(kBins - 1, (int)((key_to_float(key) - smin) * fscale)); };
 #pragma unroll 1
     while (true) {
       for (int b = tid; b < kBins; b += THREADS) sc.hist[b] = 0;
@@ -134,6 +145,23 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
       }
       // members of the threshold bin: rank them if they are few, else continue on their key interval
       const uint64_t bin_w = (uint64_t)1 << shift;
+      if constexpr (kApprox) {
+        if (need <= tol) {                      // enough high-confidence pages: sample the rest from the bin's members
+          early = true;
+          fterm = fpass;
+          t_bin = bin;
+          m_lo = bin_lo;
+          m_hi = (uint32_t)min((uint64_t)bin_lo + bin_w - 1, (uint64_t)lo + width - 1);
+          need_eq = need;
+          uint64_t z = seed + 0x9E3779B97F4A7C15ull * (uint64_t)(problem + 1);   // SplitMix64 draw
+          z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+          z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+          z ^= z >> 31;
+          rot = (int)((uint32_t)(z >> 32) % (uint32_t)cnt);
+          wrap = max(0, rot + need - cnt);      // member ranks [0, wrap) and [rot, rot + need - wrap) are taken
+          break;
+        }
+      }
       for (int j = tid; j < n_pages; j += THREADS) {
         const uint32_t key = keys[j];
         const bool in_range = key != kForcedKey && key >= lo && (uint64_t)(key - lo) < width;
@@ -179,11 +207,26 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
   const int per_warp = ((n_pages + WARPS - 1) / WARPS + kWarp - 1) / kWarp * kWarp;
   const int j_begin = min(warp * per_warp, n_pages), j_end = min(j_begin + per_warp, n_pages);
   int n_sure = 0, n_tie = 0;                    // warp-uniform
+  // class of a key: exact threshold key; (early stop) the key interval of the threshold bin; (early stop on the float pass) its float bin
+  auto classify = [&](uint32_t key, bool exists, bool& sure, bool& tie) {
+    const bool forced = key == kForcedKey;
+    if (!kApprox || !early) {
+      sure = exists && (forced || key > thr);
+      tie = exists && !forced && key == thr;
+    } else if (!fterm) {
+      sure = exists && (forced || key > m_hi);
+      tie = exists && !forced && key >= m_lo && key <= m_hi;
+    } else {
+      const int fb = forced ? kBins : fbin(key);
+      sure = exists && fb > t_bin;
+      tie = exists && fb == t_bin;
+    }
+  };
   for (int base = j_begin; base < j_end; base += kWarp) {
     const int j = base + lane;
     const uint32_t key = j < j_end ? keys[j] : 0u;
-    const bool sure = j < j_end && (key == kForcedKey || key > thr);
-    const bool tie = j < j_end && key != kForcedKey && key == thr;
+    bool sure, tie;
+    classify(key, j < j_end, sure, tie);
     n_sure += __popc(__ballot_sync(0xffffffffu, sure));
     n_tie += __popc(__ballot_sync(0xffffffffu, tie));
   }
@@ -200,12 +243,20 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
   for (int base = j_begin; base < j_end; base += kWarp) {
     const int j = base + lane;
     const uint32_t key = j < j_end ? keys[j] : 0u;
-    const bool sure = j < j_end && (key == kForcedKey || key > thr);
-    const bool tie = j < j_end && key != kForcedKey && key == thr;
+    bool sure, tie;
+    classify(key, j < j_end, sure, tie);
     const unsigned b_sure = __ballot_sync(0xffffffffu, sure), b_tie = __ballot_sync(0xffffffffu, tie);
     const int my_gt = gt + __popc(b_sure & lt_mask), my_eq = eq + __popc(b_tie & lt_mask);
-    const bool take = sure || (tie && my_eq < need_eq);
-    const int pos = my_gt + min(my_eq, need_eq);
+    bool take;
+    int pos;
+    if (kApprox && early) {                       // ranks [0, wrap) and [rot, rot + need_eq - wrap)
+      const int span = need_eq - wrap;
+      take = sure || (tie && (my_eq < wrap || (my_eq >= rot && my_eq < rot + span)));
+      pos = my_gt + min(my_eq, wrap) + min(max(my_eq - rot, 0), span);
+    } else {
+      take = sure || (tie && my_eq < need_eq);
+      pos = my_gt + min(my_eq, need_eq);
+    }
     if (take && pos < n_sel) sc.hist[pos] = j;    // (the histogram is free now)
     gt += __popc(b_sure);
     eq += __popc(b_tie);

@@ -40,7 +40,8 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
             const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices,
             const int32_t* __restrict__ seq_lens, int page_size, const int32_t* __restrict__ budget,
             int n_sink, int n_local, int max_budget, int smem_keys, int32_t* __restrict__ sel_phys,
-            int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count, int req0, const PrefetchPlan pf) {
+            int32_t* __restrict__ sel_logical, int32_t* __restrict__ sel_count, int req0, const PrefetchPlan pf,
+            const ApproxPlan ap) {
   constexpr int WARPS = THREADS / kWarp;
   constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
   static_assert(kBins % THREADS == 0 && THREADS >= kList, "shape");
@@ -87,7 +88,10 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
         if (j0 + u * THREADS < n_pages) s_keys[j0 + u * THREADS] = __float_as_uint(v[u]);
     }
     __syncthreads();
-    cta_select_pages<THREADS>(scratch, s_keys, n_pages, k, n_sink, n_local);
+    if (ap.tolerate_ratio > 0.f)                // (requests beyond the register kernel's 8,192 pages)
+      cta_select_pages<THREADS, 0, 0, true>(scratch, s_keys, n_pages, k, n_sink, n_local, ap.tolerate_ratio, ap.seed, i * num_kv_heads + kvh);
+    else
+      cta_select_pages<THREADS>(scratch, s_keys, n_pages, k, n_sink, n_local);
     pdl_trigger();
     const int per_split = (n_sel + pf.splits - 1) / pf.splits;
     for (int r = tid; r < n_sel; r += THREADS) {
@@ -330,7 +334,8 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
 template <int THREADS>
 static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_table& pt, const int32_t* budget,
                                  int32_t max_budget, int32_t* sel_phys, int32_t* sel_logical, int32_t* sel_count,
-                                 cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf) {
+                                 cudaStream_t s, bool pdl, const ReqRange& rr, const PrefetchPlan& pf,
+                                 const ApproxPlan& ap = ApproxPlan()) {
   const vx_geom& g = c->g;
   const int keys = pt.max_pages_per_req <= kTopkSmemKeys ? pt.max_pages_per_req : 0;
   const size_t smem = (size_t)(keys > 0 ? keys : 1) * sizeof(uint32_t);
@@ -338,7 +343,7 @@ static cudaError_t launch_topk_t(vx_ctx* c, const float* scores, const vx_page_t
   dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
   cudaError_t e = launch_kernel(topk_kernel<THREADS>, grid, dim3(THREADS), smem, s, pdl, scores, g.num_kv_heads,
                                 pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
-                                g.n_sink, g.n_local, max_budget, keys, sel_phys, sel_logical, sel_count, rr.begin, pf);
+                                g.n_sink, g.n_local, max_budget, keys, sel_phys, sel_logical, sel_count, rr.begin, pf, ap);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }
@@ -665,7 +670,10 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
                               int32_t* sel_logical, int32_t* sel_count, cudaStream_t s, bool pdl, const ReqRange& rr,
                               const PrefetchPlan& pf, const ApproxPlan& ap) {
   if (pt.batch == 0) return cudaSuccess;
-  if (ap.tolerate_ratio > 0.f && pt.max_pages_per_req > kTopkRegMaxPages) return cudaErrorNotSupported;
+  // the lossy selection runs in the register kernel (<= 8,192 pages) and in the shared-memory-key kernel (<= 49,152 pages,
+  // budgets of at most 2,048 pages)
+  static_assert(kTopkApproxMaxPages == kTopkSmemKeys && kTopkApproxMaxBudgetLong == kBins, "vx_internal.h states the kernel's limits");
+  if (ap.tolerate_ratio > 0.f && !approx_topk_supported(pt.max_pages_per_req, max_budget)) return cudaErrorNotSupported;
   // block size by problem size
   const int n = pt.max_pages_per_req;
   if (ap.tolerate_ratio <= 0.f && topk_pair_applies(c, c->g.num_kv_heads * (rr.count < 0 ? pt.batch : rr.count), n))
@@ -681,9 +689,9 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
 #undef VX_REG
   }
   const int th = n <= 1024 ? 256 : n <= 4096 ? 512 : 1024;
-  if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
-  if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
-  return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
+  if (th <= 256) return launch_topk_t<256>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap);
+  if (th <= 512) return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap);
+  return launch_topk_t<1024>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap);
 }
 
 }  // namespace vx

@@ -142,10 +142,42 @@ def test_seed_changes_only_the_sampled_members_and_recall_holds(dist, tau):
             assert np.array_equal(a[0, h], exact[0, h])
 
 
+@pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
+@pytest.mark.parametrize("tau", [0.05, 0.25, 1.0])
+def test_long_requests_beyond_the_register_kernel(dist, tau):
+    """requests of more than 8,192 pages: the lossy selection in the shared-memory-key kernel (cta_select_pages<.., kApprox>)"""
+    rng = np.random.default_rng(11)
+    pages = [9000, 20000, 300, 33001]
+    hkv = 2
+    T = sum(pages)
+    seq = [p * 16 - int(rng.integers(0, 16)) for p in pages]
+    indices = rng.permutation(T + 5)[:T].astype(np.int32)
+    budget = np.array([256, 1500, 64, 400], np.int32)
+    scores = appd_scores(dist, (hkv, T), seed=57).numpy()
+    (sl_r, sp_r, sc_r, early), (sl, sp, sc) = run_both(scores, pages, seq, indices, budget, 1, 2, tau, 77)
+    assert np.array_equal(sc, sc_r) and np.array_equal(sl, sl_r) and np.array_equal(sp, sp_r), (dist, tau)
+    if tau == 1.0:
+        assert early.all()
+
+
+@pytest.mark.parametrize("kind", KINDS)
+def test_long_requests_fuzz_kinds(kind):
+    rng = np.random.default_rng(177 + KINDS.index(kind))
+    n_sink, n_local = int(rng.integers(0, 3)), int(rng.integers(0, 4))
+    pages = [int(x) for x in rng.choice([8193, 10000, 16384, 25000], size=3)]
+    seq = [p * 16 - int(rng.integers(0, 16)) for p in pages]
+    T = sum(pages)
+    indices = rng.permutation(T + 3)[:T].astype(np.int32)
+    budget = np.array([int(rng.integers(n_sink + n_local + 1, 900)) for _ in pages], np.int32)
+    scores = np.stack([draw_scores(rng, kind, T) for _ in range(2)])
+    (sl_r, sp_r, sc_r, _), (sl, sp, sc) = run_both(scores, pages, seq, indices, budget, n_sink, n_local, 0.25, 5)
+    assert np.array_equal(sc, sc_r) and np.array_equal(sl, sl_r) and np.array_equal(sp, sp_r), kind
+
+
 def test_argument_checks():
     import paper_2606_06453_b200 as vx
     dev = "cuda:0"
-    P = 9000
+    P = 50000                                      # beyond the 49,152 keys the shared-memory-key kernel caches
     ctx = vx.Context(dtype=torch.bfloat16, num_q_heads=8, num_kv_heads=2, qk_dim=128, v_dim=128, page_size=16,
                      sm_scale=1.0, n_sink=1, n_local=2, max_batch=1, max_total_pages=P, max_pages_per_req=P,
                      max_budget=64, device=dev)
@@ -155,7 +187,7 @@ def test_argument_checks():
     budget = torch.tensor([64], dtype=torch.int32, device=dev)
     sl = torch.empty(1, 2, 64, dtype=torch.int32, device=dev)
     sp, sc = torch.empty_like(sl), torch.empty(1, 2, dtype=torch.int32, device=dev)
-    with pytest.raises(vx.VortexError):           # more pages per request than the register kernel holds
+    with pytest.raises(vx.VortexError):           # more pages per request than either lossy kernel holds
         ctx.topk_pages_approx(scores, pt, budget, 64, 0.25, 1, sp, sl, sc)
     with pytest.raises(vx.VortexError):
         ctx.topk_pages_approx(scores, pt, budget, 64, 1.5, 1, sp, sl, sc)
