@@ -269,7 +269,7 @@ def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=No
     return statistics.median(times), n_requests, w.spec.batch, vo.num_threads()
 
 
-SAMPLE_REQUESTS = {"C1": 1, "C2": 4, "C3": 1, "C4": 8, "C5": 8}     # cpu_baseline: requests per oracle pass
+SAMPLE_REQUESTS = {"C1": 1, "C2": 32, "C3": 8, "C4": 64, "C5": 16}  # cpu_baseline: requests per oracle pass (C1-C4: the whole batch)
 PARITY_REQUESTS = {"C1": [0], "C2": [5, 27], "C3": [6], "C4": [7, 50], "C5": [33, 90]}   # post-timing sampled parity check
 
 
