@@ -394,7 +394,7 @@ static vx_status decode_dispatch(vx_ctx* c, const void* q, const vx_kv_pool* poo
                                  const DecodeOpts& opt = DecodeOpts()) {
   if (gqa_fp8_fast_supported(c->g))
     return check_cuda(c, launch_decode_gqa_fp8(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s,
-                                               opt.pdl, opt.budget), "vx_sparse_paged_decode (fp8 KV cache)");
+                                               opt.pdl, opt.budget, opt.summary_upd), "vx_sparse_paged_decode (fp8 KV cache)");
   if (kv_is_fp8(c->g))
     return check_cuda(c, launch_decode_fp8(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s),
                       "vx_sparse_paged_decode (fp8 KV cache)");
@@ -482,7 +482,7 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   // page, 72.1 / 74.0 / 75.8 with 2 / 3 / 4 -- the decode kernel's first TMA boxes queue behind the prefetches).
   PrefetchPlan pf;
   const int64_t esz = (int64_t)elem_size(c->g.dtype);
-  if (decode_folds_summary(c) && pool->stride_token == c->g.qk_dim && c->bpp == 1) {
+  if (decode_folds_summary(c) && !kv_is_fp8(c->g) && pool->stride_token == c->g.qk_dim && c->bpp == 1) {
     pf.k = pool->k;
     pf.v = c->g.kv_shared ? nullptr : pool->v;
     pf.page_bytes = pool->stride_page * esz;

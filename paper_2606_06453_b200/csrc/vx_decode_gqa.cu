@@ -368,7 +368,7 @@ int decode_gqa_splits(const vx_ctx* c, int n_req, int max_budget) {
   return splits;
 }
 
-bool decode_folds_summary(const vx_ctx* c) { return (gqa_mma_supported(c->g) || mla_tc_supported(c->g)); }
+bool decode_folds_summary(const vx_ctx* c) { return (gqa_mma_supported(c->g) || mla_tc_supported(c->g) || gqa_fp8_fast_supported(c->g)); }
 
 cudaError_t launch_decode_gqa_mma(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,

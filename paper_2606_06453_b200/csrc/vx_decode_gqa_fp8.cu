@@ -74,11 +74,13 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
                       const int32_t* __restrict__ sel_phys, const int32_t* __restrict__ sel_logical,
                       const int32_t* __restrict__ sel_count, int max_budget, int num_splits, float* __restrict__ part_o,
                       float* __restrict__ part_lse, int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ out,
-                      float* __restrict__ lse_out, const int32_t* __restrict__ budget_opt, int bpp) {
+                      float* __restrict__ lse_out, const int32_t* __restrict__ budget_opt, int bpp,
+                      uint8_t* __restrict__ summary_upd) {
   using namespace gq8;
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float s_m[WARPS][8], s_l[WARPS][8];
-  __shared__ int s_valid[WARPS][STAGES];
+  __shared__ int s_valid[WARPS][STAGES];         // valid tokens of the page staged in each slot (bit 8: the request's newest page)
+  __shared__ int s_phys[WARPS][STAGES];          // its physical id
   __shared__ int s_last;
 
   const int split = blockIdx.x, kvh = blockIdx.y, i = blockIdx.z;
@@ -132,15 +134,17 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
     if (p < my_pages) {
       const int r = r_begin + warp + p * WARPS;
       id_phys = phys_list[r];
-      id_valid = min(PAGE, n_tok - log_list[r] * PAGE);
+      const int lg = log_list[r];
+      id_valid = min(PAGE, n_tok - lg * PAGE) | (lg == newest_page ? 256 : 0);
     }
   };
   auto issue = [&](int p) {                     // all lanes: copy page p of this warp into slot p % STAGES
     const int phys = __shfl_sync(0xffffffffu, id_phys, p & 31);
-    const int nv = __shfl_sync(0xffffffffu, id_valid, p & 31);
+    const int venc = __shfl_sync(0xffffffffu, id_valid, p & 31);
+    const int nv = venc & 255;
     const int64_t base = pool_block_base(phys, stride_page, bpp, PAGE * stride_token) + (int64_t)kvh * stride_head;
     const uint32_t dst = ring_u32 + (uint32_t)(p % STAGES) * 2 * PAGEB;
-    if (lane == 0) s_valid[warp][p % STAGES] = nv;
+    if (lane == 0) { s_valid[warp][p % STAGES] = venc; s_phys[warp][p % STAGES] = phys; }
 #pragma unroll
     for (int it = 0; it < CP_ITERS; ++it) {
       const int x = it * kWarp + lane;
@@ -167,7 +171,9 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
   for (int p = 0; p < my_pages; ++p) {
     cp_async_wait<STAGES - 2>();                // page p has landed (this lane's copies)
     __syncwarp();                               // ... and every lane's; all lanes are done with page p - 1
-    const int valid = s_valid[warp][p % STAGES];
+    const int valid_enc = s_valid[warp][p % STAGES];
+    const int valid = valid_enc & 255;
+    const int phys_p = s_phys[warp][p % STAGES];
     {
       const int nxt = p + STAGES - 1;           // refill the slot page p - 1 used
       if ((nxt & 31) == 0 && nxt < my_pages) fetch_ids(nxt);
@@ -175,6 +181,30 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
       cp_async_commit();
     }
     const uint32_t kst = ring_u32 + (uint32_t)(p % STAGES) * 2 * PAGEB, vst = kst + PAGEB;
+
+    if (summary_upd != nullptr && (valid_enc & 256)) {
+      // (a1) this is the request's newest page: rebuild its min / max summary CODES from the staged keys (
+      // exact: the envelope of representable values is representable).  Lane owns 4 consecutive channels of the row.
+      const int c = lane >> 2, o16 = (lane & 3) * 4;
+      const uint8_t* kt = ring + (size_t)(p % STAGES) * 2 * PAGEB;
+      uint32_t w0, w1;
+      fp8x4_to_f16<TKV>(*reinterpret_cast<const uint32_t*>(kt + (c * 16) + o16), w0, w1);      // token 0 (c ^ 0 = c)
+      __half2 lo0 = *reinterpret_cast<__half2*>(&w0), lo1 = *reinterpret_cast<__half2*>(&w1), hi0 = lo0, hi1 = lo1;
+      for (int t = 1; t < valid; ++t) {
+        fp8x4_to_f16<TKV>(*reinterpret_cast<const uint32_t*>(kt + t * ROWB + ((c ^ (t & 7)) * 16) + o16), w0, w1);
+        const __half2 a = *reinterpret_cast<__half2*>(&w0), b = *reinterpret_cast<__half2*>(&w1);
+        lo0 = __hmin2(lo0, a); lo1 = __hmin2(lo1, b);
+        hi0 = __hmax2(hi0, a); hi1 = __hmax2(hi1, b);
+      }
+      auto pack4 = [](__half2 x, __half2 y) -> uint32_t {                   // four f16 that are fp8 values -> their codes
+        const __nv_fp8x2_storage_t p0 = __nv_cvt_halfraw2_to_fp8x2(*reinterpret_cast<__half2_raw*>(&x), __NV_SATFINITE, Fp8Interp<TKV>::kind);
+        const __nv_fp8x2_storage_t p1 = __nv_cvt_halfraw2_to_fp8x2(*reinterpret_cast<__half2_raw*>(&y), __NV_SATFINITE, Fp8Interp<TKV>::kind);
+        return (uint32_t)p0 | ((uint32_t)p1 << 16);
+      };
+      uint8_t* dst = summary_upd + (((int64_t)phys_p * num_kv_heads + kvh) * 2) * D + lane * 4;
+      *reinterpret_cast<uint32_t*>(dst) = pack4(lo0, lo1);
+      *reinterpret_cast<uint32_t*>(dst + D) = pack4(hi0, hi1);
+    }
 
     // S^T[16 tokens x 8 heads] = K[16 x D] . Q^T : one ldmatrix.x4 = two k-steps (tokens 0-7 / 8-15 x chunks 2 kk, 2 kk + 1)
     float s[4] = {0.f, 0.f, 0.f, 0.f};
@@ -312,7 +342,8 @@ static int decode_gqa_fp8_splits(const vx_ctx* c, int n_req, int max_budget) {
 template <typename TKV>
 static cudaError_t launch_gqa_fp8_t(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                     const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
-                                    int32_t max_budget, void* out, float* lse, cudaStream_t s, bool pdl, const int32_t* budget) {
+                                    int32_t max_budget, void* out, float* lse, cudaStream_t s, bool pdl, const int32_t* budget,
+                                    void* summary_upd) {
   const vx_geom& g = c->g;
   if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_gqa_fp8_kernel<TKV>), c->device, gq8::SMEM)) return e;
   const int splits = decode_gqa_fp8_splits(c, pt.batch, max_budget);
@@ -321,17 +352,18 @@ static cudaError_t launch_gqa_fp8_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const __nv_bfloat16*>(q), static_cast<const uint8_t*>(pool.k), static_cast<const uint8_t*>(pool.v),
       pool.stride_page, pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads,
       g.sm_scale * pool.k_scale * gq8::kLog2e, pool.v_scale, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits,
-      c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(out), lse, budget, c->bpp);
+      c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(out), lse, budget, c->bpp, static_cast<uint8_t*>(summary_upd));
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
 cudaError_t launch_decode_gqa_fp8(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
-                                  int32_t max_budget, void* out, float* lse, cudaStream_t s, bool pdl, const int32_t* budget) {
+                                  int32_t max_budget, void* out, float* lse, cudaStream_t s, bool pdl, const int32_t* budget,
+                                  void* summary_upd) {
   return c->g.kv_format == VX_KV_FP8_E4M3
-             ? launch_gqa_fp8_t<fp8_e4m3>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, pdl, budget)
-             : launch_gqa_fp8_t<fp8_e5m2>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, pdl, budget);
+             ? launch_gqa_fp8_t<fp8_e4m3>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, pdl, budget, summary_upd)
+             : launch_gqa_fp8_t<fp8_e5m2>(c, q, pool, pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, pdl, budget, summary_upd);
 }
 
 }  // namespace vx

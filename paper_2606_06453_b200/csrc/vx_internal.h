@@ -230,7 +230,8 @@ cudaError_t launch_decode_fp8(vx_ctx* c, const void* q, const vx_kv_pool& pool, 
 bool gqa_fp8_fast_supported(const vx_geom& g);           // the mma kernel of vx_decode_gqa_fp8.cu (page 16, d = 128)
 cudaError_t launch_decode_gqa_fp8(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                                   const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
-                                  int32_t max_budget, void* out, float* lse, cudaStream_t s, bool pdl, const int32_t* budget);
+                                  int32_t max_budget, void* out, float* lse, cudaStream_t s, bool pdl, const int32_t* budget,
+                                  void* summary_upd);
 
 // geometry support predicates (used by vx_create validation)
 bool gqa_geometry_supported(const vx_geom& g);

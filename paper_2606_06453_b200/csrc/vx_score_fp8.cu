@@ -19,6 +19,7 @@ namespace vx {
 // [Qm | Qp] fp32 per (request, KV head): thread = one channel of one (request, KV head)
 __global__ void __launch_bounds__(256)
 qvec_fp8_kernel(const __nv_bfloat16* __restrict__ q, int batch, int num_q_heads, int num_kv_heads, int d, float* __restrict__ qvec) {
+  pdl_trigger();                                       // the score kernel may start streaming summaries under me
   const int grp = num_q_heads / num_kv_heads;
   const int64_t n = (int64_t)batch * num_kv_heads * d;
   for (int64_t x = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; x < n; x += (int64_t)gridDim.x * blockDim.x) {
@@ -101,6 +102,7 @@ score_fp8_kernel(const uint8_t* __restrict__ summary, const float* __restrict__ 
   }
   for (int p = 0; p < my_pages; ++p) {
     const int flat = begin + warp + p * kS8Warps;
+    if (cur_req < 0) pdl_wait();                         // the query vectors come from qvec_fp8_kernel, my predecessor (my copies are already in flight)
     if (flat >= cur_end || cur_req < 0) load_qreg(flat);          // (warp-uniform)
     cp_async_wait<kS8Stages - 2>();                      // page p has landed (this lane's copies; a lane reads only its own)
     float part[NT16];
@@ -267,6 +269,7 @@ score_fp8_mma_kernel(const uint8_t* __restrict__ summary, const float* __restric
   }
   for (int p = 0; p < my_tiles; ++p) {
     const int flat0 = tile_page0(p), flat1 = flat0 + 1;
+    if (cur_req < 0) pdl_wait();                          // the query vectors come from qvec_fp8_kernel, my predecessor (my copies are already in flight)
     if (flat0 >= cur_end || cur_req < 0) load_qreg(flat0);         // (warp-uniform)
     cp_async_wait<kM8Stages - 2>();
     __syncwarp();                                         // every lane's copies of tile p have landed
@@ -318,10 +321,11 @@ static cudaError_t launch_score_fp8_t(vx_ctx* c, const void* q, const void* summ
     if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(score_fp8_mma_kernel<T>), c->device, smem_bytes)) return e;
     int grid = c->num_sms * 2;
     if (grid > (pt.total_pages + 1) / 2) grid = (pt.total_pages + 1) / 2;
-    score_fp8_mma_kernel<T><<<grid, kM8Warps * kWarp, smem_bytes, s>>>(static_cast<const uint8_t*>(summary), c->ws.fp8_qvec,
-                                                                      pt.page_indptr, pt.page_indices, pt.batch, pt.total_pages, scores);
+    cudaError_t e = launch_kernel(score_fp8_mma_kernel<T>, dim3(grid), dim3(kM8Warps * kWarp), (size_t)smem_bytes, s, true,
+                                  static_cast<const uint8_t*>(summary), (const float*)c->ws.fp8_qvec, pt.page_indptr, pt.page_indices,
+                                  pt.batch, pt.total_pages, scores);
     c->launches += 1;
-    return cudaGetLastError();
+    return e != cudaSuccess ? e : cudaGetLastError();
   }
   const int pagev = g.num_kv_heads * (2 * g.qk_dim / 16);
   const int nt16 = (pagev + kWarp - 1) / kWarp;
@@ -332,8 +336,9 @@ static cudaError_t launch_score_fp8_t(vx_ctx* c, const void* q, const void* summ
   do {                                                                                                                      \
     constexpr int smem_bytes = kS8Warps * kS8Stages * N * kWarp * 16;                                                       \
     if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(score_fp8_kernel<T, N>), c->device, smem_bytes)) return e; \
-    score_fp8_kernel<T, N><<<grid, kS8Warps * kWarp, smem_bytes, s>>>(sm, c->ws.fp8_qvec, pt.page_indptr, pt.page_indices,  \
-                                                                     pt.batch, pt.total_pages, g.num_kv_heads, g.qk_dim, scores); \
+    if (cudaError_t e = launch_kernel(score_fp8_kernel<T, N>, dim3(grid), dim3(kS8Warps * kWarp), (size_t)smem_bytes, s, true, sm,  \
+                                      (const float*)c->ws.fp8_qvec, pt.page_indptr, pt.page_indices, pt.batch, pt.total_pages,    \
+                                      g.num_kv_heads, g.qk_dim, scores)) return e;                                                \
   } while (0)
   switch (nt16) {
     case 1: VX_GO(1); break;
