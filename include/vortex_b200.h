@@ -159,16 +159,8 @@ int32_t vx_last_launch_count(const vx_ctx *ctx);
  *                           counter (falls back to CHAINED for batches / requests beyond what it keeps on chip)
  *    All schedules compute the same selection bit for bit; outputs agree to rounding (different split sizes).
  *  VX_OPT_MLA_FLAT_SPLITS / VX_OPT_MLA_FLAT_WAVES   0 (default) = chosen by the library; > 0 = decode shares per request /
- *                           interleaved waves of the summary stream of the FLAT schedule (tuning knobs)
- *  VX_OPT_STEP_OVERLAP   how the kernels of vx_sparse_decode_step depend on one another (GQA geometries on the mma decode
- *                        kernel, exact selection): VX_STEP_OVERLAP_OFF = each kernel waits for the whole grid before it
- *                        (programmatic dependent launch); VX_STEP_OVERLAP_ON = the score kernel walks the batch in waves
- *                        and counts finished scores per (request, KV head), selection starts per request beside the
- *                        running score kernel, a decode CTA waits only for its own unit's selection;
- *                        VX_STEP_OVERLAP_AUTO (default) = the library's choice.  Same results bit for bit.
- *  VX_OPT_STEP_WAVES     0 (default) = chosen by the library; > 0 = waves of the overlapped step's score kernel */
-enum { VX_OPT_MLA_STEP = 1, VX_OPT_MLA_FLAT_SPLITS = 2, VX_OPT_MLA_FLAT_WAVES = 3, VX_OPT_STEP_OVERLAP = 4, VX_OPT_STEP_WAVES = 5 };
-enum { VX_STEP_OVERLAP_AUTO = 0, VX_STEP_OVERLAP_OFF = 1, VX_STEP_OVERLAP_ON = 2 };
+ *                           interleaved waves of the summary stream of the FLAT schedule (tuning knobs) */
+enum { VX_OPT_MLA_STEP = 1, VX_OPT_MLA_FLAT_SPLITS = 2, VX_OPT_MLA_FLAT_WAVES = 3 };
 enum { VX_MLA_STEP_AUTO = 0, VX_MLA_STEP_FUSED = 1, VX_MLA_STEP_CHAINED = 2, VX_MLA_STEP_FLAT = 3 };
 vx_status vx_set_option(vx_ctx *ctx, int32_t option, int32_t value);
 

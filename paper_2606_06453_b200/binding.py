@@ -22,8 +22,7 @@ VX_STEP_UPDATE_SUMMARY = 1
 VX_STEP_APPROX_TOPK = 2
 VX_TRACE_SCORE, VX_TRACE_TOPK, VX_TRACE_DECODE = 1, 2, 4
 VX_KV_SAME, VX_KV_FP8_E4M3, VX_KV_FP8_E5M2 = 0, 1, 2
-VX_OPT_MLA_STEP, VX_OPT_MLA_FLAT_SPLITS, VX_OPT_MLA_FLAT_WAVES, VX_OPT_STEP_OVERLAP, VX_OPT_STEP_WAVES = 1, 2, 3, 4, 5
-VX_STEP_OVERLAP_AUTO, VX_STEP_OVERLAP_OFF, VX_STEP_OVERLAP_ON = 0, 1, 2
+VX_OPT_MLA_STEP, VX_OPT_MLA_FLAT_SPLITS, VX_OPT_MLA_FLAT_WAVES = 1, 2, 3
 VX_MLA_STEP_AUTO, VX_MLA_STEP_FUSED, VX_MLA_STEP_CHAINED, VX_MLA_STEP_FLAT = 0, 1, 2, 3
 
 EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",

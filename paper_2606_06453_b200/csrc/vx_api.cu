@@ -50,9 +50,6 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   w.flat_sync = static_cast<int32_t*>(take(mla ? step_mla_flat_workspace_ints(max_batch) * 4 : 0));
   w.blk_indptr = static_cast<int32_t*>(take(bpp > 1 ? (B + 1) * 4 : 0));
   w.blk_indices = static_cast<int32_t*>(take(bpp > 1 ? (size_t)max_total_pages * bpp * 4 : 0));
-  w.qvec = static_cast<float*>(take(B * Hkv * 2 * (size_t)g.qk_dim * 4));
-  w.ready_cnt = static_cast<int32_t*>(take(B * Hkv * 4));
-  w.sel_flag = static_cast<int32_t*>(take(B * Hkv * 4));
   w.fp8_qvec = static_cast<float*>(take(kv_is_fp8(g) ? B * Hkv * 2 * (size_t)g.qk_dim * 4 : 0));
   w.bytes = off;
   return w;
@@ -65,10 +62,7 @@ cudaError_t ensure_dyn_smem(const void* kernel, int device, int bytes) {
   static std::set<std::pair<const void*, int>> done;
   std::lock_guard<std::mutex> lock(mu);
   if (done.count({kernel, device})) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
-  // the largest shared-memory carve-out for every kernel of a step: an SM whose carve-out was sized for the score kernel's
-  // two CTAs does not take a selection CTA beside them, however small (overlapped step)
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
   if (e == cudaSuccess) done.insert({kernel, device});
   return e;
 }
@@ -234,9 +228,6 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->launches = 0;
   c->err[0] = 0;
   c->mla_step = VX_MLA_STEP_AUTO;
-  c->epoch = 0;
-  c->overlap = VX_STEP_OVERLAP_AUTO;
-  c->waves = 0;
   c->pinned_small = nullptr;
   e = cudaHostAlloc(reinterpret_cast<void**>(&c->pinned_small), (3 * (size_t)(max_batch > 0 ? max_batch : 1) + 1) * 4, cudaHostAllocDefault);
   if (e != cudaSuccess) {
@@ -246,8 +237,6 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->flat_splits = c->flat_waves = 0;
   // split-arrival counters start at zero and every step leaves them at zero
   e = cudaMemset(c->ws.unit_counter, 0, (size_t)(max_batch > 0 ? max_batch : 1) * g->num_kv_heads * 4);
-  if (e == cudaSuccess) e = cudaMemset(c->ws.ready_cnt, 0, (size_t)(max_batch > 0 ? max_batch : 1) * g->num_kv_heads * 4);
-  if (e == cudaSuccess) e = cudaMemset(c->ws.sel_flag, 0, (size_t)(max_batch > 0 ? max_batch : 1) * g->num_kv_heads * 4);
   if (e == cudaSuccess && g->kv_shared) e = cudaMemset(c->ws.flat_sync, 0, step_mla_flat_workspace_ints(max_batch) * 4);
   if (e == cudaSuccess) e = cudaDeviceSynchronize();
   if (e != cudaSuccess) {
@@ -372,8 +361,6 @@ vx_status vx_set_option(vx_ctx* c, int32_t option, int32_t value) {
     c->mla_step = value;
     return VX_OK;
   }
-  if (option == VX_OPT_STEP_OVERLAP && value >= VX_STEP_OVERLAP_AUTO && value <= VX_STEP_OVERLAP_ON) { c->overlap = value; return VX_OK; }
-  if (option == VX_OPT_STEP_WAVES && value >= 0 && value <= 64) { c->waves = value; return VX_OK; }
   if (option == VX_OPT_MLA_FLAT_SPLITS && value >= 0 && value <= kMaxSplits) { c->flat_splits = value; return VX_OK; }
   if (option == VX_OPT_MLA_FLAT_WAVES && value >= 0 && value <= 8) { c->flat_waves = value; return VX_OK; }
   return fail(c, VX_ERR_INVALID_ARG, "unknown option %d / value %d", option, value);
@@ -485,49 +472,6 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
     } else if (vx_status st = check_cuda(c, launch_summary_update(c, *pool, *pt, nullptr, summary, s), "summary update")) {
       return st;
     }
-  }
-  // ---- overlapped step (GQA on the mma decode kernel, exact selection): the score kernel walks the
-  // batch in waves and counts finished scores per (request, KV head); the requests of all waves but the last are selected
-  // by 256-thread kernels that fit BESIDE the score kernel's CTAs and start the moment their request is complete; the
-  // last wave's requests take the fast selection kernel; every decode CTA waits for its own unit's selection only.
-  const bool overlap = c->overlap != VX_STEP_OVERLAP_OFF && !c->g.kv_shared && gqa_mma_supported(c->g) && !kv_is_fp8(c->g) &&
-                       ap.tolerate_ratio <= 0.f && pt->batch >= 2 && pt->max_pages_per_req <= kTopkRegMaxPages &&
-                       (c->overlap == VX_STEP_OVERLAP_ON || pt->batch * c->g.num_kv_heads <= 2 * c->num_sms);
-  if (overlap) {
-    c->epoch = c->epoch == 0x7fffffff ? 1 : c->epoch + 1;
-    int waves = c->waves > 0 ? c->waves : (pt->batch < 8 ? pt->batch : 8);
-    if (waves > pt->batch) waves = pt->batch;
-    ReqRange all;
-    all.waves = waves;
-    all.ready_cnt = c->ws.ready_cnt;
-    all.qvec = c->ws.qvec;
-    if (vx_status st = check_cuda(c, launch_page_score(c, q, summary, *pt, c->ws.scores, s, all), "page score")) return st;
-    // requests that (for equal lengths) are complete before the last wave -- the last two waves when the co-resident
-    // selection of a long request would not finish in time for its decode
-    const int fast_waves = (pt->max_pages_per_req > 4096 && waves > 2) ? 2 : 1;
-    const int early = (int)((int64_t)pt->batch * (waves - fast_waves) / waves);
-    PrefetchPlan pfo;
-    pfo.ready_cnt = c->ws.ready_cnt;
-    pfo.sel_flag = c->ws.sel_flag;
-    pfo.epoch = c->epoch;
-    if (early > 0) {
-      pfo.slim = true;
-      ReqRange rr;
-      rr.begin = 0;
-      rr.count = early;
-      if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, s, true, rr, pfo, ap),
-                                    "top-k pages (early requests)")) return st;
-    }
-    pfo.slim = false;
-    ReqRange rr;
-    rr.begin = early;
-    rr.count = pt->batch - early;
-    if (vx_status st = check_cuda(c, launch_topk_pages(c, c->ws.scores, *pt, budget, max_budget, sp, sl, sc, s, true, rr, pfo, ap),
-                                  "top-k pages (last wave)")) return st;
-    opt.sel_flag = c->ws.sel_flag;
-    opt.ready_cnt = c->ws.ready_cnt;
-    opt.epoch = c->epoch;
-    return decode_dispatch(c, q, pool, pt, sp, sl, sc, max_budget, out, lse, s, opt);
   }
   if (vx_status st = check_cuda(c, launch_page_score(c, q, summary, *pt, c->ws.scores, s), "page score")) return st;
   // L2 prefetch plan for the decode kernel's first pages (fast decode paths with contiguous page chunks only): the

@@ -146,51 +146,6 @@ __device__ __forceinline__ void l2_prefetch(const void* p, uint32_t bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
-// ---- the overlapped step: kernels of one step wait for the results they need, not for whole grids.
-// Producers are always launched earlier in the same stream and never wait on their consumers, so every wait terminates.
-__device__ __forceinline__ int ld_acquire_gpu_s32(const int32_t* p) {
-  int v;
-  asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-  return v;
-}
-__device__ __forceinline__ void st_release_gpu_s32(int32_t* p, int v) {
-  asm volatile("st.release.gpu.global.s32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
-}
-// (whole CTA) wait until `expected` scores of this unit have been written by the score kernel; plain PDL wait otherwise
-__device__ __forceinline__ void wait_unit_scores(const int32_t* ready_cnt, int unit, int expected) {
-  if (ready_cnt == nullptr) { pdl_wait(); return; }
-  if (threadIdx.x == 0) {
-    int spins = 0;                                 // (a producer that never reports is a bug: fail loudly after ~2 s, do not hang the GPU)
-    while (ld_acquire_gpu_s32(ready_cnt + unit) < expected) {
-      __nanosleep(200);
-      if (++spins > (1 << 23)) __trap();
-    }
-  }
-  __syncthreads();
-}
-// (whole CTA, after its last store of the unit's selection) publish it to the decode kernel
-__device__ __forceinline__ void publish_unit_selection(int32_t* sel_flag, int unit, int epoch) {
-  if (sel_flag == nullptr) return;
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    __threadfence();
-    st_release_gpu_s32(sel_flag + unit, epoch);
-  }
-}
-// (whole CTA) wait for the unit's selection; the first split also clears the unit's score counter for the next step
-__device__ __forceinline__ void wait_unit_selection(const int32_t* sel_flag, int32_t* ready_cnt, int unit, int epoch, bool first_split) {
-  if (sel_flag == nullptr) { pdl_wait(); return; }
-  if (threadIdx.x == 0) {
-    int spins = 0;
-    while (ld_acquire_gpu_s32(sel_flag + unit) != epoch) {
-      __nanosleep(200);
-      if (++spins > (1 << 23)) __trap();
-    }
-    if (first_split && ready_cnt != nullptr) ready_cnt[unit] = 0;
-  }
-  __syncthreads();
-}
-
 __device__ __forceinline__ float ldcg_f32(const float* p) {
   float v;
   asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));

@@ -64,8 +64,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
                       int max_budget, int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                       int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
                       __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0,
-                      const int32_t* __restrict__ budget_opt, int bpp, const int32_t* __restrict__ sel_flag,
-                      int32_t* __restrict__ ready_cnt, int epoch) {
+                      const int32_t* __restrict__ budget_opt, int bpp) {
   constexpr int ROWB = D * 2;                 // bytes per token row
   constexpr int CH = ROWB / 16;               // 16-byte chunks per row
   constexpr int PAGEB = kGqaPage * ROWB;      // bytes of one K (or V) page chunk
@@ -99,9 +98,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     }
   }
   if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 1);
-  // the selection lists come from the preceding kernel of the step: its whole grid (griddepcontrol.wait), or -- overlapped
-  // step -- just this (request, KV head)'s selection, while other units are still being scored or selected
-  wait_unit_selection(sel_flag, ready_cnt, i * num_kv_heads + kvh, epoch, split == 0);
+  pdl_wait();                                   // the selection lists come from the preceding kernel of the step
   if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 2);
 
   const int cnt = cnt_known >= 0 ? cnt_known : sel_count[i * num_kv_heads + kvh];
@@ -353,7 +350,7 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const __nv_bfloat16*>(pool.v), pool.stride_page, pool.stride_token, pool.stride_head,
       g.num_q_heads, g.num_kv_heads, g.sm_scale * kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget,
       splits, c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
-      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget, c->bpp, opt.sel_flag, opt.ready_cnt, opt.epoch);
+      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget, c->bpp);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

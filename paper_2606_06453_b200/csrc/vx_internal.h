@@ -31,9 +31,6 @@ struct Workspace {               // device pointers carved from the caller's wor
   int32_t* flat_sync;            // counters and per-request flags; zero between steps
   int32_t* blk_indptr;           // blocks finer than the page: the page table expanded into a block table, [max_batch + 1]
   int32_t* blk_indices;          // [max_total_pages * bpp] physical block ids
-  float* qvec;                   // overlapped step: [max_batch, Hkv, 2 qk_dim] query vectors of the score kernel
-  int32_t* ready_cnt;            // overlapped step: scores written per (request, KV head); zero between steps
-  int32_t* sel_flag;             // ... selection published per (request, KV head): the epoch of the step that wrote it
   float* fp8_qvec;               // fp8 KV cache: [max_batch, Hkv, 2 qk_dim] query vectors [Qm | Qp] of the score kernel (vx_score_fp8.cu)
   size_t bytes;                  // total
 };
@@ -66,9 +63,6 @@ struct vx_ctx {
   int32_t launches;              // kernels enqueued by the last compute call
   vx::ApproxPlan approx;         // vx_set_topk_approx: used by a fused step with VX_STEP_APPROX_TOPK
   int32_t mla_step;              // VX_OPT_MLA_STEP
-  int32_t epoch;                 // fused steps run on this context (the value the selection flags take)
-  int32_t overlap;               // VX_OPT_STEP_OVERLAP
-  int32_t waves;                 // VX_OPT_STEP_WAVES: 0 = the library's choice
   int32_t bpp;                   // selection blocks per physical page (vx_geom.block_size); g.page_size holds the BLOCK size
   int32_t user_page_size;        // tokens per physical page as the caller gave it
   int32_t* pinned_small;         // pinned host staging [3 max_batch + 1] for vx_sparse_decode_step_host's small arrays
@@ -132,13 +126,6 @@ inline cudaError_t launch_kernel_cluster(void (*kernel)(KArgs...), dim3 grid, di
 struct ReqRange {
   int begin = 0;
   int count = -1;
-  // overlapped step: the score kernel walks the flat page list in `waves` interleaved passes, so
-  // that the requests complete one after the other while the stream is still running, and counts the scores it has
-  // written per (request, KV head) in ready_cnt (release); the selection kernels wait on those counters
-  int waves = 1;
-  int32_t* ready_cnt = nullptr;
-  float* qvec = nullptr;         // [batch, Hkv, row] workspace: with many waves every CTA meets every request, so the query
-                                 // vectors [Qm | Qp] are built once by a small kernel and read from L2, not rebuilt per CTA
 };
 
 // What the selection kernel prefetches into L2 for the decode kernel that follows it in a step: the first
@@ -151,12 +138,6 @@ struct PrefetchPlan {
   int64_t page_bytes = 0, head_bytes = 0;        // byte strides of a page / a KV head in the pool
   uint32_t chunk_bytes = 0;                      // page_size * row bytes, contiguous
   int splits = 1, pages_per_split = 0;
-  // overlapped step: wait for this unit's scores (counter) instead of the whole score grid, and publish the unit's
-  // selection (flag = the step's epoch) for the decode kernel
-  const int32_t* ready_cnt = nullptr;
-  int32_t* sel_flag = nullptr;
-  int32_t epoch = 0;
-  bool slim = false;                             // take the 256-thread kernels that fit beside the score kernel's CTAs
 };
 // phase tracing (-DVX_TRACE builds; cudaErrorNotSupported otherwise): one setter per kernel file
 cudaError_t vx_trace_set_score(long long* buf, int ctas);
@@ -173,9 +154,6 @@ struct DecodeOpts {
   void* summary_upd = nullptr;   // non-null: also rebuild the summary of each request's newest page (a1), whose
                                  // keys the kernel stages anyway (it is a forced local page)
   bool pdl = false;              // launched as a programmatic dependent of the preceding kernel
-  const int32_t* sel_flag = nullptr; // overlapped step: wait for the unit's selection flag (== epoch) instead of the whole grid
-  int32_t* ready_cnt = nullptr;      // ... and clear the unit's score counter for the next step
-  int32_t epoch = 0;
   const int32_t* budget = nullptr;   // fused step: sel_count[i, h] is known to be min(budget[i], max_budget, P_i), so the kernel
                                  // need not wait for the selection kernel to read it (one L2 round trip less after the wait)
 };

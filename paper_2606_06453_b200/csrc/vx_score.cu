@@ -23,7 +23,6 @@
 
 namespace vx {
 
-constexpr int kScIndptrCache = 256;             // requests whose page_indptr a CTA of the many-wave score kernel keeps in shared memory
 constexpr int kScConsumerWarps = 8;
 constexpr int kScThreads = (kScConsumerWarps + 1) * kWarp;
 
@@ -75,11 +74,10 @@ struct GroupIter {
 };
 
 template <typename T, int D, int PG, int HKV, int kScStages, int AGG, int KIND>
-__global__ void __launch_bounds__(kScThreads, 2)   // GQA pools: <= 72 registers, so that a 256-thread selection CTA fits beside two of these (overlapped step)
+__global__ void __launch_bounds__(kScThreads, 2)
 score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int batch,
              const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices, int total_pages,
-             float* __restrict__ scores, int req_begin, int req_end, int flat_lo_host, int flat_span_host, int n_waves,
-             int32_t* __restrict__ ready_cnt, const float* __restrict__ qvec_g) {
+             float* __restrict__ scores, int req_begin, int req_end, int flat_lo_host, int flat_span_host) {
   constexpr int PER = Elem<T>::kPerVec;
   // envelope: [min | max] of one (page, KV head); centroid (block top-k): the mean key, d elements
   constexpr int ROW_ELEMS = KIND == VX_SUMMARY_CENTROID ? D : 2 * D;
@@ -98,7 +96,6 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
 
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ __align__(8) uint64_t s_full[kScStages], s_empty[kScStages];
-  __shared__ int32_t s_indptr[kScIndptrCache + 1];       // many waves: the request boundaries, read once (every slice start looks them up)
   float* s_q = reinterpret_cast<float*>(smem + (size_t)kScStages * STAGE_BYTES);   // SUM: [HKV][2*D] fp32: Qm | Qp
   T* s_qh = reinterpret_cast<T*>(smem + (size_t)kScStages * STAGE_BYTES);          // MAX: [Hq][2*D] in T: min(q_h,0) | max(q_h,0)
 
@@ -120,18 +117,8 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     for (int64_t o = off; o < min(per_cta * (blockIdx.x + 1), q_bytes); o += kScConsumerWarps * kWarp * 128)
       asm volatile("prefetch.global.L2 [%0];" ::"l"(qb + o));
   }
-  // wave w covers the flat pages [span w / W, span (w + 1) / W) of the window; inside a wave this CTA takes the blockIdx-th
-  // of gridDim equal parts.  One wave: the plain flat split.
-  auto slice = [&](int w, int& b, int& e) {
-    const int wlo = (int)((int64_t)flat_span * w / n_waves), whi = (int)((int64_t)flat_span * (w + 1) / n_waves);
-    b = flat_lo + wlo + (int)((int64_t)(whi - wlo) * blockIdx.x / gridDim.x);
-    e = flat_lo + wlo + (int)((int64_t)(whi - wlo) * (blockIdx.x + 1) / gridDim.x);
-  };
-  const int32_t* ip = page_indptr;                // where GroupIter reads the request boundaries
-  if (n_waves > 1 && batch <= kScIndptrCache) {
-    for (int x = threadIdx.x; x <= batch; x += kScThreads) s_indptr[x] = page_indptr[x];
-    ip = s_indptr;
-  }
+  const int begin = flat_lo + (int)((int64_t)flat_span * blockIdx.x / gridDim.x);
+  const int end = flat_lo + (int)((int64_t)flat_span * (blockIdx.x + 1) / gridDim.x);
   if (threadIdx.x == 0) {
     for (int s = 0; s < kScStages; ++s) {
       sc_mbar_init(smem_u32(&s_full[s]), 1);
@@ -141,36 +128,19 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
   }
   __syncthreads();
   pdl_trigger();                                // single-wave persistent grid: the selection kernel may queue up behind us
+  if (begin >= end) return;
   int first, count, req;
-  int begin, end;
 
   if (warp == kScConsumerWarps) {
     // ---- producer: one bulk copy per page (all KV heads of the page are contiguous) ----------
     // The physical ids of the CTA's flat page range are prefetched 32 at a time (one coalesced load, two chunks
     // in registers), so that no index load sits between a freed stage and its refill.
-    int g = 0;                                            // groups issued so far: the ring's phases run on across the waves
-    // the first two id chunks of the NEXT slice are requested while this slice streams: a slice start then waits for no load
-    int nx_cur = 0, nx_nxt = 0;
-    {
-      int b0, e0;
-      slice(0, b0, e0);
-      nx_cur = b0 + lane < e0 ? page_indices[b0 + lane] : 0;
-      nx_nxt = b0 + kWarp + lane < e0 ? page_indices[b0 + kWarp + lane] : 0;
-    }
-    for (int w = 0; w < n_waves; ++w) {
-    slice(w, begin, end);
-    int id_cur = nx_cur, id_nxt = nx_nxt;
-    if (w + 1 < n_waves) {
-      int b1, e1;
-      slice(w + 1, b1, e1);
-      nx_cur = b1 + lane < e1 ? page_indices[b1 + lane] : 0;
-      nx_nxt = b1 + kWarp + lane < e1 ? page_indices[b1 + kWarp + lane] : 0;
-    }
-    if (begin >= end) continue;
     int chunk0 = begin;                                   // flat index of id_cur's lane 0
-    GroupIter it(begin, end, batch, ip);                  // (its loads fly together with the id loads above)
-    if (lane == 0 && w == 0) VX_TRACE_STAMP(blockIdx.x, 1);
-    for (; it.next(PG, first, count, req); ++g) {
+    int id_cur = chunk0 + lane < end ? page_indices[chunk0 + lane] : 0;
+    int id_nxt = chunk0 + kWarp + lane < end ? page_indices[chunk0 + kWarp + lane] : 0;
+    GroupIter it(begin, end, batch, page_indptr);         // (its loads fly together with the id loads above)
+    if (lane == 0) VX_TRACE_STAMP(blockIdx.x, 1);
+    for (int g = 0; it.next(PG, first, count, req); ++g) {
       const int s = g % kScStages;
       if (g >= kScStages) sc_mbar_wait(smem_u32(&s_empty[s]), ((g / kScStages) - 1) & 1);
       const uint32_t bar = smem_u32(&s_full[s]);
@@ -191,55 +161,19 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
       if (lane == 0 && g == 0) VX_TRACE_STAMP(blockIdx.x, 2);
       if (lane == 0 && g == kScStages - 1) VX_TRACE_STAMP(blockIdx.x, 3);
     }
-    }
     if (lane == 0) VX_TRACE_STAMP(blockIdx.x, 4);
     return;
   }
 
   // ---- consumers: warp w owns KV head w % HKV and rows w + 8k of every group ---------------------
+  GroupIter it(begin, end, batch, page_indptr);
   const int grp = num_q_heads / HKV;
   const int kvh = warp % HKV;
   float qreg[NIT][PER];
   int cur_req = -1;
-  int g = 0, done_rows = 0;                      // scores this warp has written for (cur_req, kvh) and not yet reported
-  auto report = [&]() {                          // release: the warp's score stores happen-before the counter update
-    if (ready_cnt != nullptr && done_rows > 0) {
-      __syncwarp();
-      if (lane == 0) asm volatile("red.release.gpu.global.add.s32 [%0], %1;" ::"l"(ready_cnt + cur_req * HKV + kvh), "r"(done_rows) : "memory");
-    }
-    done_rows = 0;
-  };
-  for (int w = 0; w < n_waves; ++w) {
-  slice(w, begin, end);
-  if (begin >= end) continue;
-  if (threadIdx.x == 0 && w >= 1 && w <= 3) VX_TRACE_STAMP(blockIdx.x, 11 + w);      // (trace builds: consumer enters waves 1..3)
-  GroupIter it(begin, end, batch, ip);
-  for (; it.next(PG, first, count, req); ++g) {
+  for (int g = 0; it.next(PG, first, count, req); ++g) {
     const int s = g % kScStages;
-    if (req != cur_req && qvec_g != nullptr) {   // many waves: the request's query vector was built once (qvec_kernel): my slice, from L2
-      report();
-      if (cur_req < 0) pdl_wait();               // (qvec_kernel is my predecessor in the stream)
-      cur_req = req;
-      if constexpr (AGG == VX_AGG_SUM) {
-        const float* src = qvec_g + ((int64_t)req * HKV + kvh) * ROW_ELEMS;
-#pragma unroll
-        for (int t = 0; t < NIT; ++t) {
-          const int c = NARROW ? lane % NCH : lane + t * kWarp;
-          if (NCH % kWarp == 0 || c < NCH) {
-#pragma unroll
-            for (int e = 0; e < PER; e += 4) {
-              const float4 x = *reinterpret_cast<const float4*>(src + c * PER + e);
-              qreg[t][e] = x.x; qreg[t][e + 1] = x.y; qreg[t][e + 2] = x.z; qreg[t][e + 3] = x.w;
-            }
-          } else {
-#pragma unroll
-            for (int e = 0; e < PER; ++e) qreg[t][e] = 0.f;
-          }
-        }
-      }
-    }
     if (req != cur_req) {                        // new request: rebuild [Qm | Qp] for all KV heads (rare)
-      report();
       if (threadIdx.x == 0) VX_TRACE_STAMP(blockIdx.x, cur_req < 0 ? 5 : 7);
       asm volatile("bar.sync 1, %0;" ::"n"(kScConsumerWarps * kWarp));
       if constexpr (AGG == VX_AGG_MAX) {
@@ -347,7 +281,6 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     sc_mbar_wait(smem_u32(&s_full[s]), (g / kScStages) & 1);
     if (threadIdx.x == 0 && g == 0) VX_TRACE_STAMP(blockIdx.x, 9);
     const int rows = count * HKV;                // row r = page (r / HKV), head (r % HKV)
-    done_rows += rows > warp ? (rows - warp + kScConsumerWarps - 1) / kScConsumerWarps : 0;   // my rows: warp, warp + 8, ..
     if constexpr (NARROW) {
       constexpr int KIT = RPW / RPI;             // instructions per group; instruction i covers rows warp + 8 (i RPI + lane / NCH)
       const uint8_t* st = smem + (size_t)s * STAGE_BYTES + (lane % NCH) * 16;
@@ -468,8 +401,6 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     const int r = warp + (lane / LPR) * kScConsumerWarps;
     if ((lane % LPR) == 0 && r < rows) scores[(int64_t)kvh * total_pages + first + r / HKV] = tot;
   }
-  report();                                      // the wave is done: what it completed may be selected now
-  }
   if (threadIdx.x == 0) VX_TRACE_STAMP(blockIdx.x, 11);
 }
 
@@ -487,30 +418,6 @@ bool score_geometry_supported(const vx_geom& g) {
   if (hkv != 1 && hkv != 2 && hkv != 4 && hkv != 8) return false;   // a consumer warp owns one KV head
   if (g.dtype == VX_DT_BF16) return g.qk_dim == 128 || g.qk_dim == 64 || g.qk_dim == 576 || g.qk_dim == 256;
   return g.qk_dim == 64 || g.qk_dim == 128;
-}
-
-// [Qm | Qp] (envelope) or [Qsum] (centroid) of every (request, KV head), fp32, summed over the group's heads in the order the
-// score kernel's own rebuild uses (head by head), so that scores are bit-identical whichever way the vector is obtained
-template <typename T, int KIND>
-__global__ void __launch_bounds__(256)
-qvec_kernel(const T* __restrict__ q, int batch, int num_q_heads, int num_kv_heads, int d, float* __restrict__ qvec) {
-  const int grp = num_q_heads / num_kv_heads;
-  const int row = KIND == VX_SUMMARY_CENTROID ? d : 2 * d;
-  const int64_t n = (int64_t)batch * num_kv_heads * d;
-  for (int64_t x = blockIdx.x * (int64_t)blockDim.x + threadIdx.x; x < n; x += (int64_t)gridDim.x * blockDim.x) {
-    const int c = (int)(x % d);
-    const int64_t rk = x / d;                            // request * Hkv + kvh
-    const int i = (int)(rk / num_kv_heads), kvh = (int)(rk % num_kv_heads);
-    float qp = 0.f, qm = 0.f;
-    for (int h = 0; h < grp; ++h) {
-      const float v = Elem<T>::to_float(q[((int64_t)i * num_q_heads + kvh * grp + h) * d + c]);
-      if constexpr (KIND == VX_SUMMARY_CENTROID) qp += v;
-      else { qp += fmaxf(v, 0.f); qm += fminf(v, 0.f); }
-    }
-    if constexpr (KIND == VX_SUMMARY_CENTROID) qvec[rk * row + c] = qp;
-    else { qvec[rk * row + c] = qm; qvec[rk * row + d + c] = qp; }
-  }
-  pdl_trigger();
 }
 
 constexpr int pow2_floor(int x) { int p = 1; while (2 * p <= x) p *= 2; return p; }
@@ -536,21 +443,12 @@ static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summar
   const int64_t est_pages = rr.count < 0 ? pt.total_pages : (int64_t)pt.total_pages * rr.count / (pt.batch > 0 ? pt.batch : 1) + 1;
   if ((int64_t)ctas * min_pages > est_pages) ctas = (int)((est_pages + min_pages - 1) / min_pages);
   if (ctas < 1) ctas = 1;
-  const bool use_qvec = rr.qvec != nullptr && rr.waves > 1 && AGG == VX_AGG_SUM && HKV > 1 && rr.count < 0;
-  if (use_qvec) {
-    const int64_t n = (int64_t)pt.batch * HKV * D;
-    int qb = (int)((n + 255) / 256);
-    if (qb > c->num_sms * 4) qb = c->num_sms * 4;
-    qvec_kernel<T, KIND><<<qb, 256, 0, s>>>(static_cast<const T*>(q), pt.batch, g.num_q_heads, HKV, D, rr.qvec);
-    c->launches += 1;
-    if (cudaError_t e = cudaGetLastError()) return e;
-  }
-  cudaError_t e = launch_kernel(score_kernel<T, D, PG, HKV, kScStages, AGG, KIND>, dim3(ctas), dim3(kScThreads), smem, s, use_qvec,
+  score_kernel<T, D, PG, HKV, kScStages, AGG, KIND><<<ctas, kScThreads, smem, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, pt.batch, pt.page_indptr,
       pt.page_indices, pt.total_pages, scores, rr.begin, rr.begin + (rr.count < 0 ? pt.batch : rr.count), 0,
-      rr.count < 0 ? pt.total_pages : -1, rr.waves > 1 ? rr.waves : 1, rr.ready_cnt, use_qvec ? rr.qvec : nullptr);
+      rr.count < 0 ? pt.total_pages : -1);
   c->launches += 1;
-  return e != cudaSuccess ? e : cudaGetLastError();
+  return cudaGetLastError();
 }
 
 template <typename T, int D, int PG, int HKV, int KIND>

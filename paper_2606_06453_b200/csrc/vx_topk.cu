@@ -56,15 +56,10 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
 
   const int kvh = blockIdx.x, i = blockIdx.y + req0;
   const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
-  [[maybe_unused]] const int cta = i * gridDim.x + blockIdx.x;
-  if (tid == 0) { VX_TRACE_STAMP(cta, 0); VX_TRACE_SMID(cta); }
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
   const int k = max(0, min(budget[i], max_budget));   // a negative budget selects nothing (never indexes below the row)
   const int row0 = page_indptr[i];
-  const int unit = i * num_kv_heads + kvh;
-  if (pf.ready_cnt != nullptr) pdl_trigger();   // overlapped step: the kernels behind me wait for what they need themselves
-  wait_unit_scores(pf.ready_cnt, unit, page_indptr[i + 1] - row0);   // (plain step: the whole score grid, griddepcontrol.wait)
-  if (tid == 0) VX_TRACE_STAMP(cta, 2);
+  pdl_wait();                                   // the scores (and, in a step, nothing else) come from the predecessor
   const int64_t out0 = ((int64_t)i * num_kv_heads + kvh) * max_budget;
   const int n_sel = min(k, n_pages);
   if (tid == 0) sel_count[i * num_kv_heads + kvh] = n_sel;
@@ -75,7 +70,6 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
       sel_phys[out0 + r] = ok ? page_indices[row0 + r] : -1;
       if (sel_logical) sel_logical[out0 + r] = ok ? r : -1;
     }
-    publish_unit_selection(pf.sel_flag, unit, pf.epoch);
     return;
   }
 
@@ -116,8 +110,6 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
       sel_phys[out0 + r] = -1;
       if (sel_logical) sel_logical[out0 + r] = -1;
     }
-    publish_unit_selection(pf.sel_flag, unit, pf.epoch);
-    if (tid == 0) VX_TRACE_STAMP(cta, 9);
     return;
   }
   // ---- requests beyond the shared-memory key cache, or budgets beyond the staging area: the general form -------
@@ -337,7 +329,6 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
     sel_phys[out0 + r] = -1;
     if (sel_logical) sel_logical[out0 + r] = -1;
   }
-  publish_unit_selection(pf.sel_flag, unit, pf.epoch);
 }
 
 template <int THREADS>
@@ -386,16 +377,14 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
 
   const int kvh = blockIdx.x, i = blockIdx.y + req0;
   const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
-  [[maybe_unused]] const int cta = i * gridDim.x + blockIdx.x;
+  [[maybe_unused]] const int cta = blockIdx.y * gridDim.x + blockIdx.x;
   if (tid == 0) { VX_TRACE_STAMP(cta, 0); VX_TRACE_SMID(cta); }
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
   const int k = max(0, min(budget[i], max_budget));   // a negative budget selects nothing (never indexes below the row)
   const int row0 = page_indptr[i];
   for (int b = tid; b < kBins; b += THREADS) s_hist[b] = 0;      // first pass's histogram, zeroed under the loads
   if (tid == 0) VX_TRACE_STAMP(cta, 1);
-  const int unit = i * num_kv_heads + kvh;
-  if (pf.ready_cnt != nullptr) pdl_trigger();   // overlapped step: the kernels behind me wait for what they need themselves
-  wait_unit_scores(pf.ready_cnt, unit, page_indptr[i + 1] - row0);   // (plain step: the whole score grid, griddepcontrol.wait)
+  pdl_wait();                                   // the scores (and, in a step, nothing else) come from the predecessor
   if (tid == 0) VX_TRACE_STAMP(cta, 2);
   const int64_t out0 = ((int64_t)i * num_kv_heads + kvh) * max_budget;
   const int n_sel = min(k, n_pages);
@@ -407,7 +396,6 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
       sel_phys[out0 + r] = ok ? page_indices[row0 + r] : -1;
       if (sel_logical) sel_logical[out0 + r] = ok ? r : -1;
     }
-    publish_unit_selection(pf.sel_flag, unit, pf.epoch);
     return;
   }
 
@@ -657,7 +645,6 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
     sel_phys[out0 + r] = -1;
     if (sel_logical) sel_logical[out0 + r] = -1;
   }
-  publish_unit_selection(pf.sel_flag, unit, pf.epoch);
   if (tid == 0) VX_TRACE_STAMP(cta, 9);
 }
 
@@ -671,8 +658,6 @@ static cudaError_t launch_topk_reg(vx_ctx* c, const float* scores, const vx_page
   const vx_geom& g = c->g;
   dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
   auto kernel = ap.tolerate_ratio > 0.f ? topk_reg_kernel<THREADS, kKpt, true> : topk_reg_kernel<THREADS, kKpt, false>;
-  if (pf.sel_flag != nullptr)                    // (overlapped step: the carve-out preference, see ensure_dyn_smem)
-    if (cudaError_t e0 = ensure_dyn_smem(reinterpret_cast<const void*>(kernel), c->device, 0)) return e0;
   cudaError_t e = launch_kernel(kernel, grid, dim3(THREADS), 0, s, pdl, scores, g.num_kv_heads,
                                 pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
                                 g.n_sink, g.n_local, max_budget, sel_phys, sel_logical, sel_count, rr.begin, pf, ap);
@@ -691,11 +676,7 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
   if (ap.tolerate_ratio > 0.f && !approx_topk_supported(pt.max_pages_per_req, max_budget)) return cudaErrorNotSupported;
   // block size by problem size
   const int n = pt.max_pages_per_req;
-  if (pf.slim) {                                 // overlapped step, early requests: 256 threads x 48 registers fit beside the
-    if (n <= 1024) return launch_topk_reg<256, 4>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap);
-    return launch_topk_t<512>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);   // score kernel's CTAs (512 x 40 registers)
-  }
-  if (ap.tolerate_ratio <= 0.f && pf.sel_flag == nullptr && topk_pair_applies(c, c->g.num_kv_heads * (rr.count < 0 ? pt.batch : rr.count), n))
+  if (ap.tolerate_ratio <= 0.f && topk_pair_applies(c, c->g.num_kv_heads * (rr.count < 0 ? pt.batch : rr.count), n))
     return launch_topk_pair(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
   if (n <= kTopkRegMaxPages) {                   // keys fit the registers of one CTA
 #define VX_REG(T, K) return launch_topk_reg<T, K>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap)
