@@ -244,10 +244,9 @@ class Runner:
         return out
 
 
-def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None, summary="envelope", agg="sum", passes=3):
-    """Time the oracle (as it stands) on the first n_requests requests of the workload: one untimed warm-up pass, then
-    the MEDIAN of `passes` timed passes.  Returns (seconds for score + top-k + attention on the sample, requests in sample,
-    batch, threads)."""
+def oracle_prepare(cfg, n_requests, seed_offset=0, device="cpu", workload=None, summary="envelope", agg="sum"):
+    """The oracle (as it stands) on the first n_requests requests of the workload: gathers their pages to the host ONCE and
+    returns (run, requests in sample, batch, threads), run() = one timed pass (score + top-k + attention) in seconds."""
     from oracle import vx_oracle as vo
     from paper_2606_06453_b200.workloads import make_workload, subproblem
     from oracle.workload_io import to_oracle
@@ -258,19 +257,40 @@ def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=No
     s = sub.spec
     build = vo.page_centroid if summary == "centroid" else vo.page_summary
     summ = build(pool, pt, s.num_kv_heads, s.qk_dim)                    # built outside the timed step
-    times = []
-    for it in range(1 + passes):
+    page = pt.page_size                                                 # (the block size when blocks are finer than the page)
+
+    def run():
         t0 = time.perf_counter()
         vo.decode_step(q, pool, pt, vo.as_np(sub.budget), sub.max_budget, s.num_q_heads, s.num_kv_heads, s.qk_dim,
                        s.v_dim, s.sm_scale, s.n_sink, s.n_local, agg=vo.AGG_MAX if agg == "max" else vo.AGG_SUM, summary=summ,
                        kind=summary)
-        if it > 0:
-            times.append(time.perf_counter() - t0)
-    return statistics.median(times), n_requests, w.spec.batch, vo.num_threads()
+        return time.perf_counter() - t0
+
+    return run, n_requests, w.spec.batch, vo.num_threads()
+
+
+def oracle_sample_time(cfg, n_requests, seed_offset=0, device="cpu", workload=None, summary="envelope", agg="sum", passes=3):
+    """one untimed warm-up pass, then the MEDIAN of `passes` timed passes -> (seconds, requests in sample, batch, threads)"""
+    run, n, batch, threads = oracle_prepare(cfg, n_requests, seed_offset, device, workload, summary, agg)
+    run()
+    return statistics.median([run() for _ in range(passes)]), n, batch, threads
 
 
 SAMPLE_REQUESTS = {"C1": 1, "C2": 32, "C3": 8, "C4": 64, "C5": 16}  # cpu_baseline: requests per oracle pass (C1-C4: the whole batch)
 PARITY_REQUESTS = {"C1": [0], "C2": [5, 27], "C3": [6], "C4": [7, 50], "C5": [33, 90]}   # post-timing sampled parity check
+
+
+def config_dict(cfg, w, args, world, is_main=True):
+    """what both arms print under "config": the workload the metric is quoted on"""
+    s = w.spec
+    return {"workload": cfg, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
+            "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
+            "seq_len": list(s.seq_len), "budget_pages": w.max_budget, "summary": args.summary if is_main else "envelope",
+            "agg": args.agg if is_main else "sum",
+            "topk": "exact" if args.topk_approx <= 0 else f"approx tolerate_ratio={args.topk_approx} (lossy)",
+            "mla_step": args.mla_step if s.kv_shared else "n/a",
+            "kv_dtype": getattr(s, "kv_dtype", "") or s.dtype,
+            "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"}
 
 
 def run_reference(args):
@@ -278,21 +298,29 @@ def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    from paper_2606_06453_b200.workloads import make_workload
+    from paper_2606_06453_b200.workloads import make_workload, with_fp8
     nreq = SAMPLE_REQUESTS.get(args.config, 1)
-    w = make_workload(args.config, device=_gen_device())     # inputs only; the oracle runs on the host cores
-    times = []
-    steps = max(1, min(args.steps, 3))
-    for it in range(steps):
-        t, n, batch, threads = oracle_sample_time(args.config, nreq, workload=w, summary=args.summary, agg=args.agg, passes=1)
-        times.append(t)
+    spec = args.config if args.kv_dtype == "same" or args.config == "C1" else with_fp8(args.config, args.kv_dtype)
+    w = make_workload(spec, device=_gen_device())     # inputs only; the oracle runs on the host cores
+    run, n, batch, threads = oracle_prepare(args.config, nreq, workload=w, summary=args.summary, agg=args.agg)
+    t_first = run()                                   # (untimed: also sizes the run)
+    budget_s = 150.0                                  # the whole --steps K --warmup W run ends within a few minutes
+    per = max(t_first, 1e-3)
+    warmup = max(0, min(args.warmup, int(0.2 * budget_s / per)))
+    steps = max(1, min(args.steps, int(0.8 * budget_s / per)))
+    for _ in range(max(0, warmup - 1)):
+        run()
+    times = [run() for _ in range(steps)]
     us = statistics.mean(times) / n * batch * 1e6        # scaled from the sample to the whole batch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
     line = {"impl": "reference", "metric": METRIC, "value": us, "unit": "us", "n_gpus": args.gpus, "steps": steps,
-            "warmup": 1, "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
+            "warmup": max(warmup, 1), "ms_per_step": us / 1e3, "higher_is_better": False, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": args.config, "summary": args.summary, "l2": "n/a (CPU)"},
+            "config": config_dict(args.config, w, args, world),
             "cpu_baseline": {"value": us, "unit": "us", "cores": threads, "kind": "oracle",
-                             "sample": f"{n} of {batch} requests per step (one untimed warm-up pass before each), scaled by {batch}/{n}"},
+                             "sample": f"first {n} of {batch} requests per step (score + top-k + attention)"
+                                       + ("" if n == batch else f", scaled by {batch}/{n}") + "; host run, config.l2 does not apply"
+                                       + ("" if steps == args.steps else f"; {steps} of the {args.steps} steps asked for fit the time budget")},
             "e2e": {"value": us, "unit": "us", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -385,14 +413,7 @@ def measure(cfg, args, device, local, rank, world, steps, warmup, peak, peak_src
             torch.cuda.synchronize()
             parity = parity_sample(w, PARITY_REQUESTS.get(cfg, [0]), r.sel_logical, r.sel_count, r.out, r.lse)
         rec = {"value": ms * 1e3, "unit": "us", "steps": steps, "warmup": warmup, "ms_per_step": ms, "dtype": s.dtype,
-               "config": {"workload": cfg, "batch_per_gpu": s.batch, "num_q_heads": s.num_q_heads,
-                          "num_kv_heads": s.num_kv_heads, "qk_dim": s.qk_dim, "page_size": s.page_size,
-                          "seq_len": list(s.seq_len), "budget_pages": w.max_budget, "summary": summary_kind,
-                          "agg": args.agg if is_main else "sum",
-                          "topk": "exact" if args.topk_approx <= 0 else f"approx tolerate_ratio={args.topk_approx} (lossy)",
-                          "mla_step": args.mla_step if s.kv_shared else "n/a",
-                          "kv_dtype": getattr(s, "kv_dtype", "") or s.dtype,
-                          "l2": "flushed before every step (512 MiB write sweep + 256 MiB read sweep)", "parallelism": f"dp{world}"},
+               "config": config_dict(cfg, w, args, world, is_main),
                "hbm_gbs": step_gbs, "roofline_frac": step_gbs / peak, "roofline_frac_nominal_8TBs": step_gbs / NOMINAL_HBM_GBS,
                "step_bytes": bytes_, "stage_us": stage, "roofline": roofline, "cpu_baseline": cpu, "parity": parity,
                "e2e": {"value": e2e_ms * 1e3, "unit": "us", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
