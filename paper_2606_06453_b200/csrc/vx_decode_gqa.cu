@@ -54,7 +54,7 @@ __device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, 
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(valid ? 16 : 0));
 }
 
-template <int D>
+template <int D, bool CL>
 __global__ void __launch_bounds__(kGqaWarps * kWarp)
 decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* __restrict__ kpool,
                       const __nv_bfloat16* __restrict__ vpool, int64_t stride_page, int64_t stride_token,
@@ -285,6 +285,8 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   for (int w = 0; w < kGqaWarps; ++w) { mb_a = fmaxf(mb_a, s_m[w][ha]); mb_b = fmaxf(mb_b, s_m[w][ha + 1]); }
   const float f_a = m_a == -INFINITY ? 0.f : exp2f(m_a - mb_a), f_b = m_b == -INFINITY ? 0.f : exp2f(m_b - mb_b);
   float* so = reinterpret_cast<float*>(ring);   // [D][8 heads] fp32 = D * 32 bytes <= one stage
+  // cluster merge: this CTA's normalised partial [8 heads][D] + 8 lse, in warp 0's second stage (nobody's `so`)
+  [[maybe_unused]] float* cl_part = reinterpret_cast<float*>(smem + 2 * PAGEB);
 #pragma unroll
   for (int mt = 0; mt < KS; ++mt) {
     const int d0 = mt * 16 + lane / 4;
@@ -309,13 +311,51 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     if (num_splits == 1) {
       out[head_row * D + d] = __float2bfloat16_rn(val);
       if (d == 0 && lse_out != nullptr) lse_out[head_row] = lse;
+    } else if constexpr (CL) {                  // this split's partial stays in shared memory for the cluster merge
+      cl_part[h * D + d] = val;
+      if (d == 0) cl_part[8 * D + h] = lse;
     } else {
       part_o[(head_row * num_splits + split) * D + d] = val;
       if (d == 0) part_lse[head_row * num_splits + split] = lse;
     }
   }
   if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 8);
-  if (num_splits > 1) {                         // (a5) the last split of this (request, KV head) merges by LSE
+  if constexpr (CL) {
+    // (a5) the splits of this (request, KV head) are the CTAs of one thread-block cluster: every CTA merges a slice of
+    // the group's output rows out of its peers' shared memory; no partials in HBM, no counter, no fence
+    cluster_sync();
+    if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 9);
+    constexpr int VEC = D / 4;
+    const uint32_t part_u32 = smem_u32(cl_part);
+    for (int e = split * (int)blockDim.x + threadIdx.x; e < grp * VEC; e += num_splits * blockDim.x) {
+      const int h = e / VEC, c = (e % VEC) * 4;
+      float w[8];
+      float mx = -INFINITY;
+#pragma unroll
+      for (int sp = 0; sp < 8; ++sp) {
+        w[sp] = sp < num_splits ? dsmem_ld_f32(dsmem_addr(part_u32 + (8 * D + h) * 4, sp)) : -INFINITY;
+        mx = fmaxf(mx, w[sp]);
+      }
+      float z = 0.f;
+#pragma unroll
+      for (int sp = 0; sp < 8; ++sp) { w[sp] = mx == -INFINITY ? 0.f : __expf(w[sp] - mx); z += w[sp]; }
+      const float inv = z > 0.f ? 1.f / z : 0.f;
+      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+      for (int sp = 0; sp < 8; ++sp) {
+        if (sp < num_splits) {
+          const float4 v = dsmem_ld_f32x4(dsmem_addr(part_u32 + (h * D + c) * 4, sp));
+          const float ww = w[sp] * inv;
+          acc.x = fmaf(ww, v.x, acc.x); acc.y = fmaf(ww, v.y, acc.y); acc.z = fmaf(ww, v.z, acc.z); acc.w = fmaf(ww, v.w, acc.w);
+        }
+      }
+      const int64_t head_row = (int64_t)i * num_q_heads + kvh * grp + h;
+      store4(out + head_row * D + c, acc);
+      if (c == 0 && lse_out != nullptr) lse_out[head_row] = z > 0.f ? mx + logf(z) : -INFINITY;
+    }
+    if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 10);
+    cluster_sync();                               // no CTA leaves while a peer still reads its partial
+  } else if (num_splits > 1) {                  // (a5) the last split of this (request, KV head) merges by LSE
     if (last_split_arrives(unit_counter + i * num_kv_heads + kvh, num_splits, &s_last)) {
       if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 9);
       merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads + kvh * grp, grp, num_splits, D, out, lse_out,
@@ -340,12 +380,16 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
                                     int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt) {
   const vx_geom& g = c->g;
   constexpr int smem = kGqaWarps * kGqaStages * 2 * kGqaPage * D * 2;
-  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_gqa_mma_kernel<D>), c->device, smem)) return e;
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_gqa_mma_kernel<D, false>), c->device, smem)) return e;
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_gqa_mma_kernel<D, true>), c->device, smem)) return e;
   // splits: whole waves of equal CTAs.  cost(sp) = waves x (pages per warp + ~3 pages of pipeline fill)
   const int n_req = opt.rr.count < 0 ? pt.batch : opt.rr.count;
   const int splits = decode_gqa_splits(c, n_req, max_budget);
   dim3 grid(splits, g.num_kv_heads, n_req);
-  cudaError_t e = launch_kernel(decode_gqa_mma_kernel<D>, grid, dim3(kGqaWarps * kWarp), (size_t)smem, s, opt.pdl,
+  // 2, 4 or 8 splits: one thread-block cluster per (request, KV head), merged over distributed shared memory
+  const bool cl = splits == 2 || splits == 4 || splits == 8;
+  cudaError_t e = launch_kernel_cluster(cl ? decode_gqa_mma_kernel<D, true> : decode_gqa_mma_kernel<D, false>, grid,
+      dim3(kGqaWarps * kWarp), (size_t)smem, s, opt.pdl, cl ? splits : 1,
       static_cast<const __nv_bfloat16*>(q), static_cast<const __nv_bfloat16*>(pool.k),
       static_cast<const __nv_bfloat16*>(pool.v), pool.stride_page, pool.stride_token, pool.stride_head,
       g.num_q_heads, g.num_kv_heads, g.sm_scale * kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget,
