@@ -222,6 +222,44 @@ __device__ __forceinline__ float4 dsmem_ld_f32x4(uint32_t addr) {
   return v;
 }
 
+// ---- (a5) LSE merge inside a thread-block cluster: the n_part splits of a unit are the CTAs of one
+// cluster; each left its normalised partial [8 rows][v_dim] fp32 followed by 8 lse values at the same shared-memory
+// offset `part` (rows >= n_rows unused).  CTA `rank` merges every n_part-th slice of blockDim.x 4-element vectors.
+// Call between two cluster_sync(): after every CTA's partial is written, before any CTA may exit.  n_part <= 8.
+__device__ __forceinline__ void store4(float* dst, float4 v);
+__device__ __forceinline__ void store4(__nv_bfloat16* dst, float4 v);
+template <typename T>
+__device__ __forceinline__ void cluster_merge_partials(const float* part, int v_dim, int n_rows, int rank, int n_part,
+                                                       int64_t row0, T* out, float* lse) {
+  const int vec = v_dim / 4;
+  const uint32_t part_u32 = (uint32_t)__cvta_generic_to_shared(part);
+  for (int e = rank * (int)blockDim.x + threadIdx.x; e < n_rows * vec; e += n_part * blockDim.x) {
+    const int h = e / vec, c = (e % vec) * 4;
+    float w[8];
+    float mx = -INFINITY;
+#pragma unroll
+    for (int sp = 0; sp < 8; ++sp) {
+      w[sp] = sp < n_part ? dsmem_ld_f32(dsmem_addr(part_u32 + (8 * v_dim + h) * 4, sp)) : -INFINITY;
+      mx = fmaxf(mx, w[sp]);
+    }
+    float z = 0.f;
+#pragma unroll
+    for (int sp = 0; sp < 8; ++sp) { w[sp] = mx == -INFINITY ? 0.f : __expf(w[sp] - mx); z += w[sp]; }
+    const float inv = z > 0.f ? 1.f / z : 0.f;
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int sp = 0; sp < 8; ++sp) {
+      if (sp < n_part) {
+        const float4 v = dsmem_ld_f32x4(dsmem_addr(part_u32 + (h * v_dim + c) * 4, sp));
+        const float ww = w[sp] * inv;
+        acc.x = fmaf(ww, v.x, acc.x); acc.y = fmaf(ww, v.y, acc.y); acc.z = fmaf(ww, v.z, acc.z); acc.w = fmaf(ww, v.w, acc.w);
+      }
+    }
+    store4(out + (row0 + h) * v_dim + c, acc);
+    if (c == 0 && lse != nullptr) lse[row0 + h] = z > 0.f ? mx + logf(z) : -INFINITY;
+  }
+}
+
 // ---- (a5) in-kernel LSE merge: the LAST split CTA of a unit to finish merges the unit's
 // partials.  Call with the whole CTA after its own partial (o, lse) is written.  Returns true in the CTA
 // that must merge.  counter is zero on entry to the step and is left zero.

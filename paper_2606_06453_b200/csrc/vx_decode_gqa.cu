@@ -325,34 +325,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     // the group's output rows out of its peers' shared memory; no partials in HBM, no counter, no fence
     cluster_sync();
     if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 9);
-    constexpr int VEC = D / 4;
-    const uint32_t part_u32 = smem_u32(cl_part);
-    for (int e = split * (int)blockDim.x + threadIdx.x; e < grp * VEC; e += num_splits * blockDim.x) {
-      const int h = e / VEC, c = (e % VEC) * 4;
-      float w[8];
-      float mx = -INFINITY;
-#pragma unroll
-      for (int sp = 0; sp < 8; ++sp) {
-        w[sp] = sp < num_splits ? dsmem_ld_f32(dsmem_addr(part_u32 + (8 * D + h) * 4, sp)) : -INFINITY;
-        mx = fmaxf(mx, w[sp]);
-      }
-      float z = 0.f;
-#pragma unroll
-      for (int sp = 0; sp < 8; ++sp) { w[sp] = mx == -INFINITY ? 0.f : __expf(w[sp] - mx); z += w[sp]; }
-      const float inv = z > 0.f ? 1.f / z : 0.f;
-      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
-#pragma unroll
-      for (int sp = 0; sp < 8; ++sp) {
-        if (sp < num_splits) {
-          const float4 v = dsmem_ld_f32x4(dsmem_addr(part_u32 + (h * D + c) * 4, sp));
-          const float ww = w[sp] * inv;
-          acc.x = fmaf(ww, v.x, acc.x); acc.y = fmaf(ww, v.y, acc.y); acc.z = fmaf(ww, v.z, acc.z); acc.w = fmaf(ww, v.w, acc.w);
-        }
-      }
-      const int64_t head_row = (int64_t)i * num_q_heads + kvh * grp + h;
-      store4(out + head_row * D + c, acc);
-      if (c == 0 && lse_out != nullptr) lse_out[head_row] = z > 0.f ? mx + logf(z) : -INFINITY;
-    }
+    cluster_merge_partials(cl_part, D, grp, split, num_splits, (int64_t)i * num_q_heads + kvh * grp, out, lse_out);
     if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 10);
     cluster_sync();                               // no CTA leaves while a peer still reads its partial
   } else if (num_splits > 1) {                  // (a5) the last split of this (request, KV head) merges by LSE

@@ -66,7 +66,7 @@ __device__ __forceinline__ void cp16_zfill(uint32_t dst, const void* src, bool v
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(valid ? 16 : 0));
 }
 
-template <typename TKV>
+template <typename TKV, bool CL>
 __global__ void __launch_bounds__(gq8::WARPS * kWarp)
 decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __restrict__ kpool, const uint8_t* __restrict__ vpool,
                       int64_t stride_page, int64_t stride_token, int64_t stride_head, int num_q_heads, int num_kv_heads,
@@ -282,6 +282,8 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
   for (int w = 0; w < WARPS; ++w) { mb_a = fmaxf(mb_a, s_m[w][ha]); mb_b = fmaxf(mb_b, s_m[w][ha + 1]); }
   const float f_a = m_a == -INFINITY ? 0.f : exp2f(m_a - mb_a), f_b = m_b == -INFINITY ? 0.f : exp2f(m_b - mb_b);
   float* so = reinterpret_cast<float*>(ring);   // [D][8 heads] fp32 = 4 KB = one stage
+  // cluster merge: this CTA's normalised partial [8 heads][D] + 8 lse, behind warp 0's `so` (nobody else's)
+  [[maybe_unused]] float* cl_part = reinterpret_cast<float*>(smem + 2 * PAGEB);
 #pragma unroll
   for (int mt = 0; mt < KS; ++mt) {             // row slot g <-> channel 16 mt + 2 g, row slot g + 8 <-> channel 16 mt + 2 g + 1
     const int d0 = mt * 16 + 2 * (lane / 4);
@@ -306,12 +308,19 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
     if (num_splits == 1) {
       out[head_row * D + d] = __float2bfloat16_rn(val);
       if (d == 0 && lse_out != nullptr) lse_out[head_row] = lse;
+    } else if constexpr (CL) {
+      cl_part[h * D + d] = val;
+      if (d == 0) cl_part[8 * D + h] = lse;
     } else {
       part_o[(head_row * num_splits + split) * D + d] = val;
       if (d == 0) part_lse[head_row * num_splits + split] = lse;
     }
   }
-  if (num_splits > 1) {                         // (a5) the last split of this (request, KV head) merges by LSE
+  if constexpr (CL) {                           // (a5) the splits are one cluster: merge over distributed shared memory
+    cluster_sync();
+    cluster_merge_partials(cl_part, D, grp, split, num_splits, (int64_t)i * num_q_heads + kvh * grp, out, lse_out);
+    cluster_sync();
+  } else if (num_splits > 1) {                  // (a5) the last split of this (request, KV head) merges by LSE
     if (last_split_arrives(unit_counter + i * num_kv_heads + kvh, num_splits, &s_last))
       merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads + kvh * grp, grp, num_splits, D, out, lse_out,
                                      reinterpret_cast<float*>(smem));
@@ -345,10 +354,13 @@ static cudaError_t launch_gqa_fp8_t(vx_ctx* c, const void* q, const vx_kv_pool& 
                                     int32_t max_budget, void* out, float* lse, cudaStream_t s, bool pdl, const int32_t* budget,
                                     void* summary_upd) {
   const vx_geom& g = c->g;
-  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_gqa_fp8_kernel<TKV>), c->device, gq8::SMEM)) return e;
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_gqa_fp8_kernel<TKV, false>), c->device, gq8::SMEM)) return e;
+  if (cudaError_t e = ensure_dyn_smem(reinterpret_cast<const void*>(decode_gqa_fp8_kernel<TKV, true>), c->device, gq8::SMEM)) return e;
   const int splits = decode_gqa_fp8_splits(c, pt.batch, max_budget);
   dim3 grid(splits, g.num_kv_heads, pt.batch);
-  cudaError_t e = launch_kernel(decode_gqa_fp8_kernel<TKV>, grid, dim3(gq8::WARPS * kWarp), (size_t)gq8::SMEM, s, pdl,
+  const bool cl = splits == 2 || splits == 4 || splits == 8;
+  cudaError_t e = launch_kernel_cluster(cl ? decode_gqa_fp8_kernel<TKV, true> : decode_gqa_fp8_kernel<TKV, false>, grid,
+      dim3(gq8::WARPS * kWarp), (size_t)gq8::SMEM, s, pdl, cl ? splits : 1,
       static_cast<const __nv_bfloat16*>(q), static_cast<const uint8_t*>(pool.k), static_cast<const uint8_t*>(pool.v),
       pool.stride_page, pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads,
       g.sm_scale * pool.k_scale * gq8::kLog2e, pool.v_scale, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits,
