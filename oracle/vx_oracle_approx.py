@@ -31,7 +31,18 @@ follows them step by step, in this order, with plain numpy (uint32 / float32 sca
   Emission: forced pages, every candidate above the final threshold bin, the chosen members; ascending
   logical order; physical ids through the page table; count = min(k, P).
 
-tolerate_ratio = 0 never terminates early and is the exact selection.  At most floor(tolerate_ratio * k)
+REMAP (App. D.2 "we apply a monotonic transformation x' = f(x) that preserves ordering while reshaping the
+value distribution ... selected offline through profiling and fused into the histogram pass"; reading G29): an
+optional table of n knot values 0 <= u_0 <= ... <= u_{n-1} <= 1 (2 <= n <= 65) is f on the normalised score, piecewise
+linear between the knots at t = 0, 1/(n-1), ..., 1.  With a table installed the FIRST pass always bins through it (whatever
+the key range), every operation rounded to fp32 in this order:
+     x = (score - smin) * ((n-1) / (smax - smin));   i = min(n-2, int(x));   fr = x - i;
+     u = min(u_{i+1}, fr * (u_{i+1} - u_i) + u_i);   bin = min(2047, int(u * 2048))
+(the min with u_{i+1} keeps the bin non-decreasing in the score across a knot whatever the rounding, which is all the
+selection needs: the members of a bin are then a contiguous key interval, and steps 3-7 are unchanged).  The table is an
+INPUT here; how it is profiled is the product's business (paper_2606_06453_b200/remap_profile.py).
+
+tolerate_ratio = 0 never terminates early and is the exact selection (with or without a remap).  At most floor(tolerate_ratio * k)
 selected pages differ from the exact set, so recall@k >= 1 - tolerate_ratio.
 
 Pins (tests/test_oracle_approx_topk.py): tolerate_ratio 0 == the exact oracle (vx_oracle.c, a full sort) and
@@ -76,9 +87,33 @@ def _bitlen(x: int) -> int:
     return int(x).bit_length()
 
 
+def remap_bins(sc32: np.ndarray, smin, smax, knots: np.ndarray) -> np.ndarray:
+    """The first-pass bin of each fp32 score under the knot table (reading G29), fp32 operation by operation."""
+    u_k = np.ascontiguousarray(knots, dtype=np.float32)
+    n = int(u_k.shape[0])
+    with np.errstate(divide="ignore", invalid="ignore", over="ignore"):
+        tscale = np.float32(n - 1) / np.float32(smax - smin)
+        x = ((sc32 - np.float32(smin)).astype(np.float32) * tscale).astype(np.float32)
+    i = np.minimum(n - 2, x.astype(np.int64))
+    fr = (x - i.astype(np.float32)).astype(np.float32)
+    d = (u_k[i + 1] - u_k[i]).astype(np.float32)
+    u = np.minimum(u_k[i + 1], ((fr * d).astype(np.float32) + u_k[i]).astype(np.float32))
+    return np.minimum(K_BINS - 1, (u * np.float32(K_BINS)).astype(np.float32).astype(np.int64))
+
+
+def check_knots(knots) -> np.ndarray:
+    u_k = np.ascontiguousarray(knots, dtype=np.float32)
+    assert u_k.ndim == 1 and 2 <= u_k.shape[0] <= 65, "2..65 knots"
+    assert np.all(np.isfinite(u_k)) and u_k.min() >= 0.0 and u_k.max() <= 1.0 and np.all(np.diff(u_k) >= 0), \
+        "knots: finite, in [0, 1], non-decreasing"
+    return u_k
+
+
 def select_one(scores_f32: np.ndarray, k: int, n_sink: int, n_local: int, tolerate_ratio: float,
-               seed: int, problem: int):
-    """One (request, KV head): scores of its P logical pages -> (sorted selected logical ids, info)."""
+               seed: int, problem: int, remap=None):
+    """One (request, KV head): scores of its P logical pages -> (sorted selected logical ids, info).
+    remap: None, or the knot table of reading G29."""
+    knots = None if remap is None else check_knots(remap)
     P = int(scores_f32.shape[0])
     info = {"passes": 0, "early": False, "sure": np.zeros(0, np.int64), "members": np.zeros(0, np.int64),
             "need": 0, "bin_width": 0.0}
@@ -102,12 +137,14 @@ def select_one(scores_f32: np.ndarray, k: int, n_sink: int, n_local: int, tolera
     smax = key_floats(np.array([kmax], np.uint32))[0]
     with np.errstate(divide="ignore", invalid="ignore", over="ignore"):
         fscale = np.float32(K_BINS) / np.float32(smax - smin)
-    fpass = (kmax - kmin) >= (1 << 25) and bool(np.isfinite(fscale)) and bool(fscale > 0)
+    fpass = ((kmax - kmin) >= (1 << 25) or knots is not None) and bool(np.isfinite(fscale)) and bool(fscale > 0)
     taken_above = np.zeros(cand.shape[0], dtype=bool)
     while True:
         info["passes"] += 1
         live = (key >= lo) & (key - np.uint64(lo) < np.uint64(width))
-        if fpass:
+        if fpass and knots is not None:
+            b = remap_bins(sc32, smin, smax, knots)
+        elif fpass:
             b = np.minimum(K_BINS - 1, ((sc32 - smin).astype(np.float32) * fscale).astype(np.float32).astype(np.int64))
         else:
             b = ((key - np.uint64(lo)) >> np.uint64(shift)).astype(np.int64)
@@ -121,7 +158,10 @@ def select_one(scores_f32: np.ndarray, k: int, n_sink: int, n_local: int, tolera
         cnt = int(hist[t])
         m_idx = np.nonzero(members)[0]                            # ascending logical order (cand is ascending)
         info.update(need=need, members=cand[m_idx].astype(np.int64))
-        if fpass:
+        if fpass and knots is not None:
+            ms = sc32[m_idx]
+            info["bin_width"] = float(ms.max()) - float(ms.min())    # (the spread of the bin's members: f has no closed inverse)
+        elif fpass:
             info["bin_width"] = float(smax - smin) / K_BINS
         else:
             blo = lo + (t << shift)
@@ -157,7 +197,7 @@ def select_one(scores_f32: np.ndarray, k: int, n_sink: int, n_local: int, tolera
 
 
 def approx_topk_pages(scores: np.ndarray, page_indptr, page_indices, seq_lens, page_size: int, budget,
-                      n_sink: int, n_local: int, max_budget: int, tolerate_ratio: float, seed: int):
+                      n_sink: int, n_local: int, max_budget: int, tolerate_ratio: float, seed: int, remap=None):
     """scores fp32 [Hkv, T] ragged by page_indptr -> (sel_logical, sel_phys [B,Hkv,max_budget] pad -1,
     sel_count [B,Hkv], early [B,Hkv] bool)."""
     scores = np.ascontiguousarray(scores, dtype=np.float32)
@@ -174,7 +214,7 @@ def approx_topk_pages(scores: np.ndarray, page_indptr, page_indices, seq_lens, p
         k = min(int(budget[i]), max_budget)
         for h in range(hkv):
             row = scores[h, indptr[i]:indptr[i] + P]
-            sel, info = select_one(row, k, n_sink, n_local, tolerate_ratio, seed, i * hkv + h)
+            sel, info = select_one(row, k, n_sink, n_local, tolerate_ratio, seed, i * hkv + h, remap)
             n = sel.shape[0]
             assert n == min(k, P)
             sl[i, h, :n] = sel

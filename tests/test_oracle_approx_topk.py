@@ -162,3 +162,99 @@ def test_sampler_inclusion_frequency_is_need_over_cnt():
     freq = hits[members] / n
     assert abs(freq.mean() - need / len(members)) < 1e-9                    # exactly need picks per draw
     assert freq.max() < 3 * need / len(members) and freq.min() > 0          # no member favoured or starved
+
+
+# ---- the offline-profiled monotone remap (App. D.2; reading G29) ---------------------------------
+
+def _knot_tables(rng):
+    """identity, two extreme shapes, a flat table (every page in bin 0) and random monotone tables"""
+    yield np.array([0.0, 1.0], dtype=np.float32)
+    yield np.linspace(0, 1, 65, dtype=np.float32) ** 3
+    yield np.sqrt(np.linspace(0, 1, 17, dtype=np.float32))
+    yield np.zeros(9, dtype=np.float32)
+    yield np.array([0.0, 0.0, 1.0, 1.0, 1.0], dtype=np.float32)
+    for n in (2, 3, 33, 65):
+        u = np.sort(rng.random(n)).astype(np.float32)
+        yield u
+
+
+def test_remap_bins_never_decrease_with_the_score():
+    """the one property the selection needs of f (reading G29): the first-pass bin is non-decreasing in the score,
+    across knots and whatever the fp32 rounding -- checked on every fp32 value of a dense score range"""
+    rng = np.random.default_rng(7)
+    lo = np.float32(0.37)
+    dense = np.arange(np.float32(lo).view(np.uint32), np.float32(lo).view(np.uint32) + 300000, dtype=np.uint32).view(np.float32)
+    wide = np.sort(np.concatenate([-np.geomspace(1e-6, 50, 4000), np.geomspace(1e-7, 900, 6000)]).astype(np.float32))
+    for knots in _knot_tables(rng):
+        for sc in (dense, wide):
+            b = va.remap_bins(sc, sc[0], sc[-1], knots)
+            assert (np.diff(b) >= 0).all() and b.min() >= 0 and b.max() <= va.K_BINS - 1
+
+
+@pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
+def test_ratio_zero_with_any_remap_is_the_exact_selection(dist):
+    """a monotone f only reshapes the first pass's bins: with tolerate_ratio 0 the selection is still the exact one"""
+    rng = np.random.default_rng(21)
+    hkv, P_list, k = 2, [700, 2048, 300], 64
+    scores = appd_scores(dist, (hkv, sum(P_list)), seed=13).numpy()
+    budget = np.full(len(P_list), k, dtype=np.int32)
+    indptr, pt, sl_e, sc_e = exact_sets(scores, P_list, budget, 1, 2, k)
+    for knots in _knot_tables(rng):
+        sl, sp, sc, early = va.approx_topk_pages(scores, indptr, pt.page_indices, pt.seq_lens, 16, budget, 1, 2, k, 0.0, 5,
+                                                 remap=knots)
+        assert not early.any() and np.array_equal(sc, sc_e) and np.array_equal(sl, sl_e)
+
+
+def test_ratio_zero_with_remap_on_ties_and_sign_spanning_ranges():
+    rng = np.random.default_rng(5)
+    tables = list(_knot_tables(rng))
+    for trial in range(24):
+        P = int(rng.integers(20, 900))
+        k = int(rng.integers(4, min(P, 200)))
+        kind = trial % 3
+        if kind == 0:
+            s = rng.integers(0, 4, size=P).astype(np.float32)                       # heavy ties
+        elif kind == 1:
+            s = (rng.standard_normal(P) * 10 ** rng.uniform(-20, 20, size=P)).astype(np.float32)   # 40 decades, both signs
+        else:
+            s = rng.standard_normal(P).astype(np.float32)
+        budget = np.array([k], dtype=np.int32)
+        indptr, pt, sl_e, sc_e = exact_sets(s[None, :], [P], budget, 1, 1, k)
+        sl, _, sc, early = va.approx_topk_pages(s[None, :], indptr, pt.page_indices, pt.seq_lens, 16, budget, 1, 1, k, 0.0, 9,
+                                                remap=tables[trial % len(tables)])
+        assert not early.any() and np.array_equal(sc, sc_e) and np.array_equal(sl, sl_e), (trial, kind)
+
+
+@pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
+@pytest.mark.parametrize("ratio", [0.1, 0.5])
+def test_remap_keeps_the_recall_bound_and_the_sure_picks(dist, ratio):
+    from paper_2606_06453_b200.remap_profile import profile_knots
+    hkv, P_list, k = 1, [4096, 1500], 128
+    scores = appd_scores(dist, (hkv, sum(P_list)), seed=17).numpy()
+    knots = profile_knots(appd_scores(dist, (8, 4096), seed=99).numpy(), 33)       # profiled on OTHER draws of the distribution
+    budget = np.full(len(P_list), k, dtype=np.int32)
+    indptr, pt, sl_e, sc_e = exact_sets(scores, P_list, budget, 1, 2, k)
+    for seed in range(4):
+        sl, sp, sc, early = va.approx_topk_pages(scores, indptr, pt.page_indices, pt.seq_lens, 16, budget, 1, 2, k, ratio, seed,
+                                                 remap=knots)
+        assert np.array_equal(sc, sc_e)
+        for i, P in enumerate(P_list):
+            got, exact = sl[i, 0, :sc[i, 0]], sl_e[i, 0, :sc_e[i, 0]]
+            assert (np.diff(got) > 0).all() and got[0] == 0 and set(range(P - 2, P)) <= set(got.tolist())
+            assert va.recall_at_k(got, exact) >= 1.0 - ratio - 1e-9
+            row = scores[0, indptr[i]:indptr[i] + P]
+            _, info = va.select_one(row, k, 1, 2, ratio, seed, i, knots)
+            assert set(info["sure"].tolist()) <= set(exact.tolist())
+
+
+def test_profiled_remap_spreads_the_first_pass():
+    """what the offline profile is for ("improves bin separation"): under the table fitted to a distribution the
+    fullest first-pass bin holds far fewer pages than under the linear map; the table is a valid knot table"""
+    from paper_2606_06453_b200.remap_profile import profile_knots
+    for dist in ("lognormal", "bimodal"):
+        knots = va.check_knots(profile_knots(appd_scores(dist, (16, 8192), seed=3).numpy(), 65))
+        assert knots[0] == 0.0 and knots[-1] == 1.0
+        s = np.sort(appd_scores(dist, (1, 8192), seed=4).numpy()[0])
+        lin = np.minimum(va.K_BINS - 1, ((s - s[0]) * (np.float32(va.K_BINS) / (s[-1] - s[0]))).astype(np.int64))
+        rem = va.remap_bins(s, s[0], s[-1], knots)
+        assert np.bincount(rem).max() * 3 <= np.bincount(lin).max()
