@@ -218,6 +218,19 @@ vx_status vx_topk_pages_approx(vx_ctx *ctx, const float *scores, const vx_page_t
 /* tolerate_ratio and seed used by vx_sparse_decode_step when its flags carry VX_STEP_APPROX_TOPK
  * (context state, host side; default 0 = exact).  VX_ERR_INVALID_ARG outside [0, 1]. */
 vx_status vx_set_topk_approx(vx_ctx *ctx, float tolerate_ratio, uint64_t seed);
+/* The remap of PAPER.md:495 (App. D.2: "a monotonic transformation x' = f(x) that preserves ordering while reshaping the
+ * value distribution ... selected offline through profiling and fused into the histogram pass"; reading G29).
+ * knots: HOST array of n_knots floats (2 <= n_knots <= 65), each in [0, 1], never decreasing: f on the score normalised
+ * by the request's own min / max, piecewise linear between the knots at 0, 1/(n-1), ..., 1 (copied into the workspace
+ * before the call returns; the caller keeps its array).  n_knots = 0 (knots ignored) removes the table.
+ * With a table installed, vx_topk_pages_approx and a fused step with VX_STEP_APPROX_TOPK bin the FIRST radix pass through
+ * f instead of the linear map; a monotone f changes how many pages share the threshold bin, never which pages an exact
+ * selection returns: at tolerate_ratio 0 those calls still return exactly vx_topk_pages' selection (through the
+ * approximate kernels' code, so vx_topk_pages_approx's size limits apply).  vx_topk_pages itself never uses the table.
+ * paper_2606_06453_b200/remap_profile.py fits a table to sample scores (their empirical distribution function).
+ * Synchronous set-up call (one cudaMemcpy); do not call it while a selection of this context is in flight.
+ * VX_ERR_INVALID_ARG for a bad count, a NULL table, a value outside [0, 1] or a decreasing pair. */
+vx_status vx_set_topk_remap(vx_ctx *ctx, const float *knots /* host */, int32_t n_knots);
 
 /* ---- NEXT-4: head-union block table, PAPER.md:538 (Table 1 "TopK, Union: block-table selection and its
  * deduplicated union (trtllm backend)"), :200 (a paged decode backend that takes one table per request) ------

@@ -28,7 +28,7 @@ VX_MLA_STEP_AUTO, VX_MLA_STEP_FUSED, VX_MLA_STEP_CHAINED, VX_MLA_STEP_FLAT = 0, 
 EXPORTS = ["vx_workspace_bytes", "vx_create", "vx_destroy", "vx_last_error", "vx_last_launch_count",
            "vx_page_summary_update", "vx_page_score", "vx_topk_pages", "vx_sparse_paged_decode",
            "vx_sparse_decode_step", "vx_sparse_decode_step_host", "vx_trace_attach",
-           "vx_topk_pages_approx", "vx_set_topk_approx", "vx_union_pages", "vx_set_option",
+           "vx_topk_pages_approx", "vx_set_topk_approx", "vx_set_topk_remap", "vx_union_pages", "vx_set_option",
            "vx_sparse_paged_decode_static", "vx_static_scratch_bytes", "vx_static_last_error"]
 
 
@@ -84,6 +84,7 @@ def load_library():
         "vx_topk_pages": (I32, [P, P, T, P, I32, P, P, P, P]),
         "vx_topk_pages_approx": (I32, [P, P, T, P, I32, C.c_float, C.c_uint64, P, P, P, P]),
         "vx_set_topk_approx": (I32, [P, C.c_float, C.c_uint64]),
+        "vx_set_topk_remap": (I32, [P, P, I32]),
         "vx_set_option": (I32, [P, I32, I32]),
         "vx_sparse_paged_decode_static": (I32, [G, P, K, T, P, P, P, I32, P, P, P]),
         "vx_static_scratch_bytes": (C.c_size_t, []),
@@ -213,6 +214,14 @@ class Context:
 
     def set_topk_approx(self, tolerate_ratio, seed):
         self._check(self.lib.vx_set_topk_approx(self._h, float(tolerate_ratio), int(seed)))
+
+    def set_topk_remap(self, knots):
+        """knots: sequence of 2..65 floats in [0, 1], non-decreasing (remap_profile.profile_knots), or None to clear"""
+        if knots is None or len(knots) == 0:
+            self._check(self.lib.vx_set_topk_remap(self._h, None, 0))
+            return
+        arr = (C.c_float * len(knots))(*[float(v) for v in knots])
+        self._check(self.lib.vx_set_topk_remap(self._h, C.cast(arr, C.c_void_p), len(knots)))
 
     def sparse_paged_decode(self, q, pool: KvPool, pt: PageTable, sel_phys, sel_logical, sel_count,
                             max_budget, out, lse=None, stream=None):

@@ -50,6 +50,7 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   w.flat_sync = static_cast<int32_t*>(take(mla ? step_mla_flat_workspace_ints(max_batch) * 4 : 0));
   w.blk_indptr = static_cast<int32_t*>(take(bpp > 1 ? (B + 1) * 4 : 0));
   w.blk_indices = static_cast<int32_t*>(take(bpp > 1 ? (size_t)max_total_pages * bpp * 4 : 0));
+  w.topk_remap = static_cast<float*>(take(kTopkRemapMaxKnots * 4));
   w.fp8_qvec = static_cast<float*>(take(kv_is_fp8(g) ? B * Hkv * 2 * (size_t)g.qk_dim * 4 : 0));
   w.bytes = off;
   return w;
@@ -335,12 +336,12 @@ vx_status vx_topk_pages_approx(vx_ctx* c, const float* scores, const vx_page_tab
   if (max_budget <= 0) return fail(c, VX_ERR_INVALID_ARG, "max_budget must be positive");
   if (!(tolerate_ratio >= 0.f && tolerate_ratio <= 1.f))
     return fail(c, VX_ERR_INVALID_ARG, "tolerate_ratio %g outside [0, 1]", (double)tolerate_ratio);
-  if (tolerate_ratio > 0.f && !approx_topk_supported(pt->max_pages_per_req, max_budget))
-    return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (budgets above %d: %d pages); got %d",
-                kTopkApproxMaxPages, kTopkApproxMaxBudgetLong, kTopkRegMaxPages, pt->max_pages_per_req);
-  ApproxPlan ap;
+  ApproxPlan ap = c->approx;                     // (the remap table, if one is installed)
   ap.tolerate_ratio = tolerate_ratio;
   ap.seed = seed;
+  if (ap.active() && !approx_topk_supported(pt->max_pages_per_req, max_budget))
+    return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (budgets above %d: %d pages); got %d",
+                kTopkApproxMaxPages, kTopkApproxMaxBudgetLong, kTopkRegMaxPages, pt->max_pages_per_req);
   return check_cuda(c, launch_topk_pages(c, scores, *pt, budget, max_budget, sel_phys, sel_logical, sel_count,
                                          (cudaStream_t)stream, false, ReqRange(), PrefetchPlan(), ap),
                     "vx_topk_pages_approx");
@@ -352,6 +353,27 @@ vx_status vx_set_topk_approx(vx_ctx* c, float tolerate_ratio, uint64_t seed) {
     return fail(c, VX_ERR_INVALID_ARG, "tolerate_ratio %g outside [0, 1]", (double)tolerate_ratio);
   c->approx.tolerate_ratio = tolerate_ratio;
   c->approx.seed = seed;
+  return VX_OK;
+}
+
+vx_status vx_set_topk_remap(vx_ctx* c, const float* knots, int32_t n_knots) {
+  if (!c) return VX_ERR_INVALID_ARG;
+  if (n_knots == 0) {                            // back to the per-request linear map
+    c->approx.remap = nullptr;
+    c->approx.remap_n = 0;
+    return VX_OK;
+  }
+  if (!knots || n_knots < 2 || n_knots > kTopkRemapMaxKnots)
+    return fail(c, VX_ERR_INVALID_ARG, "remap: 2..%d knots (0 clears the table); got %d", kTopkRemapMaxKnots, n_knots);
+  for (int i = 0; i < n_knots; ++i)
+    if (!(knots[i] >= 0.f && knots[i] <= 1.f) || (i > 0 && knots[i] < knots[i - 1]))
+      return fail(c, VX_ERR_INVALID_ARG, "remap: knot %d = %g; knots must lie in [0, 1] and never decrease", i, (double)knots[i]);
+  if (vx_status st = check_device(c)) return st;
+  // (synchronous set-up call: the table is in place when it returns; a selection already in flight may read either table)
+  if (vx_status st = check_cuda(c, cudaMemcpy(c->ws.topk_remap, knots, (size_t)n_knots * 4, cudaMemcpyHostToDevice), "remap table"))
+    return st;
+  c->approx.remap = c->ws.topk_remap;
+  c->approx.remap_n = n_knots;
   return VX_OK;
 }
 
@@ -440,7 +462,7 @@ vx_status vx_sparse_decode_step(vx_ctx* c, const void* q, const vx_kv_pool* pool
   ApproxPlan ap;                                 // exact unless the caller asks for the lossy selection
   if (flags & VX_STEP_APPROX_TOPK) {
     ap = c->approx;
-    if (ap.tolerate_ratio > 0.f && !approx_topk_supported(pt->max_pages_per_req, max_budget))
+    if (ap.active() && !approx_topk_supported(pt->max_pages_per_req, max_budget))
       return fail(c, VX_ERR_UNSUPPORTED, "approximate top-k handles at most %d pages per request (budgets above %d: %d pages); got %d",
                   kTopkApproxMaxPages, kTopkApproxMaxBudgetLong, kTopkRegMaxPages, pt->max_pages_per_req);
   }

@@ -31,6 +31,7 @@ struct Workspace {               // device pointers carved from the caller's wor
   int32_t* flat_sync;            // counters and per-request flags; zero between steps
   int32_t* blk_indptr;           // blocks finer than the page: the page table expanded into a block table, [max_batch + 1]
   int32_t* blk_indices;          // [max_total_pages * bpp] physical block ids
+  float* topk_remap;             // [kTopkRemapMaxKnots] the knot table of vx_set_topk_remap
   float* fp8_qvec;               // fp8 KV cache: [max_batch, Hkv, 2 qk_dim] query vectors [Qm | Qp] of the score kernel (vx_score_fp8.cu)
   size_t bytes;                  // total
 };
@@ -41,9 +42,16 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
 
 // Approximate radix top-k (PAPER.md:196 stochastic early termination, :538 `approxTopK`):
 // tolerate_ratio <= 0 is the exact selection.
+// remap (App. D.2, reading G29): an offline-profiled monotone knot table through which the first radix pass
+// bins the normalised scores; remap_n == 0: none.  A plan with a remap runs the approximate kernels' code (which carry the
+// remapped pass) even at tolerate_ratio 0, where their result is the exact selection.
+constexpr int kTopkRemapMaxKnots = 65;
 struct ApproxPlan {
   float tolerate_ratio = 0.f;
   uint64_t seed = 0;
+  const float* remap = nullptr;                  // device, remap_n floats in [0, 1], non-decreasing
+  int remap_n = 0;
+  __host__ __device__ bool active() const { return tolerate_ratio > 0.f || remap_n > 0; }
 };
 constexpr int kTopkRegMaxPages = 8 * 1024;       // register-resident selection kernel: pages per request
 constexpr int kTopkApproxMaxPages = 48 * 1024;   // the lossy selection beyond that: the shared-memory-key kernel's key cache

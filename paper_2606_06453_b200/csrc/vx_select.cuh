@@ -31,6 +31,7 @@ struct SelectScratch {                          // ~10 KB of shared memory
   int2 wcnt[32];
   int bin, above, cnt, nlist, need_eq;
   uint32_t thr, bmin, bmax;
+  float knot[65];                               // kApprox: the remap's knot table (vx_internal.h kTopkRemapMaxKnots)
 };
 
 // keys[0 .. n_pages): on entry the BIT PATTERNS of the fp32 scores of logical pages 0 .. n_pages-1, on return their
@@ -51,7 +52,8 @@ __device__ __forceinline__ void select_sync() {
 // constants and order of tests as topk_reg_kernel<.., true>, so both kernels and oracle/vx_oracle_approx.py agree bit for bit.
 template <int THREADS, int BAR = 0, int TID0 = 0, bool kApprox = false>
 __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, int k, int n_sink, int n_local,
-                                float tolerate_ratio = 0.f, uint64_t seed = 0, int problem = 0) {
+                                float tolerate_ratio = 0.f, uint64_t seed = 0, int problem = 0,
+                                const float* remap = nullptr, int remap_n = 0) {
   constexpr int WARPS = THREADS / kWarp;
   constexpr int BPT = kBins / THREADS;          // bins per thread in the suffix scan
   static_assert(kBins % THREADS == 0 && WARPS <= 32, "shape");
@@ -63,6 +65,9 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
     return n_sel;
   }
 
+  const int rn = kApprox ? remap_n : 0;         // knots of the offline-profiled remap (reading G29); 0: none
+  if constexpr (kApprox)
+    for (int t = tid; t < rn; t += THREADS) sc.knot[t] = remap[t];      // (visible after the barrier below)
   // ---- keys, and the min / max key of the non-forced pages ------------------------------------
   uint32_t kmin = 0xFFFFFFFFu, kmax = 0u;
   for (int j = tid; j < n_pages; j += THREADS) {
@@ -90,7 +95,18 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
   [[maybe_unused]] int t_bin = 0, rot = 0, wrap = 0;
   const float smin = key_to_float(kmin), smax = key_to_float(kmax);
   const float fscale = (float)kBins / (smax - smin);
-  auto fbin = [&](uint32_t key) -> int { return min(kBins - 1, (int)((key_to_float(key) - smin) * fscale)); };
+  const float tscale = (float)(rn - 1) / (smax - smin);
+  auto fbin = [&](uint32_t key) -> int {        // (the same arithmetic, operation by operation, as topk_reg_kernel's)
+    const float d0 = key_to_float(key) - smin;
+    if (kApprox && rn > 0) {
+      const float x = __fmul_rn(d0, tscale);
+      const int i0 = max(0, min(rn - 2, (int)x));      // (>= 0 for every candidate; the emission also asks for absent pages)
+      const float k0 = sc.knot[i0], k1 = sc.knot[i0 + 1];
+      const float u = fminf(k1, __fadd_rn(__fmul_rn(__fsub_rn(x, (float)i0), __fsub_rn(k1, k0)), k0));
+      return min(kBins - 1, (int)__fmul_rn(u, (float)kBins));
+    }
+    return min(kBins - 1, (int)(d0 * fscale));
+  };
 
   if (need > 0) {
     // ---- radix select over the live key range [lo, lo + width) ----------------------------------
@@ -102,7 +118,7 @@ __device__ int cta_select_pages(SelectScratch& sc, uint32_t* keys, int n_pages, 
     // unlike the integer key it is linear across the sign change and across exponents.  The members of one float bin
     // are a contiguous key interval, so deeper passes continue on integer keys.  Only when the key range spans the
     // sign change or several exponents (>= 2^25 key steps): a narrow range is linear enough in the integer key.
-    bool fpass = kmax - kmin >= (1u << 25) && isfinite(fscale) && fscale > 0.f;
+    bool fpass = (kmax - kmin >= (1u << 25) || rn > 0) && isfinite(fscale) && fscale > 0.f;
 #pragma unroll 1
     while (true) {
       for (int b = tid; b < kBins; b += THREADS) sc.hist[b] = 0;

@@ -88,8 +88,9 @@ topk_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pages,
         if (j0 + u * THREADS < n_pages) s_keys[j0 + u * THREADS] = __float_as_uint(v[u]);
     }
     __syncthreads();
-    if (ap.tolerate_ratio > 0.f)                // (requests beyond the register kernel's 8,192 pages)
-      cta_select_pages<THREADS, 0, 0, true>(scratch, s_keys, n_pages, k, n_sink, n_local, ap.tolerate_ratio, ap.seed, i * num_kv_heads + kvh);
+    if (ap.active())                            // (requests beyond the register kernel's 8,192 pages)
+      cta_select_pages<THREADS, 0, 0, true>(scratch, s_keys, n_pages, k, n_sink, n_local, ap.tolerate_ratio, ap.seed, i * num_kv_heads + kvh,
+                                            ap.remap, ap.remap_n);
     else
       cta_select_pages<THREADS>(scratch, s_keys, n_pages, k, n_sink, n_local);
     pdl_trigger();
@@ -374,10 +375,14 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   __shared__ int2 s_wcnt[WARPS];
   __shared__ int s_bin, s_above, s_cnt, s_nlist, s_need_eq;
   __shared__ uint32_t s_thr, s_bmin, s_bmax;
+  __shared__ float s_knot[kApprox ? kTopkRemapMaxKnots : 1];      // the remap's knot table (reading G29)
 
   const int kvh = blockIdx.x, i = blockIdx.y + req0;
   const int tid = threadIdx.x, lane = tid % kWarp, warp = tid / kWarp;
   [[maybe_unused]] const int cta = blockIdx.y * gridDim.x + blockIdx.x;
+  const int rn = kApprox ? ap.remap_n : 0;
+  if constexpr (kApprox)
+    for (int t = tid; t < rn; t += THREADS) s_knot[t] = ap.remap[t];   // (an input of the call: read before the wait)
   if (tid == 0) { VX_TRACE_STAMP(cta, 0); VX_TRACE_SMID(cta); }
   const int n_pages = (seq_lens[i] + page_size - 1) / page_size;
   const int k = max(0, min(budget[i], max_budget));   // a negative budget selects nothing (never indexes below the row)
@@ -438,13 +443,27 @@ topk_reg_kernel(const float* __restrict__ scores, int num_kv_heads, int total_pa
   int t_bin = 0, rot = 0, wrap = 0;
   const float smin = key_to_float(kmin), smax = key_to_float(kmax);
   const float fscale = (float)kBins / (smax - smin);
-  auto fbin = [&](uint32_t kk) -> int { return min(kBins - 1, (int)((key_to_float(kk) - smin) * fscale)); };
+  const float tscale = (float)(rn - 1) / (smax - smin);
+  // first-pass bin of a key: linear in the score, or (remap installed) through the knot table -- x = the score's place
+  // among the knots, u = f there, every product and sum rounded on its own as the oracle does (no fused multiply-add);
+  // the min with the upper knot keeps the bin from ever decreasing with the score (reading G29)
+  auto fbin = [&](uint32_t kk) -> int {
+    const float d0 = key_to_float(kk) - smin;
+    if (kApprox && rn > 0) {
+      const float x = __fmul_rn(d0, tscale);
+      const int i0 = max(0, min(rn - 2, (int)x));      // (>= 0 for every candidate; the emission also asks for absent pages)
+      const float k0 = s_knot[i0], k1 = s_knot[i0 + 1];
+      const float u = fminf(k1, __fadd_rn(__fmul_rn(__fsub_rn(x, (float)i0), __fsub_rn(k1, k0)), k0));
+      return min(kBins - 1, (int)__fmul_rn(u, (float)kBins));
+    }
+    return min(kBins - 1, (int)(d0 * fscale));
+  };
 
   if (need > 0) {
     uint32_t lo = kmin;
     uint64_t width = (uint64_t)(kmax - kmin) + 1;
     int shift = max(0, (32 - __clz(kmax - kmin)) - kBinBits);     // ((kmax - kmin) >> shift) < kBins
-    bool fpass = kmax - kmin >= (1u << 25) && isfinite(fscale) && fscale > 0.f;   // float-domain first pass (see topk_kernel)
+    bool fpass = (kmax - kmin >= (1u << 25) || rn > 0) && isfinite(fscale) && fscale > 0.f;   // float-domain first pass (see topk_kernel)
     [[maybe_unused]] const int tol = kApprox ? (int)(ap.tolerate_ratio * (float)k) : 0;   // floor: both factors >= 0
     bool first = true;
 #pragma unroll 1
@@ -657,7 +676,7 @@ static cudaError_t launch_topk_reg(vx_ctx* c, const float* scores, const vx_page
                                    const ApproxPlan& ap) {
   const vx_geom& g = c->g;
   dim3 grid(g.num_kv_heads, rr.count < 0 ? pt.batch : rr.count);
-  auto kernel = ap.tolerate_ratio > 0.f ? topk_reg_kernel<THREADS, kKpt, true> : topk_reg_kernel<THREADS, kKpt, false>;
+  auto kernel = ap.active() ? topk_reg_kernel<THREADS, kKpt, true> : topk_reg_kernel<THREADS, kKpt, false>;
   cudaError_t e = launch_kernel(kernel, grid, dim3(THREADS), 0, s, pdl, scores, g.num_kv_heads,
                                 pt.total_pages, pt.page_indptr, pt.page_indices, pt.seq_lens, g.page_size, budget,
                                 g.n_sink, g.n_local, max_budget, sel_phys, sel_logical, sel_count, rr.begin, pf, ap);
@@ -673,10 +692,10 @@ cudaError_t launch_topk_pages(vx_ctx* c, const float* scores, const vx_page_tabl
   // the lossy selection runs in the register kernel (<= 8,192 pages) and in the shared-memory-key kernel (<= 49,152 pages,
   // budgets of at most 2,048 pages)
   static_assert(kTopkApproxMaxPages == kTopkSmemKeys && kTopkApproxMaxBudgetLong == kBins, "vx_internal.h states the kernel's limits");
-  if (ap.tolerate_ratio > 0.f && !approx_topk_supported(pt.max_pages_per_req, max_budget)) return cudaErrorNotSupported;
+  if (ap.active() && !approx_topk_supported(pt.max_pages_per_req, max_budget)) return cudaErrorNotSupported;
   // block size by problem size
   const int n = pt.max_pages_per_req;
-  if (ap.tolerate_ratio <= 0.f && topk_pair_applies(c, c->g.num_kv_heads * (rr.count < 0 ? pt.batch : rr.count), n))
+  if (!ap.active() && topk_pair_applies(c, c->g.num_kv_heads * (rr.count < 0 ? pt.batch : rr.count), n))
     return launch_topk_pair(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf);
   if (n <= kTopkRegMaxPages) {                   // keys fit the registers of one CTA
 #define VX_REG(T, K) return launch_topk_reg<T, K>(c, scores, pt, budget, max_budget, sel_phys, sel_logical, sel_count, s, pdl, rr, pf, ap)

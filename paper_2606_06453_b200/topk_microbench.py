@@ -7,9 +7,12 @@ the LIVE key range of each problem, so the four distributions should cost the sa
 
 With --ratios the approximate selection (vx_topk_pages_approx, PAPER.md:196 stochastic early termination) is timed
 beside it at each tolerate_ratio, with its mean / min recall@k against the exact set (PAPER.md:497 reports latency at
-recall@k > 0.97).
+recall@k > 0.97).  With --remap the two remapped variants of App. D.2 (:485 "radix topk with remap", "approx_radix_topk +
+remap") are timed as well: a knot table fitted offline (remap_profile.profile_knots) to OTHER draws of the same
+distribution is installed with vx_set_topk_remap, then tolerate_ratio 0 (the exact selection through the remapped first
+pass, checked against the exact set) and each ratio are timed again.
 
-    python -m paper_2606_06453_b200.topk_microbench [--batch 32] [--heads 8] [--iters 50] [--ratios 0.05,0.1,0.25]
+    python -m paper_2606_06453_b200.topk_microbench [--batch 32] [--heads 8] [--iters 50] [--ratios 0.05,0.1,0.25] [--remap]
 """
 from __future__ import annotations
 
@@ -33,6 +36,8 @@ def main():
     ap.add_argument("--heads", type=int, default=8)
     ap.add_argument("--iters", type=int, default=50)
     ap.add_argument("--ratios", default="0.05,0.1,0.25", help="tolerate_ratio values for vx_topk_pages_approx ('' = none)")
+    ap.add_argument("--remap", action="store_true", help="also time the selection with an offline-profiled remap table installed")
+    ap.add_argument("--knots", type=int, default=33)
     args = ap.parse_args()
     dev = "cuda:0"
     gen = torch.Generator(device=dev).manual_seed(77)
@@ -75,10 +80,14 @@ def main():
                 us = a.elapsed_time(b) * 1e3 / args.iters
                 assert torch.equal(sl.long(), want), (P, k, dist, "after graph replay")
                 row = dict(pages=P, k=k, dist=dist, problems=B * H, us=round(us, 2))
-                for tau in [float(x) for x in args.ratios.split(",") if x] if P <= 8192 else []:
+                taus = [float(x) for x in args.ratios.split(",") if x] if P <= 8192 else []
+
+                def time_approx(tau, name):
                     ctx.topk_pages_approx(scores, pt, budget, k, tau, 7, sp, sl, sc)
                     torch.cuda.synchronize()
                     hit = (sl.long().unsqueeze(-1) == want.unsqueeze(-2)).any(-1).float().sum(-1) / k   # [B, H] recall@k
+                    if tau == 0.0:
+                        assert torch.equal(sl.long(), want), (P, k, dist, name)       # ratio 0 stays exact under any table
                     g2 = torch.cuda.CUDAGraph()
                     with torch.cuda.graph(g2):
                         for _ in range(args.iters):
@@ -87,8 +96,17 @@ def main():
                     torch.cuda.synchronize()
                     a.record(); g2.replay(); b.record()
                     torch.cuda.synchronize()
-                    row[f"approx_{tau}"] = dict(us=round(a.elapsed_time(b) * 1e3 / args.iters, 2),
-                                                recall_mean=round(hit.mean().item(), 4), recall_min=round(hit.min().item(), 4))
+                    row[name] = dict(us=round(a.elapsed_time(b) * 1e3 / args.iters, 2),
+                                     recall_mean=round(hit.mean().item(), 4), recall_min=round(hit.min().item(), 4))
+
+                for tau in taus:
+                    time_approx(tau, f"approx_{tau}")
+                if args.remap and P <= 8192:
+                    from .remap_profile import profile_knots
+                    ctx.set_topk_remap(profile_knots(draw(dist, (8, P), 990000 + P + k, "cpu").numpy(), args.knots))
+                    for tau in [0.0] + taus:
+                        time_approx(tau, f"remap_{tau}")
+                    ctx.set_topk_remap(None)
                 rows.append(row)
                 print(json.dumps(rows[-1]))
             ctx.close()

@@ -52,19 +52,22 @@ def check_against_exact(scores, pages, seq, indices, budget, n_sink, n_local, ta
     return worst
 
 
-def run_both(scores, pages, seq, indices, budget, n_sink, n_local, tau, seed, b=16):
+def run_both(scores, pages, seq, indices, budget, n_sink, n_local, tau, seed, b=16, remap=None):
     import paper_2606_06453_b200 as vx
     hkv = scores.shape[0]
     indptr = np.concatenate([[0], np.cumsum(pages)]).astype(np.int32)
     T = int(indptr[-1])
     mb = int(budget.max())
-    ref = va.approx_topk_pages(scores, indptr, indices, np.array(seq, np.int32), b, budget, n_sink, n_local, mb, tau, seed)
+    ref = va.approx_topk_pages(scores, indptr, indices, np.array(seq, np.int32), b, budget, n_sink, n_local, mb, tau, seed,
+                               remap=remap)
     dev = "cuda:0"
     ctx = vx.Context(dtype=torch.bfloat16, num_q_heads=4 * hkv, num_kv_heads=hkv, qk_dim=128, v_dim=128, page_size=b,
                      sm_scale=1.0, n_sink=n_sink, n_local=n_local, max_batch=len(pages), max_total_pages=T,
                      max_pages_per_req=max(pages), max_budget=mb, device=dev)
     pt = vx.PageTable(torch.from_numpy(indptr).to(dev), torch.from_numpy(indices).to(dev),
                       torch.tensor(seq, dtype=torch.int32, device=dev), T, max(pages))
+    if remap is not None:
+        ctx.set_topk_remap(remap)
     sl = torch.full((len(pages), hkv, mb), -7, dtype=torch.int32, device=dev)
     sp = torch.full_like(sl, -7)
     sc = torch.full((len(pages), hkv), -7, dtype=torch.int32, device=dev)
@@ -236,4 +239,79 @@ def test_fused_step_with_approximate_selection(name):
     assert np.array_equal(sl.cpu().numpy(), sl_r) and np.array_equal(sp.cpu().numpy(), sp_r)
     o_ref, l_ref = oracle_attention_on(w, sl.cpu().numpy(), sc.cpu().numpy())
     check_attention(s.dtype, out.float().cpu().numpy(), lse.cpu().numpy(), o_ref, l_ref)
+    ctx.close()
+
+
+# ---- the offline-profiled remap of the first pass (App. D.2; reading G29; vx_set_topk_remap) --------
+
+def _random_knots(rng, n):
+    return np.sort(rng.random(n)).astype(np.float32)
+
+
+@pytest.mark.parametrize("dist", APPD_DISTRIBUTIONS)
+@pytest.mark.parametrize("tau", [0.0, 0.1, 0.5])
+def test_remap_profiled_on_the_distribution(dist, tau):
+    """the table fitted offline to OTHER draws of the distribution; ratio 0 must stay the exact selection (run_both's gate)"""
+    from paper_2606_06453_b200.remap_profile import profile_knots
+    rng = np.random.default_rng(15)
+    pages = [2048, 777, 8192, 40, 4100]
+    T = sum(pages)
+    seq = [p * 16 - int(rng.integers(0, 16)) for p in pages]
+    indices = rng.permutation(T + 9)[:T].astype(np.int32)
+    budget = np.array([128, 64, 256, 64, 200], np.int32)
+    scores = appd_scores(dist, (2, T), seed=131).numpy()
+    knots = profile_knots(appd_scores(dist, (8, 4096), seed=977).numpy(), 33)
+    (sl_r, sp_r, sc_r, early), (sl, sp, sc) = run_both(scores, pages, seq, indices, budget, 1, 2, tau, 4, remap=knots)
+    assert np.array_equal(sc, sc_r) and np.array_equal(sl, sl_r) and np.array_equal(sp, sp_r), (dist, tau)
+    if tau == 0.0:
+        assert not early.any()
+
+
+@pytest.mark.parametrize("kind", KINDS)
+def test_remap_random_tables_on_the_fuzz_kinds_stay_exact(kind):
+    """any monotone table, nasty score sets (ties, signed zeros, denormals, 40 decades), short and long requests:
+    at ratio 0 the selection is the exact one (held against the C oracle inside run_both) and equals the mirror oracle"""
+    rng = np.random.default_rng(277 + KINDS.index(kind))
+    n_sink, n_local = int(rng.integers(0, 3)), int(rng.integers(0, 4))
+    pages = [int(x) for x in rng.choice([3, 40, 300, 1025, 2048, 5000, 8192, 9000, 16384], size=4)]
+    seq = [p * 16 - int(rng.integers(0, 16)) for p in pages]
+    T = sum(pages)
+    indices = rng.permutation(T + 17)[:T].astype(np.int32)
+    budget = np.array([max(n_sink + n_local, int(rng.integers(1, max(2, min(p + 3, 600))))) for p in pages], np.int32)
+    scores = np.stack([draw_scores(rng, kind, T) for _ in range(2)])
+    knots = [np.zeros(5, np.float32), np.array([0, 1], np.float32), _random_knots(rng, 65), _random_knots(rng, 3)][KINDS.index(kind) % 4]
+    for tau in (0.0, 0.25):
+        (sl_r, sp_r, sc_r, _), (sl, sp, sc) = run_both(scores, pages, seq, indices, budget, n_sink, n_local, tau, 9, remap=knots)
+        assert np.array_equal(sc, sc_r) and np.array_equal(sl, sl_r) and np.array_equal(sp, sp_r), (kind, tau)
+
+
+def test_remap_in_the_fused_step_and_argument_checks():
+    """VX_STEP_APPROX_TOPK with a table and ratio 0: the step's selections and outputs are those of the exact step"""
+    import paper_2606_06453_b200 as vx
+    from paper_2606_06453_b200 import binding
+    from paper_2606_06453_b200.remap_profile import profile_knots
+    from paper_2606_06453_b200.workloads import make_workload
+    w = make_workload("C2-small", device="cuda:0")
+    s = w.spec
+    ctx = vx.context_for(w)
+    pool, pt = vx.tables_for(w)
+    summary = vx.alloc_summary(w)
+    ctx.page_summary_update(pool, pt, summary, first_new_pos=torch.zeros_like(w.seq_lens))
+    outs = []
+    for flags, knots in ((0, None), (binding.VX_STEP_APPROX_TOPK, profile_knots(np.random.default_rng(1).standard_normal((4, 500)), 17))):
+        if knots is not None:
+            ctx.set_topk_remap(knots)
+            ctx.set_topk_approx(0.0, 3)
+        out = torch.empty(s.batch, s.num_q_heads, s.v_dim, dtype=w.q.dtype, device="cuda:0")
+        sp = torch.full((s.batch, s.num_kv_heads, w.max_budget), -7, dtype=torch.int32, device="cuda:0")
+        sl, sc = torch.full_like(sp, -7), torch.full((s.batch, s.num_kv_heads), -7, dtype=torch.int32, device="cuda:0")
+        ctx.sparse_decode_step(w.q, pool, summary, pt, w.budget, w.max_budget, out, None, sp, sl, sc, flags=flags)
+        torch.cuda.synchronize()
+        outs.append((out, sp, sl, sc))
+    for a, b in zip(outs[0], outs[1]):
+        assert torch.equal(a, b)
+    for bad in ([0.5], [0.2, 0.1], [0.0, 1.5], [float("nan"), 1.0], list(np.linspace(0, 1, 66))):
+        with pytest.raises(vx.VortexError):
+            ctx.set_topk_remap(bad)
+    ctx.set_topk_remap(None)                      # cleared: back to the linear map
     ctx.close()
