@@ -86,3 +86,54 @@ def test_mla_decode_cluster_merge_at_every_cluster_size(batch, splits):
     check_selection(w, sl_h, sp.cpu().numpy(), sc_h, ref)
     o_ref, l_ref = oracle_attention_on(w, sl_h, sc_h)
     check_attention(s.dtype, out.float().cpu().numpy(), lse.cpu().numpy(), o_ref, l_ref)
+
+
+def _gqa_splits(units, budget, sms, fp8):
+    """the GQA decode kernels' split heuristics, restated (vx_decode_gqa.cu: decode_gqa_splits; vx_decode_gqa_fp8.cu)"""
+    slots = sms * (3 if fp8 else 2)
+    fixed = 30 if fp8 else 3
+    cost = lambda sp: -(-units * sp // slots) * (-(-(-(-budget // sp)) // 4) + fixed)
+    return min(range(1, min(32, budget) + 1), key=lambda sp: (cost(sp), sp))
+
+
+@pytest.mark.parametrize("fmt", ["bf16", "e4m3"])
+@pytest.mark.parametrize("batch,budget,splits", [(1, 32, 8), (8, 64, 4), (12, 64, None), (16, 64, 2), (20, 64, None)])
+def test_gqa_decode_cluster_merge_at_every_cluster_size(fmt, batch, budget, splits):
+    """The GQA decode kernels (bf16 and fp8 KV cache) merge 2, 4 or 8 splits of a (request, KV head) inside a thread-block
+    cluster over distributed shared memory, any other count through global partials and an arrival counter:
+    batches chosen so that the heuristics pick cluster sizes 8, 4 and 2 and a non-cluster count, requests with fewer pages
+    than split warps included (empty splits), run twice (no state left behind), the fused step against the oracle."""
+    from dataclasses import replace
+    import paper_2606_06453_b200 as vx
+    from paper_2606_06453_b200.workloads import make_workload, SPECS, with_fp8
+    from oracle.workload_io import oracle_step
+    from tests.parity import check_selection, oracle_attention_on
+    spec = replace(SPECS["C3-small"], name=f"C3-small-b{batch}k{budget}", batch=batch, seq_len=(300, 4000), budget=budget)
+    if fmt != "bf16":
+        spec = with_fp8(spec, fmt)
+    w = make_workload(spec, device="cuda:0")
+    s = w.spec
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    got = _gqa_splits(s.batch * s.num_kv_heads, w.max_budget, sms, fmt != "bf16")
+    if fmt == "bf16" and splits is not None:
+        assert got == splits                      # (the bf16 rows are built to hit each cluster size)
+    ctx = vx.context_for(w)
+    pool, pt = vx.tables_for(w)
+    summary = vx.alloc_summary(w)
+    ctx.page_summary_update(pool, pt, summary, first_new_pos=torch.zeros_like(w.seq_lens))
+    dev = "cuda:0"
+    out = torch.full((s.batch, s.num_q_heads, s.v_dim), float("nan"), dtype=w.q.dtype, device=dev)
+    lse = torch.full((s.batch, s.num_q_heads), float("nan"), dtype=torch.float32, device=dev)
+    sp = torch.empty(s.batch, s.num_kv_heads, w.max_budget, dtype=torch.int32, device=dev)
+    sl = torch.empty_like(sp)
+    sc = torch.empty(s.batch, s.num_kv_heads, dtype=torch.int32, device=dev)
+    for _ in range(2):
+        out.fill_(float("nan"))
+        ctx.sparse_decode_step(w.q, pool, summary, pt, w.budget, w.max_budget, out, lse, sp, sl, sc)
+    torch.cuda.synchronize()
+    ref = oracle_step(w)
+    sl_h, sc_h = sl.cpu().numpy(), sc.cpu().numpy()
+    check_selection(w, sl_h, sp.cpu().numpy(), sc_h, ref)
+    o_ref, l_ref = oracle_attention_on(w, sl_h, sc_h)
+    check_attention(s.dtype, out.float().cpu().numpy(), lse.cpu().numpy(), o_ref, l_ref)
+    print(f"[gqa cluster merge] {fmt} batch {batch} budget {w.max_budget}: {got} splits")
