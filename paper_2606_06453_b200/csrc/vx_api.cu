@@ -51,6 +51,8 @@ Workspace carve_workspace(const vx_geom& g, void* base, int32_t max_batch, int32
   w.blk_indptr = static_cast<int32_t*>(take(bpp > 1 ? (B + 1) * 4 : 0));
   w.blk_indices = static_cast<int32_t*>(take(bpp > 1 ? (size_t)max_total_pages * bpp * 4 : 0));
   w.topk_remap = static_cast<float*>(take(kTopkRemapMaxKnots * 4));
+  w.mla_stage = take(mla_fp8_stage_elems(g, max_batch, max_budget) * 2);
+  w.mla_stage_sel = static_cast<int32_t*>(take(mla_fp8_staged_supported(g) ? B * (size_t)max_budget * 4 : 0));
   w.fp8_qvec = static_cast<float*>(take(kv_is_fp8(g) ? B * Hkv * 2 * (size_t)g.qk_dim * 4 : 0));
   w.bytes = off;
   return w;
@@ -417,6 +419,9 @@ static vx_status decode_dispatch(vx_ctx* c, const void* q, const vx_kv_pool* poo
   if (gqa_fp8_fast_supported(c->g))
     return check_cuda(c, launch_decode_gqa_fp8(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s,
                                                opt.pdl, opt.budget, opt.summary_upd), "vx_sparse_paged_decode (fp8 KV cache)");
+  if (mla_fp8_staged_supported(c->g) && c->bpp == 1 && opt.rr.count < 0 && max_budget <= c->max_budget)
+    return check_cuda(c, launch_decode_mla_fp8_staged(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s, opt),
+                      "vx_sparse_paged_decode (fp8 latent cache)");
   if (kv_is_fp8(c->g))
     return check_cuda(c, launch_decode_fp8(c, q, *pool, *pt, sel_phys, sel_logical, sel_count, max_budget, out, lse, s),
                       "vx_sparse_paged_decode (fp8 KV cache)");

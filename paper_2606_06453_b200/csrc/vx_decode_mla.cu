@@ -45,7 +45,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
                   int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                   int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
                   __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0,
-                  const int32_t* __restrict__ budget_opt, int cluster_merge) {
+                  const int32_t* __restrict__ budget_opt, int cluster_merge, float out_scale) {
   using namespace mla;
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t s_bar[N_BARS];
@@ -315,7 +315,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
       }
       s_l[lane] = l_sum;
       s_m[lane] = m_ref;
-      s_inv[lane] = 1.f / l_sum;
+      s_inv[lane] = out_scale / l_sum;              // (out_scale: 1, or an fp8 pool's v_scale)
     } else {
       // helper warps: follow the softmax warp's decisions; rescale their TMEM lanes of O^T when asked (rare)
       for (int p = 0; p < n_pages; ++p) {
@@ -494,10 +494,10 @@ cudaError_t launch_decode_mla_tc(vx_ctx* c, const void* q, const vx_kv_pool& poo
   // splits of 2, 4 or 8: the splits of a request form a thread-block cluster and merge through shared memory
   const int cluster = (best == 2 || best == 4 || best == 8) ? best : 1;
   cudaError_t e = launch_kernel_cluster(decode_mla_kernel, grid, dim3(mla::THREADS_DECODE), (size_t)mla::SMEM_BYTES_DECODE, s, opt.pdl, cluster, kmap,
-                                static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * mla::kLog2e, pt.seq_lens,
+                                static_cast<const __nv_bfloat16*>(q), g.num_q_heads, g.sm_scale * opt.scale_mul * mla::kLog2e, pt.seq_lens,
                                 sel_phys, sel_logical, sel_count, max_budget, best, c->ws.part_o, c->ws.part_lse,
                                 c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
-                                static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget, cluster > 1 ? 1 : 0);
+                                static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget, cluster > 1 ? 1 : 0, opt.out_scale);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

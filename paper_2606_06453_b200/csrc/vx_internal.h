@@ -32,6 +32,8 @@ struct Workspace {               // device pointers carved from the caller's wor
   int32_t* blk_indptr;           // blocks finer than the page: the page table expanded into a block table, [max_batch + 1]
   int32_t* blk_indices;          // [max_total_pages * bpp] physical block ids
   float* topk_remap;             // [kTopkRemapMaxKnots] the knot table of vx_set_topk_remap
+  void* mla_stage;               // fp8 latent cache: [max_batch * max_budget] selected pages widened to bf16 (vx_decode_mla_fp8.cu)
+  int32_t* mla_stage_sel;        // [max_batch, max_budget] their ids in that pool
   float* fp8_qvec;               // fp8 KV cache: [max_batch, Hkv, 2 qk_dim] query vectors [Qm | Qp] of the score kernel (vx_score_fp8.cu)
   size_t bytes;                  // total
 };
@@ -162,6 +164,8 @@ struct DecodeOpts {
   void* summary_upd = nullptr;   // non-null: also rebuild the summary of each request's newest page (a1), whose
                                  // keys the kernel stages anyway (it is a forced local page)
   bool pdl = false;              // launched as a programmatic dependent of the preceding kernel
+  float scale_mul = 1.f;         // multiplies sm_scale (an fp8 pool's k_scale when the kernel runs on widened codes)
+  float out_scale = 1.f;         // multiplies the output (its v_scale)
   const int32_t* budget = nullptr;   // fused step: sel_count[i, h] is known to be min(budget[i], max_budget, P_i), so the kernel
                                  // need not wait for the selection kernel to read it (one L2 round trip less after the wait)
 };
@@ -231,6 +235,11 @@ inline bool kv_is_fp8(const vx_geom& g) { return g.kv_format != VX_KV_SAME; }
 inline size_t kv_elem_size(const vx_geom& g) { return kv_is_fp8(g) ? 1 : (g.dtype == VX_DT_BF16 ? 2 : 4); }
 bool fp8_geometry_supported(const vx_geom& g);
 cudaError_t launch_score_fp8(vx_ctx* c, const void* q, const void* summary, const vx_page_table& pt, float* scores, cudaStream_t s);
+bool mla_fp8_staged_supported(const vx_geom& g);
+size_t mla_fp8_stage_elems(const vx_geom& g, int max_batch, int max_budget);
+cudaError_t launch_decode_mla_fp8_staged(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
+                                         const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
+                                         int32_t max_budget, void* out, float* lse, cudaStream_t s, const DecodeOpts& opt);
 cudaError_t launch_decode_fp8(vx_ctx* c, const void* q, const vx_kv_pool& pool, const vx_page_table& pt,
                               const int32_t* sel_phys, const int32_t* sel_logical, const int32_t* sel_count,
                               int32_t max_budget, void* out, float* lse, cudaStream_t s);
