@@ -448,10 +448,29 @@ def main():
     peak, peak_src = measured_peak()
     main_rec = measure(args.config, args, device, local, rank, world, args.steps, max(args.warmup, 3), peak, peak_src, rank)
     also = {}
-    for name in [c for c in args.also.split(",") if c and c != args.config]:
-        rec = measure(name, args, device, local, rank, world, args.also_steps, 3, peak, peak_src, rank)
-        if rec is not None:
+    names = [c for c in args.also.split(",") if c and c != args.config]
+    if world == 1 and "WORLD_SIZE" not in os.environ:
+        # One process per workload: a step's time moves by ~1 us with where the driver places the 4-5 GB pool, and that
+        # depends on what the process allocated and freed before (C3 timed after C4 in one process: +0.7..1.0 us on every
+        # box tried, C4 after C3: -0.5 us).  A fresh process per record gives every workload the main record's conditions.
+        import subprocess
+        for name in names:
+            cmd = [sys.executable, os.path.abspath(__file__), "--config", name, "--also", "", "--steps", str(args.also_steps),
+                   "--warmup", str(max(args.warmup, 3)), "--kv-dtype", args.kv_dtype, "--mla-step", args.mla_step,
+                   "--topk-approx", str(args.topk_approx)] + (["--no-cpu-baseline"] if args.no_cpu_baseline else [])
+            out = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)
+            lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+            if out.returncode != 0 or not lines:
+                raise SystemExit(f"bench.py: the record of {name} failed (exit {out.returncode}): {out.stderr[-2000:]}")
+            rec = json.loads(lines[-1])
+            for k in ("also", "metric", "n_gpus", "higher_is_better", "scaling", "vs_baseline", "data", "also_isolation"):
+                rec.pop(k, None)
             also[name] = rec
+    else:
+        for name in names:
+            rec = measure(name, args, device, local, rank, world, args.also_steps, max(args.warmup, 3), peak, peak_src, rank)
+            if rec is not None:
+                also[name] = rec
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -460,6 +479,7 @@ def main():
                 "data": "synthetic"}
         line.update(main_rec)
         line["also"] = also
+        line["also_isolation"] = "own process per workload" if (world == 1 and "WORLD_SIZE" not in os.environ) else "in process"
         print(json.dumps(line))
 
 
