@@ -192,6 +192,12 @@ static __device__ int g_vx_trace_ctas;
 __device__ __forceinline__ void cluster_sync() {
   asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
+// ... the same barrier without the release: for the LAST hand-over of a kernel, where a CTA only tells its peers that it
+// has finished READING their shared memory (the values are consumed, so the loads are complete).  A release here would
+// also wait for the CTA's outstanding global stores -- its output rows -- to be acknowledged (~1 us on the decode kernels).
+__device__ __forceinline__ void cluster_sync_relaxed() {
+  asm volatile("barrier.cluster.arrive.relaxed.aligned;\n\tbarrier.cluster.wait.aligned;" ::: "memory");
+}
 __device__ __forceinline__ uint32_t dsmem_addr(uint32_t local, uint32_t rank) {
   uint32_t r;
   asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local), "r"(rank));

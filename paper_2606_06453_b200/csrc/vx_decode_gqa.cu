@@ -327,7 +327,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
     if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 9);
     cluster_merge_partials(cl_part, D, grp, split, num_splits, (int64_t)i * num_q_heads + kvh * grp, out, lse_out);
     if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 10);
-    cluster_sync();                               // no CTA leaves while a peer still reads its partial
+    cluster_sync_relaxed();                       // no CTA leaves while a peer still reads its partial
   } else if (num_splits > 1) {                  // (a5) the last split of this (request, KV head) merges by LSE
     if (last_split_arrives(unit_counter + i * num_kv_heads + kvh, num_splits, &s_last)) {
       if (threadIdx.x == 0) VX_TRACE_STAMP(cta, 9);

@@ -319,7 +319,7 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
   if constexpr (CL) {                           // (a5) the splits are one cluster: merge over distributed shared memory
     cluster_sync();
     cluster_merge_partials(cl_part, D, grp, split, num_splits, (int64_t)i * num_q_heads + kvh * grp, out, lse_out);
-    cluster_sync();
+    cluster_sync_relaxed();                       // no CTA leaves while a peer still reads its partial
   } else if (num_splits > 1) {                  // (a5) the last split of this (request, KV head) merges by LSE
     if (last_split_arrives(unit_counter + i * num_kv_heads + kvh, num_splits, &s_last))
       merge_partials<__nv_bfloat16>(part_o, part_lse, (int64_t)i * num_q_heads + kvh * grp, grp, num_splits, D, out, lse_out,

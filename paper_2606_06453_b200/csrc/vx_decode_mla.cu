@@ -427,7 +427,7 @@ decode_mla_kernel(const __grid_constant__ CUtensorMap kmap, const __nv_bfloat16*
     merge_cluster<THREADS_DECODE>(sm + OFF_PAIR, s_lse_all, reinterpret_cast<float (*)[NH]>(sm + OFF_PAIR + 96 * 1024), i, num_q_heads, num_splits, split,
                   out, lse_out);
     if (tid == 0) VX_TRACE_STAMP(cta, 10);
-    cluster_sync();                                      // my tile stays until every peer has read it
+    cluster_sync_relaxed();                              // my tile stays until every peer has read it
   } else if (num_splits > 1) {
     if (last_split_arrives(unit_counter + i, num_splits, &s_last))
       merge_splits(part_o, part_lse, i, num_q_heads, num_splits, out, lse_out, sm + OFF_PAIR);
