@@ -46,6 +46,15 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
+// a page-table load that asks the L2 to keep its line (evict-last): the selection kernel gathers the same ids a few
+// microseconds after 100+ MB of summaries have streamed through the cache
+__device__ __forceinline__ int ld_keep_l2(const int32_t* p) {
+  int v;
+  asm volatile("{\n\t.reg .b64 pol;\n\tcreatepolicy.fractional.L2::evict_last.b64 pol, 1.0;\n\t"
+               "ld.global.L2::cache_hint.s32 %0, [%1], pol;\n\t}" : "=r"(v) : "l"(p));
+  return v;
+}
+
 // the schedule both roles follow: groups of <= PG pages inside one request, over flat pages [begin, end)
 struct GroupIter {
   int flat, end, req, req_end;
@@ -136,8 +145,8 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     // The physical ids of the CTA's flat page range are prefetched 32 at a time (one coalesced load, two chunks
     // in registers), so that no index load sits between a freed stage and its refill.
     int chunk0 = begin;                                   // flat index of id_cur's lane 0
-    int id_cur = chunk0 + lane < end ? page_indices[chunk0 + lane] : 0;
-    int id_nxt = chunk0 + kWarp + lane < end ? page_indices[chunk0 + kWarp + lane] : 0;
+    int id_cur = chunk0 + lane < end ? ld_keep_l2(page_indices + chunk0 + lane) : 0;
+    int id_nxt = chunk0 + kWarp + lane < end ? ld_keep_l2(page_indices + chunk0 + kWarp + lane) : 0;
     GroupIter it(begin, end, batch, page_indptr);         // (its loads fly together with the id loads above)
     if (lane == 0) VX_TRACE_STAMP(blockIdx.x, 1);
     for (int g = 0; it.next(PG, first, count, req); ++g) {
@@ -150,7 +159,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
       if (first >= chunk0 + kWarp) {                      // the group starts in the next chunk: rotate, prefetch one more
         chunk0 += kWarp;
         id_cur = id_nxt;
-        id_nxt = chunk0 + kWarp + lane < end ? page_indices[chunk0 + kWarp + lane] : 0;
+        id_nxt = chunk0 + kWarp + lane < end ? ld_keep_l2(page_indices + chunk0 + kWarp + lane) : 0;
       }
       const int off = first + lane - chunk0;              // lane l copies page first + l (valid for l < count)
       const int a = __shfl_sync(0xffffffffu, id_cur, off & 31), b = __shfl_sync(0xffffffffu, id_nxt, off & 31);
