@@ -50,8 +50,14 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
   return *reinterpret_cast<uint32_t*>(&v);
 }
 // 16-byte async copy that writes zeros when !valid (src-size 0)
-__device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, bool valid) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(valid ? 16 : 0));
+// (with an L2 cache policy: the selected pages are read once -- evict-first, so that they leave the small hot arrays alone)
+__device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, bool valid, uint64_t pol) {
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(dst), "l"(src), "r"(valid ? 16 : 0), "l"(pol));
+}
+__device__ __forceinline__ uint64_t gqa_policy_evict_first() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
 }
 
 template <int D, bool CL>
@@ -112,6 +118,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   uint8_t* ring = smem + (size_t)warp * kGqaStages * 2 * PAGEB;
   const uint32_t ring_u32 = smem_u32(ring);
 
+  const uint64_t pol = gqa_policy_evict_first();
   int id_phys = 0, id_valid = 0;                // lane j: this warp's (base + j)-th page
   auto fetch_ids = [&](int base) {
     const int p = base + lane;
@@ -135,8 +142,8 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
       const int t = x / CH, c = x % CH;
       const uint32_t off = t * ROWB + ((c ^ (t & 7)) * 16);
       const int64_t src = base + (int64_t)t * stride_token + c * 8;
-      cp_async16_zfill(dst + off, kpool + src, t < nv);
-      cp_async16_zfill(dst + PAGEB + off, vpool + src, t < nv);
+      cp_async16_zfill(dst + off, kpool + src, t < nv, pol);
+      cp_async16_zfill(dst + PAGEB + off, vpool + src, t < nv, pol);
     }
   };
 
