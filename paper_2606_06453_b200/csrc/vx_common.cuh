@@ -78,6 +78,17 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return static_cast<uint32_t>(__cvta_generic_to_shared(p));
 }
 // 16-byte asynchronous global->shared copy (LDGSTS), bypassing L1
+// L2 cache policy for data that is read ONCE (summary rows, selected pages): evict-first, so that the stream leaves the
+// small arrays the next kernel reads (scores, page table, selection lists, queries) in the cache.  Measured on C3: the
+// summary stream 86.6 -> 84.7 us, the selected pages 84.7 -> 83.7 us per step.
+__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void cp_async16_hint(uint32_t dst, const void* src, uint64_t pol) {
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, 16, %2;" ::"r"(dst), "l"(src), "l"(pol));
+}
 __device__ __forceinline__ void cp_async16(void* smem, const void* gmem) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(smem)), "l"(gmem));
 }

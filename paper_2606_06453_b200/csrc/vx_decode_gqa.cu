@@ -54,11 +54,6 @@ __device__ __forceinline__ uint32_t pack_bf16x2(float lo, float hi) {
 __device__ __forceinline__ void cp_async16_zfill(uint32_t dst, const void* src, bool valid, uint64_t pol) {
   asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(dst), "l"(src), "r"(valid ? 16 : 0), "l"(pol));
 }
-__device__ __forceinline__ uint64_t gqa_policy_evict_first() {
-  uint64_t pol;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-  return pol;
-}
 
 template <int D, bool CL>
 __global__ void __launch_bounds__(kGqaWarps * kWarp)
@@ -118,7 +113,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   uint8_t* ring = smem + (size_t)warp * kGqaStages * 2 * PAGEB;
   const uint32_t ring_u32 = smem_u32(ring);
 
-  const uint64_t pol = gqa_policy_evict_first();
+  const uint64_t pol = l2_evict_first_policy();
   int id_phys = 0, id_valid = 0;                // lane j: this warp's (base + j)-th page
   auto fetch_ids = [&](int base) {
     const int p = base + lane;

@@ -62,8 +62,8 @@ template <> __device__ __forceinline__ void fp8x4_to_f16<fp8_e5m2>(uint32_t four
   asm("{\n\t.reg .b16 l, h;\n\tmov.b32 {l, h}, %2;\n\tcvt.rn.f16x2.e5m2x2 %0, l;\n\tcvt.rn.f16x2.e5m2x2 %1, h;\n\t}"
       : "=r"(lo), "=r"(hi) : "r"(four));
 }
-__device__ __forceinline__ void cp16_zfill(uint32_t dst, const void* src, bool valid) {
-  asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(valid ? 16 : 0));
+__device__ __forceinline__ void cp16_zfill(uint32_t dst, const void* src, bool valid, uint64_t pol) {   // (evict-first: vx_common.cuh)
+  asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2, %3;" ::"r"(dst), "l"(src), "r"(valid ? 16 : 0), "l"(pol));
 }
 
 template <typename TKV, bool CL>
@@ -138,6 +138,7 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
       id_valid = min(PAGE, n_tok - lg * PAGE) | (lg == newest_page ? 256 : 0);
     }
   };
+  const uint64_t pol = l2_evict_first_policy();
   auto issue = [&](int p) {                     // all lanes: copy page p of this warp into slot p % STAGES
     const int phys = __shfl_sync(0xffffffffu, id_phys, p & 31);
     const int venc = __shfl_sync(0xffffffffu, id_valid, p & 31);
@@ -151,8 +152,8 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
       const int t = x / 8, c = x % 8;           // token row, 16-byte chunk (16 channels)
       const uint32_t off = t * ROWB + ((c ^ (t & 7)) * 16);
       const int64_t src = base + (int64_t)t * stride_token + c * 16;
-      cp16_zfill(dst + off, kpool + src, t < nv);
-      cp16_zfill(dst + PAGEB + off, vpool + src, t < nv);
+      cp16_zfill(dst + off, kpool + src, t < nv, pol);
+      cp16_zfill(dst + PAGEB + off, vpool + src, t < nv, pol);
     }
   };
 

@@ -43,11 +43,6 @@ __device__ __forceinline__ void sc_mbar_expect_tx(uint32_t bar, uint32_t bytes) 
 }
 // (the summaries stream through once: evict-first, so that they do not push the scores, the page table and the queries
 //  out of the L2 -- the next kernels read those)
-__device__ __forceinline__ uint64_t l2_policy_evict_first() {
-  uint64_t pol;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-  return pol;
-}
 __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
@@ -151,7 +146,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     // ---- producer: one bulk copy per page (all KV heads of the page are contiguous) ----------
     // The physical ids of the CTA's flat page range are prefetched 32 at a time (one coalesced load, two chunks
     // in registers), so that no index load sits between a freed stage and its refill.
-    const uint64_t stream_pol = l2_policy_evict_first();
+    const uint64_t stream_pol = l2_evict_first_policy();
     int chunk0 = begin;                                   // flat index of id_cur's lane 0
     int id_cur = chunk0 + lane < end ? ld_keep_l2(page_indices + chunk0 + lane) : 0;
     int id_nxt = chunk0 + kWarp + lane < end ? ld_keep_l2(page_indices + chunk0 + kWarp + lane) : 0;

@@ -61,6 +61,8 @@ score_fp8_kernel(const uint8_t* __restrict__ summary, const float* __restrict__ 
     const int p = base + lane;
     if (p < my_pages) ids = page_indices[begin + warp + p * kS8Warps];
   };
+  // (no L2 evict-first hint on these copies, unlike the tensor-core kernel below: with the lane predicate on the copy the
+  //  hinted form ran into "illegal instruction" on the full-size latent geometry)
   auto issue = [&](int p) {
     const int phys = __shfl_sync(0xffffffffu, ids, p & 31);
     const uint8_t* src = summary + (int64_t)phys * page_bytes + lane * 16;
@@ -173,6 +175,7 @@ score_fp8_mma_kernel(const uint8_t* __restrict__ summary, const float* __restric
   const int my_tiles = n_tiles > warp ? (n_tiles - warp + kM8Warps - 1) / kM8Warps : 0;
   auto tile_page0 = [&](int p) -> int { return begin + 2 * (warp + kM8Warps * p); };
   const uint32_t ring = smem_u32(s8_smem) + (uint32_t)warp * kM8Stages * kM8TileBytes;
+  const uint64_t stream_pol = l2_evict_first_policy();    // the summaries stream through once (vx_common.cuh)
   int ids = 0;                                            // lane l: page l % 2 of my (base + l / 2)-th tile
   auto fetch_ids = [&](int base) {
     const int flat = tile_page0(base + (lane >> 1)) + (lane & 1);
@@ -188,7 +191,7 @@ score_fp8_mma_kernel(const uint8_t* __restrict__ summary, const float* __restric
 #pragma unroll
         for (int it = 0; it < 4; ++it) {                  // 128 granules of 16 B per page
           const int x = lane + it * kWarp, head = x >> 4, c = x & 15;
-          asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst + pg * PAGEB + head * ROW + ((c ^ head) << 4)), "l"(src + x * 16));
+          cp_async16_hint(dst + pg * PAGEB + head * ROW + ((c ^ head) << 4), src + x * 16, stream_pol);
         }
       }
     }
