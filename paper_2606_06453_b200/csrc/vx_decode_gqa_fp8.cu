@@ -79,6 +79,7 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
   using namespace gq8;
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float s_m[WARPS][8], s_l[WARPS][8];
+  __shared__ float s_hinv[8], s_hlse[8];           // per head of the group: v_scale / denominator and LSE of this CTA's pages
   __shared__ int s_valid[WARPS][STAGES];         // valid tokens of the page staged in each slot (bit 8: the request's newest page)
   __shared__ int s_phys[WARPS][STAGES];          // its physical id
   __shared__ int s_last;
@@ -291,30 +292,45 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
     *reinterpret_cast<float2*>(so + d0 * 8 + ha) = make_float2(o[mt][0] * f_a, o[mt][1] * f_b);
     *reinterpret_cast<float2*>(so + (d0 + 1) * 8 + ha) = make_float2(o[mt][2] * f_a, o[mt][3] * f_b);
   }
-  __syncthreads();
-  for (int e = threadIdx.x; e < grp * D; e += WARPS * kWarp) {
-    const int h = e / D, d = e % D;
+  if (threadIdx.x < 8) {                        // per head, once: the CTA's reference, v_scale / denominator and LSE
+    const int h = threadIdx.x;
     float mb = -INFINITY;
 #pragma unroll
     for (int w = 0; w < WARPS; ++w) mb = fmaxf(mb, s_m[w][h]);
-    float lsum = 0.f, acc = 0.f;
+    float lsum = 0.f;
+#pragma unroll
+    for (int w = 0; w < WARPS; ++w) lsum += s_m[w][h] == -INFINITY ? 0.f : s_l[w][h] * exp2f(s_m[w][h] - mb);
+    s_hinv[h] = lsum > 0.f ? v_scale / lsum : 0.f;
+    s_hlse[h] = lsum > 0.f ? (mb + log2f(lsum)) * kLn2 : -INFINITY;
+  }
+  __syncthreads();
+  // four heads of one channel per thread: one 16-byte read per warp partial
+  for (int e = threadIdx.x; e < ((grp + 3) / 4) * D; e += WARPS * kWarp) {
+    const int d = e % D, h0 = 4 * (e / D);
+    float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
     for (int w = 0; w < WARPS; ++w) {
-      lsum += s_m[w][h] == -INFINITY ? 0.f : s_l[w][h] * exp2f(s_m[w][h] - mb);
-      acc += reinterpret_cast<const float*>(smem + (size_t)w * STAGES * 2 * PAGEB)[d * 8 + h];
+      const float4 v = *reinterpret_cast<const float4*>(smem + (size_t)w * STAGES * 2 * PAGEB + (d * 8 + h0) * 4);
+      acc.x += v.x; acc.y += v.y; acc.z += v.z; acc.w += v.w;
     }
-    const float val = lsum > 0.f ? acc / lsum * v_scale : 0.f;
-    const float lse = lsum > 0.f ? (mb + log2f(lsum)) * kLn2 : -INFINITY;
-    const int64_t head_row = (int64_t)i * num_q_heads + kvh * grp + h;
-    if (num_splits == 1) {
-      out[head_row * D + d] = __float2bfloat16_rn(val);
-      if (d == 0 && lse_out != nullptr) lse_out[head_row] = lse;
-    } else if constexpr (CL) {
-      cl_part[h * D + d] = val;
-      if (d == 0) cl_part[8 * D + h] = lse;
-    } else {
-      part_o[(head_row * num_splits + split) * D + d] = val;
-      if (d == 0) part_lse[head_row * num_splits + split] = lse;
+    const float a4[4] = {acc.x, acc.y, acc.z, acc.w};
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const int h = h0 + k;
+      if (h < grp) {
+        const float val = a4[k] * s_hinv[h];
+        const int64_t head_row = (int64_t)i * num_q_heads + kvh * grp + h;
+        if (num_splits == 1) {
+          out[head_row * D + d] = __float2bfloat16_rn(val);
+          if (d == 0 && lse_out != nullptr) lse_out[head_row] = s_hlse[h];
+        } else if constexpr (CL) {
+          cl_part[h * D + d] = val;
+          if (d == 0) cl_part[8 * D + h] = s_hlse[h];
+        } else {
+          part_o[(head_row * num_splits + split) * D + d] = val;
+          if (d == 0) part_lse[head_row * num_splits + split] = s_hlse[h];
+        }
+      }
     }
   }
   if constexpr (CL) {                           // (a5) the splits are one cluster: merge over distributed shared memory
