@@ -71,6 +71,7 @@ def main():
     scores = torch.empty(Hkv, w.total_pages, dtype=torch.float32, device=dev)
     step = lambda: ctx.sparse_decode_step(w.q, pool, summary, pt, w.budget, w.max_budget, out, lse, sp, sl, sc)
     step()
+    fused_step = ctx.last_launch_count == 1       # AUTO takes the one-kernel MLA step for small batches only
     ctx.page_score(w.q, summary, pt, scores)
     torch.cuda.synchronize()
     alone = {"score": lambda: ctx.page_score(w.q, summary, pt, scores),
@@ -78,8 +79,8 @@ def main():
              "decode": lambda: ctx.sparse_paged_decode(w.q, pool, pt, sp, sl, sc, w.max_budget, out, lse)}[args.kernel]
     kind = {"score": binding.VX_TRACE_SCORE, "topk": binding.VX_TRACE_TOPK, "decode": binding.VX_TRACE_DECODE}[args.kernel]
     names = SLOTS[args.kernel if args.kernel != "decode" else ("decode_mla" if s.kv_shared else "decode_gqa")]
-    if args.kernel == "decode" and args.mode == "step" and s.kv_shared:
-        names = SLOTS["step_mla"]
+    if args.kernel == "decode" and args.mode == "step" and s.kv_shared and fused_step:
+        names = SLOTS["step_mla"]                  # (the one-kernel MLA step stamps its own phases)
     buf = torch.zeros(8192, 16, dtype=torch.int64, device=dev)
     ctx.trace_attach(buf, kind)
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
