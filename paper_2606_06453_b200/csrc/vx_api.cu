@@ -223,6 +223,7 @@ vx_status vx_create(vx_ctx** out, const vx_geom* g, int device, void* workspace,
   c->g.block_size = c->g.page_size;
   c->device = device;
   c->num_sms = prop.multiProcessorCount;
+  c->l2_bytes = prop.l2CacheSize;
   c->max_batch = max_batch;
   c->max_total_pages = max_total_pages;
   c->max_pages_per_req = max_pages_per_req;

@@ -81,9 +81,13 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) {
 // L2 cache policy for data that is read ONCE (summary rows, selected pages): evict-first, so that the stream leaves the
 // small arrays the next kernel reads (scores, page table, selection lists, queries) in the cache.  Measured on C3: the
 // summary stream 86.6 -> 84.7 us, the selected pages 84.7 -> 83.7 us per step.
-__device__ __forceinline__ uint64_t l2_evict_first_policy() {
+// The launchers ask for it only when the stream is larger than half the L2 (l2_stream_once): a small batch whose summaries
+// and selected pages fit the cache keeps the default policy, so that the next decode step -- which selects mostly the
+// same pages -- can still find them there.
+__device__ __forceinline__ uint64_t l2_stream_policy(bool once) {
   uint64_t pol;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  if (once) asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  else asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(pol));
   return pol;
 }
 __device__ __forceinline__ void cp_async16_hint(uint32_t dst, const void* src, uint64_t pol) {

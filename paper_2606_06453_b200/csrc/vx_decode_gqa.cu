@@ -65,7 +65,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
                       int max_budget, int num_splits, float* __restrict__ part_o, float* __restrict__ part_lse,
                       int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ summary_upd, int summary_kind,
                       __nv_bfloat16* __restrict__ out, float* __restrict__ lse_out, int req0,
-                      const int32_t* __restrict__ budget_opt, int bpp) {
+                      const int32_t* __restrict__ budget_opt, int bpp, int stream_once) {
   constexpr int ROWB = D * 2;                 // bytes per token row
   constexpr int CH = ROWB / 16;               // 16-byte chunks per row
   constexpr int PAGEB = kGqaPage * ROWB;      // bytes of one K (or V) page chunk
@@ -114,7 +114,7 @@ decode_gqa_mma_kernel(const __nv_bfloat16* __restrict__ q, const __nv_bfloat16* 
   uint8_t* ring = smem + (size_t)warp * kGqaStages * 2 * PAGEB;
   const uint32_t ring_u32 = smem_u32(ring);
 
-  const uint64_t pol = l2_evict_first_policy();
+  const uint64_t pol = l2_stream_policy(stream_once != 0);
   int id_phys = 0, id_valid = 0;                // lane j: this warp's (base + j)-th page
   auto fetch_ids = [&](int base) {
     const int p = base + lane;
@@ -385,7 +385,8 @@ static cudaError_t launch_gqa_mma_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const __nv_bfloat16*>(pool.v), pool.stride_page, pool.stride_token, pool.stride_head,
       g.num_q_heads, g.num_kv_heads, g.sm_scale * kLog2e, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget,
       splits, c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(opt.summary_upd), g.summary_kind,
-      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget, c->bpp);
+      static_cast<__nv_bfloat16*>(out), lse, opt.rr.begin, opt.budget, c->bpp,
+      l2_stream_once(c, (int64_t)n_req * g.num_kv_heads * max_budget * 2 * kGqaPage * D * 2) ? 1 : 0);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

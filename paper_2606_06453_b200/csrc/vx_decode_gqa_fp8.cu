@@ -75,7 +75,7 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
                       const int32_t* __restrict__ sel_count, int max_budget, int num_splits, float* __restrict__ part_o,
                       float* __restrict__ part_lse, int* __restrict__ unit_counter, __nv_bfloat16* __restrict__ out,
                       float* __restrict__ lse_out, const int32_t* __restrict__ budget_opt, int bpp,
-                      uint8_t* __restrict__ summary_upd) {
+                      uint8_t* __restrict__ summary_upd, int stream_once) {
   using namespace gq8;
   extern __shared__ __align__(128) uint8_t smem[];
   __shared__ float s_m[WARPS][8], s_l[WARPS][8];
@@ -139,7 +139,7 @@ decode_gqa_fp8_kernel(const __nv_bfloat16* __restrict__ q, const uint8_t* __rest
       id_valid = min(PAGE, n_tok - lg * PAGE) | (lg == newest_page ? 256 : 0);
     }
   };
-  const uint64_t pol = l2_evict_first_policy();
+  const uint64_t pol = l2_stream_policy(stream_once != 0);
   auto issue = [&](int p) {                     // all lanes: copy page p of this warp into slot p % STAGES
     const int phys = __shfl_sync(0xffffffffu, id_phys, p & 31);
     const int venc = __shfl_sync(0xffffffffu, id_valid, p & 31);
@@ -381,7 +381,8 @@ static cudaError_t launch_gqa_fp8_t(vx_ctx* c, const void* q, const vx_kv_pool& 
       static_cast<const __nv_bfloat16*>(q), static_cast<const uint8_t*>(pool.k), static_cast<const uint8_t*>(pool.v),
       pool.stride_page, pool.stride_token, pool.stride_head, g.num_q_heads, g.num_kv_heads,
       g.sm_scale * pool.k_scale * gq8::kLog2e, pool.v_scale, pt.seq_lens, sel_phys, sel_logical, sel_count, max_budget, splits,
-      c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(out), lse, budget, c->bpp, static_cast<uint8_t*>(summary_upd));
+      c->ws.part_o, c->ws.part_lse, c->ws.unit_counter, static_cast<__nv_bfloat16*>(out), lse, budget, c->bpp, static_cast<uint8_t*>(summary_upd),
+      l2_stream_once(c, (int64_t)pt.batch * g.num_kv_heads * max_budget * 2 * gq8::PAGEB) ? 1 : 0);
   c->launches += 1;
   return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -64,10 +64,13 @@ inline bool approx_topk_supported(int max_pages_per_req, int max_budget) {
 
 }  // namespace vx
 
+struct vx_ctx;
+inline bool l2_stream_once(const vx_ctx* c, int64_t bytes);
 struct vx_ctx {
   vx_geom g;
   int device;
   int num_sms;
+  int64_t l2_bytes;              // the device's L2 size (streams larger than half of it are read evict-first)
   int32_t max_batch, max_total_pages, max_pages_per_req, max_budget;
   vx::Workspace ws;
   int32_t launches;              // kernels enqueued by the last compute call
@@ -79,6 +82,8 @@ struct vx_ctx {
   int32_t flat_splits, flat_waves;   // VX_OPT_MLA_FLAT_*: 0 = the library's choice
   char err[512];
 };
+inline bool l2_stream_once(const vx_ctx* c, int64_t bytes) { return bytes > c->l2_bytes / 2; }
+
 
 namespace vx {
 

@@ -88,7 +88,7 @@ template <typename T, int D, int PG, int HKV, int kScStages, int AGG, int KIND>
 __global__ void __launch_bounds__(kScThreads, 2)
 score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_heads, int batch,
              const int32_t* __restrict__ page_indptr, const int32_t* __restrict__ page_indices, int total_pages,
-             float* __restrict__ scores, int req_begin, int req_end, int flat_lo_host, int flat_span_host) {
+             float* __restrict__ scores, int req_begin, int req_end, int flat_lo_host, int flat_span_host, int stream_once) {
   constexpr int PER = Elem<T>::kPerVec;
   // envelope: [min | max] of one (page, KV head); centroid (block top-k): the mean key, d elements
   constexpr int ROW_ELEMS = KIND == VX_SUMMARY_CENTROID ? D : 2 * D;
@@ -146,7 +146,7 @@ score_kernel(const T* __restrict__ q, const T* __restrict__ summary, int num_q_h
     // ---- producer: one bulk copy per page (all KV heads of the page are contiguous) ----------
     // The physical ids of the CTA's flat page range are prefetched 32 at a time (one coalesced load, two chunks
     // in registers), so that no index load sits between a freed stage and its refill.
-    const uint64_t stream_pol = l2_evict_first_policy();
+    const uint64_t stream_pol = l2_stream_policy(stream_once != 0);
     int chunk0 = begin;                                   // flat index of id_cur's lane 0
     int id_cur = chunk0 + lane < end ? ld_keep_l2(page_indices + chunk0 + lane) : 0;
     int id_nxt = chunk0 + kWarp + lane < end ? ld_keep_l2(page_indices + chunk0 + kWarp + lane) : 0;
@@ -458,7 +458,7 @@ static cudaError_t launch_score_agg(vx_ctx* c, const void* q, const void* summar
   score_kernel<T, D, PG, HKV, kScStages, AGG, KIND><<<ctas, kScThreads, smem, s>>>(
       static_cast<const T*>(q), static_cast<const T*>(summary), g.num_q_heads, pt.batch, pt.page_indptr,
       pt.page_indices, pt.total_pages, scores, rr.begin, rr.begin + (rr.count < 0 ? pt.batch : rr.count), 0,
-      rr.count < 0 ? pt.total_pages : -1);
+      rr.count < 0 ? pt.total_pages : -1, l2_stream_once(c, (int64_t)est_pages * (int64_t)page_bytes) ? 1 : 0);
   c->launches += 1;
   return cudaGetLastError();
 }

@@ -164,7 +164,8 @@ template <> __device__ __forceinline__ void s8_cvt4<fp8_e5m2>(uint32_t four, uin
 template <typename T>
 __global__ void __launch_bounds__(kM8Warps * kWarp, 2)
 score_fp8_mma_kernel(const uint8_t* __restrict__ summary, const float* __restrict__ qvec, const int32_t* __restrict__ page_indptr,
-                     const int32_t* __restrict__ page_indices, int batch, int total_pages, float* __restrict__ scores) {
+                     const int32_t* __restrict__ page_indices, int batch, int total_pages, float* __restrict__ scores,
+                     int stream_once) {
   constexpr int HKV = 8, ROW = 256, PAGEB = HKV * ROW, NCH = ROW / 16;      // 16 chunks of 16 codes per row
   extern __shared__ __align__(128) uint8_t s8_smem[];
   const int lane = threadIdx.x % kWarp, warp = threadIdx.x / kWarp;
@@ -175,7 +176,7 @@ score_fp8_mma_kernel(const uint8_t* __restrict__ summary, const float* __restric
   const int my_tiles = n_tiles > warp ? (n_tiles - warp + kM8Warps - 1) / kM8Warps : 0;
   auto tile_page0 = [&](int p) -> int { return begin + 2 * (warp + kM8Warps * p); };
   const uint32_t ring = smem_u32(s8_smem) + (uint32_t)warp * kM8Stages * kM8TileBytes;
-  const uint64_t stream_pol = l2_evict_first_policy();    // the summaries stream through once (vx_common.cuh)
+  const uint64_t stream_pol = l2_stream_policy(stream_once != 0);   // (vx_common.cuh)
   int ids = 0;                                            // lane l: page l % 2 of my (base + l / 2)-th tile
   auto fetch_ids = [&](int base) {
     const int flat = tile_page0(base + (lane >> 1)) + (lane & 1);
@@ -326,7 +327,7 @@ static cudaError_t launch_score_fp8_t(vx_ctx* c, const void* q, const void* summ
     if (grid > (pt.total_pages + 1) / 2) grid = (pt.total_pages + 1) / 2;
     cudaError_t e = launch_kernel(score_fp8_mma_kernel<T>, dim3(grid), dim3(kM8Warps * kWarp), (size_t)smem_bytes, s, true,
                                   static_cast<const uint8_t*>(summary), (const float*)c->ws.fp8_qvec, pt.page_indptr, pt.page_indices,
-                                  pt.batch, pt.total_pages, scores);
+                                  pt.batch, pt.total_pages, scores, l2_stream_once(c, (int64_t)pt.total_pages * 2048) ? 1 : 0);
     c->launches += 1;
     return e != cudaSuccess ? e : cudaGetLastError();
   }
