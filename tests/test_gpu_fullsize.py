@@ -94,3 +94,27 @@ def test_c3_planted_pages_are_recalled():
             hits += len(chosen & set(planted))
             tot += len(planted)
     assert hits / tot >= 0.99, f"planted recall {hits / tot:.3f}"
+
+
+@pytest.mark.parametrize("hkv,d", [(4, 64), (2, 128)])
+def test_other_geometries_at_streaming_size(hkv, d):
+    """Geometries outside C2-C5 with a summary stream larger than half the L2 (the size from which the kernels read their
+    streams with the L2 evict-first policy): the fused step on sampled requests against the oracle."""
+    from dataclasses import replace
+    from paper_2606_06453_b200.workloads import SPECS, subproblem
+    rows = 2 * d * 2 * hkv                         # summary bytes per page
+    pages = (80 << 20) // rows // 16               # 16 requests, ~80 MB of summaries in all
+    spec = replace(SPECS["C2"], name=f"stream-h{hkv}d{d}", num_q_heads=4 * hkv, num_kv_heads=hkv, qk_dim=d, v_dim=d, batch=16,
+                   seq_len=(pages * 16 - 300, pages * 16), budget=96)
+    w, summary, out, lse, sp, sl, sc = run_step(spec)
+    s = w.spec
+    assert int(w.page_indptr[-1]) * rows > (70 << 20)
+    for r in (0, 11):
+        sub = subproblem(w, [r])
+        ref = oracle_step(sub)
+        check_selection(sub, sl[r:r + 1].cpu().numpy(), sl[r:r + 1].cpu().numpy(), sc[r:r + 1].cpu().numpy(), ref,
+                        label=f"{spec.name}, request {r}")
+        q, opool, opt = to_oracle(sub)
+        o_ref, l_ref = vo.sparse_attention(q, opool, opt, sl[r:r + 1].cpu().numpy(), sc[r:r + 1].cpu().numpy(),
+                                           s.num_q_heads, s.num_kv_heads, s.qk_dim, s.v_dim, s.sm_scale)
+        check_attention(s.dtype, out[r:r + 1].float().cpu().numpy(), lse[r:r + 1].cpu().numpy(), o_ref, l_ref)
