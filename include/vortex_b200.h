@@ -77,7 +77,10 @@ typedef enum { VX_SUMMARY_ENVELOPE = 0, VX_SUMMARY_CENTROID = 1 } vx_summary_kin
  *            roles).  q, out and lse stay in geom.dtype, which must be VX_DT_BF16.  Summaries are the min / max CODES
  *            (exact); page scores are computed on decoded codes without k_scale -- a positive factor common to every
  *            page changes no selection -- so vx_page_score returns  oracle score / k_scale  (G25-G27).
- *            Envelope summaries and VX_AGG_SUM only; pool strides are in one-byte elements. */
+ *            Envelope summaries and VX_AGG_SUM only; pool strides are in one-byte elements.
+ *            Workspace: for the absorbed-MLA geometry (kv_shared, d 576, dv 512, page 64) a context holds a bf16
+ *            staging pool of max_batch * max_budget pages (73,728 B each), into which the selected fp8 pages are widened
+ *            (exactly) before the tensor-core decode kernel runs on them -- vx_workspace_bytes includes it. */
 typedef enum { VX_KV_SAME = 0, VX_KV_FP8_E4M3 = 1, VX_KV_FP8_E5M2 = 2 } vx_kv_format;
 
 typedef struct {
